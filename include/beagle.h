@@ -1,0 +1,179 @@
+/* beagle.h — C-ABI of the B200-native Beagle scoring library (libbeagle_b200.so).
+ *
+ * What it is: batched fitness evaluation ("scoring", Table 1) of a whole colony of
+ * symbolic-regression programs. PAPER.md:63 (§2.4): "the individual is sent to the GPU once and
+ * the aggregated fitness value is returned for the full batch of fitness cases"; at
+ * most 1024 fitness cases, so that one model is aggregated on chip and never through global
+ * memory; PAPER.md:40 (§2.2): populations are managed in batches when device memory is short;
+ * PAPER.md:184 (§3.2): a program is a flat list of commands run on an operand stack (RPN);
+ * the stack holds 32 entries; PAPER.md:200-294 (Table 3): command meanings and
+ * operand order; "length (i.e., the number of GCL commands)".
+ * Where the paper is silent the readings of DESIGN.md §3 (R1..R20) apply.
+ *
+ * Conventions
+ *   - Every entry point is extern "C", takes plain pointers and sizes, never throws, never aborts.
+ *   - "DEVICE" = pointer into CUDA device memory of the current device; "HOST" = host memory.
+ *   - All pointers are borrowed for the duration of the enqueued work; the library never frees or
+ *     keeps user memory. Scratch lives in a library-owned workspace (see beagle_reserve).
+ *   - Calls enqueue work on `stream` (a cudaStream_t passed as void*, NULL = legacy default
+ *     stream) and return without synchronising, unless the workspace has to grow (then one
+ *     cudaMalloc happens first; call beagle_reserve to avoid it).
+ *   - Argument errors are returned synchronously and nothing is enqueued.
+ *   - Data-dependent problems are reported in band: a malformed individual gets the canonical
+ *     quiet NaN 0x7FC00000 as its fitness and never causes an out-of-bounds access.
+ *   - Lower fitness is better; a non-finite fitness marks an invalid individual.
+ *   - One call at a time per process (the workspace is shared); calls are not re-entrant.
+ */
+#ifndef BEAGLE_H_
+#define BEAGLE_H_
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+/* ---- genome encoding (R2; north_star: "postfix int32 tokens {opcode:8, arg:24}") ----
+ * A token is a 32-bit word read as unsigned: opcode = w & 0xFF, arg = w >> 8 (24 bits).
+ * Opcode 0 is invalid on purpose so that zeroed memory is a malformed program.                  */
+#define BEAGLE_OP_CONST 0x01 /* push consts[arg], arg < n_consts */
+#define BEAGLE_OP_LOAD  0x02 /* push X[i][arg], arg < d */
+#define BEAGLE_OP_ADD   0x03 /* a b -> a + b     */
+#define BEAGLE_OP_SUB   0x04 /* a b -> a - b  (second-top minus top)     */
+#define BEAGLE_OP_MUL   0x05 /* a b -> a * b     */
+#define BEAGLE_OP_DIV   0x06 /* a b -> |b| < 1e-6f ? 1 : a / b  (protected) PAPER.md:238     */
+#define BEAGLE_OP_SIN   0x07 /* a -> sin a     */
+#define BEAGLE_OP_COS   0x08 /* a -> cos a     */
+#define BEAGLE_OP_LOG   0x09 /* a -> |a| < 1e-6f ? 0 : ln|a|    (protected) PAPER.md:253     */
+#define BEAGLE_OP_SQRT  0x0A /* a -> sqrt|a|                    (protected) PAPER.md:249     */
+#define BEAGLE_OP_EXP   0x0B /* a -> exp(a > 80 ? 80 : a)       (clamped)     */
+/* 0x10..0x1E are reserved for the rest of Table 3 (DUP SWAP DEL POW SIGN SQUARE CUBE CBRT TAN
+ * ARCSIN ARCCOS ARCTAN TANH COPY PASTE); until implemented they make a program malformed.      */
+#define BEAGLE_TOKEN(op, arg) ((int32_t)(((uint32_t)(arg) << 8) | ((uint32_t)(op) & 0xFFu)))
+
+/* ---- limits (also returned by beagle_limits) ---- */
+#define BEAGLE_MAX_LEN   512  /* tokens per individual (config 5 of BASELINE.json: 1..512)      */
+#define BEAGLE_MAX_STACK 32   /* operand stack entries                            */
+#define BEAGLE_MAX_N     1024 /* fitness cases per call                            */
+#define BEAGLE_MAX_D     32   /* input variables per case                                       */
+#define BEAGLE_MAX_CONSTS (1 << 24)
+
+typedef int32_t beagle_status;
+enum {
+    BEAGLE_OK = 0,
+    BEAGLE_ERR_INVALID_ARG = -1, /* null pointer with P > 0, size out of range                   */
+    BEAGLE_ERR_UNSUPPORTED = -2, /* device is not sm_100, or not enough shared memory            */
+    BEAGLE_ERR_CUDA = -3,        /* a CUDA call failed; see beagle_last_cuda_error               */
+    BEAGLE_ERR_NOMEM = -4        /* workspace or staging allocation failed                       */
+};
+
+/* beagle_eval — score a device-resident colony.
+ *
+ * For every individual p in [0,P): run its postfix program on each of the N fitness cases
+ * (Table 3 semantics with the protected forms above, fp32), take out_i = top of stack, and return
+ *     fitness_out[p] = (sum_i (out_i - y[i])^2) / N + tax * lengths[p]          (D5)
+ * in input order. The sum is taken before the division; the fp32 summation order is fixed (bitwise
+ * reproducible run to run, independent of P, of the order of individuals and of chunking).
+ *
+ *   genomes      DEVICE  packed tokens, T = sum(lengths) words, 4-byte aligned; individual p owns
+ *                        [off[p], off[p] + lengths[p]) with off = exclusive prefix sum of lengths
+ *   lengths      DEVICE  P entries; an entry outside [1, BEAGLE_MAX_LEN] marks the individual
+ *                        malformed and counts as 0 words in the prefix sum
+ *   P            number of individuals, >= 0; P == 0 returns BEAGLE_OK and enqueues nothing
+ *   consts       DEVICE  fp32 side table of n_consts entries; may be NULL iff n_consts == 0
+ *   n_consts     0 .. BEAGLE_MAX_CONSTS
+ *   X            DEVICE  N x d row-major fp32 (case-major)
+ *   y            DEVICE  N fp32 targets
+ *   N, d         1..BEAGLE_MAX_N, 1..BEAGLE_MAX_D
+ *   tax          length tax per token (in north_star's float form)
+ *   fitness_out  DEVICE  P fp32
+ *   stream       cudaStream_t
+ *
+ * Malformed (fitness = quiet NaN 0x7FC00000): length outside [1,512], unknown opcode, non-zero
+ * arg on an operator, CONST arg >= n_consts, LOAD arg >= d, an operator that pops more than the
+ * stack holds, depth above 32, (final depth is >= 1 whenever the rest holds).
+ * The extent of `genomes` is trusted to be sum of the in-range lengths.                          */
+beagle_status beagle_eval(const int32_t* genomes, const int32_t* lengths, int64_t P,
+                          const float* consts, int64_t n_consts,
+                          const float* X, const float* y, int32_t N, int32_t d,
+                          float tax, float* fitness_out, void* stream);
+
+/* beagle_eval_chunked — the same result for a colony held in HOST memory that may be larger than
+ * the device budget ("manages populations in batches to ensure the GPU memory is
+ * never exceeded"; R19). The colony is cut at individual boundaries into chunks of at
+ * most device_budget_bytes/2 bytes of tokens+lengths; chunk c+1 is copied host-to-device on an
+ * internal copy stream while chunk c is evaluated on `stream` (two staging buffers).
+ * fitness_out is bit-identical to beagle_eval on the whole colony, for any budget.
+ *
+ *   h_genomes, h_lengths, h_consts   HOST (pinned memory for overlap; pageable memory works but
+ *                                    the copies then do not overlap)
+ *   X, y, fitness_out                DEVICE, as in beagle_eval
+ *   device_budget_bytes              cap on device bytes used for genome staging (both buffers);
+ *                                    must hold two maximum-length individuals:
+ *                                    >= 2 * 4 * (BEAGLE_MAX_LEN + 1)
+ * Completion of `stream` implies completion of everything, copies included. The host arrays must
+ * stay valid and unchanged until then.                                                           */
+beagle_status beagle_eval_chunked(const int32_t* h_genomes, const int32_t* h_lengths, int64_t P,
+                                  const float* h_consts, int64_t n_consts,
+                                  const float* X, const float* y, int32_t N, int32_t d,
+                                  float tax, float* fitness_out,
+                                  int64_t device_budget_bytes, void* stream);
+
+/* beagle_eval_blockwise — prior art kept as a measured baseline, not the product: the paper's own
+ * mapping (one CUDA block per individual, one thread per fitness case, a 32-entry
+ * per-thread stack in local memory, block aggregation in shared memory), same arguments and the
+ * same definition of the result as beagle_eval. Its summation order differs, so results agree
+ * with beagle_eval to rounding, not bitwise.                                                     */
+beagle_status beagle_eval_blockwise(const int32_t* genomes, const int32_t* lengths, int64_t P,
+                                    const float* consts, int64_t n_consts,
+                                    const float* X, const float* y, int32_t N, int32_t d,
+                                    float tax, float* fitness_out, void* stream);
+
+/* beagle_debug_outputs — test only: per-case program outputs, out_PxN[p*N + i] (DEVICE, P*N fp32),
+ * computed by the same interpreter as beagle_eval; malformed individuals give NaN rows.          */
+beagle_status beagle_debug_outputs(const int32_t* genomes, const int32_t* lengths, int64_t P,
+                                   const float* consts, int64_t n_consts,
+                                   const float* X, int32_t N, int32_t d,
+                                   float* out_PxN, void* stream);
+
+/* beagle_debug_schedule — test only: copies what the scheduling pre-pass (offsets, per-program
+ * scan, length-sorted permutation) produced for the last beagle_eval/debug call on `stream`.
+ * Any pointer may be NULL. DEVICE outputs: off[P] (int64 exclusive prefix sum), depth[P] (int32
+ * maximum stack depth, 0 if malformed), perm[P] (int32, the evaluation order: individuals grouped
+ * by depth class, longest first). Enqueued on `stream`.                                          */
+beagle_status beagle_debug_schedule(int64_t P, int64_t* off, int32_t* depth, int32_t* perm,
+                                    void* stream);
+
+/* Limits compiled into the library (any pointer may be NULL). */
+void beagle_limits(int32_t* max_len, int32_t* max_stack, int32_t* max_n, int32_t* max_d);
+
+/* Static, NUL-terminated description of a status code. */
+const char* beagle_status_string(beagle_status s);
+
+/* The cudaError_t behind the most recent BEAGLE_ERR_CUDA / BEAGLE_ERR_NOMEM (0 if none). */
+int32_t beagle_last_cuda_error(void);
+
+/* Pre-size the workspace for colonies of up to P_max individuals and T_max tokens so that later
+ * calls are allocation-free. Synchronises the device if it has to reallocate. */
+beagle_status beagle_reserve(int64_t P_max, int64_t T_max);
+
+/* Pre-size the two staging buffers of beagle_eval_chunked for this budget. */
+beagle_status beagle_reserve_chunked(int64_t device_budget_bytes);
+
+/* Free the cached workspace and staging buffers (synchronises the device). */
+void beagle_release(void);
+
+/* Number of kernels the most recent beagle_eval* call launched (for bench.py's gpu_launches). */
+int32_t beagle_last_launch_count(void);
+
+/* Device time, in milliseconds, of the evaluation kernels alone (the interpreter launches, without
+ * the scheduling pre-pass) of the most recent beagle_eval call made while profiling was enabled
+ * with beagle_set_profiling(1). Reading it synchronises on the recorded events. Returns < 0 if
+ * nothing was recorded. */
+void  beagle_set_profiling(int32_t on);
+float beagle_last_eval_kernel_ms(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* BEAGLE_H_ */

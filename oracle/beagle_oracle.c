@@ -1,0 +1,291 @@
+/* beagle_oracle.c — TEST INFRASTRUCTURE, NOT THE PRODUCT.
+ *
+ * A plain, slow, single-threaded CPU evaluator of what the Beagle scoring path computes, written
+ * from the paper and DESIGN.md's readings, in fp64. It shares no code, header, table or constant
+ * generator with the CUDA path (paper_2607_06731_b200/csrc); the opcode numbers below are retyped
+ * from DESIGN.md D2, not included. Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline /
+ * --impl reference legs may call it.
+ *
+ * What it follows
+ *   - PAPER.md:184 (§3.2): RPN stack machine; unary commands replace the top of the stack, binary
+ *     commands replace the top two with the result.
+ *   - PAPER.md:190: the stack holds 32 entries.
+ *   - PAPER.md:200-294 (Table 3): command meanings; operand order SUB = second-top - top
+ *     (PAPER.md:231), DIV = second-top / top.
+ *   - PAPER.md:314: length = the number of GCL commands (terminals included).
+ *   - PAPER.md:63: one aggregated value per individual for the whole batch of fitness cases.
+ *   - north_star (BASELINE.json) where the paper is silent: fitness = MSE + tax*length, protected
+ *     div/log/sqrt/exp, {opcode:8,arg:24} tokens, constants in a side fp32 table. Exact forms:
+ *     DESIGN.md D1-D6.
+ *
+ * The method is an exact evaluation, so the oracle is the definition written out: for every
+ * individual, for every case, run the tokens in order on a stack; square the residual; sum; divide
+ * by N; add tax*L. No blocking, fusion or reordering.
+ *
+ * Beside the value v the stack carries e >= |v_gpu - v|, a running bound on how far an fp32
+ * evaluator whose per-op accuracy obeys `orc_contract` can be from v (DESIGN.md §4 "error bound").
+ * The bound never changes v; it only tells the parity test which tolerance class an individual is
+ * in (STRICT / CONDITIONED / UNSTABLE).
+ *
+ * Pins (tests/test_oracle_pins.py, all CPU): P1 printed lengths, P2 closed forms of the paper's
+ * printed genomes, P3 x0*x0 vs x0^2, P4 CONST/LOAD reduce to numpy, P5 identity insertion,
+ * P6 commutativity/antisymmetry, P7 protected-operator edge table, P8 brute force of all programs
+ * of <= 3 tokens against an independent recursive evaluator (oracle/infix_check.py), P9 power-of-two
+ * scaling, P10 overflow semantics, P11 the bound is a bound (fp32 mirror), P12 case duplication.
+ * Parity unpinned: nothing on the hot path.
+ */
+#include <float.h>
+#include <math.h>
+#include <stdint.h>
+#include <stddef.h>
+
+/* DESIGN.md D2 (numbers retyped, not shared) */
+enum { OP_CONST = 1, OP_LOAD = 2, OP_ADD = 3, OP_SUB = 4, OP_MUL = 5, OP_DIV = 6,
+       OP_SIN = 7, OP_COS = 8, OP_LOG = 9, OP_SQRT = 10, OP_EXP = 11 };
+
+#define ORC_MAX_LEN   512
+#define ORC_MAX_STACK 32
+#define ORC_MAX_N     1024
+
+#define ORC_FLAG_MALFORMED      1 /* DESIGN.md D3 / R9                                        */
+#define ORC_FLAG_UNSTABLE       2 /* an input interval straddles a protected-op threshold     */
+#define ORC_FLAG_CLASS_UNSTABLE 4 /* an interval straddles the fp32 overflow edge, or the sign
+                                     of an infinity depends on an uncertain zero              */
+
+/* Accuracy contract of the evaluator being checked, in units of u = 2^-24 unless said otherwise.
+ * The test passes the CUDA path's published contract or the IEEE contract
+ * (all c = 1, abs terms 0) for the fp32 mirror.                                               */
+typedef struct {
+    double c_add;        /* ADD, SUB: relative                                                */
+    double c_mul;        /* MUL: relative                                                     */
+    double c_div;        /* DIV: relative                                                     */
+    double div_bigb_abs; /* DIV: extra absolute error |a| * this when |b| can exceed 2^126    */
+    double c_sqrt;       /* SQRT: relative                                                    */
+    double abs_sqrt;     /* SQRT: absolute (denormal inputs flushed)                          */
+    double c_exp;        /* EXP: relative, constant part                                      */
+    double c_exp_arg;    /* EXP: relative, per unit of |argument|                             */
+    double c_log_rel;    /* LOG: relative                                                     */
+    double c_log_abs;    /* LOG: absolute                                                     */
+    double c_sin_abs;    /* SIN, COS: absolute, constant part                                 */
+    double c_sin_arg;    /* SIN, COS: absolute, per unit of |argument|                        */
+    double abs_floor;    /* every computed op: absolute (denormal results flushed), NOT in u  */
+    double sum_per_case; /* summation: the fp32 sum of N squares is off by at most            */
+    double sum_const;    /*   (sum_per_case * N + sum_const) * u * S  (depth of the add tree) */
+} orc_contract;
+
+static const double U32 = 5.9604644775390625e-08; /* 2^-24 */
+static const double FMAX = 3.4028234663852886e+38; /* FLT_MAX */
+#define EPS_PROT ((double)1e-6f)                   /* DESIGN.md D2: EPS = 1e-6f               */
+
+typedef struct { double v, e; } pair;
+
+/* D4: fp32 range semantics in an fp64 carrier; mirror mode rounds to fp32 instead. Also applies
+ * the overflow-edge test of DESIGN.md §4 (last row of the propagation table).                  */
+static inline pair finish(double v, double e, int mirror, int* flags) {
+    pair r;
+    if (isnan(v)) { r.v = v; r.e = 0.0; return r; }
+    if (isinf(v)) { r.v = v; r.e = 0.0; return r; }
+    double a = fabs(v);
+    if (!(e < INFINITY)) { *flags |= ORC_FLAG_CLASS_UNSTABLE; e = 0.0; }
+    else if (a - e <= FMAX && a + e >= FMAX) *flags |= ORC_FLAG_CLASS_UNSTABLE;
+    if (mirror) v = (double)(float)v;
+    else if (a > FMAX) v = v > 0 ? INFINITY : -INFINITY;
+    r.v = v; r.e = isinf(v) ? 0.0 : e;
+    return r;
+}
+
+/* Static well-formedness (D3): returns the maximum stack depth, or -1 if malformed. */
+static int check_program(const uint32_t* tok, int L, int64_t n_consts, int d) {
+    if (L < 1 || L > ORC_MAX_LEN) return -1;
+    int sp = 0, mx = 0;
+    for (int t = 0; t < L; ++t) {
+        uint32_t op = tok[t] & 0xFFu, arg = tok[t] >> 8;
+        switch (op) {
+        case OP_CONST: if ((int64_t)arg >= n_consts) return -1; sp++; break;
+        case OP_LOAD:  if ((int64_t)arg >= (int64_t)d) return -1; sp++; break;
+        case OP_ADD: case OP_SUB: case OP_MUL: case OP_DIV:
+            if (arg != 0 || sp < 2) return -1; sp--; break;
+        case OP_SIN: case OP_COS: case OP_LOG: case OP_SQRT: case OP_EXP:
+            if (arg != 0 || sp < 1) return -1; break;
+        default: return -1;
+        }
+        if (sp > ORC_MAX_STACK) return -1;
+        if (sp > mx) mx = sp;
+    }
+    return sp >= 1 ? mx : -1;
+}
+
+/* One program on one case: PAPER.md:184 stack semantics, Table 3 operand order, D2 values. */
+static pair run_case(const uint32_t* tok, int L, const float* consts, const float* x,
+                     const orc_contract* c, int mirror, int* flags) {
+    pair st[ORC_MAX_STACK];
+    int sp = 0;
+    const double fl = c->abs_floor;
+    for (int t = 0; t < L; ++t) {
+        uint32_t op = tok[t] & 0xFFu, arg = tok[t] >> 8;
+        switch (op) {
+        case OP_CONST: st[sp].v = (double)consts[arg]; st[sp].e = 0.0; sp++; break;
+        case OP_LOAD:  st[sp].v = (double)x[arg];      st[sp].e = 0.0; sp++; break;
+        case OP_ADD: case OP_SUB: {
+            pair a = st[sp - 2], b = st[sp - 1];
+            double v = (op == OP_ADD) ? a.v + b.v : a.v - b.v;
+            double e1 = a.e + b.e;
+            st[sp - 2] = finish(v, e1 + c->c_add * U32 * (fabs(v) + e1) + fl, mirror, flags);
+            sp--; break; }
+        case OP_MUL: {
+            pair a = st[sp - 2], b = st[sp - 1];
+            double v = a.v * b.v;
+            if ((isinf(a.v) && !isnan(b.v) && !isinf(b.v) && fabs(b.v) <= b.e) ||
+                (isinf(b.v) && !isnan(a.v) && !isinf(a.v) && fabs(a.v) <= a.e))
+                *flags |= ORC_FLAG_CLASS_UNSTABLE;     /* inf * (maybe zero, sign unknown) */
+            double e1 = fabs(a.v) * b.e + fabs(b.v) * a.e + a.e * b.e;
+            if (isnan(e1)) e1 = 0.0;                   /* inf * 0 inside the bound only    */
+            st[sp - 2] = finish(v, e1 + c->c_mul * U32 * (fabs(v) + e1) + fl, mirror, flags);
+            sp--; break; }
+        case OP_DIV: {                         /* P:238; protected form D2: |b|<EPS ? 1 : a/b */
+            pair a = st[sp - 2], b = st[sp - 1];
+            double ab = fabs(b.v), v, e = 0.0;
+            if (isnan(b.v) || isinf(b.v)) v = a.v / b.v;
+            else if (ab + b.e < EPS_PROT) v = 1.0;
+            else if (ab - b.e >= EPS_PROT) {
+                v = a.v / b.v;
+                if (!isnan(a.v) && !isinf(a.v)) {
+                    double e1 = (a.e + fabs(v) * b.e) / (ab - b.e);
+                    e = e1 + c->c_div * U32 * (fabs(v) + e1) + fl;
+                    if (ab + b.e > 8.507059173023462e+37) /* 2^126 */
+                        e += (fabs(a.v) + a.e) * c->div_bigb_abs;
+                }
+            } else { *flags |= ORC_FLAG_UNSTABLE; v = (ab < EPS_PROT) ? 1.0 : a.v / b.v; }
+            st[sp - 2] = finish(v, e, mirror, flags);
+            sp--; break; }
+        case OP_SIN: case OP_COS: {
+            pair a = st[sp - 1];
+            double v = (op == OP_SIN) ? sin(a.v) : cos(a.v);  /* sin(+-inf) = NaN */
+            double e = fmin(a.e, 2.0) + (c->c_sin_abs + c->c_sin_arg * (fabs(a.v) + a.e)) * U32 + fl;
+            if (!(e < 2.000001)) e = 2.000001;
+            st[sp - 1] = finish(v, e, mirror, flags);
+            break; }
+        case OP_LOG: {                         /* P:253; protected: |a|<EPS ? 0 : ln|a|      */
+            pair a = st[sp - 1];
+            double aa = fabs(a.v), v, e = 0.0;
+            if (isnan(a.v)) v = a.v;
+            else if (isinf(a.v)) v = INFINITY;
+            else if (aa + a.e < EPS_PROT) v = 0.0;
+            else if (aa - a.e >= EPS_PROT) {
+                v = log(aa);
+                double e1 = -log1p(-a.e / aa);
+                e = e1 + c->c_log_rel * U32 * (fabs(v) + e1) + c->c_log_abs * U32 + fl;
+            } else { *flags |= ORC_FLAG_UNSTABLE; v = (aa < EPS_PROT) ? 0.0 : log(aa); }
+            st[sp - 1] = finish(v, e, mirror, flags);
+            break; }
+        case OP_SQRT: {                        /* P:249; protected: sqrt|a|                  */
+            pair a = st[sp - 1];
+            double aa = fabs(a.v), v = sqrt(aa), e = 0.0;
+            if (!isnan(a.v) && !isinf(a.v)) {
+                double lo = aa > a.e ? sqrt(aa - a.e) : 0.0, hi = sqrt(aa + a.e);
+                double e1 = fmax(v - lo, hi - v);
+                e = e1 + c->c_sqrt * U32 * (v + e1) + c->abs_sqrt + fl;
+            }
+            st[sp - 1] = finish(v, e, mirror, flags);
+            break; }
+        case OP_EXP: {                         /* P:275; clamped: exp(a > 80 ? 80 : a)       */
+            pair a = st[sp - 1];
+            double t = a.v > 80.0 ? 80.0 : a.v;  /* ternary so NaN passes (R5) */
+            double v = exp(t), e = 0.0;
+            if (!isnan(a.v) && !isinf(a.v)) {
+                double up = fmin(a.v + a.e, 80.0) - t, dn = t - fmin(a.v - a.e, 80.0);
+                double dt = fmax(up, dn);
+                double e1 = v * expm1(dt);
+                e = e1 + (c->c_exp + c->c_exp_arg * (fabs(t) + dt)) * U32 * (v + e1) + fl;
+            }
+            st[sp - 1] = finish(v, e, mirror, flags);
+            break; }
+        default: break; /* unreachable: check_program ran first */
+        }
+    }
+    return st[sp - 1]; /* D3: output = top of stack */
+}
+
+/* orc_eval — the whole colony (D5-D6).
+ *   genomes/lengths/consts/X/y as in include/beagle.h (host pointers); mode 0 = truth (fp64
+ *   carrier with fp32 range), 1 = mirror (every op result rounded to fp32).
+ *   fitness_out[P] float; bound_out[P] double (E_p) or NULL; flags_out[P] int32 or NULL;
+ *   depth_out[P] int32 (max stack depth, 0 if malformed) or NULL;
+ *   outputs P*N doubles (per-case outputs, NaN rows for malformed) or NULL.
+ * Returns 0, or -1 on bad arguments.                                                          */
+int orc_eval(const int32_t* genomes, const int32_t* lengths, int64_t P,
+             const float* consts, int64_t n_consts,
+             const float* X, const float* y, int32_t N, int32_t d, float tax,
+             const orc_contract* c, int mode,
+             float* fitness_out, double* bound_out, int32_t* flags_out, int32_t* depth_out,
+             double* outputs) {
+    if (P < 0 || N < 1 || N > ORC_MAX_N || d < 1 || !c) return -1;
+    const int mirror = (mode == 1);
+    int64_t off = 0;
+    for (int64_t p = 0; p < P; ++p) {
+        int L = lengths[p];
+        const uint32_t* tok = (const uint32_t*)genomes + off;
+        int inrange = (L >= 1 && L <= ORC_MAX_LEN);
+        int depth = inrange ? check_program(tok, L, n_consts, d) : -1;
+        if (inrange) off += L;            /* out-of-range lengths count as 0 words */
+        int flags = 0;
+        if (depth < 0) {
+            union { uint32_t u; float f; } qn; qn.u = 0x7FC00000u;
+            fitness_out[p] = qn.f;
+            if (bound_out) bound_out[p] = 0.0;
+            if (flags_out) flags_out[p] = ORC_FLAG_MALFORMED;
+            if (depth_out) depth_out[p] = 0;
+            if (outputs) for (int i = 0; i < N; ++i) outputs[p * (int64_t)N + i] = NAN;
+            continue;
+        }
+        double S = 0.0, ES = 0.0;
+        for (int i = 0; i < N; ++i) {
+            pair o = run_case(tok, L, consts, X + (size_t)i * d, c, mirror, &flags);
+            if (outputs) outputs[p * (int64_t)N + i] = o.v;
+            /* D5: r = sat32(out - y), q = sat32(r^2) */
+            double r0 = o.v - (double)y[i];
+            pair r = finish(r0, o.e + U32 * (fabs(r0) + o.e) + c->abs_floor, mirror, &flags);
+            double q0 = r.v * r.v;
+            double eq1 = 2.0 * fabs(r.v) * r.e + r.e * r.e;
+            if (isnan(eq1)) eq1 = 0.0;
+            pair q = finish(q0, eq1 + U32 * (q0 + eq1) + c->abs_floor, mirror, &flags);
+            S += q.v;              /* fp64 sum; NaN and +inf propagate by IEEE rules */
+            ES += q.e;
+        }
+        if (!isnan(S) && !isinf(S)) {
+            double E = ES + (c->sum_per_case * (double)N + c->sum_const) * U32 * (S + ES);
+            if (S - E <= FMAX && S + E >= FMAX) flags |= ORC_FLAG_CLASS_UNSTABLE;
+            if (S > FMAX) S = INFINITY;   /* D5: overflow is decided on the sum, not the mean */
+            ES = E;
+        } else ES = 0.0;
+        double fit = S / (double)N + (double)tax * (double)L;
+        fitness_out[p] = (float)fit;
+        if (bound_out) bound_out[p] = (isnan(fit) || isinf(fit)) ? 0.0
+                                     : ES / (double)N + 4.0 * U32 * fabs(fit) + c->abs_floor;
+        if (flags_out) flags_out[p] = flags;
+        if (depth_out) depth_out[p] = depth;
+    }
+    return 0;
+}
+
+/* The two contracts the tests use most, so that Python does not have to retype 13 doubles.
+ * which = 0: IEEE (every op correctly rounded: c = 1, a little slack for libm, no abs terms);
+ * which = 1: the CUDA path's published contract, DESIGN.md §6 (numbers retyped from there).   */
+void orc_default_contract(int which, orc_contract* c) {
+    if (which == 0) {
+        c->c_add = 1.0; c->c_mul = 1.0; c->c_div = 1.0; c->div_bigb_abs = 0.0;
+        c->c_sqrt = 1.0; c->abs_sqrt = 0.0; c->c_exp = 1.001; c->c_exp_arg = 0.0;
+        c->c_log_rel = 1.001; c->c_log_abs = 0.0; c->c_sin_abs = 1.001; c->c_sin_arg = 0.0;
+        c->abs_floor = 1.5e-45;
+        c->sum_per_case = 1.0; c->sum_const = 0.0;   /* any summation order */
+    } else {
+        c->c_add = 1.0; c->c_mul = 1.0;
+        c->c_div = 3.5; c->div_bigb_abs = 1.1754943508222875e-38;
+        c->c_sqrt = 3.0; c->abs_sqrt = 1.1e-19;
+        c->c_exp = 6.0; c->c_exp_arg = 2.5;
+        c->c_log_rel = 5.0; c->c_log_abs = 4.0;
+        c->c_sin_abs = 12.0; c->c_sin_arg = 3.0;
+        c->abs_floor = 1.1754943508222875e-38;
+        c->sum_per_case = 1.0 / 32.0; c->sum_const = 5.0; /* per-lane chain + 5 shuffle levels */
+    }
+}

@@ -1,0 +1,381 @@
+"""Pins of the CPU oracle against what the paper and the mathematics fix.
+
+None of these retypes the oracle's formulas: each compares it with a printed value, a closed form,
+an invariant, a special case that reduces to numpy, or an independent brute-force evaluator.
+All CPU (-m "not gpu").
+"""
+import itertools
+import math
+import os
+
+import numpy as np
+import pytest
+
+from paper_2607_06731_b200 import colonies as C
+from tests.util import asm, pack, symbolic
+
+GOLD = os.path.join(os.path.dirname(__file__), "golden", "paper_genomes.txt")
+QNAN_BITS = 0x7FC00000
+
+
+def _golden():
+    rows = []
+    for line in open(GOLD):
+        if line.startswith("#") or not line.strip():
+            continue
+        cite, n, text = [s.strip() for s in line.split("|")]
+        rows.append((cite, int(n), text))
+    return rows
+
+
+def _gcl_to_asm(text):
+    """GCL text of the paper ('LOAD b:1; CONST 0.5; MUL;') -> our test assembler text."""
+    out = []
+    for cmd in [c.strip() for c in text.split(";") if c.strip()]:
+        parts = cmd.split()
+        if parts[0] == "LOAD":
+            out.append("x" + parts[1].split(":")[1])
+        elif parts[0] == "CONST":
+            out.append(parts[1])
+        else:
+            out.append({"LN": "LOG"}.get(parts[0], parts[0]))
+    return " ".join(out)
+
+
+def ev(oracle, progs, consts, X, y, tax=0.0, **kw):
+    g, l, c = pack(progs, consts)
+    return oracle.evaluate(g, l, c if len(c) else np.zeros(1, np.float32), X, y, tax, **kw)
+
+
+# ---- P1: printed lengths ------------------------------------------------------------------------
+def test_P1_printed_lengths_are_token_counts():
+    rows = _golden()
+    assert [n for _, n, _ in rows] == [12, 12, 24, 25]
+    for cite, n, text in rows:
+        cmds = [c for c in text.split(";") if c.strip()]
+        assert len(cmds) == n, cite  # PAPER.md:314 "genome length (i.e., the number of GCL commands)"
+
+
+def test_P1_oracle_taxes_every_token(oracle):
+    # fitness - MSE == tax * L with L the printed length (genome of P:157, hot-path ops only)
+    cite, n, text = _golden()[0]
+    consts = []
+    prog, c = asm(_gcl_to_asm(text), consts)
+    rng = np.random.default_rng(1)
+    X = rng.uniform(1, 3, (64, 3)).astype(np.float32)
+    y = np.zeros(64, np.float32)
+    f0 = ev(oracle, [prog], c, X, y, tax=0.0)["fitness"][0]
+    f1 = ev(oracle, [prog], c, X, y, tax=0.5)["fitness"][0]
+    assert f1 - f0 == pytest.approx(0.5 * n, rel=1e-6)
+
+
+# ---- P2: closed forms of the paper's genomes ----------------------------------------------------
+def test_P2_fig2_genome_closed_form(oracle):
+    # P:157 = (sqrt(b*b) - b)/a*0.5 - 0.01603 = (|b|-b)/(2a) - 0.01603
+    _, _, text = _golden()[0]
+    prog, c = asm(_gcl_to_asm(text))
+    rng = np.random.default_rng(2)
+    X = rng.uniform(-4, 4, (256, 3)).astype(np.float32)
+    X[np.abs(X[:, 0]) < 0.1, 0] = 1.0
+    a, b = X[:, 0].astype(np.float64), X[:, 1].astype(np.float64)
+    want = (np.abs(b) - b) / (2 * a) + np.float64(np.float32(-0.01603))
+    r = ev(oracle, [prog], c, X, np.zeros(256, np.float32), want_outputs=True)
+    np.testing.assert_allclose(r["outputs"][0], want, rtol=1e-12, atol=1e-12)
+    # exactly -0.01603 for b >= 0
+    pos = b >= 0
+    assert np.all(r["outputs"][0][pos] == np.float64(np.float32(-0.01603)))
+
+
+def test_P2_quadratic_formula_operand_order(oracle):
+    # the P:316 genome with DUP/DEL expanded by hand: (sqrt(b^2-4ac)-b)/a*0.5
+    prog, c = asm("x1 x1 MUL x0 x0 ADD x0 x0 ADD ADD x2 MUL SUB SQRT x1 SUB x0 DIV 0.5 MUL")
+    rng = np.random.default_rng(3)
+    X = np.empty((512, 3), np.float32)
+    X[:, 0] = rng.uniform(0.5, 2, 512) * rng.choice([-1, 1], 512)
+    X[:, 1] = rng.uniform(4, 8, 512)
+    X[:, 2] = rng.uniform(-1, 1, 512)
+    a, b, cc = (X[:, j].astype(np.float64) for j in range(3))
+    assert np.all(b * b >= 4 * a * cc)
+    root = (np.sqrt(b * b - 4 * a * cc) - b) / (2 * a)
+    y = root.astype(np.float32)
+    r = ev(oracle, [prog], c, X, y, want_outputs=True)
+    np.testing.assert_allclose(r["outputs"][0], root, rtol=1e-13)
+    mse_want = np.mean((root - y.astype(np.float64)) ** 2)
+    assert r["fitness"][0] == pytest.approx(mse_want, rel=1e-6, abs=1e-25)
+    # it IS a root: a r^2 + b r + c ~ 0 (pins SUB/DIV order independently of the formula above)
+    o = r["outputs"][0]
+    assert np.max(np.abs(a * o * o + b * o + cc)) < 1e-9
+
+
+# ---- P3: north_star's example --------------------------------------------------------------------
+def test_P3_x0_squared_is_exact(oracle):
+    X = (np.arange(-256, 256, dtype=np.float64)[:, None] / 2048.0).astype(np.float32)  # <= 12 bits
+    y = (X[:, 0].astype(np.float64) ** 2).astype(np.float32)
+    assert np.all(y.astype(np.float64) == X[:, 0].astype(np.float64) ** 2)
+    prog, c = asm("x0 x0 MUL")
+    tax = np.float32(0.001)
+    f = ev(oracle, [prog], c, X, y, tax=tax)["fitness"][0]
+    assert f == np.float32(np.float64(tax) * 3)      # MSE exactly 0, fitness = (float)(tax*3)
+    assert f == tax * np.float32(3)                  # same bits as the fp32 product
+
+
+# ---- P4: single-terminal programs reduce to numpy -----------------------------------------------
+def test_P4_terminals_reduce_to_numpy(oracle):
+    rng = np.random.default_rng(4)
+    X = rng.normal(size=(300, 4)).astype(np.float32)
+    y = rng.normal(size=300).astype(np.float32)
+    y64 = y.astype(np.float64)
+    consts = []
+    progs = [asm("1.75", consts, 0)[0]] + [asm(f"x{j}")[0] for j in range(4)]
+    r = ev(oracle, progs, consts, X, y)
+    assert r["fitness"][0] == pytest.approx((1.75 - y64.mean()) ** 2 + y64.var(), rel=1e-6)
+    for j in range(4):
+        assert r["fitness"][1 + j] == pytest.approx(np.mean((X[:, j].astype(np.float64) - y64) ** 2), rel=1e-6)
+    assert list(r["depth"]) == [1] * 5
+
+
+# ---- P5: identity insertion ----------------------------------------------------------------------
+def test_P5_identity_insertion(oracle):
+    col = C.make_colony(1, P=64)
+    off = np.concatenate([[0], np.cumsum(col.lengths)])
+    nC = len(col.consts)
+    consts = list(col.consts) + [np.float32(0.0), np.float32(1.0)]
+    zero, one = C.token(C.OP["CONST"], nC), C.token(C.OP["CONST"], nC + 1)
+    ADD, MUL, DIV = (C.token(C.OP[k]) for k in ("ADD", "MUL", "DIV"))
+    base = [col.genomes[off[p]:off[p + 1]] for p in range(64)]
+    variants = {
+        "post0add": [np.concatenate([b, [zero, ADD]]) for b in base],
+        "post1mul": [np.concatenate([b, [one, MUL]]) for b in base],
+        "post1div": [np.concatenate([b, [one, DIV]]) for b in base],
+        "pre0add": [np.concatenate([[zero], b, [ADD]]) for b in base],
+    }
+    tax = 0.001
+    r0 = ev(oracle, base, consts, col.X, col.y, tax=tax, want_outputs=True)
+    m0 = ev(oracle, base, consts, col.X, col.y, tax=0.0)["fitness"]
+    for name, progs in variants.items():
+        r1 = ev(oracle, progs, consts, col.X, col.y, tax=tax, want_outputs=True)
+        a, b = r0["outputs"], r1["outputs"]
+        assert np.array_equal(np.isnan(a), np.isnan(b)), name
+        ok = ~np.isnan(a)
+        assert np.array_equal(a[ok], b[ok]), name              # bitwise (x+0, x*1, x/1 exact)
+        m1 = ev(oracle, progs, consts, col.X, col.y, tax=0.0)["fitness"]
+        np.testing.assert_array_equal(m0, m1)
+        fin = np.isfinite(r0["fitness"])
+        diff = r1["fitness"][fin].astype(np.float64) - r0["fitness"][fin]
+        assert np.all(np.abs(diff - 2 * tax) <= 2e-7 * np.maximum(1, np.abs(r0["fitness"][fin])))
+
+
+# ---- P6: commutativity, antisymmetry -> stack order ------------------------------------------------
+def test_P6_commutativity_and_sub_antisymmetry(oracle):
+    rng = np.random.default_rng(6)
+    X = rng.uniform(-2, 2, (128, 2)).astype(np.float32)
+    y = rng.normal(size=128).astype(np.float32)
+    A, B = "x0 1.5 MUL SIN", "x1 x0 DIV 0.25 ADD"
+    consts = []
+    progs = [asm(f"{A} {B} ADD", consts)[0], asm(f"{B} {A} ADD", consts)[0],
+             asm(f"{A} {B} MUL", consts)[0], asm(f"{B} {A} MUL", consts)[0],
+             asm(f"{A} {B} SUB", consts)[0], asm(f"{B} {A} SUB", consts)[0],
+             asm(f"{A} {B} DIV", consts)[0], asm(f"{B} {A} DIV", consts)[0]]
+    r = ev(oracle, progs, consts, X, y, want_outputs=True)["outputs"]
+    assert np.array_equal(r[0], r[1]) and np.array_equal(r[2], r[3])
+    assert np.array_equal(r[4], -r[5]) and not np.array_equal(r[4], r[5])
+    assert not np.allclose(r[6], r[7])
+    # SUB is second-top minus top: "3 1 SUB" = 2; DIV second-top / top: "3 2 DIV" = 1.5
+    r = ev(oracle, [asm("3 1 SUB")[0]], asm("3 1 SUB")[1], X, y, want_outputs=True)["outputs"]
+    assert np.all(r == 2.0)
+    r = ev(oracle, [asm("3 2 DIV")[0]], asm("3 2 DIV")[1], X, y, want_outputs=True)["outputs"]
+    assert np.all(r == 1.5)
+
+
+# ---- P7: protected operators at their edges (D2) ----------------------------------------
+INF, NAN = math.inf, math.nan
+EPSF = float(np.float32(1e-6))
+E80 = math.exp(80.0)
+EDGES = [
+    ("x0 x1 DIV", (3.0, 0.0), 1.0), ("x0 x1 DIV", (0.0, 0.0), 1.0), ("x0 x1 DIV", (NAN, 0.0), 1.0),
+    ("x0 x1 DIV", (1.0, INF), 0.0), ("x0 x1 DIV", (1.0, -INF), -0.0), ("x0 x1 DIV", (INF, INF), NAN),
+    ("x0 x1 DIV", (2.0, EPSF), 2.0 / EPSF),                      # strict '<': |b| == EPS divides
+    ("x0 x1 DIV", (2.0, float(np.nextafter(np.float32(1e-6), np.float32(0)))), 1.0),
+    ("x0 x1 DIV", (2.0, -0.5e-6), 1.0), ("x0 x1 DIV", (2.0, NAN), NAN), ("x0 x1 DIV", (INF, 2.0), INF),
+    ("x0 x1 DIV", (-INF, 2.0), -INF), ("x0 x1 DIV", (6.0, -3.0), -2.0),
+    ("x0 LOG", (0.0,), 0.0), ("x0 LOG", (-math.e,), math.log(float(np.float32(math.e)))),
+    ("x0 LOG", (INF,), INF), ("x0 LOG", (-INF,), INF), ("x0 LOG", (NAN,), NAN),
+    ("x0 LOG", (0.5e-6,), 0.0), ("x0 LOG", (EPSF,), math.log(EPSF)), ("x0 LOG", (1.0,), 0.0),
+    ("x0 SQRT", (-4.0,), 2.0), ("x0 SQRT", (0.0,), 0.0), ("x0 SQRT", (-0.0,), 0.0),
+    ("x0 SQRT", (INF,), INF), ("x0 SQRT", (-INF,), INF), ("x0 SQRT", (NAN,), NAN),
+    ("x0 SQRT", (1e-45,), math.sqrt(float(np.float32(1e-45)))),
+    ("x0 EXP", (81.0,), E80), ("x0 EXP", (INF,), E80), ("x0 EXP", (80.0,), E80),
+    ("x0 EXP", (-INF,), 0.0), ("x0 EXP", (NAN,), NAN), ("x0 EXP", (0.0,), 1.0),
+    ("x0 EXP", (3.0e38,), E80), ("x0 EXP", (-200.0,), math.exp(-200.0)),
+    ("x0 SIN", (INF,), NAN), ("x0 SIN", (-INF,), NAN), ("x0 COS", (INF,), NAN), ("x0 SIN", (0.0,), 0.0),
+    ("x0 COS", (0.0,), 1.0), ("x0 SIN", (NAN,), NAN),
+    ("x0 x1 ADD", (3.0e38, 3.0e38), INF), ("x0 x1 SUB", (INF, INF), NAN), ("x0 x1 MUL", (INF, 0.0), NAN),
+    ("x0 x1 MUL", (3.0e38, -2.0), -INF), ("x0 x1 ADD", (3.4028234663852886e38, 0.0), 3.4028234663852886e38),
+    ("x0 x1 SUB", (1.0, 2.5), -1.5),
+]
+
+
+@pytest.mark.parametrize("text,xs,want", EDGES)
+def test_P7_edge_table(oracle, text, xs, want):
+    X = np.array([list(xs) + [0.0] * (2 - len(xs))], np.float32)
+    prog, c = asm(text)
+    out = ev(oracle, [prog], c, X, np.zeros(1, np.float32), want_outputs=True)["outputs"][0, 0]
+    if isinstance(want, float) and math.isnan(want):
+        assert math.isnan(out)
+    else:
+        assert out == pytest.approx(want, rel=1e-15, abs=0.0)
+        if want == 0.0:
+            assert out == 0.0
+
+
+def test_P7_signed_zero_constant_survives(oracle):
+    # "CONST -0" is printed in the paper; -0 + b must give b, and 1/(-0 protected) = 1
+    X = np.array([[2.0, 0.0]], np.float32)
+    prog, c = asm("-0.0 x0 ADD")
+    assert np.signbit(c[0])
+    assert ev(oracle, [prog], c, X, np.zeros(1, np.float32), want_outputs=True)["outputs"][0, 0] == 2.0
+
+
+# ---- P8: brute force against the independent recursive evaluator ----------------------------------
+def test_P8_bruteforce_up_to_3_tokens(oracle):
+    from oracle import infix_check
+    consts = np.array([0.5, -2.25], np.float32)
+    X = np.array([[0.0, 1.0], [-1.5, 2.0e-7], [3.0e19, -4.0], [88.0, 1.0e30]], np.float32)
+    y = np.array([0.25, -1.0, 2.0, 0.0], np.float32)
+    terms = [C.token(C.OP["LOAD"], 0), C.token(C.OP["LOAD"], 1), C.token(C.OP["CONST"], 0), C.token(C.OP["CONST"], 1)]
+    un = [C.token(C.OP[k]) for k in ("SIN", "COS", "LOG", "SQRT", "EXP")]
+    bn = [C.token(C.OP[k]) for k in ("ADD", "SUB", "MUL", "DIV")]
+    progs = [[t] for t in terms]
+    progs += [[t, u] for t in terms for u in un]
+    progs += [[t, u1, u2] for t in terms for u1 in un for u2 in un]
+    progs += [[t1, t2, b] for t1 in terms for t2 in terms for b in bn]
+    assert len(progs) == 4 + 20 + 100 + 64  # = 188
+    arrs = [np.array(p, np.int32) for p in progs]
+    tax = 0.001
+    r = ev(oracle, arrs, consts, X, y, tax=tax)
+    n_nonfinite = 0
+    for p, a in enumerate(arrs):
+        want = infix_check.fitness(symbolic(a, consts), X, y, np.float32(tax))
+        got = float(r["fitness"][p])
+        want32 = float(np.float32(want)) if not math.isnan(want) else want
+        if math.isnan(want32):
+            assert math.isnan(got), (p, symbolic(a, consts))
+            n_nonfinite += 1
+        elif math.isinf(want32):
+            assert got == want32, (p, symbolic(a, consts))
+            n_nonfinite += 1
+        else:
+            assert got == pytest.approx(want32, rel=2e-7), (p, symbolic(a, consts))
+    assert n_nonfinite > 10  # the cases were picked so that overflow/NaN paths are exercised
+
+
+# ---- P9: power-of-two scaling ----------------------------------------------------------------------
+@pytest.mark.parametrize("mode", [0, 1])
+def test_P9_power_of_two_scaling(oracle, mode):
+    col = C.make_colony(1, P=128)
+    off = np.concatenate([[0], np.cumsum(col.lengths)])
+    nC = len(col.consts)
+    consts = list(col.consts) + [np.float32(2.0)]
+    two, MUL = C.token(C.OP["CONST"], nC), C.token(C.OP["MUL"])
+    base = [col.genomes[off[p]:off[p + 1]] for p in range(128)]
+    scaled = [np.concatenate([b, [two, MUL]]) for b in base]
+    f0 = ev(oracle, base, consts, col.X, col.y, tax=0.0, mode=mode)["fitness"].astype(np.float64)
+    f1 = ev(oracle, scaled, consts, col.X, 2 * col.y, tax=0.0, mode=mode)["fitness"].astype(np.float64)
+    fin = np.isfinite(f0) & np.isfinite(f1) & (f0 > 1e-30) & (f1 < 1e37)
+    assert fin.sum() > 100
+    assert np.array_equal(4.0 * f0[fin], f1[fin])   # exact, fp64 carrier and fp32 mirror alike
+
+
+# ---- P10: overflow semantics (D4-D6) ---------------------------------------------------------------
+def test_P10_overflow_semantics(oracle):
+    X = np.ones((8, 1), np.float32)
+    y0 = np.zeros(8, np.float32)
+    consts = []
+    progs = [asm("100 EXP 100 EXP MUL", consts)[0],                       # e80*e80 -> +inf
+             asm("100 EXP 100 EXP MUL 100 EXP 100 EXP MUL SUB", consts)[0],  # inf - inf -> NaN
+             asm("69 EXP", consts)[0],                                    # 9.3e29 finite, square overflows
+             asm("40 EXP", consts)[0]]                                    # 2.35e17, square 5.5e34 finite
+    r = ev(oracle, progs, consts, X, y0, want_outputs=True)
+    assert np.all(np.isposinf(r["outputs"][0])) and np.isposinf(r["fitness"][0])
+    assert np.all(np.isnan(r["outputs"][1])) and np.isnan(r["fitness"][1])
+    assert np.all(np.isfinite(r["outputs"][2])) and np.isposinf(r["fitness"][2])
+    assert np.isfinite(r["fitness"][3]) and r["fitness"][3] == pytest.approx(math.exp(80.0), rel=1e-6)
+    # D5: the sum overflows before the division by N: 8 terms of 1e38 -> +inf although the mean is 1e38
+    X2 = np.full((8, 1), 1.0e19, np.float32)
+    r2 = ev(oracle, [asm("x0")[0]], np.zeros(1, np.float32), X2, y0)
+    assert np.isposinf(r2["fitness"][0])
+    r3 = ev(oracle, [asm("x0")[0]], np.zeros(1, np.float32), X2[:2], y0[:2])
+    assert np.isfinite(r3["fitness"][0])
+
+
+def test_malformed_programs_get_canonical_nan(oracle):
+    X = np.ones((4, 2), np.float32)
+    y = np.zeros(4, np.float32)
+    consts = np.array([1.0], np.float32)
+    T = C.token
+    bad = [
+        np.array([T(C.OP["ADD"])], np.int32),                               # pops from empty
+        np.array([T(C.OP["LOAD"], 0), T(C.OP["ADD"])], np.int32),           # binary with one operand
+        np.array([T(C.OP["LOAD"], 2)], np.int32),                           # LOAD arg >= d
+        np.array([T(C.OP["CONST"], 1)], np.int32),                          # CONST arg >= n_consts
+        np.array([T(0)], np.int32),                                         # opcode 0
+        np.array([T(0x10)], np.int32),                                      # reserved (DUP)
+        np.array([T(C.OP["LOAD"], 0), T(C.OP["SIN"], 5)], np.int32),        # operator with arg
+        np.array([T(C.OP["LOAD"], 0)] * 33 + [T(C.OP["ADD"])] * 32, np.int32),  # depth 33
+    ]
+    good = [np.array([T(C.OP["LOAD"], 0)] * 32 + [T(C.OP["ADD"])] * 31, np.int32),  # depth 32 is fine
+            np.array([T(C.OP["LOAD"], 0), T(C.OP["LOAD"], 1)], np.int32)]            # final depth 2 (R8)
+    r = ev(oracle, bad + good, consts, X, y)
+    bits = r["fitness"].view(np.uint32)
+    assert np.all(bits[:len(bad)] == QNAN_BITS)
+    assert np.all(r["flags"][:len(bad)] & oracle.FLAG_MALFORMED)
+    assert np.all(r["depth"][:len(bad)] == 0)
+    assert r["fitness"][len(bad)] == 32.0 ** 2 and r["depth"][len(bad)] == 32
+    assert r["fitness"][len(bad) + 1] == 1.0 and r["depth"][len(bad) + 1] == 2   # top of stack = x1
+    # lengths outside [1,512] are malformed and count as 0 words
+    g = np.array([T(C.OP["LOAD"], 0)], np.int32)
+    l = np.array([0, -3, 600, 1], np.int32)
+    rr = oracle.evaluate(g, l, consts, X, y, 0.0)
+    assert np.all(rr["fitness"].view(np.uint32)[:3] == QNAN_BITS) and rr["fitness"][3] == 1.0
+
+
+# ---- P11: the bound is a bound (fp32 mirror vs fp64 truth) -----------------------------------------
+@pytest.mark.parametrize("cfg,P", [(1, 1024), (2, 6144)])
+def test_P11_error_bound_covers_fp32_mirror(oracle, cfg, P):
+    col = C.make_colony(cfg, P=P)
+    ieee = oracle.contract(oracle.CONTRACT_IEEE)
+    ieee.sum_per_case, ieee.sum_const = 0.0, 1.0   # the mirror sums in fp64: no fp32 summation error
+    t = oracle.evaluate_parallel(col.genomes, col.lengths, col.consts, col.X, col.y, col.tax, contract_=ieee, mode=0)
+    m = oracle.evaluate_parallel(col.genomes, col.lengths, col.consts, col.X, col.y, col.tax, contract_=ieee, mode=1)
+    stable = (t["flags"] & (oracle.FLAG_UNSTABLE | oracle.FLAG_CLASS_UNSTABLE)) == 0
+    ft, fm = t["fitness"].astype(np.float64), m["fitness"].astype(np.float64)
+    # class parity on stable individuals
+    assert np.array_equal(np.isnan(ft[stable]), np.isnan(fm[stable]))
+    assert np.array_equal(np.isinf(ft[stable]), np.isinf(fm[stable]))
+    fin = stable & np.isfinite(ft)
+    slack = 2.0 ** -23 * np.abs(ft[fin])             # the two final float casts
+    viol = np.abs(ft[fin] - fm[fin]) > t["bound"][fin] + slack
+    assert not viol.any(), (np.flatnonzero(fin)[viol][:5], ft[fin][viol][:5], fm[fin][viol][:5], t["bound"][fin][viol][:5])
+    assert stable.mean() > 0.98
+    # and the bound is not vacuous: most individuals certify the north_star tolerance
+    tol = np.maximum(1e-4 * np.abs(ft[fin]), 1e-6)
+    assert (4 * t["bound"][fin] <= tol).mean() > 0.85
+
+
+# ---- P12: duplicating the case set leaves the MSE unchanged ----------------------------------------
+def test_P12_case_duplication(oracle):
+    col = C.make_colony(1, P=256)
+    X2, y2 = np.concatenate([col.X, col.X]), np.concatenate([col.y, col.y])
+    a = oracle.evaluate(col.genomes, col.lengths, col.consts, col.X, col.y, 0.0)["fitness"]
+    b = oracle.evaluate(col.genomes, col.lengths, col.consts, X2, y2, 0.0)["fitness"]
+    fin = np.isfinite(a)
+    assert np.array_equal(np.isfinite(a), np.isfinite(b))
+    np.testing.assert_allclose(a[fin], b[fin], rtol=2e-7)
+
+
+def test_parallel_fanout_equals_single_thread(oracle):
+    col = C.make_colony(1)
+    a = oracle.evaluate(col.genomes, col.lengths, col.consts, col.X, col.y, col.tax)
+    b = oracle.evaluate_parallel(col.genomes, col.lengths, col.consts, col.X, col.y, col.tax, threads=4)
+    for k in ("fitness", "bound", "flags", "depth"):
+        assert np.array_equal(a[k], b[k], equal_nan=True)

@@ -1,0 +1,46 @@
+"""Test helpers: a tiny assembler from text to packed tokens (encoding only, no arithmetic)."""
+import numpy as np
+
+from paper_2607_06731_b200.colonies import OP, token
+
+_NAMES = {"ADD": "add", "SUB": "sub", "MUL": "mul", "DIV": "div", "SIN": "sin", "COS": "cos",
+          "LOG": "log", "SQRT": "sqrt", "EXP": "exp"}
+
+
+def asm(text, consts=None, const_base=0):
+    """'x0 x1 ADD 2.5 MUL' -> (tokens int32[], consts float32[]). Numbers become CONST entries
+    appended to `consts` (a list that is extended in place if given)."""
+    cl = [] if consts is None else consts
+    toks = []
+    for w in text.replace(";", " ").split():
+        u = w.upper()
+        if u in OP and u not in ("CONST", "LOAD"):
+            toks.append(token(OP[u]))
+        elif u.startswith("X") and u[1:].isdigit():
+            toks.append(token(OP["LOAD"], int(u[1:])))
+        else:
+            cl.append(np.float32(float(w)))
+            toks.append(token(OP["CONST"], const_base + len(cl) - 1))
+    return np.array(toks, np.int32), np.array(cl, np.float32)
+
+
+def symbolic(tokens, consts):
+    """Packed tokens -> the symbolic form oracle/infix_check.py takes."""
+    out = []
+    inv = {v: k for k, v in OP.items()}
+    for w in np.asarray(tokens).astype(np.uint32):
+        op, arg = int(w & 0xFF), int(w >> 8)
+        if op == OP["CONST"]:
+            out.append(("c", float(consts[arg])))
+        elif op == OP["LOAD"]:
+            out.append(("x", arg))
+        else:
+            out.append(_NAMES[inv[op]])
+    return out
+
+
+def pack(programs, consts):
+    """list of token arrays -> (genomes, lengths, consts)."""
+    lengths = np.array([len(p) for p in programs], np.int32)
+    genomes = np.concatenate(programs).astype(np.int32) if programs else np.zeros(0, np.int32)
+    return genomes, lengths, np.asarray(consts, np.float32)
