@@ -166,12 +166,14 @@ void beagle_release(void);
 /* Number of kernels the most recent beagle_eval* call launched (for bench.py's gpu_launches). */
 int32_t beagle_last_launch_count(void);
 
-/* Device time, in milliseconds, of the evaluation kernels alone (the interpreter launches, without
- * the scheduling pre-pass) of the most recent beagle_eval call made while profiling was enabled
- * with beagle_set_profiling(1). Reading it synchronises on the recorded events. Returns < 0 if
- * nothing was recorded. */
+/* Profiling hooks for bench.py's roofline line. While profiling is on, every beagle_eval call
+ * brackets its evaluation kernels (the interpreter launches, without the scheduling pre-pass) with
+ * a pair of CUDA events on `stream` (at most 256 calls are recorded; later ones are not).
+ * beagle_profiled_eval_kernel_ms synchronises on the recorded events, stores the number of
+ * recorded calls in *n_calls (may be NULL) and returns their mean device time in milliseconds
+ * (< 0 if nothing was recorded). beagle_set_profiling(1) clears the record. */
 void  beagle_set_profiling(int32_t on);
-float beagle_last_eval_kernel_ms(void);
+float beagle_profiled_eval_kernel_ms(int32_t* n_calls);
 
 #ifdef __cplusplus
 }

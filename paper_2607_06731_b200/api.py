@@ -1,0 +1,161 @@
+"""Thin ctypes binding of libbeagle_b200.so (include/beagle.h) — argument marshalling only.
+
+Every function has the name and argument order of its C entry point; tensors are passed as raw
+pointers (`tensor.data_ptr()`), streams as `torch.cuda.current_stream().cuda_stream`. PyTorch
+supplies device memory and streams, nothing else: every step of the path runs in the library's
+kernels. There is no CPU fallback: if the library is missing or a call fails, this raises.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+
+from . import build as _build
+
+OK = 0
+ERR_INVALID_ARG = -1
+ERR_UNSUPPORTED = -2
+ERR_CUDA = -3
+ERR_NOMEM = -4
+
+
+class BeagleError(RuntimeError):
+    def __init__(self, status: int, where: str):
+        self.status = status
+        msg = lib().beagle_status_string(status).decode()
+        extra = f" (cudaError {lib().beagle_last_cuda_error()})" if status in (ERR_CUDA, ERR_NOMEM) else ""
+        super().__init__(f"{where}: {msg}{extra}")
+
+
+_lib = None
+_i32, _i64, _f32, _vp = ctypes.c_int32, ctypes.c_int64, ctypes.c_float, ctypes.c_void_p
+
+_SIGNATURES = {
+    "beagle_eval": (_i32, [_vp, _vp, _i64, _vp, _i64, _vp, _vp, _i32, _i32, _f32, _vp, _vp]),
+    "beagle_eval_chunked": (_i32, [_vp, _vp, _i64, _vp, _i64, _vp, _vp, _i32, _i32, _f32, _vp, _i64, _vp]),
+    "beagle_eval_blockwise": (_i32, [_vp, _vp, _i64, _vp, _i64, _vp, _vp, _i32, _i32, _f32, _vp, _vp]),
+    "beagle_debug_outputs": (_i32, [_vp, _vp, _i64, _vp, _i64, _vp, _i32, _i32, _vp, _vp]),
+    "beagle_debug_schedule": (_i32, [_i64, _vp, _vp, _vp, _vp]),
+    "beagle_limits": (None, [ctypes.POINTER(_i32)] * 4),
+    "beagle_status_string": (ctypes.c_char_p, [_i32]),
+    "beagle_last_cuda_error": (_i32, []),
+    "beagle_reserve": (_i32, [_i64, _i64]),
+    "beagle_reserve_chunked": (_i32, [_i64]),
+    "beagle_release": (None, []),
+    "beagle_last_launch_count": (_i32, []),
+    "beagle_set_profiling": (None, [_i32]),
+    "beagle_profiled_eval_kernel_ms": (_f32, [ctypes.POINTER(_i32)]),
+}
+EXPORTS = tuple(_SIGNATURES)
+
+
+def library_path() -> str:
+    return _build.LIB
+
+
+def lib():
+    """Load (building first if the in-tree .so is missing or stale). Fails loudly."""
+    global _lib
+    if _lib is None:
+        path = _build.LIB
+        if not os.path.exists(path) or os.environ.get("BEAGLE_REBUILD") == "1":
+            path = _build.build()
+        l = ctypes.CDLL(path)
+        for name, (res, args) in _SIGNATURES.items():
+            fn = getattr(l, name)       # AttributeError if a declared symbol is not exported
+            fn.restype, fn.argtypes = res, args
+        _lib = l
+    return _lib
+
+
+def _ptr(t):
+    """torch tensor / numpy array / int / None -> address."""
+    if t is None:
+        return None
+    if isinstance(t, int):
+        return t
+    if hasattr(t, "data_ptr"):
+        return t.data_ptr()
+    return t.ctypes.data
+
+
+def _check(status: int, where: str):
+    if status != OK:
+        raise BeagleError(status, where)
+
+
+def beagle_eval(genomes, lengths, P, consts, n_consts, X, y, N, d, tax, fitness_out, stream=0):
+    _check(lib().beagle_eval(_ptr(genomes), _ptr(lengths), int(P), _ptr(consts), int(n_consts),
+                             _ptr(X), _ptr(y), int(N), int(d), float(tax), _ptr(fitness_out),
+                             int(stream) or None), "beagle_eval")
+
+
+def beagle_eval_chunked(h_genomes, h_lengths, P, h_consts, n_consts, X, y, N, d, tax, fitness_out,
+                        device_budget_bytes, stream=0):
+    _check(lib().beagle_eval_chunked(_ptr(h_genomes), _ptr(h_lengths), int(P), _ptr(h_consts),
+                                     int(n_consts), _ptr(X), _ptr(y), int(N), int(d), float(tax),
+                                     _ptr(fitness_out), int(device_budget_bytes), int(stream) or None),
+           "beagle_eval_chunked")
+
+
+def beagle_eval_blockwise(genomes, lengths, P, consts, n_consts, X, y, N, d, tax, fitness_out, stream=0):
+    _check(lib().beagle_eval_blockwise(_ptr(genomes), _ptr(lengths), int(P), _ptr(consts),
+                                       int(n_consts), _ptr(X), _ptr(y), int(N), int(d), float(tax),
+                                       _ptr(fitness_out), int(stream) or None), "beagle_eval_blockwise")
+
+
+def beagle_debug_outputs(genomes, lengths, P, consts, n_consts, X, N, d, out_PxN, stream=0):
+    _check(lib().beagle_debug_outputs(_ptr(genomes), _ptr(lengths), int(P), _ptr(consts),
+                                      int(n_consts), _ptr(X), int(N), int(d), _ptr(out_PxN),
+                                      int(stream) or None), "beagle_debug_outputs")
+
+
+def beagle_debug_schedule(P, off, depth, perm, stream=0):
+    _check(lib().beagle_debug_schedule(int(P), _ptr(off), _ptr(depth), _ptr(perm), int(stream) or None),
+           "beagle_debug_schedule")
+
+
+def beagle_limits():
+    v = [_i32() for _ in range(4)]
+    lib().beagle_limits(*[ctypes.byref(x) for x in v])
+    return dict(max_len=v[0].value, max_stack=v[1].value, max_n=v[2].value, max_d=v[3].value)
+
+
+def beagle_status_string(status: int) -> str:
+    return lib().beagle_status_string(int(status)).decode()
+
+
+def beagle_last_cuda_error() -> int:
+    return lib().beagle_last_cuda_error()
+
+
+def beagle_reserve(P_max, T_max=0):
+    _check(lib().beagle_reserve(int(P_max), int(T_max)), "beagle_reserve")
+
+
+def beagle_reserve_chunked(device_budget_bytes):
+    _check(lib().beagle_reserve_chunked(int(device_budget_bytes)), "beagle_reserve_chunked")
+
+
+def beagle_release():
+    lib().beagle_release()
+
+
+def beagle_last_launch_count() -> int:
+    return lib().beagle_last_launch_count()
+
+
+def beagle_set_profiling(on: bool):
+    lib().beagle_set_profiling(1 if on else 0)
+
+
+def beagle_profiled_eval_kernel_ms():
+    """(number of recorded calls, mean device ms of their evaluation kernels)."""
+    n = _i32(0)
+    ms = float(lib().beagle_profiled_eval_kernel_ms(ctypes.byref(n)))
+    return n.value, ms
+
+
+def raw_status(name: str, *args) -> int:
+    """Call an entry point and return its status instead of raising (for the argument-error tests)."""
+    return getattr(lib(), name)(*args)

@@ -190,10 +190,11 @@ def make_dataset(cfg: ColonyConfig):
     return X.astype(np.float32), y.astype(np.float32), expr
 
 
-def generate_programs(cfg: ColonyConfig, P: int | None = None):
-    """tokens int32[T], lengths int32[P], consts float32[C] for the first P individuals of cfg."""
+def generate_programs(cfg: ColonyConfig, P: int | None = None, seed_offset: int = 0):
+    """tokens int32[T], lengths int32[P], consts float32[C] for the first P individuals of cfg.
+    seed_offset != 0 draws a different colony of the same shape (bench.py: one per rank)."""
     P = cfg.P if P is None else int(P)
-    seed = 0xBEA61E00 + cfg.number
+    seed = 0xBEA61E00 + cfg.number + int(seed_offset)
     un = (ctypes.c_int * len(cfg.unary))(*cfg.unary)
     bn = (ctypes.c_int * len(cfg.binary))(*cfg.binary)
     lengths = np.empty(P, np.int32)

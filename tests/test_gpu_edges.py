@@ -1,0 +1,226 @@
+"""-m gpu: edge cases, in-band error reporting and self-consistency of the CUDA path (SURVEY.md §4
+items 2 and 4): bitwise determinism, permutation/duplication/chunking invariance, malformed programs,
+limits, exact length tax, exact power-of-two scaling, and bit-exact per-case outputs for programs
+made of correctly rounded commands only.
+"""
+import ctypes
+
+import numpy as np
+import pytest
+
+from paper_2607_06731_b200 import colonies
+from paper_2607_06731_b200.colonies import OP, token
+from tests import parity
+from tests.util import asm, pack
+
+pytestmark = pytest.mark.gpu
+
+QNAN = np.uint32(0x7FC00000)
+
+
+def _bits(a):
+    return np.asarray(a, np.float32).view(np.uint32)
+
+
+def _cases(N=64, d=2, seed=3):
+    rng = np.random.default_rng(seed)
+    X = (rng.integers(-2048, 2048, (N, d)) / 2048.0).astype(np.float32)   # 12 significant bits
+    return X
+
+
+def test_empty_population():
+    import torch
+    from paper_2607_06731_b200 import api
+    X = torch.zeros((4, 1), device="cuda")
+    y = torch.zeros(4, device="cuda")
+    api.beagle_eval(None, None, 0, None, 0, X, y, 4, 1, 0.0, None, 0)
+    assert api.beagle_last_launch_count() == 0
+
+
+def test_argument_errors():
+    import torch
+    from paper_2607_06731_b200 import api
+    l = api.lib()
+    X = torch.zeros((4, 1), device="cuda"); y = torch.zeros(4, device="cuda")
+    g = torch.zeros(4, dtype=torch.int32, device="cuda"); ln = torch.ones(4, dtype=torch.int32, device="cuda")
+    out = torch.zeros(4, device="cuda")
+    def call(**kw):
+        a = dict(genomes=g.data_ptr(), lengths=ln.data_ptr(), P=4, consts=None, n_consts=0, X=X.data_ptr(),
+                 y=y.data_ptr(), N=4, d=1, tax=0.0, out=out.data_ptr())
+        a.update(kw)
+        return l.beagle_eval(a["genomes"], a["lengths"], a["P"], a["consts"], a["n_consts"], a["X"], a["y"],
+                             a["N"], a["d"], a["tax"], a["out"], None)
+    assert call() == api.OK
+    assert call(P=-1) == api.ERR_INVALID_ARG
+    assert call(N=0) == api.ERR_INVALID_ARG
+    assert call(N=1025) == api.ERR_INVALID_ARG
+    assert call(d=0) == api.ERR_INVALID_ARG
+    assert call(d=33) == api.ERR_INVALID_ARG
+    assert call(n_consts=1) == api.ERR_INVALID_ARG            # consts NULL with n_consts > 0
+    assert call(n_consts=(1 << 24) + 1, consts=g.data_ptr()) == api.ERR_INVALID_ARG
+    assert call(genomes=None) == api.ERR_INVALID_ARG
+    assert call(out=None) == api.ERR_INVALID_ARG
+    assert l.beagle_eval_chunked(None, None, 4, None, 0, X.data_ptr(), y.data_ptr(), 4, 1, 0.0,
+                                 out.data_ptr(), 1 << 20, None) == api.ERR_INVALID_ARG
+    torch.cuda.synchronize()
+    assert "invalid" in api.beagle_status_string(api.ERR_INVALID_ARG)
+
+
+def test_malformed_programs_give_canonical_nan(oracle):
+    """DESIGN.md D3 / R9-R10: every kind of malformed program, mixed with valid ones."""
+    from tests.gpu_util import gpu_eval
+    X = _cases(64, 2)
+    y = (X[:, 0] * X[:, 0]).astype(np.float32)
+    consts = [np.float32(1.5)]
+    good = asm("x0 x0 MUL")[0]
+    progs = [
+        good,
+        np.array([token(OP["ADD"])], np.int32),                               # pops an empty stack
+        np.array([token(OP["LOAD"], 0), token(OP["ADD"])], np.int32),         # binary on depth 1
+        np.array([token(OP["SIN"])], np.int32),                               # unary on depth 0
+        np.array([token(0)], np.int32),                                       # opcode 0
+        np.array([token(0x10)], np.int32),                                    # reserved opcode (DUP)
+        np.array([token(0xFF, 5)], np.int32),                                 # unknown opcode
+        np.array([token(OP["LOAD"], 2)], np.int32),                           # variable >= d
+        np.array([token(OP["CONST"], 1)], np.int32),                          # constant >= n_consts
+        np.array([token(OP["LOAD"], 0), token(OP["SIN"], 1)], np.int32),      # operator with arg != 0
+        np.array([token(OP["LOAD"], 0)] * 33 + [token(OP["ADD"])] * 32, np.int32),   # depth 33
+        good,
+        np.array([token(OP["LOAD"], 0)] * 32 + [token(OP["ADD"])] * 31, np.int32),   # depth 32: fine
+        np.array([token(OP["LOAD"], 0), token(OP["LOAD"], 1)], np.int32),     # final depth 2: fine (R8)
+    ]
+    g, l, c = pack(progs, consts)
+    fit = gpu_eval(g, l, c, X, y, 0.25)
+    orc = oracle.evaluate(g, l, c, X, y, 0.25)
+    assert np.all(_bits(fit[1:11]) == QNAN)
+    assert np.all((orc["flags"][1:11] & 1) == 1)
+    rep = parity.compare(fit, orc)
+    assert len(rep["bad"]) == 0, parity.describe(rep, fit, orc)
+    assert _bits(fit[0]) == _bits(np.float32(0.75)) and _bits(fit[11]) == _bits(np.float32(0.75))
+
+
+def test_out_of_range_lengths_count_as_zero_words(oracle):
+    from tests.gpu_util import gpu_eval
+    X = _cases(32, 2)
+    y = X[:, 1].copy()
+    p = asm("x1")[0]
+    genomes = np.concatenate([p, p, p]).astype(np.int32)
+    lengths = np.array([1, 0, -7, 513, 1, 1 << 30, 1], np.int32)
+    fit = gpu_eval(genomes, lengths, np.zeros(0, np.float32), X, y, 0.5)
+    assert np.all(_bits(fit[[1, 2, 3, 5]]) == QNAN)
+    assert np.all(fit[[0, 4, 6]] == np.float32(0.5))
+    orc = oracle.evaluate(genomes, lengths, np.zeros(0, np.float32), X, y, 0.5)
+    assert np.array_equal(_bits(fit), _bits(orc["fitness"]))
+
+
+def test_length_tax_exact():
+    """R15: a program with MSE exactly 0 returns (float)(tax*L) bit-exactly, for every length class."""
+    from tests.gpu_util import gpu_eval
+    X = _cases(96, 2)
+    y = X[:, 0].copy()
+    progs, consts = [], [np.float32(0.0)]
+    for extra in (0, 1, 5, 30, 100, 255):
+        t = [token(OP["LOAD"], 0)] + [token(OP["CONST"], 0), token(OP["ADD"])] * extra
+        progs.append(np.array(t, np.int32))
+    progs.append(np.array([token(OP["LOAD"], 0)] + [token(OP["CONST"], 0)] * 20 + [token(OP["ADD"])] * 20, np.int32))
+    g, l, c = pack(progs, consts)
+    for tax in (0.001, 0.3, 7.0):
+        fit = gpu_eval(g, l, c, X, y, tax)
+        want = (np.float32(tax) * l.astype(np.float32)).astype(np.float32)
+        assert np.array_equal(_bits(fit), _bits(want)), (fit, want)
+
+
+def test_power_of_two_scaling_exact():
+    """Pin P9 on the GPU: `A 2 MUL` against 2y has exactly 4x the MSE of `A` against y."""
+    from tests.gpu_util import gpu_eval
+    col = colonies.make_colony(1)
+    consts = list(col.consts)
+    two = len(consts); consts.append(np.float32(2.0))
+    off = np.concatenate([[0], np.cumsum(col.lengths)])
+    progs2 = [np.concatenate([col.genomes[off[p]:off[p + 1]],
+                              np.array([token(OP["CONST"], two), token(OP["MUL"])], np.int32)]) for p in range(col.P)]
+    g2, l2, c2 = pack(progs2, consts)
+    f1 = gpu_eval(col.genomes, col.lengths, c2, col.X, col.y, 0.0)
+    f2 = gpu_eval(g2, l2, c2, col.X, (2 * col.y).astype(np.float32), 0.0)
+    ok = np.isfinite(f1) & np.isfinite(f2) & (f1 > 1e-30) & (f1 < 1e30)
+    assert ok.sum() > 900
+    assert np.array_equal(_bits(f2[ok]), _bits((4 * f1[ok]).astype(np.float32)))
+    assert np.array_equal(np.isnan(f1), np.isnan(f2))
+
+
+def test_determinism_permutation_duplication():
+    from tests.gpu_util import gpu_eval
+    col = colonies.make_colony(5, 6000)
+    f1 = gpu_eval(col.genomes, col.lengths, col.consts, col.X, col.y, col.tax)
+    f2 = gpu_eval(col.genomes, col.lengths, col.consts, col.X, col.y, col.tax)
+    assert np.array_equal(_bits(f1), _bits(f2))
+    off = np.concatenate([[0], np.cumsum(col.lengths, dtype=np.int64)])
+    rng = np.random.default_rng(11)
+    perm = rng.permutation(col.P)
+    perm = np.concatenate([perm, perm[:777]])                     # duplicates too
+    gp = np.concatenate([col.genomes[off[p]:off[p + 1]] for p in perm])
+    fp = gpu_eval(gp, col.lengths[perm], col.consts, col.X, col.y, col.tax)
+    assert np.array_equal(_bits(fp), _bits(f1[perm]))
+
+
+def test_blockwise_baseline_bitwise_equal():
+    from tests.gpu_util import gpu_eval
+    col = colonies.make_colony(2, 3000)
+    for N in (1024, 517):
+        a = gpu_eval(col.genomes, col.lengths, col.consts, col.X[:N], col.y[:N], col.tax)
+        b = gpu_eval(col.genomes, col.lengths, col.consts, col.X[:N], col.y[:N], col.tax, fn="beagle_eval_blockwise")
+        assert np.array_equal(_bits(a), _bits(b))
+
+
+@pytest.mark.parametrize("budget_frac,pinned", [(2.5, True), (0.37, True), (0.11, False), (0.013, True)])
+def test_chunked_bitwise_equals_unchunked(budget_frac, pinned):
+    from tests.gpu_util import gpu_eval, gpu_eval_chunked
+    col = colonies.make_colony(5, 20000)
+    ref = gpu_eval(col.genomes, col.lengths, col.consts, col.X, col.y, col.tax)
+    budget = max(int(col.T * 4 * budget_frac), 2 * 4 * 513 + 64)
+    out = gpu_eval_chunked(col.genomes, col.lengths, col.consts, col.X, col.y, col.tax, budget, pinned)
+    assert np.array_equal(_bits(out), _bits(ref))
+
+
+def test_chunked_minimum_budget_and_errors():
+    import torch
+    from paper_2607_06731_b200 import api
+    from tests.gpu_util import gpu_eval, gpu_eval_chunked
+    col = colonies.make_colony(5, 300)
+    ref = gpu_eval(col.genomes, col.lengths, col.consts, col.X, col.y, col.tax)
+    out = gpu_eval_chunked(col.genomes, col.lengths, col.consts, col.X, col.y, col.tax, 2 * 4 * 513 + 512)
+    assert np.array_equal(_bits(out), _bits(ref))
+    with pytest.raises(api.BeagleError):
+        gpu_eval_chunked(col.genomes, col.lengths, col.consts, col.X, col.y, col.tax, 1000)
+    torch.cuda.synchronize()
+
+
+def test_outputs_bit_exact_for_correctly_rounded_commands(oracle):
+    """SURVEY.md §8(c) cross-check: for programs made of ADD, SUB, MUL only the fp32-mirror oracle
+    (fp64 result of two fp32 operands, rounded to fp32 = the correctly rounded fp32 result) must
+    equal the GPU's per-case outputs bit for bit."""
+    from tests.gpu_util import gpu_outputs
+    cfg = colonies.CONFIGS[3]
+    tokens, lengths, consts = colonies.generate_programs(cfg, 30000)
+    X, y, _ = colonies.make_dataset(cfg)
+    off = np.concatenate([[0], np.cumsum(lengths, dtype=np.int64)])
+    ops = tokens & 0xFF
+    bad = (ops >= OP["DIV"]).astype(np.int64)
+    nbad = np.add.reduceat(bad, off[:-1])
+    sel = np.nonzero(nbad == 0)[0][:1500]
+    assert len(sel) > 500
+    g = np.concatenate([tokens[off[p]:off[p + 1]] for p in sel])
+    l = lengths[sel]
+    out = gpu_outputs(g, l, consts, X)
+    orc = oracle.evaluate(g, l, consts, X, y, 0.0, contract_=oracle.contract(oracle.CONTRACT_IEEE), mode=1,
+                          want_outputs=True)
+    want = orc["outputs"].astype(np.float32)
+    # denormal results are not flushed by IEEE add/sub/mul; compare every bit (NaN payloads aside)
+    same = (_bits(out) == _bits(want)) | (np.isnan(out) & np.isnan(want))
+    assert np.all(same), np.argwhere(~same)[:5]
+
+
+def test_limits_and_exports():
+    from paper_2607_06731_b200 import api
+    lim = api.beagle_limits()
+    assert lim == dict(max_len=512, max_stack=32, max_n=1024, max_d=32)

@@ -1,0 +1,111 @@
+"""-m gpu: the CUDA path (through the C-ABI binding) against the CPU oracle, element by element.
+
+Tolerance: north_star's rtol 1e-4 / atol 1e-6 on STRICT individuals, class parity exact, the
+three-class rule of tests/parity.py for the rest. Sizes: whole colonies for configs
+1-2, leading slices for configs 3-5 (the oracle finishes in seconds on all host cores; several
+work-queue batches, all depth classes and ragged tails are covered), and sampled individuals of the
+full-size colonies in the launch configuration bench.py times.
+"""
+import numpy as np
+import pytest
+
+from paper_2607_06731_b200 import colonies
+from tests import parity
+from tests.util import asm, pack
+
+pytestmark = pytest.mark.gpu
+
+
+def _check(col, oracle, gpu_fit, sel=None):
+    g, l, c = col.genomes, col.lengths, col.consts
+    if sel is not None:
+        off = np.concatenate([[0], np.cumsum(l, dtype=np.int64)])
+        g = np.concatenate([g[off[p]:off[p + 1]] for p in sel]) if len(sel) else np.zeros(0, np.int32)
+        l = l[sel]
+        gpu_fit = gpu_fit[sel]
+    orc = oracle.evaluate_parallel(g, l, c, col.X, col.y, col.tax)
+    rep = parity.compare(gpu_fit, orc)
+    msg = parity.describe(rep, gpu_fit, orc)
+    print(f"config {col.cfg.number}: {msg}")
+    assert len(rep["bad"]) == 0, msg
+    # the rule must not be vacuous: most individuals are STRICT (SURVEY.md §8(c) probe: 89-99 %)
+    assert rep["strict"] >= 0.70 * (rep["P"] - rep["malformed"] - rep["invalid"]), msg
+    return rep
+
+
+@pytest.mark.parametrize("number,P", [(1, None), (2, None), (3, 16384), (4, 8192), (5, 8192)])
+def test_parity_configs(oracle, number, P):
+    from tests.gpu_util import gpu_eval
+    col = colonies.make_colony(number, P)
+    fit = gpu_eval(col.genomes, col.lengths, col.consts, col.X, col.y, col.tax)
+    _check(col, oracle, fit)
+
+
+@pytest.mark.parametrize("number", [1, 3])
+def test_parity_blockwise_baseline(oracle, number):
+    """The prior-art mapping kept as a baseline computes the same definition."""
+    from tests.gpu_util import gpu_eval
+    col = colonies.make_colony(number, 4096 if number > 1 else None)
+    fit = gpu_eval(col.genomes, col.lengths, col.consts, col.X, col.y, col.tax, fn="beagle_eval_blockwise")
+    _check(col, oracle, fit)
+
+
+@pytest.mark.parametrize("number,stride", [(3, 401), (4, 1601)])
+def test_parity_full_size_sampled(oracle, number, stride):
+    """BASELINE.json's full sizes in the configuration bench.py times; the oracle checks every
+    `stride`-th individual plus the longest and the deepest ones."""
+    from tests.gpu_util import gpu_eval
+    col = colonies.make_colony(number)
+    fit = gpu_eval(col.genomes, col.lengths, col.consts, col.X, col.y, col.tax)
+    sel = np.arange(0, col.P, stride)
+    longest = np.argsort(-col.lengths, kind="stable")[:256]
+    sel = np.unique(np.concatenate([sel, longest]))
+    _check(col, oracle, fit, sel)
+    # properties that hold at any size: every individual got a value; tax*L is a lower bound of
+    # any finite fitness (MSE >= 0), up to one rounding
+    assert not np.any(fit == np.float32(-12345.0))
+    fin = np.isfinite(fit)
+    assert np.all(fit[fin] >= np.float32(col.tax) * col.lengths[fin] * np.float32(1 - 1e-6))
+
+
+def test_parity_config5_chunked_sampled(oracle):
+    """Config 5's mechanism (chunked streaming from pinned host memory under a device budget) at a
+    reduced population; the budget is scaled so that the same number of chunks (~3) results."""
+    from tests.gpu_util import gpu_eval_chunked, gpu_eval
+    col = colonies.make_colony(5, 262144)
+    budget = int(col.T * 4 * 0.8) & ~255
+    fit = gpu_eval_chunked(col.genomes, col.lengths, col.consts, col.X, col.y, col.tax, budget)
+    ref = gpu_eval(col.genomes, col.lengths, col.consts, col.X, col.y, col.tax)
+    assert np.array_equal(fit.view(np.uint32), ref.view(np.uint32))   # DESIGN.md R19: bit-identical
+    sel = np.unique(np.concatenate([np.arange(0, col.P, 61), np.arange(0, col.P, 20)[:2000]]))
+    rep = _check(col, oracle, fit, sel)
+    assert rep["invalid"] > 0     # the designed-invalid programs are in the sample
+
+
+@pytest.mark.parametrize("N", [1, 2, 31, 32, 33, 127, 128, 129, 500, 512, 513, 1000, 1023, 1024])
+def test_parity_ragged_case_counts(oracle, N):
+    from tests.gpu_util import gpu_eval
+    col = colonies.make_colony(2, 700)
+    X, y = col.X[:N], col.y[:N]
+    fit = gpu_eval(col.genomes, col.lengths, col.consts, X, y, col.tax)
+    orc = oracle.evaluate(col.genomes, col.lengths, col.consts, X, y, col.tax)
+    rep = parity.compare(fit, orc)
+    assert len(rep["bad"]) == 0, parity.describe(rep, fit, orc)
+
+
+def test_parity_wide_inputs_d32(oracle):
+    """d at its limit (32 variables, 1024 cases: the largest staged case block)."""
+    from tests.gpu_util import gpu_eval
+    rng = np.random.default_rng(7)
+    d, N = 32, 1024
+    X = rng.uniform(-2, 2, (N, d)).astype(np.float32)
+    y = (X[:, 31] * X[:, 0]).astype(np.float32)
+    consts = []
+    progs = []
+    for j in range(d):
+        progs.append(asm(f"x{j} x{(j * 7 + 3) % d} MUL x31 ADD", consts)[0])
+    g, l, c = pack(progs, consts if consts else np.zeros(0, np.float32))
+    fit = gpu_eval(g, l, c, X, y, 0.01)
+    orc = oracle.evaluate(g, l, c, X, y, 0.01)
+    rep = parity.compare(fit, orc)
+    assert len(rep["bad"]) == 0, parity.describe(rep, fit, orc)
