@@ -1,13 +1,13 @@
 // beagle.cu — libbeagle_b200.so: the C-ABI of include/beagle.h and every kernel behind it.
 //
 // Hot path:
-//   a2  k_block_sums / k_scan_block_sums            exclusive prefix sum of lengths -> off[]
-//   a3  k_program_scan / k_bins_and_cases / k_scatter
-//                                                    per-program scan (max stack depth, well-formedness),
-//                                                    counting sort by (depth class, length) -> perm[]
-//   a4  k_bins_and_cases + TMA in the eval kernel   X,y transposed/padded once, bulk-copied per CTA
-//   a5-a7  k_eval_* (eval_kernel.inc)               fetch, decode, interpret, reduce, tax, store
-//   a8  beagle_eval_chunked                         double-buffered H2D on a copy stream
+//   a2  k_len_pass1 / k_len_pass2      block sums + length histogram; exclusive scans -> offsets, bins
+//   a3  k_scatter                      off[], counting sort by length (longest first) -> perm[]
+//       k_compile                      per-program well-formedness, tree compile to micro-ops (uop.cuh):
+//                                      terminal folding, Sethi-Ullman slot allocation
+//   a4  k_len_pass2 + TMA in k_eval    X,y transposed/padded once, bulk-copied per CTA
+//   a5-a7  k_eval_* (eval_kernel.inc)  TMA-fed interpreter: fetch, interpret, reduce, tax, store
+//   a8  beagle_eval_chunked            double-buffered H2D on a copy stream
 // PyTorch is not involved: only the CUDA runtime. sm_100a only.
 #include <cuda_runtime.h>
 #include <stdint.h>
@@ -16,41 +16,46 @@
 
 #include "../../include/beagle.h"
 #include "ops.cuh"
+#include "uop.cuh"
+#include "interp.cuh"
 
 namespace beagle {
 
 // ---- opcode numbers on the device side (include/beagle.h) -------------------------------------------
-enum : uint32_t { UOP_END = 0, OPC_CONST = BEAGLE_OP_CONST, OPC_LOAD = BEAGLE_OP_LOAD, OPC_ADD = BEAGLE_OP_ADD,
+enum : uint32_t { OPC_CONST = BEAGLE_OP_CONST, OPC_LOAD = BEAGLE_OP_LOAD, OPC_ADD = BEAGLE_OP_ADD,
                   OPC_SUB = BEAGLE_OP_SUB, OPC_MUL = BEAGLE_OP_MUL, OPC_DIV = BEAGLE_OP_DIV,
                   OPC_SIN = BEAGLE_OP_SIN, OPC_COS = BEAGLE_OP_COS, OPC_LOG = BEAGLE_OP_LOG,
-                  OPC_SQRT = BEAGLE_OP_SQRT, OPC_EXP = BEAGLE_OP_EXP, UOP_MOV0 = 12 };
+                  OPC_SQRT = BEAGLE_OP_SQRT, OPC_EXP = BEAGLE_OP_EXP };
 
-constexpr int kNumClasses = 3;                 // depth classes: <=8, <=16, <=32 stack entries
-constexpr int kClassDepth[kNumClasses] = { 8, 16, 32 };
-constexpr int kNumBins = BEAGLE_MAX_LEN + 1;   // bin = 512 - length  (longest first)
+constexpr int kNumBins = BEAGLE_MAX_LEN + 1;   // bin = 512 - length  (longest first); bin 512 unused
 constexpr int kScanThreads = 256;              // programs per block in the pre-pass
-constexpr int kEvalThreads = 384;              // 12 warps: 65536 regs / 384 = 170 per thread
-constexpr int kUopBytes = (BEAGLE_MAX_LEN + 4) * 8;
-constexpr int kRawBytes = (BEAGLE_MAX_LEN + 8) * 4;
-constexpr int kWarpBytes = 2 * kUopBytes + 2 * kRawBytes;
+constexpr int kCompileThreads = 128;
+constexpr int kStagesMax = 8;                  // micro-op stages in flight per warp
+constexpr int kMainThreads = 512;              // 16 warps (4 per scheduler): 128 registers per thread
+constexpr int kMainSlots = 5;                  // s[] slots of the main interpreter
+constexpr int kDeepThreads = 384;              // 12 warps (3 per scheduler): 168 registers per thread
 constexpr int kProfMax = 256;                  // beagle_set_profiling: recorded calls
-constexpr int kCasePad = 512;                  // staged cases are padded to a multiple of 32*K for every K
+constexpr int kCasePad = 512;                  // staged cases are padded to a multiple of 32*K
+constexpr int kStageBytesMax = ((BEAGLE_MAX_LEN + 2 + 1) & ~1) * 8;   // 4112
 
 struct Header {                                // device-resident results of the pre-pass
     long long T;                               // total tokens = sum of in-range lengths
-    int cls_start[kNumClasses + 1];            // perm[] range of each depth class
-    unsigned int queue[kNumClasses];           // work-queue cursors of the evaluation kernels
+    long long uop_entries;                     // micro-op entries reserved by the bins
+    int n_sorted;                              // individuals with an in-range length (= entries of perm[])
+    int max_len;                               // longest in-range length (>= 1 if n_sorted > 0)
+    int n_deep;                                // individuals that need more than kMainSlots slots
+    int n_slow;                                // individuals whose micro-ops did not fit the workspace
     int n_malformed;
+    unsigned int queue[2];                     // work-queue cursors of the interpreter kernels
 };
 
 struct EvalParams {
-    const int32_t* genomes; const long long* off; const int32_t* lengths; const int32_t* perm;
-    const float* consts; const float* xt; const Header* hdr; unsigned int* queue;
-    float* fitness; float* outputs;
-    float tax; int n; int npad; int d; int cls;
+    const int4* meta; const uint2* uops; const int* list; const Header* hdr; unsigned int* queue;
+    const float* xt; float* fitness; float* outputs;
+    float tax; int n; int npad; int d; int ring_bytes;
 };
 
-// ---- PTX helpers: mbarrier, TMA bulk copy, cp.async --------------------------------------------------
+// ---- PTX helpers: mbarrier, TMA bulk copy -----------------------------------------------------------
 __device__ __forceinline__ uint32_t smem_u32(const void* p) { return (uint32_t)__cvta_generic_to_shared(p); }
 __device__ __forceinline__ void mbar_init(uint64_t* bar, uint32_t count) {
     asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count));
@@ -69,24 +74,22 @@ __device__ __forceinline__ void tma_bulk_g2s(void* dst, const void* src, uint32_
     asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
                  ::"r"(smem_u32(dst)), "l"(src), "r"(bytes), "r"(smem_u32(bar)) : "memory");
 }
-__device__ __forceinline__ void cp_async_16(void* dst, const void* src) {
-    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(smem_u32(dst)), "l"(src) : "memory");
-}
-__device__ __forceinline__ void cp_async_4(void* dst, const void* src) {
-    asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" ::"r"(smem_u32(dst)), "l"(src) : "memory");
-}
-__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
-template <int N> __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory"); }
 
 __device__ __forceinline__ int clamp_len(int l) { return (l >= 1 && l <= BEAGLE_MAX_LEN) ? l : 0; }
+__device__ __host__ __forceinline__ int uop_stride(int len) { return (len + 2 + 1) & ~1; }   // entries: nu <= len, END, pad; even
 
-// ---- a2: offsets ------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(kScanThreads) k_block_sums(const int32_t* __restrict__ lengths, long long P,
-                                                             long long* __restrict__ bsum)
+// ---- a2: block sums of the lengths + histogram of the lengths -----------------------------------------
+__global__ void __launch_bounds__(kScanThreads) k_len_pass1(const int32_t* __restrict__ lengths, long long P,
+                                                            long long* __restrict__ bsum, int* __restrict__ bins)
 {
     __shared__ int wsum[kScanThreads / 32];
+    __shared__ int hist[kNumBins];
+    for (int i = threadIdx.x; i < kNumBins; i += kScanThreads) hist[i] = 0;
+    __syncthreads();
     const long long p = (long long)blockIdx.x * kScanThreads + threadIdx.x;
-    int v = (p < P) ? clamp_len(lengths[p]) : 0;
+    const int len = (p < P) ? clamp_len(lengths[p]) : 0;
+    if (len > 0) atomicAdd(&hist[BEAGLE_MAX_LEN - len], 1);
+    int v = len;
 #pragma unroll
     for (int m = 16; m >= 1; m >>= 1) v += __shfl_xor_sync(0xffffffffu, v, m);
     if ((threadIdx.x & 31) == 0) wsum[threadIdx.x >> 5] = v;
@@ -97,17 +100,26 @@ __global__ void __launch_bounds__(kScanThreads) k_block_sums(const int32_t* __re
         for (int w = 0; w < kScanThreads / 32; ++w) t += wsum[w];
         bsum[blockIdx.x] = t;
     }
+    for (int i = threadIdx.x; i < kNumBins; i += kScanThreads)
+        if (hist[i]) atomicAdd(&bins[i], hist[i]);
 }
 
-// one block: exclusive scan of the block sums in place; also clears the bins and the header
-__global__ void __launch_bounds__(1024) k_scan_block_sums(long long* __restrict__ bsum, int nblocks,
-                                                          Header* __restrict__ hdr, int* __restrict__ bins)
+// one block: exclusive scan of the block sums in place; exclusive scan of the bins -> binstart[] (positions
+// in perm[]) and binubase[] (micro-op entries); resets bins/cursors/header for the next use; and a4's
+// transpose of the fitness cases into the variable-major, zero-padded block every interpreter CTA bulk-copies.
+__global__ void __launch_bounds__(1024) k_len_pass2(long long* __restrict__ bsum, int nblocks, Header* __restrict__ hdr,
+                                                    int* __restrict__ bins, int* __restrict__ cursor,
+                                                    int* __restrict__ binstart, long long* __restrict__ binubase,
+                                                    const float* __restrict__ X, const float* __restrict__ y,
+                                                    int n, int d, int npad, float* __restrict__ xt)
 {
     __shared__ long long wtot[32];
     __shared__ long long carry_s;
+    __shared__ long long wtot2[32];
+    __shared__ long long carry2_s;
+    __shared__ int maxlen_s;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    if (threadIdx.x == 0) carry_s = 0;
-    for (int i = threadIdx.x; i < 2 * kNumClasses * kNumBins; i += blockDim.x) bins[i] = 0;  // counts + cursors
+    if (threadIdx.x == 0) { carry_s = 0; carry2_s = 0; maxlen_s = 0; }
     __syncthreads();
     for (int base = 0; base < nblocks; base += 1024) {
         const int i = base + threadIdx.x;
@@ -129,113 +141,47 @@ __global__ void __launch_bounds__(1024) k_scan_block_sums(long long* __restrict_
         if (threadIdx.x == 1023) carry_s = carry + wtot[31] + inc;
         __syncthreads();
     }
-    if (threadIdx.x == 0) {
-        hdr->T = carry_s;
-        hdr->n_malformed = 0;
-        for (int c = 0; c < kNumClasses; ++c) hdr->queue[c] = 0;
-    }
-}
-
-// ---- a3: per-program scan, histogram of (depth class, length) ------------------------------------------
-// One thread per program: off[p], then one walk over its tokens (max stack depth, well-formedness:
-// DESIGN.md D3). Malformed individuals get the canonical NaN here and never reach the interpreter.
-__global__ void __launch_bounds__(kScanThreads) k_program_scan(
-    const int32_t* __restrict__ genomes, const int32_t* __restrict__ lengths, long long P,
-    const long long* __restrict__ bsum, long long n_consts, int d,
-    long long* __restrict__ off, int* __restrict__ key, int* __restrict__ depth_out,
-    int* __restrict__ bins, float* __restrict__ fitness, float* __restrict__ outputs, int n_cases,
-    Header* __restrict__ hdr)
-{
-    __shared__ int wsum[kScanThreads / 32];
-    __shared__ int hist[kNumClasses * kNumBins];
-    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    for (int i = threadIdx.x; i < kNumClasses * kNumBins; i += kScanThreads) hist[i] = 0;
-    const long long p = (long long)blockIdx.x * kScanThreads + threadIdx.x;
-    const int raw_len = (p < P) ? lengths[p] : 0;
-    const int len = clamp_len(raw_len);
-    int inc = len;
+    // bins: one element per thread (kNumBins = 513 <= 1024)
+    {
+        const int i = threadIdx.x;
+        const int cnt = (i < kNumBins) ? bins[i] : 0;
+        const int len = BEAGLE_MAX_LEN - i;
+        const long long v = cnt, u = (long long)cnt * uop_stride(len);
+        long long inc = v, uinc = u;
+        if (cnt > 0) atomicMax(&maxlen_s, len);
 #pragma unroll
-    for (int s = 1; s < 32; s <<= 1) { int o = __shfl_up_sync(0xffffffffu, inc, s); if (lane >= s) inc += o; }
-    if (lane == 31) wsum[warp] = inc;
-    __syncthreads();
-    int wbase = 0;
-#pragma unroll
-    for (int w = 0; w < kScanThreads / 32; ++w) wbase += (w < warp) ? wsum[w] : 0;
-    const long long o = bsum[blockIdx.x] + wbase + inc - len;
-    if (p < P) {
-        off[p] = o;
-        int sp = 0, mx = 0;
-        bool ok = len > 0;
-        const uint32_t* tok = reinterpret_cast<const uint32_t*>(genomes) + o;
-        for (int t = 0; t < len; ++t) {
-            const uint32_t w = __ldg(tok + t);
-            const uint32_t op = tok_op(w), arg = tok_arg(w);
-            if (op == OPC_CONST) { ok &= ((long long)arg < n_consts); ++sp; }
-            else if (op == OPC_LOAD) { ok &= ((int)arg < d); ++sp; }
-            else if (op >= OPC_ADD && op <= OPC_DIV) { ok &= (arg == 0) & (sp >= 2); --sp; }
-            else if (op >= OPC_SIN && op <= OPC_EXP) { ok &= (arg == 0) & (sp >= 1); }
-            else ok = false;
-            ok &= (sp <= BEAGLE_MAX_STACK);
-            mx = max(mx, sp);
-            if (!ok) break;
+        for (int s = 1; s < 32; s <<= 1) {
+            const long long o = __shfl_up_sync(0xffffffffu, inc, s), o2 = __shfl_up_sync(0xffffffffu, uinc, s);
+            if (lane >= s) { inc += o; uinc += o2; }
         }
-        ok &= (sp >= 1);
-        int k = -1;
-        if (ok) {
-            const int cls = mx <= kClassDepth[0] ? 0 : (mx <= kClassDepth[1] ? 1 : 2);
-            k = cls * kNumBins + (BEAGLE_MAX_LEN - len);
-            atomicAdd(&hist[k], 1);
-        } else {
-            if (fitness) fitness[p] = __uint_as_float(0x7FC00000u);
-            if (outputs) for (int i = 0; i < n_cases; ++i) outputs[(size_t)p * n_cases + i] = __uint_as_float(0x7FC00000u);
-            atomicAdd(&hdr->n_malformed, 1);
-        }
-        key[p] = k;
-        depth_out[p] = ok ? mx : 0;
-    }
-    __syncthreads();
-    for (int i = threadIdx.x; i < kNumClasses * kNumBins; i += kScanThreads)
-        if (hist[i]) atomicAdd(&bins[i], hist[i]);
-}
-
-// one block: exclusive scan of the bins -> bin starts and class ranges; and a4's transpose of the
-// fitness cases into the variable-major, zero-padded block every evaluation CTA bulk-copies.
-__global__ void __launch_bounds__(1024) k_bins_and_cases(const int* __restrict__ bins, int* __restrict__ binstart,
-                                                         Header* __restrict__ hdr,
-                                                         const float* __restrict__ X, const float* __restrict__ y,
-                                                         int n, int d, int npad, float* __restrict__ xt)
-{
-    __shared__ int wtot[32];
-    __shared__ int carry_s;
-    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    if (threadIdx.x == 0) carry_s = 0;
-    __syncthreads();
-    constexpr int total = kNumClasses * kNumBins;
-    for (int base = 0; base < total; base += 1024) {
-        const int i = base + threadIdx.x;
-        int v = (i < total) ? bins[i] : 0, inc = v;
-#pragma unroll
-        for (int s = 1; s < 32; s <<= 1) { int o = __shfl_up_sync(0xffffffffu, inc, s); if (lane >= s) inc += o; }
-        if (lane == 31) wtot[warp] = inc;
+        if (lane == 31) { wtot[warp] = inc; wtot2[warp] = uinc; }
         __syncthreads();
         if (warp == 0) {
-            int w = wtot[lane], winc = w;
+            const long long w = wtot[lane], w2 = wtot2[lane];
+            long long winc = w, winc2 = w2;
 #pragma unroll
-            for (int s = 1; s < 32; s <<= 1) { int o = __shfl_up_sync(0xffffffffu, winc, s); if (lane >= s) winc += o; }
-            wtot[lane] = winc - w;
+            for (int s = 1; s < 32; s <<= 1) {
+                const long long o = __shfl_up_sync(0xffffffffu, winc, s), o2 = __shfl_up_sync(0xffffffffu, winc2, s);
+                if (lane >= s) { winc += o; winc2 += o2; }
+            }
+            wtot[lane] = winc - w; wtot2[lane] = winc2 - w2;       // exclusive warp bases
+            if (lane == 31) { carry2_s = winc; hdr->uop_entries = winc2; }
         }
         __syncthreads();
-        const int carry = carry_s;
-        const int ex = carry + wtot[warp] + inc - v;
-        if (i < total) {
-            binstart[i] = ex;
-            if (i % kNumBins == 0) hdr->cls_start[i / kNumBins] = ex;
+        if (i < kNumBins) {
+            binstart[i] = (int)(wtot[warp] + inc - v);
+            binubase[i] = wtot2[warp] + uinc - u;
+            bins[i] = 0; cursor[i] = 0;            // ready for the next call
         }
-        __syncthreads();
-        if (threadIdx.x == 1023) carry_s = carry + wtot[31] + inc;
-        __syncthreads();
     }
-    if (threadIdx.x == 0) hdr->cls_start[kNumClasses] = carry_s;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        hdr->T = carry_s;
+        hdr->n_sorted = (int)carry2_s;
+        hdr->max_len = maxlen_s;
+        hdr->n_deep = 0; hdr->n_slow = 0; hdr->n_malformed = 0;
+        hdr->queue[0] = 0; hdr->queue[1] = 0;
+    }
     // transpose: xt[j][i] = X[i][j] (j < d), xt[d][i] = y[i]; cases i >= n are zero
     for (int e = threadIdx.x; e < (d + 1) * npad; e += blockDim.x) {
         const int j = e / npad, i = e - j * npad;
@@ -245,115 +191,291 @@ __global__ void __launch_bounds__(1024) k_bins_and_cases(const int* __restrict__
     }
 }
 
-__global__ void __launch_bounds__(kScanThreads) k_scatter(const int* __restrict__ key, long long P,
-                                                          const int* __restrict__ binstart, int* __restrict__ cursor,
-                                                          int* __restrict__ perm)
+// ---- a3: offsets and the counting sort by length ---------------------------------------------------------
+__global__ void __launch_bounds__(kScanThreads) k_scatter(
+    const int32_t* __restrict__ lengths, long long P, const long long* __restrict__ bsum,
+    const int* __restrict__ binstart, int* __restrict__ cursor, long long* __restrict__ off,
+    int* __restrict__ perm, int* __restrict__ depth_out, float* __restrict__ fitness,
+    float* __restrict__ outputs, int n_cases)
 {
-    __shared__ int cnt[kNumClasses * kNumBins];
-    for (int i = threadIdx.x; i < kNumClasses * kNumBins; i += kScanThreads) cnt[i] = 0;
-    __syncthreads();
+    __shared__ int wsum[kScanThreads / 32];
+    __shared__ int cnt[kNumBins];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    for (int i = threadIdx.x; i < kNumBins; i += kScanThreads) cnt[i] = 0;
     const long long p = (long long)blockIdx.x * kScanThreads + threadIdx.x;
-    const int k = (p < P) ? key[p] : -1;
+    const int len = (p < P) ? clamp_len(lengths[p]) : 0;
+    int inc = len;
+#pragma unroll
+    for (int s = 1; s < 32; s <<= 1) { int o = __shfl_up_sync(0xffffffffu, inc, s); if (lane >= s) inc += o; }
+    if (lane == 31) wsum[warp] = inc;
+    __syncthreads();
+    int wbase = 0;
+#pragma unroll
+    for (int w = 0; w < kScanThreads / 32; ++w) wbase += (w < warp) ? wsum[w] : 0;
+    const int k = len > 0 ? BEAGLE_MAX_LEN - len : -1;
     int r = 0;
-    if (k >= 0) r = atomicAdd(&cnt[k], 1);
+    if (p < P) {
+        off[p] = bsum[blockIdx.x] + wbase + inc - len;
+        if (k >= 0) r = atomicAdd(&cnt[k], 1);
+        else {                                   // length out of range: malformed (D3)
+            depth_out[p] = 0;
+            if (fitness) fitness[p] = __uint_as_float(0x7FC00000u);
+            if (outputs) for (int i = 0; i < n_cases; ++i) outputs[(size_t)p * n_cases + i] = __uint_as_float(0x7FC00000u);
+        }
+    }
     __syncthreads();
     // one global reservation per (block, non-empty bin); cnt[] becomes the block's base in that bin
-    for (int i = threadIdx.x; i < kNumClasses * kNumBins; i += kScanThreads)
+    for (int i = threadIdx.x; i < kNumBins; i += kScanThreads)
         if (cnt[i]) cnt[i] = atomicAdd(&cursor[i], cnt[i]);
     __syncthreads();
     if (k >= 0) perm[binstart[k] + cnt[k] + r] = (int)p;
 }
 
-// ---- the evaluation kernels: one instantiation per depth class ------------------------------------------
-#define BG_NAME k_eval_k16d8
+// ---- a3/a5: the tree compiler ----------------------------------------------------------------------------
+// One thread per individual, in length-sorted order (the threads of a warp run programs of equal
+// length). Pass 1 walks the postfix program once: well-formedness (D3), and per token the
+// size of its subtree and the number of s[] slots its evaluation needs. Pass 2 walks the tree from
+// the root and emits micro-ops (uop.cuh) in evaluation order.
+struct CompileParams {
+    const uint32_t* genomes; const long long* off; const int32_t* lengths; const int* perm;
+    const float* consts; long long n_consts; int d; int npad;
+    const int* binstart; const long long* binubase; Header* hdr;
+    uint2* uops; long long ucap; int4* meta; int* depth; int* deep_list; int* slow_list;
+    float* fitness; float* outputs; int n_cases; int slots_main; int emit;
+};
+
+__global__ void __launch_bounds__(kCompileThreads) k_compile(const CompileParams q)
+{
+    const int i = blockIdx.x * kCompileThreads + threadIdx.x;
+    if (i >= q.hdr->n_sorted) return;
+    const int p = q.perm[i];
+    const int len = q.lengths[p];
+    const int bin = BEAGLE_MAX_LEN - len;
+    const int stride = uop_stride(len);
+    const long long ua = q.binubase[bin] + (long long)(i - q.binstart[bin]) * stride;
+    const uint32_t* tok = q.genomes + q.off[p];
+
+    // info[t]: bits 0-9 subtree size, bits 10-12 slots needed, bit 15 terminal
+    unsigned short info[BEAGLE_MAX_LEN];
+    int sp = 0, mx = 0;
+    bool ok = true;
+    for (int t = 0; t < len; ++t) {
+        const uint32_t w = __ldg(tok + t);
+        const uint32_t op = tok_op(w), arg = tok_arg(w);
+        unsigned int inf = 0;
+        if (op == OPC_CONST) { ok &= ((long long)arg < q.n_consts); ++sp; inf = 0x8001u; }
+        else if (op == OPC_LOAD) { ok &= ((int)arg < q.d); ++sp; inf = 0x8001u; }
+        else if (op >= OPC_ADD && op <= OPC_DIV) {
+            ok &= (arg == 0) & (sp >= 2);
+            if (!ok) break;
+            const unsigned int ir = info[t - 1];
+            const int sr = ir & 0x3FF;
+            const unsigned int il = info[t - 1 - sr];
+            const int sl = il & 0x3FF;
+            const int nr = (ir >> 10) & 7, nl = (il >> 10) & 7;
+            const bool tr = ir >> 15, tl = il >> 15;
+            int need;
+            if (tl && tr) need = 0;
+            else if (tr) need = nl;
+            else if (tl) need = nr;
+            else need = max(max(nl, nr), min(nl, nr) + 1);
+            inf = (unsigned)(sl + sr + 1) | ((unsigned)need << 10);
+            --sp;
+        }
+        else if (op >= OPC_SIN && op <= OPC_EXP) {
+            ok &= (arg == 0) & (sp >= 1);
+            if (!ok) break;
+            const unsigned int ic = info[t - 1];
+            inf = (unsigned)((ic & 0x3FF) + 1) | ((ic >> 15) ? 0u : (ic & 0x1C00u));
+        }
+        else ok = false;
+        ok &= (sp <= BEAGLE_MAX_STACK);
+        if (!ok) break;
+        info[t] = (unsigned short)inf;
+        mx = max(mx, sp);
+    }
+    ok &= (sp >= 1);
+    if (!ok) {
+        q.depth[p] = 0;
+        if (q.fitness) q.fitness[p] = __uint_as_float(0x7FC00000u);
+        if (q.outputs) for (int c = 0; c < q.n_cases; ++c) q.outputs[(size_t)p * q.n_cases + c] = __uint_as_float(0x7FC00000u);
+        q.meta[i] = make_int4(p, 0, KIND_SKIP << 24, len);
+        atomicAdd(&q.hdr->n_malformed, 1);
+        return;
+    }
+    q.depth[p] = mx;
+    if (!q.emit) { q.meta[i] = make_int4(p, 0, KIND_SKIP << 24, len); return; }
+    if (ua + stride > q.ucap) {                  // the workspace promise of beagle_reserve was broken: slow path
+        q.slow_list[atomicAdd(&q.hdr->n_slow, 1)] = p;
+        q.meta[i] = make_int4(p, 0, KIND_SKIP << 24, len);
+        return;
+    }
+
+    // pass 2: work stack entries = pos | kind << 9
+    enum { W_VISIT = 0, W_UN = 1, W_BINT = 2, W_TBIN = 3, W_BINS = 4, W_BINSR = 5 };
+    unsigned short ws[BEAGLE_MAX_LEN];
+    int wsp = 0, n = 0, R = 0, Rmax = 0;
+    uint2* out = q.uops + ua;
+    const uint32_t xrow = (uint32_t)q.npad * 4u;
+    auto materialise = [&](int t) {              // terminal t becomes the accumulator (the old one is pushed)
+        const uint32_t w = __ldg(tok + t);
+        const bool isx = tok_op(w) == OPC_LOAD;
+        const uint32_t h = R >= 1 ? (isx ? H_PUSHX : H_PUSHC) + (uint32_t)(R - 1) : (isx ? H_LOADX : H_CONST);
+        out[n++] = isx ? make_uint2(h | (tok_arg(w) * xrow) << 8, 0u)
+                       : make_uint2(h, __float_as_uint(__ldg(q.consts + tok_arg(w))));
+        ++R; Rmax = max(Rmax, R);
+    };
+    auto with_terminal = [&](uint32_t hx, uint32_t hc, int t) {   // a command with terminal t folded in
+        const uint32_t w = __ldg(tok + t);
+        out[n++] = tok_op(w) == OPC_LOAD ? make_uint2(hx | (tok_arg(w) * xrow) << 8, 0u)
+                                         : make_uint2(hc, __float_as_uint(__ldg(q.consts + tok_arg(w))));
+    };
+    ws[wsp++] = (unsigned short)((len - 1) | (W_VISIT << 9));
+    while (wsp > 0) {
+        const unsigned int e = ws[--wsp];
+        const int t = e & 0x1FF, kind = e >> 9;
+        const uint32_t op = tok_op(__ldg(tok + t));
+        if (kind == W_VISIT) {
+            if (op <= OPC_LOAD) materialise(t);
+            else if (op >= OPC_SIN) {
+                ws[wsp++] = (unsigned short)(t | (W_UN << 9));
+                ws[wsp++] = (unsigned short)((t - 1) | (W_VISIT << 9));
+            } else {
+                const int r = t - 1;
+                const unsigned int ir = info[r];
+                const int l = r - (int)(ir & 0x3FF);
+                const unsigned int il = info[l];
+                const bool tr = ir >> 15, tl = il >> 15;
+                if (tl && tr) { materialise(l); with_terminal(H_ADDX + (op - OPC_ADD), H_ADDC + (op - OPC_ADD), r); }
+                else if (tr) { ws[wsp++] = (unsigned short)(t | (W_BINT << 9)); ws[wsp++] = (unsigned short)(l | (W_VISIT << 9)); }
+                else if (tl) { ws[wsp++] = (unsigned short)(t | (W_TBIN << 9)); ws[wsp++] = (unsigned short)(r | (W_VISIT << 9)); }
+                else if (((ir >> 10) & 7) > ((il >> 10) & 7)) {     // Sethi-Ullman: the needier subtree first
+                    ws[wsp++] = (unsigned short)(t | (W_BINSR << 9));
+                    ws[wsp++] = (unsigned short)(l | (W_VISIT << 9));
+                    ws[wsp++] = (unsigned short)(r | (W_VISIT << 9));
+                } else {
+                    ws[wsp++] = (unsigned short)(t | (W_BINS << 9));
+                    ws[wsp++] = (unsigned short)(r | (W_VISIT << 9));
+                    ws[wsp++] = (unsigned short)(l | (W_VISIT << 9));
+                }
+            }
+        } else if (kind == W_UN) {
+            out[n++] = make_uint2(H_SIN + (op - OPC_SIN), 0u);
+        } else if (kind == W_BINT) {             // acc = acc op terminal(t-1)
+            with_terminal(H_ADDX + (op - OPC_ADD), H_ADDC + (op - OPC_ADD), t - 1);
+        } else if (kind == W_TBIN) {             // acc = terminal(l) op acc; ADD and MUL commute bit for bit
+            const int l = t - 1 - (int)(info[t - 1] & 0x3FF);
+            const uint32_t hx = op == OPC_ADD ? H_ADDX : op == OPC_MUL ? H_MULX : op == OPC_SUB ? H_XSUB : H_XDIV;
+            const uint32_t hc = op == OPC_ADD ? H_ADDC : op == OPC_MUL ? H_MULC : op == OPC_SUB ? H_CSUB : H_CDIV;
+            with_terminal(hx, hc, l);
+        } else {                                 // both operands computed: s[R-2] and acc
+            const uint32_t S = (uint32_t)(R - 2);
+            uint32_t h;
+            if (kind == W_BINS) h = H_ADDS + (op - OPC_ADD) * kSlotsMax;          // acc = s[S] op acc
+            else h = op == OPC_ADD ? H_ADDS : op == OPC_MUL ? H_MULS : op == OPC_SUB ? H_RSUBS : H_RDIVS;   // acc = acc op s[S]
+            out[n++] = make_uint2(h + S, 0u);
+            --R;
+        }
+    }
+    out[n] = make_uint2(H_END, 0u);
+    out[n + 1] = make_uint2(H_END, 0u);
+    const int slots = Rmax - 1;
+    const int kind = slots > q.slots_main ? KIND_DEEP : KIND_MAIN;
+    if (kind == KIND_DEEP) q.deep_list[atomicAdd(&q.hdr->n_deep, 1)] = i;
+    q.meta[i] = make_int4(p, (int)(ua >> 1), n | (slots << 16) | (kind << 24), len);
+}
+
+// ---- the interpreter kernels ---------------------------------------------------------------------------
+#define BG_NAME k_eval_main
+#define BG_K 16
+#define BG_D 5
+#define BG_THREADS kMainThreads
+#define BG_KIND KIND_MAIN
+#define BG_LIST 0
+#define BG_INTERP interp_run_d5
+#include "eval_kernel.inc"
+#undef BG_NAME
+#undef BG_K
+#undef BG_D
+#undef BG_THREADS
+#undef BG_KIND
+#undef BG_LIST
+#undef BG_INTERP
+
+#define BG_NAME k_eval_deep
 #define BG_K 16
 #define BG_D 8
-#define BG_SLOTS(M) M(0) M(1) M(2) M(3) M(4) M(5) M(6) M(7)
-#define BG_SLOTS_BIN(M) M(0) M(1) M(2) M(3) M(4) M(5) M(6)
+#define BG_THREADS kDeepThreads
+#define BG_KIND KIND_DEEP
+#define BG_LIST 1
+#define BG_INTERP interp_run_d8
 #include "eval_kernel.inc"
 #undef BG_NAME
 #undef BG_K
 #undef BG_D
-#undef BG_SLOTS
-#undef BG_SLOTS_BIN
+#undef BG_THREADS
+#undef BG_KIND
+#undef BG_LIST
+#undef BG_INTERP
 
-#define BG_NAME k_eval_k8d16
-#define BG_K 8
-#define BG_D 16
-#define BG_SLOTS(M) M(0) M(1) M(2) M(3) M(4) M(5) M(6) M(7) M(8) M(9) M(10) M(11) M(12) M(13) M(14) M(15)
-#define BG_SLOTS_BIN(M) M(0) M(1) M(2) M(3) M(4) M(5) M(6) M(7) M(8) M(9) M(10) M(11) M(12) M(13) M(14)
-#include "eval_kernel.inc"
-#undef BG_NAME
-#undef BG_K
-#undef BG_D
-#undef BG_SLOTS
-#undef BG_SLOTS_BIN
-
-#define BG_NAME k_eval_k4d32
-#define BG_K 4
-#define BG_D 32
-#define BG_SLOTS(M) M(0) M(1) M(2) M(3) M(4) M(5) M(6) M(7) M(8) M(9) M(10) M(11) M(12) M(13) M(14) M(15) \
-    M(16) M(17) M(18) M(19) M(20) M(21) M(22) M(23) M(24) M(25) M(26) M(27) M(28) M(29) M(30) M(31)
-#define BG_SLOTS_BIN(M) M(0) M(1) M(2) M(3) M(4) M(5) M(6) M(7) M(8) M(9) M(10) M(11) M(12) M(13) M(14) M(15) \
-    M(16) M(17) M(18) M(19) M(20) M(21) M(22) M(23) M(24) M(25) M(26) M(27) M(28) M(29) M(30)
-#include "eval_kernel.inc"
-#undef BG_NAME
-#undef BG_K
-#undef BG_D
-#undef BG_SLOTS
-#undef BG_SLOTS_BIN
-
-// ---- prior art as a baseline: the paper's mapping ------------------------------------------
+// ---- prior art as a baseline, and the slow path: the paper's mapping ------------------------
 // One block per individual, one thread per fitness case, a 32-entry per-thread stack in local
 // memory, every thread decodes every token. The residuals go through shared memory so that warp 0
 // can add them in the canonical order: results are bit-identical to the warp-per-individual kernels.
+// With list != nullptr the blocks walk list[0..*count) (individuals whose micro-ops did not fit).
 __global__ void __launch_bounds__(1024) k_eval_blockwise(
     const int32_t* __restrict__ genomes, const long long* __restrict__ off, const int32_t* __restrict__ lengths,
     const int* __restrict__ depth, const float* __restrict__ consts, const float* __restrict__ X,
-    const float* __restrict__ y, int n, int d, float tax, float* __restrict__ fitness)
+    const float* __restrict__ y, int n, int d, float tax, float* __restrict__ fitness, float* __restrict__ outputs,
+    const int* __restrict__ list, const int* __restrict__ count, long long P)
 {
     __shared__ float res[BEAGLE_MAX_N];
-    const int p = blockIdx.x;
-    if (depth[p] == 0) return;                 // malformed: NaN already written by the pre-pass
-    const int len = lengths[p];
-    const uint32_t* tok = reinterpret_cast<const uint32_t*>(genomes) + off[p];
-    const int i = threadIdx.x;
-    if (i < n) {
-        float st[BEAGLE_MAX_STACK];
-        int sp = 0;
-        for (int t = 0; t < len; ++t) {
-            const uint32_t w = __ldg(tok + t);
-            const uint32_t op = tok_op(w), arg = tok_arg(w);
-            switch (op) {
-            case OPC_CONST: st[sp++] = __ldg(consts + arg); break;
-            case OPC_LOAD: st[sp++] = __ldg(X + (size_t)i * d + arg); break;
-            case OPC_ADD: st[sp - 2] = op_add(st[sp - 2], st[sp - 1]); --sp; break;
-            case OPC_SUB: st[sp - 2] = op_sub(st[sp - 2], st[sp - 1]); --sp; break;
-            case OPC_MUL: st[sp - 2] = op_mul(st[sp - 2], st[sp - 1]); --sp; break;
-            case OPC_DIV: st[sp - 2] = op_div(st[sp - 2], st[sp - 1]); --sp; break;
-            case OPC_SIN: st[sp - 1] = op_sin(st[sp - 1]); break;
-            case OPC_COS: st[sp - 1] = op_cos(st[sp - 1]); break;
-            case OPC_LOG: st[sp - 1] = op_log(st[sp - 1]); break;
-            case OPC_SQRT: st[sp - 1] = op_sqrt(st[sp - 1]); break;
-            case OPC_EXP: st[sp - 1] = op_exp(st[sp - 1]); break;
-            default: break;
+    const long long total = list ? (long long)*count : P;
+    for (long long idx = blockIdx.x; idx < total; idx += gridDim.x) {
+        const long long p = list ? (long long)list[idx] : idx;
+        if (depth[p] == 0) continue;               // malformed: NaN already written by the pre-pass
+        const int len = lengths[p];
+        const uint32_t* tok = reinterpret_cast<const uint32_t*>(genomes) + off[p];
+        const int i = threadIdx.x;
+        if (i < n) {
+            float st[BEAGLE_MAX_STACK];
+            int sp = 0;
+            for (int t = 0; t < len; ++t) {
+                const uint32_t w = __ldg(tok + t);
+                const uint32_t op = tok_op(w), arg = tok_arg(w);
+                switch (op) {
+                case OPC_CONST: st[sp++] = __ldg(consts + arg); break;
+                case OPC_LOAD: st[sp++] = __ldg(X + (size_t)i * d + arg); break;
+                case OPC_ADD: st[sp - 2] = op_add(st[sp - 2], st[sp - 1]); --sp; break;
+                case OPC_SUB: st[sp - 2] = op_sub(st[sp - 2], st[sp - 1]); --sp; break;
+                case OPC_MUL: st[sp - 2] = op_mul(st[sp - 2], st[sp - 1]); --sp; break;
+                case OPC_DIV: st[sp - 2] = op_div(st[sp - 2], st[sp - 1]); --sp; break;
+                case OPC_SIN: st[sp - 1] = op_sin(st[sp - 1]); break;
+                case OPC_COS: st[sp - 1] = op_cos(st[sp - 1]); break;
+                case OPC_LOG: st[sp - 1] = op_log(st[sp - 1]); break;
+                case OPC_SQRT: st[sp - 1] = op_sqrt(st[sp - 1]); break;
+                case OPC_EXP: st[sp - 1] = op_exp(st[sp - 1]); break;
+                default: break;
+                }
             }
+            if (outputs) outputs[(size_t)p * n + i] = st[sp - 1];
+            res[i] = y ? __fsub_rn(st[sp - 1], __ldg(y + i)) : 0.f;
         }
-        res[i] = __fsub_rn(st[sp - 1], __ldg(y + i));
-    }
-    __syncthreads();
-    if (threadIdx.x < 32) {
-        const int lane = threadIdx.x;
-        float acc = 0.f;
-        for (int m = 0; m * 128 < n; ++m)
+        __syncthreads();
+        if (threadIdx.x < 32 && fitness) {
+            const int lane = threadIdx.x;
+            float acc = 0.f;
+            for (int m = 0; m * 128 < n; ++m)
 #pragma unroll
-            for (int e = 0; e < 4; ++e) {
-                const int ci = m * 128 + lane * 4 + e;
-                if (ci < n) { const float r = res[ci]; acc = __fmaf_rn(r, r, acc); }
-            }
+                for (int e = 0; e < 4; ++e) {
+                    const int ci = m * 128 + lane * 4 + e;
+                    if (ci < n) { const float r = res[ci]; acc = __fmaf_rn(r, r, acc); }
+                }
 #pragma unroll
-        for (int m = 16; m >= 1; m >>= 1) acc = __fadd_rn(acc, __shfl_xor_sync(0xffffffffu, acc, m));
-        if (lane == 0) fitness[p] = __fmaf_rn(tax, (float)len, __fdiv_rn(acc, (float)n));
+            for (int m = 16; m >= 1; m >>= 1) acc = __fadd_rn(acc, __shfl_xor_sync(0xffffffffu, acc, m));
+            if (lane == 0) fitness[p] = __fmaf_rn(tax, (float)len, __fdiv_rn(acc, (float)n));
+        }
+        __syncthreads();
     }
 }
 
@@ -361,10 +483,13 @@ __global__ void __launch_bounds__(1024) k_eval_blockwise(
 //                                        host side
 // ======================================================================================================
 struct Workspace {
-    long long cap_P = 0;
-    long long* off = nullptr; int* key = nullptr; int* depth = nullptr; int* perm = nullptr;
-    long long* bsum = nullptr; int* bins = nullptr; int* binstart = nullptr; float* xt = nullptr;
-    Header* hdr = nullptr;
+    long long cap_P = 0, cap_U = 0;            // individuals / micro-op entries the workspace holds
+    long long promised_P = 0, promised_T = 0;  // beagle_reserve: calls with P <= promised_P have T <= promised_T
+    long long* off = nullptr; int* depth = nullptr; int* perm = nullptr; int4* meta = nullptr;
+    int* deep_list = nullptr; int* slow_list = nullptr; long long* bsum = nullptr;
+    uint2* uops = nullptr;
+    int* bins = nullptr; int* cursor = nullptr; int* binstart = nullptr; long long* binubase = nullptr;
+    float* xt = nullptr; Header* hdr = nullptr; long long* h_T = nullptr;
     // chunked staging
     long long stage_bytes = 0; unsigned char* stage[2] = { nullptr, nullptr };
     float* stage_consts = nullptr; long long stage_consts_cap = 0;
@@ -391,13 +516,18 @@ static beagle_status init_once()
     w.device_ok = (prop.major == 10);
     w.inited = true;
     if (!w.device_ok) return BEAGLE_ERR_UNSUPPORTED;
-    CU(cudaFuncSetAttribute(k_eval_k16d8, cudaFuncAttributeMaxDynamicSharedMemorySize, w.smem_optin));
-    CU(cudaFuncSetAttribute(k_eval_k8d16, cudaFuncAttributeMaxDynamicSharedMemorySize, w.smem_optin));
-    CU(cudaFuncSetAttribute(k_eval_k4d32, cudaFuncAttributeMaxDynamicSharedMemorySize, w.smem_optin));
-    CU(cudaMalloc(&w.bins, sizeof(int) * 2 * kNumClasses * kNumBins));
-    CU(cudaMalloc(&w.binstart, sizeof(int) * kNumClasses * kNumBins));
+    CU(cudaFuncSetAttribute(k_eval_main, cudaFuncAttributeMaxDynamicSharedMemorySize, w.smem_optin));
+    CU(cudaFuncSetAttribute(k_eval_deep, cudaFuncAttributeMaxDynamicSharedMemorySize, w.smem_optin));
+    CU(cudaMalloc(&w.bins, sizeof(int) * kNumBins));
+    CU(cudaMalloc(&w.cursor, sizeof(int) * kNumBins));
+    CU(cudaMemset(w.bins, 0, sizeof(int) * kNumBins));
+    CU(cudaMemset(w.cursor, 0, sizeof(int) * kNumBins));
+    CU(cudaMalloc(&w.binstart, sizeof(int) * kNumBins));
+    CU(cudaMalloc(&w.binubase, sizeof(long long) * kNumBins));
     CU(cudaMalloc(&w.xt, sizeof(float) * (BEAGLE_MAX_D + 1) * BEAGLE_MAX_N));
     CU(cudaMalloc(&w.hdr, sizeof(Header)));
+    CU(cudaMemset(w.hdr, 0, sizeof(Header)));
+    CU(cudaMallocHost(&w.h_T, sizeof(long long)));
     return BEAGLE_OK;
 }
 
@@ -406,17 +536,34 @@ static beagle_status reserve_P(long long P)
     Workspace& w = g_ws;
     if (P <= w.cap_P) return BEAGLE_OK;
     CU(cudaDeviceSynchronize());
-    cudaFree(w.off); cudaFree(w.key); cudaFree(w.depth); cudaFree(w.perm); cudaFree(w.bsum);
-    w.off = nullptr; w.key = nullptr; w.depth = nullptr; w.perm = nullptr; w.bsum = nullptr; w.cap_P = 0;
+    cudaFree(w.off); cudaFree(w.depth); cudaFree(w.perm); cudaFree(w.meta); cudaFree(w.deep_list);
+    cudaFree(w.slow_list); cudaFree(w.bsum);
+    w.off = nullptr; w.depth = nullptr; w.perm = nullptr; w.meta = nullptr; w.deep_list = nullptr;
+    w.slow_list = nullptr; w.bsum = nullptr; w.cap_P = 0;
     const long long nb = (P + kScanThreads - 1) / kScanThreads;
     CU(cudaMalloc(&w.off, sizeof(long long) * (P + 1)));
-    CU(cudaMalloc(&w.key, sizeof(int) * P));
     CU(cudaMalloc(&w.depth, sizeof(int) * P));
     CU(cudaMalloc(&w.perm, sizeof(int) * P));
+    CU(cudaMalloc(&w.meta, sizeof(int4) * P));
+    CU(cudaMalloc(&w.deep_list, sizeof(int) * P));
+    CU(cudaMalloc(&w.slow_list, sizeof(int) * P));
     CU(cudaMalloc(&w.bsum, sizeof(long long) * (nb + 1)));
     w.cap_P = P;
     return BEAGLE_OK;
 }
+
+static beagle_status reserve_U(long long U)
+{
+    Workspace& w = g_ws;
+    if (U <= w.cap_U) return BEAGLE_OK;
+    CU(cudaDeviceSynchronize());
+    cudaFree(w.uops); w.uops = nullptr; w.cap_U = 0;
+    CU(cudaMalloc(&w.uops, sizeof(uint2) * U));
+    w.cap_U = U;
+    return BEAGLE_OK;
+}
+
+static long long uop_entries_bound(long long P, long long T) { return T + 3 * P + 2; }   // sum of uop_stride(len)
 
 static beagle_status check_args(const void* genomes, const void* lengths, int64_t P, const void* consts,
                                 int64_t n_consts, const void* X, const void* y, int32_t N, int32_t d, const void* out)
@@ -430,54 +577,86 @@ static beagle_status check_args(const void* genomes, const void* lengths, int64_
     return BEAGLE_OK;
 }
 
-// a2 + a3 (+ the transpose of a4). After this: off, depth, perm, hdr are valid on `st`.
-static beagle_status run_prepass(const int32_t* genomes, const int32_t* lengths, long long P, long long n_consts,
-                                 const float* X, const float* y, int N, int d, float* fitness, float* outputs,
-                                 cudaStream_t st)
+// a2 + a3 + the compile step of a5 (+ the transpose of a4). T_known < 0: the token count is not known
+// on the host; unless beagle_reserve promised a bound, it is read back once (one stream synchronisation).
+static beagle_status run_prepass(const int32_t* genomes, const int32_t* lengths, long long P, const float* consts,
+                                 long long n_consts, const float* X, const float* y, int N, int d, float* fitness,
+                                 float* outputs, long long T_known, bool emit, cudaStream_t st)
 {
     Workspace& w = g_ws;
     const int nb = (int)((P + kScanThreads - 1) / kScanThreads);
     const int npad = (N + kCasePad - 1) / kCasePad * kCasePad;
-    k_block_sums<<<nb, kScanThreads, 0, st>>>(lengths, P, w.bsum);
-    k_scan_block_sums<<<1, 1024, 0, st>>>(w.bsum, nb, w.hdr, w.bins);
-    k_program_scan<<<nb, kScanThreads, 0, st>>>(genomes, lengths, P, w.bsum, n_consts, d, w.off, w.key, w.depth,
-                                                w.bins, fitness, outputs, N, w.hdr);
-    k_bins_and_cases<<<1, 1024, 0, st>>>(w.bins, w.binstart, w.hdr, X, y, N, d, npad, w.xt);
-    k_scatter<<<nb, kScanThreads, 0, st>>>(w.key, P, w.binstart, w.bins + kNumClasses * kNumBins, w.perm);
-    g_launches += 5;
+    k_len_pass1<<<nb, kScanThreads, 0, st>>>(lengths, P, w.bsum, w.bins);
+    k_len_pass2<<<1, 1024, 0, st>>>(w.bsum, nb, w.hdr, w.bins, w.cursor, w.binstart, w.binubase, X, y, N, d, npad, w.xt);
+    g_launches += 2;
+    if (emit) {
+        long long need = -1;
+        if (T_known >= 0) need = uop_entries_bound(P, T_known);
+        else if (w.cap_U >= (long long)uop_stride(BEAGLE_MAX_LEN) * P) need = 0;            // worst case fits
+        else if (P <= w.promised_P && w.promised_T > 0) need = 0;                           // promised by beagle_reserve
+        else {
+            CU(cudaMemcpyAsync(w.h_T, &w.hdr->T, sizeof(long long), cudaMemcpyDeviceToHost, st));
+            CU(cudaStreamSynchronize(st));
+            need = uop_entries_bound(P, *w.h_T);
+        }
+        if (need > w.cap_U) { beagle_status s = reserve_U(need); if (s != BEAGLE_OK) return s; }
+    }
+    k_scatter<<<nb, kScanThreads, 0, st>>>(lengths, P, w.bsum, w.binstart, w.cursor, w.off, w.perm, w.depth,
+                                           fitness, outputs, N);
+    ++g_launches;
+    {
+        CompileParams q;
+        q.genomes = reinterpret_cast<const uint32_t*>(genomes); q.off = w.off; q.lengths = lengths; q.perm = w.perm;
+        q.consts = consts; q.n_consts = n_consts; q.d = d; q.npad = npad; q.binstart = w.binstart; q.binubase = w.binubase;
+        q.hdr = w.hdr; q.uops = w.uops; q.ucap = w.cap_U; q.meta = w.meta; q.depth = w.depth; q.deep_list = w.deep_list;
+        q.slow_list = w.slow_list; q.fitness = fitness; q.outputs = outputs; q.n_cases = N; q.slots_main = kMainSlots; q.emit = emit ? 1 : 0;
+        k_compile<<<(unsigned)((P + kCompileThreads - 1) / kCompileThreads), kCompileThreads, 0, st>>>(q);
+        ++g_launches;
+    }
     CU(cudaGetLastError());
     return BEAGLE_OK;
 }
 
-static beagle_status run_eval(const int32_t* genomes, const int32_t* lengths, const float* consts, int N, int d,
-                              float tax, float* fitness, float* outputs, cudaStream_t st)
+static int ring_bytes_for(int threads, long long xs_bytes, int smem_optin, size_t* smem_out)
+{
+    const int warps = threads / 32;
+    const long long fixed = ((64 + warps * kStagesMax * 8 + 127) & ~127) + ((xs_bytes + 127) & ~127ll);
+    long long ring = ((smem_optin - fixed) / warps) & ~127ll;
+    if (ring > (long long)kStagesMax * kStageBytesMax) ring = (long long)kStagesMax * kStageBytesMax;
+    *smem_out = (size_t)(fixed + ring * warps);
+    return (int)ring;
+}
+
+static beagle_status run_eval(const int32_t* genomes, const int32_t* lengths, const float* consts, const float* X,
+                              const float* y, long long P, int N, int d, float tax, float* fitness, float* outputs,
+                              cudaStream_t st)
 {
     Workspace& w = g_ws;
     const int npad = (N + kCasePad - 1) / kCasePad * kCasePad;
     const long long xs_bytes = (long long)(d + 1) * npad * 4;
-    const long long fixed = 128 + ((xs_bytes + 127) & ~127ll);
-    int warps = (int)((w.smem_optin - fixed) / kWarpBytes);
-    if (warps > kEvalThreads / 32) warps = kEvalThreads / 32;
-    if (warps < 1) return BEAGLE_ERR_UNSUPPORTED;
-    const size_t smem = (size_t)(fixed + (long long)warps * kWarpBytes);
     EvalParams prm;
-    prm.genomes = genomes; prm.off = w.off; prm.lengths = lengths; prm.perm = w.perm; prm.consts = consts;
-    prm.xt = w.xt; prm.hdr = w.hdr; prm.fitness = fitness; prm.outputs = outputs;
-    prm.tax = tax; prm.n = N; prm.npad = npad; prm.d = d;
+    prm.meta = w.meta; prm.uops = w.uops; prm.list = w.deep_list; prm.hdr = w.hdr; prm.xt = w.xt;
+    prm.fitness = fitness; prm.outputs = outputs; prm.tax = tax; prm.n = N; prm.npad = npad; prm.d = d;
     const bool prof = g_profiling && w.prof_n < kProfMax;
     if (prof) {
         for (int i = 0; i < 2; ++i)
             if (!w.ev_k[2 * w.prof_n + i]) CU(cudaEventCreate(&w.ev_k[2 * w.prof_n + i]));
         CU(cudaEventRecord(w.ev_k[2 * w.prof_n], st));
     }
-    for (int c = 0; c < kNumClasses; ++c) {
-        prm.cls = c; prm.queue = &w.hdr->queue[c];
-        if (c == 0) k_eval_k16d8<<<w.num_sms, warps * 32, smem, st>>>(prm);
-        else if (c == 1) k_eval_k8d16<<<w.num_sms, warps * 32, smem, st>>>(prm);
-        else k_eval_k4d32<<<w.num_sms, warps * 32, smem, st>>>(prm);
-        ++g_launches;
-    }
+    size_t smem = 0;
+    prm.ring_bytes = ring_bytes_for(kMainThreads, xs_bytes, w.smem_optin, &smem);
+    if (prm.ring_bytes < kStageBytesMax) return BEAGLE_ERR_UNSUPPORTED;
+    prm.queue = &w.hdr->queue[0];
+    k_eval_main<<<w.num_sms, kMainThreads, smem, st>>>(prm);
+    prm.ring_bytes = ring_bytes_for(kDeepThreads, xs_bytes, w.smem_optin, &smem);
+    prm.queue = &w.hdr->queue[1];
+    k_eval_deep<<<w.num_sms, kDeepThreads, smem, st>>>(prm);
+    g_launches += 2;
     if (prof) { CU(cudaEventRecord(w.ev_k[2 * w.prof_n + 1], st)); ++w.prof_n; }
+    // slow path: individuals whose micro-ops did not fit the promised workspace (normally none)
+    k_eval_blockwise<<<w.num_sms * 2, (N + 31) / 32 * 32, 0, st>>>(genomes, w.off, lengths, w.depth, consts, X, y, N, d, tax,
+                                                                   fitness, outputs, w.slow_list, &w.hdr->n_slow, P);
+    ++g_launches;
     CU(cudaGetLastError());
     return BEAGLE_OK;
 }
@@ -499,8 +678,8 @@ beagle_status beagle_eval(const int32_t* genomes, const int32_t* lengths, int64_
     if ((s = init_once()) != BEAGLE_OK) return s;
     if ((s = reserve_P(P)) != BEAGLE_OK) return s;
     cudaStream_t st = (cudaStream_t)stream;
-    if ((s = run_prepass(genomes, lengths, P, n_consts, X, y, N, d, fitness_out, nullptr, st)) != BEAGLE_OK) return s;
-    return run_eval(genomes, lengths, consts, N, d, tax, fitness_out, nullptr, st);
+    if ((s = run_prepass(genomes, lengths, P, consts, n_consts, X, y, N, d, fitness_out, nullptr, -1, true, st)) != BEAGLE_OK) return s;
+    return run_eval(genomes, lengths, consts, X, y, P, N, d, tax, fitness_out, nullptr, st);
 }
 
 beagle_status beagle_debug_outputs(const int32_t* genomes, const int32_t* lengths, int64_t P,
@@ -514,9 +693,8 @@ beagle_status beagle_debug_outputs(const int32_t* genomes, const int32_t* length
     if ((s = init_once()) != BEAGLE_OK) return s;
     if ((s = reserve_P(P)) != BEAGLE_OK) return s;
     cudaStream_t st = (cudaStream_t)stream;
-    // y is not used for outputs; X's first column stands in so that the staging kernel has a valid pointer
-    if ((s = run_prepass(genomes, lengths, P, n_consts, X, nullptr, N, d, nullptr, out_PxN, st)) != BEAGLE_OK) return s;
-    return run_eval(genomes, lengths, consts, N, d, 0.f, nullptr, out_PxN, st);
+    if ((s = run_prepass(genomes, lengths, P, consts, n_consts, X, nullptr, N, d, nullptr, out_PxN, -1, true, st)) != BEAGLE_OK) return s;
+    return run_eval(genomes, lengths, consts, X, nullptr, P, N, d, 0.f, nullptr, out_PxN, st);
 }
 
 beagle_status beagle_eval_blockwise(const int32_t* genomes, const int32_t* lengths, int64_t P,
@@ -530,9 +708,12 @@ beagle_status beagle_eval_blockwise(const int32_t* genomes, const int32_t* lengt
     if ((s = init_once()) != BEAGLE_OK) return s;
     if ((s = reserve_P(P)) != BEAGLE_OK) return s;
     cudaStream_t st = (cudaStream_t)stream;
-    if ((s = run_prepass(genomes, lengths, P, n_consts, X, y, N, d, fitness_out, nullptr, st)) != BEAGLE_OK) return s;
+    Workspace& w = g_ws;
+    // k_compile runs as the well-formedness check only (depth[]); it emits no micro-ops
+    if ((s = run_prepass(genomes, lengths, P, consts, n_consts, X, y, N, d, fitness_out, nullptr, -1, false, st)) != BEAGLE_OK) return s;
     const int threads = (N + 31) / 32 * 32;
-    k_eval_blockwise<<<(unsigned)P, threads, 0, st>>>(genomes, g_ws.off, lengths, g_ws.depth, consts, X, y, N, d, tax, fitness_out);
+    k_eval_blockwise<<<(unsigned)P, threads, 0, st>>>(genomes, w.off, lengths, w.depth, consts, X, y, N, d, tax,
+                                                      fitness_out, nullptr, nullptr, nullptr, P);
     ++g_launches;
     CU(cudaGetLastError());
     return BEAGLE_OK;
@@ -569,6 +750,9 @@ beagle_status beagle_reserve_chunked(int64_t device_budget_bytes)
         CU(cudaMalloc(&w.stage[1], half));
         w.stage_bytes = half;
     }
+    // workspace of one chunk: at most cap_words individuals and 2 * cap_words micro-op entries
+    const long long cap_words = half / 4 - 3;
+    if ((s = reserve_U(2 * cap_words + 2)) != BEAGLE_OK) return s;
     return BEAGLE_OK;
 }
 
@@ -621,8 +805,8 @@ beagle_status beagle_eval_chunked(const int32_t* h_genomes, const int32_t* h_len
             CU(cudaMemcpyAsync(d_tok, h_genomes + tok0, sizeof(int32_t) * ntok, cudaMemcpyHostToDevice, w.copy_stream));
         CU(cudaEventRecord(w.ev_copied[b], w.copy_stream));
         CU(cudaStreamWaitEvent(st, w.ev_copied[b], 0));
-        if ((s = run_prepass(d_tok, d_len, np, n_consts, X, y, N, d, fitness_out + p0, nullptr, st)) != BEAGLE_OK) return s;
-        if ((s = run_eval(d_tok, d_len, w.stage_consts, N, d, tax, fitness_out + p0, nullptr, st)) != BEAGLE_OK) return s;
+        if ((s = run_prepass(d_tok, d_len, np, w.stage_consts, n_consts, X, y, N, d, fitness_out + p0, nullptr, ntok, true, st)) != BEAGLE_OK) return s;
+        if ((s = run_eval(d_tok, d_len, w.stage_consts, X, y, np, N, d, tax, fitness_out + p0, nullptr, st)) != BEAGLE_OK) return s;
         CU(cudaEventRecord(w.ev_free[b], st));
         total_launches += g_launches; g_launches = 0;
         p0 = p1; tok0 += ntok;
@@ -655,20 +839,27 @@ int32_t beagle_last_cuda_error(void) { return g_last_cuda; }
 
 beagle_status beagle_reserve(int64_t P_max, int64_t T_max)
 {
-    (void)T_max;   // the workspace does not depend on the token count (tokens are read in place)
-    if (P_max < 0 || P_max > 0x7FFFFFFFll) return BEAGLE_ERR_INVALID_ARG;
+    if (P_max < 0 || P_max > 0x7FFFFFFFll || T_max < 0) return BEAGLE_ERR_INVALID_ARG;
     beagle_status s = init_once();
     if (s != BEAGLE_OK) return s;
-    return reserve_P(P_max);
+    if ((s = reserve_P(P_max)) != BEAGLE_OK) return s;
+    if (T_max > 0) {
+        if ((s = reserve_U(uop_entries_bound(P_max, T_max))) != BEAGLE_OK) return s;
+        g_ws.promised_P = P_max; g_ws.promised_T = T_max;
+    }
+    return BEAGLE_OK;
 }
 
 void beagle_release(void)
 {
     Workspace& w = g_ws;
     cudaDeviceSynchronize();
-    cudaFree(w.off); cudaFree(w.key); cudaFree(w.depth); cudaFree(w.perm); cudaFree(w.bsum);
+    cudaFree(w.off); cudaFree(w.depth); cudaFree(w.perm); cudaFree(w.meta); cudaFree(w.deep_list);
+    cudaFree(w.slow_list); cudaFree(w.bsum); cudaFree(w.uops);
     cudaFree(w.stage[0]); cudaFree(w.stage[1]); cudaFree(w.stage_consts);
-    w.off = nullptr; w.key = nullptr; w.depth = nullptr; w.perm = nullptr; w.bsum = nullptr; w.cap_P = 0;
+    w.off = nullptr; w.depth = nullptr; w.perm = nullptr; w.meta = nullptr; w.deep_list = nullptr;
+    w.slow_list = nullptr; w.bsum = nullptr; w.uops = nullptr; w.cap_P = 0; w.cap_U = 0;
+    w.promised_P = 0; w.promised_T = 0;
     w.stage[0] = w.stage[1] = nullptr; w.stage_bytes = 0; w.stage_consts = nullptr; w.stage_consts_cap = 0;
 }
 
