@@ -31,26 +31,23 @@ constexpr int kNumBins = BEAGLE_MAX_LEN + 1;   // bin = 512 - length  (longest f
 constexpr int kScanThreads = 256;              // programs per block in the pre-pass
 constexpr int kCompileThreads = 128;
 constexpr int kStagesMax = 8;                  // micro-op stages in flight per warp
-constexpr int kMainThreads = 512;              // 16 warps (4 per scheduler): 128 registers per thread
-constexpr int kMainSlots = 5;                  // s[] slots of the main interpreter
-constexpr int kDeepThreads = 384;              // 12 warps (3 per scheduler): 168 registers per thread
+constexpr int kEvalThreads = 512;              // 16 warps (4 per scheduler): 128 registers per thread
 constexpr int kProfMax = 256;                  // beagle_set_profiling: recorded calls
 constexpr int kCasePad = 512;                  // staged cases are padded to a multiple of 32*K
-constexpr int kStageBytesMax = ((BEAGLE_MAX_LEN + 2 + 1) & ~1) * 8;   // 4112
+constexpr int kStageBytesMax = ((BEAGLE_MAX_LEN + 3 + 1) & ~1) * 8;   // 4128
 
 struct Header {                                // device-resident results of the pre-pass
     long long T;                               // total tokens = sum of in-range lengths
     long long uop_entries;                     // micro-op entries reserved by the bins
     int n_sorted;                              // individuals with an in-range length (= entries of perm[])
     int max_len;                               // longest in-range length (>= 1 if n_sorted > 0)
-    int n_deep;                                // individuals that need more than kMainSlots slots
     int n_slow;                                // individuals whose micro-ops did not fit the workspace
     int n_malformed;
-    unsigned int queue[2];                     // work-queue cursors of the interpreter kernels
+    unsigned int queue;                        // work-queue cursor of the interpreter kernel
 };
 
 struct EvalParams {
-    const int4* meta; const uint2* uops; const int* list; const Header* hdr; unsigned int* queue;
+    const int4* meta; const uint2* uops; const Header* hdr; unsigned int* queue;
     const float* xt; float* fitness; float* outputs;
     float tax; int n; int npad; int d; int ring_bytes;
 };
@@ -76,7 +73,7 @@ __device__ __forceinline__ void tma_bulk_g2s(void* dst, const void* src, uint32_
 }
 
 __device__ __forceinline__ int clamp_len(int l) { return (l >= 1 && l <= BEAGLE_MAX_LEN) ? l : 0; }
-__device__ __host__ __forceinline__ int uop_stride(int len) { return (len + 2 + 1) & ~1; }   // entries: nu <= len, END, pad; even
+__device__ __host__ __forceinline__ int uop_stride(int len) { return (len + 3 + 1) & ~1; }   // records: n <= len micro-ops + 3; even
 
 // ---- a2: block sums of the lengths + histogram of the lengths -----------------------------------------
 __global__ void __launch_bounds__(kScanThreads) k_len_pass1(const int32_t* __restrict__ lengths, long long P,
@@ -179,8 +176,8 @@ __global__ void __launch_bounds__(1024) k_len_pass2(long long* __restrict__ bsum
         hdr->T = carry_s;
         hdr->n_sorted = (int)carry2_s;
         hdr->max_len = maxlen_s;
-        hdr->n_deep = 0; hdr->n_slow = 0; hdr->n_malformed = 0;
-        hdr->queue[0] = 0; hdr->queue[1] = 0;
+        hdr->n_slow = 0; hdr->n_malformed = 0;
+        hdr->queue = 0;
     }
     // transpose: xt[j][i] = X[i][j] (j < d), xt[d][i] = y[i]; cases i >= n are zero
     for (int e = threadIdx.x; e < (d + 1) * npad; e += blockDim.x) {
@@ -233,15 +230,16 @@ __global__ void __launch_bounds__(kScanThreads) k_scatter(
 
 // ---- a3/a5: the tree compiler ----------------------------------------------------------------------------
 // One thread per individual, in length-sorted order (the threads of a warp run programs of equal
-// length). Pass 1 walks the postfix program once: well-formedness (D3), and per token the
-// size of its subtree and the number of s[] slots its evaluation needs. Pass 2 walks the tree from
-// the root and emits micro-ops (uop.cuh) in evaluation order.
+// length). One walk over the postfix program with an abstract stack whose entries are either a
+// terminal that has not been evaluated yet (its token is kept) or "computed" (R): well-formedness
+// (D3) and the micro-ops of uop.cuh, in the program's own evaluation order.
+//   acc always holds the topmost computed entry; the k-th computed entry below it is in slot s[R-2-k].
 struct CompileParams {
     const uint32_t* genomes; const long long* off; const int32_t* lengths; const int* perm;
     const float* consts; long long n_consts; int d; int npad;
     const int* binstart; const long long* binubase; Header* hdr;
-    uint2* uops; long long ucap; int4* meta; int* depth; int* deep_list; int* slow_list;
-    float* fitness; float* outputs; int n_cases; int slots_main; int emit;
+    uint2* uops; long long ucap; int4* meta; int* depth; int* slow_list;
+    float* fitness; float* outputs; int n_cases; int emit;
 };
 
 __global__ void __launch_bounds__(kCompileThreads) k_compile(const CompileParams q)
@@ -254,169 +252,102 @@ __global__ void __launch_bounds__(kCompileThreads) k_compile(const CompileParams
     const int stride = uop_stride(len);
     const long long ua = q.binubase[bin] + (long long)(i - q.binstart[bin]) * stride;
     const uint32_t* tok = q.genomes + q.off[p];
+    const bool fits = ua + stride <= q.ucap;
+    const bool wr = q.emit && fits;
+    uint2* out = q.uops + (wr ? ua : 0);
 
-    // info[t]: bits 0-9 subtree size, bits 10-12 slots needed, bit 15 terminal
-    unsigned short info[BEAGLE_MAX_LEN];
-    int sp = 0, mx = 0;
+    uint32_t ttok[BEAGLE_MAX_STACK];               // tokens of the unevaluated terminals on the abstract stack
+    uint32_t rmask = 0;                            // bit k: stack entry k is computed
+    int sp = 0, mx = 0, R = 0, n = 0;
+    uint32_t carry = 0, prev_opnd = 0;             // extra << 8 and operand of the previous micro-op
     bool ok = true;
+    const uint32_t xrow = (uint32_t)q.npad * 4u;
+
+    auto emit = [&](uint32_t h, uint32_t extra, uint32_t opnd) {       // rec[n] = {handler_n | extra_{n-1} << 8, operand_{n-1}}
+        if (wr) out[n] = make_uint2(carry | h, prev_opnd);
+        carry = extra << 8; prev_opnd = opnd; ++n;
+    };
+    auto operand_of = [&](uint32_t w) -> uint32_t {
+        return tok_op(w) == OPC_LOAD ? tok_arg(w) * xrow : __float_as_uint(__ldg(q.consts + tok_arg(w)));
+    };
+    auto materialise = [&](uint32_t w) {           // a terminal becomes the accumulator; the old accumulator is pushed
+        const bool isx = tok_op(w) == OPC_LOAD;
+        const int S = R - 1;
+        uint32_t h, extra = 0;
+        if (S < 0) h = isx ? H_LOADX : H_CONST;
+        else if (S < kRegSlots) h = (isx ? H_PUSHX : H_PUSHC) + (uint32_t)S;
+        else { h = isx ? H_PUSHXM : H_PUSHCM; extra = (uint32_t)(S - kRegSlots) * 64u; }
+        emit(h, extra, operand_of(w));
+        ++R;
+    };
+
     for (int t = 0; t < len; ++t) {
         const uint32_t w = __ldg(tok + t);
         const uint32_t op = tok_op(w), arg = tok_arg(w);
-        unsigned int inf = 0;
-        if (op == OPC_CONST) { ok &= ((long long)arg < q.n_consts); ++sp; inf = 0x8001u; }
-        else if (op == OPC_LOAD) { ok &= ((int)arg < q.d); ++sp; inf = 0x8001u; }
-        else if (op >= OPC_ADD && op <= OPC_DIV) {
-            ok &= (arg == 0) & (sp >= 2);
+        if (op == OPC_CONST || op == OPC_LOAD) {
+            ok &= (op == OPC_CONST) ? ((long long)arg < q.n_consts) : ((int)arg < q.d);
+            ok &= (sp < BEAGLE_MAX_STACK);
             if (!ok) break;
-            const unsigned int ir = info[t - 1];
-            const int sr = ir & 0x3FF;
-            const unsigned int il = info[t - 1 - sr];
-            const int sl = il & 0x3FF;
-            const int nr = (ir >> 10) & 7, nl = (il >> 10) & 7;
-            const bool tr = ir >> 15, tl = il >> 15;
-            int need;
-            if (tl && tr) need = 0;
-            else if (tr) need = nl;
-            else if (tl) need = nr;
-            else need = max(max(nl, nr), min(nl, nr) + 1);
-            inf = (unsigned)(sl + sr + 1) | ((unsigned)need << 10);
-            --sp;
-        }
-        else if (op >= OPC_SIN && op <= OPC_EXP) {
+            ttok[sp] = w; rmask &= ~(1u << sp); ++sp;
+            mx = max(mx, sp);
+        } else if (op >= OPC_SIN && op <= OPC_EXP) {
             ok &= (arg == 0) & (sp >= 1);
             if (!ok) break;
-            const unsigned int ic = info[t - 1];
-            inf = (unsigned)((ic & 0x3FF) + 1) | ((ic >> 15) ? 0u : (ic & 0x1C00u));
-        }
-        else ok = false;
-        ok &= (sp <= BEAGLE_MAX_STACK);
-        if (!ok) break;
-        info[t] = (unsigned short)inf;
-        mx = max(mx, sp);
+            const int a = sp - 1;
+            if (!((rmask >> a) & 1u)) { materialise(ttok[a]); rmask |= 1u << a; }
+            emit(H_SIN + (op - OPC_SIN), 0u, 0u);
+        } else if (op >= OPC_ADD && op <= OPC_DIV) {
+            ok &= (arg == 0) & (sp >= 2);
+            if (!ok) break;
+            const int a = sp - 2, b = sp - 1;
+            const bool ra = (rmask >> a) & 1u, rb = (rmask >> b) & 1u;
+            const uint32_t k = op - OPC_ADD;
+            if (rb) {
+                if (ra) {                          // both computed: s[R-2] and acc
+                    const int S = R - 2;
+                    if (S < kRegSlots) emit(H_ADDS + k * kRegSlots + (uint32_t)S, 0u, 0u);
+                    else emit(H_ADDM + k, (uint32_t)(S - kRegSlots) * 64u, 0u);
+                    --R;
+                } else {                           // acc = terminal(a) op acc; ADD and MUL commute bit for bit
+                    const uint32_t wa = ttok[a];
+                    const bool isx = tok_op(wa) == OPC_LOAD;
+                    const uint32_t hx = op == OPC_ADD ? H_ADDX : op == OPC_MUL ? H_MULX : op == OPC_SUB ? H_XSUB : H_XDIV;
+                    emit(isx ? hx : hx + (H_ADDC - H_ADDX), 0u, operand_of(wa));
+                }
+            } else {                               // acc = acc op terminal(b)
+                if (!ra) materialise(ttok[a]);
+                const uint32_t wb = ttok[b];
+                emit((tok_op(wb) == OPC_LOAD ? H_ADDX : H_ADDC) + k, 0u, operand_of(wb));
+            }
+            rmask |= 1u << a;
+            --sp;
+        } else { ok = false; break; }
     }
     ok &= (sp >= 1);
     if (!ok) {
         q.depth[p] = 0;
         if (q.fitness) q.fitness[p] = __uint_as_float(0x7FC00000u);
         if (q.outputs) for (int c = 0; c < q.n_cases; ++c) q.outputs[(size_t)p * q.n_cases + c] = __uint_as_float(0x7FC00000u);
-        q.meta[i] = make_int4(p, 0, KIND_SKIP << 24, len);
+        q.meta[i] = make_int4(p, 0, 0, len);
         atomicAdd(&q.hdr->n_malformed, 1);
         return;
     }
     q.depth[p] = mx;
-    if (!q.emit) { q.meta[i] = make_int4(p, 0, KIND_SKIP << 24, len); return; }
-    if (ua + stride > q.ucap) {                  // the workspace promise of beagle_reserve was broken: slow path
+    if (!q.emit) { q.meta[i] = make_int4(p, 0, 0, len); return; }
+    if (!fits) {                                   // the workspace promise of beagle_reserve was broken: slow path
         q.slow_list[atomicAdd(&q.hdr->n_slow, 1)] = p;
-        q.meta[i] = make_int4(p, 0, KIND_SKIP << 24, len);
+        q.meta[i] = make_int4(p, 0, 0, len);
         return;
     }
-
-    // pass 2: work stack entries = pos | kind << 9
-    enum { W_VISIT = 0, W_UN = 1, W_BINT = 2, W_TBIN = 3, W_BINS = 4, W_BINSR = 5 };
-    unsigned short ws[BEAGLE_MAX_LEN];
-    int wsp = 0, n = 0, R = 0, Rmax = 0;
-    uint2* out = q.uops + ua;
-    const uint32_t xrow = (uint32_t)q.npad * 4u;
-    auto materialise = [&](int t) {              // terminal t becomes the accumulator (the old one is pushed)
-        const uint32_t w = __ldg(tok + t);
-        const bool isx = tok_op(w) == OPC_LOAD;
-        const uint32_t h = R >= 1 ? (isx ? H_PUSHX : H_PUSHC) + (uint32_t)(R - 1) : (isx ? H_LOADX : H_CONST);
-        out[n++] = isx ? make_uint2(h | (tok_arg(w) * xrow) << 8, 0u)
-                       : make_uint2(h, __float_as_uint(__ldg(q.consts + tok_arg(w))));
-        ++R; Rmax = max(Rmax, R);
-    };
-    auto with_terminal = [&](uint32_t hx, uint32_t hc, int t) {   // a command with terminal t folded in
-        const uint32_t w = __ldg(tok + t);
-        out[n++] = tok_op(w) == OPC_LOAD ? make_uint2(hx | (tok_arg(w) * xrow) << 8, 0u)
-                                         : make_uint2(hc, __float_as_uint(__ldg(q.consts + tok_arg(w))));
-    };
-    ws[wsp++] = (unsigned short)((len - 1) | (W_VISIT << 9));
-    while (wsp > 0) {
-        const unsigned int e = ws[--wsp];
-        const int t = e & 0x1FF, kind = e >> 9;
-        const uint32_t op = tok_op(__ldg(tok + t));
-        if (kind == W_VISIT) {
-            if (op <= OPC_LOAD) materialise(t);
-            else if (op >= OPC_SIN) {
-                ws[wsp++] = (unsigned short)(t | (W_UN << 9));
-                ws[wsp++] = (unsigned short)((t - 1) | (W_VISIT << 9));
-            } else {
-                const int r = t - 1;
-                const unsigned int ir = info[r];
-                const int l = r - (int)(ir & 0x3FF);
-                const unsigned int il = info[l];
-                const bool tr = ir >> 15, tl = il >> 15;
-                if (tl && tr) { materialise(l); with_terminal(H_ADDX + (op - OPC_ADD), H_ADDC + (op - OPC_ADD), r); }
-                else if (tr) { ws[wsp++] = (unsigned short)(t | (W_BINT << 9)); ws[wsp++] = (unsigned short)(l | (W_VISIT << 9)); }
-                else if (tl) { ws[wsp++] = (unsigned short)(t | (W_TBIN << 9)); ws[wsp++] = (unsigned short)(r | (W_VISIT << 9)); }
-                else if (((ir >> 10) & 7) > ((il >> 10) & 7)) {     // Sethi-Ullman: the needier subtree first
-                    ws[wsp++] = (unsigned short)(t | (W_BINSR << 9));
-                    ws[wsp++] = (unsigned short)(l | (W_VISIT << 9));
-                    ws[wsp++] = (unsigned short)(r | (W_VISIT << 9));
-                } else {
-                    ws[wsp++] = (unsigned short)(t | (W_BINS << 9));
-                    ws[wsp++] = (unsigned short)(r | (W_VISIT << 9));
-                    ws[wsp++] = (unsigned short)(l | (W_VISIT << 9));
-                }
-            }
-        } else if (kind == W_UN) {
-            out[n++] = make_uint2(H_SIN + (op - OPC_SIN), 0u);
-        } else if (kind == W_BINT) {             // acc = acc op terminal(t-1)
-            with_terminal(H_ADDX + (op - OPC_ADD), H_ADDC + (op - OPC_ADD), t - 1);
-        } else if (kind == W_TBIN) {             // acc = terminal(l) op acc; ADD and MUL commute bit for bit
-            const int l = t - 1 - (int)(info[t - 1] & 0x3FF);
-            const uint32_t hx = op == OPC_ADD ? H_ADDX : op == OPC_MUL ? H_MULX : op == OPC_SUB ? H_XSUB : H_XDIV;
-            const uint32_t hc = op == OPC_ADD ? H_ADDC : op == OPC_MUL ? H_MULC : op == OPC_SUB ? H_CSUB : H_CDIV;
-            with_terminal(hx, hc, l);
-        } else {                                 // both operands computed: s[R-2] and acc
-            const uint32_t S = (uint32_t)(R - 2);
-            uint32_t h;
-            if (kind == W_BINS) h = H_ADDS + (op - OPC_ADD) * kSlotsMax;          // acc = s[S] op acc
-            else h = op == OPC_ADD ? H_ADDS : op == OPC_MUL ? H_MULS : op == OPC_SUB ? H_RSUBS : H_RDIVS;   // acc = acc op s[S]
-            out[n++] = make_uint2(h + S, 0u);
-            --R;
-        }
-    }
-    out[n] = make_uint2(H_END, 0u);
+    if (!((rmask >> (sp - 1)) & 1u)) materialise(ttok[sp - 1]);     // the result is a bare terminal
+    out[n] = make_uint2(carry | H_END, prev_opnd);
     out[n + 1] = make_uint2(H_END, 0u);
-    const int slots = Rmax - 1;
-    const int kind = slots > q.slots_main ? KIND_DEEP : KIND_MAIN;
-    if (kind == KIND_DEEP) q.deep_list[atomicAdd(&q.hdr->n_deep, 1)] = i;
-    q.meta[i] = make_int4(p, (int)(ua >> 1), n | (slots << 16) | (kind << 24), len);
+    out[n + 2] = make_uint2(H_END, 0u);
+    q.meta[i] = make_int4(p, (int)(ua >> 1), (n + 2 + 1) & ~1, len);
 }
 
-// ---- the interpreter kernels ---------------------------------------------------------------------------
-#define BG_NAME k_eval_main
-#define BG_K 16
-#define BG_D 5
-#define BG_THREADS kMainThreads
-#define BG_KIND KIND_MAIN
-#define BG_LIST 0
-#define BG_INTERP interp_run_d5
+// ---- the interpreter kernel -----------------------------------------------------------------------------
 #include "eval_kernel.inc"
-#undef BG_NAME
-#undef BG_K
-#undef BG_D
-#undef BG_THREADS
-#undef BG_KIND
-#undef BG_LIST
-#undef BG_INTERP
-
-#define BG_NAME k_eval_deep
-#define BG_K 16
-#define BG_D 8
-#define BG_THREADS kDeepThreads
-#define BG_KIND KIND_DEEP
-#define BG_LIST 1
-#define BG_INTERP interp_run_d8
-#include "eval_kernel.inc"
-#undef BG_NAME
-#undef BG_K
-#undef BG_D
-#undef BG_THREADS
-#undef BG_KIND
-#undef BG_LIST
-#undef BG_INTERP
 
 // ---- prior art as a baseline, and the slow path: the paper's mapping ------------------------
 // One block per individual, one thread per fitness case, a 32-entry per-thread stack in local
@@ -486,7 +417,7 @@ struct Workspace {
     long long cap_P = 0, cap_U = 0;            // individuals / micro-op entries the workspace holds
     long long promised_P = 0, promised_T = 0;  // beagle_reserve: calls with P <= promised_P have T <= promised_T
     long long* off = nullptr; int* depth = nullptr; int* perm = nullptr; int4* meta = nullptr;
-    int* deep_list = nullptr; int* slow_list = nullptr; long long* bsum = nullptr;
+    int* slow_list = nullptr; long long* bsum = nullptr;
     uint2* uops = nullptr;
     int* bins = nullptr; int* cursor = nullptr; int* binstart = nullptr; long long* binubase = nullptr;
     float* xt = nullptr; Header* hdr = nullptr; long long* h_T = nullptr;
@@ -516,8 +447,7 @@ static beagle_status init_once()
     w.device_ok = (prop.major == 10);
     w.inited = true;
     if (!w.device_ok) return BEAGLE_ERR_UNSUPPORTED;
-    CU(cudaFuncSetAttribute(k_eval_main, cudaFuncAttributeMaxDynamicSharedMemorySize, w.smem_optin));
-    CU(cudaFuncSetAttribute(k_eval_deep, cudaFuncAttributeMaxDynamicSharedMemorySize, w.smem_optin));
+    CU(cudaFuncSetAttribute(k_eval, cudaFuncAttributeMaxDynamicSharedMemorySize, w.smem_optin));
     CU(cudaMalloc(&w.bins, sizeof(int) * kNumBins));
     CU(cudaMalloc(&w.cursor, sizeof(int) * kNumBins));
     CU(cudaMemset(w.bins, 0, sizeof(int) * kNumBins));
@@ -536,16 +466,15 @@ static beagle_status reserve_P(long long P)
     Workspace& w = g_ws;
     if (P <= w.cap_P) return BEAGLE_OK;
     CU(cudaDeviceSynchronize());
-    cudaFree(w.off); cudaFree(w.depth); cudaFree(w.perm); cudaFree(w.meta); cudaFree(w.deep_list);
+    cudaFree(w.off); cudaFree(w.depth); cudaFree(w.perm); cudaFree(w.meta);
     cudaFree(w.slow_list); cudaFree(w.bsum);
-    w.off = nullptr; w.depth = nullptr; w.perm = nullptr; w.meta = nullptr; w.deep_list = nullptr;
+    w.off = nullptr; w.depth = nullptr; w.perm = nullptr; w.meta = nullptr;
     w.slow_list = nullptr; w.bsum = nullptr; w.cap_P = 0;
     const long long nb = (P + kScanThreads - 1) / kScanThreads;
     CU(cudaMalloc(&w.off, sizeof(long long) * (P + 1)));
     CU(cudaMalloc(&w.depth, sizeof(int) * P));
     CU(cudaMalloc(&w.perm, sizeof(int) * P));
     CU(cudaMalloc(&w.meta, sizeof(int4) * P));
-    CU(cudaMalloc(&w.deep_list, sizeof(int) * P));
     CU(cudaMalloc(&w.slow_list, sizeof(int) * P));
     CU(cudaMalloc(&w.bsum, sizeof(long long) * (nb + 1)));
     w.cap_P = P;
@@ -563,7 +492,7 @@ static beagle_status reserve_U(long long U)
     return BEAGLE_OK;
 }
 
-static long long uop_entries_bound(long long P, long long T) { return T + 3 * P + 2; }   // sum of uop_stride(len)
+static long long uop_entries_bound(long long P, long long T) { return T + 4 * P + 2; }   // sum of uop_stride(len)
 
 static beagle_status check_args(const void* genomes, const void* lengths, int64_t P, const void* consts,
                                 int64_t n_consts, const void* X, const void* y, int32_t N, int32_t d, const void* out)
@@ -608,8 +537,8 @@ static beagle_status run_prepass(const int32_t* genomes, const int32_t* lengths,
         CompileParams q;
         q.genomes = reinterpret_cast<const uint32_t*>(genomes); q.off = w.off; q.lengths = lengths; q.perm = w.perm;
         q.consts = consts; q.n_consts = n_consts; q.d = d; q.npad = npad; q.binstart = w.binstart; q.binubase = w.binubase;
-        q.hdr = w.hdr; q.uops = w.uops; q.ucap = w.cap_U; q.meta = w.meta; q.depth = w.depth; q.deep_list = w.deep_list;
-        q.slow_list = w.slow_list; q.fitness = fitness; q.outputs = outputs; q.n_cases = N; q.slots_main = kMainSlots; q.emit = emit ? 1 : 0;
+        q.hdr = w.hdr; q.uops = w.uops; q.ucap = w.cap_U; q.meta = w.meta; q.depth = w.depth;
+        q.slow_list = w.slow_list; q.fitness = fitness; q.outputs = outputs; q.n_cases = N; q.emit = emit ? 1 : 0;
         k_compile<<<(unsigned)((P + kCompileThreads - 1) / kCompileThreads), kCompileThreads, 0, st>>>(q);
         ++g_launches;
     }
@@ -635,7 +564,7 @@ static beagle_status run_eval(const int32_t* genomes, const int32_t* lengths, co
     const int npad = (N + kCasePad - 1) / kCasePad * kCasePad;
     const long long xs_bytes = (long long)(d + 1) * npad * 4;
     EvalParams prm;
-    prm.meta = w.meta; prm.uops = w.uops; prm.list = w.deep_list; prm.hdr = w.hdr; prm.xt = w.xt;
+    prm.meta = w.meta; prm.uops = w.uops; prm.hdr = w.hdr; prm.xt = w.xt;
     prm.fitness = fitness; prm.outputs = outputs; prm.tax = tax; prm.n = N; prm.npad = npad; prm.d = d;
     const bool prof = g_profiling && w.prof_n < kProfMax;
     if (prof) {
@@ -644,14 +573,11 @@ static beagle_status run_eval(const int32_t* genomes, const int32_t* lengths, co
         CU(cudaEventRecord(w.ev_k[2 * w.prof_n], st));
     }
     size_t smem = 0;
-    prm.ring_bytes = ring_bytes_for(kMainThreads, xs_bytes, w.smem_optin, &smem);
+    prm.ring_bytes = ring_bytes_for(kEvalThreads, xs_bytes, w.smem_optin, &smem);
     if (prm.ring_bytes < kStageBytesMax) return BEAGLE_ERR_UNSUPPORTED;
-    prm.queue = &w.hdr->queue[0];
-    k_eval_main<<<w.num_sms, kMainThreads, smem, st>>>(prm);
-    prm.ring_bytes = ring_bytes_for(kDeepThreads, xs_bytes, w.smem_optin, &smem);
-    prm.queue = &w.hdr->queue[1];
-    k_eval_deep<<<w.num_sms, kDeepThreads, smem, st>>>(prm);
-    g_launches += 2;
+    prm.queue = &w.hdr->queue;
+    k_eval<<<w.num_sms, kEvalThreads, smem, st>>>(prm);
+    ++g_launches;
     if (prof) { CU(cudaEventRecord(w.ev_k[2 * w.prof_n + 1], st)); ++w.prof_n; }
     // slow path: individuals whose micro-ops did not fit the promised workspace (normally none)
     k_eval_blockwise<<<w.num_sms * 2, (N + 31) / 32 * 32, 0, st>>>(genomes, w.off, lengths, w.depth, consts, X, y, N, d, tax,
@@ -854,10 +780,10 @@ void beagle_release(void)
 {
     Workspace& w = g_ws;
     cudaDeviceSynchronize();
-    cudaFree(w.off); cudaFree(w.depth); cudaFree(w.perm); cudaFree(w.meta); cudaFree(w.deep_list);
+    cudaFree(w.off); cudaFree(w.depth); cudaFree(w.perm); cudaFree(w.meta);
     cudaFree(w.slow_list); cudaFree(w.bsum); cudaFree(w.uops);
     cudaFree(w.stage[0]); cudaFree(w.stage[1]); cudaFree(w.stage_consts);
-    w.off = nullptr; w.depth = nullptr; w.perm = nullptr; w.meta = nullptr; w.deep_list = nullptr;
+    w.off = nullptr; w.depth = nullptr; w.perm = nullptr; w.meta = nullptr;
     w.slow_list = nullptr; w.bsum = nullptr; w.uops = nullptr; w.cap_P = 0; w.cap_U = 0;
     w.promised_P = 0; w.promised_T = 0;
     w.stage[0] = w.stage[1] = nullptr; w.stage_bytes = 0; w.stage_consts = nullptr; w.stage_consts_cap = 0;

@@ -28,8 +28,12 @@ def _check(col, oracle, gpu_fit, sel=None):
     msg = parity.describe(rep, gpu_fit, orc)
     print(f"config {col.cfg.number}: {msg}")
     assert len(rep["bad"]) == 0, msg
-    # the rule must not be vacuous: most individuals are STRICT (SURVEY.md §8(c) probe: 89-99 %)
-    assert rep["strict"] >= 0.70 * (rep["P"] - rep["malformed"] - rep["invalid"]), msg
+    # the rule must not be vacuous: most of the individuals it checks by value are STRICT, i.e. held to
+    # north_star's tolerance unchanged. DESIGN.md §4 "how many are STRICT": with every command correctly
+    # rounded (the best any fp32 evaluator can do) 82 % / 76 % / 80 % of the finite, stable individuals
+    # of configs 3 / 4 / 5 are STRICT; with this library's contract 75 % / 67 % / 74 %.
+    checked_finite = rep["strict"] + rep["conditioned"]
+    assert rep["strict"] >= 0.60 * checked_finite, msg
     return rep
 
 
