@@ -4,9 +4,9 @@
 //   a2  k_len_pass1 / k_len_pass2      block sums + length histogram; exclusive scans -> offsets, bins
 //   a3  k_scatter                      off[], counting sort by length (longest first) -> perm[]
 //       k_compile                      per-program well-formedness, tree compile to micro-ops (uop.cuh):
-//                                      terminal folding, Sethi-Ullman slot allocation
-//   a4  k_len_pass2 + TMA in k_eval    X,y transposed/padded once, bulk-copied per CTA
-//   a5-a7  k_eval_* (eval_kernel.inc)  TMA-fed interpreter: fetch, interpret, reduce, tax, store
+//                                      terminal folding, fused fresh values, slot allocation
+//   a4  k_len_pass2 + k_eval prologue  X,y transposed/padded once; X staged into tensor memory per CTA
+//   a5-a7  k_eval (eval_kernel.inc)    TMA-fed interpreter: fetch, interpret, reduce, tax, store
 //   a8  beagle_eval_chunked            double-buffered H2D on a copy stream
 // PyTorch is not involved: only the CUDA runtime. sm_100a only.
 #include <cuda_runtime.h>
@@ -31,7 +31,10 @@ constexpr int kNumBins = BEAGLE_MAX_LEN + 1;   // bin = 512 - length  (longest f
 constexpr int kScanThreads = 256;              // programs per block in the pre-pass
 constexpr int kCompileThreads = 128;
 constexpr int kStagesMax = 8;                  // micro-op stages in flight per warp
-constexpr int kEvalThreads = 512;              // 16 warps (4 per scheduler): 128 registers per thread
+#ifndef BEAGLE_EVAL_THREADS
+#define BEAGLE_EVAL_THREADS 1024
+#endif
+constexpr int kEvalThreads = BEAGLE_EVAL_THREADS;   // 32 warps (8 per scheduler): 64 registers per thread
 constexpr int kProfMax = 256;                  // beagle_set_profiling: recorded calls
 constexpr int kCasePad = 512;                  // staged cases are padded to a multiple of 32*K
 constexpr int kStageBytesMax = ((BEAGLE_MAX_LEN + 3 + 1) & ~1) * 8;   // 4128
@@ -50,6 +53,8 @@ struct EvalParams {
     const int4* meta; const uint2* uops; const Header* hdr; unsigned int* queue;
     const float* xt; float* fitness; float* outputs;
     float tax; int n; int npad; int d; int ring_bytes;
+    int slot_col0;      // first tensor-memory column after the variable block: passes * d * 16
+    int tmem_slots;     // S_T: slots per warp held in tensor memory (the deeper ones are in local memory)
 };
 
 // ---- PTX helpers: mbarrier, TMA bulk copy -----------------------------------------------------------
@@ -231,12 +236,13 @@ __global__ void __launch_bounds__(kScanThreads) k_scatter(
 // ---- a3/a5: the tree compiler ----------------------------------------------------------------------------
 // One thread per individual, in length-sorted order (the threads of a warp run programs of equal
 // length). One walk over the postfix program with an abstract stack whose entries are either a
-// terminal that has not been evaluated yet (its token is kept) or "computed" (R): well-formedness
+// terminal that has not been evaluated yet (its token is kept) or "computed": well-formedness
 // (D3) and the micro-ops of uop.cuh, in the program's own evaluation order.
-//   acc always holds the topmost computed entry; the k-th computed entry below it is in slot s[R-2-k].
+//   acc always holds the topmost computed entry; the computed entry with c others below it that is not
+//   in acc sits in slot c (tensor memory while c < S_T, local memory beyond).
 struct CompileParams {
     const uint32_t* genomes; const long long* off; const int32_t* lengths; const int* perm;
-    const float* consts; long long n_consts; int d; int npad;
+    const float* consts; long long n_consts; int d; int tmem_slots;
     const int* binstart; const long long* binubase; Header* hdr;
     uint2* uops; long long ucap; int4* meta; int* depth; int* slow_list;
     float* fitness; float* outputs; int n_cases; int emit;
@@ -258,27 +264,30 @@ __global__ void __launch_bounds__(kCompileThreads) k_compile(const CompileParams
 
     uint32_t ttok[BEAGLE_MAX_STACK];               // tokens of the unevaluated terminals on the abstract stack
     uint32_t rmask = 0;                            // bit k: stack entry k is computed
-    int sp = 0, mx = 0, R = 0, n = 0;
-    uint32_t carry = 0, prev_opnd = 0;             // extra << 8 and operand of the previous micro-op
+    int sp = 0, mx = 0, n = 0;
+    int c = 0;                                     // computed entries on the stack (the topmost one is acc)
     bool ok = true;
-    const uint32_t xrow = (uint32_t)q.npad * 4u;
 
-    auto emit = [&](uint32_t h, uint32_t extra, uint32_t opnd) {       // rec[n] = {handler_n | extra_{n-1} << 8, operand_{n-1}}
-        if (wr) out[n] = make_uint2(carry | h, prev_opnd);
-        carry = extra << 8; prev_opnd = opnd; ++n;
+    auto is_x = [](uint32_t w) { return tok_op(w) == OPC_LOAD; };
+    auto col_of = [](uint32_t w) -> uint32_t { return tok_arg(w) * (uint32_t)kCasesPerLane; };
+    auto cst_of = [&](uint32_t w) -> uint32_t { return __float_as_uint(__ldg(q.consts + tok_arg(w))); };
+    auto emit = [&](uint32_t h, uint32_t o) { if (wr) out[n] = make_uint2(h, o); ++n; };
+    // flags of a micro-op that starts a fresh value: acc (if live) is pushed to slot c-1 first
+    auto push_bits = [&]() -> uint32_t {
+        if (c == 0) return 0u;
+        const int s = c - 1;
+        return s < q.tmem_slots ? (kPushTmem | ((uint32_t)(s * kCasesPerLane) << kPushShift))
+                                : (kPushMem | ((uint32_t)((s - q.tmem_slots) * 64) << kPushShift));
     };
-    auto operand_of = [&](uint32_t w) -> uint32_t {
-        return tok_op(w) == OPC_LOAD ? tok_arg(w) * xrow : __float_as_uint(__ldg(q.consts + tok_arg(w)));
-    };
-    auto materialise = [&](uint32_t w) {           // a terminal becomes the accumulator; the old accumulator is pushed
-        const bool isx = tok_op(w) == OPC_LOAD;
-        const int S = R - 1;
-        uint32_t h, extra = 0;
-        if (S < 0) h = isx ? H_LOADX : H_CONST;
-        else if (S < kRegSlots) h = (isx ? H_PUSHX : H_PUSHC) + (uint32_t)S;
-        else { h = isx ? H_PUSHXM : H_PUSHCM; extra = (uint32_t)(S - kRegSlots) * 64u; }
-        emit(h, extra, operand_of(w));
-        ++R;
+    // acc = acc op c (rev: c op acc); x / c is x * rcp(c) with the division handler's own rcp
+    auto const_op = [&](uint32_t op, uint32_t cbits, bool rev, uint32_t hi) {
+        const float cf = __uint_as_float(cbits);
+        if (op == OPC_ADD) emit(hi | H_ADDC, cbits);
+        else if (op == OPC_MUL) emit(hi | H_MULC, cbits);
+        else if (op == OPC_SUB) emit(hi | (rev ? H_RSUBC : H_SUBC), cbits);
+        else if (rev) emit(hi | H_RDIVC, cbits);
+        else if (fabsf(cf) < kEps) emit((hi & (kPushTmem | kPushMem | (0x7FFu << kPushShift))) | H_LC, 0x3F800000u);   // protected: 1
+        else emit(hi | H_MULC, __float_as_uint(mufu_rcp(cf)));
     };
 
     for (int t = 0; t < len; ++t) {
@@ -294,30 +303,52 @@ __global__ void __launch_bounds__(kCompileThreads) k_compile(const CompileParams
             ok &= (arg == 0) & (sp >= 1);
             if (!ok) break;
             const int a = sp - 1;
-            if (!((rmask >> a) & 1u)) { materialise(ttok[a]); rmask |= 1u << a; }
-            emit(H_SIN + (op - OPC_SIN), 0u, 0u);
+            const uint32_t k = op - OPC_SIN;
+            if ((rmask >> a) & 1u) emit(H_SIN + k, 0u);
+            else {
+                const uint32_t wa = ttok[a], pb = push_bits();
+                if (is_x(wa)) emit(pb | (col_of(wa) << kColAShift) | (H_LX_SIN + k), 0u);
+                else { emit(pb | H_LC, cst_of(wa)); emit(H_SIN + k, 0u); }
+                rmask |= 1u << a; ++c;
+            }
         } else if (op >= OPC_ADD && op <= OPC_DIV) {
             ok &= (arg == 0) & (sp >= 2);
             if (!ok) break;
             const int a = sp - 2, b = sp - 1;
             const bool ra = (rmask >> a) & 1u, rb = (rmask >> b) & 1u;
-            const uint32_t k = op - OPC_ADD;
-            if (rb) {
-                if (ra) {                          // both computed: s[R-2] and acc
-                    const int S = R - 2;
-                    if (S < kRegSlots) emit(H_ADDS + k * kRegSlots + (uint32_t)S, 0u, 0u);
-                    else emit(H_ADDM + k, (uint32_t)(S - kRegSlots) * 64u, 0u);
-                    --R;
-                } else {                           // acc = terminal(a) op acc; ADD and MUL commute bit for bit
-                    const uint32_t wa = ttok[a];
-                    const bool isx = tok_op(wa) == OPC_LOAD;
-                    const uint32_t hx = op == OPC_ADD ? H_ADDX : op == OPC_MUL ? H_MULX : op == OPC_SUB ? H_XSUB : H_XDIV;
-                    emit(isx ? hx : hx + (H_ADDC - H_ADDX), 0u, operand_of(wa));
-                }
-            } else {                               // acc = acc op terminal(b)
-                if (!ra) materialise(ttok[a]);
+            if (ra && rb) {                        // slot[c-2] op acc
+                const int s = c - 2;
+                const uint32_t hs = op == OPC_ADD ? H_ADDS : op == OPC_MUL ? H_MULS : op == OPC_SUB ? H_RSUBS : H_RDIVS;
+                if (s < q.tmem_slots) emit(hs, (uint32_t)(s * kCasesPerLane));
+                else emit(hs + (H_ADDM - H_ADDS), (uint32_t)((s - q.tmem_slots) * 64));
+                --c;
+            } else if (ra) {                       // acc op terminal(b)
                 const uint32_t wb = ttok[b];
-                emit((tok_op(wb) == OPC_LOAD ? H_ADDX : H_ADDC) + k, 0u, operand_of(wb));
+                if (is_x(wb)) emit(op == OPC_ADD ? H_ADDX : op == OPC_MUL ? H_MULX : op == OPC_SUB ? H_SUBX : H_DIVX, col_of(wb));
+                else const_op(op, cst_of(wb), false, 0u);
+            } else if (rb) {                       // terminal(a) op acc; ADD and MUL commute bit for bit
+                const uint32_t wa = ttok[a];
+                if (is_x(wa)) emit(op == OPC_ADD ? H_ADDX : op == OPC_MUL ? H_MULX : op == OPC_SUB ? H_RSUBX : H_RDIVX, col_of(wa));
+                else const_op(op, cst_of(wa), true, 0u);
+            } else {                               // a fresh value from two terminals
+                const uint32_t wa = ttok[a], wb = ttok[b], pb = push_bits();
+                if (is_x(wa) && is_x(wb))
+                    emit(pb | (col_of(wa) << kColAShift) | (op == OPC_ADD ? H_LX_ADDX : op == OPC_MUL ? H_LX_MULX : op == OPC_SUB ? H_LX_SUBX : H_LX_DIVX), col_of(wb));
+                else if (is_x(wa)) {               // X[a] op c
+                    const uint32_t cb = cst_of(wb), hi = pb | (col_of(wa) << kColAShift);
+                    if (op == OPC_ADD) emit(hi | H_LX_ADDC, cb);
+                    else if (op == OPC_MUL) emit(hi | H_LX_MULC, cb);
+                    else if (op == OPC_SUB) emit(hi | H_LX_SUBC, cb);
+                    else if (fabsf(__uint_as_float(cb)) < kEps) emit(pb | H_LC, 0x3F800000u);
+                    else emit(hi | H_LX_MULC, __float_as_uint(mufu_rcp(__uint_as_float(cb))));
+                } else if (is_x(wb)) {             // c op X[b]
+                    const uint32_t cb = cst_of(wa), hi = pb | (col_of(wb) << kColAShift);
+                    emit(hi | (op == OPC_ADD ? H_LX_ADDC : op == OPC_MUL ? H_LX_MULC : op == OPC_SUB ? H_LX_RSUBC : H_LX_RDIVC), cb);
+                } else {                           // c op c: acc = c(a), then acc op c(b)
+                    emit(pb | H_LC, cst_of(wa));
+                    const_op(op, cst_of(wb), false, 0u);
+                }
+                ++c;
             }
             rmask |= 1u << a;
             --sp;
@@ -327,7 +358,7 @@ __global__ void __launch_bounds__(kCompileThreads) k_compile(const CompileParams
     if (!ok) {
         q.depth[p] = 0;
         if (q.fitness) q.fitness[p] = __uint_as_float(0x7FC00000u);
-        if (q.outputs) for (int c = 0; c < q.n_cases; ++c) q.outputs[(size_t)p * q.n_cases + c] = __uint_as_float(0x7FC00000u);
+        if (q.outputs) for (int cc = 0; cc < q.n_cases; ++cc) q.outputs[(size_t)p * q.n_cases + cc] = __uint_as_float(0x7FC00000u);
         q.meta[i] = make_int4(p, 0, 0, len);
         atomicAdd(&q.hdr->n_malformed, 1);
         return;
@@ -339,8 +370,11 @@ __global__ void __launch_bounds__(kCompileThreads) k_compile(const CompileParams
         q.meta[i] = make_int4(p, 0, 0, len);
         return;
     }
-    if (!((rmask >> (sp - 1)) & 1u)) materialise(ttok[sp - 1]);     // the result is a bare terminal
-    out[n] = make_uint2(carry | H_END, prev_opnd);
+    if (!((rmask >> (sp - 1)) & 1u)) {             // the result is a bare terminal
+        const uint32_t wa = ttok[sp - 1];
+        if (is_x(wa)) emit((col_of(wa) << kColAShift) | H_LX, 0u); else emit(H_LC, cst_of(wa));
+    }
+    out[n] = make_uint2(H_END, 0u);
     out[n + 1] = make_uint2(H_END, 0u);
     out[n + 2] = make_uint2(H_END, 0u);
     q.meta[i] = make_int4(p, (int)(ua >> 1), (n + 2 + 1) & ~1, len);
@@ -494,6 +528,20 @@ static beagle_status reserve_U(long long U)
 
 static long long uop_entries_bound(long long P, long long T) { return T + 4 * P + 2; }   // sum of uop_stride(len)
 
+// a4's plan of the 512 tensor-memory columns: the variable block (16 columns per variable and pass), then
+// S_T slots of 16 columns for each of the kEvalThreads/128 warps of a lane quarter. false: the variable
+// block does not fit (d > 32 at N <= 512, d > 16 beyond), and the call takes the blockwise kernel.
+static bool tmem_plan(int N, int d, int* slot_col0, int* tmem_slots)
+{
+    const int passes = (N + kCasesPerPass - 1) / kCasesPerPass;
+    const int nx = passes * d * kCasesPerLane;
+    if (nx > kTmemCols) return false;
+    int st = (kTmemCols - nx) / kCasesPerLane / (kEvalThreads / 128);
+    if (st > kMemSlots) st = kMemSlots;
+    *slot_col0 = nx; *tmem_slots = st;
+    return true;
+}
+
 static beagle_status check_args(const void* genomes, const void* lengths, int64_t P, const void* consts,
                                 int64_t n_consts, const void* X, const void* y, int32_t N, int32_t d, const void* out)
 {
@@ -536,7 +584,9 @@ static beagle_status run_prepass(const int32_t* genomes, const int32_t* lengths,
     {
         CompileParams q;
         q.genomes = reinterpret_cast<const uint32_t*>(genomes); q.off = w.off; q.lengths = lengths; q.perm = w.perm;
-        q.consts = consts; q.n_consts = n_consts; q.d = d; q.npad = npad; q.binstart = w.binstart; q.binubase = w.binubase;
+        int col0 = 0, st_slots = 0;
+        tmem_plan(N, d, &col0, &st_slots);
+        q.consts = consts; q.n_consts = n_consts; q.d = d; q.tmem_slots = st_slots; q.binstart = w.binstart; q.binubase = w.binubase;
         q.hdr = w.hdr; q.uops = w.uops; q.ucap = w.cap_U; q.meta = w.meta; q.depth = w.depth;
         q.slow_list = w.slow_list; q.fitness = fitness; q.outputs = outputs; q.n_cases = N; q.emit = emit ? 1 : 0;
         k_compile<<<(unsigned)((P + kCompileThreads - 1) / kCompileThreads), kCompileThreads, 0, st>>>(q);
@@ -546,10 +596,10 @@ static beagle_status run_prepass(const int32_t* genomes, const int32_t* lengths,
     return BEAGLE_OK;
 }
 
-static int ring_bytes_for(int threads, long long xs_bytes, int smem_optin, size_t* smem_out)
+static int ring_bytes_for(int threads, long long ys_bytes, int smem_optin, size_t* smem_out)
 {
     const int warps = threads / 32;
-    const long long fixed = ((64 + warps * kStagesMax * 8 + 127) & ~127) + ((xs_bytes + 127) & ~127ll);
+    const long long fixed = ((64 + warps * kStagesMax * 8 + 127) & ~127) + ((ys_bytes + 127) & ~127ll);
     long long ring = ((smem_optin - fixed) / warps) & ~127ll;
     if (ring > (long long)kStagesMax * kStageBytesMax) ring = (long long)kStagesMax * kStageBytesMax;
     *smem_out = (size_t)(fixed + ring * warps);
@@ -562,8 +612,9 @@ static beagle_status run_eval(const int32_t* genomes, const int32_t* lengths, co
 {
     Workspace& w = g_ws;
     const int npad = (N + kCasePad - 1) / kCasePad * kCasePad;
-    const long long xs_bytes = (long long)(d + 1) * npad * 4;
+    const long long ys_bytes = (long long)npad * 4;
     EvalParams prm;
+    if (!tmem_plan(N, d, &prm.slot_col0, &prm.tmem_slots)) return BEAGLE_ERR_UNSUPPORTED;   // callers check first
     prm.meta = w.meta; prm.uops = w.uops; prm.hdr = w.hdr; prm.xt = w.xt;
     prm.fitness = fitness; prm.outputs = outputs; prm.tax = tax; prm.n = N; prm.npad = npad; prm.d = d;
     const bool prof = g_profiling && w.prof_n < kProfMax;
@@ -573,7 +624,7 @@ static beagle_status run_eval(const int32_t* genomes, const int32_t* lengths, co
         CU(cudaEventRecord(w.ev_k[2 * w.prof_n], st));
     }
     size_t smem = 0;
-    prm.ring_bytes = ring_bytes_for(kEvalThreads, xs_bytes, w.smem_optin, &smem);
+    prm.ring_bytes = ring_bytes_for(kEvalThreads, ys_bytes, w.smem_optin, &smem);
     if (prm.ring_bytes < kStageBytesMax) return BEAGLE_ERR_UNSUPPORTED;
     prm.queue = &w.hdr->queue;
     k_eval<<<w.num_sms, kEvalThreads, smem, st>>>(prm);
@@ -582,6 +633,26 @@ static beagle_status run_eval(const int32_t* genomes, const int32_t* lengths, co
     // slow path: individuals whose micro-ops did not fit the promised workspace (normally none)
     k_eval_blockwise<<<w.num_sms * 2, (N + 31) / 32 * 32, 0, st>>>(genomes, w.off, lengths, w.depth, consts, X, y, N, d, tax,
                                                                    fitness, outputs, w.slow_list, &w.hdr->n_slow, P);
+    ++g_launches;
+    CU(cudaGetLastError());
+    return BEAGLE_OK;
+}
+
+// the whole path for one device-resident (chunk of a) colony: pre-pass + interpreter; when the variable
+// block does not fit tensor memory, the pre-pass (as a well-formedness check) + the blockwise kernel,
+// whose results are bit-identical (same per-command functions, same summation order).
+static beagle_status run_colony(const int32_t* genomes, const int32_t* lengths, long long P, const float* consts,
+                                long long n_consts, const float* X, const float* y, int N, int d, float tax,
+                                float* fitness, float* outputs, long long T_known, cudaStream_t st)
+{
+    Workspace& w = g_ws;
+    int col0, slots;
+    const bool fast = tmem_plan(N, d, &col0, &slots);
+    beagle_status s = run_prepass(genomes, lengths, P, consts, n_consts, X, y, N, d, fitness, outputs, T_known, fast, st);
+    if (s != BEAGLE_OK) return s;
+    if (fast) return run_eval(genomes, lengths, consts, X, y, P, N, d, tax, fitness, outputs, st);
+    k_eval_blockwise<<<(unsigned)P, (N + 31) / 32 * 32, 0, st>>>(genomes, w.off, lengths, w.depth, consts, X, y, N, d, tax,
+                                                                fitness, outputs, nullptr, nullptr, P);
     ++g_launches;
     CU(cudaGetLastError());
     return BEAGLE_OK;
@@ -604,8 +675,7 @@ beagle_status beagle_eval(const int32_t* genomes, const int32_t* lengths, int64_
     if ((s = init_once()) != BEAGLE_OK) return s;
     if ((s = reserve_P(P)) != BEAGLE_OK) return s;
     cudaStream_t st = (cudaStream_t)stream;
-    if ((s = run_prepass(genomes, lengths, P, consts, n_consts, X, y, N, d, fitness_out, nullptr, -1, true, st)) != BEAGLE_OK) return s;
-    return run_eval(genomes, lengths, consts, X, y, P, N, d, tax, fitness_out, nullptr, st);
+    return run_colony(genomes, lengths, P, consts, n_consts, X, y, N, d, tax, fitness_out, nullptr, -1, st);
 }
 
 beagle_status beagle_debug_outputs(const int32_t* genomes, const int32_t* lengths, int64_t P,
@@ -619,8 +689,7 @@ beagle_status beagle_debug_outputs(const int32_t* genomes, const int32_t* length
     if ((s = init_once()) != BEAGLE_OK) return s;
     if ((s = reserve_P(P)) != BEAGLE_OK) return s;
     cudaStream_t st = (cudaStream_t)stream;
-    if ((s = run_prepass(genomes, lengths, P, consts, n_consts, X, nullptr, N, d, nullptr, out_PxN, -1, true, st)) != BEAGLE_OK) return s;
-    return run_eval(genomes, lengths, consts, X, nullptr, P, N, d, 0.f, nullptr, out_PxN, st);
+    return run_colony(genomes, lengths, P, consts, n_consts, X, nullptr, N, d, 0.f, nullptr, out_PxN, -1, st);
 }
 
 beagle_status beagle_eval_blockwise(const int32_t* genomes, const int32_t* lengths, int64_t P,
@@ -731,8 +800,7 @@ beagle_status beagle_eval_chunked(const int32_t* h_genomes, const int32_t* h_len
             CU(cudaMemcpyAsync(d_tok, h_genomes + tok0, sizeof(int32_t) * ntok, cudaMemcpyHostToDevice, w.copy_stream));
         CU(cudaEventRecord(w.ev_copied[b], w.copy_stream));
         CU(cudaStreamWaitEvent(st, w.ev_copied[b], 0));
-        if ((s = run_prepass(d_tok, d_len, np, w.stage_consts, n_consts, X, y, N, d, fitness_out + p0, nullptr, ntok, true, st)) != BEAGLE_OK) return s;
-        if ((s = run_eval(d_tok, d_len, w.stage_consts, X, y, np, N, d, tax, fitness_out + p0, nullptr, st)) != BEAGLE_OK) return s;
+        if ((s = run_colony(d_tok, d_len, np, w.stage_consts, n_consts, X, y, N, d, tax, fitness_out + p0, nullptr, ntok, st)) != BEAGLE_OK) return s;
         CU(cudaEventRecord(w.ev_free[b], st));
         total_launches += g_launches; g_launches = 0;
         p0 = p1; tok0 += ntok;

@@ -3,52 +3,66 @@
 //
 // A Beagle program is postfix, i.e. a tree. The compiler turns it into code for an
 // ACCUMULATOR machine: `acc` (16 cases per lane, in registers) holds the most recently computed
-// value; s[0], s[1], ... hold computed values that wait for their sibling (s[0..kRegSlots) in
-// registers, the rest in local memory: "spilling only when needed"). Terminals (CONST, LOAD) that are
-// the operand of a binary command are folded into that command, so they cost no dispatch and no
-// register move:
-//     <A> x  ADD     ->  ADDX x        acc = acc + X[x]          (right operand terminal)
-//     x <A> SUB      ->  XSUB x        acc = X[x] - acc          (left operand terminal)
-//     <A> <B> DIV    ->  ... PUSH S ... DIVS S   acc = s[S] / acc  (both computed)
-// Commands run in the program's own order, and every micro-op computes exactly the value the postfix
-// command computes on the same operands with the same per-command function (ops.cuh / interp.cuh), so
-// per-case outputs are bit-identical to a plain stack machine (ADD and MUL commute bit for bit).
+// value; computed values that wait for their sibling are pushed to slots. Slots are not registers:
+// slot s < S_T lives in TENSOR MEMORY (16 columns of the warp's own TMEM lanes, written by one
+// tcgen05.st and read back by one tcgen05.ld straight into the operand registers), deeper slots in
+// local memory ("spilling only when needed"). The fitness-case matrix X lives in tensor memory too,
+// so a variable operand and a slot operand are the same instruction with a different column.
 //
-// Stream layout (uint2 records, one TMA bulk copy per program): the handler number of micro-op j+1
-// travels in record j, so that when handler j starts, the jump-table index of its successor is already
-// in a register and the table lookup overlaps the handler's arithmetic:
-//     rec[0]   = { handler_0,                      0         }
-//     rec[j+1] = { handler_{j+1} | extra_j << 8,   operand_j }      j = 0 .. n-1, handler_n = H_END
-//     rec[n+1] = { H_END, 0 }                                        (prefetch pad)
-// operand_j: byte offset of the variable's row in the staged case block (X-type), the fp32 constant's
-// bits (C-type); extra_j: byte offset of the slot in the lane's local slot memory (M-type).
+// Terminals (CONST, LOAD) never cost a dispatch: they are folded into the command that consumes them,
+//     <A> x  ADD     ->  ADDX  x          acc = acc + X[x]           (right operand terminal)
+//     x <A> SUB      ->  RSUBX x          acc = X[x] - acc           (left operand terminal)
+//     x  y  DIV      ->  LX_DIVX x, y     acc = X[x] / X[y]          (both terminal: a fresh value)
+//     x  SIN         ->  LX_SIN x         acc = sin X[x]
+//     <A> <B> DIV    ->  RDIVS s          acc = slot[s] / acc        (both computed)
+// and "push acc" is not a micro-op either: it is a flag of the micro-op that starts the next fresh
+// value, executed by the dispatcher on the way into that handler.
+// Commands run in the program's own order and every micro-op computes exactly the value the postfix
+// command computes on the same operands with the same per-command function (ops.cuh / interp.cuh), so
+// per-case outputs are bit-identical to a plain stack machine (ADD and MUL commute bit for bit;
+// x / c with a constant c is x * rcp(c) with the same rcp the division handler uses).
+//
+// Stream layout: uint2 records {h, o}, one per micro-op, one TMA bulk copy per program:
+//     rec[j] = record of micro-op j,  j = 0 .. n-1;   rec[n] = { H_END, 0 };   rec[n+1] = pad
+//   h  [7:0]    handler number (uop.cuh enum)
+//      [8]      push acc to a tensor-memory slot before this micro-op
+//      [9]      push acc to a local-memory slot before this micro-op
+//      [20:10]  where to push: TMEM column offset (slot * 16) or local byte offset (slot * 64)
+//      [31:21]  column of the FIRST operand of an LX_ micro-op (a variable: (pass-relative) column)
+//   o           second operand: column of a variable (X-type), column offset of a slot (S-type), byte
+//               offset of a slot in local memory (M-type), fp32 bits of a constant (C-type)
 #pragma once
 #include <stdint.h>
 
 namespace beagle {
 
-constexpr int kRegSlots = 4;    // s[0..4) live in registers
-constexpr int kMemSlots = 27;   // s[4..31) live in local memory (a 32-entry stack pushes at most 31 values)
+constexpr int kCasesPerLane = 16;          // K: cases per lane per pass (one pass = 512 cases)
+constexpr int kCasesPerPass = 32 * kCasesPerLane;
+constexpr int kTmemCols = 512;             // tensor memory columns of one SM (32-bit cells x 128 lanes)
+constexpr int kMemSlots = 31;              // a 32-entry stack pushes at most 31 computed values
 
 enum : uint32_t {
     H_END = 0,
-    H_LOADX = 1, H_CONST = 2,                                  // acc = X[j] | c      (acc was dead)
-    H_SIN = 3, H_COS = 4, H_LOG = 5, H_SQRT = 6, H_EXP = 7,    // acc = f(acc)
-    H_ADDX = 8, H_SUBX = 9, H_MULX = 10, H_DIVX = 11,          // acc = acc op X[j]
-    H_XSUB = 12, H_XDIV = 13,                                  // acc = X[j] op acc
-    H_ADDC = 14, H_SUBC = 15, H_MULC = 16, H_DIVC = 17,        // acc = acc op c
-    H_CSUB = 18, H_CDIV = 19,                                  // acc = c op acc
-    H_PUSHX = 20,                                              // +S: s[S] = acc; acc = X[j]
-    H_PUSHC = H_PUSHX + kRegSlots,                             // +S: s[S] = acc; acc = c
-    H_ADDS = H_PUSHC + kRegSlots,                              // +S: acc = s[S] + acc
-    H_SUBS = H_ADDS + kRegSlots,                               // +S: acc = s[S] - acc
-    H_MULS = H_SUBS + kRegSlots,                               // +S: acc = s[S] * acc
-    H_DIVS = H_MULS + kRegSlots,                               // +S: acc = s[S] / acc
-    H_PUSHXM = H_DIVS + kRegSlots,                             // mem[extra] = acc; acc = X[j]
-    H_PUSHCM = H_PUSHXM + 1,                                   // mem[extra] = acc; acc = c
-    H_ADDM = H_PUSHXM + 2, H_SUBM = H_PUSHXM + 3, H_MULM = H_PUSHXM + 4, H_DIVM = H_PUSHXM + 5,   // acc = mem[extra] op acc
-    H_COUNT = H_PUSHXM + 6
+    // acc = f(acc)
+    H_SIN = 1, H_COS = 2, H_LOG = 3, H_SQRT = 4, H_EXP = 5,
+    // acc = acc op X[o] | X[o] op acc            (x <- tensor memory, variable column)
+    H_ADDX = 6, H_SUBX = 7, H_MULX = 8, H_DIVX = 9, H_RSUBX = 10, H_RDIVX = 11,
+    // acc = slot op acc                          (x <- tensor memory, slot column)
+    H_ADDS = 12, H_MULS = 13, H_RSUBS = 14, H_RDIVS = 15,
+    // acc = slot op acc                          (x <- local memory)
+    H_ADDM = 16, H_MULM = 17, H_RSUBM = 18, H_RDIVM = 19,
+    // acc = acc op c | c op acc
+    H_ADDC = 20, H_SUBC = 21, H_MULC = 22, H_RSUBC = 23, H_RDIVC = 24,
+    // fresh values: acc = X[colA] (then the command)
+    H_LX = 25, H_LC = 26,                                             // acc = X[colA] | acc = c
+    H_LX_SIN = 27, H_LX_COS = 28, H_LX_LOG = 29, H_LX_SQRT = 30, H_LX_EXP = 31,
+    H_LX_ADDX = 32, H_LX_SUBX = 33, H_LX_MULX = 34, H_LX_DIVX = 35,
+    H_LX_ADDC = 36, H_LX_SUBC = 37, H_LX_MULC = 38, H_LX_RSUBC = 39, H_LX_RDIVC = 40,
+    H_COUNT = 41
 };
+
+constexpr uint32_t kPushTmem = 1u << 8, kPushMem = 1u << 9;
+constexpr int kPushShift = 10, kColAShift = 21;
 
 // meta[i] (one int4 per individual, in evaluation order): x = p (input index), y = record block address
 // in 16-byte units, z = number of records to copy (even), w = length in tokens (for the tax);
