@@ -36,6 +36,7 @@ constexpr int kStagesMax = 8;                  // micro-op stages in flight per 
 #endif
 constexpr int kEvalThreads = BEAGLE_EVAL_THREADS;   // 32 warps (8 per scheduler): 64 registers per thread
 constexpr int kProfMax = 256;                  // beagle_set_profiling: recorded calls
+constexpr int kEvalMetaBytes = 64 * 16;           // per-warp window of the work queue (64 x int4)
 constexpr int kCasePad = 512;                  // staged cases are padded to a multiple of 32*K
 constexpr int kStageBytesMax = ((BEAGLE_MAX_LEN + 3 + 1) & ~1) * 8;   // 4128
 
@@ -272,22 +273,22 @@ __global__ void __launch_bounds__(kCompileThreads) k_compile(const CompileParams
     auto col_of = [](uint32_t w) -> uint32_t { return tok_arg(w) * (uint32_t)kCasesPerLane; };
     auto cst_of = [&](uint32_t w) -> uint32_t { return __float_as_uint(__ldg(q.consts + tok_arg(w))); };
     auto emit = [&](uint32_t h, uint32_t o) { if (wr) out[n] = make_uint2(h, o); ++n; };
-    // flags of a micro-op that starts a fresh value: acc (if live) is pushed to slot c-1 first
+    // a micro-op that starts a fresh value while acc is live goes to the push entry of its handler:
+    // slot c-1 is on the tensor-memory slot stack while c-1 < S_T, in local memory beyond
     auto push_bits = [&]() -> uint32_t {
         if (c == 0) return 0u;
         const int s = c - 1;
-        return s < q.tmem_slots ? (kPushTmem | ((uint32_t)(s * kCasesPerLane) << kPushShift))
-                                : (kPushMem | ((uint32_t)((s - q.tmem_slots) * 64) << kPushShift));
+        return s < q.tmem_slots ? (uint32_t)H_PUSHT : ((uint32_t)H_PUSHM + ((uint32_t)((s - q.tmem_slots) * 64) << kPushShift));
     };
     // acc = acc op c (rev: c op acc); x / c is x * rcp(c) with the division handler's own rcp
-    auto const_op = [&](uint32_t op, uint32_t cbits, bool rev, uint32_t hi) {
+    auto const_op = [&](uint32_t op, uint32_t cbits, bool rev) {
         const float cf = __uint_as_float(cbits);
-        if (op == OPC_ADD) emit(hi | H_ADDC, cbits);
-        else if (op == OPC_MUL) emit(hi | H_MULC, cbits);
-        else if (op == OPC_SUB) emit(hi | (rev ? H_RSUBC : H_SUBC), cbits);
-        else if (rev) emit(hi | H_RDIVC, cbits);
-        else if (fabsf(cf) < kEps) emit((hi & (kPushTmem | kPushMem | (0x7FFu << kPushShift))) | H_LC, 0x3F800000u);   // protected: 1
-        else emit(hi | H_MULC, __float_as_uint(mufu_rcp(cf)));
+        if (op == OPC_ADD) emit(H_ADDC, cbits);
+        else if (op == OPC_MUL) emit(H_MULC, cbits);
+        else if (op == OPC_SUB) emit(rev ? H_RSUBC : H_SUBC, cbits);
+        else if (rev) emit(H_RDIVC, cbits);
+        else if (fabsf(cf) < kEps) emit(H_LC, 0x3F800000u);                       // protected: 1, whatever acc is
+        else emit(H_MULC, __float_as_uint(mufu_rcp(cf)));
     };
 
     for (int t = 0; t < len; ++t) {
@@ -307,8 +308,8 @@ __global__ void __launch_bounds__(kCompileThreads) k_compile(const CompileParams
             if ((rmask >> a) & 1u) emit(H_SIN + k, 0u);
             else {
                 const uint32_t wa = ttok[a], pb = push_bits();
-                if (is_x(wa)) emit(pb | (col_of(wa) << kColAShift) | (H_LX_SIN + k), 0u);
-                else { emit(pb | H_LC, cst_of(wa)); emit(H_SIN + k, 0u); }
+                if (is_x(wa)) emit(pb + ((col_of(wa) << kColAShift) | (H_LX_SIN + k)), 0u);
+                else { emit(pb + H_LC, cst_of(wa)); emit(H_SIN + k, 0u); }
                 rmask |= 1u << a; ++c;
             }
         } else if (op >= OPC_ADD && op <= OPC_DIV) {
@@ -319,34 +320,34 @@ __global__ void __launch_bounds__(kCompileThreads) k_compile(const CompileParams
             if (ra && rb) {                        // slot[c-2] op acc
                 const int s = c - 2;
                 const uint32_t hs = op == OPC_ADD ? H_ADDS : op == OPC_MUL ? H_MULS : op == OPC_SUB ? H_RSUBS : H_RDIVS;
-                if (s < q.tmem_slots) emit(hs, (uint32_t)(s * kCasesPerLane));
+                if (s < q.tmem_slots) emit(hs, 0u);                                   // pops the tensor-memory slot stack
                 else emit(hs + (H_ADDM - H_ADDS), (uint32_t)((s - q.tmem_slots) * 64));
                 --c;
             } else if (ra) {                       // acc op terminal(b)
                 const uint32_t wb = ttok[b];
                 if (is_x(wb)) emit(op == OPC_ADD ? H_ADDX : op == OPC_MUL ? H_MULX : op == OPC_SUB ? H_SUBX : H_DIVX, col_of(wb));
-                else const_op(op, cst_of(wb), false, 0u);
+                else const_op(op, cst_of(wb), false);
             } else if (rb) {                       // terminal(a) op acc; ADD and MUL commute bit for bit
                 const uint32_t wa = ttok[a];
                 if (is_x(wa)) emit(op == OPC_ADD ? H_ADDX : op == OPC_MUL ? H_MULX : op == OPC_SUB ? H_RSUBX : H_RDIVX, col_of(wa));
-                else const_op(op, cst_of(wa), true, 0u);
+                else const_op(op, cst_of(wa), true);
             } else {                               // a fresh value from two terminals
                 const uint32_t wa = ttok[a], wb = ttok[b], pb = push_bits();
                 if (is_x(wa) && is_x(wb))
-                    emit(pb | (col_of(wa) << kColAShift) | (op == OPC_ADD ? H_LX_ADDX : op == OPC_MUL ? H_LX_MULX : op == OPC_SUB ? H_LX_SUBX : H_LX_DIVX), col_of(wb));
+                    emit(pb + ((col_of(wa) << kColAShift) | (op == OPC_ADD ? H_LX_ADDX : op == OPC_MUL ? H_LX_MULX : op == OPC_SUB ? H_LX_SUBX : H_LX_DIVX)), col_of(wb));
                 else if (is_x(wa)) {               // X[a] op c
-                    const uint32_t cb = cst_of(wb), hi = pb | (col_of(wa) << kColAShift);
-                    if (op == OPC_ADD) emit(hi | H_LX_ADDC, cb);
-                    else if (op == OPC_MUL) emit(hi | H_LX_MULC, cb);
-                    else if (op == OPC_SUB) emit(hi | H_LX_SUBC, cb);
-                    else if (fabsf(__uint_as_float(cb)) < kEps) emit(pb | H_LC, 0x3F800000u);
-                    else emit(hi | H_LX_MULC, __float_as_uint(mufu_rcp(__uint_as_float(cb))));
+                    const uint32_t cb = cst_of(wb), hi = pb + (col_of(wa) << kColAShift);
+                    if (op == OPC_ADD) emit(hi + H_LX_ADDC, cb);
+                    else if (op == OPC_MUL) emit(hi + H_LX_MULC, cb);
+                    else if (op == OPC_SUB) emit(hi + H_LX_SUBC, cb);
+                    else if (fabsf(__uint_as_float(cb)) < kEps) emit(pb + H_LC, 0x3F800000u);
+                    else emit(hi + H_LX_MULC, __float_as_uint(mufu_rcp(__uint_as_float(cb))));
                 } else if (is_x(wb)) {             // c op X[b]
-                    const uint32_t cb = cst_of(wa), hi = pb | (col_of(wb) << kColAShift);
-                    emit(hi | (op == OPC_ADD ? H_LX_ADDC : op == OPC_MUL ? H_LX_MULC : op == OPC_SUB ? H_LX_RSUBC : H_LX_RDIVC), cb);
+                    const uint32_t cb = cst_of(wa), hi = pb + (col_of(wb) << kColAShift);
+                    emit(hi + (op == OPC_ADD ? H_LX_ADDC : op == OPC_MUL ? H_LX_MULC : op == OPC_SUB ? H_LX_RSUBC : H_LX_RDIVC), cb);
                 } else {                           // c op c: acc = c(a), then acc op c(b)
-                    emit(pb | H_LC, cst_of(wa));
-                    const_op(op, cst_of(wb), false, 0u);
+                    emit(pb + H_LC, cst_of(wa));
+                    const_op(op, cst_of(wb), false);
                 }
                 ++c;
             }
@@ -599,7 +600,7 @@ static beagle_status run_prepass(const int32_t* genomes, const int32_t* lengths,
 static int ring_bytes_for(int threads, long long ys_bytes, int smem_optin, size_t* smem_out)
 {
     const int warps = threads / 32;
-    const long long fixed = ((64 + warps * kStagesMax * 8 + 127) & ~127) + ((ys_bytes + 127) & ~127ll);
+    const long long fixed = ((64 + warps * kStagesMax * 8 + 127) & ~127) + ((ys_bytes + 127) & ~127ll) + (long long)kEvalMetaBytes * warps;
     long long ring = ((smem_optin - fixed) / warps) & ~127ll;
     if (ring > (long long)kStagesMax * kStageBytesMax) ring = (long long)kStagesMax * kStageBytesMax;
     *smem_out = (size_t)(fixed + ring * warps);

@@ -12,7 +12,9 @@
 // delivers a variable's 16 cases, or a pushed slot, straight into x[16] (or into acc[16] for a fresh
 // value). Measured on B200 (profiles/): 226 B/clk/SM against 85 B/clk/SM for the same operand fetched
 // with 4 x LDS.128, one issue slot instead of five, and no shared-memory traffic at all.
-// "push acc" is one tcgen05.st executed by the dispatcher when the next micro-op's record asks for it.
+// "push acc" is one tcgen05.st in front of the handler of a fresh value (the P_ entry of that handler); the
+// tensor-memory slots of a warp are a stack, so the interpreter keeps their top (spt) and a pop is one
+// tcgen05.ld at spt - 16.
 //
 // Per-command arithmetic is instruction for instruction that of ops.cuh (same PTX opcodes, same constants),
 // so per-case outputs are bit-identical to the C++ kernel that uses ops.cuh (k_eval_blockwise).
@@ -89,19 +91,37 @@
     "ld.local.v4.f32 {x8, x9, x10, x11}, [ma+32];\n" \
     "ld.local.v4.f32 {x12, x13, x14, x15}, [ma+48];\n"
 
+// "push acc" in front of a fresh value: P_<entry> pushes to the warp's tensor-memory slot stack (spt), M_<entry>
+// to the local-memory slot at byte offset h[20:10]; both fall / branch into the entry itself.
+#define BGI_PUSHT \
+    "tcgen05.st.sync.aligned.32x32b.x16.b32 [spt], {" BGI_R16("a") "};\n" \
+    "tcgen05.wait::st.sync.aligned;\n" \
+    "add.u32 spt, spt, 16;\n"
+#define BGI_PUSHM \
+    "bfe.u32 e, h, 10, 11;\n" \
+    "cvt.u64.u32 ma, e;\n" \
+    "add.u64 ma, ma, mbase;\n" \
+    "st.local.v4.f32 [ma], {a0, a1, a2, a3};\n" \
+    "st.local.v4.f32 [ma+16], {a4, a5, a6, a7};\n" \
+    "st.local.v4.f32 [ma+32], {a8, a9, a10, a11};\n" \
+    "st.local.v4.f32 [ma+48], {a12, a13, a14, a15};\n"
+#define BGI_PUSHES(ENTRY) \
+    "M_" #ENTRY "_%=:\n" BGI_PUSHM "bra.uni L_" #ENTRY "_%=;\n" \
+    "P_" #ENTRY "_%=:\n" BGI_PUSHT
+
 // acc = acc OP x: entry points for a variable (X), a tensor-memory slot (S), a local-memory slot (M) and a
 // fresh first operand (LX_) share one body. J_: x is being addressed by xa; K_: x is already on its way.
 #define BGI_BIN_X(OP, BODY) \
     "L_" #OP "X_%=:\n" "add.u32 xa, o, xb;\n" \
     "J_" #OP "_%=:\n" BGI_LDTM("x", "xa") \
     "K_" #OP "_%=:\n" BGI_NEXT BGI_WAITLD BGI_K16(BODY) BGI_DISPATCH
-#define BGI_ENTRY_S(OP)  "L_" #OP "S_%=:\n" "add.u32 xa, o, sb;\n" "bra.uni J_" #OP "_%=;\n"
+#define BGI_ENTRY_S(OP)  "L_" #OP "S_%=:\n" "sub.u32 spt, spt, 16;\n" "mov.u32 xa, spt;\n" "bra.uni J_" #OP "_%=;\n"
 #define BGI_ENTRY_M(OP)  "L_" #OP "M_%=:\n" BGI_GETM "bra.uni K_" #OP "_%=;\n"
-#define BGI_ENTRY_LXX(OP) "L_LX_" #OP "X_%=:\n" BGI_LXA "add.u32 xa, o, xb;\n" "bra.uni J_" #OP "_%=;\n"
+#define BGI_ENTRY_LXX(OP) BGI_PUSHES(LX_##OP##X) "L_LX_" #OP "X_%=:\n" BGI_LXA "add.u32 xa, o, xb;\n" "bra.uni J_" #OP "_%=;\n"
 // acc = acc OP c, acc = f(acc); LX_ entry: acc = X[colA] first
 #define BGI_BIN_C(OP, BODY) "L_" #OP "C_%=:\n" "mov.b32 cv, o;\n" BGI_NEXT BGI_K16(BODY) BGI_DISPATCH
 #define BGI_UNARY(OP, BODY) "L_" #OP "_%=:\n" BGI_NEXT BGI_K16(BODY) BGI_DISPATCH
-#define BGI_ENTRY_LX(OP)  "L_LX_" #OP "_%=:\n" BGI_LXA BGI_WAITLD "bra.uni L_" #OP "_%=;\n"
+#define BGI_ENTRY_LX(OP)  BGI_PUSHES(LX_##OP) "L_LX_" #OP "_%=:\n" BGI_LXA BGI_WAITLD "bra.uni L_" #OP "_%=;\n"
 
 #define BGI_HANDLERS \
     BGI_UNARY(SIN, BGI_SIN) BGI_UNARY(COS, BGI_COS) BGI_UNARY(LOG, BGI_LOG) BGI_UNARY(SQRT, BGI_SQRT) BGI_UNARY(EXP, BGI_EXP) \
@@ -114,37 +134,22 @@
     BGI_BIN_X(RDIV, BGI_RDIVX) BGI_ENTRY_S(RDIV) BGI_ENTRY_M(RDIV) \
     BGI_BIN_C(ADD, BGI_ADDC) BGI_BIN_C(SUB, BGI_SUBC) BGI_BIN_C(MUL, BGI_MULC) BGI_BIN_C(RSUB, BGI_RSUBC) BGI_BIN_C(RDIV, BGI_RDIVC) \
     BGI_ENTRY_LX(ADDC) BGI_ENTRY_LX(SUBC) BGI_ENTRY_LX(MULC) BGI_ENTRY_LX(RSUBC) BGI_ENTRY_LX(RDIVC) \
-    "L_LX_%=:\n" BGI_LXA BGI_NEXT BGI_WAITLD BGI_DISPATCH \
-    "L_LC_%=:\n" "mov.b32 cv, o;\n" BGI_NEXT BGI_K16(BGI_LC) BGI_DISPATCH
+    BGI_PUSHES(LX) "L_LX_%=:\n" BGI_LXA BGI_NEXT BGI_WAITLD BGI_DISPATCH \
+    BGI_PUSHES(LC) "L_LC_%=:\n" "mov.b32 cv, o;\n" BGI_NEXT BGI_K16(BGI_LC) BGI_DISPATCH
 
-// ---- the dispatcher: optional push of acc (the record's flags), then the one indexed branch ---------------
+// ---- the dispatcher: the one indexed branch ----------------------------------------------------------------
 #define BGI_DISPATCHER \
     "DISP_%=:\n" \
-    "and.b32 e, h, 768;\n" \
-    "setp.ne.u32 pp, e, 0;\n" \
-    "@pp bra.uni PUSH_%=;\n" \
-    "DISP2_%=:\n" \
     "and.b32 hn, h, 255;\n" \
-    "brx.idx.uni hn, TBL_%=;\n" \
-    "PUSH_%=:\n" \
-    "and.b32 e, h, 512;\n" \
-    "setp.ne.u32 pp, e, 0;\n" \
-    "bfe.u32 e, h, 10, 11;\n" \
-    "@pp bra.uni PUSHM_%=;\n" \
-    "add.u32 e, e, sb;\n" \
-    "tcgen05.st.sync.aligned.32x32b.x16.b32 [e], {" BGI_R16("a") "};\n" \
-    "tcgen05.wait::st.sync.aligned;\n" \
-    "bra.uni DISP2_%=;\n" \
-    "PUSHM_%=:\n" \
-    "cvt.u64.u32 ma, e;\n" \
-    "add.u64 ma, ma, mbase;\n" \
-    "st.local.v4.f32 [ma], {a0, a1, a2, a3};\n" \
-    "st.local.v4.f32 [ma+16], {a4, a5, a6, a7};\n" \
-    "st.local.v4.f32 [ma+32], {a8, a9, a10, a11};\n" \
-    "st.local.v4.f32 [ma+48], {a12, a13, a14, a15};\n" \
-    "bra.uni DISP2_%=;\n"
+    "brx.idx.uni hn, TBL_%=;\n"
 
 #define BGI_T(L) "L_" #L "_%=, "
+#define BGI_TP(L) "P_" #L "_%=, "
+#define BGI_TM(L) "M_" #L "_%=, "
+#define BGI_FRESH(T) \
+    T(LX) T(LC) T(LX_SIN) T(LX_COS) T(LX_LOG) T(LX_SQRT) T(LX_EXP) \
+    T(LX_ADDX) T(LX_SUBX) T(LX_MULX) T(LX_DIVX) \
+    T(LX_ADDC) T(LX_SUBC) T(LX_MULC) T(LX_RSUBC) T(LX_RDIVC)
 #define BGI_TABLE \
     "TBL_%=: .branchtargets " \
     BGI_T(END) BGI_T(SIN) BGI_T(COS) BGI_T(LOG) BGI_T(SQRT) BGI_T(EXP) \
@@ -152,10 +157,7 @@
     BGI_T(ADDS) BGI_T(MULS) BGI_T(RSUBS) BGI_T(RDIVS) \
     BGI_T(ADDM) BGI_T(MULM) BGI_T(RSUBM) BGI_T(RDIVM) \
     BGI_T(ADDC) BGI_T(SUBC) BGI_T(MULC) BGI_T(RSUBC) BGI_T(RDIVC) \
-    BGI_T(LX) BGI_T(LC) \
-    BGI_T(LX_SIN) BGI_T(LX_COS) BGI_T(LX_LOG) BGI_T(LX_SQRT) BGI_T(LX_EXP) \
-    BGI_T(LX_ADDX) BGI_T(LX_SUBX) BGI_T(LX_MULX) BGI_T(LX_DIVX) \
-    BGI_T(LX_ADDC) BGI_T(LX_SUBC) BGI_T(LX_MULC) BGI_T(LX_RSUBC) BGI_T(LX_RDIVC) \
+    BGI_FRESH(BGI_T) BGI_FRESH(BGI_TP) BGI_FRESH(BGI_TM) \
     "L_END_%=;\n"
 
 #define BGI_OUT(k) "mov.f32 %" #k ", a" #k ";\n"
@@ -164,14 +166,14 @@
 #define BGI_ASM \
     "{\n" \
     ".reg .f32 a<16>, x<16>, t<16>, q<16>, cv;\n" \
-    ".reg .pred p<16>, pp;\n" \
-    ".reg .b32 h, o, hn, pc, xa, xb, sb, e;\n" \
+    ".reg .pred p<16>;\n" \
+    ".reg .b32 h, o, hn, pc, xa, xb, spt, e;\n" \
     ".reg .b64 ma, mbase;\n" \
     ".local .align 16 .b8 slotmem[1984];\n"      /* kMemSlots * 64 */ \
     BGI_TABLE \
     "mov.u32 pc, %16;\n" \
     "mov.u32 xb, %17;\n" \
-    "mov.u32 sb, %18;\n" \
+    "mov.u32 spt, %18;\n" \
     "mov.u64 mbase, slotmem;\n" \
     "ld.shared.v2.b32 {h, o}, [pc];\n" \
     BGI_DISPATCHER \
@@ -186,7 +188,7 @@
 namespace beagle {
 
 static_assert(kMemSlots * 64 == 1984 && kCasesPerLane == 16, "interp.cuh is written for 16 cases per lane and 31 memory slots");
-static_assert(H_COUNT == 41, "BGI_TABLE lists the handlers in the order of uop.cuh's enum");
+static_assert(H_COUNT == 73, "BGI_TABLE lists the handlers in the order of uop.cuh's enum");
 
 // acc[k] = the program's output on case (pass * 512 + (k/4)*128 + lane*4 + k%4)
 __device__ __forceinline__ void interp_run(uint32_t rec, uint32_t xb, uint32_t sb, float (&acc)[16])

@@ -15,8 +15,8 @@
 //     x  y  DIV      ->  LX_DIVX x, y     acc = X[x] / X[y]          (both terminal: a fresh value)
 //     x  SIN         ->  LX_SIN x         acc = sin X[x]
 //     <A> <B> DIV    ->  RDIVS s          acc = slot[s] / acc        (both computed)
-// and "push acc" is not a micro-op either: it is a flag of the micro-op that starts the next fresh
-// value, executed by the dispatcher on the way into that handler.
+// and "push acc" is not a micro-op either: the micro-op that starts the next fresh value is dispatched to
+// the push entry of its handler (handler number + H_PUSHT or + H_PUSHM).
 // Commands run in the program's own order and every micro-op computes exactly the value the postfix
 // command computes on the same operands with the same per-command function (ops.cuh / interp.cuh), so
 // per-case outputs are bit-identical to a plain stack machine (ADD and MUL commute bit for bit;
@@ -24,13 +24,11 @@
 //
 // Stream layout: uint2 records {h, o}, one per micro-op, one TMA bulk copy per program:
 //     rec[j] = record of micro-op j,  j = 0 .. n-1;   rec[n] = { H_END, 0 };   rec[n+1] = pad
-//   h  [7:0]    handler number (uop.cuh enum)
-//      [8]      push acc to a tensor-memory slot before this micro-op
-//      [9]      push acc to a local-memory slot before this micro-op
-//      [20:10]  where to push: TMEM column offset (slot * 16) or local byte offset (slot * 64)
+//   h  [7:0]    handler number (uop.cuh enum; fresh values: + H_PUSHT / + H_PUSHM when acc is pushed first)
+//      [20:10]  H_PUSHM entries: local byte offset of the slot (slot * 64)
 //      [31:21]  column of the FIRST operand of an LX_ micro-op (a variable: (pass-relative) column)
-//   o           second operand: column of a variable (X-type), column offset of a slot (S-type), byte
-//               offset of a slot in local memory (M-type), fp32 bits of a constant (C-type)
+//   o           second operand: column of a variable (X-type), byte offset of a slot in local memory
+//               (M-type), fp32 bits of a constant (C-type); S-type pops the tensor-memory slot stack
 #pragma once
 #include <stdint.h>
 
@@ -58,10 +56,12 @@ enum : uint32_t {
     H_LX_SIN = 27, H_LX_COS = 28, H_LX_LOG = 29, H_LX_SQRT = 30, H_LX_EXP = 31,
     H_LX_ADDX = 32, H_LX_SUBX = 33, H_LX_MULX = 34, H_LX_DIVX = 35,
     H_LX_ADDC = 36, H_LX_SUBC = 37, H_LX_MULC = 38, H_LX_RSUBC = 39, H_LX_RDIVC = 40,
-    H_COUNT = 41
+    H_FRESH0 = H_LX, H_NFRESH = 16,             // the fresh-value handlers H_LX .. H_LX_RDIVC
+    H_PUSHT = H_NFRESH,                         // + handler: push acc to the tensor-memory slot stack first
+    H_PUSHM = 2 * H_NFRESH,                     // + handler: push acc to the local slot at byte offset h[20:10] first
+    H_COUNT = 41 + 2 * H_NFRESH
 };
 
-constexpr uint32_t kPushTmem = 1u << 8, kPushMem = 1u << 9;
 constexpr int kPushShift = 10, kColAShift = 21;
 
 // meta[i] (one int4 per individual, in evaluation order): x = p (input index), y = record block address
