@@ -234,6 +234,57 @@ __global__ void __launch_bounds__(kScanThreads) k_scatter(
     if (k >= 0) perm[binstart[k] + cnt[k] + r] = (int)p;
 }
 
+// ---- the compiler's decision table ------------------------------------------------------------------------
+// What an operator token emits depends only on (command, is each operand computed, is each terminal operand a
+// variable): 20 + 64 cases. They are tabulated once on the host (make_compile_lut, the rules in words in
+// uop.cuh) so that the per-token walk of k_compile is the same straight-line code for every lane of a warp.
+enum : uint32_t {
+    LUT_OSEL_A = 1u << 8, LUT_OSEL_B = 2u << 8,      // o = the value of operand a | b (a column or a constant)
+    LUT_CSEL_A = 1u << 10, LUT_CSEL_B = 2u << 10,    // first-operand column (h[31:21]) = operand a | b
+    LUT_PUSH = 1u << 12,                             // a fresh value: the handler's push entry if acc is live
+    LUT_DCP = 1u << 13, LUT_DCM = 1u << 14,          // computed entries +1 | -1
+    LUT_SLOT = 1u << 15,                             // pops a slot: local-memory variant beyond S_T
+    LUT_DIVC = 1u << 16,                             // o is a constant divisor: o = rcp(o), or acc = 1 if |o| < eps
+    LUT_DBL = 1u << 17,                              // two records: first acc = c (LC), then this one
+    LUT_EMIT = 1u << 18,
+    LUT_FSEL_A = 1u << 19                            // LUT_DBL: the first record's constant is operand a (else b)
+};
+constexpr int kLutUnary = 0, kLutBinary = 32, kLutNone = 127, kLutSize = 128;
+__device__ uint32_t g_compile_lut[kLutSize];
+
+static void make_compile_lut(uint32_t* lut)
+{
+    for (int i = 0; i < kLutSize; ++i) lut[i] = 0;
+    for (uint32_t kk = 0; kk < 5; ++kk)
+        for (int rb = 0; rb < 2; ++rb)
+            for (int xb = 0; xb < 2; ++xb) {
+                uint32_t e;
+                if (rb) e = LUT_EMIT | (H_SIN + kk);
+                else if (xb) e = LUT_EMIT | LUT_PUSH | LUT_DCP | LUT_CSEL_B | (H_LX_SIN + kk);
+                else e = LUT_EMIT | LUT_DBL | LUT_DCP | (H_SIN + kk);
+                lut[kLutUnary + (kk << 2 | rb << 1 | xb)] = e;
+            }
+    const uint32_t hS[4] = { H_ADDS, H_RSUBS, H_MULS, H_RDIVS };            // j: ADD SUB MUL DIV
+    const uint32_t hX[4] = { H_ADDX, H_SUBX, H_MULX, H_DIVX }, hRX[4] = { H_ADDX, H_RSUBX, H_MULX, H_RDIVX };
+    const uint32_t hC[4] = { H_ADDC, H_SUBC, H_MULC, H_MULC | LUT_DIVC }, hRC[4] = { H_ADDC, H_RSUBC, H_MULC, H_RDIVC };
+    const uint32_t hLXX[4] = { H_LX_ADDX, H_LX_SUBX, H_LX_MULX, H_LX_DIVX };
+    const uint32_t hLXC[4] = { H_LX_ADDC, H_LX_SUBC, H_LX_MULC, H_LX_MULC | LUT_DIVC };
+    const uint32_t hLXRC[4] = { H_LX_ADDC, H_LX_RSUBC, H_LX_MULC, H_LX_RDIVC };
+    for (int j = 0; j < 4; ++j)
+        for (int ra = 0; ra < 2; ++ra) for (int rb = 0; rb < 2; ++rb)
+            for (int xa = 0; xa < 2; ++xa) for (int xb = 0; xb < 2; ++xb) {
+                uint32_t e;
+                if (ra && rb) e = LUT_EMIT | LUT_SLOT | LUT_DCM | hS[j];
+                else if (ra) e = LUT_EMIT | LUT_OSEL_B | (xb ? hX[j] : hC[j]);
+                else if (rb) e = LUT_EMIT | LUT_OSEL_A | (xa ? hRX[j] : hRC[j]);
+                else if (xa && xb) e = LUT_EMIT | LUT_PUSH | LUT_DCP | LUT_CSEL_A | LUT_OSEL_B | hLXX[j];
+                else if (xa) e = LUT_EMIT | LUT_PUSH | LUT_DCP | LUT_CSEL_A | LUT_OSEL_B | hLXC[j];
+                else if (xb) e = LUT_EMIT | LUT_PUSH | LUT_DCP | LUT_CSEL_B | LUT_OSEL_A | hLXRC[j];
+                else e = LUT_EMIT | LUT_DBL | LUT_DCP | LUT_FSEL_A | LUT_OSEL_B | hC[j];
+                lut[kLutBinary + (j << 4 | ra << 3 | rb << 2 | xa << 1 | xb)] = e;
+            }
+}
+
 // ---- a3/a5: the tree compiler ----------------------------------------------------------------------------
 // One thread per individual, in length-sorted order (the threads of a warp run programs of equal
 // length). One walk over the postfix program with an abstract stack whose entries are either a
@@ -249,112 +300,150 @@ struct CompileParams {
     float* fitness; float* outputs; int n_cases; int emit;
 };
 
+// Tokens are not read one by one from global memory: a warp owns 32 consecutive individuals of the sorted
+// order and walks them in chunks of kCompChunk tokens. Per chunk: (1) the 32 x kCompChunk tokens are copied
+// with coalesced loads into shared memory (a CONST token is replaced by its constant in the same sweep, so
+// that the serial walk never waits on a dependent global load), (2) every lane walks its own program from
+// shared memory, table-driven and without data-dependent branches, and appends micro-op records to its
+// shared-memory row, (3) the rows are written out with coalesced stores.
+constexpr int kCompChunk = 32;
+constexpr int kCompTokStride = kCompChunk + 1;        // bank-conflict-free rows
+constexpr int kCompRecStride = kCompChunk + 3;        // a chunk of 32 tokens yields at most 33 records (see k_compile)
+struct CompileSmem {
+    uint32_t tok[32 * kCompTokStride];
+    uint2 rec[32 * kCompRecStride];
+};
+
 __global__ void __launch_bounds__(kCompileThreads) k_compile(const CompileParams q)
 {
-    const int i = blockIdx.x * kCompileThreads + threadIdx.x;
-    if (i >= q.hdr->n_sorted) return;
-    const int p = q.perm[i];
-    const int len = q.lengths[p];
+    extern __shared__ __align__(16) unsigned char csm_raw[];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    uint32_t* lut = reinterpret_cast<uint32_t*>(csm_raw);
+    CompileSmem& sm = reinterpret_cast<CompileSmem*>(csm_raw + kLutSize * 4)[warp];
+    if (threadIdx.x < kLutSize) lut[threadIdx.x] = g_compile_lut[threadIdx.x];
+    __syncthreads();
+    const int n_sorted = q.hdr->n_sorted;
+    const int i0 = (blockIdx.x * (kCompileThreads / 32) + warp) * 32;
+    if (i0 >= n_sorted) return;
+    const int i = i0 + lane;
+    const bool valid = i < n_sorted;
+    const int p = valid ? q.perm[i] : 0;
+    const int len = valid ? q.lengths[p] : 0;
+    const long long toff = valid ? q.off[p] : 0;
     const int bin = BEAGLE_MAX_LEN - len;
     const int stride = uop_stride(len);
-    const long long ua = q.binubase[bin] + (long long)(i - q.binstart[bin]) * stride;
-    const uint32_t* tok = q.genomes + q.off[p];
+    const long long ua = valid ? q.binubase[bin] + (long long)(i - q.binstart[bin]) * stride : 0;
     const bool fits = ua + stride <= q.ucap;
-    const bool wr = q.emit && fits;
-    uint2* out = q.uops + (wr ? ua : 0);
+    const bool wr = valid && q.emit && fits;
+    int maxlen = len;
+#pragma unroll
+    for (int m = 16; m >= 1; m >>= 1) maxlen = max(maxlen, __shfl_xor_sync(0xffffffffu, maxlen, m));
 
-    uint32_t ttok[BEAGLE_MAX_STACK];               // tokens of the unevaluated terminals on the abstract stack
+    uint32_t stk[BEAGLE_MAX_STACK];                // unevaluated terminals: a variable's column or a constant's bits
     uint32_t rmask = 0;                            // bit k: stack entry k is computed
+    uint32_t xmask = 0;                            // bit k: stack entry k is a variable (else a constant)
     int sp = 0, mx = 0, n = 0;
     int c = 0;                                     // computed entries on the stack (the topmost one is acc)
-    bool ok = true;
+    bool ok = valid;
+    uint2* rec = sm.rec + lane * kCompRecStride;
+    const int S_T = q.tmem_slots;
 
-    auto is_x = [](uint32_t w) { return tok_op(w) == OPC_LOAD; };
-    auto col_of = [](uint32_t w) -> uint32_t { return tok_arg(w) * (uint32_t)kCasesPerLane; };
-    auto cst_of = [&](uint32_t w) -> uint32_t { return __float_as_uint(__ldg(q.consts + tok_arg(w))); };
-    auto emit = [&](uint32_t h, uint32_t o) { if (wr) out[n] = make_uint2(h, o); ++n; };
-    // a micro-op that starts a fresh value while acc is live goes to the push entry of its handler:
-    // slot c-1 is on the tensor-memory slot stack while c-1 < S_T, in local memory beyond
-    auto push_bits = [&]() -> uint32_t {
-        if (c == 0) return 0u;
-        const int s = c - 1;
-        return s < q.tmem_slots ? (uint32_t)H_PUSHT : ((uint32_t)H_PUSHM + ((uint32_t)((s - q.tmem_slots) * 64) << kPushShift));
-    };
-    // acc = acc op c (rev: c op acc); x / c is x * rcp(c) with the division handler's own rcp
-    auto const_op = [&](uint32_t op, uint32_t cbits, bool rev) {
-        const float cf = __uint_as_float(cbits);
-        if (op == OPC_ADD) emit(H_ADDC, cbits);
-        else if (op == OPC_MUL) emit(H_MULC, cbits);
-        else if (op == OPC_SUB) emit(rev ? H_RSUBC : H_SUBC, cbits);
-        else if (rev) emit(H_RDIVC, cbits);
-        else if (fabsf(cf) < kEps) emit(H_LC, 0x3F800000u);                       // protected: 1, whatever acc is
-        else emit(H_MULC, __float_as_uint(mufu_rcp(cf)));
-    };
-
-    for (int t = 0; t < len; ++t) {
-        const uint32_t w = __ldg(tok + t);
-        const uint32_t op = tok_op(w), arg = tok_arg(w);
-        if (op == OPC_CONST || op == OPC_LOAD) {
-            ok &= (op == OPC_CONST) ? ((long long)arg < q.n_consts) : ((int)arg < q.d);
-            ok &= (sp < BEAGLE_MAX_STACK);
-            if (!ok) break;
-            ttok[sp] = w; rmask &= ~(1u << sp); ++sp;
-            mx = max(mx, sp);
-        } else if (op >= OPC_SIN && op <= OPC_EXP) {
-            ok &= (arg == 0) & (sp >= 1);
-            if (!ok) break;
-            const int a = sp - 1;
-            const uint32_t k = op - OPC_SIN;
-            if ((rmask >> a) & 1u) emit(H_SIN + k, 0u);
-            else {
-                const uint32_t wa = ttok[a], pb = push_bits();
-                if (is_x(wa)) emit(pb + ((col_of(wa) << kColAShift) | (H_LX_SIN + k)), 0u);
-                else { emit(pb + H_LC, cst_of(wa)); emit(H_SIN + k, 0u); }
-                rmask |= 1u << a; ++c;
+    for (int c0 = 0; c0 < maxlen; c0 += kCompChunk) {
+        // (1) stage the chunk: program qi's tokens c0 .. c0+31, one coalesced load each, eight programs in flight.
+        // A CONST token with a valid index is replaced by its constant; cmask (bit t) remembers which ones.
+        uint32_t cmask = 0;
+        for (int q0 = 0; q0 < 32; q0 += 8) {
+            uint32_t w8[8]; bool in8[8];
+#pragma unroll
+            for (int u = 0; u < 8; ++u) {
+                const int lq = __shfl_sync(0xffffffffu, len, q0 + u);
+                const long long oq = __shfl_sync(0xffffffffu, toff, q0 + u);
+                in8[u] = c0 + lane < lq;
+                w8[u] = in8[u] ? __ldg(q.genomes + oq + c0 + lane) : 0u;
             }
-        } else if (op >= OPC_ADD && op <= OPC_DIV) {
-            ok &= (arg == 0) & (sp >= 2);
-            if (!ok) break;
-            const int a = sp - 2, b = sp - 1;
-            const bool ra = (rmask >> a) & 1u, rb = (rmask >> b) & 1u;
-            if (ra && rb) {                        // slot[c-2] op acc
-                const int s = c - 2;
-                const uint32_t hs = op == OPC_ADD ? H_ADDS : op == OPC_MUL ? H_MULS : op == OPC_SUB ? H_RSUBS : H_RDIVS;
-                if (s < q.tmem_slots) emit(hs, 0u);                                   // pops the tensor-memory slot stack
-                else emit(hs + (H_ADDM - H_ADDS), (uint32_t)((s - q.tmem_slots) * 64));
-                --c;
-            } else if (ra) {                       // acc op terminal(b)
-                const uint32_t wb = ttok[b];
-                if (is_x(wb)) emit(op == OPC_ADD ? H_ADDX : op == OPC_MUL ? H_MULX : op == OPC_SUB ? H_SUBX : H_DIVX, col_of(wb));
-                else const_op(op, cst_of(wb), false);
-            } else if (rb) {                       // terminal(a) op acc; ADD and MUL commute bit for bit
-                const uint32_t wa = ttok[a];
-                if (is_x(wa)) emit(op == OPC_ADD ? H_ADDX : op == OPC_MUL ? H_MULX : op == OPC_SUB ? H_RSUBX : H_RDIVX, col_of(wa));
-                else const_op(op, cst_of(wa), true);
-            } else {                               // a fresh value from two terminals
-                const uint32_t wa = ttok[a], wb = ttok[b], pb = push_bits();
-                if (is_x(wa) && is_x(wb))
-                    emit(pb + ((col_of(wa) << kColAShift) | (op == OPC_ADD ? H_LX_ADDX : op == OPC_MUL ? H_LX_MULX : op == OPC_SUB ? H_LX_SUBX : H_LX_DIVX)), col_of(wb));
-                else if (is_x(wa)) {               // X[a] op c
-                    const uint32_t cb = cst_of(wb), hi = pb + (col_of(wa) << kColAShift);
-                    if (op == OPC_ADD) emit(hi + H_LX_ADDC, cb);
-                    else if (op == OPC_MUL) emit(hi + H_LX_MULC, cb);
-                    else if (op == OPC_SUB) emit(hi + H_LX_SUBC, cb);
-                    else if (fabsf(__uint_as_float(cb)) < kEps) emit(pb + H_LC, 0x3F800000u);
-                    else emit(hi + H_LX_MULC, __float_as_uint(mufu_rcp(__uint_as_float(cb))));
-                } else if (is_x(wb)) {             // c op X[b]
-                    const uint32_t cb = cst_of(wa), hi = pb + (col_of(wb) << kColAShift);
-                    emit(hi + (op == OPC_ADD ? H_LX_ADDC : op == OPC_MUL ? H_LX_MULC : op == OPC_SUB ? H_LX_RSUBC : H_LX_RDIVC), cb);
-                } else {                           // c op c: acc = c(a), then acc op c(b)
-                    emit(pb + H_LC, cst_of(wa));
-                    const_op(op, cst_of(wb), false);
-                }
-                ++c;
+#pragma unroll
+            for (int u = 0; u < 8; ++u) {
+                const bool isc = in8[u] && tok_op(w8[u]) == OPC_CONST && (long long)tok_arg(w8[u]) < q.n_consts;
+                if (isc) w8[u] = __float_as_uint(__ldg(q.consts + tok_arg(w8[u])));
+                const uint32_t m = __ballot_sync(0xffffffffu, isc);
+                if (lane == q0 + u) cmask = m;
             }
-            rmask |= 1u << a;
-            --sp;
-        } else { ok = false; break; }
+#pragma unroll
+            for (int u = 0; u < 8; ++u)
+                if (in8[u]) sm.tok[(q0 + u) * kCompTokStride + lane] = w8[u];
+        }
+        __syncwarp();
+        // (2) the serial walk, one program per lane; the same instructions for every lane
+        int k = 0;                                 // records of this chunk
+        const int tend = len - c0;                 // this lane's tokens in the chunk (may be <= 0 or > 32)
+        const int tmax = min(kCompChunk, maxlen - c0);
+        for (int t = 0; t < tmax; ++t) {
+            const bool live = ok && t < tend;
+            const uint32_t w = sm.tok[lane * kCompTokStride + t];
+            const bool isc = (cmask >> t) & 1u;
+            const uint32_t op = isc ? (uint32_t)OPC_CONST : tok_op(w), arg = tok_arg(w);
+            const bool isT = (op - OPC_CONST) < 2u, isB = (op - OPC_ADD) < 4u, isU = (op - OPC_SIN) < 5u;
+            const int ai = (sp - 2) & 31, bi = (sp - 1) & 31;
+            const uint32_t va = stk[ai], vb = stk[bi];
+            const uint32_t ra = (rmask >> ai) & 1u, rb = (rmask >> bi) & 1u, xa = (xmask >> ai) & 1u, xb = (xmask >> bi) & 1u;
+            const uint32_t key = isB ? (uint32_t)kLutBinary + ((op - OPC_ADD) << 4 | ra << 3 | rb << 2 | xa << 1 | xb)
+                               : isU ? (uint32_t)kLutUnary + ((op - OPC_SIN) << 2 | rb << 1 | xb) : (uint32_t)kLutNone;
+            const uint32_t e = lut[key];
+            // well-formedness (D3); a CONST token that was not replaced has an index out of range
+            const bool okT = (isc || (op == OPC_LOAD && (int)arg < q.d)) && sp < BEAGLE_MAX_STACK;
+            const bool okO = (arg == 0) && (sp >= (isB ? 2 : 1));
+            const bool good = isT ? okT : ((isB || isU) && okO);
+            ok = ok && (good || t >= tend);
+            const bool run = live && good;
+            // the record
+            const int s1 = c - 1;
+            const uint32_t pb = (c == 0 || !(e & (LUT_PUSH | LUT_DBL))) ? 0u
+                              : (s1 < S_T ? (uint32_t)H_PUSHT : (uint32_t)H_PUSHM + ((uint32_t)((s1 - S_T) * 64) << kPushShift));
+            uint32_t o = (e & LUT_OSEL_A) ? va : (e & LUT_OSEL_B) ? vb : 0u;
+            const uint32_t colA = (e & LUT_CSEL_A) ? va : (e & LUT_CSEL_B) ? vb : 0u;
+            uint32_t h = (e & 0xFFu) + (colA << kColAShift) + ((e & LUT_PUSH) ? pb : 0u);
+            if (e & LUT_SLOT) { const int s2 = c - 2; if (s2 >= S_T) { h += H_ADDM - H_ADDS; o = (uint32_t)((s2 - S_T) * 64); } }
+            if (e & LUT_DIVC) {                    // x / c = x * rcp(c) with the division handler's own rcp; protected: 1
+                const float cf = __uint_as_float(o);
+                const bool tiny = fabsf(cf) < kEps;
+                o = tiny ? 0x3F800000u : __float_as_uint(mufu_rcp(cf));
+                h = tiny ? ((e & LUT_PUSH) ? pb : 0u) + (uint32_t)H_LC : h;
+            }
+            if (run && (e & LUT_DBL)) {            // rare: a constant has to become acc first
+                if (k < kCompRecStride) rec[k] = make_uint2(pb + H_LC, (e & LUT_FSEL_A) ? va : vb);
+                ++k;
+            }
+            if (run && (e & LUT_EMIT)) {
+                if (k < kCompRecStride) rec[k] = make_uint2(h, o);
+                ++k;
+            }
+            // the abstract stack
+            if (run) {
+                if (isT) {
+                    const bool isx = !isc;
+                    stk[sp & 31] = isx ? arg * (uint32_t)kCasesPerLane : w;
+                    xmask = isx ? (xmask | (1u << sp)) : (xmask & ~(1u << sp));
+                    rmask &= ~(1u << sp);
+                    ++sp; mx = max(mx, sp);
+                } else if (isU) rmask |= 1u << bi;
+                else { rmask |= 1u << ai; --sp; }
+                c += (e & LUT_DCP) ? 1 : (e & LUT_DCM) ? -1 : 0;
+            }
+        }
+        __syncwarp();
+        // (3) write the chunk's records out, one program at a time, coalesced. A chunk of 32 tokens yields at most
+        // 33 records: a token emits two only when it consumes a constant that emitted nothing, and at most one
+        // such constant is left over from earlier chunks at the top of the stack.
+        for (int qi = 0; qi < 32; ++qi) {
+            const int kq = __shfl_sync(0xffffffffu, wr ? k : 0, qi);
+            if (kq == 0) continue;
+            const long long bq = __shfl_sync(0xffffffffu, ua + n, qi);
+            for (int j = lane; j < kq; j += 32) q.uops[bq + j] = sm.rec[qi * kCompRecStride + j];
+        }
+        n += k;
+        __syncwarp();
     }
+    if (!valid) return;
     ok &= (sp >= 1);
     if (!ok) {
         q.depth[p] = 0;
@@ -371,9 +460,11 @@ __global__ void __launch_bounds__(kCompileThreads) k_compile(const CompileParams
         q.meta[i] = make_int4(p, 0, 0, len);
         return;
     }
+    uint2* out = q.uops + ua;
     if (!((rmask >> (sp - 1)) & 1u)) {             // the result is a bare terminal
-        const uint32_t wa = ttok[sp - 1];
-        if (is_x(wa)) emit((col_of(wa) << kColAShift) | H_LX, 0u); else emit(H_LC, cst_of(wa));
+        const uint32_t va = stk[sp - 1];
+        out[n] = ((xmask >> (sp - 1)) & 1u) ? make_uint2((va << kColAShift) | H_LX, 0u) : make_uint2(H_LC, va);
+        ++n;
     }
     out[n] = make_uint2(H_END, 0u);
     out[n + 1] = make_uint2(H_END, 0u);
@@ -483,6 +574,8 @@ static beagle_status init_once()
     w.inited = true;
     if (!w.device_ok) return BEAGLE_ERR_UNSUPPORTED;
     CU(cudaFuncSetAttribute(k_eval, cudaFuncAttributeMaxDynamicSharedMemorySize, w.smem_optin));
+    CU(cudaFuncSetAttribute(k_compile, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(kLutSize * 4 + sizeof(CompileSmem) * (kCompileThreads / 32))));
+    { uint32_t lut[kLutSize]; make_compile_lut(lut); CU(cudaMemcpyToSymbol(g_compile_lut, lut, sizeof(lut))); }
     CU(cudaMalloc(&w.bins, sizeof(int) * kNumBins));
     CU(cudaMalloc(&w.cursor, sizeof(int) * kNumBins));
     CU(cudaMemset(w.bins, 0, sizeof(int) * kNumBins));
@@ -590,7 +683,7 @@ static beagle_status run_prepass(const int32_t* genomes, const int32_t* lengths,
         q.consts = consts; q.n_consts = n_consts; q.d = d; q.tmem_slots = st_slots; q.binstart = w.binstart; q.binubase = w.binubase;
         q.hdr = w.hdr; q.uops = w.uops; q.ucap = w.cap_U; q.meta = w.meta; q.depth = w.depth;
         q.slow_list = w.slow_list; q.fitness = fitness; q.outputs = outputs; q.n_cases = N; q.emit = emit ? 1 : 0;
-        k_compile<<<(unsigned)((P + kCompileThreads - 1) / kCompileThreads), kCompileThreads, 0, st>>>(q);
+        k_compile<<<(unsigned)((P + kCompileThreads - 1) / kCompileThreads), kCompileThreads, kLutSize * 4 + sizeof(CompileSmem) * (kCompileThreads / 32), st>>>(q);
         ++g_launches;
     }
     CU(cudaGetLastError());
