@@ -300,26 +300,16 @@ struct CompileParams {
     float* fitness; float* outputs; int n_cases; int emit;
 };
 
-// Tokens are not read one by one from global memory: a warp owns 32 consecutive individuals of the sorted
-// order and walks them in chunks of kCompChunk tokens. Per chunk: (1) the 32 x kCompChunk tokens are copied
-// with coalesced loads into shared memory (a CONST token is replaced by its constant in the same sweep, so
-// that the serial walk never waits on a dependent global load), (2) every lane walks its own program from
-// shared memory, table-driven and without data-dependent branches, and appends micro-op records to its
-// shared-memory row, (3) the rows are written out with coalesced stores.
-constexpr int kCompChunk = 32;
-constexpr int kCompTokStride = kCompChunk + 1;        // bank-conflict-free rows
-constexpr int kCompRecStride = kCompChunk + 3;        // a chunk of 32 tokens yields at most 33 records (see k_compile)
-struct CompileSmem {
-    uint32_t tok[32 * kCompTokStride];
-    uint2 rec[32 * kCompRecStride];
-};
+// A warp owns 32 consecutive individuals of the sorted order (equal or nearly equal lengths), one per lane.
+// Every lane walks its own program eight tokens at a time: the eight tokens, then the constants they name,
+// are fetched by two batches of independent loads (the 128-byte line a lane reads serves its next 32 tokens
+// from L1), and the walk itself is table-driven, the same straight-line code for every lane.
+constexpr int kCompBatch = 8;
 
 __global__ void __launch_bounds__(kCompileThreads) k_compile(const CompileParams q)
 {
-    extern __shared__ __align__(16) unsigned char csm_raw[];
+    __shared__ uint32_t lut[kLutSize];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    uint32_t* lut = reinterpret_cast<uint32_t*>(csm_raw);
-    CompileSmem& sm = reinterpret_cast<CompileSmem*>(csm_raw + kLutSize * 4)[warp];
     if (threadIdx.x < kLutSize) lut[threadIdx.x] = g_compile_lut[threadIdx.x];
     __syncthreads();
     const int n_sorted = q.hdr->n_sorted;
@@ -345,41 +335,26 @@ __global__ void __launch_bounds__(kCompileThreads) k_compile(const CompileParams
     int sp = 0, mx = 0, n = 0;
     int c = 0;                                     // computed entries on the stack (the topmost one is acc)
     bool ok = valid;
-    uint2* rec = sm.rec + lane * kCompRecStride;
     const int S_T = q.tmem_slots;
+    const uint32_t* gtok = q.genomes + toff;
+    uint2* out = q.uops + ua;
 
-    for (int c0 = 0; c0 < maxlen; c0 += kCompChunk) {
-        // (1) stage the chunk: program qi's tokens c0 .. c0+31, one coalesced load each, eight programs in flight.
-        // A CONST token with a valid index is replaced by its constant; cmask (bit t) remembers which ones.
-        uint32_t cmask = 0;
-        for (int q0 = 0; q0 < 32; q0 += 8) {
-            uint32_t w8[8]; bool in8[8];
+    for (int c0 = 0; c0 < maxlen; c0 += kCompBatch) {
+        uint32_t w8[kCompBatch];
+        uint32_t cmask = 0;                        // bit u: token u was a CONST with a valid index, replaced by its constant
 #pragma unroll
-            for (int u = 0; u < 8; ++u) {
-                const int lq = __shfl_sync(0xffffffffu, len, q0 + u);
-                const long long oq = __shfl_sync(0xffffffffu, toff, q0 + u);
-                in8[u] = c0 + lane < lq;
-                w8[u] = in8[u] ? __ldg(q.genomes + oq + c0 + lane) : 0u;
+        for (int u = 0; u < kCompBatch; ++u) w8[u] = (c0 + u < len) ? __ldg(gtok + c0 + u) : 0u;
+#pragma unroll
+        for (int u = 0; u < kCompBatch; ++u)
+            if (tok_op(w8[u]) == OPC_CONST && (long long)tok_arg(w8[u]) < q.n_consts) {
+                w8[u] = __float_as_uint(__ldg(q.consts + tok_arg(w8[u])));
+                cmask |= 1u << u;
             }
+        const int tend = len - c0;                 // this lane's tokens in the batch (may be <= 0 or > 8)
 #pragma unroll
-            for (int u = 0; u < 8; ++u) {
-                const bool isc = in8[u] && tok_op(w8[u]) == OPC_CONST && (long long)tok_arg(w8[u]) < q.n_consts;
-                if (isc) w8[u] = __float_as_uint(__ldg(q.consts + tok_arg(w8[u])));
-                const uint32_t m = __ballot_sync(0xffffffffu, isc);
-                if (lane == q0 + u) cmask = m;
-            }
-#pragma unroll
-            for (int u = 0; u < 8; ++u)
-                if (in8[u]) sm.tok[(q0 + u) * kCompTokStride + lane] = w8[u];
-        }
-        __syncwarp();
-        // (2) the serial walk, one program per lane; the same instructions for every lane
-        int k = 0;                                 // records of this chunk
-        const int tend = len - c0;                 // this lane's tokens in the chunk (may be <= 0 or > 32)
-        const int tmax = min(kCompChunk, maxlen - c0);
-        for (int t = 0; t < tmax; ++t) {
+        for (int t = 0; t < kCompBatch; ++t) {
             const bool live = ok && t < tend;
-            const uint32_t w = sm.tok[lane * kCompTokStride + t];
+            const uint32_t w = w8[t];
             const bool isc = (cmask >> t) & 1u;
             const uint32_t op = isc ? (uint32_t)OPC_CONST : tok_op(w), arg = tok_arg(w);
             const bool isT = (op - OPC_CONST) < 2u, isB = (op - OPC_ADD) < 4u, isU = (op - OPC_SIN) < 5u;
@@ -410,12 +385,12 @@ __global__ void __launch_bounds__(kCompileThreads) k_compile(const CompileParams
                 h = tiny ? ((e & LUT_PUSH) ? pb : 0u) + (uint32_t)H_LC : h;
             }
             if (run && (e & LUT_DBL)) {            // rare: a constant has to become acc first
-                if (k < kCompRecStride) rec[k] = make_uint2(pb + H_LC, (e & LUT_FSEL_A) ? va : vb);
-                ++k;
+                if (wr) out[n] = make_uint2(pb + H_LC, (e & LUT_FSEL_A) ? va : vb);
+                ++n;
             }
             if (run && (e & LUT_EMIT)) {
-                if (k < kCompRecStride) rec[k] = make_uint2(h, o);
-                ++k;
+                if (wr) out[n] = make_uint2(h, o);
+                ++n;
             }
             // the abstract stack
             if (run) {
@@ -430,18 +405,6 @@ __global__ void __launch_bounds__(kCompileThreads) k_compile(const CompileParams
                 c += (e & LUT_DCP) ? 1 : (e & LUT_DCM) ? -1 : 0;
             }
         }
-        __syncwarp();
-        // (3) write the chunk's records out, one program at a time, coalesced. A chunk of 32 tokens yields at most
-        // 33 records: a token emits two only when it consumes a constant that emitted nothing, and at most one
-        // such constant is left over from earlier chunks at the top of the stack.
-        for (int qi = 0; qi < 32; ++qi) {
-            const int kq = __shfl_sync(0xffffffffu, wr ? k : 0, qi);
-            if (kq == 0) continue;
-            const long long bq = __shfl_sync(0xffffffffu, ua + n, qi);
-            for (int j = lane; j < kq; j += 32) q.uops[bq + j] = sm.rec[qi * kCompRecStride + j];
-        }
-        n += k;
-        __syncwarp();
     }
     if (!valid) return;
     ok &= (sp >= 1);
@@ -460,7 +423,6 @@ __global__ void __launch_bounds__(kCompileThreads) k_compile(const CompileParams
         q.meta[i] = make_int4(p, 0, 0, len);
         return;
     }
-    uint2* out = q.uops + ua;
     if (!((rmask >> (sp - 1)) & 1u)) {             // the result is a bare terminal
         const uint32_t va = stk[sp - 1];
         out[n] = ((xmask >> (sp - 1)) & 1u) ? make_uint2((va << kColAShift) | H_LX, 0u) : make_uint2(H_LC, va);
@@ -574,7 +536,6 @@ static beagle_status init_once()
     w.inited = true;
     if (!w.device_ok) return BEAGLE_ERR_UNSUPPORTED;
     CU(cudaFuncSetAttribute(k_eval, cudaFuncAttributeMaxDynamicSharedMemorySize, w.smem_optin));
-    CU(cudaFuncSetAttribute(k_compile, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(kLutSize * 4 + sizeof(CompileSmem) * (kCompileThreads / 32))));
     { uint32_t lut[kLutSize]; make_compile_lut(lut); CU(cudaMemcpyToSymbol(g_compile_lut, lut, sizeof(lut))); }
     CU(cudaMalloc(&w.bins, sizeof(int) * kNumBins));
     CU(cudaMalloc(&w.cursor, sizeof(int) * kNumBins));
@@ -683,7 +644,7 @@ static beagle_status run_prepass(const int32_t* genomes, const int32_t* lengths,
         q.consts = consts; q.n_consts = n_consts; q.d = d; q.tmem_slots = st_slots; q.binstart = w.binstart; q.binubase = w.binubase;
         q.hdr = w.hdr; q.uops = w.uops; q.ucap = w.cap_U; q.meta = w.meta; q.depth = w.depth;
         q.slow_list = w.slow_list; q.fitness = fitness; q.outputs = outputs; q.n_cases = N; q.emit = emit ? 1 : 0;
-        k_compile<<<(unsigned)((P + kCompileThreads - 1) / kCompileThreads), kCompileThreads, kLutSize * 4 + sizeof(CompileSmem) * (kCompileThreads / 32), st>>>(q);
+        k_compile<<<(unsigned)((P + kCompileThreads - 1) / kCompileThreads), kCompileThreads, 0, st>>>(q);
         ++g_launches;
     }
     CU(cudaGetLastError());
