@@ -329,53 +329,65 @@ __global__ void __launch_bounds__(kCompileThreads) k_compile(const CompileParams
 #pragma unroll
     for (int m = 16; m >= 1; m >>= 1) maxlen = max(maxlen, __shfl_xor_sync(0xffffffffu, maxlen, m));
 
-    uint32_t stk[BEAGLE_MAX_STACK];                // unevaluated terminals: a variable's column or a constant's bits
-    uint32_t rmask = 0;                            // bit k: stack entry k is computed
-    uint32_t xmask = 0;                            // bit k: stack entry k is a variable (else a constant)
-    int sp = 0, mx = 0, n = 0;
+    // The abstract stack. rmask / xmask are shift registers with the top of the stack at bit 0 (bit k: the
+    // entry k below the top is computed / is a variable, else a constant); t0, t1 are the values of the two
+    // topmost entries (a variable's column or a constant's bits), the deeper ones wait in stk[].
+    uint32_t stk[BEAGLE_MAX_STACK];
+    uint32_t rmask = 0, xmask = 0, t0 = 0, t1 = 0;
+    int sp = 0, mx = 0;
     int c = 0;                                     // computed entries on the stack (the topmost one is acc)
     bool ok = valid;
     const int S_T = q.tmem_slots;
     const uint32_t* gtok = q.genomes + toff;
-    uint2* out = q.uops + ua;
+    uint2* po = q.uops + ua;                       // where the next record goes
+    uint2* const po0 = po;
 
-    for (int c0 = 0; c0 < maxlen; c0 += kCompBatch) {
-        uint32_t w8[kCompBatch];
-        uint32_t cmask = 0;                        // bit u: token u was a CONST with a valid index, replaced by its constant
+    auto load_batch = [&](int c0, uint32_t (&w)[kCompBatch]) {
 #pragma unroll
-        for (int u = 0; u < kCompBatch; ++u) w8[u] = (c0 + u < len) ? __ldg(gtok + c0 + u) : 0u;
+        for (int u = 0; u < kCompBatch; ++u) w[u] = (c0 + u < len) ? __ldg(gtok + c0 + u) : 0u;
+    };
+    // a CONST token with a valid index is replaced by its constant; the mask (bit u) remembers which ones
+    auto resolve = [&](uint32_t (&w)[kCompBatch]) -> uint32_t {
+        uint32_t cm = 0;
 #pragma unroll
         for (int u = 0; u < kCompBatch; ++u)
-            if (tok_op(w8[u]) == OPC_CONST && (long long)tok_arg(w8[u]) < q.n_consts) {
-                w8[u] = __float_as_uint(__ldg(q.consts + tok_arg(w8[u])));
-                cmask |= 1u << u;
+            if (tok_op(w[u]) == OPC_CONST && (long long)tok_arg(w[u]) < q.n_consts) {
+                w[u] = __float_as_uint(__ldg(q.consts + tok_arg(w[u])));
+                cm |= 1u << u;
             }
+        return cm;
+    };
+    // two batches ahead: tokens of batch i+2 and constants of batch i+1 are in flight while batch i is walked
+    uint32_t wA[kCompBatch], wB[kCompBatch], wC[kCompBatch];
+    load_batch(0, wA);
+    load_batch(kCompBatch, wB);
+    uint32_t cmA = resolve(wA), cmB = 0;
+
+    for (int c0 = 0; c0 < maxlen; c0 += kCompBatch) {
+        load_batch(c0 + 2 * kCompBatch, wC);
+        cmB = resolve(wB);
         const int tend = len - c0;                 // this lane's tokens in the batch (may be <= 0 or > 8)
 #pragma unroll
         for (int t = 0; t < kCompBatch; ++t) {
             const bool live = ok && t < tend;
-            const uint32_t w = w8[t];
-            const bool isc = (cmask >> t) & 1u;
+            const uint32_t w = wA[t];
+            const bool isc = (cmA >> t) & 1u;
             const uint32_t op = isc ? (uint32_t)OPC_CONST : tok_op(w), arg = tok_arg(w);
             const bool isT = (op - OPC_CONST) < 2u, isB = (op - OPC_ADD) < 4u, isU = (op - OPC_SIN) < 5u;
-            const int ai = (sp - 2) & 31, bi = (sp - 1) & 31;
-            const uint32_t va = stk[ai], vb = stk[bi];
-            const uint32_t ra = (rmask >> ai) & 1u, rb = (rmask >> bi) & 1u, xa = (xmask >> ai) & 1u, xb = (xmask >> bi) & 1u;
-            const uint32_t key = isB ? (uint32_t)kLutBinary + ((op - OPC_ADD) << 4 | ra << 3 | rb << 2 | xa << 1 | xb)
-                               : isU ? (uint32_t)kLutUnary + ((op - OPC_SIN) << 2 | rb << 1 | xb) : (uint32_t)kLutNone;
+            const uint32_t key = isB ? (uint32_t)kLutBinary + ((op - OPC_ADD) << 4) + ((rmask & 3u) << 2 | (xmask & 3u))
+                               : isU ? (uint32_t)kLutUnary + ((op - OPC_SIN) << 2) + ((rmask & 1u) << 1 | (xmask & 1u)) : (uint32_t)kLutNone;
             const uint32_t e = lut[key];
             // well-formedness (D3); a CONST token that was not replaced has an index out of range
-            const bool okT = (isc || (op == OPC_LOAD && (int)arg < q.d)) && sp < BEAGLE_MAX_STACK;
-            const bool okO = (arg == 0) && (sp >= (isB ? 2 : 1));
-            const bool good = isT ? okT : ((isB || isU) && okO);
+            const bool good = isT ? ((isc || (op == OPC_LOAD && (int)arg < q.d)) && sp < BEAGLE_MAX_STACK)
+                                  : ((isB || isU) && arg == 0 && sp >= (isB ? 2 : 1));
             ok = ok && (good || t >= tend);
             const bool run = live && good;
-            // the record
+            // the record (operand a = second from the top = t1, operand b = top = t0)
             const int s1 = c - 1;
             const uint32_t pb = (c == 0 || !(e & (LUT_PUSH | LUT_DBL))) ? 0u
                               : (s1 < S_T ? (uint32_t)H_PUSHT : (uint32_t)H_PUSHM + ((uint32_t)((s1 - S_T) * 64) << kPushShift));
-            uint32_t o = (e & LUT_OSEL_A) ? va : (e & LUT_OSEL_B) ? vb : 0u;
-            const uint32_t colA = (e & LUT_CSEL_A) ? va : (e & LUT_CSEL_B) ? vb : 0u;
+            uint32_t o = (e & LUT_OSEL_A) ? t1 : (e & LUT_OSEL_B) ? t0 : 0u;
+            const uint32_t colA = (e & LUT_CSEL_A) ? t1 : (e & LUT_CSEL_B) ? t0 : 0u;
             uint32_t h = (e & 0xFFu) + (colA << kColAShift) + ((e & LUT_PUSH) ? pb : 0u);
             if (e & LUT_SLOT) { const int s2 = c - 2; if (s2 >= S_T) { h += H_ADDM - H_ADDS; o = (uint32_t)((s2 - S_T) * 64); } }
             if (e & LUT_DIVC) {                    // x / c = x * rcp(c) with the division handler's own rcp; protected: 1
@@ -385,27 +397,30 @@ __global__ void __launch_bounds__(kCompileThreads) k_compile(const CompileParams
                 h = tiny ? ((e & LUT_PUSH) ? pb : 0u) + (uint32_t)H_LC : h;
             }
             if (run && (e & LUT_DBL)) {            // rare: a constant has to become acc first
-                if (wr) out[n] = make_uint2(pb + H_LC, (e & LUT_FSEL_A) ? va : vb);
-                ++n;
+                if (wr) *po = make_uint2(pb + H_LC, (e & LUT_FSEL_A) ? t1 : t0);
+                ++po;
             }
-            if (run && (e & LUT_EMIT)) {
-                if (wr) out[n] = make_uint2(h, o);
-                ++n;
-            }
-            // the abstract stack
-            if (run) {
-                if (isT) {
-                    const bool isx = !isc;
-                    stk[sp & 31] = isx ? arg * (uint32_t)kCasesPerLane : w;
-                    xmask = isx ? (xmask | (1u << sp)) : (xmask & ~(1u << sp));
-                    rmask &= ~(1u << sp);
-                    ++sp; mx = max(mx, sp);
-                } else if (isU) rmask |= 1u << bi;
-                else { rmask |= 1u << ai; --sp; }
-                c += (e & LUT_DCP) ? 1 : (e & LUT_DCM) ? -1 : 0;
-            }
+            const bool em = run && (e & LUT_EMIT);
+            if (wr && em) *po = make_uint2(h, o);
+            po += em ? 1 : 0;
+            // the abstract stack, without branches
+            const bool pushT = run && isT, popB = run && isB, unU = run && isU;
+            const uint32_t val = isc ? w : arg * (uint32_t)kCasesPerLane;
+            if (pushT) stk[sp & 31] = val;
+            const uint32_t deeper = stk[(sp - 3) & 31];
+            t1 = pushT ? t0 : popB ? deeper : t1;
+            t0 = pushT ? val : t0;
+            rmask = pushT ? rmask << 1 : popB ? (rmask >> 1) | 1u : unU ? rmask | 1u : rmask;
+            xmask = pushT ? (xmask << 1) | (isc ? 0u : 1u) : popB ? xmask >> 1 : xmask;
+            sp += pushT ? 1 : popB ? -1 : 0;
+            mx = max(mx, sp);
+            c += !run ? 0 : (e & LUT_DCP) ? 1 : (e & LUT_DCM) ? -1 : 0;
         }
+#pragma unroll
+        for (int u = 0; u < kCompBatch; ++u) { wA[u] = wB[u]; wB[u] = wC[u]; }
+        cmA = cmB;
     }
+    int n = (int)(po - po0);
     if (!valid) return;
     ok &= (sp >= 1);
     if (!ok) {
@@ -423,9 +438,9 @@ __global__ void __launch_bounds__(kCompileThreads) k_compile(const CompileParams
         q.meta[i] = make_int4(p, 0, 0, len);
         return;
     }
-    if (!((rmask >> (sp - 1)) & 1u)) {             // the result is a bare terminal
-        const uint32_t va = stk[sp - 1];
-        out[n] = ((xmask >> (sp - 1)) & 1u) ? make_uint2((va << kColAShift) | H_LX, 0u) : make_uint2(H_LC, va);
+    uint2* out = po0;
+    if (!(rmask & 1u)) {                           // the result is a bare terminal
+        out[n] = (xmask & 1u) ? make_uint2((t0 << kColAShift) | H_LX, 0u) : make_uint2(H_LC, t0);
         ++n;
     }
     out[n] = make_uint2(H_END, 0u);
