@@ -48,13 +48,16 @@ struct Header {                                // device-resident results of the
     int n_slow;                                // individuals whose micro-ops did not fit the workspace
     int n_malformed;
     unsigned int queue;                        // work-queue cursor of the interpreter kernel
+    unsigned int rcp_unsafe;                   // bit j: some case of variable j has |x| < 1e-6f (its division is protected)
 };
 
 struct EvalParams {
     const int4* meta; const uint2* uops; const Header* hdr; unsigned int* queue;
     const float* xt; float* fitness; float* outputs;
     float tax; int n; int npad; int d; int ring_bytes;
-    int slot_col0;      // first tensor-memory column after the variable block: passes * d * 16
+    int rcp_col0;       // first tensor-memory column of the reciprocal rows: passes * d * 16
+    int k_rcp;          // variables 0 .. k_rcp-1 have a reciprocal row (per pass)
+    int slot_col0;      // first tensor-memory column of the slot blocks
     int tmem_slots;     // S_T: slots per warp held in tensor memory (the deeper ones are in local memory)
 };
 
@@ -121,8 +124,13 @@ __global__ void __launch_bounds__(1024) k_len_pass2(long long* __restrict__ bsum
     __shared__ long long wtot2[32];
     __shared__ long long carry2_s;
     __shared__ int maxlen_s;
+    __shared__ unsigned int unsafe_s;
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    if (threadIdx.x == 0) { carry_s = 0; carry2_s = 0; maxlen_s = 0; }
+    if (threadIdx.x == 0) { carry_s = 0; carry2_s = 0; maxlen_s = 0; unsafe_s = 0; }
+    __syncthreads();
+    // which variables ever trigger the division protection (D2): their reciprocal row may not be used
+    for (int e = threadIdx.x; e < n * d; e += blockDim.x)
+        if (fabsf(X[e]) < kEps) atomicOr(&unsafe_s, 1u << (e % d));
     __syncthreads();
     for (int base = 0; base < nblocks; base += 1024) {
         const int i = base + threadIdx.x;
@@ -184,6 +192,7 @@ __global__ void __launch_bounds__(1024) k_len_pass2(long long* __restrict__ bsum
         hdr->max_len = maxlen_s;
         hdr->n_slow = 0; hdr->n_malformed = 0;
         hdr->queue = 0;
+        hdr->rcp_unsafe = unsafe_s;
     }
     // transpose: xt[j][i] = X[i][j] (j < d), xt[d][i] = y[i]; cases i >= n are zero
     for (int e = threadIdx.x; e < (d + 1) * npad; e += blockDim.x) {
@@ -247,7 +256,8 @@ enum : uint32_t {
     LUT_DIVC = 1u << 16,                             // o is a constant divisor: o = rcp(o), or acc = 1 if |o| < eps
     LUT_DBL = 1u << 17,                              // two records: first acc = c (LC), then this one
     LUT_EMIT = 1u << 18,
-    LUT_FSEL_A = 1u << 19                            // LUT_DBL: the first record's constant is operand a (else b)
+    LUT_FSEL_A = 1u << 19,                           // LUT_DBL: the first record's constant is operand a (else b)
+    LUT_DIVV = 1u << 20                              // o is a variable divisor: a reciprocal row may replace the division
 };
 constexpr int kLutUnary = 0, kLutBinary = 32, kLutNone = 127, kLutSize = 128;
 __device__ uint32_t g_compile_lut[kLutSize];
@@ -265,9 +275,9 @@ static void make_compile_lut(uint32_t* lut)
                 lut[kLutUnary + (kk << 2 | rb << 1 | xb)] = e;
             }
     const uint32_t hS[4] = { H_ADDS, H_RSUBS, H_MULS, H_RDIVS };            // j: ADD SUB MUL DIV
-    const uint32_t hX[4] = { H_ADDX, H_SUBX, H_MULX, H_DIVX }, hRX[4] = { H_ADDX, H_RSUBX, H_MULX, H_RDIVX };
+    const uint32_t hX[4] = { H_ADDX, H_SUBX, H_MULX, H_DIVX | LUT_DIVV }, hRX[4] = { H_ADDX, H_RSUBX, H_MULX, H_RDIVX };
     const uint32_t hC[4] = { H_ADDC, H_SUBC, H_MULC, H_MULC | LUT_DIVC }, hRC[4] = { H_ADDC, H_RSUBC, H_MULC, H_RDIVC };
-    const uint32_t hLXX[4] = { H_LX_ADDX, H_LX_SUBX, H_LX_MULX, H_LX_DIVX };
+    const uint32_t hLXX[4] = { H_LX_ADDX, H_LX_SUBX, H_LX_MULX, H_LX_DIVX | LUT_DIVV };
     const uint32_t hLXC[4] = { H_LX_ADDC, H_LX_SUBC, H_LX_MULC, H_LX_MULC | LUT_DIVC };
     const uint32_t hLXRC[4] = { H_LX_ADDC, H_LX_RSUBC, H_LX_MULC, H_LX_RDIVC };
     for (int j = 0; j < 4; ++j)
@@ -294,7 +304,7 @@ static void make_compile_lut(uint32_t* lut)
 //   in acc sits in slot c (tensor memory while c < S_T, local memory beyond).
 struct CompileParams {
     const uint32_t* genomes; const long long* off; const int32_t* lengths; const int* perm;
-    const float* consts; long long n_consts; int d; int tmem_slots;
+    const float* consts; long long n_consts; int d; int tmem_slots; int k_rcp;
     const int* binstart; const long long* binubase; Header* hdr;
     uint2* uops; long long ucap; int4* meta; int* depth; int* slow_list;
     float* fitness; float* outputs; int n_cases; int emit;
@@ -338,6 +348,8 @@ __global__ void __launch_bounds__(kCompileThreads) k_compile(const CompileParams
     int c = 0;                                     // computed entries on the stack (the topmost one is acc)
     bool ok = valid;
     const int S_T = q.tmem_slots;
+    // variables whose division is a multiplication by a staged reciprocal row
+    const uint32_t rcp_ok = ~q.hdr->rcp_unsafe & ((q.k_rcp >= 32) ? 0xFFFFFFFFu : ((1u << q.k_rcp) - 1u));
     const uint32_t* gtok = q.genomes + toff;
     uint2* po = q.uops + ua;                       // where the next record goes
     uint2* const po0 = po;
@@ -390,6 +402,8 @@ __global__ void __launch_bounds__(kCompileThreads) k_compile(const CompileParams
             const uint32_t colA = (e & LUT_CSEL_A) ? t1 : (e & LUT_CSEL_B) ? t0 : 0u;
             uint32_t h = (e & 0xFFu) + (colA << kColAShift) + ((e & LUT_PUSH) ? pb : 0u);
             if (e & LUT_SLOT) { const int s2 = c - 2; if (s2 >= S_T) { h += H_ADDM - H_ADDS; o = (uint32_t)((s2 - S_T) * 64); } }
+            if ((e & LUT_DIVV) && ((rcp_ok >> (o / kCasesPerLane)) & 1u))     // acc / X[o] = acc * (1/X)[o]
+                h += (e & LUT_PUSH) ? (uint32_t)(H_LX_MULR - H_LX_DIVX) : (uint32_t)(H_MULR - H_DIVX);
             if (e & LUT_DIVC) {                    // x / c = x * rcp(c) with the division handler's own rcp; protected: 1
                 const float cf = __uint_as_float(o);
                 const bool tiny = fabsf(cf) < kEps;
@@ -598,18 +612,34 @@ static beagle_status reserve_U(long long U)
 
 static long long uop_entries_bound(long long P, long long T) { return T + 4 * P + 2; }   // sum of uop_stride(len)
 
-// a4's plan of the 512 tensor-memory columns: the variable block (16 columns per variable and pass), then
-// S_T slots of 16 columns for each of the kEvalThreads/128 warps of a lane quarter. false: the variable
-// block does not fit (d > 32 at N <= 512, d > 16 beyond), and the call takes the blockwise kernel.
-static bool tmem_plan(int N, int d, int* slot_col0, int* tmem_slots)
+// a4's plan of the 512 tensor-memory columns (16 per row: a lane's 16 cases): the variable block (one row per
+// variable and pass), the reciprocal rows of variables 0 .. k_rcp-1 (division by a variable becomes a
+// multiplication, uop.cuh), then S_T slot rows for each warp of a lane quarter. The number of warps per
+// quarter (8, 7 or 6: 1024, 896 or 768 threads) is chosen so that three slot rows per warp remain when
+// possible. fast == false: the variable block alone does not fit (d > 32 at N <= 512, d > 16 beyond), and the
+// call takes the blockwise kernel.
+struct TmemPlan { bool fast; int threads; int rcp_col0; int k_rcp; int slot_col0; int tmem_slots; };
+static TmemPlan tmem_plan(int N, int d)
 {
+    TmemPlan t = { false, kEvalThreads, 0, 0, 0, 0 };
     const int passes = (N + kCasesPerPass - 1) / kCasesPerPass;
-    const int nx = passes * d * kCasesPerLane;
-    if (nx > kTmemCols) return false;
-    int st = (kTmemCols - nx) / kCasesPerLane / (kEvalThreads / 128);
+    const int rows = kTmemCols / kCasesPerLane;                  // 32
+    const int xrows = passes * d;
+    if (xrows > rows) return t;
+    t.fast = true;
+    const int wq_max = kEvalThreads / 128;
+    // reciprocal rows: as many variables as leave one slot row per warp at the full warp count
+    int k = (rows - xrows - wq_max) / passes;
+    k = k < 0 ? 0 : (k > d ? d : k);
+    const int free_rows = rows - xrows - passes * k;
+    int wq = wq_max;                                            // the most warps that still get three slot rows each
+    for (int c = wq_max; c >= 6; --c) if (free_rows / c >= 3) { wq = c; break; }
+    int st = free_rows / wq;
     if (st > kMemSlots) st = kMemSlots;
-    *slot_col0 = nx; *tmem_slots = st;
-    return true;
+    t.threads = wq * 128;
+    t.rcp_col0 = xrows * kCasesPerLane; t.k_rcp = k;
+    t.slot_col0 = (xrows + passes * k) * kCasesPerLane; t.tmem_slots = st;
+    return t;
 }
 
 static beagle_status check_args(const void* genomes, const void* lengths, int64_t P, const void* consts,
@@ -654,9 +684,9 @@ static beagle_status run_prepass(const int32_t* genomes, const int32_t* lengths,
     {
         CompileParams q;
         q.genomes = reinterpret_cast<const uint32_t*>(genomes); q.off = w.off; q.lengths = lengths; q.perm = w.perm;
-        int col0 = 0, st_slots = 0;
-        tmem_plan(N, d, &col0, &st_slots);
-        q.consts = consts; q.n_consts = n_consts; q.d = d; q.tmem_slots = st_slots; q.binstart = w.binstart; q.binubase = w.binubase;
+        const TmemPlan tp = tmem_plan(N, d);
+        q.consts = consts; q.n_consts = n_consts; q.d = d; q.tmem_slots = tp.tmem_slots; q.k_rcp = tp.k_rcp;
+        q.binstart = w.binstart; q.binubase = w.binubase;
         q.hdr = w.hdr; q.uops = w.uops; q.ucap = w.cap_U; q.meta = w.meta; q.depth = w.depth;
         q.slow_list = w.slow_list; q.fitness = fitness; q.outputs = outputs; q.n_cases = N; q.emit = emit ? 1 : 0;
         k_compile<<<(unsigned)((P + kCompileThreads - 1) / kCompileThreads), kCompileThreads, 0, st>>>(q);
@@ -684,7 +714,9 @@ static beagle_status run_eval(const int32_t* genomes, const int32_t* lengths, co
     const int npad = (N + kCasePad - 1) / kCasePad * kCasePad;
     const long long ys_bytes = (long long)npad * 4;
     EvalParams prm;
-    if (!tmem_plan(N, d, &prm.slot_col0, &prm.tmem_slots)) return BEAGLE_ERR_UNSUPPORTED;   // callers check first
+    const TmemPlan tp = tmem_plan(N, d);
+    if (!tp.fast) return BEAGLE_ERR_UNSUPPORTED;   // callers check first
+    prm.rcp_col0 = tp.rcp_col0; prm.k_rcp = tp.k_rcp; prm.slot_col0 = tp.slot_col0; prm.tmem_slots = tp.tmem_slots;
     prm.meta = w.meta; prm.uops = w.uops; prm.hdr = w.hdr; prm.xt = w.xt;
     prm.fitness = fitness; prm.outputs = outputs; prm.tax = tax; prm.n = N; prm.npad = npad; prm.d = d;
     const bool prof = g_profiling && w.prof_n < kProfMax;
@@ -694,10 +726,10 @@ static beagle_status run_eval(const int32_t* genomes, const int32_t* lengths, co
         CU(cudaEventRecord(w.ev_k[2 * w.prof_n], st));
     }
     size_t smem = 0;
-    prm.ring_bytes = ring_bytes_for(kEvalThreads, ys_bytes, w.smem_optin, &smem);
+    prm.ring_bytes = ring_bytes_for(tp.threads, ys_bytes, w.smem_optin, &smem);
     if (prm.ring_bytes < kStageBytesMax) return BEAGLE_ERR_UNSUPPORTED;
     prm.queue = &w.hdr->queue;
-    k_eval<<<w.num_sms, kEvalThreads, smem, st>>>(prm);
+    k_eval<<<w.num_sms, tp.threads, smem, st>>>(prm);
     ++g_launches;
     if (prof) { CU(cudaEventRecord(w.ev_k[2 * w.prof_n + 1], st)); ++w.prof_n; }
     // slow path: individuals whose micro-ops did not fit the promised workspace (normally none)
@@ -716,8 +748,7 @@ static beagle_status run_colony(const int32_t* genomes, const int32_t* lengths, 
                                 float* fitness, float* outputs, long long T_known, cudaStream_t st)
 {
     Workspace& w = g_ws;
-    int col0, slots;
-    const bool fast = tmem_plan(N, d, &col0, &slots);
+    const bool fast = tmem_plan(N, d).fast;
     beagle_status s = run_prepass(genomes, lengths, P, consts, n_consts, X, y, N, d, fitness, outputs, T_known, fast, st);
     if (s != BEAGLE_OK) return s;
     if (fast) return run_eval(genomes, lengths, consts, X, y, P, N, d, tax, fitness, outputs, st);

@@ -21,7 +21,8 @@
 //
 // Register names inside the block: a<k> accumulator, x<k> second operand, t<k>/q<k>/p<k> temporaries;
 // (h, o) = the record of the micro-op being dispatched / run (uop.cuh); pc = its shared-memory address;
-// xb = tensor-memory address of this pass's variable block, sb = of this warp's slot block.
+// xb = tensor-memory address of this pass's variable block, rb = of its reciprocal rows, sb = of this warp's
+// slot block.
 #pragma once
 #include "uop.cuh"
 
@@ -117,6 +118,9 @@
     "K_" #OP "_%=:\n" BGI_NEXT BGI_WAITLD BGI_K16(BODY) BGI_DISPATCH
 #define BGI_ENTRY_S(OP)  "L_" #OP "S_%=:\n" "sub.u32 spt, spt, 16;\n" "mov.u32 xa, spt;\n" "bra.uni J_" #OP "_%=;\n"
 #define BGI_ENTRY_M(OP)  "L_" #OP "M_%=:\n" BGI_GETM "bra.uni K_" #OP "_%=;\n"
+// acc = acc * (1/X)[o]: the reciprocal rows have their own base (rb); the body is MUL's
+#define BGI_ENTRY_R      "L_MULR_%=:\n" "add.u32 xa, o, rb;\n" "bra.uni J_MUL_%=;\n" \
+    BGI_PUSHES(LX_MULR) "L_LX_MULR_%=:\n" BGI_LXA "add.u32 xa, o, rb;\n" "bra.uni J_MUL_%=;\n"
 #define BGI_ENTRY_LXX(OP) BGI_PUSHES(LX_##OP##X) "L_LX_" #OP "X_%=:\n" BGI_LXA "add.u32 xa, o, xb;\n" "bra.uni J_" #OP "_%=;\n"
 // acc = acc OP c, acc = f(acc); LX_ entry: acc = X[colA] first
 #define BGI_BIN_C(OP, BODY) "L_" #OP "C_%=:\n" "mov.b32 cv, o;\n" BGI_NEXT BGI_K16(BODY) BGI_DISPATCH
@@ -127,7 +131,7 @@
     BGI_UNARY(SIN, BGI_SIN) BGI_UNARY(COS, BGI_COS) BGI_UNARY(LOG, BGI_LOG) BGI_UNARY(SQRT, BGI_SQRT) BGI_UNARY(EXP, BGI_EXP) \
     BGI_ENTRY_LX(SIN) BGI_ENTRY_LX(COS) BGI_ENTRY_LX(LOG) BGI_ENTRY_LX(SQRT) BGI_ENTRY_LX(EXP) \
     BGI_BIN_X(ADD, BGI_ADDX) BGI_ENTRY_S(ADD) BGI_ENTRY_M(ADD) BGI_ENTRY_LXX(ADD) \
-    BGI_BIN_X(MUL, BGI_MULX) BGI_ENTRY_S(MUL) BGI_ENTRY_M(MUL) BGI_ENTRY_LXX(MUL) \
+    BGI_BIN_X(MUL, BGI_MULX) BGI_ENTRY_S(MUL) BGI_ENTRY_M(MUL) BGI_ENTRY_LXX(MUL) BGI_ENTRY_R \
     BGI_BIN_X(SUB, BGI_SUBX) BGI_ENTRY_LXX(SUB) \
     BGI_BIN_X(DIV, BGI_DIVX) BGI_ENTRY_LXX(DIV) \
     BGI_BIN_X(RSUB, BGI_RSUBX) BGI_ENTRY_S(RSUB) BGI_ENTRY_M(RSUB) \
@@ -149,7 +153,7 @@
 #define BGI_FRESH(T) \
     T(LX) T(LC) T(LX_SIN) T(LX_COS) T(LX_LOG) T(LX_SQRT) T(LX_EXP) \
     T(LX_ADDX) T(LX_SUBX) T(LX_MULX) T(LX_DIVX) \
-    T(LX_ADDC) T(LX_SUBC) T(LX_MULC) T(LX_RSUBC) T(LX_RDIVC)
+    T(LX_ADDC) T(LX_SUBC) T(LX_MULC) T(LX_RSUBC) T(LX_RDIVC) T(LX_MULR)
 #define BGI_TABLE \
     "TBL_%=: .branchtargets " \
     BGI_T(END) BGI_T(SIN) BGI_T(COS) BGI_T(LOG) BGI_T(SQRT) BGI_T(EXP) \
@@ -157,23 +161,24 @@
     BGI_T(ADDS) BGI_T(MULS) BGI_T(RSUBS) BGI_T(RDIVS) \
     BGI_T(ADDM) BGI_T(MULM) BGI_T(RSUBM) BGI_T(RDIVM) \
     BGI_T(ADDC) BGI_T(SUBC) BGI_T(MULC) BGI_T(RSUBC) BGI_T(RDIVC) \
-    BGI_FRESH(BGI_T) BGI_FRESH(BGI_TP) BGI_FRESH(BGI_TM) \
+    BGI_FRESH(BGI_T) BGI_FRESH(BGI_TP) BGI_FRESH(BGI_TM) BGI_T(MULR) \
     "L_END_%=;\n"
 
 #define BGI_OUT(k) "mov.f32 %" #k ", a" #k ";\n"
 
-// Operands: %0..%15 = acc out, %16 = shared address of the records, %17 = xb, %18 = sb.
+// Operands: %0..%15 = acc out, %16 = shared address of the records, %17 = xb, %18 = sb, %19 = rb.
 #define BGI_ASM \
     "{\n" \
     ".reg .f32 a<16>, x<16>, t<16>, q<16>, cv;\n" \
     ".reg .pred p<16>;\n" \
-    ".reg .b32 h, o, hn, pc, xa, xb, spt, e;\n" \
+    ".reg .b32 h, o, hn, pc, xa, xb, rb, spt, e;\n" \
     ".reg .b64 ma, mbase;\n" \
     ".local .align 16 .b8 slotmem[1984];\n"      /* kMemSlots * 64 */ \
     BGI_TABLE \
     "mov.u32 pc, %16;\n" \
     "mov.u32 xb, %17;\n" \
     "mov.u32 spt, %18;\n" \
+    "mov.u32 rb, %19;\n" \
     "mov.u64 mbase, slotmem;\n" \
     "ld.shared.v2.b32 {h, o}, [pc];\n" \
     BGI_DISPATCHER \
@@ -188,12 +193,12 @@
 namespace beagle {
 
 static_assert(kMemSlots * 64 == 1984 && kCasesPerLane == 16, "interp.cuh is written for 16 cases per lane and 31 memory slots");
-static_assert(H_COUNT == 73, "BGI_TABLE lists the handlers in the order of uop.cuh's enum");
+static_assert(H_COUNT == 77, "BGI_TABLE lists the handlers in the order of uop.cuh's enum");
 
 // acc[k] = the program's output on case (pass * 512 + (k/4)*128 + lane*4 + k%4)
-__device__ __forceinline__ void interp_run(uint32_t rec, uint32_t xb, uint32_t sb, float (&acc)[16])
+__device__ __forceinline__ void interp_run(uint32_t rec, uint32_t xb, uint32_t sb, uint32_t rb, float (&acc)[16])
 {
-    asm volatile(BGI_ASM : BGI_ACC_OUT(acc) : "r"(rec), "r"(xb), "r"(sb) : "memory");
+    asm volatile(BGI_ASM : BGI_ACC_OUT(acc) : "r"(rec), "r"(xb), "r"(sb), "r"(rb) : "memory");
 }
 
 } // namespace beagle

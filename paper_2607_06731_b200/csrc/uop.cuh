@@ -15,6 +15,8 @@
 //     x  y  DIV      ->  LX_DIVX x, y     acc = X[x] / X[y]          (both terminal: a fresh value)
 //     x  SIN         ->  LX_SIN x         acc = sin X[x]
 //     <A> <B> DIV    ->  RDIVS s          acc = slot[s] / acc        (both computed)
+//     <A> x  DIV     ->  MULR  x          acc = acc * (1/X)[x]       (division by a variable is loop-invariant:
+//                                         when no case of x is protected, its reciprocals are a staged row)
 // and "push acc" is not a micro-op either: the micro-op that starts the next fresh value is dispatched to
 // the push entry of its handler (handler number + H_PUSHT or + H_PUSHM).
 // Commands run in the program's own order and every micro-op computes exactly the value the postfix
@@ -56,10 +58,12 @@ enum : uint32_t {
     H_LX_SIN = 27, H_LX_COS = 28, H_LX_LOG = 29, H_LX_SQRT = 30, H_LX_EXP = 31,
     H_LX_ADDX = 32, H_LX_SUBX = 33, H_LX_MULX = 34, H_LX_DIVX = 35,
     H_LX_ADDC = 36, H_LX_SUBC = 37, H_LX_MULC = 38, H_LX_RSUBC = 39, H_LX_RDIVC = 40,
-    H_FRESH0 = H_LX, H_NFRESH = 16,             // the fresh-value handlers H_LX .. H_LX_RDIVC
+    H_LX_MULR = 41,                             // acc = X[colA] * (1 / X)[o]: division by a variable whose reciprocal row is staged
+    H_FRESH0 = H_LX, H_NFRESH = 17,             // the fresh-value handlers H_LX .. H_LX_MULR
     H_PUSHT = H_NFRESH,                         // + handler: push acc to the tensor-memory slot stack first
     H_PUSHM = 2 * H_NFRESH,                     // + handler: push acc to the local slot at byte offset h[20:10] first
-    H_COUNT = 41 + 2 * H_NFRESH
+    H_MULR = H_FRESH0 + 3 * H_NFRESH,           // acc = acc * (1 / X)[o]
+    H_COUNT = H_MULR + 1
 };
 
 constexpr int kPushShift = 10, kColAShift = 21;
