@@ -19,7 +19,7 @@
 // Per-command arithmetic is instruction for instruction that of ops.cuh (same PTX opcodes, same constants),
 // so per-case outputs are bit-identical to the C++ kernel that uses ops.cuh (k_eval_blockwise).
 //
-// Register names inside the block: a<k> accumulator, x<k> second operand, t<k>/q<k>/p<k> temporaries;
+// Register names inside the block: %0..%15 (the asm's output operands) are the accumulator, x<k> second operand, t<k>/q<k>/p<k> temporaries;
 // (h, o) = the record of the micro-op being dispatched / run (uop.cuh); pc = its shared-memory address;
 // xb = tensor-memory address of this pass's variable block, rb = of its reciprocal rows, sb = of this warp's
 // slot block.
@@ -45,34 +45,34 @@
     "abs.f32 t" #k ", " B ";\n" \
     "setp.lt.f32 p" #k ", t" #k ", " BGI_EPS ";\n" \
     "selp.f32 " DST ", " BGI_ONE ", q" #k ", p" #k ";\n"
-#define BGI_SIN(k)  "sin.approx.ftz.f32 a" #k ", a" #k ";\n"
-#define BGI_COS(k)  "cos.approx.ftz.f32 a" #k ", a" #k ";\n"
-#define BGI_SQRT(k) "abs.f32 t" #k ", a" #k ";\n" "sqrt.approx.ftz.f32 a" #k ", t" #k ";\n"
+#define BGI_SIN(k)  "sin.approx.ftz.f32 %" #k ", %" #k ";\n"
+#define BGI_COS(k)  "cos.approx.ftz.f32 %" #k ", %" #k ";\n"
+#define BGI_SQRT(k) "abs.f32 t" #k ", %" #k ";\n" "sqrt.approx.ftz.f32 %" #k ", t" #k ";\n"
 #define BGI_LOG(k) \
-    "abs.f32 t" #k ", a" #k ";\n" \
+    "abs.f32 t" #k ", %" #k ";\n" \
     "lg2.approx.ftz.f32 q" #k ", t" #k ";\n" \
     "mul.rn.f32 q" #k ", q" #k ", " BGI_LN2 ";\n" \
     "setp.lt.f32 p" #k ", t" #k ", " BGI_EPS ";\n" \
-    "selp.f32 a" #k ", " BGI_ZERO ", q" #k ", p" #k ";\n"
+    "selp.f32 %" #k ", " BGI_ZERO ", q" #k ", p" #k ";\n"
 #define BGI_EXP(k) \
-    "min.NaN.f32 t" #k ", a" #k ", " BGI_80 ";\n" \
+    "min.NaN.f32 t" #k ", %" #k ", " BGI_80 ";\n" \
     "mul.rn.f32 t" #k ", t" #k ", " BGI_LOG2E ";\n" \
-    "ex2.approx.ftz.f32 a" #k ", t" #k ";\n"
+    "ex2.approx.ftz.f32 %" #k ", t" #k ";\n"
 
 // second operand in x<k> (a variable or a slot, loaded from tensor / local memory)
-#define BGI_ADDX(k)  "add.rn.f32 a" #k ", a" #k ", x" #k ";\n"
-#define BGI_SUBX(k)  "sub.rn.f32 a" #k ", a" #k ", x" #k ";\n"
-#define BGI_MULX(k)  "mul.rn.f32 a" #k ", a" #k ", x" #k ";\n"
-#define BGI_RSUBX(k) "sub.rn.f32 a" #k ", x" #k ", a" #k ";\n"
-#define BGI_DIVX(k)  BGI_DIV("a" #k, "a" #k, "x" #k, k)
-#define BGI_RDIVX(k) BGI_DIV("a" #k, "x" #k, "a" #k, k)
+#define BGI_ADDX(k)  "add.rn.f32 %" #k ", %" #k ", x" #k ";\n"
+#define BGI_SUBX(k)  "sub.rn.f32 %" #k ", %" #k ", x" #k ";\n"
+#define BGI_MULX(k)  "mul.rn.f32 %" #k ", %" #k ", x" #k ";\n"
+#define BGI_RSUBX(k) "sub.rn.f32 %" #k ", x" #k ", %" #k ";\n"
+#define BGI_DIVX(k)  BGI_DIV("%" #k, "%" #k, "x" #k, k)
+#define BGI_RDIVX(k) BGI_DIV("%" #k, "x" #k, "%" #k, k)
 // second operand = constant (cv)
-#define BGI_LC(k)    "mov.f32 a" #k ", cv;\n"
-#define BGI_ADDC(k)  "add.rn.f32 a" #k ", a" #k ", cv;\n"
-#define BGI_SUBC(k)  "sub.rn.f32 a" #k ", a" #k ", cv;\n"
-#define BGI_MULC(k)  "mul.rn.f32 a" #k ", a" #k ", cv;\n"
-#define BGI_RSUBC(k) "sub.rn.f32 a" #k ", cv, a" #k ";\n"
-#define BGI_RDIVC(k) BGI_DIV("a" #k, "cv", "a" #k, k)
+#define BGI_LC(k)    "mov.f32 %" #k ", cv;\n"
+#define BGI_ADDC(k)  "add.rn.f32 %" #k ", %" #k ", cv;\n"
+#define BGI_SUBC(k)  "sub.rn.f32 %" #k ", %" #k ", cv;\n"
+#define BGI_MULC(k)  "mul.rn.f32 %" #k ", %" #k ", cv;\n"
+#define BGI_RSUBC(k) "sub.rn.f32 %" #k ", cv, %" #k ";\n"
+#define BGI_RDIVC(k) BGI_DIV("%" #k, "cv", "%" #k, k)
 
 // ---- handler frame ---------------------------------------------------------------------------------------
 // entry: (h, o) = this micro-op's record, pc = its shared-memory address. NEXT replaces (h, o) by the next
@@ -82,7 +82,7 @@
 #define BGI_LDTM(R, ADDR) "tcgen05.ld.sync.aligned.32x32b.x16.b32 {" BGI_R16(R) "}, [" ADDR "];\n"
 #define BGI_DISPATCH "bra.uni DISP_%=;\n"
 // fresh value: acc = X[colA], colA = h[31:21]
-#define BGI_LXA     "shr.u32 e, h, 21;\n" "add.u32 e, e, xb;\n" BGI_LDTM("a", "e")
+#define BGI_LXA     "shr.u32 e, h, 21;\n" "add.u32 e, e, xb;\n" BGI_LDTM("%", "e")
 // x = local slot memory, 16 floats per slot per lane at byte offset o
 #define BGI_GETM \
     "cvt.u64.u32 ma, o;\n" \
@@ -95,17 +95,17 @@
 // "push acc" in front of a fresh value: P_<entry> pushes to the warp's tensor-memory slot stack (spt), M_<entry>
 // to the local-memory slot at byte offset h[20:10]; both fall / branch into the entry itself.
 #define BGI_PUSHT \
-    "tcgen05.st.sync.aligned.32x32b.x16.b32 [spt], {" BGI_R16("a") "};\n" \
+    "tcgen05.st.sync.aligned.32x32b.x16.b32 [spt], {" BGI_R16("%") "};\n" \
     "tcgen05.wait::st.sync.aligned;\n" \
     "add.u32 spt, spt, 16;\n"
 #define BGI_PUSHM \
     "bfe.u32 e, h, 10, 11;\n" \
     "cvt.u64.u32 ma, e;\n" \
     "add.u64 ma, ma, mbase;\n" \
-    "st.local.v4.f32 [ma], {a0, a1, a2, a3};\n" \
-    "st.local.v4.f32 [ma+16], {a4, a5, a6, a7};\n" \
-    "st.local.v4.f32 [ma+32], {a8, a9, a10, a11};\n" \
-    "st.local.v4.f32 [ma+48], {a12, a13, a14, a15};\n"
+    "st.local.v4.f32 [ma], {%0, %1, %2, %3};\n" \
+    "st.local.v4.f32 [ma+16], {%4, %5, %6, %7};\n" \
+    "st.local.v4.f32 [ma+32], {%8, %9, %10, %11};\n" \
+    "st.local.v4.f32 [ma+48], {%12, %13, %14, %15};\n"
 #define BGI_PUSHES(ENTRY) \
     "M_" #ENTRY "_%=:\n" BGI_PUSHM "bra.uni L_" #ENTRY "_%=;\n" \
     "P_" #ENTRY "_%=:\n" BGI_PUSHT
@@ -164,12 +164,12 @@
     BGI_FRESH(BGI_T) BGI_FRESH(BGI_TP) BGI_FRESH(BGI_TM) BGI_T(MULR) \
     "L_END_%=;\n"
 
-#define BGI_OUT(k) "mov.f32 %" #k ", a" #k ";\n"
+#define BGI_OUT(k) "mov.f32 %" #k ", %" #k ";\n"
 
-// Operands: %0..%15 = acc out, %16 = shared address of the records, %17 = xb, %18 = sb, %19 = rb.
+// Operands: %0..%15 = acc (used in place), %16 = shared address of the records, %17 = xb, %18 = sb, %19 = rb.
 #define BGI_ASM \
     "{\n" \
-    ".reg .f32 a<16>, x<16>, t<16>, q<16>, cv;\n" \
+    ".reg .f32 x<16>, t<16>, q<16>, cv;\n" \
     ".reg .pred p<16>;\n" \
     ".reg .b32 h, o, hn, pc, xa, xb, rb, spt, e;\n" \
     ".reg .b64 ma, mbase;\n" \
@@ -184,11 +184,10 @@
     BGI_DISPATCHER \
     BGI_HANDLERS \
     "L_END_%=:\n" \
-    BGI_K16(BGI_OUT) \
     "}\n"
 
-#define BGI_ACC_OUT(A) "=f"(A[0]), "=f"(A[1]), "=f"(A[2]), "=f"(A[3]), "=f"(A[4]), "=f"(A[5]), "=f"(A[6]), "=f"(A[7]), \
-                       "=f"(A[8]), "=f"(A[9]), "=f"(A[10]), "=f"(A[11]), "=f"(A[12]), "=f"(A[13]), "=f"(A[14]), "=f"(A[15])
+#define BGI_ACC_OUT(A) "=&f"(A[0]), "=&f"(A[1]), "=&f"(A[2]), "=&f"(A[3]), "=&f"(A[4]), "=&f"(A[5]), "=&f"(A[6]), "=&f"(A[7]), \
+                       "=&f"(A[8]), "=&f"(A[9]), "=&f"(A[10]), "=&f"(A[11]), "=&f"(A[12]), "=&f"(A[13]), "=&f"(A[14]), "=&f"(A[15])
 
 namespace beagle {
 
