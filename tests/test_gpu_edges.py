@@ -224,3 +224,32 @@ def test_limits_and_exports():
     from paper_2607_06731_b200 import api
     lim = api.beagle_limits()
     assert lim == dict(max_len=512, max_stack=32, max_n=1024, max_d=32)
+
+
+@pytest.mark.parametrize("N", [512, 700, 1024])
+def test_division_by_variable_reciprocal_rows(oracle, N):
+    """Division by a variable runs as a multiplication by a staged reciprocal row only when no case of that
+    variable is protected. x0 never triggers the protection; x1 does, in one case only (the
+    last one, also inside a ragged tail); x2 is exactly zero everywhere. Outputs must be bit-identical to the
+    blockwise kernel (the plain per-case division) and agree with the oracle."""
+    from tests.gpu_util import gpu_eval, gpu_outputs
+    rng = np.random.default_rng(11)
+    d = 3
+    X = rng.uniform(0.5, 4.0, (N, d)).astype(np.float32)
+    X[N - 1, 1] = np.float32(3e-7)
+    X[:, 2] = 0.0
+    y = (X[:, 0] / 3.0).astype(np.float32)
+    consts = []
+    texts = ["x1 x0 DIV", "x0 x1 DIV", "x0 x2 DIV", "x0 x0 MUL x0 DIV", "x0 x0 MUL x1 DIV", "x1 SIN x2 DIV",
+             "x0 x1 ADD x0 x1 MUL DIV x0 DIV", "2.5 x0 DIV", "x0 2.5 DIV x1 DIV", "x0 COS x0 x0 DIV x1 x0 DIV ADD SUB"]
+    progs = [asm(t, consts)[0] for t in texts]
+    g, l, c = pack(progs, consts)
+    a = gpu_eval(g, l, c, X, y, 0.001)
+    b = gpu_eval(g, l, c, X, y, 0.001, fn="beagle_eval_blockwise")
+    assert np.array_equal(_bits(a), _bits(b))
+    orc = oracle.evaluate(g, l, c, X, y, 0.001)
+    rep = parity.compare(a, orc)
+    assert len(rep["bad"]) == 0, parity.describe(rep, a, orc)
+    out = gpu_outputs(g, l, c, X)
+    assert np.all(out[1, N - 1] == np.float32(1.0))          # x0 / 3e-7 is protected: 1
+    assert np.all(out[2] == np.float32(1.0))                 # x0 / 0 is protected everywhere
