@@ -57,6 +57,7 @@ struct EvalParams {
     float tax; int n; int npad; int d; int ring_bytes;
     int rcp_col0;       // first tensor-memory column of the reciprocal rows: passes * d * 16
     int k_rcp;          // variables 0 .. k_rcp-1 have a reciprocal row (per pass)
+    int k_un;           // variables 0 .. k_un-1 have their five unary rows staged in shared memory
     int slot_col0;      // first tensor-memory column of the slot blocks
     int tmem_slots;     // S_T: slots per warp held in tensor memory (the deeper ones are in local memory)
 };
@@ -257,7 +258,8 @@ enum : uint32_t {
     LUT_DBL = 1u << 17,                              // two records: first acc = c (LC), then this one
     LUT_EMIT = 1u << 18,
     LUT_FSEL_A = 1u << 19,                           // LUT_DBL: the first record's constant is operand a (else b)
-    LUT_DIVV = 1u << 20                              // o is a variable divisor: a reciprocal row may replace the division
+    LUT_DIVV = 1u << 20,                             // o is a variable divisor: a reciprocal row may replace the division
+    LUT_UNV = 1u << 21                               // a unary command on a variable: its staged row may replace it
 };
 constexpr int kLutUnary = 0, kLutBinary = 32, kLutNone = 127, kLutSize = 128;
 __device__ uint32_t g_compile_lut[kLutSize];
@@ -270,7 +272,7 @@ static void make_compile_lut(uint32_t* lut)
             for (int xb = 0; xb < 2; ++xb) {
                 uint32_t e;
                 if (rb) e = LUT_EMIT | (H_SIN + kk);
-                else if (xb) e = LUT_EMIT | LUT_PUSH | LUT_DCP | LUT_CSEL_B | (H_LX_SIN + kk);
+                else if (xb) e = LUT_EMIT | LUT_PUSH | LUT_DCP | LUT_CSEL_B | LUT_UNV | (H_LX_SIN + kk);
                 else e = LUT_EMIT | LUT_DBL | LUT_DCP | (H_SIN + kk);
                 lut[kLutUnary + (kk << 2 | rb << 1 | xb)] = e;
             }
@@ -304,7 +306,7 @@ static void make_compile_lut(uint32_t* lut)
 //   in acc sits in slot c (tensor memory while c < S_T, local memory beyond).
 struct CompileParams {
     const uint32_t* genomes; const long long* off; const int32_t* lengths; const int* perm;
-    const float* consts; long long n_consts; int d; int tmem_slots; int k_rcp;
+    const float* consts; long long n_consts; int d; int tmem_slots; int k_rcp; int k_un; int un_row_bytes;
     const int* binstart; const long long* binubase; Header* hdr;
     uint2* uops; long long ucap; int4* meta; int* depth; int* slow_list;
     float* fitness; float* outputs; int n_cases; int emit;
@@ -402,6 +404,10 @@ __global__ void __launch_bounds__(kCompileThreads) k_compile(const CompileParams
             const uint32_t colA = (e & LUT_CSEL_A) ? t1 : (e & LUT_CSEL_B) ? t0 : 0u;
             uint32_t h = (e & 0xFFu) + (colA << kColAShift) + ((e & LUT_PUSH) ? pb : 0u);
             if (e & LUT_SLOT) { const int s2 = c - 2; if (s2 >= S_T) { h += H_ADDM - H_ADDS; o = (uint32_t)((s2 - S_T) * 64); } }
+            if ((e & LUT_UNV) && (int)(t0 / kCasesPerLane) < q.k_un) {        // f(X[j]) = the staged row (f, j)
+                h = pb + (uint32_t)H_LS;
+                o = (uint32_t)(((int)(op - OPC_SIN) * q.k_un + (int)(t0 / kCasesPerLane)) * q.un_row_bytes);
+            }
             if ((e & LUT_DIVV) && ((rcp_ok >> (o / kCasesPerLane)) & 1u))     // acc / X[o] = acc * (1/X)[o]
                 h += (e & LUT_PUSH) ? (uint32_t)(H_LX_MULR - H_LX_DIVX) : (uint32_t)(H_MULR - H_DIVX);
             if (e & LUT_DIVC) {                    // x / c = x * rcp(c) with the division handler's own rcp; protected: 1
@@ -618,10 +624,10 @@ static long long uop_entries_bound(long long P, long long T) { return T + 4 * P 
 // quarter (8, 7 or 6: 1024, 896 or 768 threads) is chosen so that three slot rows per warp remain when
 // possible. fast == false: the variable block alone does not fit (d > 32 at N <= 512, d > 16 beyond), and the
 // call takes the blockwise kernel.
-struct TmemPlan { bool fast; int threads; int rcp_col0; int k_rcp; int slot_col0; int tmem_slots; };
+struct TmemPlan { bool fast; int threads; int rcp_col0; int k_rcp; int slot_col0; int tmem_slots; int k_un; int ring_bytes; size_t smem; };
 static TmemPlan tmem_plan(int N, int d)
 {
-    TmemPlan t = { false, kEvalThreads, 0, 0, 0, 0 };
+    TmemPlan t = { false, kEvalThreads, 0, 0, 0, 0, 0, 0, 0 };
     const int passes = (N + kCasesPerPass - 1) / kCasesPerPass;
     const int rows = kTmemCols / kCasesPerLane;                  // 32
     const int xrows = passes * d;
@@ -639,6 +645,20 @@ static TmemPlan tmem_plan(int N, int d)
     t.threads = wq * 128;
     t.rcp_col0 = xrows * kCasesPerLane; t.k_rcp = k;
     t.slot_col0 = (xrows + passes * k) * kCasesPerLane; t.tmem_slots = st;
+    // shared memory: barriers, y, the warps' queue windows, then the staged rows f(X[j]) of the five unary commands
+    // for variables 0 .. k_un-1 (a unary command on a variable is loop-invariant: uop.cuh H_LS), then the rings;
+    // every warp keeps room for at least one stage of the longest program
+    const int warps = t.threads / 32;
+    const int npad = (N + kCasePad - 1) / kCasePad * kCasePad;
+    const long long fixed = ((64 + warps * kStagesMax * 8 + 127) & ~127) + (long long)npad * 4 + (long long)kEvalMetaBytes * warps;
+    const long long spare = (long long)g_ws.smem_optin - fixed - (long long)warps * kStageBytesMax;
+    long long ku = spare / (5ll * npad * 4);
+    t.k_un = (int)(ku < 0 ? 0 : (ku > d ? d : ku));
+    const long long un_bytes = 5ll * t.k_un * npad * 4;
+    long long ring = ((g_ws.smem_optin - fixed - un_bytes) / warps) & ~127ll;
+    if (ring > (long long)kStagesMax * kStageBytesMax) ring = (long long)kStagesMax * kStageBytesMax;
+    t.ring_bytes = (int)ring;
+    t.smem = (size_t)(fixed + un_bytes + ring * warps);
     return t;
 }
 
@@ -685,7 +705,7 @@ static beagle_status run_prepass(const int32_t* genomes, const int32_t* lengths,
         CompileParams q;
         q.genomes = reinterpret_cast<const uint32_t*>(genomes); q.off = w.off; q.lengths = lengths; q.perm = w.perm;
         const TmemPlan tp = tmem_plan(N, d);
-        q.consts = consts; q.n_consts = n_consts; q.d = d; q.tmem_slots = tp.tmem_slots; q.k_rcp = tp.k_rcp;
+        q.consts = consts; q.n_consts = n_consts; q.d = d; q.tmem_slots = tp.tmem_slots; q.k_rcp = tp.k_rcp; q.k_un = tp.k_un; q.un_row_bytes = npad * 4;
         q.binstart = w.binstart; q.binubase = w.binubase;
         q.hdr = w.hdr; q.uops = w.uops; q.ucap = w.cap_U; q.meta = w.meta; q.depth = w.depth;
         q.slow_list = w.slow_list; q.fitness = fitness; q.outputs = outputs; q.n_cases = N; q.emit = emit ? 1 : 0;
@@ -694,16 +714,6 @@ static beagle_status run_prepass(const int32_t* genomes, const int32_t* lengths,
     }
     CU(cudaGetLastError());
     return BEAGLE_OK;
-}
-
-static int ring_bytes_for(int threads, long long ys_bytes, int smem_optin, size_t* smem_out)
-{
-    const int warps = threads / 32;
-    const long long fixed = ((64 + warps * kStagesMax * 8 + 127) & ~127) + ((ys_bytes + 127) & ~127ll) + (long long)kEvalMetaBytes * warps;
-    long long ring = ((smem_optin - fixed) / warps) & ~127ll;
-    if (ring > (long long)kStagesMax * kStageBytesMax) ring = (long long)kStagesMax * kStageBytesMax;
-    *smem_out = (size_t)(fixed + ring * warps);
-    return (int)ring;
 }
 
 static beagle_status run_eval(const int32_t* genomes, const int32_t* lengths, const float* consts, const float* X,
@@ -725,8 +735,8 @@ static beagle_status run_eval(const int32_t* genomes, const int32_t* lengths, co
             if (!w.ev_k[2 * w.prof_n + i]) CU(cudaEventCreate(&w.ev_k[2 * w.prof_n + i]));
         CU(cudaEventRecord(w.ev_k[2 * w.prof_n], st));
     }
-    size_t smem = 0;
-    prm.ring_bytes = ring_bytes_for(tp.threads, ys_bytes, w.smem_optin, &smem);
+    const size_t smem = tp.smem;
+    prm.ring_bytes = tp.ring_bytes; prm.k_un = tp.k_un;
     if (prm.ring_bytes < kStageBytesMax) return BEAGLE_ERR_UNSUPPORTED;
     prm.queue = &w.hdr->queue;
     k_eval<<<w.num_sms, tp.threads, smem, st>>>(prm);

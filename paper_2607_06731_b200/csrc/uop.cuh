@@ -15,6 +15,7 @@
 //     x  y  DIV      ->  LX_DIVX x, y     acc = X[x] / X[y]          (both terminal: a fresh value)
 //     x  SIN         ->  LX_SIN x         acc = sin X[x]
 //     <A> <B> DIV    ->  RDIVS s          acc = slot[s] / acc        (both computed)
+//     x  SIN         ->  LS row           acc = (sin X[x]) staged once per CTA, when the row fits shared memory
 //     <A> x  DIV     ->  MULR  x          acc = acc * (1/X)[x]       (division by a variable is loop-invariant:
 //                                         when no case of x is protected, its reciprocals are a staged row)
 // and "push acc" is not a micro-op either: the micro-op that starts the next fresh value is dispatched to
@@ -59,7 +60,8 @@ enum : uint32_t {
     H_LX_ADDX = 32, H_LX_SUBX = 33, H_LX_MULX = 34, H_LX_DIVX = 35,
     H_LX_ADDC = 36, H_LX_SUBC = 37, H_LX_MULC = 38, H_LX_RSUBC = 39, H_LX_RDIVC = 40,
     H_LX_MULR = 41,                             // acc = X[colA] * (1 / X)[o]: division by a variable whose reciprocal row is staged
-    H_FRESH0 = H_LX, H_NFRESH = 17,             // the fresh-value handlers H_LX .. H_LX_MULR
+    H_LS = 42,                                  // acc = F[o]: a staged row of f(X[j]) in shared memory (f unary, loop-invariant)
+    H_FRESH0 = H_LX, H_NFRESH = 18,             // the fresh-value handlers H_LX .. H_LS
     H_PUSHT = H_NFRESH,                         // + handler: push acc to the tensor-memory slot stack first
     H_PUSHM = 2 * H_NFRESH,                     // + handler: push acc to the local slot at byte offset h[20:10] first
     H_MULR = H_FRESH0 + 3 * H_NFRESH,           // acc = acc * (1 / X)[o]
