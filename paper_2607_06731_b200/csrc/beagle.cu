@@ -53,7 +53,7 @@ struct Header {                                // device-resident results of the
 
 struct EvalParams {
     const int4* meta; const uint2* uops; const Header* hdr; unsigned int* queue;
-    const float* xt; float* fitness; float* outputs;
+    const float* xt; const float* ung; float* fitness; float* outputs;
     float tax; int n; int npad; int d; int ring_bytes;
     int rcp_col0;       // first tensor-memory column of the reciprocal rows: passes * d * 16
     int k_rcp;          // variables 0 .. k_rcp-1 have a reciprocal row (per pass)
@@ -118,7 +118,7 @@ __global__ void __launch_bounds__(1024) k_len_pass2(long long* __restrict__ bsum
                                                     int* __restrict__ bins, int* __restrict__ cursor,
                                                     int* __restrict__ binstart, long long* __restrict__ binubase,
                                                     const float* __restrict__ X, const float* __restrict__ y,
-                                                    int n, int d, int npad, float* __restrict__ xt)
+                                                    int n, int d, int npad, float* __restrict__ xt, float* __restrict__ ung)
 {
     __shared__ long long wtot[32];
     __shared__ long long carry_s;
@@ -201,6 +201,10 @@ __global__ void __launch_bounds__(1024) k_len_pass2(long long* __restrict__ bsum
         float v = 0.f;
         if (i < n) v = (j < d) ? X[(size_t)i * d + j] : (y ? y[i] : 0.f);
         xt[e] = v;
+        if (j < d) {                               // the unary rows f(X[j]) (uop.cuh H_LS / H_LG), the handlers' own functions
+            const size_t fs = (size_t)d * npad;
+            ung[e] = op_sin(v); ung[fs + e] = op_cos(v); ung[2 * fs + e] = op_log(v); ung[3 * fs + e] = op_sqrt(v); ung[4 * fs + e] = op_exp(v);
+        }
     }
 }
 
@@ -404,9 +408,10 @@ __global__ void __launch_bounds__(kCompileThreads) k_compile(const CompileParams
             const uint32_t colA = (e & LUT_CSEL_A) ? t1 : (e & LUT_CSEL_B) ? t0 : 0u;
             uint32_t h = (e & 0xFFu) + (colA << kColAShift) + ((e & LUT_PUSH) ? pb : 0u);
             if (e & LUT_SLOT) { const int s2 = c - 2; if (s2 >= S_T) { h += H_ADDM - H_ADDS; o = (uint32_t)((s2 - S_T) * 64); } }
-            if ((e & LUT_UNV) && (int)(t0 / kCasesPerLane) < q.k_un) {        // f(X[j]) = the staged row (f, j)
-                h = pb + (uint32_t)H_LS;
-                o = (uint32_t)(((int)(op - OPC_SIN) * q.k_un + (int)(t0 / kCasesPerLane)) * q.un_row_bytes);
+            if (e & LUT_UNV) {                     // f(X[j]) = the staged row (f, j): shared memory, else global
+                const int j = (int)(t0 / kCasesPerLane), f = (int)(op - OPC_SIN);
+                h = pb + (j < q.k_un ? (uint32_t)H_LS : (uint32_t)H_LG);
+                o = (uint32_t)((j < q.k_un ? f * q.k_un + j : f * q.d + j) * q.un_row_bytes);
             }
             if ((e & LUT_DIVV) && ((rcp_ok >> (o / kCasesPerLane)) & 1u))     // acc / X[o] = acc * (1/X)[o]
                 h += (e & LUT_PUSH) ? (uint32_t)(H_LX_MULR - H_LX_DIVX) : (uint32_t)(H_MULR - H_DIVX);
@@ -543,7 +548,7 @@ struct Workspace {
     int* slow_list = nullptr; long long* bsum = nullptr;
     uint2* uops = nullptr;
     int* bins = nullptr; int* cursor = nullptr; int* binstart = nullptr; long long* binubase = nullptr;
-    float* xt = nullptr; Header* hdr = nullptr; long long* h_T = nullptr;
+    float* xt = nullptr; float* ung = nullptr; Header* hdr = nullptr; long long* h_T = nullptr;
     // chunked staging
     long long stage_bytes = 0; unsigned char* stage[2] = { nullptr, nullptr };
     float* stage_consts = nullptr; long long stage_consts_cap = 0;
@@ -579,6 +584,7 @@ static beagle_status init_once()
     CU(cudaMalloc(&w.binstart, sizeof(int) * kNumBins));
     CU(cudaMalloc(&w.binubase, sizeof(long long) * kNumBins));
     CU(cudaMalloc(&w.xt, sizeof(float) * (BEAGLE_MAX_D + 1) * BEAGLE_MAX_N));
+    CU(cudaMalloc(&w.ung, sizeof(float) * 5 * BEAGLE_MAX_D * BEAGLE_MAX_N));
     CU(cudaMalloc(&w.hdr, sizeof(Header)));
     CU(cudaMemset(w.hdr, 0, sizeof(Header)));
     CU(cudaMallocHost(&w.h_T, sizeof(long long)));
@@ -694,7 +700,7 @@ static beagle_status run_prepass(const int32_t* genomes, const int32_t* lengths,
     const int nb = (int)((P + kScanThreads - 1) / kScanThreads);
     const int npad = (N + kCasePad - 1) / kCasePad * kCasePad;
     k_len_pass1<<<nb, kScanThreads, 0, st>>>(lengths, P, w.bsum, w.bins);
-    k_len_pass2<<<1, 1024, 0, st>>>(w.bsum, nb, w.hdr, w.bins, w.cursor, w.binstart, w.binubase, X, y, N, d, npad, w.xt);
+    k_len_pass2<<<1, 1024, 0, st>>>(w.bsum, nb, w.hdr, w.bins, w.cursor, w.binstart, w.binubase, X, y, N, d, npad, w.xt, w.ung);
     g_launches += 2;
     if (emit) {
         long long need = -1;
@@ -736,7 +742,7 @@ static beagle_status run_eval(const int32_t* genomes, const int32_t* lengths, co
     const TmemPlan tp = tmem_plan(N, d);
     if (!tp.fast) return BEAGLE_ERR_UNSUPPORTED;   // callers check first
     prm.rcp_col0 = tp.rcp_col0; prm.k_rcp = tp.k_rcp; prm.slot_col0 = tp.slot_col0; prm.tmem_slots = tp.tmem_slots;
-    prm.meta = w.meta; prm.uops = w.uops; prm.hdr = w.hdr; prm.xt = w.xt;
+    prm.meta = w.meta; prm.uops = w.uops; prm.hdr = w.hdr; prm.xt = w.xt; prm.ung = w.ung;
     prm.fitness = fitness; prm.outputs = outputs; prm.tax = tax; prm.n = N; prm.npad = npad; prm.d = d;
     const bool prof = g_profiling && w.prof_n < kProfMax;
     if (prof) {

@@ -144,7 +144,12 @@
     "ld.shared.v4.f32 {%0, %1, %2, %3}, [xa];\n" \
     "ld.shared.v4.f32 {%4, %5, %6, %7}, [xa+512];\n" \
     "ld.shared.v4.f32 {%8, %9, %10, %11}, [xa+1024];\n" \
-    "ld.shared.v4.f32 {%12, %13, %14, %15}, [xa+1536];\n" BGI_DISPATCH
+    "ld.shared.v4.f32 {%12, %13, %14, %15}, [xa+1536];\n" BGI_DISPATCH \
+    BGI_PUSHES(LG) "L_LG_%=:\n" "cvt.u64.u32 ma, o;\n" "add.u64 ma, ma, gb;\n" BGI_NEXT \
+    "ld.global.nc.v4.f32 {%0, %1, %2, %3}, [ma];\n" \
+    "ld.global.nc.v4.f32 {%4, %5, %6, %7}, [ma+512];\n" \
+    "ld.global.nc.v4.f32 {%8, %9, %10, %11}, [ma+1024];\n" \
+    "ld.global.nc.v4.f32 {%12, %13, %14, %15}, [ma+1536];\n" BGI_DISPATCH
 
 // ---- the dispatcher: the one indexed branch ----------------------------------------------------------------
 #define BGI_DISPATCHER \
@@ -158,7 +163,7 @@
 #define BGI_FRESH(T) \
     T(LX) T(LC) T(LX_SIN) T(LX_COS) T(LX_LOG) T(LX_SQRT) T(LX_EXP) \
     T(LX_ADDX) T(LX_SUBX) T(LX_MULX) T(LX_DIVX) \
-    T(LX_ADDC) T(LX_SUBC) T(LX_MULC) T(LX_RSUBC) T(LX_RDIVC) T(LX_MULR) T(LS)
+    T(LX_ADDC) T(LX_SUBC) T(LX_MULC) T(LX_RSUBC) T(LX_RDIVC) T(LX_MULR) T(LS) T(LG)
 #define BGI_TABLE \
     "TBL_%=: .branchtargets " \
     BGI_T(END) BGI_T(SIN) BGI_T(COS) BGI_T(LOG) BGI_T(SQRT) BGI_T(EXP) \
@@ -172,13 +177,13 @@
 #define BGI_OUT(k) "mov.f32 %" #k ", %" #k ";\n"
 
 // Operands: %0..%15 = acc (used in place), %16 = shared address of the records, %17 = xb, %18 = sb, %19 = rb, %20 = db (this lane's
-// shared-memory address of the staged unary rows of this pass).
+// shared-memory address of the staged unary rows of this pass), %21 = gb (the same in global memory).
 #define BGI_ASM \
     "{\n" \
     ".reg .f32 x<16>, t<16>, q<16>, cv;\n" \
     ".reg .pred p<16>;\n" \
     ".reg .b32 h, o, hn, pc, xa, xb, rb, db, spt, e;\n" \
-    ".reg .b64 ma, mbase;\n" \
+    ".reg .b64 ma, mbase, gb;\n" \
     ".local .align 16 .b8 slotmem[1984];\n"      /* kMemSlots * 64 */ \
     BGI_TABLE \
     "mov.u32 pc, %16;\n" \
@@ -186,6 +191,7 @@
     "mov.u32 spt, %18;\n" \
     "mov.u32 rb, %19;\n" \
     "mov.u32 db, %20;\n" \
+    "mov.u64 gb, %21;\n" \
     "mov.u64 mbase, slotmem;\n" \
     "ld.shared.v2.b32 {h, o}, [pc];\n" \
     BGI_DISPATCHER \
@@ -199,12 +205,12 @@
 namespace beagle {
 
 static_assert(kMemSlots * 64 == 1984 && kCasesPerLane == 16, "interp.cuh is written for 16 cases per lane and 31 memory slots");
-static_assert(H_COUNT == 80, "BGI_TABLE lists the handlers in the order of uop.cuh's enum");
+static_assert(H_COUNT == 83, "BGI_TABLE lists the handlers in the order of uop.cuh's enum");
 
 // acc[k] = the program's output on case (pass * 512 + (k/4)*128 + lane*4 + k%4)
-__device__ __forceinline__ void interp_run(uint32_t rec, uint32_t xb, uint32_t sb, uint32_t rb, uint32_t db, float (&acc)[16])
+__device__ __forceinline__ void interp_run(uint32_t rec, uint32_t xb, uint32_t sb, uint32_t rb, uint32_t db, const float* gb, float (&acc)[16])
 {
-    asm volatile(BGI_ASM : BGI_ACC_OUT(acc) : "r"(rec), "r"(xb), "r"(sb), "r"(rb), "r"(db) : "memory");
+    asm volatile(BGI_ASM : BGI_ACC_OUT(acc) : "r"(rec), "r"(xb), "r"(sb), "r"(rb), "r"(db), "l"(gb) : "memory");
 }
 
 } // namespace beagle

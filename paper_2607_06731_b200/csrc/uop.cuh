@@ -61,7 +61,8 @@ enum : uint32_t {
     H_LX_ADDC = 36, H_LX_SUBC = 37, H_LX_MULC = 38, H_LX_RSUBC = 39, H_LX_RDIVC = 40,
     H_LX_MULR = 41,                             // acc = X[colA] * (1 / X)[o]: division by a variable whose reciprocal row is staged
     H_LS = 42,                                  // acc = F[o]: a staged row of f(X[j]) in shared memory (f unary, loop-invariant)
-    H_FRESH0 = H_LX, H_NFRESH = 18,             // the fresh-value handlers H_LX .. H_LS
+    H_LG = 43,                                  // acc = F[o]: the same row read from global memory (L2) when shared memory is full
+    H_FRESH0 = H_LX, H_NFRESH = 19,             // the fresh-value handlers H_LX .. H_LG
     H_PUSHT = H_NFRESH,                         // + handler: push acc to the tensor-memory slot stack first
     H_PUSHM = 2 * H_NFRESH,                     // + handler: push acc to the local slot at byte offset h[20:10] first
     H_MULR = H_FRESH0 + 3 * H_NFRESH,           // acc = acc * (1 / X)[o]
