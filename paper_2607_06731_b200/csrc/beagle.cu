@@ -213,7 +213,8 @@ __global__ void __launch_bounds__(kScanThreads) k_scatter(
     const int32_t* __restrict__ lengths, long long P, const long long* __restrict__ bsum,
     const int* __restrict__ binstart, int* __restrict__ cursor, long long* __restrict__ off,
     int* __restrict__ perm, int* __restrict__ depth_out, float* __restrict__ fitness,
-    float* __restrict__ outputs, int n_cases)
+    float* __restrict__ outputs, int n_cases, const long long* __restrict__ binubase,
+    int4* __restrict__ sched, long long* __restrict__ sched_u)
 {
     __shared__ int wsum[kScanThreads / 32];
     __shared__ int cnt[kNumBins];
@@ -245,7 +246,14 @@ __global__ void __launch_bounds__(kScanThreads) k_scatter(
     for (int i = threadIdx.x; i < kNumBins; i += kScanThreads)
         if (cnt[i]) cnt[i] = atomicAdd(&cursor[i], cnt[i]);
     __syncthreads();
-    if (k >= 0) perm[binstart[k] + cnt[k] + r] = (int)p;
+    if (k >= 0) {
+        // everything the compiler's lane needs to start, at the individual's place in the sorted order
+        const int pos = binstart[k] + cnt[k] + r;
+        const long long o = bsum[blockIdx.x] + wbase + inc - len;
+        perm[pos] = (int)p;
+        sched[pos] = make_int4((int)p, len, (int)(unsigned int)o, (int)(o >> 32));
+        sched_u[pos] = binubase[k] + (long long)(cnt[k] + r) * uop_stride(len);
+    }
 }
 
 // ---- the compiler's decision table ------------------------------------------------------------------------
@@ -309,7 +317,7 @@ static void make_compile_lut(uint32_t* lut)
 //   acc always holds the topmost computed entry; the computed entry with c others below it that is not
 //   in acc sits in slot c (tensor memory while c < S_T, local memory beyond).
 struct CompileParams {
-    const uint32_t* genomes; const long long* off; const int32_t* lengths; const int* perm;
+    const uint32_t* genomes; const int4* sched; const long long* sched_u;
     const float* consts; long long n_consts; int d; int tmem_slots; int k_rcp; int k_un; int un_row_bytes;
     const int* binstart; const long long* binubase; Header* hdr;
     uint2* uops; long long ucap; int4* meta; int* depth; int* slow_list;
@@ -322,7 +330,7 @@ struct CompileParams {
 // from L1), and the walk itself is table-driven, the same straight-line code for every lane.
 constexpr int kCompBatch = 8;
 
-__global__ void __launch_bounds__(kCompileThreads) k_compile(const CompileParams q)
+__global__ void __launch_bounds__(kCompileThreads, 8) k_compile(const CompileParams q)
 {
     __shared__ uint32_t lut[kLutSize];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
@@ -333,12 +341,11 @@ __global__ void __launch_bounds__(kCompileThreads) k_compile(const CompileParams
     if (i0 >= n_sorted) return;
     const int i = i0 + lane;
     const bool valid = i < n_sorted;
-    const int p = valid ? q.perm[i] : 0;
-    const int len = valid ? q.lengths[p] : 0;
-    const long long toff = valid ? q.off[p] : 0;
-    const int bin = BEAGLE_MAX_LEN - len;
+    const int4 sc = valid ? q.sched[i] : make_int4(0, 0, 0, 0);     // k_scatter: {p, length, token offset}
+    const int p = sc.x, len = sc.y;
+    const long long toff = (long long)(((unsigned long long)(unsigned int)sc.w << 32) | (unsigned int)sc.z);
     const int stride = uop_stride(len);
-    const long long ua = valid ? q.binubase[bin] + (long long)(i - q.binstart[bin]) * stride : 0;
+    const long long ua = valid ? q.sched_u[i] : 0;
     const bool fits = ua + stride <= q.ucap;
     const bool wr = valid && q.emit && fits;
     int maxlen = len;
@@ -346,10 +353,10 @@ __global__ void __launch_bounds__(kCompileThreads) k_compile(const CompileParams
     for (int m = 16; m >= 1; m >>= 1) maxlen = max(maxlen, __shfl_xor_sync(0xffffffffu, maxlen, m));
 
     // The abstract stack. rmask / xmask are shift registers with the top of the stack at bit 0 (bit k: the
-    // entry k below the top is computed / is a variable, else a constant); t0, t1 are the values of the two
+    // entry k below the top is computed / is a variable, else a constant); t0 .. t3 are the values of the four
     // topmost entries (a variable's column or a constant's bits), the deeper ones wait in stk[].
     uint32_t stk[BEAGLE_MAX_STACK];
-    uint32_t rmask = 0, xmask = 0, t0 = 0, t1 = 0;
+    uint32_t rmask = 0, xmask = 0, t0 = 0, t1 = 0, t2 = 0, t3 = 0;
     int sp = 0, mx = 0;
     int c = 0;                                     // computed entries on the stack (the topmost one is acc)
     bool ok = valid;
@@ -432,9 +439,9 @@ __global__ void __launch_bounds__(kCompileThreads) k_compile(const CompileParams
             const bool pushT = run && isT, popB = run && isB, unU = run && isU;
             const uint32_t val = isc ? w : arg * (uint32_t)kCasesPerLane;
             if (pushT) stk[sp & 31] = val;
-            const uint32_t deeper = stk[(sp - 3) & 31];
-            t1 = pushT ? t0 : popB ? deeper : t1;
-            t0 = pushT ? val : t0;
+            const uint32_t deeper = stk[(sp - 5) & 31];        // wanted two pops from now at the earliest: its latency hides
+            const uint32_t n1 = pushT ? t0 : popB ? t2 : t1, n2 = pushT ? t1 : popB ? t3 : t2, n3 = pushT ? t2 : popB ? deeper : t3;
+            t0 = pushT ? val : t0; t1 = n1; t2 = n2; t3 = n3;
             rmask = pushT ? rmask << 1 : popB ? (rmask >> 1) | 1u : unU ? rmask | 1u : rmask;
             xmask = pushT ? (xmask << 1) | (isc ? 0u : 1u) : popB ? xmask >> 1 : xmask;
             sp += pushT ? 1 : popB ? -1 : 0;
@@ -544,7 +551,7 @@ __global__ void __launch_bounds__(1024) k_eval_blockwise(
 struct Workspace {
     long long cap_P = 0, cap_U = 0;            // individuals / micro-op entries the workspace holds
     long long promised_P = 0, promised_T = 0;  // beagle_reserve: calls with P <= promised_P have T <= promised_T
-    long long* off = nullptr; int* depth = nullptr; int* perm = nullptr; int4* meta = nullptr;
+    long long* off = nullptr; int* depth = nullptr; int* perm = nullptr; int4* meta = nullptr; int4* sched = nullptr; long long* sched_u = nullptr;
     int* slow_list = nullptr; long long* bsum = nullptr;
     uint2* uops = nullptr;
     int* bins = nullptr; int* cursor = nullptr; int* binstart = nullptr; long long* binubase = nullptr;
@@ -596,7 +603,7 @@ static beagle_status reserve_P(long long P)
     Workspace& w = g_ws;
     if (P <= w.cap_P) return BEAGLE_OK;
     CU(cudaDeviceSynchronize());
-    cudaFree(w.off); cudaFree(w.depth); cudaFree(w.perm); cudaFree(w.meta);
+    cudaFree(w.off); cudaFree(w.depth); cudaFree(w.perm); cudaFree(w.meta); cudaFree(w.sched); cudaFree(w.sched_u);
     cudaFree(w.slow_list); cudaFree(w.bsum);
     w.off = nullptr; w.depth = nullptr; w.perm = nullptr; w.meta = nullptr;
     w.slow_list = nullptr; w.bsum = nullptr; w.cap_P = 0;
@@ -604,6 +611,8 @@ static beagle_status reserve_P(long long P)
     CU(cudaMalloc(&w.off, sizeof(long long) * (P + 1)));
     CU(cudaMalloc(&w.depth, sizeof(int) * P));
     CU(cudaMalloc(&w.perm, sizeof(int) * P));
+    CU(cudaMalloc(&w.sched, sizeof(int4) * P));
+    CU(cudaMalloc(&w.sched_u, sizeof(long long) * P));
     CU(cudaMalloc(&w.meta, sizeof(int4) * P));
     CU(cudaMalloc(&w.slow_list, sizeof(int) * P));
     CU(cudaMalloc(&w.bsum, sizeof(long long) * (nb + 1)));
@@ -715,11 +724,11 @@ static beagle_status run_prepass(const int32_t* genomes, const int32_t* lengths,
         if (need > w.cap_U) { beagle_status s = reserve_U(need); if (s != BEAGLE_OK) return s; }
     }
     k_scatter<<<nb, kScanThreads, 0, st>>>(lengths, P, w.bsum, w.binstart, w.cursor, w.off, w.perm, w.depth,
-                                           fitness, outputs, N);
+                                           fitness, outputs, N, w.binubase, w.sched, w.sched_u);
     ++g_launches;
     {
         CompileParams q;
-        q.genomes = reinterpret_cast<const uint32_t*>(genomes); q.off = w.off; q.lengths = lengths; q.perm = w.perm;
+        q.genomes = reinterpret_cast<const uint32_t*>(genomes); q.sched = w.sched; q.sched_u = w.sched_u;
         const TmemPlan tp = tmem_plan(N, d);
         q.consts = consts; q.n_consts = n_consts; q.d = d; q.tmem_slots = tp.tmem_slots; q.k_rcp = tp.k_rcp; q.k_un = tp.k_un; q.un_row_bytes = npad * 4;
         q.binstart = w.binstart; q.binubase = w.binubase;
@@ -974,7 +983,7 @@ void beagle_release(void)
 {
     Workspace& w = g_ws;
     cudaDeviceSynchronize();
-    cudaFree(w.off); cudaFree(w.depth); cudaFree(w.perm); cudaFree(w.meta);
+    cudaFree(w.off); cudaFree(w.depth); cudaFree(w.perm); cudaFree(w.meta); cudaFree(w.sched); cudaFree(w.sched_u);
     cudaFree(w.slow_list); cudaFree(w.bsum); cudaFree(w.uops);
     cudaFree(w.stage[0]); cudaFree(w.stage[1]); cudaFree(w.stage_consts);
     w.off = nullptr; w.depth = nullptr; w.perm = nullptr; w.meta = nullptr;
