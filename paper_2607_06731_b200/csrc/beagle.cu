@@ -660,7 +660,7 @@ static TmemPlan tmem_plan(int N, int d)
     int wq = wq_max, k = 0, best = -1;
     for (int c = 6; c <= wq_max; ++c)
         for (int kk = 0; kk <= d; ++kk) {
-            if ((free0 - passes * kk) / c < S) break;
+            if (free0 - passes * kk < 0 || (free0 - passes * kk) / c < S) break;
             const int score = (c >= 7 ? 10000 : 0) + kk * 10 + c;
             if (score > best) { best = score; wq = c; k = kk; }
         }

@@ -253,3 +253,31 @@ def test_division_by_variable_reciprocal_rows(oracle, N):
     out = gpu_outputs(g, l, c, X)
     assert np.all(out[1, N - 1] == np.float32(1.0))          # x0 / 3e-7 is protected: 1
     assert np.all(out[2] == np.float32(1.0))                 # x0 / 0 is protected everywhere
+
+
+@pytest.mark.parametrize("N,d", [(512, 32), (1024, 16), (512, 20), (1000, 12)])
+def test_full_tensor_memory_and_deep_stacks(oracle, N, d):
+    """Shapes at the edge of the tensor-memory plan: the variable block fills all 32 rows
+    (N <= 512 with d = 32, N > 512 with d = 16: no slot row at all, every push spills to local memory), or
+    leaves only a few. Programs: right-deep chains that keep up to 31 computed values waiting, unary commands
+    and divisions on every variable (staged rows in shared memory, in global memory, or none)."""
+    from tests.gpu_util import gpu_eval
+    rng = np.random.default_rng(5)
+    X = rng.uniform(0.5, 3.0, (N, d)).astype(np.float32)
+    y = np.sin(X[:, 0]).astype(np.float32)
+    consts, progs = [], []
+    for depth in (1, 2, 3, 4, 5, 8, 16, 30):
+        # (x0*x1) (x1*x2) ... pushed one after the other, then folded from the right with alternating commands
+        parts = [f"x{k % d} x{(k + 1) % d} MUL" for k in range(depth + 1)]
+        ops = " ".join(("ADD", "SUB", "MUL", "DIV")[k % 4] for k in range(depth))
+        progs.append(asm(" ".join(parts) + " " + ops, consts)[0])
+    for j in range(d):
+        progs.append(asm(f"x{j} SIN x{j} COS ADD x{j} LOG x{j} SQRT MUL SUB x{j} 0.1 MUL EXP ADD x{(j + 1) % d} DIV", consts)[0])
+    g, l, c = pack(progs, consts)
+    a = gpu_eval(g, l, c, X, y, 0.001)
+    b = gpu_eval(g, l, c, X, y, 0.001, fn="beagle_eval_blockwise")
+    assert np.array_equal(_bits(a), _bits(b))
+    orc = oracle.evaluate(g, l, c, X, y, 0.001)
+    rep = parity.compare(a, orc)
+    assert len(rep["bad"]) == 0, parity.describe(rep, a, orc)
+    assert rep["malformed"] == 0
