@@ -281,3 +281,38 @@ def test_full_tensor_memory_and_deep_stacks(oracle, N, d):
     rep = parity.compare(a, orc)
     assert len(rep["bad"]) == 0, parity.describe(rep, a, orc)
     assert rep["malformed"] == 0
+
+
+@pytest.mark.parametrize("N,d", [(96, 2), (1024, 16)])
+def test_every_operand_kind_combination(oracle, N, d):
+    """Every case of the compiler's decision table: each binary command with each pair of operand
+    kinds (variable, constant, tiny constant, computed value), each unary command on each kind, alone and with a
+    computed value waiting underneath (the push entries; with d = 16, N = 1024 no slot row exists and every push
+    goes to local memory). Bit-identical to the blockwise kernel and within the parity rule of the oracle."""
+    from tests.gpu_util import gpu_eval
+    rng = np.random.default_rng(9)
+    X = rng.uniform(0.5, 3.0, (N, d)).astype(np.float32)
+    X[0, 1] = 0.0                                           # x1 triggers the division protection in one case
+    y = np.cos(X[:, 0]).astype(np.float32)
+    kinds = {"x": "x0", "y": "x1", "c": "1.75", "t": "3e-7", "R": "x0 x1 ADD", "S": "x1 x0 SUB"}
+    consts, progs = [], []
+    bodies = []
+    for op in ("ADD", "SUB", "MUL", "DIV"):
+        for a in kinds.values():
+            for b in kinds.values():
+                bodies.append(f"{a} {b} {op}")
+    for op in ("SIN", "COS", "LOG", "SQRT", "EXP"):
+        for a in kinds.values():
+            bodies.append(f"{a} {op}")
+    for body in bodies:
+        progs.append(asm(body, consts)[0])
+        progs.append(asm(f"x1 SIN {body} ADD", consts)[0])                       # one value waiting
+        progs.append(asm(f"x0 COS x1 SIN {body} MUL SUB", consts)[0])            # two values waiting
+    g, l, c = pack(progs, consts)
+    a = gpu_eval(g, l, c, X, y, 0.001)
+    b = gpu_eval(g, l, c, X, y, 0.001, fn="beagle_eval_blockwise")
+    assert np.array_equal(_bits(a), _bits(b))
+    orc = oracle.evaluate(g, l, c, X, y, 0.001)
+    rep = parity.compare(a, orc)
+    assert len(rep["bad"]) == 0, parity.describe(rep, a, orc)
+    assert rep["malformed"] == 0
