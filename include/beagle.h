@@ -89,6 +89,11 @@ enum {
  *   fitness_out  DEVICE  P fp32
  *   stream       cudaStream_t
  *
+ * Device resources: the interpreter kernel takes all 512 tensor-memory columns and up to 227 KB of shared
+ * memory of every SM for the duration of the call (one CTA per SM). When the fitness cases do not fit tensor
+ * memory (d > 32 at N <= 512, d > 16 at N > 512) the call runs the blockwise kernel instead: same result bit for
+ * bit, lower throughput.
+ *
  * Malformed (fitness = quiet NaN 0x7FC00000): length outside [1,512], unknown opcode, non-zero
  * arg on an operator, CONST arg >= n_consts, LOAD arg >= d, an operator that pops more than the
  * stack holds, depth above 32, (final depth is >= 1 whenever the rest holds).
