@@ -41,7 +41,10 @@
 
 /* DESIGN.md D2 (numbers retyped, not shared) */
 enum { OP_CONST = 1, OP_LOAD = 2, OP_ADD = 3, OP_SUB = 4, OP_MUL = 5, OP_DIV = 6,
-       OP_SIN = 7, OP_COS = 8, OP_LOG = 9, OP_SQRT = 10, OP_EXP = 11 };
+       OP_SIN = 7, OP_COS = 8, OP_LOG = 9, OP_SQRT = 10, OP_EXP = 11,
+       /* the rest of Table 3 in its own order from 0x10 (D2); built so far: the three
+        * stack commands and the three exact unary ones. POW 0x13 and CBRT .. PASTE 0x17-0x1E stay malformed. */
+       OP_DUP = 0x10, OP_SWAP = 0x11, OP_DEL = 0x12, OP_SIGN = 0x14, OP_SQUARE = 0x15, OP_CUBE = 0x16 };
 
 #define ORC_MAX_LEN   512
 #define ORC_MAX_STACK 32
@@ -106,13 +109,28 @@ static int check_program(const uint32_t* tok, int L, int64_t n_consts, int d) {
         case OP_ADD: case OP_SUB: case OP_MUL: case OP_DIV:
             if (arg != 0 || sp < 2) return -1; sp--; break;
         case OP_SIN: case OP_COS: case OP_LOG: case OP_SQRT: case OP_EXP:
+        case OP_SIGN: case OP_SQUARE: case OP_CUBE:
             if (arg != 0 || sp < 1) return -1; break;
+        case OP_DUP:  if (arg != 0 || sp < 1) return -1; sp++; break;       /* P:221 */
+        case OP_SWAP: if (arg != 0 || sp < 2) return -1; break;             /* P:225 */
+        case OP_DEL:  if (arg != 0 || sp < 1) return -1; sp--; break;       /* P:226 */
         default: return -1;
         }
         if (sp > ORC_MAX_STACK) return -1;
         if (sp > mx) mx = sp;
     }
     return sp >= 1 ? mx : -1;
+}
+
+/* a * b with its bound (P:235); also the two products of CUBE and the one of SQUARE. */
+static pair mul_pair(pair a, pair b, const orc_contract* c, int mirror, int* flags) {
+    double v = a.v * b.v;
+    if ((isinf(a.v) && !isnan(b.v) && !isinf(b.v) && fabs(b.v) <= b.e) ||
+        (isinf(b.v) && !isnan(a.v) && !isinf(a.v) && fabs(a.v) <= a.e))
+        *flags |= ORC_FLAG_CLASS_UNSTABLE;     /* inf * (maybe zero, sign unknown) */
+    double e1 = fabs(a.v) * b.e + fabs(b.v) * a.e + a.e * b.e;
+    if (isnan(e1)) e1 = 0.0;                   /* inf * 0 inside the bound only    */
+    return finish(v, e1 + c->c_mul * U32 * (fabs(v) + e1) + c->abs_floor, mirror, flags);
 }
 
 /* One program on one case: PAPER.md:184 stack semantics, Table 3 operand order, D2 values. */
@@ -132,16 +150,18 @@ static pair run_case(const uint32_t* tok, int L, const float* consts, const floa
             double e1 = a.e + b.e;
             st[sp - 2] = finish(v, e1 + c->c_add * U32 * (fabs(v) + e1) + fl, mirror, flags);
             sp--; break; }
-        case OP_MUL: {                                                     /* P:235 */
-            pair a = st[sp - 2], b = st[sp - 1];
-            double v = a.v * b.v;
-            if ((isinf(a.v) && !isnan(b.v) && !isinf(b.v) && fabs(b.v) <= b.e) ||
-                (isinf(b.v) && !isnan(a.v) && !isinf(a.v) && fabs(a.v) <= a.e))
-                *flags |= ORC_FLAG_CLASS_UNSTABLE;     /* inf * (maybe zero, sign unknown) */
-            double e1 = fabs(a.v) * b.e + fabs(b.v) * a.e + a.e * b.e;
-            if (isnan(e1)) e1 = 0.0;                   /* inf * 0 inside the bound only    */
-            st[sp - 2] = finish(v, e1 + c->c_mul * U32 * (fabs(v) + e1) + fl, mirror, flags);
-            sp--; break; }
+        case OP_MUL:                                                       /* P:235 */
+            st[sp - 2] = mul_pair(st[sp - 2], st[sp - 1], c, mirror, flags);
+            sp--; break;
+        case OP_DUP:  st[sp] = st[sp - 1]; sp++; break;                    /* P:221: the two top-most are identical */
+        case OP_SWAP: { pair b = st[sp - 1]; st[sp - 1] = st[sp - 2]; st[sp - 2] = b; break; }   /* P:225 */
+        case OP_DEL:  sp--; break;                                         /* P:226: pops the stack */
+        case OP_SIGN: st[sp - 1].v = -st[sp - 1].v; break;                 /* P:243: changes the sign; exact */
+        case OP_SQUARE: st[sp - 1] = mul_pair(st[sp - 1], st[sp - 1], c, mirror, flags); break;   /* P:245: a * a */
+        case OP_CUBE: {                                                    /* P:246: (a * a) * a, two products */
+            pair a = st[sp - 1];
+            st[sp - 1] = mul_pair(mul_pair(a, a, c, mirror, flags), a, c, mirror, flags);
+            break; }
         case OP_DIV: {                         /* P:238; protected form D2: |b|<EPS ? 1 : a/b */
             pair a = st[sp - 2], b = st[sp - 1];
             double ab = fabs(b.v), v, e = 0.0;

@@ -19,7 +19,8 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 _SRC = os.path.join(_HERE, "gen.c")
 _LIB = os.path.join(_HERE, "libcolony_gen.so")
 
-OP = dict(CONST=1, LOAD=2, ADD=3, SUB=4, MUL=5, DIV=6, SIN=7, COS=8, LOG=9, SQRT=10, EXP=11)
+OP = dict(CONST=1, LOAD=2, ADD=3, SUB=4, MUL=5, DIV=6, SIN=7, COS=8, LOG=9, SQRT=10, EXP=11,
+          DUP=0x10, SWAP=0x11, DEL=0x12, SIGN=0x14, SQUARE=0x15, CUBE=0x16)
 OP_NAME = {v: k for k, v in OP.items()}
 
 
@@ -219,7 +220,7 @@ def generate_programs(cfg: ColonyConfig, P: int | None = None, seed_offset: int 
 
 def colony_stats(tokens, lengths):
     ops = (tokens & 0xFF).astype(np.int64)
-    hist = np.bincount(ops, minlength=16)[:16]
+    hist = np.bincount(ops, minlength=32)[:32]
     T = int(tokens.shape[0])
     chk = int(np.bitwise_xor.reduce(
         (tokens.astype(np.uint32).astype(np.uint64) + np.arange(T, dtype=np.uint64))

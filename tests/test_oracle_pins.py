@@ -379,3 +379,121 @@ def test_parallel_fanout_equals_single_thread(oracle):
     b = oracle.evaluate_parallel(col.genomes, col.lengths, col.consts, col.X, col.y, col.tax, threads=4)
     for k in ("fitness", "bound", "flags", "depth"):
         assert np.array_equal(a[k], b[k], equal_nan=True)
+
+
+# ---- P13-P15: the rest of GCL built so far: DUP SWAP DEL SIGN SQUARE CUBE ----------
+def _quadratic_cases(seed, n=512):
+    rng = np.random.default_rng(seed)
+    X = np.empty((n, 3), np.float32)
+    X[:, 0] = rng.uniform(0.5, 2, n) * rng.choice([-1, 1], n)
+    X[:, 1] = rng.uniform(4, 8, n)
+    X[:, 2] = rng.uniform(-1, 1, n)
+    return X
+
+
+@pytest.mark.parametrize("row", [2, 3])
+def test_P13_paper_genomes_verbatim_are_the_quadratic_formula(oracle, row):
+    """The 24- and 25-command genomes the paper prints (ASR 1.0 on its QuadraticEq setup, P:314,
+    P:322) run verbatim, DUP / DEL / SQUARE included, and equal (sqrt(b^2 - 4ac) - b) / (2a): a closed form that
+    pins what DUP duplicates, what DEL removes and the operand order around them. The leading 'CONST CONST CONST
+    ADD DEL' of the first and 'CONST 3; CONST 4; SUB; CONST e; SUB; DUP; DIV; DEL' of the second are dead code."""
+    cite, n, text = _golden()[row]
+    prog, c = asm(_gcl_to_asm(text))
+    assert len(prog) == n
+    X = _quadratic_cases(13 + row)
+    a, b, cc = (X[:, j].astype(np.float64) for j in range(3))
+    root = (np.sqrt(b * b - 4 * a * cc) - b) / (2 * a)
+    r = ev(oracle, [prog], c, X, root.astype(np.float32), want_outputs=True)
+    if row == 2:      # b + (-0) is b; (b*b) - ((a+a)+(a+a))*c
+        np.testing.assert_allclose(r["outputs"][0], root, rtol=1e-13)
+    else:             # (c*a*-2) doubled is -4ac; added to b^2
+        np.testing.assert_allclose(r["outputs"][0], root, rtol=1e-13)
+    o = r["outputs"][0]
+    assert np.max(np.abs(a * o * o + b * o + cc)) < 1e-9          # it is a root, whatever the formula above says
+    assert r["depth"][0] >= 3 and not (r["flags"][0] & oracle.FLAG_MALFORMED)
+
+
+def test_P14_stack_command_identities(oracle):
+    rng = np.random.default_rng(14)
+    X = rng.uniform(-3, 3, (64, 2)).astype(np.float32)
+    y = np.zeros(64, np.float32)
+    A, B = "x0 x1 MUL 1.5 ADD", "x1 SIN x0 SUB"
+    pairs = [
+        (f"{A} DUP DEL", A),                          # a duplicate removed again
+        (f"{A} {B} SWAP SWAP", f"{A} {B}"),           # two swaps undo each other (output = top)
+        (f"{A} {B} SWAP SUB", f"{B} {A} SUB"),        # SWAP exchanges the operands of SUB
+        (f"{A} {B} SWAP DIV", f"{B} {A} DIV"),
+        (f"{A} DUP MUL", f"{A} SQUARE"),              # SQUARE is a * a
+        (f"{A} {A} MUL", f"{A} SQUARE"),
+        (f"{A} DUP DUP MUL MUL", f"{A} CUBE"),        # CUBE is (a * a) * a; the product commutes bit for bit
+        (f"{A} SIGN SIGN", A),
+        (f"{A} {B} DEL", A),                          # a deleted value is dead code
+        (f"x0 DEL {A}", A),                           # depth may touch zero in between
+        (f"{A} {B} DUP DEL ADD", f"{A} {B} ADD"),
+    ]
+    for left, right in pairs:
+        consts = []
+        pl, pr = asm(left, consts)[0], asm(right, consts)[0]
+        r = ev(oracle, [pl, pr], np.array(consts, np.float32), X, y, want_outputs=True, mode=1)
+        assert np.array_equal(r["outputs"][0], r["outputs"][1]), (left, right)
+    # SIGN is 0 - a (as values: the sign of a zero aside)
+    consts = []
+    r = ev(oracle, [asm(f"{A} SIGN", consts)[0], asm(f"0 {A} SUB", consts)[0]], np.array(consts, np.float32), X, y,
+           want_outputs=True)
+    assert np.all(r["outputs"][0] == r["outputs"][1])
+    # the tax counts every command, stack commands included (P:314)
+    consts = []
+    r = ev(oracle, [asm(A, consts)[0], asm(f"{A} DUP DEL", consts)[0]], np.array(consts, np.float32), X, y, tax=0.25)
+    assert r["fitness"][1] - r["fitness"][0] == pytest.approx(0.5, rel=1e-6)
+
+
+def test_P15_stack_command_well_formedness(oracle):
+    X = np.ones((4, 2), np.float32)
+    y = np.zeros(4, np.float32)
+    T = C.token
+    x0, x1 = T(C.OP["LOAD"], 0), T(C.OP["LOAD"], 1)
+    bad = [
+        np.array([T(C.OP["DUP"])], np.int32),                         # nothing to duplicate
+        np.array([x0, T(C.OP["SWAP"])], np.int32),                    # SWAP needs two
+        np.array([T(C.OP["DEL"])], np.int32),
+        np.array([x0, T(C.OP["DEL"])], np.int32),                     # ends with an empty stack
+        np.array([x0, T(C.OP["DUP"], 1)], np.int32),                  # operator with an argument
+        np.array([x0] + [T(C.OP["DUP"])] * 32, np.int32),             # depth 33
+        np.array([x0, T(0x13)], np.int32),                            # POW: reserved, not built yet
+        np.array([x0, T(0x17)], np.int32),                            # CBRT: reserved
+    ]
+    good = [np.array([x0] + [T(C.OP["DUP"])] * 31 + [T(C.OP["ADD"])] * 31, np.int32),   # depth 32: 32 * x0
+            np.array([x0, T(C.OP["DEL"]), x1, T(C.OP["SQUARE"])], np.int32)]
+    r = ev(oracle, bad + good, np.zeros(1, np.float32), X, y)
+    assert np.all(r["fitness"][:len(bad)].view(np.uint32) == QNAN_BITS)
+    assert np.all(r["flags"][:len(bad)] & oracle.FLAG_MALFORMED)
+    assert r["fitness"][len(bad)] == 32.0 ** 2 and r["depth"][len(bad)] == 32
+    assert r["fitness"][len(bad) + 1] == 1.0
+
+
+def test_P11b_bound_holds_with_the_new_commands(oracle):
+    """|fit64 - fit32mirror| <= E_p on random programs that use the stack commands and SIGN SQUARE CUBE."""
+    rng = np.random.default_rng(15)
+    X = rng.uniform(-2, 2, (128, 3)).astype(np.float32)
+    y = (X[:, 0] * X[:, 1]).astype(np.float32)
+    names = ["ADD", "SUB", "MUL", "DIV", "SIN", "COS", "SQRT", "SIGN", "SQUARE", "CUBE", "DUP", "SWAP", "DEL"]
+    progs, consts = [], []
+    while len(progs) < 400:
+        toks, depth = [], 0
+        for _ in range(int(rng.integers(3, 40))):
+            nm = names[int(rng.integers(len(names)))]
+            need = 2 if nm in ("ADD", "SUB", "MUL", "DIV", "SWAP") else 1
+            if depth < need or (nm == "DUP" and depth >= 8) or rng.random() < 0.35:
+                toks.append(f"x{int(rng.integers(3))}" if rng.random() < 0.8 else f"{rng.uniform(-3, 3):.4f}"); depth += 1
+            else:
+                toks.append(nm); depth += {"DUP": 1, "DEL": -1}.get(nm, -1 if need == 2 and nm != "SWAP" else 0)
+        if depth >= 1:
+            progs.append(asm(" ".join(toks), consts)[0])
+    c = np.array(consts, np.float32)
+    t = ev(oracle, progs, c, X, y, contract_=oracle.contract(oracle.CONTRACT_IEEE))
+    m = ev(oracle, progs, c, X, y, contract_=oracle.contract(oracle.CONTRACT_IEEE), mode=1)
+    assert not np.any(t["flags"] & oracle.FLAG_MALFORMED)
+    fin = np.isfinite(t["fitness"]) & np.isfinite(m["fitness"]) & ((t["flags"] & 6) == 0)
+    assert fin.sum() > 200
+    diff = np.abs(t["fitness"].astype(np.float64) - m["fitness"].astype(np.float64))
+    assert np.all(diff[fin] <= t["bound"][fin] + 1e-30)
