@@ -47,8 +47,17 @@ extern "C" {
 #define BEAGLE_OP_LOG   0x09 /* a -> |a| < 1e-6f ? 0 : ln|a|    (protected) PAPER.md:253     */
 #define BEAGLE_OP_SQRT  0x0A /* a -> sqrt|a|                    (protected) PAPER.md:249     */
 #define BEAGLE_OP_EXP   0x0B /* a -> exp(a > 80 ? 80 : a)       (clamped)     */
-/* 0x10..0x1E are reserved for the rest of Table 3 (DUP SWAP DEL POW SIGN SQUARE CUBE CBRT TAN
- * ARCSIN ARCCOS ARCTAN TANH COPY PASTE); until implemented they make a program malformed.      */
+/* The rest of Table 3 in its own order from 0x10. Built: the stack commands and the exact unary ones. An
+ * individual that uses one of them is evaluated by the blockwise kernel inside the same call (same definition,
+ * same summation order, lower throughput); the interpreter's micro-ops cover the eleven commands above.         */
+#define BEAGLE_OP_DUP    0x10 /* a -> a a     */
+#define BEAGLE_OP_SWAP   0x11 /* a b -> b a     */
+#define BEAGLE_OP_DEL    0x12 /* a ->     */
+#define BEAGLE_OP_SIGN   0x14 /* a -> -a     */
+#define BEAGLE_OP_SQUARE 0x15 /* a -> a * a     */
+#define BEAGLE_OP_CUBE   0x16 /* a -> (a * a) * a     */
+/* 0x13 POW and 0x17..0x1E (CBRT TAN ARCSIN ARCCOS ARCTAN TANH COPY PASTE) are reserved; until implemented
+ * they make a program malformed.                                                                */
 #define BEAGLE_TOKEN(op, arg) ((int32_t)(((uint32_t)(arg) << 8) | ((uint32_t)(op) & 0xFFu)))
 
 /* ---- limits (also returned by beagle_limits) ---- */
@@ -95,8 +104,8 @@ enum {
  * bit, lower throughput.
  *
  * Malformed (fitness = quiet NaN 0x7FC00000): length outside [1,512], unknown opcode, non-zero
- * arg on an operator, CONST arg >= n_consts, LOAD arg >= d, an operator that pops more than the
- * stack holds, depth above 32, (final depth is >= 1 whenever the rest holds).
+ * arg on an operator, CONST arg >= n_consts, LOAD arg >= d, a command that needs more entries than the
+ * stack holds, depth above 32, an empty stack at the end (DEL can empty it in between).
  * The extent of `genomes` is trusted to be sum of the in-range lengths.                          */
 beagle_status beagle_eval(const int32_t* genomes, const int32_t* lengths, int64_t P,
                           const float* consts, int64_t n_consts,

@@ -25,7 +25,9 @@ namespace beagle {
 enum : uint32_t { OPC_CONST = BEAGLE_OP_CONST, OPC_LOAD = BEAGLE_OP_LOAD, OPC_ADD = BEAGLE_OP_ADD,
                   OPC_SUB = BEAGLE_OP_SUB, OPC_MUL = BEAGLE_OP_MUL, OPC_DIV = BEAGLE_OP_DIV,
                   OPC_SIN = BEAGLE_OP_SIN, OPC_COS = BEAGLE_OP_COS, OPC_LOG = BEAGLE_OP_LOG,
-                  OPC_SQRT = BEAGLE_OP_SQRT, OPC_EXP = BEAGLE_OP_EXP };
+                  OPC_SQRT = BEAGLE_OP_SQRT, OPC_EXP = BEAGLE_OP_EXP,
+                  OPC_DUP = BEAGLE_OP_DUP, OPC_SWAP = BEAGLE_OP_SWAP, OPC_DEL = BEAGLE_OP_DEL,
+                  OPC_SIGN = BEAGLE_OP_SIGN, OPC_SQUARE = BEAGLE_OP_SQUARE, OPC_CUBE = BEAGLE_OP_CUBE };
 
 constexpr int kNumBins = BEAGLE_MAX_LEN + 1;   // bin = 512 - length  (longest first); bin 512 unused
 constexpr int kScanThreads = 256;              // programs per block in the pre-pass
@@ -359,7 +361,7 @@ __global__ void __launch_bounds__(kCompileThreads, 8) k_compile(const CompilePar
     uint32_t rmask = 0, xmask = 0, t0 = 0, t1 = 0, t2 = 0, t3 = 0;
     int sp = 0, mx = 0;
     int c = 0;                                     // computed entries on the stack (the topmost one is acc)
-    bool ok = valid;
+    bool ok = valid, slow = false;
     const int S_T = q.tmem_slots;
     // variables whose division is a multiplication by a staged reciprocal row
     const uint32_t rcp_ok = ~q.hdr->rcp_unsafe & ((q.k_rcp >= 32) ? 0xFFFFFFFFu : ((1u << q.k_rcp) - 1u));
@@ -403,10 +405,17 @@ __global__ void __launch_bounds__(kCompileThreads, 8) k_compile(const CompilePar
                                : isU ? (uint32_t)kLutUnary + ((op - OPC_SIN) << 2) + ((rmask & 1u) << 1 | (xmask & 1u)) : (uint32_t)kLutNone;
             const uint32_t e = lut[key];
             // well-formedness (D3); a CONST token that was not replaced has an index out of range
+            // DUP SWAP DEL SIGN SQUARE CUBE are checked here (stack effect, depth) but not compiled:
+            // an individual that uses one is evaluated by the blockwise kernel (slow list), the interpreter's
+            // micro-ops stay those of the eleven hot-path commands
+            const bool isK = (op - OPC_DUP) < 3u || (op - OPC_SIGN) < 3u;
+            const int kneed = op == OPC_SWAP ? 2 : 1, kpush = op == OPC_DUP ? 1 : (op == OPC_DEL ? -1 : 0);
+            const bool goodK = isK && arg == 0 && sp >= kneed && sp + kpush <= BEAGLE_MAX_STACK;
             const bool good = isT ? ((isc || (op == OPC_LOAD && (int)arg < q.d)) && sp < BEAGLE_MAX_STACK)
-                                  : ((isB || isU) && arg == 0 && sp >= (isB ? 2 : 1));
+                                  : (((isB || isU) && arg == 0 && sp >= (isB ? 2 : 1)) || goodK);
             ok = ok && (good || t >= tend);
-            const bool run = live && good;
+            const bool run = live && good && !isK;
+            if (live && goodK) { slow = true; sp += kpush; mx = max(mx, sp); }
             // the record (operand a = second from the top = t1, operand b = top = t0)
             const int s1 = c - 1;
             const uint32_t pb = (c == 0 || !(e & (LUT_PUSH | LUT_DBL))) ? 0u
@@ -465,7 +474,8 @@ __global__ void __launch_bounds__(kCompileThreads, 8) k_compile(const CompilePar
     }
     q.depth[p] = mx;
     if (!q.emit) { q.meta[i] = make_int4(p, 0, 0, len); return; }
-    if (!fits) {                                   // the workspace promise of beagle_reserve was broken: slow path
+    if (!fits || slow) {                           // the workspace promise of beagle_reserve was broken, or a command
+                                                   // beyond the interpreter's eleven: the blockwise kernel takes it
         q.slow_list[atomicAdd(&q.hdr->n_slow, 1)] = p;
         q.meta[i] = make_int4(p, 0, 0, len);
         return;
@@ -521,6 +531,12 @@ __global__ void __launch_bounds__(1024) k_eval_blockwise(
                 case OPC_LOG: st[sp - 1] = op_log(st[sp - 1]); break;
                 case OPC_SQRT: st[sp - 1] = op_sqrt(st[sp - 1]); break;
                 case OPC_EXP: st[sp - 1] = op_exp(st[sp - 1]); break;
+                case OPC_SIGN: st[sp - 1] = op_sign(st[sp - 1]); break;
+                case OPC_SQUARE: st[sp - 1] = op_square(st[sp - 1]); break;
+                case OPC_CUBE: st[sp - 1] = op_cube(st[sp - 1]); break;
+                case OPC_DUP: st[sp] = st[sp - 1]; ++sp; break;
+                case OPC_SWAP: { const float b = st[sp - 1]; st[sp - 1] = st[sp - 2]; st[sp - 2] = b; break; }
+                case OPC_DEL: --sp; break;
                 default: break;
                 }
             }

@@ -42,6 +42,10 @@ __device__ __forceinline__ float op_exp(float a) {                              
     return mufu_ex2(__fmul_rn(min_nan(a, 80.0f), 1.44269504088896341f));
 }
 
+__device__ __forceinline__ float op_sign(float a) { return -a; }                                 // PAPER.md:243, exact
+__device__ __forceinline__ float op_square(float a) { return __fmul_rn(a, a); }
+__device__ __forceinline__ float op_cube(float a) { return __fmul_rn(__fmul_rn(a, a), a); }      // (a*a)*a
+
 // token fields (D1)
 __device__ __forceinline__ uint32_t tok_op(uint32_t w) { return w & 0xFFu; }
 __device__ __forceinline__ uint32_t tok_arg(uint32_t w) { return w >> 8; }

@@ -316,3 +316,72 @@ def test_every_operand_kind_combination(oracle, N, d):
     rep = parity.compare(a, orc)
     assert len(rep["bad"]) == 0, parity.describe(rep, a, orc)
     assert rep["malformed"] == 0
+
+
+def _random_gcl_programs(rng, n_prog, d, names):
+    progs_text = []
+    while len(progs_text) < n_prog:
+        toks, depth = [], 0
+        for _ in range(int(rng.integers(3, 60))):
+            nm = names[int(rng.integers(len(names)))]
+            need = 2 if nm in ("ADD", "SUB", "MUL", "DIV", "SWAP") else 1
+            if depth < need or (nm == "DUP" and depth >= 30) or rng.random() < 0.35:
+                toks.append(f"x{int(rng.integers(d))}" if rng.random() < 0.8 else f"{rng.uniform(-3, 3):.4f}"); depth += 1
+            else:
+                toks.append(nm); depth += {"DUP": 1, "DEL": -1}.get(nm, -1 if need == 2 and nm != "SWAP" else 0)
+        if depth >= 1:
+            progs_text.append(" ".join(toks))
+    return progs_text
+
+
+@pytest.mark.parametrize("N,d", [(512, 3), (1024, 9), (200, 16)])
+def test_stack_commands_and_exact_unaries(oracle, N, d):
+    """DUP SWAP DEL SIGN SQUARE CUBE (Table 3): random programs mixing them with the eleven
+    hot-path commands, and the paper's two printed genomes verbatim: bit-identical to the blockwise kernel, within
+    the parity rule of the oracle; programs of + - * SIGN SQUARE CUBE and stack commands only are bit-exact per case."""
+    from tests.gpu_util import gpu_eval, gpu_outputs
+    rng = np.random.default_rng(21)
+    X = rng.uniform(-2, 2, (N, d)).astype(np.float32)
+    y = (X[:, 0] * X[:, 1]).astype(np.float32)
+    names = ["ADD", "SUB", "MUL", "DIV", "SIN", "COS", "LOG", "SQRT", "EXP", "SIGN", "SQUARE", "CUBE", "DUP", "SWAP", "DEL"]
+    texts = _random_gcl_programs(rng, 600, d, names)
+    texts += ["0 -9.280686 8.983309 ADD DEL x1 ADD DUP MUL x0 DUP ADD DUP ADD x2 MUL SUB SQRT x1 SUB x0 DIV 0.5 MUL",
+              "x2 x0 MUL -2 MUL DUP ADD 3 4 SUB 2.7182817 SUB DUP DIV DEL x1 SQUARE ADD SQRT x1 SUB x0 DIV 0.5 MUL"]
+    consts = []
+    progs = [asm(t, consts)[0] for t in texts]
+    g, l, c = pack(progs, consts)
+    a = gpu_eval(g, l, c, X, y, 0.001)
+    b = gpu_eval(g, l, c, X, y, 0.001, fn="beagle_eval_blockwise")
+    assert np.array_equal(_bits(a), _bits(b))
+    orc = oracle.evaluate(g, l, c, X, y, 0.001)
+    rep = parity.compare(a, orc)
+    assert len(rep["bad"]) == 0, parity.describe(rep, a, orc)
+    assert rep["malformed"] == 0 and rep["strict"] > 100
+    # correctly rounded commands only: per-case outputs equal the oracle's fp32 mirror bit for bit
+    exact = _random_gcl_programs(rng, 200, d, ["ADD", "SUB", "MUL", "SIGN", "SQUARE", "CUBE", "DUP", "SWAP", "DEL"])
+    consts2 = []
+    progs2 = [asm(t, consts2)[0] for t in exact]
+    g2, l2, c2 = pack(progs2, consts2)
+    out = gpu_outputs(g2, l2, c2, X)
+    mir = oracle.evaluate(g2, l2, c2, X, y, 0.0, mode=1, want_outputs=True, contract_=oracle.contract(oracle.CONTRACT_IEEE))
+    want = mir["outputs"].astype(np.float32)
+    same = (out.view(np.uint32) == want.view(np.uint32)) | (np.isnan(out) & np.isnan(want)) | ((out == 0) & (want == 0))
+    assert np.all(same)
+
+
+def test_stack_command_malformed_programs(oracle):
+    from tests.gpu_util import gpu_eval
+    T = token
+    x0 = T(OP["LOAD"], 0)
+    progs = [np.array([T(OP["DUP"])], np.int32), np.array([x0, T(OP["SWAP"])], np.int32),
+             np.array([x0, T(OP["DEL"])], np.int32), np.array([x0] + [T(OP["DUP"])] * 32, np.int32),
+             np.array([x0, T(0x13)], np.int32), np.array([x0, T(OP["SQUARE"], 3)], np.int32),
+             np.array([x0] + [T(OP["DUP"])] * 31 + [T(OP["ADD"])] * 31, np.int32),      # well-formed: depth 32
+             np.array([x0, T(OP["DEL"]), x0, T(OP["CUBE"])], np.int32)]                 # well-formed
+    g, l, c = pack(progs, np.zeros(1, np.float32))
+    X = np.full((64, 1), 2.0, np.float32); y = np.zeros(64, np.float32)
+    a = gpu_eval(g, l, c, X, y, 0.0)
+    assert np.all(_bits(a[:6]) == QNAN)
+    assert a[6] == np.float32(64.0 ** 2) and a[7] == np.float32(64.0)
+    orc = oracle.evaluate(g, l, c, X, y, 0.0)
+    assert len(parity.compare(a, orc)["bad"]) == 0
