@@ -100,6 +100,7 @@ class ClockSampler:
 
     def __init__(self, gpu_index: int):
         self.p = None
+        self.gpu_index = gpu_index
         try:
             self.p = subprocess.Popen(["nvidia-smi", f"--id={gpu_index}", f"--query-gpu={self.Q}",
                                        "--format=csv,noheader,nounits", "-lms", "20"],
@@ -129,8 +130,24 @@ class ClockSampler:
             for n, v in zip(names, f[3:7]):
                 if v.lower().startswith("active"):
                     reasons.add(n)
-        return {"sm_mhz": statistics.median(sm) if sm else None, "sm_max_mhz": max(mx) if mx else None,
-                "samples": len(sm), "reasons": sorted(reasons)}
+        note = None
+        if not sm:          # the timed region was shorter than one sampling period: one query right after it
+            try:
+                out = subprocess.run(["nvidia-smi", f"--id={self.gpu_index}", f"--query-gpu={self.Q}",
+                                      "--format=csv,noheader,nounits"], capture_output=True, text=True, timeout=10).stdout
+                f = [x.strip() for x in out.strip().splitlines()[0].split(",")]
+                sm.append(float(f[0])); mx.append(float(f[1]))
+                for n, v in zip(names, f[3:7]):
+                    if v.lower().startswith("active"):
+                        reasons.add(n)
+                note = "timed region shorter than the sampling period: one query right after it"
+            except Exception:
+                pass
+        r = {"sm_mhz": statistics.median(sm) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+             "samples": len(sm), "reasons": sorted(reasons)}
+        if note:
+            r["note"] = note
+        return r
 
 
 # ------------------------------------------------------------------------------------------------

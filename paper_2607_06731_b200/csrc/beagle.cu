@@ -405,17 +405,19 @@ __global__ void __launch_bounds__(kCompileThreads, 8) k_compile(const CompilePar
                                : isU ? (uint32_t)kLutUnary + ((op - OPC_SIN) << 2) + ((rmask & 1u) << 1 | (xmask & 1u)) : (uint32_t)kLutNone;
             const uint32_t e = lut[key];
             // well-formedness (D3); a CONST token that was not replaced has an index out of range
-            // DUP SWAP DEL SIGN SQUARE CUBE are checked here (stack effect, depth) but not compiled:
-            // an individual that uses one is evaluated by the blockwise kernel (slow list), the interpreter's
-            // micro-ops stay those of the eleven hot-path commands
-            const bool isK = (op - OPC_DUP) < 3u || (op - OPC_SIGN) < 3u;
-            const int kneed = op == OPC_SWAP ? 2 : 1, kpush = op == OPC_DUP ? 1 : (op == OPC_DEL ? -1 : 0);
-            const bool goodK = isK && arg == 0 && sp >= kneed && sp + kpush <= BEAGLE_MAX_STACK;
             const bool good = isT ? ((isc || (op == OPC_LOAD && (int)arg < q.d)) && sp < BEAGLE_MAX_STACK)
-                                  : (((isB || isU) && arg == 0 && sp >= (isB ? 2 : 1)) || goodK);
-            ok = ok && (good || t >= tend);
-            const bool run = live && good && !isK;
-            if (live && goodK) { slow = true; sp += kpush; mx = max(mx, sp); }
+                                  : ((isB || isU) && arg == 0 && sp >= (isB ? 2 : 1));
+            bool bad = live && !good;
+            if (bad) {
+                // not one of the eleven hot-path commands (rare, off the straight-line path). DUP SWAP DEL SIGN SQUARE
+                // CUBE are checked here (stack effect, depth) but not compiled: an individual that uses
+                // one is evaluated by the blockwise kernel (slow list)
+                const bool isK = (op - OPC_DUP) < 3u || (op - OPC_SIGN) < 3u;
+                const int kneed = op == OPC_SWAP ? 2 : 1, kpush = op == OPC_DUP ? 1 : (op == OPC_DEL ? -1 : 0);
+                if (isK && arg == 0 && sp >= kneed && sp + kpush <= BEAGLE_MAX_STACK) { slow = true; sp += kpush; mx = max(mx, sp); bad = false; }
+            }
+            ok = ok && !bad;
+            const bool run = live && good;
             // the record (operand a = second from the top = t1, operand b = top = t0)
             const int s1 = c - 1;
             const uint32_t pb = (c == 0 || !(e & (LUT_PUSH | LUT_DBL))) ? 0u
