@@ -312,16 +312,17 @@ static void make_compile_lut(uint32_t* lut)
 }
 
 // ---- a3/a5: the tree compiler ----------------------------------------------------------------------------
-// One thread per individual, in length-sorted order (the threads of a warp run programs of equal
-// length). One walk over the postfix program with an abstract stack whose entries are either a
-// terminal that has not been evaluated yet (its token is kept) or "computed": well-formedness
+// One lane per individual, in length-sorted order (the lanes of a warp run programs of equal length; k_scatter
+// left each lane's start record: index, length, token offset, record base). One walk over the postfix program
+// with an abstract stack whose entries are either a terminal that has not been evaluated yet (its value is
+// kept) or "computed": well-formedness
 // (D3) and the micro-ops of uop.cuh, in the program's own evaluation order.
 //   acc always holds the topmost computed entry; the computed entry with c others below it that is not
 //   in acc sits in slot c (tensor memory while c < S_T, local memory beyond).
 struct CompileParams {
     const uint32_t* genomes; const int4* sched; const long long* sched_u;
     const float* consts; long long n_consts; int d; int tmem_slots; int k_rcp; int k_un; int un_row_bytes;
-    const int* binstart; const long long* binubase; Header* hdr;
+    Header* hdr;
     uint2* uops; long long ucap; int4* meta; int* depth; int* slow_list;
     float* fitness; float* outputs; int n_cases; int emit;
 };
@@ -749,7 +750,6 @@ static beagle_status run_prepass(const int32_t* genomes, const int32_t* lengths,
         q.genomes = reinterpret_cast<const uint32_t*>(genomes); q.sched = w.sched; q.sched_u = w.sched_u;
         const TmemPlan tp = tmem_plan(N, d);
         q.consts = consts; q.n_consts = n_consts; q.d = d; q.tmem_slots = tp.tmem_slots; q.k_rcp = tp.k_rcp; q.k_un = tp.k_un; q.un_row_bytes = npad * 4;
-        q.binstart = w.binstart; q.binubase = w.binubase;
         q.hdr = w.hdr; q.uops = w.uops; q.ucap = w.cap_U; q.meta = w.meta; q.depth = w.depth;
         q.slow_list = w.slow_list; q.fitness = fitness; q.outputs = outputs; q.n_cases = N; q.emit = emit ? 1 : 0;
         k_compile<<<(unsigned)((P + kCompileThreads - 1) / kCompileThreads), kCompileThreads, 0, st>>>(q);
