@@ -43,8 +43,11 @@
 enum { OP_CONST = 1, OP_LOAD = 2, OP_ADD = 3, OP_SUB = 4, OP_MUL = 5, OP_DIV = 6,
        OP_SIN = 7, OP_COS = 8, OP_LOG = 9, OP_SQRT = 10, OP_EXP = 11,
        /* the rest of Table 3 in its own order from 0x10 (D2); built so far: the three
-        * stack commands and the three exact unary ones. POW 0x13 and CBRT .. PASTE 0x17-0x1E stay malformed. */
-       OP_DUP = 0x10, OP_SWAP = 0x11, OP_DEL = 0x12, OP_SIGN = 0x14, OP_SQUARE = 0x15, OP_CUBE = 0x16 };
+        * stack commands, the three exact unary ones and six more unary functions. POW 0x13, COPY 0x1D and PASTE 0x1E
+        * stay malformed. */
+       OP_DUP = 0x10, OP_SWAP = 0x11, OP_DEL = 0x12, OP_SIGN = 0x14, OP_SQUARE = 0x15, OP_CUBE = 0x16,
+       /* unprotected, as the paper's are: plain mathematical functions, NaN outside their domain */
+       OP_CBRT = 0x17, OP_TAN = 0x18, OP_ARCSIN = 0x19, OP_ARCCOS = 0x1A, OP_ARCTAN = 0x1B, OP_TANH = 0x1C };
 
 #define ORC_MAX_LEN   512
 #define ORC_MAX_STACK 32
@@ -74,6 +77,7 @@ typedef struct {
     double abs_floor;    /* every computed op: absolute (denormal results flushed), NOT in u  */
     double sum_per_case; /* summation: the fp32 sum of N squares is off by at most            */
     double sum_const;    /*   (sum_per_case * N + sum_const) * u * S  (depth of the add tree) */
+    double c_fun[6];     /* CBRT TAN ARCSIN ARCCOS ARCTAN TANH: relative                      */
 } orc_contract;
 
 static const double U32 = 5.9604644775390625e-08; /* 2^-24 */
@@ -110,6 +114,7 @@ static int check_program(const uint32_t* tok, int L, int64_t n_consts, int d) {
             if (arg != 0 || sp < 2) return -1; sp--; break;
         case OP_SIN: case OP_COS: case OP_LOG: case OP_SQRT: case OP_EXP:
         case OP_SIGN: case OP_SQUARE: case OP_CUBE:
+        case OP_CBRT: case OP_TAN: case OP_ARCSIN: case OP_ARCCOS: case OP_ARCTAN: case OP_TANH:
             if (arg != 0 || sp < 1) return -1; break;
         case OP_DUP:  if (arg != 0 || sp < 1) return -1; sp++; break;       /* P:221 */
         case OP_SWAP: if (arg != 0 || sp < 2) return -1; break;             /* P:225 */
@@ -131,6 +136,37 @@ static pair mul_pair(pair a, pair b, const orc_contract* c, int mirror, int* fla
     double e1 = fabs(a.v) * b.e + fabs(b.v) * a.e + a.e * b.e;
     if (isnan(e1)) e1 = 0.0;                   /* inf * 0 inside the bound only    */
     return finish(v, e1 + c->c_mul * U32 * (fabs(v) + e1) + c->abs_floor, mirror, flags);
+}
+
+/* CBRT TAN ARCSIN ARCCOS ARCTAN TANH: the plain function; each is monotone on every interval of
+ * its domain, so the input's uncertainty maps to max |f(a +- e) - f(a)|. An interval that reaches past the domain of
+ * ARCSIN / ARCCOS, or across a pole of TAN, makes the individual UNSTABLE.                                          */
+static double fun_eval(uint32_t op, double a) {
+    switch (op) {
+    case OP_CBRT: return cbrt(a);
+    case OP_TAN: return tan(a);
+    case OP_ARCSIN: return asin(a);
+    case OP_ARCCOS: return acos(a);
+    case OP_ARCTAN: return atan(a);
+    default: return tanh(a);
+    }
+}
+static pair fun_pair(uint32_t op, pair a, const orc_contract* c, int mirror, int* flags) {
+    double v = fun_eval(op, a.v), e = 0.0;
+    if (!isnan(a.v) && !isinf(a.v) && !isnan(v)) {
+        double lo = a.v - a.e, hi = a.v + a.e;
+        if (op == OP_ARCSIN || op == OP_ARCCOS) {
+            if (lo < -1.0 || hi > 1.0) { *flags |= ORC_FLAG_UNSTABLE; lo = fmax(lo, -1.0); hi = fmin(hi, 1.0); }
+        } else if (op == OP_TAN) {
+            const double pi = 3.14159265358979323846;
+            if (floor(lo / pi + 0.5) != floor(hi / pi + 0.5)) { *flags |= ORC_FLAG_UNSTABLE; lo = hi = a.v; }
+        }
+        double e1 = fmax(fabs(fun_eval(op, lo) - v), fabs(fun_eval(op, hi) - v));
+        if (isnan(e1)) e1 = 0.0;
+        e = e1 + c->c_fun[op - OP_CBRT] * U32 * (fabs(v) + e1) + c->abs_floor;
+    } else if (isnan(v) && !isnan(a.v) && (fabs(a.v) - a.e <= 1.0) && (op == OP_ARCSIN || op == OP_ARCCOS))
+        *flags |= ORC_FLAG_UNSTABLE;           /* outside the domain, but the interval reaches into it */
+    return finish(v, e, mirror, flags);
 }
 
 /* One program on one case: PAPER.md:184 stack semantics, Table 3 operand order, D2 values. */
@@ -158,6 +194,8 @@ static pair run_case(const uint32_t* tok, int L, const float* consts, const floa
         case OP_DEL:  sp--; break;                                         /* pops the stack */
         case OP_SIGN: st[sp - 1].v = -st[sp - 1].v; break;                 /* changes the sign; exact */
         case OP_SQUARE: st[sp - 1] = mul_pair(st[sp - 1], st[sp - 1], c, mirror, flags); break;   /* a * a */
+        case OP_CBRT: case OP_TAN: case OP_ARCSIN: case OP_ARCCOS: case OP_ARCTAN: case OP_TANH:
+            st[sp - 1] = fun_pair(op, st[sp - 1], c, mirror, flags); break;
         case OP_CUBE: {                                                    /* (a * a) * a, two products */
             pair a = st[sp - 1];
             st[sp - 1] = mul_pair(mul_pair(a, a, c, mirror, flags), a, c, mirror, flags);
@@ -298,6 +336,7 @@ void orc_default_contract(int which, orc_contract* c) {
         c->c_log_rel = 1.001; c->c_log_abs = 0.0; c->c_sin_abs = 1.001; c->c_sin_arg = 0.0;
         c->abs_floor = 1.5e-45;
         c->sum_per_case = 1.0; c->sum_const = 0.0;   /* any summation order */
+        for (int k = 0; k < 6; ++k) c->c_fun[k] = 1.001;
     } else {
         c->c_add = 1.0; c->c_mul = 1.0;
         c->c_div = 3.5; c->div_bigb_abs = 1.1754943508222875e-38;
@@ -307,5 +346,7 @@ void orc_default_contract(int which, orc_contract* c) {
         c->c_sin_abs = 12.0; c->c_sin_arg = 3.0;
         c->abs_floor = 1.1754943508222875e-38;
         c->sum_per_case = 1.0 / 32.0; c->sum_const = 5.0; /* per-lane chain + 5 shuffle levels */
+        /* CUDA math library cbrtf tanf asinf acosf atanf tanhf: documented 1 4 2 2 2 2 ulp, + 1 for the rounding of the input side */
+        c->c_fun[0] = 3.0; c->c_fun[1] = 6.0; c->c_fun[2] = 4.0; c->c_fun[3] = 4.0; c->c_fun[4] = 4.0; c->c_fun[5] = 4.0;
     }
 }

@@ -460,7 +460,7 @@ def test_P15_stack_command_well_formedness(oracle):
         np.array([x0, T(C.OP["DUP"], 1)], np.int32),                  # operator with an argument
         np.array([x0] + [T(C.OP["DUP"])] * 32, np.int32),             # depth 33
         np.array([x0, T(0x13)], np.int32),                            # POW: reserved, not built yet
-        np.array([x0, T(0x17)], np.int32),                            # CBRT: reserved
+        np.array([x0, T(0x1D)], np.int32),                            # COPY: reserved
     ]
     good = [np.array([x0] + [T(C.OP["DUP"])] * 31 + [T(C.OP["ADD"])] * 31, np.int32),   # depth 32: 32 * x0
             np.array([x0, T(C.OP["DEL"]), x1, T(C.OP["SQUARE"])], np.int32)]
@@ -495,5 +495,69 @@ def test_P11b_bound_holds_with_the_new_commands(oracle):
     assert not np.any(t["flags"] & oracle.FLAG_MALFORMED)
     fin = np.isfinite(t["fitness"]) & np.isfinite(m["fitness"]) & ((t["flags"] & 6) == 0)
     assert fin.sum() > 200
+    diff = np.abs(t["fitness"].astype(np.float64) - m["fitness"].astype(np.float64))
+    assert np.all(diff[fin] <= t["bound"][fin] + 1e-30)
+
+
+# ---- P16: CBRT TAN ARCSIN ARCCOS ARCTAN TANH reduce to library routines; identities; domain edges ----------
+def test_P16_unary_functions_reduce_to_numpy_and_identities(oracle):
+    rng = np.random.default_rng(16)
+    X = np.empty((512, 2), np.float32)
+    X[:, 0] = rng.uniform(-0.95, 0.95, 512)
+    X[:, 1] = rng.uniform(-6, 6, 512)
+    y = np.zeros(512, np.float32)
+    a, b = X[:, 0].astype(np.float64), X[:, 1].astype(np.float64)
+    cases = [("x1 CBRT", np.cbrt(b)), ("x0 TAN", np.tan(a)), ("x0 ARCSIN", np.arcsin(a)), ("x0 ARCCOS", np.arccos(a)),
+             ("x1 ARCTAN", np.arctan(b)), ("x1 TANH", np.tanh(b))]
+    for text, want in cases:
+        r = ev(oracle, [asm(text)[0]], np.zeros(1, np.float32), X, y, want_outputs=True)
+        np.testing.assert_allclose(r["outputs"][0], want, rtol=1e-14, atol=1e-300, err_msg=text)
+    ident = [("x0 ARCSIN SIN", a), ("x0 ARCCOS COS", a), ("x0 TAN ARCTAN", a), ("x1 CBRT CUBE", b),
+             ("x0 SIN x0 COS DIV", np.tan(a)),                       # tan = sin / cos
+             ("x0 ARCSIN x0 ARCCOS ADD", np.full(512, np.pi / 2))]   # asin + acos = pi/2
+    for text, want in ident:
+        r = ev(oracle, [asm(text)[0]], np.zeros(1, np.float32), X, y, want_outputs=True)
+        np.testing.assert_allclose(r["outputs"][0], want, rtol=1e-12, atol=1e-14, err_msg=text)
+    # tanh through the exponential: (e^{2x} - 1) / (e^{2x} + 1)
+    consts = []
+    p1 = asm("x1 2 MUL EXP 1 SUB x1 2 MUL EXP 1 ADD DIV", consts)[0]
+    p2 = asm("x1 TANH", consts)[0]
+    r = ev(oracle, [p1, p2], np.array(consts, np.float32), X, y, want_outputs=True)
+    np.testing.assert_allclose(r["outputs"][0], r["outputs"][1], rtol=1e-11, atol=1e-15)
+
+
+def test_P16_domain_edges(oracle):
+    vals = np.array([0.0, -0.0, 1.0, -1.0, 1.0000001, -2.0, np.inf, -np.inf, np.nan, 1e-30, -8.0, 27.0], np.float32)
+    X = vals[:, None].copy()
+    y = np.zeros(len(vals), np.float32)
+    out = {}
+    for nm in ("CBRT", "TAN", "ARCSIN", "ARCCOS", "ARCTAN", "TANH"):
+        out[nm] = ev(oracle, [asm(f"x0 {nm}")[0]], np.zeros(1, np.float32), X, y, want_outputs=True)["outputs"][0]
+    assert out["CBRT"][10] == -2.0 and out["CBRT"][11] == pytest.approx(3.0, rel=1e-15) and out["CBRT"][6] == np.inf and out["CBRT"][0] == 0.0
+    assert out["ARCSIN"][2] == pytest.approx(np.pi / 2) and out["ARCSIN"][3] == pytest.approx(-np.pi / 2)
+    assert np.isnan(out["ARCSIN"][4]) and np.isnan(out["ARCSIN"][5]) and np.isnan(out["ARCSIN"][6])   # outside [-1, 1]: NaN
+    assert out["ARCCOS"][2] == 0.0 and out["ARCCOS"][3] == pytest.approx(np.pi) and np.isnan(out["ARCCOS"][4])
+    assert out["ARCTAN"][6] == pytest.approx(np.pi / 2) and out["ARCTAN"][7] == pytest.approx(-np.pi / 2)
+    assert out["TANH"][6] == 1.0 and out["TANH"][7] == -1.0 and out["TANH"][0] == 0.0
+    assert np.isnan(out["TAN"][6]) and out["TAN"][0] == 0.0
+    for nm in out:
+        assert np.isnan(out[nm][8])                       # NaN in, NaN out
+
+
+def test_P16_bound_is_a_bound_for_the_functions(oracle):
+    rng = np.random.default_rng(17)
+    X = rng.uniform(-1.5, 1.5, (128, 2)).astype(np.float32)
+    y = np.zeros(128, np.float32)
+    progs, consts = [], []
+    fns = ["CBRT", "TAN", "ARCSIN", "ARCCOS", "ARCTAN", "TANH"]
+    for i in range(300):
+        f1, f2 = fns[int(rng.integers(6))], fns[int(rng.integers(6))]
+        progs.append(asm(f"x0 x1 {['ADD','MUL','SUB'][i % 3]} {f1} x1 {f2} {['MUL','ADD'][i % 2]} {rng.uniform(0.2, 2):.3f} MUL", consts)[0])
+    c = np.array(consts, np.float32)
+    ieee = oracle.contract(oracle.CONTRACT_IEEE)
+    t = ev(oracle, progs, c, X, y, contract_=ieee)
+    m = ev(oracle, progs, c, X, y, contract_=ieee, mode=1)
+    fin = np.isfinite(t["fitness"]) & np.isfinite(m["fitness"]) & ((t["flags"] & 6) == 0)
+    assert fin.sum() > 60
     diff = np.abs(t["fitness"].astype(np.float64) - m["fitness"].astype(np.float64))
     assert np.all(diff[fin] <= t["bound"][fin] + 1e-30)
