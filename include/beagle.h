@@ -56,8 +56,13 @@ extern "C" {
 #define BEAGLE_OP_SIGN   0x14 /* a -> -a     */
 #define BEAGLE_OP_SQUARE 0x15 /* a -> a * a     */
 #define BEAGLE_OP_CUBE   0x16 /* a -> (a * a) * a     */
-/* 0x13 POW and 0x17..0x1E (CBRT TAN ARCSIN ARCCOS ARCTAN TANH COPY PASTE) are reserved; until implemented
- * they make a program malformed.                                                                */
+#define BEAGLE_OP_CBRT   0x17 /* a -> cbrt a     */
+#define BEAGLE_OP_TAN    0x18 /* a -> tan a     */
+#define BEAGLE_OP_ARCSIN 0x19 /* a -> asin a   (NaN outside [-1, 1])     */
+#define BEAGLE_OP_ARCCOS 0x1A /* a -> acos a   (NaN outside [-1, 1])     */
+#define BEAGLE_OP_ARCTAN 0x1B /* a -> atan a     */
+#define BEAGLE_OP_TANH   0x1C /* a -> tanh a     */
+/* 0x13 POW, 0x1D COPY and 0x1E PASTE are reserved; until implemented they make a program malformed.   */
 #define BEAGLE_TOKEN(op, arg) ((int32_t)(((uint32_t)(arg) << 8) | ((uint32_t)(op) & 0xFFu)))
 
 /* ---- limits (also returned by beagle_limits) ---- */

@@ -27,7 +27,9 @@ enum : uint32_t { OPC_CONST = BEAGLE_OP_CONST, OPC_LOAD = BEAGLE_OP_LOAD, OPC_AD
                   OPC_SIN = BEAGLE_OP_SIN, OPC_COS = BEAGLE_OP_COS, OPC_LOG = BEAGLE_OP_LOG,
                   OPC_SQRT = BEAGLE_OP_SQRT, OPC_EXP = BEAGLE_OP_EXP,
                   OPC_DUP = BEAGLE_OP_DUP, OPC_SWAP = BEAGLE_OP_SWAP, OPC_DEL = BEAGLE_OP_DEL,
-                  OPC_SIGN = BEAGLE_OP_SIGN, OPC_SQUARE = BEAGLE_OP_SQUARE, OPC_CUBE = BEAGLE_OP_CUBE };
+                  OPC_SIGN = BEAGLE_OP_SIGN, OPC_SQUARE = BEAGLE_OP_SQUARE, OPC_CUBE = BEAGLE_OP_CUBE,
+                  OPC_CBRT = BEAGLE_OP_CBRT, OPC_TAN = BEAGLE_OP_TAN, OPC_ARCSIN = BEAGLE_OP_ARCSIN,
+                  OPC_ARCCOS = BEAGLE_OP_ARCCOS, OPC_ARCTAN = BEAGLE_OP_ARCTAN, OPC_TANH = BEAGLE_OP_TANH };
 
 constexpr int kNumBins = BEAGLE_MAX_LEN + 1;   // bin = 512 - length  (longest first); bin 512 unused
 constexpr int kScanThreads = 256;              // programs per block in the pre-pass
@@ -411,9 +413,9 @@ __global__ void __launch_bounds__(kCompileThreads, 8) k_compile(const CompilePar
             bool bad = live && !good;
             if (bad) {
                 // not one of the eleven hot-path commands (rare, off the straight-line path). DUP SWAP DEL SIGN SQUARE
-                // CUBE are checked here (stack effect, depth) but not compiled: an individual that uses
+                // CUBE CBRT TAN ARCSIN ARCCOS ARCTAN TANH are checked here (stack effect, depth) but not compiled: an individual that uses
                 // one is evaluated by the blockwise kernel (slow list)
-                const bool isK = (op - OPC_DUP) < 3u || (op - OPC_SIGN) < 3u;
+                const bool isK = (op - OPC_DUP) < 3u || (op - OPC_SIGN) <= (OPC_TANH - OPC_SIGN);
                 const int kneed = op == OPC_SWAP ? 2 : 1, kpush = op == OPC_DUP ? 1 : (op == OPC_DEL ? -1 : 0);
                 if (isK && arg == 0 && sp >= kneed && sp + kpush <= BEAGLE_MAX_STACK) { slow = true; sp += kpush; mx = max(mx, sp); bad = false; }
             }
@@ -537,6 +539,12 @@ __global__ void __launch_bounds__(1024) k_eval_blockwise(
                 case OPC_SIGN: st[sp - 1] = op_sign(st[sp - 1]); break;
                 case OPC_SQUARE: st[sp - 1] = op_square(st[sp - 1]); break;
                 case OPC_CUBE: st[sp - 1] = op_cube(st[sp - 1]); break;
+                case OPC_CBRT: st[sp - 1] = op_cbrt(st[sp - 1]); break;
+                case OPC_TAN: st[sp - 1] = op_tan(st[sp - 1]); break;
+                case OPC_ARCSIN: st[sp - 1] = op_arcsin(st[sp - 1]); break;
+                case OPC_ARCCOS: st[sp - 1] = op_arccos(st[sp - 1]); break;
+                case OPC_ARCTAN: st[sp - 1] = op_arctan(st[sp - 1]); break;
+                case OPC_TANH: st[sp - 1] = op_tanh(st[sp - 1]); break;
                 case OPC_DUP: st[sp] = st[sp - 1]; ++sp; break;
                 case OPC_SWAP: { const float b = st[sp - 1]; st[sp - 1] = st[sp - 2]; st[sp - 2] = b; break; }
                 case OPC_DEL: --sp; break;

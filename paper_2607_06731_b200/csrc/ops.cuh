@@ -46,6 +46,14 @@ __device__ __forceinline__ float op_sign(float a) { return -a; }                
 __device__ __forceinline__ float op_square(float a) { return __fmul_rn(a, a); }
 __device__ __forceinline__ float op_cube(float a) { return __fmul_rn(__fmul_rn(a, a), a); }      // (a*a)*a
 
+// unprotected, as the paper's are; the CUDA math library's accurate versions (documented 1 4 2 2 2 2 ulp)
+__device__ __forceinline__ float op_cbrt(float a) { return cbrtf(a); }
+__device__ __forceinline__ float op_tan(float a) { return tanf(a); }
+__device__ __forceinline__ float op_arcsin(float a) { return asinf(a); }
+__device__ __forceinline__ float op_arccos(float a) { return acosf(a); }
+__device__ __forceinline__ float op_arctan(float a) { return atanf(a); }
+__device__ __forceinline__ float op_tanh(float a) { return tanhf(a); }
+
 // token fields (D1)
 __device__ __forceinline__ uint32_t tok_op(uint32_t w) { return w & 0xFFu; }
 __device__ __forceinline__ uint32_t tok_arg(uint32_t w) { return w >> 8; }

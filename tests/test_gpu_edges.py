@@ -343,7 +343,8 @@ def test_stack_commands_and_exact_unaries(oracle, N, d):
     rng = np.random.default_rng(21)
     X = rng.uniform(-2, 2, (N, d)).astype(np.float32)
     y = (X[:, 0] * X[:, 1]).astype(np.float32)
-    names = ["ADD", "SUB", "MUL", "DIV", "SIN", "COS", "LOG", "SQRT", "EXP", "SIGN", "SQUARE", "CUBE", "DUP", "SWAP", "DEL"]
+    names = ["ADD", "SUB", "MUL", "DIV", "SIN", "COS", "LOG", "SQRT", "EXP", "SIGN", "SQUARE", "CUBE", "DUP", "SWAP", "DEL",
+             "CBRT", "TAN", "ARCSIN", "ARCCOS", "ARCTAN", "TANH"]
     texts = _random_gcl_programs(rng, 600, d, names)
     texts += ["0 -9.280686 8.983309 ADD DEL x1 ADD DUP MUL x0 DUP ADD DUP ADD x2 MUL SUB SQRT x1 SUB x0 DIV 0.5 MUL",
               "x2 x0 MUL -2 MUL DUP ADD 3 4 SUB 2.7182817 SUB DUP DIV DEL x1 SQUARE ADD SQRT x1 SUB x0 DIV 0.5 MUL"]
@@ -375,7 +376,7 @@ def test_stack_command_malformed_programs(oracle):
     x0 = T(OP["LOAD"], 0)
     progs = [np.array([T(OP["DUP"])], np.int32), np.array([x0, T(OP["SWAP"])], np.int32),
              np.array([x0, T(OP["DEL"])], np.int32), np.array([x0] + [T(OP["DUP"])] * 32, np.int32),
-             np.array([x0, T(0x13)], np.int32), np.array([x0, T(OP["SQUARE"], 3)], np.int32),
+             np.array([x0, T(0x13)], np.int32), np.array([x0, T(OP["SQUARE"], 3)], np.int32),     # POW: reserved
              np.array([x0] + [T(OP["DUP"])] * 31 + [T(OP["ADD"])] * 31, np.int32),      # well-formed: depth 32
              np.array([x0, T(OP["DEL"]), x0, T(OP["CUBE"])], np.int32)]                 # well-formed
     g, l, c = pack(progs, np.zeros(1, np.float32))

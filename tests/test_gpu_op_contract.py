@@ -174,3 +174,37 @@ def test_protected_edge_table_bitwise():
     assert np.all(np.isnan(_unary("SIN", np.array([inf, -inf, nan], np.float32))))
     assert np.all(np.isnan(_unary("COS", np.array([inf, -inf, nan], np.float32))))
     assert _unary("SIN", np.array([0.0], np.float32))[0] == 0 and _unary("COS", np.array([0.0], np.float32))[0] == 1
+
+
+def test_f1_exact_commands_bit_exact():
+    """SIGN SQUARE CUBE: exact / correctly rounded products, bit for bit on swept inputs."""
+    rng = np.random.default_rng(11)
+    a = np.concatenate([_sweep(rng, -60, 60, 20000), _sweep(rng, -140, -100, 2000), np.array([0.0, -0.0, np.inf, -np.inf], np.float32)])
+    a64 = a.astype(np.float64)
+    with np.errstate(all="ignore"):
+        want = {"SIGN": (-a64).astype(np.float32), "SQUARE": (a64 * a64).astype(np.float32),
+                "CUBE": ((a64 * a64).astype(np.float32).astype(np.float64) * a64).astype(np.float32)}
+    for op, w in want.items():
+        got = _unary(op, a)
+        assert np.array_equal(got.view(np.uint32), w.view(np.uint32)), op
+
+
+def test_f1_function_contract(oracle):
+    """CBRT TAN ARCSIN ARCCOS ARCTAN TANH on swept inputs against numpy in fp64: relative error within the
+    contract the oracle's bound assumes (c_fun), domain behaviour (NaN outside [-1, 1]) exact."""
+    c = _contract(oracle)
+    rng = np.random.default_rng(12)
+    wide = np.concatenate([_sweep(rng, -100, 100, 40000), _sweep(rng, -4, 4, 40000)])
+    unit = np.concatenate([rng.uniform(-1, 1, 40000).astype(np.float32), np.array([1.0, -1.0, 0.0], np.float32)])
+    ang = np.concatenate([rng.uniform(-100, 100, 40000).astype(np.float32), _sweep(rng, -30, 0, 10000)])
+    fns = [("CBRT", wide, np.cbrt, 0), ("TAN", ang, np.tan, 1), ("ARCSIN", unit, np.arcsin, 2), ("ARCCOS", unit, np.arccos, 3),
+           ("ARCTAN", wide, np.arctan, 4), ("TANH", wide, np.tanh, 5)]
+    for op, a, f, k in fns:
+        got = _unary(op, a).astype(np.float64)
+        want = f(a.astype(np.float64))
+        err = np.abs(got - want)
+        bound = c.c_fun[k] * U * np.abs(want) + c.abs_floor
+        assert np.all(err <= bound), (op, float(np.max(err / bound)))
+    out = np.array([1.0000001, -1.5, 3.0, np.inf], np.float32)
+    assert np.all(np.isnan(_unary("ARCSIN", out))) and np.all(np.isnan(_unary("ARCCOS", out)))
+    assert np.all(np.isnan(_unary("TAN", np.array([np.inf, -np.inf, np.nan], np.float32))))
