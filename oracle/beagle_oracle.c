@@ -43,11 +43,15 @@
 enum { OP_CONST = 1, OP_LOAD = 2, OP_ADD = 3, OP_SUB = 4, OP_MUL = 5, OP_DIV = 6,
        OP_SIN = 7, OP_COS = 8, OP_LOG = 9, OP_SQRT = 10, OP_EXP = 11,
        /* the rest of Table 3 in its own order from 0x10 (D2); built so far: the three
-        * stack commands, the three exact unary ones and six more unary functions. POW 0x13, COPY 0x1D and PASTE 0x1E
-        * stay malformed. */
+        * stack commands, the three exact unary ones, six more unary functions, POW and the COPY / PASTE variables. */
        OP_DUP = 0x10, OP_SWAP = 0x11, OP_DEL = 0x12, OP_SIGN = 0x14, OP_SQUARE = 0x15, OP_CUBE = 0x16,
        /* unprotected, as the paper's are: plain mathematical functions, NaN outside their domain */
-       OP_CBRT = 0x17, OP_TAN = 0x18, OP_ARCSIN = 0x19, OP_ARCCOS = 0x1A, OP_ARCTAN = 0x1B, OP_TANH = 0x1C };
+       OP_CBRT = 0x17, OP_TAN = 0x18, OP_ARCSIN = 0x19, OP_ARCCOS = 0x1A, OP_ARCTAN = 0x1B, OP_TANH = 0x1C,
+       OP_POW = 0x13,    /* second-top to the power of top, the C pow function: NaN for a negative base with a
+                            non-integer exponent */
+       OP_COPY = 0x1D,   /* top of stack -> variable @arg, stack unchanged                              */
+       OP_PASTE = 0x1E };/* variable @arg -> pushed; the variable is destroyed                                      */
+#define ORC_MAX_VARS 32  /* variable identifiers @0 .. @31 (D2 extension)                                  */
 
 #define ORC_MAX_LEN   512
 #define ORC_MAX_STACK 32
@@ -78,6 +82,7 @@ typedef struct {
     double sum_per_case; /* summation: the fp32 sum of N squares is off by at most            */
     double sum_const;    /*   (sum_per_case * N + sum_const) * u * S  (depth of the add tree) */
     double c_fun[6];     /* CBRT TAN ARCSIN ARCCOS ARCTAN TANH: relative                      */
+    double c_pow;        /* POW: relative                                                     */
 } orc_contract;
 
 static const double U32 = 5.9604644775390625e-08; /* 2^-24 */
@@ -105,12 +110,15 @@ static inline pair finish(double v, double e, int mirror, int* flags) {
 static int check_program(const uint32_t* tok, int L, int64_t n_consts, int d) {
     if (L < 1 || L > ORC_MAX_LEN) return -1;
     int sp = 0, mx = 0;
+    uint32_t live = 0;   /* variables that hold a value: COPY and PASTE come in pairs */
     for (int t = 0; t < L; ++t) {
         uint32_t op = tok[t] & 0xFFu, arg = tok[t] >> 8;
         switch (op) {
+        case OP_COPY:  if (arg >= ORC_MAX_VARS || sp < 1 || ((live >> arg) & 1u)) return -1; live |= 1u << arg; break;
+        case OP_PASTE: if (arg >= ORC_MAX_VARS || !((live >> arg) & 1u)) return -1; live &= ~(1u << arg); sp++; break;
         case OP_CONST: if ((int64_t)arg >= n_consts) return -1; sp++; break;
         case OP_LOAD:  if ((int64_t)arg >= (int64_t)d) return -1; sp++; break;
-        case OP_ADD: case OP_SUB: case OP_MUL: case OP_DIV:
+        case OP_ADD: case OP_SUB: case OP_MUL: case OP_DIV: case OP_POW:
             if (arg != 0 || sp < 2) return -1; sp--; break;
         case OP_SIN: case OP_COS: case OP_LOG: case OP_SQRT: case OP_EXP:
         case OP_SIGN: case OP_SQUARE: case OP_CUBE:
@@ -124,7 +132,7 @@ static int check_program(const uint32_t* tok, int L, int64_t n_consts, int d) {
         if (sp > ORC_MAX_STACK) return -1;
         if (sp > mx) mx = sp;
     }
-    return sp >= 1 ? mx : -1;
+    return (sp >= 1 && live == 0) ? mx : -1;   /* a COPY without its PASTE is not a valid program */
 }
 
 /* a * b with its bound; also the two products of CUBE and the one of SQUARE. */
@@ -172,7 +180,7 @@ static pair fun_pair(uint32_t op, pair a, const orc_contract* c, int mirror, int
 /* One program on one case: PAPER.md:184 stack semantics, Table 3 operand order, D2 values. */
 static pair run_case(const uint32_t* tok, int L, const float* consts, const float* x,
                      const orc_contract* c, int mirror, int* flags) {
-    pair st[ORC_MAX_STACK];
+    pair st[ORC_MAX_STACK], var[ORC_MAX_VARS];
     int sp = 0;
     const double fl = c->abs_floor;
     for (int t = 0; t < L; ++t) {
@@ -196,6 +204,27 @@ static pair run_case(const uint32_t* tok, int L, const float* consts, const floa
         case OP_SQUARE: st[sp - 1] = mul_pair(st[sp - 1], st[sp - 1], c, mirror, flags); break;   /* a * a */
         case OP_CBRT: case OP_TAN: case OP_ARCSIN: case OP_ARCCOS: case OP_ARCTAN: case OP_TANH:
             st[sp - 1] = fun_pair(op, st[sp - 1], c, mirror, flags); break;
+        case OP_COPY:  var[arg] = st[sp - 1]; break;                       /* no change to the stack */
+        case OP_PASTE: st[sp] = var[arg]; sp++; break;                     /* pushes the variable    */
+        case OP_POW: {                         /* second-top ^ top. Bound: the corners of the input box */
+            pair a = st[sp - 2], b = st[sp - 1];
+            double v = pow(a.v, b.v), e = 0.0;
+            if (!isnan(v) && !isinf(v) && !isnan(a.v) && !isinf(a.v) && !isnan(b.v) && !isinf(b.v)) {
+                double e1 = 0.0;
+                int unstable = 0;
+                if (a.v < 0.0 && b.e > 0.0) unstable = 1;                  /* a non-integer exponent nearby: NaN */
+                if (fabs(a.v) <= a.e && (a.e > 0.0 || b.v <= 0.0)) unstable = 1;   /* the base may be zero or change sign */
+                for (int ia = -1; ia <= 1 && !unstable; ia += 2)
+                    for (int ib = -1; ib <= 1; ib += 2) {
+                        double w = pow(a.v + ia * a.e, b.v + ib * b.e);
+                        if (isnan(w)) { unstable = 1; break; }
+                        e1 = fmax(e1, fabs(w - v));
+                    }
+                if (unstable) { *flags |= ORC_FLAG_UNSTABLE; e1 = 0.0; }
+                e = e1 + c->c_pow * U32 * (fabs(v) + e1) + fl;
+            }
+            st[sp - 2] = finish(v, e, mirror, flags);
+            sp--; break; }
         case OP_CUBE: {                                                    /* (a * a) * a, two products */
             pair a = st[sp - 1];
             st[sp - 1] = mul_pair(mul_pair(a, a, c, mirror, flags), a, c, mirror, flags);
@@ -337,6 +366,7 @@ void orc_default_contract(int which, orc_contract* c) {
         c->abs_floor = 1.5e-45;
         c->sum_per_case = 1.0; c->sum_const = 0.0;   /* any summation order */
         for (int k = 0; k < 6; ++k) c->c_fun[k] = 1.001;
+        c->c_pow = 1.001;
     } else {
         c->c_add = 1.0; c->c_mul = 1.0;
         c->c_div = 3.5; c->div_bigb_abs = 1.1754943508222875e-38;
@@ -348,5 +378,6 @@ void orc_default_contract(int which, orc_contract* c) {
         c->sum_per_case = 1.0 / 32.0; c->sum_const = 5.0; /* per-lane chain + 5 shuffle levels */
         /* CUDA math library cbrtf tanf asinf acosf atanf tanhf: documented 1 4 2 2 2 2 ulp, + 1 for the rounding of the input side */
         c->c_fun[0] = 3.0; c->c_fun[1] = 6.0; c->c_fun[2] = 4.0; c->c_fun[3] = 4.0; c->c_fun[4] = 4.0; c->c_fun[5] = 4.0;
+        c->c_pow = 10.0;                                   /* powf: documented 4 ulp (older toolkits 8) */
     }
 }

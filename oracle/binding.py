@@ -30,7 +30,7 @@ class Contract(ctypes.Structure):
     _fields_ = [(n, ctypes.c_double) for n in (
         "c_add", "c_mul", "c_div", "div_bigb_abs", "c_sqrt", "abs_sqrt", "c_exp", "c_exp_arg",
         "c_log_rel", "c_log_abs", "c_sin_abs", "c_sin_arg", "abs_floor", "sum_per_case",
-        "sum_const")] + [("c_fun", ctypes.c_double * 6)]
+        "sum_const")] + [("c_fun", ctypes.c_double * 6), ("c_pow", ctypes.c_double)]
 
 
 def build(force: bool = False) -> str:

@@ -21,7 +21,8 @@ _LIB = os.path.join(_HERE, "libcolony_gen.so")
 
 OP = dict(CONST=1, LOAD=2, ADD=3, SUB=4, MUL=5, DIV=6, SIN=7, COS=8, LOG=9, SQRT=10, EXP=11,
           DUP=0x10, SWAP=0x11, DEL=0x12, SIGN=0x14, SQUARE=0x15, CUBE=0x16,
-          CBRT=0x17, TAN=0x18, ARCSIN=0x19, ARCCOS=0x1A, ARCTAN=0x1B, TANH=0x1C)
+          CBRT=0x17, TAN=0x18, ARCSIN=0x19, ARCCOS=0x1A, ARCTAN=0x1B, TANH=0x1C,
+          POW=0x13, COPY=0x1D, PASTE=0x1E)
 OP_NAME = {v: k for k, v in OP.items()}
 
 

@@ -561,3 +561,53 @@ def test_P16_bound_is_a_bound_for_the_functions(oracle):
     assert fin.sum() > 60
     diff = np.abs(t["fitness"].astype(np.float64) - m["fitness"].astype(np.float64))
     assert np.all(diff[fin] <= t["bound"][fin] + 1e-30)
+
+
+# ---- P17: POW; P18: COPY / PASTE ----------------------------------------------------------------------------
+def test_P17_pow_reduces_to_numpy_and_identities(oracle):
+    rng = np.random.default_rng(18)
+    X = np.empty((512, 2), np.float32)
+    X[:, 0] = rng.uniform(0.2, 4, 512)
+    X[:, 1] = rng.uniform(-3, 3, 512)
+    y = np.zeros(512, np.float32)
+    a, b = X[:, 0].astype(np.float64), X[:, 1].astype(np.float64)
+    r = ev(oracle, [asm("x0 x1 POW")[0]], np.zeros(1, np.float32), X, y, want_outputs=True)
+    np.testing.assert_allclose(r["outputs"][0], np.power(a, b), rtol=1e-14)       # second-top ^ top
+    consts = []
+    progs = [asm(t, consts)[0] for t in ("x0 2 POW", "x0 SQUARE", "x0 3 POW", "x0 CUBE", "x0 0.5 POW", "x0 SQRT",
+                                         "x0 x1 POW", "x0 LOG x1 MUL EXP", "x0 -1 POW", "1 x0 DIV")]
+    r = ev(oracle, progs, np.array(consts, np.float32), X, y, want_outputs=True)
+    for k in range(0, 10, 2):
+        np.testing.assert_allclose(r["outputs"][k], r["outputs"][k + 1], rtol=1e-12, err_msg=str(k))
+    # the C pow function at its edges: negative base with an integer / non-integer exponent, zero base, zero exponent
+    vals = np.array([[-2.0, 3.0], [-2.0, 2.0], [-2.0, 0.5], [0.0, 2.0], [0.0, -1.0], [5.0, 0.0], [np.nan, 0.0], [-8.0, 1.0 / 3.0]], np.float32)
+    o = ev(oracle, [asm("x0 x1 POW")[0]], np.zeros(1, np.float32), vals, np.zeros(len(vals), np.float32), want_outputs=True)["outputs"][0]
+    assert o[0] == -8.0 and o[1] == 4.0 and np.isnan(o[2]) and o[3] == 0.0 and o[4] == np.inf and o[5] == 1.0 and o[6] == 1.0 and np.isnan(o[7])
+
+
+def test_P18_copy_paste_variables(oracle):
+    rng = np.random.default_rng(19)
+    X = rng.uniform(-3, 3, (64, 2)).astype(np.float32)
+    y = np.zeros(64, np.float32)
+    A, B = "x0 x1 MUL 1.5 ADD", "x1 SIN x0 SUB"
+    pairs = [
+        (f"{A} COPY@1 PASTE@1 MUL", f"{A} SQUARE"),                 # COPY leaves the stack alone, PASTE pushes the copy
+        (f"{A} COPY@2 DEL {B} PASTE@2 SUB", f"{B} {A} SUB"),        # the value survives while the stack moves on
+        (f"{A} COPY@0 {B} COPY@31 DEL DEL PASTE@31 PASTE@0 DIV", f"{B} {A} DIV"),
+        (f"{A} COPY@5 PASTE@5 DEL", A),
+        (f"{A} COPY@1 PASTE@1 COPY@1 PASTE@1 ADD ADD", f"{A} DUP DUP ADD ADD"),   # a variable can be used again after its PASTE
+    ]
+    for left, right in pairs:
+        consts = []
+        pl, pr = asm(left, consts)[0], asm(right, consts)[0]
+        r = ev(oracle, [pl, pr], np.array(consts, np.float32), X, y, want_outputs=True, mode=1)
+        assert np.array_equal(r["outputs"][0], r["outputs"][1]), (left, right)
+    bad = ["x0 PASTE@1", "x0 COPY@1", "x0 COPY@1 COPY@1 PASTE@1", "x0 COPY@1 PASTE@1 PASTE@1", "COPY@1 x0 PASTE@1", "x0 COPY@32 PASTE@32",
+           "x0 COPY@1 PASTE@2"]
+    progs = [asm(t)[0] for t in bad]
+    r = ev(oracle, progs, np.zeros(1, np.float32), X, y)
+    assert np.all(r["fitness"].view(np.uint32) == QNAN_BITS) and np.all(r["flags"] & oracle.FLAG_MALFORMED)
+    # depth 32 through PASTE
+    deep = asm("x0 COPY@3 " + "x0 " * 30 + "PASTE@3 " + "ADD " * 31)[0]
+    r = ev(oracle, [deep], np.zeros(1, np.float32), np.ones((4, 2), np.float32), np.zeros(4, np.float32))
+    assert r["depth"][0] == 32 and r["fitness"][0] == 32.0 ** 2

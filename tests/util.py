@@ -14,7 +14,9 @@ def asm(text, consts=None, const_base=0):
     toks = []
     for w in text.replace(";", " ").split():
         u = w.upper()
-        if u in OP and u not in ("CONST", "LOAD"):
+        if u.startswith(("COPY@", "PASTE@")):                   # GCL's variables: COPY@2, PASTE@2
+            toks.append(token(OP[u.split("@")[0]], int(u.split("@")[1])))
+        elif u in OP and u not in ("CONST", "LOAD"):
             toks.append(token(OP[u]))
         elif u.startswith("X") and u[1:].isdigit():
             toks.append(token(OP["LOAD"], int(u[1:])))
