@@ -62,7 +62,12 @@ extern "C" {
 #define BEAGLE_OP_ARCCOS 0x1A /* a -> acos a   (NaN outside [-1, 1])     */
 #define BEAGLE_OP_ARCTAN 0x1B /* a -> atan a     */
 #define BEAGLE_OP_TANH   0x1C /* a -> tanh a     */
-/* 0x13 POW, 0x1D COPY and 0x1E PASTE are reserved; until implemented they make a program malformed.   */
+#define BEAGLE_OP_POW    0x13 /* a b -> pow(a, b)  (the C function)     */
+#define BEAGLE_OP_COPY   0x1D /* variable @arg = top; stack unchanged     */
+#define BEAGLE_OP_PASTE  0x1E /* push variable @arg; the variable is gone     */
+#define BEAGLE_MAX_VARS  32   /* variable identifiers @0 .. @31; COPY and PASTE come in pairs: PASTE of a variable
+                                 that holds nothing, COPY to one that does, or a COPY left without its PASTE make
+                                 the program malformed                                                        */
 #define BEAGLE_TOKEN(op, arg) ((int32_t)(((uint32_t)(arg) << 8) | ((uint32_t)(op) & 0xFFu)))
 
 /* ---- limits (also returned by beagle_limits) ---- */

@@ -29,7 +29,8 @@ enum : uint32_t { OPC_CONST = BEAGLE_OP_CONST, OPC_LOAD = BEAGLE_OP_LOAD, OPC_AD
                   OPC_DUP = BEAGLE_OP_DUP, OPC_SWAP = BEAGLE_OP_SWAP, OPC_DEL = BEAGLE_OP_DEL,
                   OPC_SIGN = BEAGLE_OP_SIGN, OPC_SQUARE = BEAGLE_OP_SQUARE, OPC_CUBE = BEAGLE_OP_CUBE,
                   OPC_CBRT = BEAGLE_OP_CBRT, OPC_TAN = BEAGLE_OP_TAN, OPC_ARCSIN = BEAGLE_OP_ARCSIN,
-                  OPC_ARCCOS = BEAGLE_OP_ARCCOS, OPC_ARCTAN = BEAGLE_OP_ARCTAN, OPC_TANH = BEAGLE_OP_TANH };
+                  OPC_ARCCOS = BEAGLE_OP_ARCCOS, OPC_ARCTAN = BEAGLE_OP_ARCTAN, OPC_TANH = BEAGLE_OP_TANH,
+                  OPC_POW = BEAGLE_OP_POW, OPC_COPY = BEAGLE_OP_COPY, OPC_PASTE = BEAGLE_OP_PASTE };
 
 constexpr int kNumBins = BEAGLE_MAX_LEN + 1;   // bin = 512 - length  (longest first); bin 512 unused
 constexpr int kScanThreads = 256;              // programs per block in the pre-pass
@@ -365,6 +366,7 @@ __global__ void __launch_bounds__(kCompileThreads, 8) k_compile(const CompilePar
     int sp = 0, mx = 0;
     int c = 0;                                     // computed entries on the stack (the topmost one is acc)
     bool ok = valid, slow = false;
+    uint32_t vlive = 0;                            // COPY / PASTE variables that hold a value
     const int S_T = q.tmem_slots;
     // variables whose division is a multiplication by a staged reciprocal row
     const uint32_t rcp_ok = ~q.hdr->rcp_unsafe & ((q.k_rcp >= 32) ? 0xFFFFFFFFu : ((1u << q.k_rcp) - 1u));
@@ -415,9 +417,16 @@ __global__ void __launch_bounds__(kCompileThreads, 8) k_compile(const CompilePar
                 // not one of the eleven hot-path commands (rare, off the straight-line path). DUP SWAP DEL SIGN SQUARE
                 // CUBE CBRT TAN ARCSIN ARCCOS ARCTAN TANH are checked here (stack effect, depth) but not compiled: an individual that uses
                 // one is evaluated by the blockwise kernel (slow list)
-                const bool isK = (op - OPC_DUP) < 3u || (op - OPC_SIGN) <= (OPC_TANH - OPC_SIGN);
-                const int kneed = op == OPC_SWAP ? 2 : 1, kpush = op == OPC_DUP ? 1 : (op == OPC_DEL ? -1 : 0);
-                if (isK && arg == 0 && sp >= kneed && sp + kpush <= BEAGLE_MAX_STACK) { slow = true; sp += kpush; mx = max(mx, sp); bad = false; }
+                const bool isVar = op == OPC_COPY || op == OPC_PASTE;          // COPY @arg / PASTE @arg come in pairs
+                const bool isK = (op - OPC_DUP) <= (OPC_TANH - OPC_DUP) || isVar;
+                const int kneed = (op == OPC_SWAP || op == OPC_POW) ? 2 : (op == OPC_PASTE ? 0 : 1);
+                const int kpush = (op == OPC_DUP || op == OPC_PASTE) ? 1 : ((op == OPC_DEL || op == OPC_POW) ? -1 : 0);
+                const bool held = arg < (uint32_t)BEAGLE_MAX_VARS && ((vlive >> (arg & 31u)) & 1u);
+                const bool argok = isVar ? (arg < (uint32_t)BEAGLE_MAX_VARS && held == (op == OPC_PASTE)) : arg == 0;
+                if (isK && argok && sp >= kneed && sp + kpush <= BEAGLE_MAX_STACK) {
+                    slow = true; sp += kpush; mx = max(mx, sp); bad = false;
+                    if (isVar) vlive ^= 1u << (arg & 31u);
+                }
             }
             ok = ok && !bad;
             const bool run = live && good;
@@ -468,7 +477,7 @@ __global__ void __launch_bounds__(kCompileThreads, 8) k_compile(const CompilePar
     }
     int n = (int)(po - po0);
     if (!valid) return;
-    ok &= (sp >= 1);
+    ok &= (sp >= 1) && (vlive == 0);               // a COPY left without its PASTE is malformed
     if (!ok) {
         q.depth[p] = 0;
         if (q.fitness) q.fitness[p] = __uint_as_float(0x7FC00000u);
@@ -519,7 +528,7 @@ __global__ void __launch_bounds__(1024) k_eval_blockwise(
         const uint32_t* tok = reinterpret_cast<const uint32_t*>(genomes) + off[p];
         const int i = threadIdx.x;
         if (i < n) {
-            float st[BEAGLE_MAX_STACK];
+            float st[BEAGLE_MAX_STACK], var[BEAGLE_MAX_VARS];
             int sp = 0;
             for (int t = 0; t < len; ++t) {
                 const uint32_t w = __ldg(tok + t);
@@ -545,6 +554,9 @@ __global__ void __launch_bounds__(1024) k_eval_blockwise(
                 case OPC_ARCCOS: st[sp - 1] = op_arccos(st[sp - 1]); break;
                 case OPC_ARCTAN: st[sp - 1] = op_arctan(st[sp - 1]); break;
                 case OPC_TANH: st[sp - 1] = op_tanh(st[sp - 1]); break;
+                case OPC_POW: st[sp - 2] = op_pow(st[sp - 2], st[sp - 1]); --sp; break;
+                case OPC_COPY: var[arg & 31u] = st[sp - 1]; break;
+                case OPC_PASTE: st[sp++] = var[arg & 31u]; break;
                 case OPC_DUP: st[sp] = st[sp - 1]; ++sp; break;
                 case OPC_SWAP: { const float b = st[sp - 1]; st[sp - 1] = st[sp - 2]; st[sp - 2] = b; break; }
                 case OPC_DEL: --sp; break;

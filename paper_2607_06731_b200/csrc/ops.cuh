@@ -54,6 +54,8 @@ __device__ __forceinline__ float op_arccos(float a) { return acosf(a); }        
 __device__ __forceinline__ float op_arctan(float a) { return atanf(a); }
 __device__ __forceinline__ float op_tanh(float a) { return tanhf(a); }
 
+__device__ __forceinline__ float op_pow(float a, float b) { return powf(a, b); }
+
 // token fields (D1)
 __device__ __forceinline__ uint32_t tok_op(uint32_t w) { return w & 0xFFu; }
 __device__ __forceinline__ uint32_t tok_arg(uint32_t w) { return w >> 8; }

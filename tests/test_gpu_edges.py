@@ -324,7 +324,7 @@ def _random_gcl_programs(rng, n_prog, d, names):
         toks, depth = [], 0
         for _ in range(int(rng.integers(3, 60))):
             nm = names[int(rng.integers(len(names)))]
-            need = 2 if nm in ("ADD", "SUB", "MUL", "DIV", "SWAP") else 1
+            need = 2 if nm in ("ADD", "SUB", "MUL", "DIV", "SWAP", "POW") else 1
             if depth < need or (nm == "DUP" and depth >= 30) or rng.random() < 0.35:
                 toks.append(f"x{int(rng.integers(d))}" if rng.random() < 0.8 else f"{rng.uniform(-3, 3):.4f}"); depth += 1
             else:
@@ -344,7 +344,7 @@ def test_stack_commands_and_exact_unaries(oracle, N, d):
     X = rng.uniform(-2, 2, (N, d)).astype(np.float32)
     y = (X[:, 0] * X[:, 1]).astype(np.float32)
     names = ["ADD", "SUB", "MUL", "DIV", "SIN", "COS", "LOG", "SQRT", "EXP", "SIGN", "SQUARE", "CUBE", "DUP", "SWAP", "DEL",
-             "CBRT", "TAN", "ARCSIN", "ARCCOS", "ARCTAN", "TANH"]
+             "CBRT", "TAN", "ARCSIN", "ARCCOS", "ARCTAN", "TANH", "POW"]
     texts = _random_gcl_programs(rng, 600, d, names)
     texts += ["0 -9.280686 8.983309 ADD DEL x1 ADD DUP MUL x0 DUP ADD DUP ADD x2 MUL SUB SQRT x1 SUB x0 DIV 0.5 MUL",
               "x2 x0 MUL -2 MUL DUP ADD 3 4 SUB 2.7182817 SUB DUP DIV DEL x1 SQUARE ADD SQRT x1 SUB x0 DIV 0.5 MUL"]
@@ -376,7 +376,7 @@ def test_stack_command_malformed_programs(oracle):
     x0 = T(OP["LOAD"], 0)
     progs = [np.array([T(OP["DUP"])], np.int32), np.array([x0, T(OP["SWAP"])], np.int32),
              np.array([x0, T(OP["DEL"])], np.int32), np.array([x0] + [T(OP["DUP"])] * 32, np.int32),
-             np.array([x0, T(0x13)], np.int32), np.array([x0, T(OP["SQUARE"], 3)], np.int32),     # POW: reserved
+             np.array([x0, T(OP["POW"])], np.int32), np.array([x0, T(OP["SQUARE"], 3)], np.int32),   # POW needs two
              np.array([x0] + [T(OP["DUP"])] * 31 + [T(OP["ADD"])] * 31, np.int32),      # well-formed: depth 32
              np.array([x0, T(OP["DEL"]), x0, T(OP["CUBE"])], np.int32)]                 # well-formed
     g, l, c = pack(progs, np.zeros(1, np.float32))
@@ -385,4 +385,73 @@ def test_stack_command_malformed_programs(oracle):
     assert np.all(_bits(a[:6]) == QNAN)
     assert a[6] == np.float32(64.0 ** 2) and a[7] == np.float32(64.0)
     orc = oracle.evaluate(g, l, c, X, y, 0.0)
+    assert len(parity.compare(a, orc)["bad"]) == 0
+
+
+def _with_variables(rng, text, d):
+    """Wrap a well-formed postfix text in COPY/PASTE pairs: some sub-results are copied to a variable
+    and pasted back later; every COPY has its PASTE, no variable is copied to twice while it holds a value."""
+    toks = text.split()
+    out, live, free = [], [], list(rng.permutation(32))
+    depth = 0
+    for t in toks:
+        out.append(t)
+        depth += {"ADD": -1, "SUB": -1, "MUL": -1, "DIV": -1, "POW": -1, "DEL": -1, "DUP": 1}.get(t, 0 if t.isalpha() else 1)
+        r = rng.random()
+        if depth < 1 or depth > 30:
+            continue
+        if r < 0.15 and free:
+            k = int(free.pop()); live.append(k); out.append(f"COPY@{k}")
+        elif r < 0.30 and live:
+            k = live.pop(int(rng.integers(len(live)))); free.append(k)
+            out += [f"PASTE@{k}", ["ADD", "MUL", "SUB"][int(rng.integers(3))]]
+    for k in live:
+        out += [f"PASTE@{k}", "ADD"]
+    return " ".join(out)
+
+
+def test_copy_paste_variables(oracle):
+    """COPY / PASTE: identities bit for bit, random programs with pairs against the
+    oracle and the blockwise kernel, and the malformed cases of the pairing rule."""
+    from tests.gpu_util import gpu_eval, gpu_outputs
+    rng = np.random.default_rng(33)
+    N, d = 700, 4
+    X = rng.uniform(-2, 2, (N, d)).astype(np.float32)
+    y = (X[:, 0] - X[:, 2]).astype(np.float32)
+    consts = []
+    pairs = [("x0 COPY@3 DEL x1 PASTE@3 SUB", "x1 x0 SUB"),
+             ("x0 SIN COPY@31 x1 MUL PASTE@31 DIV", "x0 SIN x1 MUL x0 SIN DIV"),
+             ("x2 COPY@0 PASTE@0 MUL COPY@0 PASTE@0 ADD", "x2 x2 MUL DUP ADD"),
+             ("x0 COPY@1 x1 COPY@2 ADD PASTE@1 PASTE@2 DIV MUL", "x0 x1 ADD x0 x1 DIV MUL")]
+    progs = [asm(t, consts)[0] for pr in pairs for t in pr]
+    g, l, c = pack(progs, consts)
+    out = gpu_outputs(g, l, c, X)
+    for i in range(len(pairs)):
+        assert np.array_equal(out[2 * i].view(np.uint32), out[2 * i + 1].view(np.uint32)), pairs[i]
+    names = ["ADD", "SUB", "MUL", "DIV", "SIN", "COS", "SQRT", "EXP", "SQUARE", "DUP", "SWAP", "DEL", "TANH"]
+    texts = [_with_variables(rng, t, d) for t in _random_gcl_programs(rng, 400, d, names)]
+    texts = [t for t in texts if len(t.split()) <= 200]
+    consts = []
+    progs = [asm(t, consts)[0] for t in texts]
+    g, l, c = pack(progs, consts)
+    a = gpu_eval(g, l, c, X, y, 0.001)
+    b = gpu_eval(g, l, c, X, y, 0.001, fn="beagle_eval_blockwise")
+    assert np.array_equal(_bits(a), _bits(b))
+    orc = oracle.evaluate(g, l, c, X, y, 0.001)
+    rep = parity.compare(a, orc)
+    assert len(rep["bad"]) == 0, parity.describe(rep, a, orc)
+    assert rep["malformed"] == 0 and rep["strict"] > 50
+    T = token
+    x0 = T(OP["LOAD"], 0)
+    bad = [[T(OP["PASTE"], 0)], [x0, T(OP["COPY"], 0)], [x0, T(OP["COPY"], 1), T(OP["COPY"], 1), T(OP["PASTE"], 1), T(OP["ADD"])],
+           [x0, T(OP["COPY"], 32), T(OP["PASTE"], 32), T(OP["ADD"])], [x0, T(OP["COPY"], 2), T(OP["PASTE"], 3), T(OP["ADD"])],
+           [T(OP["COPY"], 0), x0, T(OP["PASTE"], 0), T(OP["ADD"])],
+           [x0, T(OP["COPY"], 5)] + [T(OP["DUP"])] * 31 + [T(OP["PASTE"], 5)]]                       # PASTE overflows the stack
+    good = [[x0, T(OP["COPY"], 5)] + [T(OP["DUP"])] * 30 + [T(OP["PASTE"], 5)] + [T(OP["ADD"])] * 31]
+    progs = [np.array(q, np.int32) for q in bad + good]
+    g, l, c = pack(progs, np.zeros(1, np.float32))
+    X1 = np.full((64, 1), 2.0, np.float32); y1 = np.zeros(64, np.float32)
+    a = gpu_eval(g, l, c, X1, y1, 0.0)
+    assert np.all(_bits(a[:len(bad)]) == QNAN) and a[len(bad)] == np.float32(64.0 ** 2)
+    orc = oracle.evaluate(g, l, c, X1, y1, 0.0)
     assert len(parity.compare(a, orc)["bad"]) == 0

@@ -208,3 +208,30 @@ def test_f1_function_contract(oracle):
     out = np.array([1.0000001, -1.5, 3.0, np.inf], np.float32)
     assert np.all(np.isnan(_unary("ARCSIN", out))) and np.all(np.isnan(_unary("ARCCOS", out)))
     assert np.all(np.isnan(_unary("TAN", np.array([np.inf, -np.inf, np.nan], np.float32))))
+
+
+def test_pow_contract(oracle):
+    """POW = the C pow function against numpy in fp64: relative error within the contract the oracle's
+    bound assumes (c_pow), the special cases of the C function exact."""
+    c = _contract(oracle)
+    rng = np.random.default_rng(13)
+    a = np.concatenate([_sweep(rng, -20, 20, 60000, signed=False), rng.uniform(0.5, 2.0, 20000).astype(np.float32)])
+    b = np.concatenate([rng.uniform(-6, 6, 60000), rng.uniform(-40, 40, 20000)]).astype(np.float32)
+    got = _binary("POW", a, b).astype(np.float64)
+    with np.errstate(all="ignore"):
+        want = np.power(a.astype(np.float64), b.astype(np.float64))
+    fin = (np.abs(want) < 1e38) & (np.abs(want) > 1e-37)
+    err = np.abs(got - want)[fin]
+    bound = (c.c_pow * U * np.abs(want) + c.abs_floor)[fin]
+    assert fin.sum() > 60000 and np.all(err <= bound), float(np.max(err / bound))
+    an = -_sweep(rng, -6, 6, 4000, signed=False)
+    bn = rng.integers(-7, 8, 4000).astype(np.float32)
+    got = _binary("POW", an, bn).astype(np.float64)
+    want = np.power(an.astype(np.float64), bn.astype(np.float64))
+    assert np.all(np.abs(got - want) <= c.c_pow * U * np.abs(want) + c.abs_floor)
+    sa = np.array([-8.0, 3.0, 0.0, 0.0, 1.0, -1.0, np.nan, 2.0, 0.5], np.float32)
+    sb = np.array([0.5, 0.0, -1.0, 2.0, np.nan, np.inf, 0.0, np.inf, np.inf], np.float32)
+    got = _binary("POW", sa, sb)
+    with np.errstate(all="ignore"):
+        want = np.power(sa.astype(np.float64), sb.astype(np.float64)).astype(np.float32)
+    assert np.array_equal(np.isnan(got), np.isnan(want)) and np.array_equal(got[~np.isnan(got)], want[~np.isnan(want)])
