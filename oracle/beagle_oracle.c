@@ -32,6 +32,7 @@
  * P6 commutativity/antisymmetry, P7 protected-operator edge table, P8 brute force of all programs
  * of <= 3 tokens against an independent recursive evaluator (oracle/infix_check.py), P9 power-of-two
  * scaling, P10 overflow semantics, P11 the bound is a bound (fp32 mirror), P12 case duplication.
+ * P13-P18 the rest of Table 3, P19 the correlation fitness (orc_eval_corr).
  * Parity unpinned: nothing on the hot path.
  */
 #include <float.h>
@@ -351,6 +352,89 @@ int orc_eval(const int32_t* genomes, const int32_t* lengths, int64_t P,
                                      : ES / (double)N + 4.0 * U32 * fabs(fit) + c->abs_floor;
         if (flags_out) flags_out[p] = flags;
         if (depth_out) depth_out[p] = depth;
+    }
+    return 0;
+}
+
+/* orc_eval_corr — the paper's default objective, the correlation fitness (Eq. 1-2, printed again
+ * as Eq. 3-4 at P:494-501; D7). For every individual:
+ *   a case is a VALID pair when both the model output f_i and the target y_i are finite ("NaN, Inf, etc.");
+ *   c1 = number of valid/invalid pairs (exactly one side finite), c2 = number of invalid/invalid pairs;
+ *   r  = Pearson correlation of f and y over the valid pairs, means taken over the valid pairs (Eq. 1);
+ *   score = M r^4 (N - (c1 + c2)) - M (c1 - c2)                                                  (Eq. 2);
+ *   fitness = score - tax * L   (maximised; the length tax is a rate per command taken off the score).
+ * Readings (R23): r = 0 when fewer than two valid pairs are left or either side has zero variance there.
+ * Written as the definition: the textbook two-pass sums in fp64, nothing reordered.
+ * The bound follows the perturbation of r^2 = Sfy^2 / (Sff Syy) under |f_gpu,i - f_i| <= e_i plus the rounding of an
+ * fp32 two-pass summation in the contract's order (means of values shifted by one of them); it never changes a value.
+ * stats (NULL or P*4 doubles): r^2, valid pairs, c1, c2.                                                          */
+int orc_eval_corr(const int32_t* genomes, const int32_t* lengths, int64_t P,
+                  const float* consts, int64_t n_consts,
+                  const float* X, const float* y, int32_t N, int32_t d, float M, float tax,
+                  const orc_contract* c,
+                  float* fitness_out, double* bound_out, int32_t* flags_out, int32_t* depth_out, double* stats) {
+    if (P < 0 || N < 1 || N > ORC_MAX_N || d < 1 || !c) return -1;
+    double f[ORC_MAX_N], e[ORC_MAX_N];
+    int64_t off = 0;
+    for (int64_t p = 0; p < P; ++p) {
+        int L = lengths[p];
+        const uint32_t* tok = (const uint32_t*)genomes + off;
+        int inrange = (L >= 1 && L <= ORC_MAX_LEN);
+        int depth = inrange ? check_program(tok, L, n_consts, d) : -1;
+        if (inrange) off += L;
+        int flags = 0;
+        if (depth < 0) {
+            union { uint32_t u; float f; } qn; qn.u = 0x7FC00000u;
+            fitness_out[p] = qn.f;
+            if (bound_out) bound_out[p] = 0.0;
+            if (flags_out) flags_out[p] = ORC_FLAG_MALFORMED;
+            if (depth_out) depth_out[p] = 0;
+            if (stats) for (int k = 0; k < 4; ++k) stats[4 * p + k] = NAN;
+            continue;
+        }
+        int nv = 0, c1 = 0, c2 = 0;
+        for (int i = 0; i < N; ++i) {
+            pair o = run_case(tok, L, consts, X + (size_t)i * d, c, 0, &flags);
+            f[i] = o.v; e[i] = o.e;
+            int vf = isfinite(o.v), vy = isfinite((double)y[i]);
+            if (vf && vy) ++nv; else if (vf != vy) ++c1; else ++c2;
+        }
+        double r2 = 0.0, dr2 = 0.0;
+        if (nv >= 2) {
+            double sf = 0.0, sy = 0.0;
+            for (int i = 0; i < N; ++i) if (isfinite(f[i]) && isfinite((double)y[i])) { sf += f[i]; sy += (double)y[i]; }
+            const double mf = sf / nv, my = sy / nv;                       /* Eq. 1: the two means */
+            double Sff = 0.0, Syy = 0.0, Sfy = 0.0, A = 0.0, B = 0.0, Df = 0.0, Dy = 0.0;
+            for (int i = 0; i < N; ++i) if (isfinite(f[i]) && isfinite((double)y[i])) {
+                const double df = f[i] - mf, dy = (double)y[i] - my;
+                Sfy += dy * df; Sff += df * df; Syy += dy * dy;           /* Eq. 1: numerator, the two sums under the root */
+                A += fabs(dy) * e[i]; B += 2.0 * fabs(df) * e[i] + e[i] * e[i];
+                Df = fmax(Df, fabs(df)); Dy = fmax(Dy, fabs(dy));
+            }
+            const double g = (c->sum_per_case * (double)N + c->sum_const + 4.0) * U32;
+            const double dSfy = A + g * sqrt(Sff * Syy) + nv * g * g * 4.0 * Df * Dy + c->abs_floor;
+            const double dSff = B + g * Sff + nv * g * g * 4.0 * Df * Df;
+            const double dSyy = g * Syy + nv * g * g * 4.0 * Dy * Dy;
+            if (!(Sff <= FMAX && Syy <= FMAX && fabs(Sfy) <= FMAX) || Df * Df > FMAX || Dy * Dy > FMAX)
+                flags |= ORC_FLAG_CLASS_UNSTABLE;                        /* fp32 sums of squares overflow           */
+            if (Sff > 0.0 && Syy > 0.0) {
+                r2 = (Sfy * Sfy) / (Sff * Syy);                           /* "the r value is then squared"    */
+                if (dSff > 0.5 * Sff || dSyy > 0.5 * Syy) flags |= ORC_FLAG_UNSTABLE;    /* variance within its own error */
+                else {
+                    const double hi = (Sfy * Sfy + 2.0 * fabs(Sfy) * dSfy + dSfy * dSfy) / ((Sff - dSff) * (Syy - dSyy));
+                    const double lo = fmax(0.0, Sfy * Sfy - 2.0 * fabs(Sfy) * dSfy) / ((Sff + dSff) * (Syy + dSyy));
+                    dr2 = fmax(hi - r2, r2 - lo) + 4.0 * U32 * r2;
+                }
+            } else if (dSff > 0.0 && Syy > 0.0) flags |= ORC_FLAG_UNSTABLE;  /* zero variance here, maybe not in fp32 */
+        }
+        const double r4 = r2 * r2, dr4 = 2.0 * r2 * dr2 + dr2 * dr2;
+        const double score = (double)M * r4 * (double)nv - (double)M * (double)(c1 - c2);      /* Eq. 2 */
+        const double fit = score - (double)tax * (double)L;
+        fitness_out[p] = (float)fit;
+        if (bound_out) bound_out[p] = (double)M * nv * dr4 + 4.0 * U32 * (fabs((double)M * r4 * nv) + fabs((double)M * (c1 - c2)) + fabs(fit)) + c->abs_floor;
+        if (flags_out) flags_out[p] = flags;
+        if (depth_out) depth_out[p] = depth;
+        if (stats) { stats[4 * p] = r2; stats[4 * p + 1] = nv; stats[4 * p + 2] = c1; stats[4 * p + 3] = c2; }
     }
     return 0;
 }

@@ -55,6 +55,11 @@ def lib():
                                   ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p,
                                   ctypes.c_void_p]
         _lib.orc_default_contract.restype = None
+        _lib.orc_eval_corr.restype = ctypes.c_int
+        _lib.orc_eval_corr.argtypes = [ctypes.c_void_p, ctypes.c_void_p, ctypes.c_int64, ctypes.c_void_p, ctypes.c_int64,
+                                       ctypes.c_void_p, ctypes.c_void_p, ctypes.c_int32, ctypes.c_int32,
+                                       ctypes.c_float, ctypes.c_float, ctypes.POINTER(Contract),
+                                       ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p]
         _lib.orc_default_contract.argtypes = [ctypes.c_int, ctypes.POINTER(Contract)]
     return _lib
 
@@ -91,6 +96,30 @@ def evaluate(genomes, lengths, consts, X, y, tax, *, contract_=None, mode=0, wan
     if rc != 0:
         raise ValueError("orc_eval: bad arguments")
     return dict(fitness=fit, bound=bound, flags=flags, depth=depth, outputs=outs)
+
+
+def evaluate_corr(genomes, lengths, consts, X, y, M, tax, *, contract_=None):
+    """The correlation fitness (Eq. 1-2): dict(fitness, bound, flags, depth, stats f64[P,4] = r^2, valid, c1, c2)."""
+    genomes = np.ascontiguousarray(genomes, dtype=np.int32)
+    lengths = np.ascontiguousarray(lengths, dtype=np.int32)
+    consts = np.ascontiguousarray(consts, dtype=np.float32)
+    X = np.ascontiguousarray(X, dtype=np.float32)
+    y = np.ascontiguousarray(y, dtype=np.float32)
+    P = int(lengths.shape[0])
+    N, d = int(X.shape[0]), int(X.shape[1])
+    assert y.shape[0] == N
+    c = contract_ if contract_ is not None else contract(CONTRACT_B200)
+    fit = np.empty(P, np.float32)
+    bound = np.empty(P, np.float64)
+    flags = np.empty(P, np.int32)
+    depth = np.empty(P, np.int32)
+    stats = np.empty((P, 4), np.float64)
+    rc = lib().orc_eval_corr(_ptr(genomes), _ptr(lengths), P, _ptr(consts), int(consts.shape[0]),
+                             _ptr(X), _ptr(y), N, d, float(M), float(tax), ctypes.byref(c),
+                             _ptr(fit), _ptr(bound), _ptr(flags), _ptr(depth), _ptr(stats))
+    if rc != 0:
+        raise ValueError("orc_eval_corr: bad arguments")
+    return dict(fitness=fit, bound=bound, flags=flags, depth=depth, stats=stats)
 
 
 def evaluate_parallel(genomes, lengths, consts, X, y, tax, *, threads=None, contract_=None, mode=0):

@@ -611,3 +611,140 @@ def test_P18_copy_paste_variables(oracle):
     deep = asm("x0 COPY@3 " + "x0 " * 30 + "PASTE@3 " + "ADD " * 31)[0]
     r = ev(oracle, [deep], np.zeros(1, np.float32), np.ones((4, 2), np.float32), np.zeros(4, np.float32))
     assert r["depth"][0] == 32 and r["fitness"][0] == 32.0 ** 2
+
+
+# ---- P19: the correlation fitness (Eq. 1-2; oracle orc_eval_corr) ---------------------------------
+M_SCORE = 10000.0     # BConfig.MaxScore as the paper's logs imply it: ASR 0.32808 = 1,679,752 / 5,120,000 at N = 512
+
+
+def evc(oracle, texts, X, y, M=M_SCORE, tax=0.0):
+    consts = []
+    progs = [asm(t, consts)[0] for t in texts]
+    g, l, c = pack(progs, consts if consts else np.zeros(1, np.float32))
+    return oracle.evaluate_corr(g, l, c, X, y, M, tax), l
+
+
+def test_P19_correlation_worked_example_and_library(oracle):
+    # by hand: y = 1 2 3 4, f = 1 3 2 4: both centred sums of squares are 5, the cross sum is 4: r = 0.8, r^4 = 0.4096
+    X = np.array([[1.0], [3.0], [2.0], [4.0]], np.float32)
+    y = np.array([1.0, 2.0, 3.0, 4.0], np.float32)
+    r, _ = evc(oracle, ["x0"], X, y)
+    assert abs(r["fitness"][0] - 10000.0 * 0.4096 * 4) < 1e-6 * 16384 and abs(r["stats"][0, 0] - 0.64) < 1e-14
+    # the library routine on random data, outputs taken from the (pinned) evaluator
+    rng = np.random.default_rng(5)
+    X = rng.uniform(-2, 2, (300, 3)).astype(np.float32)
+    y = (X[:, 0] * X[:, 1] + 0.3 * rng.standard_normal(300)).astype(np.float32)
+    texts = ["x0 x1 MUL", "x0 x1 ADD SIN", "x2 x0 MUL x1 SUB", "x0 x1 MUL x2 0.1 MUL ADD"]
+    r, _ = evc(oracle, texts, X, y)
+    consts = []
+    progs = [asm(t, consts)[0] for t in texts]
+    outs = ev(oracle, progs, np.array(consts, np.float32), X, y, want_outputs=True)["outputs"]
+    for k in range(len(texts)):
+        rr = np.corrcoef(outs[k], y.astype(np.float64))[0, 1]
+        assert abs(r["stats"][k, 0] - rr * rr) < 1e-12
+        assert abs(r["fitness"][k] - M_SCORE * rr ** 4 * 300) <= 1e-6 * M_SCORE * 300
+        assert r["stats"][k, 1] == 300 and r["stats"][k, 2] == 0 and r["stats"][k, 3] == 0
+
+
+def test_P19_correlation_invariances_and_degenerate_cases(oracle):
+    rng = np.random.default_rng(6)
+    N = 128
+    X = rng.uniform(-2, 2, (N, 2)).astype(np.float32)
+    y = (X[:, 0] - 0.5 * X[:, 1]).astype(np.float32)
+    # r^2 does not change under f -> a f + b (a != 0, either sign): power-of-two a and a small b keep fp64 exactness close
+    r, l = evc(oracle, ["x0 x1 MUL x0 ADD", "x0 x1 MUL x0 ADD 4 MUL 3 ADD", "x0 x1 MUL x0 ADD -0.5 MUL 1 SUB"], X, y)
+    assert np.allclose(r["stats"][:, 0], r["stats"][0, 0], rtol=1e-12) and 0.0 < r["stats"][0, 0] < 1.0
+    # a perfect model, its negative and any increasing affine map of it all score M N; the score is linear in M
+    r, _ = evc(oracle, ["x0 x1 0.5 MUL SUB", "x1 0.5 MUL x0 SUB", "x0 x1 0.5 MUL SUB 8 MUL 2 ADD"], X, y)
+    assert np.allclose(r["fitness"], M_SCORE * N, rtol=1e-6)
+    r2, _ = evc(oracle, ["x0 x1 MUL"], X, y, M=2.0 * M_SCORE)
+    r1, _ = evc(oracle, ["x0 x1 MUL"], X, y)
+    assert abs(r2["fitness"][0] - 2.0 * r1["fitness"][0]) <= 1e-6 * abs(r2["fitness"][0])
+    # zero variance on the model's side: r = 0 (reading R23); the length tax is taken off the score per command
+    r, l = evc(oracle, ["1.5", "x0 x1 MUL"], X, y, tax=7.0)
+    assert r["fitness"][0] == -7.0 and r["stats"][0, 0] == 0.0
+    assert abs(r["fitness"][1] - (r1["fitness"][0] - 7.0 * 3)) <= 1e-6 * abs(r1["fitness"][0])
+    # independent of the order of the cases
+    perm = rng.permutation(N)
+    rp, _ = evc(oracle, ["x0 x1 MUL"], X[perm], y[perm])
+    assert abs(rp["stats"][0, 0] - r1["stats"][0, 0]) < 1e-13
+
+
+def test_P19_correlation_invalid_pairs(oracle):
+    """Eq. 2's counts: c1 valid/invalid pairs cost M each, c2 invalid/invalid pairs earn M each, and r is taken over the
+    valid pairs only. f = x0 * x1 with x1 = 1e30 where the model is to overflow, ARCSIN of 2 where it is to be NaN."""
+    N = 16
+    x0 = np.arange(1, N + 1, dtype=np.float32)
+    big = np.ones(N, np.float32)
+    big[[1, 5, 9]] = 1e30                       # f = x0 * big * big overflows at cases 1, 5, 9
+    x0[12] = 40.0
+    X = np.stack([x0, big], axis=1)
+    y = (3.0 * x0 + 1.0).astype(np.float32)     # perfectly correlated with x0 wherever both are finite
+    y[5] = np.nan                               # invalid / invalid at 5
+    y[2] = np.inf                               # valid model / invalid target at 2
+    r, _ = evc(oracle, ["x0 x1 MUL x1 MUL"], X, y)
+    nv, c1, c2 = r["stats"][0, 1:]
+    assert (nv, c1, c2) == (12, 3, 1)           # c1: cases 1, 9 (model) and 2 (target); c2: case 5
+    assert abs(r["stats"][0, 0] - 1.0) < 1e-12
+    assert abs(r["fitness"][0] - (M_SCORE * 12 - M_SCORE * (3 - 1))) < 1e-3
+    # NaN on the model's side counts like Inf; the valid pairs that are left decide r
+    X2 = np.stack([x0, np.where(np.arange(N) % 4 == 0, 2.0, 0.5).astype(np.float32)], axis=1)
+    y2 = (x0 * 2).astype(np.float32)
+    r, _ = evc(oracle, ["x1 ARCSIN 0 MUL x0 ADD"], X2, y2)
+    assert tuple(r["stats"][0, 1:]) == (12, 4, 0) and abs(r["stats"][0, 0] - 1.0) < 1e-12
+    assert abs(r["fitness"][0] - (M_SCORE * 12 - M_SCORE * 4)) < 1e-3
+    # fewer than two valid pairs: r = 0, the counts still score
+    y3 = np.full(N, np.nan, np.float32); y3[0] = 1.0
+    r, _ = evc(oracle, ["x0"], np.stack([x0, big], axis=1), y3)
+    assert tuple(r["stats"][0, :]) == (0.0, 1, 15, 0) and r["fitness"][0] == -M_SCORE * 15
+    # brute force over tiny data: the definition retyped with numpy on every subset mask of valid targets
+    rng = np.random.default_rng(9)
+    xs = rng.uniform(-1, 1, (6, 1)).astype(np.float32)
+    for mask in range(1, 64):
+        yy = rng.uniform(-1, 1, 6).astype(np.float32)
+        inv = np.array([(mask >> k) & 1 for k in range(6)], bool)
+        yy[inv] = np.inf
+        r, _ = evc(oracle, ["x0 SQUARE"], xs, yy)
+        v = ~inv
+        fo = xs[v, 0].astype(np.float64) ** 2
+        want = 0.0
+        if v.sum() >= 2:
+            want = np.corrcoef(fo, yy[v].astype(np.float64))[0, 1] ** 4
+        assert abs(r["fitness"][0] - (M_SCORE * want * v.sum() - M_SCORE * inv.sum())) <= 1e-6 * M_SCORE * 6 + 1e-3
+
+
+def test_P19_correlation_bound_is_a_bound(oracle):
+    """An fp32 evaluation of the same definition (IEEE per-command mirror outputs, numpy float32 two-pass sums) stays
+    within the oracle's certified bound wherever the oracle does not flag the individual."""
+    rng = np.random.default_rng(10)
+    N, d = 512, 3
+    X = rng.uniform(-3, 3, (N, d)).astype(np.float32)
+    y = (X[:, 0] * X[:, 1] - X[:, 2]).astype(np.float32)
+    from tests.test_gpu_edges import _random_gcl_programs
+    texts = _random_gcl_programs(rng, 400, d, ["ADD", "SUB", "MUL", "DIV", "SIN", "COS", "SQRT", "EXP", "LOG"])
+    consts = []
+    progs = [asm(t, consts)[0] for t in texts]
+    g, l, cst = pack(progs, consts)
+    ieee = oracle.contract(oracle.CONTRACT_IEEE)
+    ieee.sum_per_case = 1.0                          # numpy's pairwise float32 sums: any order
+    r = oracle.evaluate_corr(g, l, cst, X, y, M_SCORE, 0.0, contract_=ieee)
+    outs = oracle.evaluate(g, l, cst, X, y, 0.0, mode=1, want_outputs=True, contract_=ieee)["outputs"].astype(np.float32)
+    ok = (r["flags"] == 0)
+    assert ok.sum() > 100
+    worst = 0.0
+    for p in np.nonzero(ok)[0]:
+        f = outs[p]
+        v = np.isfinite(f) & np.isfinite(y)
+        nv = int(v.sum()); c1 = int((np.isfinite(f) != np.isfinite(y)).sum()); c2 = N - nv - c1
+        score = np.float32(0)
+        if nv >= 2:
+            fv, yv = f[v] - f[v][0], y[v] - y[v][0]
+            df = fv - np.float32(fv.sum(dtype=np.float32) / np.float32(nv)); dy = yv - np.float32(yv.sum(dtype=np.float32) / np.float32(nv))
+            sff, syy, sfy = (df * df).sum(dtype=np.float32), (dy * dy).sum(dtype=np.float32), (df * dy).sum(dtype=np.float32)
+            r2 = np.float32(sfy * sfy) / np.float32(sff * syy) if sff > 0 and syy > 0 else np.float32(0)
+            score = np.float32(M_SCORE) * np.float32(r2 * r2) * np.float32(nv)
+        score = float(score) - M_SCORE * (c1 - c2)
+        err = abs(score - float(r["fitness"][p]))
+        assert err <= r["bound"][p] + np.spacing(np.float32(abs(score))), (p, err, r["bound"][p])
+        worst = max(worst, err / max(r["bound"][p], 1e-300))
+    print("worst err / bound:", worst)
