@@ -122,6 +122,27 @@ beagle_status beagle_eval(const int32_t* genomes, const int32_t* lengths, int64_
                           const float* X, const float* y, int32_t N, int32_t d,
                           float tax, float* fitness_out, void* stream);
 
+/* beagle_eval_fit — the same path with the fitness function chosen by `fit`.
+ *
+ *   BEAGLE_FIT_MSE          fitness = MSE + tax * L (beagle_eval; M is ignored)
+ *   BEAGLE_FIT_CORRELATION  the paper's default objective (Eq. 1-2; Eq. 3-4 at P:494-501):
+ *                           a case is a valid pair when the model output and the target are both finite;
+ *                           c1 = pairs with exactly one side finite, c2 = pairs with neither;
+ *                           r = Pearson correlation over the valid pairs (means over the valid pairs);
+ *                           score = M r^4 (N - (c1 + c2)) - M (c1 - c2);  fitness = score - tax * L, MAXIMISED.
+ *                           r = 0 when fewer than two valid pairs are left or either side has zero variance
+ *                           there (R23). y may hold NaN / Inf. A well-formed program always gets a
+ *                           finite-or-NaN float; malformed programs get the canonical quiet NaN as in beagle_eval.
+ *   M                       the maximum score per case (BConfig.MaxScore; the paper's logs imply 10000)
+ *
+ * All other arguments, limits and errors as beagle_eval; an unknown `fit` returns BEAGLE_ERR_INVALID_ARG.       */
+#define BEAGLE_FIT_MSE         0
+#define BEAGLE_FIT_CORRELATION 1
+beagle_status beagle_eval_fit(const int32_t* genomes, const int32_t* lengths, int64_t P,
+                              const float* consts, int64_t n_consts,
+                              const float* X, const float* y, int32_t N, int32_t d,
+                              int32_t fit, float M, float tax, float* fitness_out, void* stream);
+
 /* beagle_eval_chunked — the same result for a colony held in HOST memory that may be larger than
  * the device budget ("manages populations in batches to ensure the GPU memory is
  * never exceeded"; R19). The colony is cut at individual boundaries into chunks of at

@@ -32,6 +32,7 @@ _i32, _i64, _f32, _vp = ctypes.c_int32, ctypes.c_int64, ctypes.c_float, ctypes.c
 
 _SIGNATURES = {
     "beagle_eval": (_i32, [_vp, _vp, _i64, _vp, _i64, _vp, _vp, _i32, _i32, _f32, _vp, _vp]),
+    "beagle_eval_fit": (_i32, [_vp, _vp, _i64, _vp, _i64, _vp, _vp, _i32, _i32, _i32, _f32, _f32, _vp, _vp]),
     "beagle_eval_chunked": (_i32, [_vp, _vp, _i64, _vp, _i64, _vp, _vp, _i32, _i32, _f32, _vp, _i64, _vp]),
     "beagle_eval_blockwise": (_i32, [_vp, _vp, _i64, _vp, _i64, _vp, _vp, _i32, _i32, _f32, _vp, _vp]),
     "beagle_debug_outputs": (_i32, [_vp, _vp, _i64, _vp, _i64, _vp, _i32, _i32, _vp, _vp]),
@@ -88,6 +89,15 @@ def beagle_eval(genomes, lengths, P, consts, n_consts, X, y, N, d, tax, fitness_
     _check(lib().beagle_eval(_ptr(genomes), _ptr(lengths), int(P), _ptr(consts), int(n_consts),
                              _ptr(X), _ptr(y), int(N), int(d), float(tax), _ptr(fitness_out),
                              int(stream) or None), "beagle_eval")
+
+
+FIT_MSE, FIT_CORRELATION = 0, 1
+
+
+def beagle_eval_fit(genomes, lengths, P, consts, n_consts, X, y, N, d, fit, M, tax, fitness_out, stream=0):
+    _check(lib().beagle_eval_fit(_ptr(genomes), _ptr(lengths), int(P), _ptr(consts), int(n_consts),
+                                 _ptr(X), _ptr(y), int(N), int(d), int(fit), float(M), float(tax), _ptr(fitness_out),
+                                 int(stream) or None), "beagle_eval_fit")
 
 
 def beagle_eval_chunked(h_genomes, h_lengths, P, h_consts, n_consts, X, y, N, d, tax, fitness_out,

@@ -18,6 +18,7 @@
 #include "ops.cuh"
 #include "uop.cuh"
 #include "interp.cuh"
+#include "fit_corr.cuh"
 
 namespace beagle {
 
@@ -59,7 +60,7 @@ struct Header {                                // device-resident results of the
 struct EvalParams {
     const int4* meta; const uint2* uops; const Header* hdr; unsigned int* queue;
     const float* xt; const float* ung; float* fitness; float* outputs;
-    float tax; int n; int npad; int d; int ring_bytes;
+    float tax; float M; int n; int npad; int d; int ring_bytes;   // M: the maximum score of the correlation fitness (f2)
     int rcp_col0;       // first tensor-memory column of the reciprocal rows: passes * d * 16
     int k_rcp;          // variables 0 .. k_rcp-1 have a reciprocal row (per pass)
     int k_un;           // variables 0 .. k_un-1 have their five unary rows staged in shared memory
@@ -517,7 +518,7 @@ __global__ void __launch_bounds__(1024) k_eval_blockwise(
     const int32_t* __restrict__ genomes, const long long* __restrict__ off, const int32_t* __restrict__ lengths,
     const int* __restrict__ depth, const float* __restrict__ consts, const float* __restrict__ X,
     const float* __restrict__ y, int n, int d, float tax, float* __restrict__ fitness, float* __restrict__ outputs,
-    const int* __restrict__ list, const int* __restrict__ count, long long P)
+    const int* __restrict__ list, const int* __restrict__ count, long long P, int fit, float M)
 {
     __shared__ float res[BEAGLE_MAX_N];
     const long long total = list ? (long long)*count : P;
@@ -564,10 +565,24 @@ __global__ void __launch_bounds__(1024) k_eval_blockwise(
                 }
             }
             if (outputs) outputs[(size_t)p * n + i] = st[sp - 1];
-            res[i] = y ? __fsub_rn(st[sp - 1], __ldg(y + i)) : 0.f;
+            res[i] = fit == BEAGLE_FIT_CORRELATION ? st[sp - 1] : (y ? __fsub_rn(st[sp - 1], __ldg(y + i)) : 0.f);
         }
         __syncthreads();
-        if (threadIdx.x < 32 && fitness) {
+        if (threadIdx.x < 32 && fitness && fit == BEAGLE_FIT_CORRELATION) {       // f2: fit_corr.cuh, the layout of k_eval
+            const int lane = threadIdx.x;
+            CorrState cs = { 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0 };
+            for (int c0 = 0; c0 < n; c0 += kCasesPerPass) {
+                float fv[16], yv[16];
+#pragma unroll
+                for (int k = 0; k < 16; ++k) {
+                    const int ci = c0 + (k >> 2) * 128 + lane * 4 + (k & 3);
+                    fv[k] = ci < n ? res[ci] : 0.f;
+                    yv[k] = ci < n ? __ldg(y + ci) : 0.f;
+                }
+                corr_pass(fv, yv, c0, n, lane, cs);
+            }
+            if (lane == 0) fitness[p] = corr_finish(cs, n, len, M, tax);
+        } else if (threadIdx.x < 32 && fitness) {
             const int lane = threadIdx.x;
             float acc = 0.f;
             for (int m = 0; m * 128 < n; ++m)
@@ -606,6 +621,8 @@ static Workspace g_ws;
 static int32_t g_last_cuda = 0;
 static int32_t g_launches = 0;
 static int32_t g_profiling = 0;
+struct FitSel { int kind; float M; };
+static FitSel g_fit = { BEAGLE_FIT_MSE, 0.f };   // set by the entry point for the duration of its call
 
 #define CU(call) do { cudaError_t e_ = (call); if (e_ != cudaSuccess) { g_last_cuda = (int32_t)e_; \
     return (e_ == cudaErrorMemoryAllocation) ? BEAGLE_ERR_NOMEM : BEAGLE_ERR_CUDA; } } while (0)
@@ -621,7 +638,8 @@ static beagle_status init_once()
     w.device_ok = (prop.major == 10);
     w.inited = true;
     if (!w.device_ok) return BEAGLE_ERR_UNSUPPORTED;
-    CU(cudaFuncSetAttribute(k_eval, cudaFuncAttributeMaxDynamicSharedMemorySize, w.smem_optin));
+    CU(cudaFuncSetAttribute(k_eval<BEAGLE_FIT_MSE>, cudaFuncAttributeMaxDynamicSharedMemorySize, w.smem_optin));
+    CU(cudaFuncSetAttribute(k_eval<BEAGLE_FIT_CORRELATION>, cudaFuncAttributeMaxDynamicSharedMemorySize, w.smem_optin));
     { uint32_t lut[kLutSize]; make_compile_lut(lut); CU(cudaMemcpyToSymbol(g_compile_lut, lut, sizeof(lut))); }
     CU(cudaMalloc(&w.bins, sizeof(int) * kNumBins));
     CU(cudaMalloc(&w.cursor, sizeof(int) * kNumBins));
@@ -790,7 +808,7 @@ static beagle_status run_eval(const int32_t* genomes, const int32_t* lengths, co
     if (!tp.fast) return BEAGLE_ERR_UNSUPPORTED;   // callers check first
     prm.rcp_col0 = tp.rcp_col0; prm.k_rcp = tp.k_rcp; prm.slot_col0 = tp.slot_col0; prm.tmem_slots = tp.tmem_slots;
     prm.meta = w.meta; prm.uops = w.uops; prm.hdr = w.hdr; prm.xt = w.xt; prm.ung = w.ung;
-    prm.fitness = fitness; prm.outputs = outputs; prm.tax = tax; prm.n = N; prm.npad = npad; prm.d = d;
+    prm.fitness = fitness; prm.outputs = outputs; prm.tax = tax; prm.M = g_fit.M; prm.n = N; prm.npad = npad; prm.d = d;
     const bool prof = g_profiling && w.prof_n < kProfMax;
     if (prof) {
         for (int i = 0; i < 2; ++i)
@@ -801,12 +819,13 @@ static beagle_status run_eval(const int32_t* genomes, const int32_t* lengths, co
     prm.ring_bytes = tp.ring_bytes; prm.k_un = tp.k_un;
     if (prm.ring_bytes < kStageBytesMax) return BEAGLE_ERR_UNSUPPORTED;
     prm.queue = &w.hdr->queue;
-    k_eval<<<w.num_sms, tp.threads, smem, st>>>(prm);
+    if (g_fit.kind == BEAGLE_FIT_CORRELATION) k_eval<BEAGLE_FIT_CORRELATION><<<w.num_sms, tp.threads, smem, st>>>(prm);
+    else k_eval<BEAGLE_FIT_MSE><<<w.num_sms, tp.threads, smem, st>>>(prm);
     ++g_launches;
     if (prof) { CU(cudaEventRecord(w.ev_k[2 * w.prof_n + 1], st)); ++w.prof_n; }
     // slow path: individuals whose micro-ops did not fit the promised workspace (normally none)
     k_eval_blockwise<<<w.num_sms * 2, (N + 31) / 32 * 32, 0, st>>>(genomes, w.off, lengths, w.depth, consts, X, y, N, d, tax,
-                                                                   fitness, outputs, w.slow_list, &w.hdr->n_slow, P);
+                                                                   fitness, outputs, w.slow_list, &w.hdr->n_slow, P, g_fit.kind, g_fit.M);
     ++g_launches;
     CU(cudaGetLastError());
     return BEAGLE_OK;
@@ -825,7 +844,7 @@ static beagle_status run_colony(const int32_t* genomes, const int32_t* lengths, 
     if (s != BEAGLE_OK) return s;
     if (fast) return run_eval(genomes, lengths, consts, X, y, P, N, d, tax, fitness, outputs, st);
     k_eval_blockwise<<<(unsigned)P, (N + 31) / 32 * 32, 0, st>>>(genomes, w.off, lengths, w.depth, consts, X, y, N, d, tax,
-                                                                fitness, outputs, nullptr, nullptr, P);
+                                                                fitness, outputs, nullptr, nullptr, P, g_fit.kind, g_fit.M);
     ++g_launches;
     CU(cudaGetLastError());
     return BEAGLE_OK;
@@ -849,6 +868,17 @@ beagle_status beagle_eval(const int32_t* genomes, const int32_t* lengths, int64_
     if ((s = reserve_P(P)) != BEAGLE_OK) return s;
     cudaStream_t st = (cudaStream_t)stream;
     return run_colony(genomes, lengths, P, consts, n_consts, X, y, N, d, tax, fitness_out, nullptr, -1, st);
+}
+
+beagle_status beagle_eval_fit(const int32_t* genomes, const int32_t* lengths, int64_t P,
+                              const float* consts, int64_t n_consts, const float* X, const float* y,
+                              int32_t N, int32_t d, int32_t fit, float M, float tax, float* fitness_out, void* stream)
+{
+    if (fit != BEAGLE_FIT_MSE && fit != BEAGLE_FIT_CORRELATION) return BEAGLE_ERR_INVALID_ARG;
+    g_fit.kind = fit; g_fit.M = M;
+    const beagle_status s = beagle_eval(genomes, lengths, P, consts, n_consts, X, y, N, d, tax, fitness_out, stream);
+    g_fit.kind = BEAGLE_FIT_MSE; g_fit.M = 0.f;
+    return s;
 }
 
 beagle_status beagle_debug_outputs(const int32_t* genomes, const int32_t* lengths, int64_t P,
@@ -881,7 +911,7 @@ beagle_status beagle_eval_blockwise(const int32_t* genomes, const int32_t* lengt
     if ((s = run_prepass(genomes, lengths, P, consts, n_consts, X, y, N, d, fitness_out, nullptr, -1, false, st)) != BEAGLE_OK) return s;
     const int threads = (N + 31) / 32 * 32;
     k_eval_blockwise<<<(unsigned)P, threads, 0, st>>>(genomes, w.off, lengths, w.depth, consts, X, y, N, d, tax,
-                                                      fitness_out, nullptr, nullptr, nullptr, P);
+                                                      fitness_out, nullptr, nullptr, nullptr, P, g_fit.kind, g_fit.M);
     ++g_launches;
     CU(cudaGetLastError());
     return BEAGLE_OK;

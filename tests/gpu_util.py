@@ -24,6 +24,19 @@ def gpu_eval(genomes, lengths, consts, X, y, tax, fn="beagle_eval"):
     return out[:P].cpu().numpy()
 
 
+def gpu_eval_fit(genomes, lengths, consts, X, y, fit, M, tax):
+    """float32[P] through beagle_eval_fit."""
+    P = int(len(lengths))
+    N, d = int(X.shape[0]), int(X.shape[1])
+    g, l = dev(genomes, np.int32), dev(lengths, np.int32)
+    c = dev(consts, np.float32) if len(consts) else None
+    Xd, yd = dev(X, np.float32), dev(y, np.float32)
+    out = torch.full((max(P, 1),), -12345.0, dtype=torch.float32, device="cuda")
+    api.beagle_eval_fit(g, l, P, c, len(consts), Xd, yd, N, d, fit, M, tax, out, torch.cuda.current_stream().cuda_stream)
+    torch.cuda.synchronize()
+    return out[:P].cpu().numpy()
+
+
 def gpu_eval_chunked(genomes, lengths, consts, X, y, tax, budget, pinned=True):
     P = int(len(lengths))
     N, d = int(X.shape[0]), int(X.shape[1])
