@@ -252,11 +252,23 @@ def run_ours(args):
     budget = cfg.budget_bytes or args.e2e_budget
     api.beagle_reserve_chunked(budget)
 
+    # --fit correlation: the paper's own objective (Eq. 1-2) on the same colony; M as the paper's
+    # logs imply it, the tax at the paper's default rate M N / 85 per command
+    fit = api.FIT_CORRELATION if args.fit == "correlation" else api.FIT_MSE
+    fit_M = 10000.0
+    tax = fit_M * N / 85.0 if fit == api.FIT_CORRELATION else cfg.tax
+
     def step_resident():
-        api.beagle_eval(g, l, P, c, len(consts), X, y, N, d, cfg.tax, out, sp)
+        if fit == api.FIT_MSE:
+            api.beagle_eval(g, l, P, c, len(consts), X, y, N, d, tax, out, sp)
+        else:
+            api.beagle_eval_fit(g, l, P, c, len(consts), X, y, N, d, fit, fit_M, tax, out, sp)
 
     def step_e2e():
-        api.beagle_eval_chunked(hg, hl, P, hc, len(consts), X, y, N, d, cfg.tax, out, budget, sp)
+        if fit == api.FIT_MSE:
+            api.beagle_eval_chunked(hg, hl, P, hc, len(consts), X, y, N, d, tax, out, budget, sp)
+        else:
+            api.beagle_eval_chunked_fit(hg, hl, P, hc, len(consts), X, y, N, d, fit, fit_M, tax, out, budget, sp)
         hout.copy_(out, non_blocking=True)
         stream.synchronize()
 
@@ -309,6 +321,7 @@ def run_ours(args):
         "warmup": args.warmup, "ms_per_step": ms_max / args.steps, "higher_is_better": True,
         "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
         "config": {"workload": workload_name(cfg) + ("" if args.population is None else f" [first {P}]"),
+                   "fitness": args.fit,
                    "tokens": T, "gp_ops_per_step": units, "timed": "beagle_eval, inputs resident in HBM" if resident
                    else "beagle_eval_chunked from pinned host memory (the colony exceeds its device budget)",
                    "l2": f"token stream {4 * T / 1e6:.0f} MB per step vs 126 MB L2 (inputs larger than L2)"
@@ -351,6 +364,8 @@ def main():
     ap.add_argument("--config", type=int, default=3, choices=[1, 2, 3, 4, 5])
     ap.add_argument("--population", type=int, default=None, help="first P individuals only (debugging; not a bench value)")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--fit", default="mse", choices=["mse", "correlation"],
+                    help="fitness function; mse is BASELINE.json's metric, correlation the paper's default objective (f2)")
     ap.add_argument("--e2e-steps", type=int, default=5)
     ap.add_argument("--e2e-budget", type=int, default=64 << 20, help="device genome budget of the end-to-end leg, bytes")
     ap.add_argument("--ref-sample", type=int, default=8192, help="individuals per step of --impl reference")

@@ -164,6 +164,14 @@ beagle_status beagle_eval_chunked(const int32_t* h_genomes, const int32_t* h_len
                                   float tax, float* fitness_out,
                                   int64_t device_budget_bytes, void* stream);
 
+/* beagle_eval_chunked_fit — beagle_eval_chunked with the fitness function of beagle_eval_fit (`fit`, `M` as there);
+ * bit-identical to beagle_eval_fit on the whole colony, for any budget.                                          */
+beagle_status beagle_eval_chunked_fit(const int32_t* h_genomes, const int32_t* h_lengths, int64_t P,
+                                      const float* h_consts, int64_t n_consts,
+                                      const float* X, const float* y, int32_t N, int32_t d,
+                                      int32_t fit, float M, float tax, float* fitness_out,
+                                      int64_t device_budget_bytes, void* stream);
+
 /* beagle_eval_blockwise — prior art kept as a measured baseline, not the product: the paper's own
  * mapping (one CUDA block per individual, one thread per fitness case, a 32-entry
  * per-thread stack in local memory, block aggregation in shared memory), same arguments and the

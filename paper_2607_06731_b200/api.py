@@ -34,6 +34,7 @@ _SIGNATURES = {
     "beagle_eval": (_i32, [_vp, _vp, _i64, _vp, _i64, _vp, _vp, _i32, _i32, _f32, _vp, _vp]),
     "beagle_eval_fit": (_i32, [_vp, _vp, _i64, _vp, _i64, _vp, _vp, _i32, _i32, _i32, _f32, _f32, _vp, _vp]),
     "beagle_eval_chunked": (_i32, [_vp, _vp, _i64, _vp, _i64, _vp, _vp, _i32, _i32, _f32, _vp, _i64, _vp]),
+    "beagle_eval_chunked_fit": (_i32, [_vp, _vp, _i64, _vp, _i64, _vp, _vp, _i32, _i32, _i32, _f32, _f32, _vp, _i64, _vp]),
     "beagle_eval_blockwise": (_i32, [_vp, _vp, _i64, _vp, _i64, _vp, _vp, _i32, _i32, _f32, _vp, _vp]),
     "beagle_debug_outputs": (_i32, [_vp, _vp, _i64, _vp, _i64, _vp, _i32, _i32, _vp, _vp]),
     "beagle_debug_schedule": (_i32, [_i64, _vp, _vp, _vp, _vp]),
@@ -106,6 +107,14 @@ def beagle_eval_chunked(h_genomes, h_lengths, P, h_consts, n_consts, X, y, N, d,
                                      int(n_consts), _ptr(X), _ptr(y), int(N), int(d), float(tax),
                                      _ptr(fitness_out), int(device_budget_bytes), int(stream) or None),
            "beagle_eval_chunked")
+
+
+def beagle_eval_chunked_fit(h_genomes, h_lengths, P, h_consts, n_consts, X, y, N, d, fit, M, tax, fitness_out,
+                            device_budget_bytes, stream=0):
+    _check(lib().beagle_eval_chunked_fit(_ptr(h_genomes), _ptr(h_lengths), int(P), _ptr(h_consts), int(n_consts),
+                                         _ptr(X), _ptr(y), int(N), int(d), int(fit), float(M), float(tax),
+                                         _ptr(fitness_out), int(device_budget_bytes), int(stream) or None),
+           "beagle_eval_chunked_fit")
 
 
 def beagle_eval_blockwise(genomes, lengths, P, consts, n_consts, X, y, N, d, tax, fitness_out, stream=0):

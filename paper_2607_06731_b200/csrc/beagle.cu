@@ -521,6 +521,8 @@ __global__ void __launch_bounds__(1024) k_eval_blockwise(
     const int* __restrict__ list, const int* __restrict__ count, long long P, int fit, float M)
 {
     __shared__ float res[BEAGLE_MAX_N];
+    bool y_finite = true;
+    if (fit == BEAGLE_FIT_CORRELATION) y_finite = __syncthreads_and(threadIdx.x >= n || finite32(__ldg(y + threadIdx.x)));
     const long long total = list ? (long long)*count : P;
     for (long long idx = blockIdx.x; idx < total; idx += gridDim.x) {
         const long long p = list ? (long long)list[idx] : idx;
@@ -579,7 +581,7 @@ __global__ void __launch_bounds__(1024) k_eval_blockwise(
                     fv[k] = ci < n ? res[ci] : 0.f;
                     yv[k] = ci < n ? __ldg(y + ci) : 0.f;
                 }
-                corr_pass(fv, yv, c0, n, lane, cs);
+                corr_pass(fv, yv, c0, n, lane, y_finite, cs);
             }
             if (lane == 0) fitness[p] = corr_finish(cs, n, len, M, tax);
         } else if (threadIdx.x < 32 && fitness) {
@@ -732,7 +734,8 @@ static TmemPlan tmem_plan(int N, int d)
     // every warp keeps room for at least one stage of the longest program
     const int warps = t.threads / 32;
     const int npad = (N + kCasePad - 1) / kCasePad * kCasePad;
-    const long long fixed = ((64 + warps * kStagesMax * 8 + 127) & ~127) + (long long)npad * 4 + (long long)kEvalMetaBytes * warps;
+    const long long fixed = ((64 + warps * kStagesMax * 8 + 127) & ~127) + (long long)npad * 4 * (g_fit.kind == BEAGLE_FIT_CORRELATION ? 2 : 1)
+                            + (long long)kEvalMetaBytes * warps;      // correlation: y and the centred y (eval_kernel.inc)
     const long long spare = (long long)g_ws.smem_optin - fixed - (long long)warps * ((kStageBytesMax + 127) & ~127);
     long long ku = spare / (5ll * npad * 4);
     t.k_un = (int)(ku < 0 ? 0 : (ku > d ? d : ku));
@@ -952,6 +955,21 @@ beagle_status beagle_reserve_chunked(int64_t device_budget_bytes)
     const long long cap_words = half / 4 - 3;
     if ((s = reserve_U(2 * cap_words + 2)) != BEAGLE_OK) return s;
     return BEAGLE_OK;
+}
+
+beagle_status beagle_eval_chunked(const int32_t*, const int32_t*, int64_t, const float*, int64_t, const float*, const float*,
+                                  int32_t, int32_t, float, float*, int64_t, void*);
+beagle_status beagle_eval_chunked_fit(const int32_t* h_genomes, const int32_t* h_lengths, int64_t P,
+                                      const float* h_consts, int64_t n_consts, const float* X, const float* y,
+                                      int32_t N, int32_t d, int32_t fit, float M, float tax, float* fitness_out,
+                                      int64_t device_budget_bytes, void* stream)
+{
+    if (fit != BEAGLE_FIT_MSE && fit != BEAGLE_FIT_CORRELATION) return BEAGLE_ERR_INVALID_ARG;
+    g_fit.kind = fit; g_fit.M = M;
+    const beagle_status s = beagle_eval_chunked(h_genomes, h_lengths, P, h_consts, n_consts, X, y, N, d, tax, fitness_out,
+                                                device_budget_bytes, stream);
+    g_fit.kind = BEAGLE_FIT_MSE; g_fit.M = 0.f;
+    return s;
 }
 
 beagle_status beagle_eval_chunked(const int32_t* h_genomes, const int32_t* h_lengths, int64_t P,
