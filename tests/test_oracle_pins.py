@@ -748,3 +748,43 @@ def test_P19_correlation_bound_is_a_bound(oracle):
         assert err <= r["bound"][p] + np.spacing(np.float32(abs(score))), (p, err, r["bound"][p])
         worst = max(worst, err / max(r["bound"][p], 1e-300))
     print("worst err / bound:", worst)
+
+
+# ---- P20: Monte-Carlo ranking (Table 2; oracle/ranking.py) ------------------------------------------
+def test_P20_ranking_table_and_deciles():
+    from oracle import ranking as R
+    # Table 2 as printed, top row first; its mean is exactly one child per individual: a stable population
+    printed = [4, 2.5, 1.5, 1, 0.5, 0.25, 0.15, 0.06, 0.03, 0.01]
+    assert list(R.EXPECTED_CHILDREN[::-1]) == printed and abs(sum(printed) - 10.0) < 1e-12
+    # distinct fitnesses 0..999 (to be maximised), sample = 5, 15, 25, ...: individual i has ceil((i - 5) / 10) samples below it
+    f = np.arange(1000, dtype=np.float32)
+    sample = np.arange(5, 1000, 10)
+    dec, hist, kids = R.rank_deciles(f, sample, True)
+    want = np.minimum(9, np.maximum(0, -(-(np.arange(1000) - 5) // 10)) // 10)
+    assert np.array_equal(dec, want) and hist.sum() == 1000 and np.all(np.abs(hist - 100) <= 10)
+    assert abs(kids.mean() - 1.0) < 0.05
+    # minimised (MSE): the order flips
+    dec2, _, _ = R.rank_deciles(f, sample, False)
+    assert np.array_equal(dec2, R.rank_deciles(-f, sample, True)[0]) and dec2[0] == 9 and dec2[999] == 0
+    # NaN is worse than everything, +inf MSE is worse than any finite MSE; ties share the lower group
+    f3 = np.array([1.0, np.nan, np.inf, 2.0, 2.0, 0.5], np.float32)
+    dec3, _, _ = R.rank_deciles(f3, np.arange(6), False)      # the sample is the whole population: 6 samples
+    # strictly worse counts: 1.0 -> {nan, inf, 2, 2} = 4; nan -> 0; inf -> 0 (nan ties at -inf); 2.0 -> {nan, inf} = 2; 0.5 -> 5
+    assert list(dec3) == [min(9, 10 * c // 6) for c in (4, 0, 0, 2, 2, 5)]
+
+
+def test_P20_ranking_brute_force_against_sorting():
+    from oracle import ranking as R
+    rng = np.random.default_rng(20)
+    for trial in range(20):
+        P = int(rng.integers(5, 400))
+        f = rng.standard_normal(P).astype(np.float32)
+        f[rng.random(P) < 0.05] = np.nan
+        f = np.round(f, 1) if trial % 2 else f                # ties
+        sample = rng.integers(0, P, 100)
+        for mx in (True, False):
+            dec, hist, _ = R.rank_deciles(f, sample, mx)
+            g = np.where(np.isnan(f), -np.inf, f if mx else -f).astype(np.float64)
+            srt = np.sort(g[sample])
+            worse = np.searchsorted(srt, g, side="left")      # samples strictly below
+            assert np.array_equal(dec, np.minimum(9, worse // 10)) and np.array_equal(hist, np.bincount(dec, minlength=10))
