@@ -172,6 +172,26 @@ beagle_status beagle_eval_chunked_fit(const int32_t* h_genomes, const int32_t* h
                                       int32_t fit, float M, float tax, float* fitness_out,
                                       int64_t device_budget_bytes, void* stream);
 
+/* beagle_rank — Monte-Carlo ranking, the step that follows scoring:
+ * "Beagle takes a random sample of 100 individuals and uses those 100 individuals to estimate the population
+ * percentiles. Through one pass of the population then, individuals are assigned to their specific percentile and are
+ * given rank proportional breeding rights" (Table 2). The random draw is the caller's, so the call is deterministic.
+ *
+ *   fitness      DEVICE  P fp32, as written by beagle_eval / beagle_eval_fit (stays on the device: no D2H of P floats)
+ *   sample_idx   DEVICE  n_sample int64 indices into fitness, each in [0, P)  (trusted; the paper draws 100)
+ *   n_sample     1 .. 1024
+ *   maximise     0: lower fitness is better (MSE); non-zero: higher is better (correlation score)
+ *   decile_out   DEVICE  P bytes: g = min(9, 10 * worse / n_sample), worse = number of sampled individuals strictly
+ *                        worse than this one; group g is Table 2's row "percentile >= 10 g". A NaN fitness is worse
+ *                        than every number; equal fitnesses are not strictly worse (R24).
+ *   hist_out     DEVICE  10 int64: individuals per group (zeroed by the call); may be NULL
+ *
+ * BEAGLE_TABLE2[g] = expected number of children of group g (Table 2): expected births of the next
+ * generation = sum over g of hist_out[g] * BEAGLE_TABLE2[g].                                                    */
+static const float BEAGLE_TABLE2[10] = { 0.01f, 0.03f, 0.06f, 0.15f, 0.25f, 0.5f, 1.0f, 1.5f, 2.5f, 4.0f };
+beagle_status beagle_rank(const float* fitness, int64_t P, const int64_t* sample_idx, int32_t n_sample,
+                          int32_t maximise, uint8_t* decile_out, int64_t* hist_out, void* stream);
+
 /* beagle_eval_blockwise — prior art kept as a measured baseline, not the product: the paper's own
  * mapping (one CUDA block per individual, one thread per fitness case, a 32-entry
  * per-thread stack in local memory, block aggregation in shared memory), same arguments and the

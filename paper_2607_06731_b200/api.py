@@ -35,6 +35,7 @@ _SIGNATURES = {
     "beagle_eval_fit": (_i32, [_vp, _vp, _i64, _vp, _i64, _vp, _vp, _i32, _i32, _i32, _f32, _f32, _vp, _vp]),
     "beagle_eval_chunked": (_i32, [_vp, _vp, _i64, _vp, _i64, _vp, _vp, _i32, _i32, _f32, _vp, _i64, _vp]),
     "beagle_eval_chunked_fit": (_i32, [_vp, _vp, _i64, _vp, _i64, _vp, _vp, _i32, _i32, _i32, _f32, _f32, _vp, _i64, _vp]),
+    "beagle_rank": (_i32, [_vp, _i64, _vp, _i32, _i32, _vp, _vp, _vp]),
     "beagle_eval_blockwise": (_i32, [_vp, _vp, _i64, _vp, _i64, _vp, _vp, _i32, _i32, _f32, _vp, _vp]),
     "beagle_debug_outputs": (_i32, [_vp, _vp, _i64, _vp, _i64, _vp, _i32, _i32, _vp, _vp]),
     "beagle_debug_schedule": (_i32, [_i64, _vp, _vp, _vp, _vp]),
@@ -115,6 +116,14 @@ def beagle_eval_chunked_fit(h_genomes, h_lengths, P, h_consts, n_consts, X, y, N
                                          _ptr(X), _ptr(y), int(N), int(d), int(fit), float(M), float(tax),
                                          _ptr(fitness_out), int(device_budget_bytes), int(stream) or None),
            "beagle_eval_chunked_fit")
+
+
+TABLE2 = (0.01, 0.03, 0.06, 0.15, 0.25, 0.5, 1.0, 1.5, 2.5, 4.0)   # include/beagle.h BEAGLE_TABLE2 (Table 2)
+
+
+def beagle_rank(fitness, P, sample_idx, n_sample, maximise, decile_out, hist_out=None, stream=0):
+    _check(lib().beagle_rank(_ptr(fitness), int(P), _ptr(sample_idx), int(n_sample), int(bool(maximise)),
+                             _ptr(decile_out), _ptr(hist_out), int(stream) or None), "beagle_rank")
 
 
 def beagle_eval_blockwise(genomes, lengths, P, consts, n_consts, X, y, N, d, tax, fitness_out, stream=0):

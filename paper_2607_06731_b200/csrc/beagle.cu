@@ -19,6 +19,7 @@
 #include "uop.cuh"
 #include "interp.cuh"
 #include "fit_corr.cuh"
+#include "rank.cuh"
 
 namespace beagle {
 
@@ -612,6 +613,7 @@ struct Workspace {
     uint2* uops = nullptr;
     int* bins = nullptr; int* cursor = nullptr; int* binstart = nullptr; long long* binubase = nullptr;
     float* xt = nullptr; float* ung = nullptr; Header* hdr = nullptr; long long* h_T = nullptr;
+    unsigned long long* rank_hist = nullptr;   // beagle_rank's histogram when the caller wants none
     // chunked staging
     long long stage_bytes = 0; unsigned char* stage[2] = { nullptr, nullptr };
     float* stage_consts = nullptr; long long stage_consts_cap = 0;
@@ -884,6 +886,30 @@ beagle_status beagle_eval_fit(const int32_t* genomes, const int32_t* lengths, in
     return s;
 }
 
+beagle_status beagle_rank(const float* fitness, int64_t P, const int64_t* sample_idx, int32_t n_sample,
+                          int32_t maximise, uint8_t* decile_out, int64_t* hist_out, void* stream)
+{
+    if (P < 0 || n_sample < 1 || n_sample > kRankMaxSample) return BEAGLE_ERR_INVALID_ARG;
+    if (P > 0 && (!fitness || !sample_idx || !decile_out)) return BEAGLE_ERR_INVALID_ARG;
+    g_launches = 0;
+    beagle_status s;
+    if ((s = init_once()) != BEAGLE_OK) return s;
+    cudaStream_t st = (cudaStream_t)stream;
+    Workspace& w = g_ws;
+    if (!w.rank_hist) CU(cudaMalloc(&w.rank_hist, 10 * sizeof(unsigned long long)));
+    unsigned long long* hist = hist_out ? reinterpret_cast<unsigned long long*>(hist_out) : w.rank_hist;
+    CU(cudaMemsetAsync(hist, 0, 10 * sizeof(unsigned long long), st));
+    if (P == 0) return BEAGLE_OK;
+    long long blocks = (P + kRankThreads * 8 - 1) / (kRankThreads * 8);
+    const long long cap = (long long)w.num_sms * 8;
+    blocks = blocks > cap ? cap : blocks;
+    k_rank<<<(unsigned)blocks, kRankThreads, 0, st>>>(fitness, P, reinterpret_cast<const long long*>(sample_idx), n_sample,
+                                                      maximise != 0, decile_out, hist);
+    ++g_launches;
+    CU(cudaGetLastError());
+    return BEAGLE_OK;
+}
+
 beagle_status beagle_debug_outputs(const int32_t* genomes, const int32_t* lengths, int64_t P,
                                    const float* consts, int64_t n_consts, const float* X, int32_t N, int32_t d,
                                    float* out_PxN, void* stream)
@@ -1071,7 +1097,7 @@ void beagle_release(void)
     cudaDeviceSynchronize();
     cudaFree(w.off); cudaFree(w.depth); cudaFree(w.perm); cudaFree(w.meta); cudaFree(w.sched); cudaFree(w.sched_u);
     cudaFree(w.slow_list); cudaFree(w.bsum); cudaFree(w.uops);
-    cudaFree(w.stage[0]); cudaFree(w.stage[1]); cudaFree(w.stage_consts);
+    cudaFree(w.stage[0]); cudaFree(w.stage[1]); cudaFree(w.stage_consts); cudaFree(w.rank_hist); w.rank_hist = nullptr;
     w.off = nullptr; w.depth = nullptr; w.perm = nullptr; w.meta = nullptr;
     w.slow_list = nullptr; w.bsum = nullptr; w.uops = nullptr; w.cap_P = 0; w.cap_U = 0;
     w.promised_P = 0; w.promised_T = 0;
