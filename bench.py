@@ -254,21 +254,21 @@ def run_ours(args):
 
     # --fit correlation: the paper's own objective (Eq. 1-2) on the same colony; M as the paper's
     # logs imply it, the tax at the paper's default rate M N / 85 per command
-    fit = api.FIT_CORRELATION if args.fit == "correlation" else api.FIT_MSE
+    fit_kind = api.FIT_CORRELATION if args.fit == "correlation" else api.FIT_MSE
     fit_M = 10000.0
-    tax = fit_M * N / 85.0 if fit == api.FIT_CORRELATION else cfg.tax
+    tax = fit_M * N / 85.0 if fit_kind == api.FIT_CORRELATION else cfg.tax
 
     def step_resident():
-        if fit == api.FIT_MSE:
+        if fit_kind == api.FIT_MSE:
             api.beagle_eval(g, l, P, c, len(consts), X, y, N, d, tax, out, sp)
         else:
-            api.beagle_eval_fit(g, l, P, c, len(consts), X, y, N, d, fit, fit_M, tax, out, sp)
+            api.beagle_eval_fit(g, l, P, c, len(consts), X, y, N, d, fit_kind, fit_M, tax, out, sp)
 
     def step_e2e():
-        if fit == api.FIT_MSE:
+        if fit_kind == api.FIT_MSE:
             api.beagle_eval_chunked(hg, hl, P, hc, len(consts), X, y, N, d, tax, out, budget, sp)
         else:
-            api.beagle_eval_chunked_fit(hg, hl, P, hc, len(consts), X, y, N, d, fit, fit_M, tax, out, budget, sp)
+            api.beagle_eval_chunked_fit(hg, hl, P, hc, len(consts), X, y, N, d, fit_kind, fit_M, tax, out, budget, sp)
         hout.copy_(out, non_blocking=True)
         stream.synchronize()
 
@@ -343,6 +343,22 @@ def run_ours(args):
         "result_check": {"finite": int(np.isfinite(fit).sum()), "nan": int(np.isnan(fit).sum()),
                          "inf": int(np.isinf(fit).sum())},
     }
+    # the step that follows scoring: Monte-Carlo ranking of the fitness vector left on the device; timed on its
+    # own after the main measurement (not part of `value`), against the HBM roofline: 4 bytes in + 1 byte out per individual
+    if rank == 0:
+        rs = torch.from_numpy(np.random.default_rng(7).integers(0, P, 100).astype(np.int64)).to(dev)
+        dec = torch.empty(P, dtype=torch.uint8, device=dev); hist = torch.empty(10, dtype=torch.int64, device=dev)
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        for _ in range(3):
+            api.beagle_rank(out, P, rs, 100, fit_kind != api.FIT_MSE, dec, hist, sp)
+        e0.record(stream)
+        for _ in range(20):
+            api.beagle_rank(out, P, rs, 100, fit_kind != api.FIT_MSE, dec, hist, sp)
+        e1.record(stream); stream.synchronize()
+        rms = e0.elapsed_time(e1) / 20
+        births = float((hist.cpu().numpy() * np.array(api.TABLE2)).sum())
+        line["ranking"] = {"ms": rms, "hbm_gbs": 5.0 * P / (rms * 1e-3) / 1e9, "expected_births_over_P": births / P,
+                           "note": "beagle_rank (memset + k_rank) on the resident fitness vector; fits L2, launch-bound at this P"}
     if not args.no_cpu_baseline and world == 1:
         n_ind = min(P, 1 << 16)
         col = colonies.Colony(cfg, tokens[: int(lengths[:n_ind].sum())], lengths[:n_ind], consts, Xh, yh, cfg.tax)
