@@ -67,6 +67,7 @@ struct EvalParams {
     int k_un;           // variables 0 .. k_un-1 have their five unary rows staged in shared memory
     int slot_col0;      // first tensor-memory column of the slot blocks
     int tmem_slots;     // S_T: slots per warp held in tensor memory (the deeper ones are in local memory)
+    int off_ys, off_meta, off_un, off_ring;   // shared-memory layout, byte offsets: y (and centred y), queue windows, unary rows, rings
 };
 
 // ---- PTX helpers: mbarrier, TMA bulk copy -----------------------------------------------------------
@@ -700,7 +701,7 @@ static long long uop_entries_bound(long long P, long long T) { return T + 4 * P 
 // quarter (8, 7 or 6: 1024, 896 or 768 threads) is chosen so that three slot rows per warp remain when
 // possible. fast == false: the variable block alone does not fit (d > 32 at N <= 512, d > 16 beyond), and the
 // call takes the blockwise kernel.
-struct TmemPlan { bool fast; int threads; int rcp_col0; int k_rcp; int slot_col0; int tmem_slots; int k_un; int ring_bytes; size_t smem; };
+struct TmemPlan { bool fast; int threads; int rcp_col0; int k_rcp; int slot_col0; int tmem_slots; int k_un; int ring_bytes; size_t smem; int off_ys, off_meta, off_un, off_ring; };
 static TmemPlan tmem_plan(int N, int d)
 {
     TmemPlan t = { false, kEvalThreads, 0, 0, 0, 0, 0, 0, 0 };
@@ -746,6 +747,9 @@ static TmemPlan tmem_plan(int N, int d)
     if (ring > (long long)kStagesMax * kStageBytesMax) ring = (long long)kStagesMax * kStageBytesMax;
     t.ring_bytes = (int)ring;
     t.smem = (size_t)(fixed + un_bytes + ring * warps);
+    t.off_ys = (64 + warps * kStagesMax * 8 + 127) & ~127;
+    t.off_meta = (int)(fixed - (long long)kEvalMetaBytes * warps);
+    t.off_un = (int)fixed; t.off_ring = (int)(fixed + un_bytes);
     return t;
 }
 
@@ -822,6 +826,7 @@ static beagle_status run_eval(const int32_t* genomes, const int32_t* lengths, co
     }
     const size_t smem = tp.smem;
     prm.ring_bytes = tp.ring_bytes; prm.k_un = tp.k_un;
+    prm.off_ys = tp.off_ys; prm.off_meta = tp.off_meta; prm.off_un = tp.off_un; prm.off_ring = tp.off_ring;
     if (prm.ring_bytes < kStageBytesMax) return BEAGLE_ERR_UNSUPPORTED;
     prm.queue = &w.hdr->queue;
     if (g_fit.kind == BEAGLE_FIT_CORRELATION) k_eval<BEAGLE_FIT_CORRELATION><<<w.num_sms, tp.threads, smem, st>>>(prm);
