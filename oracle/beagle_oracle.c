@@ -439,6 +439,85 @@ int orc_eval_corr(const int32_t* genomes, const int32_t* lengths, int64_t P,
     return 0;
 }
 
+/* orc_eval_std — the point-to-point integer-reward family StdFitFunc / StdSquareFitFunc / StdCubeFitFunc /
+ * StdHyperFitFunc (PAPER.md:490 and Eq. 5 at P:503-506; D9). For every valid pair (both sides finite):
+ *     M                                       if max(|f|, |y|) = 0
+ *     round(M q^p - M/11)                      if f y < 0          q = min(|f|, |y|) / max(|f|, |y|)
+ *     round(M q^p)                             otherwise
+ * with p = 1 (Eq. 5 as printed), 2, 3, 8 for the Square, Cube and Hyper variants; a pair with exactly one side finite
+ * scores -M, a pair with neither +M (the convention of Eq. 2; FitFunctionIfInvalid's values are not printed);
+ * score = sum over the cases; fitness = score - tax * L, maximised.
+ * Readings (R25): `round` is round-half-to-even (the default of the paper's implementation language); the
+ * powers apply to the ratio q before scaling by M (applied to the integer reward they would turn the penalty of an
+ * opposite sign into a bonus); "f y < 0" is decided on the signs (no underflow of the product).
+ * The reward is an integer decided by floating point, so it is taken in the paper's precision, fp32, on both sides:
+ * the arithmetic below is fp32, in the order |.|, min/max, one division, the power by squarings, * M, - M/11, rintf.
+ * The bound: a case can differ from the device's by |dt| + 1 when its unrounded value t is within dt of a rounding
+ * boundary, where dt follows from the output bound e; otherwise by nothing.                                       */
+int orc_eval_std(const int32_t* genomes, const int32_t* lengths, int64_t P,
+                 const float* consts, int64_t n_consts,
+                 const float* X, const float* y, int32_t N, int32_t d, int32_t power, float M, float tax,
+                 const orc_contract* c,
+                 float* fitness_out, double* bound_out, int32_t* flags_out, int32_t* depth_out) {
+    if (P < 0 || N < 1 || N > ORC_MAX_N || d < 1 || !c) return -1;
+    if (power != 1 && power != 2 && power != 3 && power != 8) return -1;
+    int64_t off = 0;
+    const float pen = M / 11.0f;
+    for (int64_t p = 0; p < P; ++p) {
+        int L = lengths[p];
+        const uint32_t* tok = (const uint32_t*)genomes + off;
+        int inrange = (L >= 1 && L <= ORC_MAX_LEN);
+        int depth = inrange ? check_program(tok, L, n_consts, d) : -1;
+        if (inrange) off += L;
+        int flags = 0;
+        if (depth < 0) {
+            union { uint32_t u; float f; } qn; qn.u = 0x7FC00000u;
+            fitness_out[p] = qn.f;
+            if (bound_out) bound_out[p] = 0.0;
+            if (flags_out) flags_out[p] = ORC_FLAG_MALFORMED;
+            if (depth_out) depth_out[p] = 0;
+            continue;
+        }
+        double score = 0.0, E = 0.0;
+        for (int i = 0; i < N; ++i) {
+            pair o = run_case(tok, L, consts, X + (size_t)i * d, c, 0, &flags);
+            const int vf = isfinite(o.v), vy = isfinite((double)y[i]);
+            if (!(vf && vy)) { score += (vf != vy) ? -(double)M : (double)M; continue; }
+            const float f = (float)o.v, yy = y[i];
+            const float a = fabsf(f), b = fabsf(yy);
+            const float mx = fmaxf(a, b), mn = fminf(a, b);
+            if (mx == 0.0f) {
+                score += (double)M;
+                if (o.e > 0.0) E += (double)M;              /* the device's output may be non-zero */
+                continue;
+            }
+            const float q = mn / mx;
+            float qp = q;
+            if (power == 2) qp = q * q;
+            else if (power == 3) qp = (q * q) * q;
+            else if (power == 8) { qp = q * q; qp = qp * qp; qp = qp * qp; }
+            const int opposite = (f < 0.0f && yy > 0.0f) || (f > 0.0f && yy < 0.0f);
+            float t = M * qp;
+            if (opposite) t = t - pen;
+            score += (double)rintf(t);
+            /* how far the device's t can be: dq <= 2 e / mx (q <= 1), d(q^p) <= p q^(p-1) dq, plus fp32 roundings */
+            const double e = o.e + U32 * fabs(o.v);
+            const double dq = 2.0 * e / (double)mx;
+            double dt = (double)M * (double)power * pow((double)q, (double)(power - 1)) * dq + 8.0 * U32 * (double)M;
+            if (fabs(o.v) <= e && yy != 0.0f) dt += (double)pen;          /* the sign of the output is not certain */
+            const double fr = (double)t - floor((double)t);
+            const double dist = fabs(fr - 0.5);                            /* distance to the rounding boundary */
+            if (o.e > 0.0 && dist <= dt) E += dt + 1.0;
+        }
+        const double fit = score - (double)tax * (double)L;
+        fitness_out[p] = (float)fit;
+        if (bound_out) bound_out[p] = E + 4.0 * U32 * fabs(fit);
+        if (flags_out) flags_out[p] = flags;
+        if (depth_out) depth_out[p] = depth;
+    }
+    return 0;
+}
+
 /* The two contracts the tests use most, so that Python does not have to retype 13 doubles.
  * which = 0: IEEE (every op correctly rounded: c = 1, a little slack for libm, no abs terms);
  * which = 1: the CUDA path's published contract, DESIGN.md §6 (numbers retyped from there).   */

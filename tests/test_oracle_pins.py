@@ -788,3 +788,50 @@ def test_P20_ranking_brute_force_against_sorting():
             srt = np.sort(g[sample])
             worse = np.searchsorted(srt, g, side="left")      # samples strictly below
             assert np.array_equal(dec, np.minimum(9, worse // 10)) and np.array_equal(hist, np.bincount(dec, minlength=10))
+
+
+# ---- P21: the Std integer-reward family (Eq. 5 at P:503-506; oracle orc_eval_std) ----------------------
+def evs(oracle, texts, X, y, power=1, M=M_SCORE, tax=0.0):
+    consts = []
+    progs = [asm(t, consts)[0] for t in texts]
+    g, l, c = pack(progs, consts if consts else np.zeros(1, np.float32))
+    return oracle.evaluate_std(g, l, c, X, y, power, M, tax)
+
+
+def test_P21_std_rewards_by_hand(oracle):
+    # Eq. 5 case by case, M = 10000, model f = x0:
+    #   f = 1, y = 2: 10000 * 1/2 = 5000;  f = -1, y = 2: round(5000 - 909.09..) = 4091;  f = y = 0: M;
+    #   f = 3, y = 3: M;  f = 0, y = 5: 0;  f = -4, y = -1: 2500;  f = 2, y = -2: round(10000 - 909.09) = 9091;
+    #   f = 1, y = 3: round(3333.33) = 3333;  f = 2, y = 3: round(6666.67) = 6667
+    f = np.array([1, -1, 0, 3, 0, -4, 2, 1, 2], np.float32)
+    y = np.array([2, 2, 0, 3, 5, -1, -2, 3, 3], np.float32)
+    want = [5000, 4091, 10000, 10000, 0, 2500, 9091, 3333, 6667]
+    for k in range(len(f)):
+        r = evs(oracle, ["x0"], f[k:k + 1].reshape(1, 1), y[k:k + 1])
+        assert r["fitness"][0] == want[k], (k, r["fitness"][0])
+    r = evs(oracle, ["x0"], f.reshape(-1, 1), y)
+    assert r["fitness"][0] == sum(want)                        # the score is the sum over the cases
+    # Square, Cube, Hyper: the ratio to the power 2, 3, 8 (f = 1, y = 2: 2500, 1250, 39.0625 -> 39; opposite signs keep the penalty)
+    for power, w in ((2, 2500), (3, 1250), (8, 39)):
+        assert evs(oracle, ["x0"], np.array([[1.0]], np.float32), np.array([2.0], np.float32), power)["fitness"][0] == w
+    assert evs(oracle, ["x0"], np.array([[-1.0]], np.float32), np.array([2.0], np.float32), 2)["fitness"][0] == 2500 - 909
+    # round half to even: M = 1, q = 1/2 -> 0.5 -> 0;  M = 3, q = 1/2 -> 1.5 -> 2;  M = 5 -> 2.5 -> 2
+    for M, w in ((1.0, 0), (3.0, 2), (5.0, 2), (7.0, 4)):
+        assert evs(oracle, ["x0"], np.array([[1.0]], np.float32), np.array([2.0], np.float32), 1, M)["fitness"][0] == w
+    # invalid pairs as in Eq. 2: one side finite -1 M each, neither +1 M; the tax per command comes off the score
+    X = np.array([[1.0], [1e30], [1.0], [1e30]], np.float32)
+    yy = np.array([1.0, 1.0, np.nan, np.inf], np.float32)
+    r = evs(oracle, ["x0 x0 MUL"], X, yy, 1, M_SCORE, tax=3.0)           # f = 1, inf, 1, inf
+    assert r["fitness"][0] == 10000 - 10000 - 10000 + 10000 - 3.0 * 3
+    # symmetric in (f, y); a perfect model scores M N
+    rng = np.random.default_rng(21)
+    a = rng.uniform(-3, 3, 200).astype(np.float32); b = rng.uniform(-3, 3, 200).astype(np.float32)
+    r1 = evs(oracle, ["x0"], a.reshape(-1, 1), b); r2 = evs(oracle, ["x0"], b.reshape(-1, 1), a)
+    assert r1["fitness"][0] == r2["fitness"][0]
+    assert evs(oracle, ["x0"], a.reshape(-1, 1), a)["fitness"][0] == M_SCORE * 200
+    # numpy restatement on random data (float32 arithmetic, np.rint = half to even)
+    q = np.minimum(np.abs(a), np.abs(b)) / np.maximum(np.abs(a), np.abs(b))
+    for power in (1, 2, 3, 8):
+        qp = {1: q, 2: q * q, 3: (q * q) * q, 8: ((q * q) * (q * q)) * ((q * q) * (q * q))}[power]
+        t = np.float32(M_SCORE) * qp - np.where(a * b < 0, np.float32(M_SCORE) / np.float32(11), np.float32(0))
+        assert evs(oracle, ["x0"], a.reshape(-1, 1), b, power)["fitness"][0] == np.rint(t.astype(np.float32)).sum()
