@@ -254,9 +254,9 @@ def run_ours(args):
 
     # --fit correlation: the paper's own objective (Eq. 1-2) on the same colony; M as the paper's
     # logs imply it, the tax at the paper's default rate M N / 85 per command
-    fit_kind = api.FIT_CORRELATION if args.fit == "correlation" else api.FIT_MSE
+    fit_kind = {"mse": api.FIT_MSE, "correlation": api.FIT_CORRELATION, "std": api.FIT_STD, "std_hyper": api.FIT_STD_HYPER}[args.fit]
     fit_M = 10000.0
-    tax = fit_M * N / 85.0 if fit_kind == api.FIT_CORRELATION else cfg.tax
+    tax = fit_M * N / 85.0 if fit_kind != api.FIT_MSE else cfg.tax
 
     def step_resident():
         if fit_kind == api.FIT_MSE:
@@ -380,7 +380,7 @@ def main():
     ap.add_argument("--config", type=int, default=3, choices=[1, 2, 3, 4, 5])
     ap.add_argument("--population", type=int, default=None, help="first P individuals only (debugging; not a bench value)")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--fit", default="mse", choices=["mse", "correlation"],
+    ap.add_argument("--fit", default="mse", choices=["mse", "correlation", "std", "std_hyper"],
                     help="fitness function; mse is BASELINE.json's metric, correlation the paper's default objective (f2)")
     ap.add_argument("--e2e-steps", type=int, default=5)
     ap.add_argument("--e2e-budget", type=int, default=64 << 20, help="device genome budget of the end-to-end leg, bytes")

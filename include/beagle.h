@@ -133,11 +133,21 @@ beagle_status beagle_eval(const int32_t* genomes, const int32_t* lengths, int64_
  *                           r = 0 when fewer than two valid pairs are left or either side has zero variance
  *                           there (R23). y may hold NaN / Inf. A well-formed program always gets a
  *                           finite-or-NaN float; malformed programs get the canonical quiet NaN as in beagle_eval.
+ *   BEAGLE_FIT_STD, _SQUARE, _CUBE, _HYPER   the point-to-point integer-reward family (Eq. 5 at
+ *                           P:503-506), p = 1, 2, 3, 8: per valid pair  M  if max(|f|,|y|) = 0, else
+ *                           round(M q^p - [f, y of opposite sign] M/11), q = min(|f|,|y|) / max(|f|,|y|), computed in
+ *                           fp32, round half to even; a pair with one side finite scores -M, with neither +M;
+ *                           fitness = sum over the cases - tax * L, MAXIMISED (D9, R25). Exact (integers) while
+ *                           M * N < 2^24.
  *   M                       the maximum score per case (BConfig.MaxScore; the paper's logs imply 10000)
  *
  * All other arguments, limits and errors as beagle_eval; an unknown `fit` returns BEAGLE_ERR_INVALID_ARG.       */
 #define BEAGLE_FIT_MSE         0
 #define BEAGLE_FIT_CORRELATION 1
+#define BEAGLE_FIT_STD         2   /* StdFitFunc        (Eq. 5)                       */
+#define BEAGLE_FIT_STD_SQUARE  3   /* StdSquareFitFunc: the ratio of Eq. 5 squared    */
+#define BEAGLE_FIT_STD_CUBE    4   /* StdCubeFitFunc:   ... cubed                     */
+#define BEAGLE_FIT_STD_HYPER   5   /* StdHyperFitFunc:  ... to the power 8            */
 beagle_status beagle_eval_fit(const int32_t* genomes, const int32_t* lengths, int64_t P,
                               const float* consts, int64_t n_consts,
                               const float* X, const float* y, int32_t N, int32_t d,

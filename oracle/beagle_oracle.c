@@ -453,11 +453,12 @@ int orc_eval_corr(const int32_t* genomes, const int32_t* lengths, int64_t P,
  * The reward is an integer decided by floating point, so it is taken in the paper's precision, fp32, on both sides:
  * the arithmetic below is fp32, in the order |.|, min/max, one division, the power by squarings, * M, - M/11, rintf.
  * The bound: a case can differ from the device's by |dt| + 1 when its unrounded value t is within dt of a rounding
- * boundary, where dt follows from the output bound e; otherwise by nothing.                                       */
+ * boundary, where dt follows from the output bound e; otherwise by nothing.
+ * mode as in orc_eval: 0 = outputs in fp64, 1 = mirror (every command's result rounded to fp32).                   */
 int orc_eval_std(const int32_t* genomes, const int32_t* lengths, int64_t P,
                  const float* consts, int64_t n_consts,
                  const float* X, const float* y, int32_t N, int32_t d, int32_t power, float M, float tax,
-                 const orc_contract* c,
+                 const orc_contract* c, int mode,
                  float* fitness_out, double* bound_out, int32_t* flags_out, int32_t* depth_out) {
     if (P < 0 || N < 1 || N > ORC_MAX_N || d < 1 || !c) return -1;
     if (power != 1 && power != 2 && power != 3 && power != 8) return -1;
@@ -480,7 +481,7 @@ int orc_eval_std(const int32_t* genomes, const int32_t* lengths, int64_t P,
         }
         double score = 0.0, E = 0.0;
         for (int i = 0; i < N; ++i) {
-            pair o = run_case(tok, L, consts, X + (size_t)i * d, c, 0, &flags);
+            pair o = run_case(tok, L, consts, X + (size_t)i * d, c, mode == 1, &flags);
             const int vf = isfinite(o.v), vy = isfinite((double)y[i]);
             if (!(vf && vy)) { score += (vf != vy) ? -(double)M : (double)M; continue; }
             const float f = (float)o.v, yy = y[i];

@@ -63,7 +63,7 @@ def lib():
         _lib.orc_eval_std.restype = ctypes.c_int
         _lib.orc_eval_std.argtypes = [ctypes.c_void_p, ctypes.c_void_p, ctypes.c_int64, ctypes.c_void_p, ctypes.c_int64,
                                       ctypes.c_void_p, ctypes.c_void_p, ctypes.c_int32, ctypes.c_int32, ctypes.c_int32,
-                                      ctypes.c_float, ctypes.c_float, ctypes.POINTER(Contract),
+                                      ctypes.c_float, ctypes.c_float, ctypes.POINTER(Contract), ctypes.c_int,
                                       ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p]
         _lib.orc_default_contract.argtypes = [ctypes.c_int, ctypes.POINTER(Contract)]
     return _lib
@@ -127,7 +127,7 @@ def evaluate_corr(genomes, lengths, consts, X, y, M, tax, *, contract_=None):
     return dict(fitness=fit, bound=bound, flags=flags, depth=depth, stats=stats)
 
 
-def evaluate_std(genomes, lengths, consts, X, y, power, M, tax, *, contract_=None):
+def evaluate_std(genomes, lengths, consts, X, y, power, M, tax, *, contract_=None, mode=0):
     """The Std integer-reward family (Eq. 5; power 1, 2, 3, 8): dict(fitness, bound, flags, depth)."""
     genomes = np.ascontiguousarray(genomes, dtype=np.int32)
     lengths = np.ascontiguousarray(lengths, dtype=np.int32)
@@ -143,7 +143,7 @@ def evaluate_std(genomes, lengths, consts, X, y, power, M, tax, *, contract_=Non
     flags = np.empty(P, np.int32)
     depth = np.empty(P, np.int32)
     rc = lib().orc_eval_std(_ptr(genomes), _ptr(lengths), P, _ptr(consts), int(consts.shape[0]),
-                            _ptr(X), _ptr(y), N, d, int(power), float(M), float(tax), ctypes.byref(c),
+                            _ptr(X), _ptr(y), N, d, int(power), float(M), float(tax), ctypes.byref(c), int(mode),
                             _ptr(fit), _ptr(bound), _ptr(flags), _ptr(depth))
     if rc != 0:
         raise ValueError("orc_eval_std: bad arguments")

@@ -93,7 +93,7 @@ def beagle_eval(genomes, lengths, P, consts, n_consts, X, y, N, d, tax, fitness_
                              int(stream) or None), "beagle_eval")
 
 
-FIT_MSE, FIT_CORRELATION = 0, 1
+FIT_MSE, FIT_CORRELATION, FIT_STD, FIT_STD_SQUARE, FIT_STD_CUBE, FIT_STD_HYPER = 0, 1, 2, 3, 4, 5
 
 
 def beagle_eval_fit(genomes, lengths, P, consts, n_consts, X, y, N, d, fit, M, tax, fitness_out, stream=0):

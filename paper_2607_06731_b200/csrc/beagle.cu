@@ -19,6 +19,7 @@
 #include "uop.cuh"
 #include "interp.cuh"
 #include "fit_corr.cuh"
+#include "fit_std.cuh"
 #include "rank.cuh"
 
 namespace beagle {
@@ -61,7 +62,7 @@ struct Header {                                // device-resident results of the
 struct EvalParams {
     const int4* meta; const uint2* uops; const Header* hdr; unsigned int* queue;
     const float* xt; const float* ung; float* fitness; float* outputs;
-    float tax; float M; int n; int npad; int d; int ring_bytes;   // M: the maximum score of the correlation fitness (f2)
+    float tax; float M; int power; int n; int npad; int d; int ring_bytes;   // M: the maximum score of the correlation fitness (f2)
     int rcp_col0;       // first tensor-memory column of the reciprocal rows: passes * d * 16
     int k_rcp;          // variables 0 .. k_rcp-1 have a reciprocal row (per pass)
     int k_un;           // variables 0 .. k_un-1 have their five unary rows staged in shared memory
@@ -520,7 +521,7 @@ __global__ void __launch_bounds__(1024) k_eval_blockwise(
     const int32_t* __restrict__ genomes, const long long* __restrict__ off, const int32_t* __restrict__ lengths,
     const int* __restrict__ depth, const float* __restrict__ consts, const float* __restrict__ X,
     const float* __restrict__ y, int n, int d, float tax, float* __restrict__ fitness, float* __restrict__ outputs,
-    const int* __restrict__ list, const int* __restrict__ count, long long P, int fit, float M)
+    const int* __restrict__ list, const int* __restrict__ count, long long P, int fit, float M, int power)
 {
     __shared__ float res[BEAGLE_MAX_N];
     bool y_finite = true;
@@ -569,7 +570,9 @@ __global__ void __launch_bounds__(1024) k_eval_blockwise(
                 }
             }
             if (outputs) outputs[(size_t)p * n + i] = st[sp - 1];
-            res[i] = fit == BEAGLE_FIT_CORRELATION ? st[sp - 1] : (y ? __fsub_rn(st[sp - 1], __ldg(y + i)) : 0.f);
+            res[i] = fit == BEAGLE_FIT_CORRELATION ? st[sp - 1]
+                   : fit == BEAGLE_FIT_STD ? std_reward(st[sp - 1], __ldg(y + i), M, __fdiv_rn(M, 11.f), power)
+                   : (y ? __fsub_rn(st[sp - 1], __ldg(y + i)) : 0.f);
         }
         __syncthreads();
         if (threadIdx.x < 32 && fitness && fit == BEAGLE_FIT_CORRELATION) {       // f2: fit_corr.cuh, the layout of k_eval
@@ -593,11 +596,11 @@ __global__ void __launch_bounds__(1024) k_eval_blockwise(
 #pragma unroll
                 for (int e = 0; e < 4; ++e) {
                     const int ci = m * 128 + lane * 4 + e;
-                    if (ci < n) { const float r = res[ci]; acc = __fmaf_rn(r, r, acc); }
+                    if (ci < n) { const float r = res[ci]; acc = fit == BEAGLE_FIT_STD ? __fadd_rn(acc, r) : __fmaf_rn(r, r, acc); }
                 }
 #pragma unroll
             for (int m = 16; m >= 1; m >>= 1) acc = __fadd_rn(acc, __shfl_xor_sync(0xffffffffu, acc, m));
-            if (lane == 0) fitness[p] = __fmaf_rn(tax, (float)len, __fdiv_rn(acc, (float)n));
+            if (lane == 0) fitness[p] = fit == BEAGLE_FIT_STD ? __fmaf_rn(-tax, (float)len, acc) : __fmaf_rn(tax, (float)len, __fdiv_rn(acc, (float)n));
         }
         __syncthreads();
     }
@@ -626,8 +629,8 @@ static Workspace g_ws;
 static int32_t g_last_cuda = 0;
 static int32_t g_launches = 0;
 static int32_t g_profiling = 0;
-struct FitSel { int kind; float M; };
-static FitSel g_fit = { BEAGLE_FIT_MSE, 0.f };   // set by the entry point for the duration of its call
+struct FitSel { int kind; float M; int power; };
+static FitSel g_fit = { BEAGLE_FIT_MSE, 0.f, 1 };   // set by the entry point for the duration of its call
 
 #define CU(call) do { cudaError_t e_ = (call); if (e_ != cudaSuccess) { g_last_cuda = (int32_t)e_; \
     return (e_ == cudaErrorMemoryAllocation) ? BEAGLE_ERR_NOMEM : BEAGLE_ERR_CUDA; } } while (0)
@@ -645,6 +648,7 @@ static beagle_status init_once()
     if (!w.device_ok) return BEAGLE_ERR_UNSUPPORTED;
     CU(cudaFuncSetAttribute(k_eval<BEAGLE_FIT_MSE>, cudaFuncAttributeMaxDynamicSharedMemorySize, w.smem_optin));
     CU(cudaFuncSetAttribute(k_eval<BEAGLE_FIT_CORRELATION>, cudaFuncAttributeMaxDynamicSharedMemorySize, w.smem_optin));
+    CU(cudaFuncSetAttribute(k_eval<BEAGLE_FIT_STD>, cudaFuncAttributeMaxDynamicSharedMemorySize, w.smem_optin));
     { uint32_t lut[kLutSize]; make_compile_lut(lut); CU(cudaMemcpyToSymbol(g_compile_lut, lut, sizeof(lut))); }
     CU(cudaMalloc(&w.bins, sizeof(int) * kNumBins));
     CU(cudaMalloc(&w.cursor, sizeof(int) * kNumBins));
@@ -817,7 +821,7 @@ static beagle_status run_eval(const int32_t* genomes, const int32_t* lengths, co
     if (!tp.fast) return BEAGLE_ERR_UNSUPPORTED;   // callers check first
     prm.rcp_col0 = tp.rcp_col0; prm.k_rcp = tp.k_rcp; prm.slot_col0 = tp.slot_col0; prm.tmem_slots = tp.tmem_slots;
     prm.meta = w.meta; prm.uops = w.uops; prm.hdr = w.hdr; prm.xt = w.xt; prm.ung = w.ung;
-    prm.fitness = fitness; prm.outputs = outputs; prm.tax = tax; prm.M = g_fit.M; prm.n = N; prm.npad = npad; prm.d = d;
+    prm.fitness = fitness; prm.outputs = outputs; prm.tax = tax; prm.M = g_fit.M; prm.power = g_fit.power; prm.n = N; prm.npad = npad; prm.d = d;
     const bool prof = g_profiling && w.prof_n < kProfMax;
     if (prof) {
         for (int i = 0; i < 2; ++i)
@@ -830,12 +834,13 @@ static beagle_status run_eval(const int32_t* genomes, const int32_t* lengths, co
     if (prm.ring_bytes < kStageBytesMax) return BEAGLE_ERR_UNSUPPORTED;
     prm.queue = &w.hdr->queue;
     if (g_fit.kind == BEAGLE_FIT_CORRELATION) k_eval<BEAGLE_FIT_CORRELATION><<<w.num_sms, tp.threads, smem, st>>>(prm);
+    else if (g_fit.kind == BEAGLE_FIT_STD) k_eval<BEAGLE_FIT_STD><<<w.num_sms, tp.threads, smem, st>>>(prm);
     else k_eval<BEAGLE_FIT_MSE><<<w.num_sms, tp.threads, smem, st>>>(prm);
     ++g_launches;
     if (prof) { CU(cudaEventRecord(w.ev_k[2 * w.prof_n + 1], st)); ++w.prof_n; }
     // slow path: individuals whose micro-ops did not fit the promised workspace (normally none)
     k_eval_blockwise<<<w.num_sms * 2, (N + 31) / 32 * 32, 0, st>>>(genomes, w.off, lengths, w.depth, consts, X, y, N, d, tax,
-                                                                   fitness, outputs, w.slow_list, &w.hdr->n_slow, P, g_fit.kind, g_fit.M);
+                                                                   fitness, outputs, w.slow_list, &w.hdr->n_slow, P, g_fit.kind, g_fit.M, g_fit.power);
     ++g_launches;
     CU(cudaGetLastError());
     return BEAGLE_OK;
@@ -854,7 +859,7 @@ static beagle_status run_colony(const int32_t* genomes, const int32_t* lengths, 
     if (s != BEAGLE_OK) return s;
     if (fast) return run_eval(genomes, lengths, consts, X, y, P, N, d, tax, fitness, outputs, st);
     k_eval_blockwise<<<(unsigned)P, (N + 31) / 32 * 32, 0, st>>>(genomes, w.off, lengths, w.depth, consts, X, y, N, d, tax,
-                                                                fitness, outputs, nullptr, nullptr, P, g_fit.kind, g_fit.M);
+                                                                fitness, outputs, nullptr, nullptr, P, g_fit.kind, g_fit.M, g_fit.power);
     ++g_launches;
     CU(cudaGetLastError());
     return BEAGLE_OK;
@@ -863,6 +868,20 @@ static beagle_status run_colony(const int32_t* genomes, const int32_t* lengths, 
 } // namespace beagle
 
 using namespace beagle;
+
+// BEAGLE_FIT_* of include/beagle.h -> kernel variant and power of the Std family
+static bool decode_fit(int32_t fit, int* kind, int* power)
+{
+    *power = 1;
+    switch (fit) {
+    case BEAGLE_FIT_MSE: case BEAGLE_FIT_CORRELATION: *kind = fit; return true;
+    case BEAGLE_FIT_STD: *kind = BEAGLE_FIT_STD; *power = 1; return true;
+    case BEAGLE_FIT_STD_SQUARE: *kind = BEAGLE_FIT_STD; *power = 2; return true;
+    case BEAGLE_FIT_STD_CUBE: *kind = BEAGLE_FIT_STD; *power = 3; return true;
+    case BEAGLE_FIT_STD_HYPER: *kind = BEAGLE_FIT_STD; *power = 8; return true;
+    default: return false;
+    }
+}
 
 extern "C" {
 
@@ -884,8 +903,9 @@ beagle_status beagle_eval_fit(const int32_t* genomes, const int32_t* lengths, in
                               const float* consts, int64_t n_consts, const float* X, const float* y,
                               int32_t N, int32_t d, int32_t fit, float M, float tax, float* fitness_out, void* stream)
 {
-    if (fit != BEAGLE_FIT_MSE && fit != BEAGLE_FIT_CORRELATION) return BEAGLE_ERR_INVALID_ARG;
-    g_fit.kind = fit; g_fit.M = M;
+    int kind, power;
+    if (!decode_fit(fit, &kind, &power)) return BEAGLE_ERR_INVALID_ARG;
+    g_fit.kind = kind; g_fit.M = M; g_fit.power = power;
     const beagle_status s = beagle_eval(genomes, lengths, P, consts, n_consts, X, y, N, d, tax, fitness_out, stream);
     g_fit.kind = BEAGLE_FIT_MSE; g_fit.M = 0.f;
     return s;
@@ -945,7 +965,7 @@ beagle_status beagle_eval_blockwise(const int32_t* genomes, const int32_t* lengt
     if ((s = run_prepass(genomes, lengths, P, consts, n_consts, X, y, N, d, fitness_out, nullptr, -1, false, st)) != BEAGLE_OK) return s;
     const int threads = (N + 31) / 32 * 32;
     k_eval_blockwise<<<(unsigned)P, threads, 0, st>>>(genomes, w.off, lengths, w.depth, consts, X, y, N, d, tax,
-                                                      fitness_out, nullptr, nullptr, nullptr, P, g_fit.kind, g_fit.M);
+                                                      fitness_out, nullptr, nullptr, nullptr, P, g_fit.kind, g_fit.M, g_fit.power);
     ++g_launches;
     CU(cudaGetLastError());
     return BEAGLE_OK;
@@ -995,8 +1015,9 @@ beagle_status beagle_eval_chunked_fit(const int32_t* h_genomes, const int32_t* h
                                       int32_t N, int32_t d, int32_t fit, float M, float tax, float* fitness_out,
                                       int64_t device_budget_bytes, void* stream)
 {
-    if (fit != BEAGLE_FIT_MSE && fit != BEAGLE_FIT_CORRELATION) return BEAGLE_ERR_INVALID_ARG;
-    g_fit.kind = fit; g_fit.M = M;
+    int kind, power;
+    if (!decode_fit(fit, &kind, &power)) return BEAGLE_ERR_INVALID_ARG;
+    g_fit.kind = kind; g_fit.M = M; g_fit.power = power;
     const beagle_status s = beagle_eval_chunked(h_genomes, h_lengths, P, h_consts, n_consts, X, y, N, d, tax, fitness_out,
                                                 device_budget_bytes, stream);
     g_fit.kind = BEAGLE_FIT_MSE; g_fit.M = 0.f;
