@@ -340,6 +340,23 @@ struct CompileParams {
 // from L1), and the walk itself is table-driven, the same straight-line code for every lane.
 constexpr int kCompBatch = 8;
 
+// The rest of Table 3 as the compiler sees it (rare, kept out of line so that it costs the straight-line walk no
+// registers): stack effect and well-formedness of DUP SWAP DEL POW SIGN .. TANH COPY PASTE. Returns 0 in the high word
+// when the token makes the program malformed, else 2 + the change of the stack depth; the low word is the new
+// "variable holds a value" mask (COPY @arg / PASTE @arg come in pairs).
+__device__ __noinline__ unsigned long long compile_rare(uint32_t op, uint32_t arg, int sp, uint32_t vlive)
+{
+    const bool isVar = op == OPC_COPY || op == OPC_PASTE;
+    const bool isK = (op - OPC_DUP) <= (OPC_TANH - OPC_DUP) || isVar;
+    const int kneed = (op == OPC_SWAP || op == OPC_POW) ? 2 : (op == OPC_PASTE ? 0 : 1);
+    const int kpush = (op == OPC_DUP || op == OPC_PASTE) ? 1 : ((op == OPC_DEL || op == OPC_POW) ? -1 : 0);
+    const bool held = arg < (uint32_t)BEAGLE_MAX_VARS && ((vlive >> (arg & 31u)) & 1u);
+    const bool argok = isVar ? (arg < (uint32_t)BEAGLE_MAX_VARS && held == (op == OPC_PASTE)) : arg == 0;
+    if (!(isK && argok && sp >= kneed && sp + kpush <= BEAGLE_MAX_STACK)) return (unsigned long long)vlive;
+    if (isVar) vlive ^= 1u << (arg & 31u);
+    return ((unsigned long long)(uint32_t)(kpush + 2) << 32) | vlive;
+}
+
 __global__ void __launch_bounds__(kCompileThreads, 8) k_compile(const CompileParams q)
 {
     __shared__ uint32_t lut[kLutSize];
@@ -421,16 +438,9 @@ __global__ void __launch_bounds__(kCompileThreads, 8) k_compile(const CompilePar
                 // not one of the eleven hot-path commands (rare, off the straight-line path). DUP SWAP DEL SIGN SQUARE
                 // CUBE CBRT TAN ARCSIN ARCCOS ARCTAN TANH are checked here (stack effect, depth) but not compiled: an individual that uses
                 // one is evaluated by the blockwise kernel (slow list)
-                const bool isVar = op == OPC_COPY || op == OPC_PASTE;          // COPY @arg / PASTE @arg come in pairs
-                const bool isK = (op - OPC_DUP) <= (OPC_TANH - OPC_DUP) || isVar;
-                const int kneed = (op == OPC_SWAP || op == OPC_POW) ? 2 : (op == OPC_PASTE ? 0 : 1);
-                const int kpush = (op == OPC_DUP || op == OPC_PASTE) ? 1 : ((op == OPC_DEL || op == OPC_POW) ? -1 : 0);
-                const bool held = arg < (uint32_t)BEAGLE_MAX_VARS && ((vlive >> (arg & 31u)) & 1u);
-                const bool argok = isVar ? (arg < (uint32_t)BEAGLE_MAX_VARS && held == (op == OPC_PASTE)) : arg == 0;
-                if (isK && argok && sp >= kneed && sp + kpush <= BEAGLE_MAX_STACK) {
-                    slow = true; sp += kpush; mx = max(mx, sp); bad = false;
-                    if (isVar) vlive ^= 1u << (arg & 31u);
-                }
+                const unsigned long long rr = compile_rare(op, arg, sp, vlive);     // out of line: keeps the walk's registers free
+                const int code = (int)(rr >> 32);                                   // 0: malformed; else 2 + stack effect
+                if (code) { slow = true; sp += code - 2; mx = max(mx, sp); bad = false; vlive = (uint32_t)rr; }
             }
             ok = ok && !bad;
             const bool run = live && good;
