@@ -340,21 +340,39 @@ struct CompileParams {
 // from L1), and the walk itself is table-driven, the same straight-line code for every lane.
 constexpr int kCompBatch = 8;
 
-// The rest of Table 3 as the compiler sees it (rare, kept out of line so that it costs the straight-line walk no
-// registers): stack effect and well-formedness of DUP SWAP DEL POW SIGN .. TANH COPY PASTE. Returns 0 in the high word
-// when the token makes the program malformed, else 2 + the change of the stack depth; the low word is the new
-// "variable holds a value" mask (COPY @arg / PASTE @arg come in pairs).
-__device__ __noinline__ unsigned long long compile_rare(uint32_t op, uint32_t arg, int sp, uint32_t vlive)
+// The rest of Table 3 as the compiler sees it. The walk of k_compile knows the interpreter's eleven commands only
+// and calls anything else malformed, in straight-line code. A lane whose program failed that test walks it once more
+// here with the rules of the whole language (stack effect and depth of DUP SWAP DEL POW SIGN .. TANH, COPY @k /
+// PASTE @k in pairs): a program that passes is well-formed and goes to the blockwise kernel (slow list); the walk
+// costs about ten instructions per token and only the lanes that need it take it.
+// Returns the maximum stack depth, or 0 when the program is malformed.
+__device__ __noinline__ int check_full_language(const uint32_t* __restrict__ tok, int len, int d, long long n_consts)
 {
-    const bool isVar = op == OPC_COPY || op == OPC_PASTE;
-    const bool isK = (op - OPC_DUP) <= (OPC_TANH - OPC_DUP) || isVar;
-    const int kneed = (op == OPC_SWAP || op == OPC_POW) ? 2 : (op == OPC_PASTE ? 0 : 1);
-    const int kpush = (op == OPC_DUP || op == OPC_PASTE) ? 1 : ((op == OPC_DEL || op == OPC_POW) ? -1 : 0);
-    const bool held = arg < (uint32_t)BEAGLE_MAX_VARS && ((vlive >> (arg & 31u)) & 1u);
-    const bool argok = isVar ? (arg < (uint32_t)BEAGLE_MAX_VARS && held == (op == OPC_PASTE)) : arg == 0;
-    if (!(isK && argok && sp >= kneed && sp + kpush <= BEAGLE_MAX_STACK)) return (unsigned long long)vlive;
-    if (isVar) vlive ^= 1u << (arg & 31u);
-    return ((unsigned long long)(uint32_t)(kpush + 2) << 32) | vlive;
+    int sp = 0, mx = 0;
+    uint32_t vlive = 0;                            // COPY / PASTE variables that hold a value
+    for (int t = 0; t < len; ++t) {
+        const uint32_t w = __ldg(tok + t);
+        const uint32_t op = tok_op(w), arg = tok_arg(w);
+        int need, push;
+        bool argok = arg == 0;
+        if (op == OPC_CONST) { need = 0; push = 1; argok = (long long)arg < n_consts; }
+        else if (op == OPC_LOAD) { need = 0; push = 1; argok = (int)arg < d; }
+        else if ((op - OPC_ADD) < 4u || op == OPC_POW) { need = 2; push = -1; }
+        else if ((op - OPC_SIN) < 5u || (op - OPC_SIGN) <= (uint32_t)(OPC_TANH - OPC_SIGN)) { need = 1; push = 0; }
+        else if (op == OPC_DUP) { need = 1; push = 1; }
+        else if (op == OPC_SWAP) { need = 2; push = 0; }
+        else if (op == OPC_DEL) { need = 1; push = -1; }
+        else if (op == OPC_COPY || op == OPC_PASTE) {
+            const bool paste = op == OPC_PASTE;
+            need = paste ? 0 : 1; push = paste ? 1 : 0;
+            argok = arg < (uint32_t)BEAGLE_MAX_VARS && (((vlive >> (arg & 31u)) & 1u) != 0) == paste;
+            vlive ^= 1u << (arg & 31u);
+        }
+        else return 0;
+        if (!argok || sp < need || sp + push > BEAGLE_MAX_STACK) return 0;
+        sp += push; mx = max(mx, sp);
+    }
+    return (sp >= 1 && vlive == 0) ? mx : 0;       // a COPY left without its PASTE is malformed
 }
 
 __global__ void __launch_bounds__(kCompileThreads, 8) k_compile(const CompileParams q)
@@ -387,7 +405,6 @@ __global__ void __launch_bounds__(kCompileThreads, 8) k_compile(const CompilePar
     int sp = 0, mx = 0;
     int c = 0;                                     // computed entries on the stack (the topmost one is acc)
     bool ok = valid, slow = false;
-    uint32_t vlive = 0;                            // COPY / PASTE variables that hold a value
     const int S_T = q.tmem_slots;
     // variables whose division is a multiplication by a staged reciprocal row
     const uint32_t rcp_ok = ~q.hdr->rcp_unsafe & ((q.k_rcp >= 32) ? 0xFFFFFFFFu : ((1u << q.k_rcp) - 1u));
@@ -433,16 +450,7 @@ __global__ void __launch_bounds__(kCompileThreads, 8) k_compile(const CompilePar
             // well-formedness (D3); a CONST token that was not replaced has an index out of range
             const bool good = isT ? ((isc || (op == OPC_LOAD && (int)arg < q.d)) && sp < BEAGLE_MAX_STACK)
                                   : ((isB || isU) && arg == 0 && sp >= (isB ? 2 : 1));
-            bool bad = live && !good;
-            if (bad) {
-                // not one of the eleven hot-path commands (rare, off the straight-line path). DUP SWAP DEL SIGN SQUARE
-                // CUBE CBRT TAN ARCSIN ARCCOS ARCTAN TANH are checked here (stack effect, depth) but not compiled: an individual that uses
-                // one is evaluated by the blockwise kernel (slow list)
-                const unsigned long long rr = compile_rare(op, arg, sp, vlive);     // out of line: keeps the walk's registers free
-                const int code = (int)(rr >> 32);                                   // 0: malformed; else 2 + stack effect
-                if (code) { slow = true; sp += code - 2; mx = max(mx, sp); bad = false; vlive = (uint32_t)rr; }
-            }
-            ok = ok && !bad;
+            ok = ok && (good || t >= tend);
             const bool run = live && good;
             // the record (operand a = second from the top = t1, operand b = top = t0)
             const int s1 = c - 1;
@@ -491,7 +499,11 @@ __global__ void __launch_bounds__(kCompileThreads, 8) k_compile(const CompilePar
     }
     int n = (int)(po - po0);
     if (!valid) return;
-    ok &= (sp >= 1) && (vlive == 0);               // a COPY left without its PASTE is malformed
+    ok &= (sp >= 1);
+    if (!ok) {                                     // not a program of the eleven commands: the whole language? (rare)
+        mx = check_full_language(gtok, len, q.d, q.n_consts);
+        ok = slow = mx > 0;
+    }
     if (!ok) {
         q.depth[p] = 0;
         if (q.fitness) q.fitness[p] = __uint_as_float(0x7FC00000u);
