@@ -36,7 +36,10 @@ enum : uint32_t { OPC_CONST = BEAGLE_OP_CONST, OPC_LOAD = BEAGLE_OP_LOAD, OPC_AD
                   OPC_POW = BEAGLE_OP_POW, OPC_COPY = BEAGLE_OP_COPY, OPC_PASTE = BEAGLE_OP_PASTE };
 
 constexpr int kNumBins = BEAGLE_MAX_LEN + 1;   // bin = 512 - length  (longest first); bin 512 unused
-constexpr int kScanThreads = 256;              // programs per block in the pre-pass
+constexpr int kScanThreads = 256;              // threads per block in the pre-pass
+constexpr int kScanItems = 8;                  // programs per thread: a block owns 2048 consecutive programs, so that the
+                                               // per-(block, bin) global atomics are 8 times fewer
+constexpr int kScanBlock = kScanThreads * kScanItems;
 constexpr int kCompileThreads = 128;
 constexpr int kStagesMax = 8;                  // micro-op stages in flight per warp
 #ifndef BEAGLE_EVAL_THREADS
@@ -102,10 +105,14 @@ __global__ void __launch_bounds__(kScanThreads) k_len_pass1(const int32_t* __res
     __shared__ int hist[kNumBins];
     for (int i = threadIdx.x; i < kNumBins; i += kScanThreads) hist[i] = 0;
     __syncthreads();
-    const long long p = (long long)blockIdx.x * kScanThreads + threadIdx.x;
-    const int len = (p < P) ? clamp_len(lengths[p]) : 0;
-    if (len > 0) atomicAdd(&hist[BEAGLE_MAX_LEN - len], 1);
-    int v = len;
+    int v = 0;
+#pragma unroll
+    for (int it = 0; it < kScanItems; ++it) {
+        const long long p = (long long)blockIdx.x * kScanBlock + it * kScanThreads + threadIdx.x;
+        const int len = (p < P) ? clamp_len(lengths[p]) : 0;
+        if (len > 0) atomicAdd(&hist[BEAGLE_MAX_LEN - len], 1);
+        v += len;
+    }
 #pragma unroll
     for (int m = 16; m >= 1; m >>= 1) v += __shfl_xor_sync(0xffffffffu, v, m);
     if ((threadIdx.x & 31) == 0) wsum[threadIdx.x >> 5] = v;
@@ -229,25 +236,31 @@ __global__ void __launch_bounds__(kScanThreads) k_scatter(
     __shared__ int cnt[kNumBins];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     for (int i = threadIdx.x; i < kNumBins; i += kScanThreads) cnt[i] = 0;
-    const long long p = (long long)blockIdx.x * kScanThreads + threadIdx.x;
-    const int len = (p < P) ? clamp_len(lengths[p]) : 0;
-    int inc = len;
-#pragma unroll
-    for (int s = 1; s < 32; s <<= 1) { int o = __shfl_up_sync(0xffffffffu, inc, s); if (lane >= s) inc += o; }
-    if (lane == 31) wsum[warp] = inc;
     __syncthreads();
-    int wbase = 0;
+    int lens[kScanItems], rs[kScanItems], offs[kScanItems];
+    int carry = 0;                                   // tokens of the block before the current chunk of 256 programs
 #pragma unroll
-    for (int w = 0; w < kScanThreads / 32; ++w) wbase += (w < warp) ? wsum[w] : 0;
-    const int k = len > 0 ? BEAGLE_MAX_LEN - len : -1;
-    int r = 0;
-    if (p < P) {
-        off[p] = bsum[blockIdx.x] + wbase + inc - len;
-        if (k >= 0) r = atomicAdd(&cnt[k], 1);
-        else {                                   // length out of range: malformed (D3)
-            depth_out[p] = 0;
-            if (fitness) fitness[p] = __uint_as_float(0x7FC00000u);
-            if (outputs) for (int i = 0; i < n_cases; ++i) outputs[(size_t)p * n_cases + i] = __uint_as_float(0x7FC00000u);
+    for (int it = 0; it < kScanItems; ++it) {
+        const long long p = (long long)blockIdx.x * kScanBlock + it * kScanThreads + threadIdx.x;
+        const int len = (p < P) ? clamp_len(lengths[p]) : 0;
+        int inc = len;
+#pragma unroll
+        for (int s = 1; s < 32; s <<= 1) { int o = __shfl_up_sync(0xffffffffu, inc, s); if (lane >= s) inc += o; }
+        if (lane == 31) wsum[warp] = inc;
+        __syncthreads();
+        int wbase = 0, tot = 0;
+#pragma unroll
+        for (int w = 0; w < kScanThreads / 32; ++w) { wbase += (w < warp) ? wsum[w] : 0; tot += wsum[w]; }
+        __syncthreads();
+        lens[it] = len; offs[it] = carry + wbase + inc - len; rs[it] = 0;
+        carry += tot;
+        if (p < P) {
+            if (len > 0) rs[it] = atomicAdd(&cnt[BEAGLE_MAX_LEN - len], 1);
+            else {                                   // length out of range: malformed (D3)
+                depth_out[p] = 0;
+                if (fitness) fitness[p] = __uint_as_float(0x7FC00000u);
+                if (outputs) for (int i = 0; i < n_cases; ++i) outputs[(size_t)p * n_cases + i] = __uint_as_float(0x7FC00000u);
+            }
         }
     }
     __syncthreads();
@@ -255,13 +268,22 @@ __global__ void __launch_bounds__(kScanThreads) k_scatter(
     for (int i = threadIdx.x; i < kNumBins; i += kScanThreads)
         if (cnt[i]) cnt[i] = atomicAdd(&cursor[i], cnt[i]);
     __syncthreads();
-    if (k >= 0) {
-        // everything the compiler's lane needs to start, at the individual's place in the sorted order
-        const int pos = binstart[k] + cnt[k] + r;
-        const long long o = bsum[blockIdx.x] + wbase + inc - len;
-        perm[pos] = (int)p;
-        sched[pos] = make_int4((int)p, len, (int)(unsigned int)o, (int)(o >> 32));
-        sched_u[pos] = binubase[k] + (long long)(cnt[k] + r) * uop_stride(len);
+    const long long b0 = bsum[blockIdx.x];
+#pragma unroll
+    for (int it = 0; it < kScanItems; ++it) {
+        const long long p = (long long)blockIdx.x * kScanBlock + it * kScanThreads + threadIdx.x;
+        if (p >= P) continue;
+        const int len = lens[it];
+        const long long o = b0 + offs[it];
+        off[p] = o;
+        if (len > 0) {
+            // everything the compiler's lane needs to start, at the individual's place in the sorted order
+            const int k = BEAGLE_MAX_LEN - len;
+            const int pos = binstart[k] + cnt[k] + rs[it];
+            perm[pos] = (int)p;
+            sched[pos] = make_int4((int)p, len, (int)(unsigned int)o, (int)(o >> 32));
+            sched_u[pos] = binubase[k] + (long long)(cnt[k] + rs[it]) * uop_stride(len);
+        }
     }
 }
 
@@ -695,7 +717,7 @@ static beagle_status reserve_P(long long P)
     cudaFree(w.slow_list); cudaFree(w.bsum);
     w.off = nullptr; w.depth = nullptr; w.perm = nullptr; w.meta = nullptr;
     w.slow_list = nullptr; w.bsum = nullptr; w.cap_P = 0;
-    const long long nb = (P + kScanThreads - 1) / kScanThreads;
+    const long long nb = (P + kScanBlock - 1) / kScanBlock;
     CU(cudaMalloc(&w.off, sizeof(long long) * (P + 1)));
     CU(cudaMalloc(&w.depth, sizeof(int) * P));
     CU(cudaMalloc(&w.perm, sizeof(int) * P));
@@ -798,7 +820,7 @@ static beagle_status run_prepass(const int32_t* genomes, const int32_t* lengths,
                                  float* outputs, long long T_known, bool emit, cudaStream_t st)
 {
     Workspace& w = g_ws;
-    const int nb = (int)((P + kScanThreads - 1) / kScanThreads);
+    const int nb = (int)((P + kScanBlock - 1) / kScanBlock);
     const int npad = (N + kCasePad - 1) / kCasePad * kCasePad;
     k_len_pass1<<<nb, kScanThreads, 0, st>>>(lengths, P, w.bsum, w.bins);
     k_len_pass2<<<1, 1024, 0, st>>>(w.bsum, nb, w.hdr, w.bins, w.cursor, w.binstart, w.binubase, X, y, N, d, npad, w.xt, w.ung);
