@@ -279,7 +279,7 @@ def run_ours(args):
         step()
     torch.cuda.synchronize(); dist_barrier(world)
     clocks = ClockSampler(local_rank) if rank == 0 else None
-    api.beagle_set_profiling(True)
+    api.beagle_set_profiling(4)                 # CUDA events around k_eval on every 4th step of the timed region
     ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     ev0.record(stream)
     launches = 0
@@ -337,7 +337,7 @@ def run_ours(args):
                      "peak": peak / 1e12, "unit": "T lane-instr/s (1 GP op = 1 FP32 lane-instruction)",
                      "frac": None if kernel_rate is None else kernel_rate / peak,
                      "peak_basis": f"148 SMs x 128 FP32 lanes x {sm_max:.0f} MHz (MEASURED_PEAKS.json sm_max_mhz; DESIGN.md §8)",
-                     "kernel_ms": eval_ms if n_prof else None, "kernel_share_of_step": (eval_ms / (ms_local / args.steps)) if n_prof else None,
+                     "kernel_ms": eval_ms if n_prof else None, "kernel_launches_timed": n_prof, "kernel_share_of_step": (eval_ms / (ms_local / args.steps)) if n_prof else None,
                      "hbm_gbs_on_genome_stream": None if kernel_rate is None else (4 * T + 12 * P) / (eval_ms * 1e-3) / 1e9,
                      "traffic": TRAFFIC_BYTES.get(args.config)},
         "result_check": {"finite": int(np.isfinite(fit).sum()), "nan": int(np.isnan(fit).sum()),

@@ -249,9 +249,11 @@ void beagle_release(void);
 /* Number of kernels the most recent beagle_eval* call launched (for bench.py's gpu_launches). */
 int32_t beagle_last_launch_count(void);
 
-/* Profiling hooks for bench.py's roofline line. While profiling is on, every beagle_eval call
- * brackets its evaluation kernels (the interpreter launches, without the scheduling pre-pass) with
- * a pair of CUDA events on `stream` (at most 256 calls are recorded; later ones are not).
+/* Profiling hooks for bench.py's roofline line. While profiling is on (on = n > 0), every n-th beagle_eval
+ * call, starting with the first, brackets its evaluation kernels (the interpreter launches, without the scheduling
+ * pre-pass) with a pair of CUDA events on `stream` (at most 256 calls are recorded; later ones are not). The two
+ * event records cost a call about 12 us of stream bubbles and keep k_eval from starting under the tail of
+ * k_compile, which is why a bench may want n > 1.
  * beagle_profiled_eval_kernel_ms synchronises on the recorded events, stores the number of
  * recorded calls in *n_calls (may be NULL) and returns their mean device time in milliseconds
  * (< 0 if nothing was recorded). beagle_set_profiling(1) clears the record. */

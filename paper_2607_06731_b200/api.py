@@ -173,8 +173,9 @@ def beagle_last_launch_count() -> int:
     return lib().beagle_last_launch_count()
 
 
-def beagle_set_profiling(on: bool):
-    lib().beagle_set_profiling(1 if on else 0)
+def beagle_set_profiling(on):
+    """False / 0: off; True / 1: every call; n > 1: every n-th call."""
+    lib().beagle_set_profiling(int(on))
 
 
 def beagle_profiled_eval_kernel_ms():

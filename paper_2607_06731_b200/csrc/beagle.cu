@@ -400,6 +400,10 @@ __device__ __noinline__ int check_full_language(const uint32_t* __restrict__ tok
 __global__ void __launch_bounds__(kCompileThreads, 8) k_compile(const CompileParams q)
 {
     __shared__ uint32_t lut[kLutSize];
+    // release the dependent launch (k_eval, run_eval): once every block of this grid has started, the interpreter's
+    // CTAs may take the SMs that fall idle and run their prologue; they wait for this grid's completion before
+    // they read its output
+    asm volatile("griddepcontrol.launch_dependents;");
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     if (threadIdx.x < kLutSize) lut[threadIdx.x] = g_compile_lut[threadIdx.x];
     __syncthreads();
@@ -672,7 +676,8 @@ struct Workspace {
 static Workspace g_ws;
 static int32_t g_last_cuda = 0;
 static int32_t g_launches = 0;
-static int32_t g_profiling = 0;
+static int32_t g_profiling = 0;     // 0: off; n > 0: every n-th call is bracketed by events
+static int32_t g_prof_calls = 0;
 struct FitSel { int kind; float M; int power; };
 static FitSel g_fit = { BEAGLE_FIT_MSE, 0.f, 1 };   // set by the entry point for the duration of its call
 
@@ -866,7 +871,7 @@ static beagle_status run_eval(const int32_t* genomes, const int32_t* lengths, co
     prm.rcp_col0 = tp.rcp_col0; prm.k_rcp = tp.k_rcp; prm.slot_col0 = tp.slot_col0; prm.tmem_slots = tp.tmem_slots;
     prm.meta = w.meta; prm.uops = w.uops; prm.hdr = w.hdr; prm.xt = w.xt; prm.ung = w.ung;
     prm.fitness = fitness; prm.outputs = outputs; prm.tax = tax; prm.M = g_fit.M; prm.power = g_fit.power; prm.n = N; prm.npad = npad; prm.d = d;
-    const bool prof = g_profiling && w.prof_n < kProfMax;
+    const bool prof = g_profiling && w.prof_n < kProfMax && (g_prof_calls++ % g_profiling) == 0;
     if (prof) {
         for (int i = 0; i < 2; ++i)
             if (!w.ev_k[2 * w.prof_n + i]) CU(cudaEventCreate(&w.ev_k[2 * w.prof_n + i]));
@@ -877,9 +882,18 @@ static beagle_status run_eval(const int32_t* genomes, const int32_t* lengths, co
     prm.off_ys = tp.off_ys; prm.off_meta = tp.off_meta; prm.off_un = tp.off_un; prm.off_ring = tp.off_ring;
     if (prm.ring_bytes < kStageBytesMax) return BEAGLE_ERR_UNSUPPORTED;
     prm.queue = &w.hdr->queue;
-    if (g_fit.kind == BEAGLE_FIT_CORRELATION) k_eval<BEAGLE_FIT_CORRELATION><<<w.num_sms, tp.threads, smem, st>>>(prm);
-    else if (g_fit.kind == BEAGLE_FIT_STD) k_eval<BEAGLE_FIT_STD><<<w.num_sms, tp.threads, smem, st>>>(prm);
-    else k_eval<BEAGLE_FIT_MSE><<<w.num_sms, tp.threads, smem, st>>>(prm);
+    // programmatic dependent launch: k_eval's prologue (tensor-memory allocation, staging of X, y and the unary rows)
+    // overlaps the tail of k_compile, which releases its dependents at its start; k_eval waits (griddepcontrol.wait)
+    // before it touches the compiler's output
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3(w.num_sms); cfg.blockDim = dim3(tp.threads); cfg.dynamicSmemBytes = smem; cfg.stream = st;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = attr; cfg.numAttrs = 1;
+    if (g_fit.kind == BEAGLE_FIT_CORRELATION) CU(cudaLaunchKernelEx(&cfg, k_eval<BEAGLE_FIT_CORRELATION>, prm));
+    else if (g_fit.kind == BEAGLE_FIT_STD) CU(cudaLaunchKernelEx(&cfg, k_eval<BEAGLE_FIT_STD>, prm));
+    else CU(cudaLaunchKernelEx(&cfg, k_eval<BEAGLE_FIT_MSE>, prm));
     ++g_launches;
     if (prof) { CU(cudaEventRecord(w.ev_k[2 * w.prof_n + 1], st)); ++w.prof_n; }
     // slow path: individuals whose micro-ops did not fit the promised workspace (normally none)
@@ -1176,7 +1190,7 @@ void beagle_release(void)
 
 int32_t beagle_last_launch_count(void) { return g_launches; }
 
-void beagle_set_profiling(int32_t on) { g_profiling = on; if (on) g_ws.prof_n = 0; }
+void beagle_set_profiling(int32_t on) { g_profiling = on < 0 ? 0 : on; g_prof_calls = 0; if (on) g_ws.prof_n = 0; }
 
 float beagle_profiled_eval_kernel_ms(int32_t* n_calls)
 {
