@@ -11,21 +11,24 @@
 
 namespace beagle {
 
+// Straight-line (selects, no branches: the cases of a lane take the same path); the arithmetic and its order are the
+// oracle's. yv: the target is finite (it does not change with the individual).
 __device__ __forceinline__ float std_reward(float f, float y, float M, float pen, int power)
 {
-    const bool vf = fabsf(f) < __int_as_float(0x7f800000), vy = fabsf(y) < __int_as_float(0x7f800000);
-    if (!(vf && vy)) return vf != vy ? -M : M;
     const float a = fabsf(f), b = fabsf(y);
+    const bool vf = a < __int_as_float(0x7f800000), vy = b < __int_as_float(0x7f800000);
     const float mx = fmaxf(a, b), mn = fminf(a, b);
-    if (mx == 0.f) return M;
-    const float q = __fdiv_rn(mn, mx);
+    const float q = __fdiv_rn(mn, mx);                       // 0/0, inf/inf: NaN, replaced below
     float qp = q;
-    if (power == 2) qp = __fmul_rn(q, q);
+    if (power == 2) qp = __fmul_rn(q, q);                    // warp-uniform
     else if (power == 3) qp = __fmul_rn(__fmul_rn(q, q), q);
     else if (power == 8) { qp = __fmul_rn(q, q); qp = __fmul_rn(qp, qp); qp = __fmul_rn(qp, qp); }
-    float t = __fmul_rn(M, qp);
-    if ((f < 0.f && y > 0.f) || (f > 0.f && y < 0.f)) t = __fsub_rn(t, pen);
-    return rintf(t);
+    const float t = __fmul_rn(M, qp);
+    // opposite signs: both non-zero and the sign bits differ (decided on the signs, not on a product that may underflow)
+    const bool opp = mn > 0.f && ((__float_as_int(f) ^ __float_as_int(y)) < 0);
+    float r = rintf(opp ? __fsub_rn(t, pen) : t);
+    r = mx == 0.f ? M : r;
+    return (vf && vy) ? r : (vf != vy ? -M : M);
 }
 
 } // namespace beagle
