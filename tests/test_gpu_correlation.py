@@ -154,3 +154,27 @@ def test_correlation_config_colony_sampled(oracle):
     rep = parity.compare(a, orc)
     assert len(rep["bad"]) == 0, parity.describe(rep, a, orc)
     assert rep["strict"] > 900 and rep["exempt"] < 1500, parity.describe(rep, a, orc)
+
+
+@pytest.mark.parametrize("fit,M_", [(FIT_CORR, M), (2, M), (5, M)])
+def test_chunked_fit_bit_identical_to_resident(oracle, fit, M_):
+    """beagle_eval_chunked_fit (host genomes, small device budget: several chunks) against beagle_eval_fit, bit for bit,
+    for the correlation fitness and two of the Std family."""
+    import torch
+    from paper_2607_06731_b200 import api
+    from tests.gpu_util import gpu_eval_fit
+    col = C.make_colony(2, P=30000)
+    g, l, c, X, y = col.genomes, col.lengths, col.consts, col.X, col.y
+    a = gpu_eval_fit(g, l, c, X, y, fit, M_, 25.0)
+    P, (N, d) = len(l), X.shape
+    hg = torch.from_numpy(np.ascontiguousarray(g, np.int32)).pin_memory()
+    hl = torch.from_numpy(np.ascontiguousarray(l, np.int32)).pin_memory()
+    hc = torch.from_numpy(np.ascontiguousarray(c, np.float32)).pin_memory()
+    Xd, yd = torch.from_numpy(X).cuda(), torch.from_numpy(y).cuda()
+    out = torch.full((P,), -1.0, dtype=torch.float32, device="cuda")
+    budget = 1 << 20                                           # about 1 MiB of staging: several chunks
+    api.beagle_eval_chunked_fit(hg, hl, P, hc, len(c), Xd, yd, N, d, fit, M_, 25.0, out, budget, torch.cuda.current_stream().cuda_stream)
+    torch.cuda.synchronize()
+    assert np.array_equal(_bits(a), _bits(out.cpu().numpy()))
+    assert api.raw_status("beagle_eval_chunked_fit", api._ptr(hg), api._ptr(hl), P, api._ptr(hc), len(c), api._ptr(Xd), api._ptr(yd),
+                          N, d, 9, M_, 25.0, api._ptr(out), budget, None) != 0
