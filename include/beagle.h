@@ -8,7 +8,7 @@
  * PAPER.md:184 (§3.2): a program is a flat list of commands run on an operand stack (RPN);
  * the stack holds 32 entries; PAPER.md:200-294 (Table 3): command meanings and
  * operand order; "length (i.e., the number of GCL commands)".
- * Where the paper is silent the readings of DESIGN.md §3 (R1..R20) apply.
+ * Where the paper is silent the readings of DESIGN.md §3 (R1..R25) apply.
  *
  * Conventions
  *   - Every entry point is extern "C", takes plain pointers and sizes, never throws, never aborts.
@@ -21,7 +21,8 @@
  *   - Argument errors are returned synchronously and nothing is enqueued.
  *   - Data-dependent problems are reported in band: a malformed individual gets the canonical
  *     quiet NaN 0x7FC00000 as its fitness and never causes an out-of-bounds access.
- *   - Lower fitness is better; a non-finite fitness marks an invalid individual.
+ *   - Lower fitness is better for beagle_eval (MSE); the score-type fitness functions of beagle_eval_fit are
+ *     maximised. A non-finite fitness marks an invalid individual.
  *   - One call at a time per process (the workspace is shared); calls are not re-entrant.
  */
 #ifndef BEAGLE_H_
