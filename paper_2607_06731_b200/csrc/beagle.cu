@@ -228,9 +228,9 @@ __global__ void __launch_bounds__(1024) k_len_pass2(long long* __restrict__ bsum
 __global__ void __launch_bounds__(kScanThreads) k_scatter(
     const int32_t* __restrict__ lengths, long long P, const long long* __restrict__ bsum,
     const int* __restrict__ binstart, int* __restrict__ cursor, long long* __restrict__ off,
-    int* __restrict__ perm, int* __restrict__ depth_out, float* __restrict__ fitness,
+    int* __restrict__ depth_out, float* __restrict__ fitness,
     float* __restrict__ outputs, int n_cases, const long long* __restrict__ binubase,
-    int4* __restrict__ sched, long long* __restrict__ sched_u)
+    int4* __restrict__ sched)
 {
     __shared__ int wsum[kScanThreads / 32];
     __shared__ int cnt[kNumBins];
@@ -280,11 +280,20 @@ __global__ void __launch_bounds__(kScanThreads) k_scatter(
             // everything the compiler's lane needs to start, at the individual's place in the sorted order
             const int k = BEAGLE_MAX_LEN - len;
             const int pos = binstart[k] + cnt[k] + rs[it];
-            perm[pos] = (int)p;
-            sched[pos] = make_int4((int)p, len, (int)(unsigned int)o, (int)(o >> 32));
-            sched_u[pos] = binubase[k] + (long long)(cnt[k] + rs[it]) * uop_stride(len);
+            // one 16-byte start record: x = p, y = token offset (low 32), z = record base (low 32),
+            // w = length (10 bits) | offset bits 39..32 << 10 | record base bits 39..32 << 18
+            const long long ub = binubase[k] + (long long)(cnt[k] + rs[it]) * uop_stride(len);
+            sched[pos] = make_int4((int)p, (int)(unsigned int)o, (int)(unsigned int)ub,
+                                   len | (int)((o >> 32) & 0xff) << 10 | (int)((ub >> 32) & 0xff) << 18);
         }
     }
+}
+
+// debug only (beagle_debug_schedule): the sorted order as an index array; entries past the sorted ones are -1
+__global__ void k_perm_from_sched(const int4* __restrict__ sched, const Header* __restrict__ hdr, long long P, int* __restrict__ perm)
+{
+    const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < P) perm[i] = i < hdr->n_sorted ? sched[i].x : -1;
 }
 
 // ---- the compiler's decision table ------------------------------------------------------------------------
@@ -349,7 +358,7 @@ static void make_compile_lut(uint32_t* lut)
 //   acc always holds the topmost computed entry; the computed entry with c others below it that is not
 //   in acc sits in slot c (tensor memory while c < S_T, local memory beyond).
 struct CompileParams {
-    const uint32_t* genomes; const int4* sched; const long long* sched_u;
+    const uint32_t* genomes; const int4* sched;   // one start record per sorted position (k_scatter)
     const float* consts; long long n_consts; int d; int tmem_slots; int k_rcp; int k_un; int un_row_bytes;
     Header* hdr;
     uint2* uops; long long ucap; int4* meta; int* depth; int* slow_list;
@@ -412,11 +421,12 @@ __global__ void __launch_bounds__(kCompileThreads, 8) k_compile(const CompilePar
     if (i0 >= n_sorted) return;
     const int i = i0 + lane;
     const bool valid = i < n_sorted;
-    const int4 sc = valid ? q.sched[i] : make_int4(0, 0, 0, 0);     // k_scatter: {p, length, token offset}
-    const int p = sc.x, len = sc.y;
-    const long long toff = (long long)(((unsigned long long)(unsigned int)sc.w << 32) | (unsigned int)sc.z);
+    const int4 sc = valid ? q.sched[i] : make_int4(0, 0, 0, 0);     // k_scatter's start record: p, token offset, record base, length
+    const int len = sc.w & 0x3ff;                  // (p and the record base are read again after the walk: three registers
+                                                   // fewer to keep through it)
+    const long long toff = (long long)(((unsigned long long)((unsigned int)sc.w >> 10 & 0xffu) << 32) | (unsigned int)sc.y);
     const int stride = uop_stride(len);
-    const long long ua = valid ? q.sched_u[i] : 0;
+    const long long ua = (long long)(((unsigned long long)((unsigned int)sc.w >> 18 & 0xffu) << 32) | (unsigned int)sc.z);
     const bool fits = ua + stride <= q.ucap;
     const bool wr = valid && q.emit && fits;
     int maxlen = len;
@@ -436,7 +446,6 @@ __global__ void __launch_bounds__(kCompileThreads, 8) k_compile(const CompilePar
     const uint32_t rcp_ok = ~q.hdr->rcp_unsafe & ((q.k_rcp >= 32) ? 0xFFFFFFFFu : ((1u << q.k_rcp) - 1u));
     const uint32_t* gtok = q.genomes + toff;
     uint2* po = q.uops + ua;                       // where the next record goes
-    uint2* const po0 = po;
 
     auto load_batch = [&](int c0, uint32_t (&w)[kCompBatch]) {
 #pragma unroll
@@ -523,8 +532,12 @@ __global__ void __launch_bounds__(kCompileThreads, 8) k_compile(const CompilePar
         for (int u = 0; u < kCompBatch; ++u) { wA[u] = wB[u]; wB[u] = wC[u]; }
         cmA = cmB;
     }
-    int n = (int)(po - po0);
     if (!valid) return;
+    const int4 sce = q.sched[i];
+    const int p = sce.x;
+    const long long ua_e = (long long)(((unsigned long long)((unsigned int)sce.w >> 18 & 0xffu) << 32) | (unsigned int)sce.z);
+    uint2* const po0 = q.uops + ua_e;
+    int n = (int)(po - po0);
     ok &= (sp >= 1);
     if (!ok) {                                     // not a program of the eleven commands: the whole language? (rare)
         mx = check_full_language(gtok, len, q.d, q.n_consts);
@@ -554,7 +567,7 @@ __global__ void __launch_bounds__(kCompileThreads, 8) k_compile(const CompilePar
     out[n] = make_uint2(H_END, 0u);
     out[n + 1] = make_uint2(H_END, 0u);
     out[n + 2] = make_uint2(H_END, 0u);
-    q.meta[i] = make_int4(p, (int)(ua >> 1), (n + 2 + 1) & ~1, len);
+    q.meta[i] = make_int4(p, (int)(ua_e >> 1), (n + 2 + 1) & ~1, len);
 }
 
 // ---- the interpreter kernel -----------------------------------------------------------------------------
@@ -660,7 +673,7 @@ __global__ void __launch_bounds__(1024) k_eval_blockwise(
 struct Workspace {
     long long cap_P = 0, cap_U = 0;            // individuals / micro-op entries the workspace holds
     long long promised_P = 0, promised_T = 0;  // beagle_reserve: calls with P <= promised_P have T <= promised_T
-    long long* off = nullptr; int* depth = nullptr; int* perm = nullptr; int4* meta = nullptr; int4* sched = nullptr; long long* sched_u = nullptr;
+    long long* off = nullptr; int* depth = nullptr; int4* meta = nullptr; int4* sched = nullptr;
     int* slow_list = nullptr; long long* bsum = nullptr;
     uint2* uops = nullptr;
     int* bins = nullptr; int* cursor = nullptr; int* binstart = nullptr; long long* binubase = nullptr;
@@ -718,16 +731,14 @@ static beagle_status reserve_P(long long P)
     Workspace& w = g_ws;
     if (P <= w.cap_P) return BEAGLE_OK;
     CU(cudaDeviceSynchronize());
-    cudaFree(w.off); cudaFree(w.depth); cudaFree(w.perm); cudaFree(w.meta); cudaFree(w.sched); cudaFree(w.sched_u);
+    cudaFree(w.off); cudaFree(w.depth); cudaFree(w.meta); cudaFree(w.sched);
     cudaFree(w.slow_list); cudaFree(w.bsum);
-    w.off = nullptr; w.depth = nullptr; w.perm = nullptr; w.meta = nullptr;
+    w.off = nullptr; w.depth = nullptr; w.meta = nullptr;
     w.slow_list = nullptr; w.bsum = nullptr; w.cap_P = 0;
     const long long nb = (P + kScanBlock - 1) / kScanBlock;
     CU(cudaMalloc(&w.off, sizeof(long long) * (P + 1)));
     CU(cudaMalloc(&w.depth, sizeof(int) * P));
-    CU(cudaMalloc(&w.perm, sizeof(int) * P));
     CU(cudaMalloc(&w.sched, sizeof(int4) * P));
-    CU(cudaMalloc(&w.sched_u, sizeof(long long) * P));
     CU(cudaMalloc(&w.meta, sizeof(int4) * P));
     CU(cudaMalloc(&w.slow_list, sizeof(int) * P));
     CU(cudaMalloc(&w.bsum, sizeof(long long) * (nb + 1)));
@@ -842,12 +853,12 @@ static beagle_status run_prepass(const int32_t* genomes, const int32_t* lengths,
         }
         if (need > w.cap_U) { beagle_status s = reserve_U(need); if (s != BEAGLE_OK) return s; }
     }
-    k_scatter<<<nb, kScanThreads, 0, st>>>(lengths, P, w.bsum, w.binstart, w.cursor, w.off, w.perm, w.depth,
-                                           fitness, outputs, N, w.binubase, w.sched, w.sched_u);
+    k_scatter<<<nb, kScanThreads, 0, st>>>(lengths, P, w.bsum, w.binstart, w.cursor, w.off, w.depth,
+                                           fitness, outputs, N, w.binubase, w.sched);
     ++g_launches;
     {
         CompileParams q;
-        q.genomes = reinterpret_cast<const uint32_t*>(genomes); q.sched = w.sched; q.sched_u = w.sched_u;
+        q.genomes = reinterpret_cast<const uint32_t*>(genomes); q.sched = w.sched;
         const TmemPlan tp = tmem_plan(N, d);
         q.consts = consts; q.n_consts = n_consts; q.d = d; q.tmem_slots = tp.tmem_slots; q.k_rcp = tp.k_rcp; q.k_un = tp.k_un; q.un_row_bytes = npad * 4;
         q.hdr = w.hdr; q.uops = w.uops; q.ucap = w.cap_U; q.meta = w.meta; q.depth = w.depth;
@@ -1035,7 +1046,10 @@ beagle_status beagle_debug_schedule(int64_t P, int64_t* off, int32_t* depth, int
     cudaStream_t st = (cudaStream_t)stream;
     if (off) CU(cudaMemcpyAsync(off, g_ws.off, sizeof(long long) * P, cudaMemcpyDeviceToDevice, st));
     if (depth) CU(cudaMemcpyAsync(depth, g_ws.depth, sizeof(int) * P, cudaMemcpyDeviceToDevice, st));
-    if (perm) CU(cudaMemcpyAsync(perm, g_ws.perm, sizeof(int) * P, cudaMemcpyDeviceToDevice, st));
+    if (perm && P > 0) {                           // the sorted order is the first word of the start records
+        k_perm_from_sched<<<(unsigned)((P + 255) / 256), 256, 0, st>>>(g_ws.sched, g_ws.hdr, P, perm);
+        CU(cudaGetLastError());
+    }
     return BEAGLE_OK;
 }
 
@@ -1179,10 +1193,10 @@ void beagle_release(void)
 {
     Workspace& w = g_ws;
     cudaDeviceSynchronize();
-    cudaFree(w.off); cudaFree(w.depth); cudaFree(w.perm); cudaFree(w.meta); cudaFree(w.sched); cudaFree(w.sched_u);
+    cudaFree(w.off); cudaFree(w.depth); cudaFree(w.meta); cudaFree(w.sched);
     cudaFree(w.slow_list); cudaFree(w.bsum); cudaFree(w.uops);
     cudaFree(w.stage[0]); cudaFree(w.stage[1]); cudaFree(w.stage_consts); cudaFree(w.rank_hist); w.rank_hist = nullptr;
-    w.off = nullptr; w.depth = nullptr; w.perm = nullptr; w.meta = nullptr;
+    w.off = nullptr; w.depth = nullptr; w.meta = nullptr;
     w.slow_list = nullptr; w.bsum = nullptr; w.uops = nullptr; w.cap_P = 0; w.cap_U = 0;
     w.promised_P = 0; w.promised_T = 0;
     w.stage[0] = w.stage[1] = nullptr; w.stage_bytes = 0; w.stage_consts = nullptr; w.stage_consts_cap = 0;
