@@ -455,3 +455,31 @@ def test_copy_paste_variables(oracle):
     assert np.all(_bits(a[:len(bad)]) == QNAN) and a[len(bad)] == np.float32(64.0 ** 2)
     orc = oracle.evaluate(g, l, c, X1, y1, 0.0)
     assert len(parity.compare(a, orc)["bad"]) == 0
+
+
+def test_eval_is_cuda_graph_capturable(oracle):
+    """After beagle_reserve the call allocates nothing and never synchronises, so a generation loop can capture it in a
+    CUDA graph (launch-bound small colonies); a replay gives the bits of a plain call, also after the inputs changed."""
+    import torch
+    from paper_2607_06731_b200 import api, colonies as C
+    col = C.make_colony(1)
+    dev = lambda a: torch.from_numpy(np.ascontiguousarray(a)).cuda()
+    g, l, c, X, y = dev(col.genomes), dev(col.lengths), dev(col.consts), dev(col.X), dev(col.y)
+    P, (N, d) = len(col.lengths), col.X.shape
+    api.beagle_reserve(P, int(col.lengths.sum()))
+    plain = torch.empty(P, dtype=torch.float32, device="cuda")
+    api.beagle_eval(g, l, P, c, len(col.consts), X, y, N, d, col.tax, plain, torch.cuda.current_stream().cuda_stream)
+    torch.cuda.synchronize()
+    out = torch.zeros(P, dtype=torch.float32, device="cuda")
+    graph = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(graph):
+        api.beagle_eval(g, l, P, c, len(col.consts), X, y, N, d, col.tax, out, torch.cuda.current_stream().cuda_stream)
+    for _ in range(3):
+        graph.replay()
+    torch.cuda.synchronize()
+    assert np.array_equal(_bits(out.cpu().numpy()), _bits(plain.cpu().numpy()))
+    y.add_(1.0)                                                # same buffers, new targets: the graph reads them at replay
+    graph.replay()
+    api.beagle_eval(g, l, P, c, len(col.consts), X, y, N, d, col.tax, plain, torch.cuda.current_stream().cuda_stream)
+    torch.cuda.synchronize()
+    assert np.array_equal(_bits(out.cpu().numpy()), _bits(plain.cpu().numpy()))
