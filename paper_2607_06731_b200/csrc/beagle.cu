@@ -1130,6 +1130,15 @@ beagle_status beagle_eval_chunked(const int32_t* h_genomes, const int32_t* h_len
     int total_launches = 0;
     for (int c = 0; p0 < P; ++c) {
         long long words = 0, p1 = p0, ntok = 0;
+        // whole blocks of 4096 lengths first (a branch-free sum the host compiler vectorises: the scan of the first
+        // chunk is on the critical path, nothing is in flight yet), then one by one up to the boundary
+        while (p1 + 4096 <= P) {
+            long long bt = 0;
+            const int32_t* hl = h_lengths + p1;
+            for (int k = 0; k < 4096; ++k) { const int32_t v = hl[k]; bt += (v >= 1 && v <= BEAGLE_MAX_LEN) ? v : 0; }
+            if (words + bt + 4096 > cap_words) break;
+            words += bt + 4096; ntok += bt; p1 += 4096;
+        }
         while (p1 < P) {
             const int l = (h_lengths[p1] >= 1 && h_lengths[p1] <= BEAGLE_MAX_LEN) ? h_lengths[p1] : 0;
             if (words + l + 1 > cap_words) break;
