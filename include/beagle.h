@@ -157,8 +157,9 @@ beagle_status beagle_eval_fit(const int32_t* genomes, const int32_t* lengths, in
 /* beagle_eval_chunked — the same result for a colony held in HOST memory that may be larger than
  * the device budget ("manages populations in batches to ensure the GPU memory is
  * never exceeded"; R19). The colony is cut at individual boundaries into chunks of at
- * most device_budget_bytes/2 bytes of tokens+lengths; chunk c+1 is copied host-to-device on an
- * internal copy stream while chunk c is evaluated on `stream` (two staging buffers).
+ * most device_budget_bytes/K bytes of tokens+lengths, K = device_budget_bytes / 32 MiB clamped to 2..8 staging
+ * buffers; the chunks after chunk c are copied host-to-device on an internal copy stream while chunk c is
+ * evaluated on `stream`.
  * fitness_out is bit-identical to beagle_eval on the whole colony, for any budget.
  *
  *   h_genomes, h_lengths, h_consts   HOST (pinned memory for overlap; pageable memory works but
@@ -241,7 +242,7 @@ int32_t beagle_last_cuda_error(void);
  * calls are allocation-free. Synchronises the device if it has to reallocate. */
 beagle_status beagle_reserve(int64_t P_max, int64_t T_max);
 
-/* Pre-size the two staging buffers of beagle_eval_chunked for this budget. */
+/* Pre-size the staging buffers of beagle_eval_chunked for this budget. */
 beagle_status beagle_reserve_chunked(int64_t device_budget_bytes);
 
 /* Free the cached workspace and staging buffers (synchronises the device). */

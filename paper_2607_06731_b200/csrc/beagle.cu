@@ -46,6 +46,8 @@ constexpr int kStagesMax = 8;                  // micro-op stages in flight per 
 #define BEAGLE_EVAL_THREADS 1024
 #endif
 constexpr int kEvalThreads = BEAGLE_EVAL_THREADS;   // 32 warps (8 per scheduler): 64 registers per thread
+constexpr int kStageBufsMax = 8;               // beagle_eval_chunked: staging buffers the device budget is cut into
+constexpr long long kStageTarget = 32ll << 20;  // ... of about this size each (at least two)
 constexpr int kProfMax = 256;                  // beagle_set_profiling: recorded calls
 constexpr int kEvalMetaBytes = 64 * 16;           // per-warp window of the work queue (64 x int4)
 constexpr int kCasePad = 512;                  // staged cases are padded to a multiple of 32*K
@@ -680,9 +682,9 @@ struct Workspace {
     float* xt = nullptr; float* ung = nullptr; Header* hdr = nullptr; long long* h_T = nullptr;
     unsigned long long* rank_hist = nullptr;   // beagle_rank's histogram when the caller wants none
     // chunked staging
-    long long stage_bytes = 0; unsigned char* stage[2] = { nullptr, nullptr };
+    long long stage_bytes = 0; int stage_n = 0; unsigned char* stage[kStageBufsMax] = {};   // stage[0] owns the allocation
     float* stage_consts = nullptr; long long stage_consts_cap = 0;
-    cudaStream_t copy_stream = nullptr; cudaEvent_t ev_copied[2] = { nullptr, nullptr }, ev_free[2] = { nullptr, nullptr };
+    cudaStream_t copy_stream = nullptr; cudaEvent_t ev_copied[kStageBufsMax] = {}, ev_free[kStageBufsMax] = {};
     cudaEvent_t ev_k[2 * kProfMax] = {}; int prof_n = 0;
     int num_sms = 0; int smem_optin = 0; bool device_ok = false; bool inited = false;
 };
@@ -1058,21 +1060,25 @@ beagle_status beagle_reserve_chunked(int64_t device_budget_bytes)
     Workspace& w = g_ws;
     beagle_status s = init_once();
     if (s != BEAGLE_OK) return s;
-    const long long half = (device_budget_bytes / 2) & ~255ll;
+    // the budget is cut into K staging buffers of about 32 MiB (2 <= K <= 8): a chunk is copied while the ones before it
+    // are evaluated, and the finer the chunks the less of the first copy and of the last evaluation is exposed
+    long long K = device_budget_bytes / kStageTarget;
+    K = K < 2 ? 2 : (K > kStageBufsMax ? kStageBufsMax : K);
+    const long long half = (device_budget_bytes / K) & ~255ll;
     if (half < 4ll * (BEAGLE_MAX_LEN + 1)) return BEAGLE_ERR_INVALID_ARG;
     if (!w.copy_stream) {
         CU(cudaStreamCreateWithFlags(&w.copy_stream, cudaStreamNonBlocking));
-        for (int i = 0; i < 2; ++i) {
+        for (int i = 0; i < kStageBufsMax; ++i) {
             CU(cudaEventCreateWithFlags(&w.ev_copied[i], cudaEventDisableTiming));
             CU(cudaEventCreateWithFlags(&w.ev_free[i], cudaEventDisableTiming));
         }
     }
-    if (half != w.stage_bytes) {
+    if (half != w.stage_bytes || (int)K != w.stage_n) {
         CU(cudaDeviceSynchronize());
-        cudaFree(w.stage[0]); cudaFree(w.stage[1]); w.stage[0] = w.stage[1] = nullptr; w.stage_bytes = 0;
-        CU(cudaMalloc(&w.stage[0], half));
-        CU(cudaMalloc(&w.stage[1], half));
-        w.stage_bytes = half;
+        cudaFree(w.stage[0]); w.stage[0] = nullptr; w.stage_bytes = 0; w.stage_n = 0;
+        CU(cudaMalloc(&w.stage[0], half * K));
+        for (int i = 1; i < (int)K; ++i) w.stage[i] = w.stage[0] + (size_t)i * half;
+        w.stage_bytes = half; w.stage_n = (int)K;
     }
     // workspace of one chunk: at most cap_words individuals and 2 * cap_words micro-op entries
     const long long cap_words = half / 4 - 3;
@@ -1118,7 +1124,7 @@ beagle_status beagle_eval_chunked(const int32_t* h_genomes, const int32_t* h_len
     }
     // the copy stream must not start before work already queued on `stream` (e.g. the producer of X)
     CU(cudaEventRecord(w.ev_free[0], st)); CU(cudaStreamWaitEvent(w.copy_stream, w.ev_free[0], 0));
-    CU(cudaEventRecord(w.ev_free[1], st));
+    for (int i = 1; i < w.stage_n; ++i) CU(cudaEventRecord(w.ev_free[i], st));
     if (n_consts > 0)
         CU(cudaMemcpyAsync(w.stage_consts, h_consts, sizeof(float) * n_consts, cudaMemcpyHostToDevice, w.copy_stream));
     // chunk plan at individual boundaries: lengths first, then (16-byte aligned) tokens, in one staging
@@ -1145,7 +1151,7 @@ beagle_status beagle_eval_chunked(const int32_t* h_genomes, const int32_t* h_len
             words += l + 1; ntok += l; ++p1;
         }
         const long long np = p1 - p0;
-        const int b = c & 1;
+        const int b = c % w.stage_n;
         int32_t* d_len = reinterpret_cast<int32_t*>(w.stage[b]);
         int32_t* d_tok = d_len + ((np + 3) & ~3ll);
         CU(cudaStreamWaitEvent(w.copy_stream, w.ev_free[b], 0));      // buffer b is free again
@@ -1204,11 +1210,11 @@ void beagle_release(void)
     cudaDeviceSynchronize();
     cudaFree(w.off); cudaFree(w.depth); cudaFree(w.meta); cudaFree(w.sched);
     cudaFree(w.slow_list); cudaFree(w.bsum); cudaFree(w.uops);
-    cudaFree(w.stage[0]); cudaFree(w.stage[1]); cudaFree(w.stage_consts); cudaFree(w.rank_hist); w.rank_hist = nullptr;
+    cudaFree(w.stage[0]); cudaFree(w.stage_consts); cudaFree(w.rank_hist); w.rank_hist = nullptr;
     w.off = nullptr; w.depth = nullptr; w.meta = nullptr;
     w.slow_list = nullptr; w.bsum = nullptr; w.uops = nullptr; w.cap_P = 0; w.cap_U = 0;
     w.promised_P = 0; w.promised_T = 0;
-    w.stage[0] = w.stage[1] = nullptr; w.stage_bytes = 0; w.stage_consts = nullptr; w.stage_consts_cap = 0;
+    w.stage[0] = nullptr; w.stage_bytes = 0; w.stage_n = 0; w.stage_consts = nullptr; w.stage_consts_cap = 0;
 }
 
 int32_t beagle_last_launch_count(void) { return g_launches; }
