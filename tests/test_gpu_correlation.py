@@ -178,3 +178,45 @@ def test_chunked_fit_bit_identical_to_resident(oracle, fit, M_):
     assert np.array_equal(_bits(a), _bits(out.cpu().numpy()))
     assert api.raw_status("beagle_eval_chunked_fit", api._ptr(hg), api._ptr(hl), P, api._ptr(hc), len(c), api._ptr(Xd), api._ptr(yd),
                           N, d, 9, M_, 25.0, api._ptr(out), budget, None) != 0
+
+
+@pytest.mark.parametrize("fit,power", [(FIT_CORR, 0), (2, 1)])
+def test_full_size_config3_sampled_then_ranked(oracle, fit, power):
+    """BASELINE.json's config 3 at full size (the launch configuration `bench.py --fit ...` times): every 701st
+    individual and the 128 longest against the oracle; properties that hold at any size; then beagle_rank on the
+    resident fitness vector against oracle/ranking.py's sort-based restatement (pinned by P20)."""
+    import torch
+    from paper_2607_06731_b200 import api
+    from oracle import ranking as R
+    col = C.make_colony(3)
+    P, (N, d) = col.P, col.X.shape
+    tax = M * N / 85.0
+    dev = lambda a: torch.from_numpy(np.ascontiguousarray(a)).cuda()
+    g, l, c, X, y = dev(col.genomes), dev(col.lengths), dev(col.consts), dev(col.X), dev(col.y)
+    out = torch.full((P,), -12345.0, dtype=torch.float32, device="cuda")
+    st = torch.cuda.current_stream().cuda_stream
+    api.beagle_eval_fit(g, l, P, c, len(col.consts), X, y, N, d, fit, M, tax, out, st)
+    torch.cuda.synchronize()
+    a = out.cpu().numpy()
+    sel = np.unique(np.concatenate([np.arange(0, P, 701), np.argsort(-col.lengths, kind="stable")[:128]]))
+    off = np.concatenate([[0], np.cumsum(col.lengths, dtype=np.int64)])
+    gs = np.concatenate([col.genomes[off[p]:off[p + 1]] for p in sel]); ls = col.lengths[sel]
+    orc = (oracle.evaluate_corr(gs, ls, col.consts, col.X, col.y, M, tax) if fit == FIT_CORR
+           else oracle.evaluate_std(gs, ls, col.consts, col.X, col.y, power, M, tax))
+    rep = parity.compare(a[sel], orc)
+    assert len(rep["bad"]) == 0, parity.describe(rep, a[sel], orc)
+    assert rep["strict"] + rep["conditioned"] > 0.4 * len(sel), parity.describe(rep, a[sel], orc)
+    # any size: every individual got a value; a score cannot exceed M per case, nor fall below -M per case, tax aside
+    assert not np.any(a == np.float32(-12345.0))
+    fin = np.isfinite(a)
+    sc = a[fin].astype(np.float64) + tax * col.lengths[fin]
+    assert np.all(sc <= M * N * (1 + 1e-5)) and np.all(sc >= -M * N * (1 + 1e-5))
+    # the step after scoring, on the vector still on the device
+    rng = np.random.default_rng(3)
+    sample = rng.integers(0, P, 100)
+    dec = torch.empty(P, dtype=torch.uint8, device="cuda"); hist = torch.empty(10, dtype=torch.int64, device="cuda")
+    api.beagle_rank(out, P, dev(sample.astype(np.int64)), 100, True, dec, hist, st)
+    torch.cuda.synchronize()
+    gd = R.goodness(a, True)
+    want = np.minimum(9, np.searchsorted(np.sort(gd[sample]), gd, side="left") // 10).astype(np.uint8)
+    assert np.array_equal(dec.cpu().numpy(), want) and np.array_equal(hist.cpu().numpy(), np.bincount(want, minlength=10))
