@@ -42,6 +42,14 @@ constexpr int kScanItems = 8;                  // programs per thread: a block o
 constexpr int kScanBlock = kScanThreads * kScanItems;
 constexpr int kCompileThreads = 128;
 constexpr int kStagesMax = 8;                  // micro-op stages in flight per warp
+#ifndef BEAGLE_GROUP_STAGES
+#define BEAGLE_GROUP_STAGES 2
+#endif
+#ifndef BEAGLE_GROUP_MAX
+#define BEAGLE_GROUP_MAX 32
+#endif
+constexpr int kGroupMax = BEAGLE_GROUP_MAX;         // individuals per group at most (one visit to the queue brings 32)
+constexpr int kGroupStages = BEAGLE_GROUP_STAGES;   // stages per ring when the longest program leaves room (eval_kernel.inc)
 #ifndef BEAGLE_EVAL_THREADS
 #define BEAGLE_EVAL_THREADS 1024
 #endif
