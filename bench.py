@@ -369,7 +369,7 @@ def run_ours(args):
 
 # dram__bytes_read.sum + dram__bytes_write.sum of the dominant kernel, per launch, from the ncu --set full
 # capture summarised under profiles/ (None until a capture exists for that config).
-TRAFFIC_BYTES = {3: 293007104 + 34012416}   # profiles/r1_ncu_config3_final.md (k_eval, config 3: dram read + write)
+TRAFFIC_BYTES = {3: 358849024 + 31903232}   # profiles/r1_ncu_config3_grouped.md (k_eval, config 3: dram read + write)
 
 
 def main():
