@@ -172,6 +172,26 @@ def test_blockwise_baseline_bitwise_equal():
         assert np.array_equal(_bits(a), _bits(b))
 
 
+def test_grouped_record_copies_bitwise_equal_blockwise():
+    """A colony large enough for the interpreter's warps to take several entries per visit to the work queue, so
+    that one bulk copy brings a group of neighbouring programs (eval_kernel.inc; the small cases above never form
+    a group). Malformed programs are sprinkled in: they end a group. Every fitness bit-identical to the blockwise
+    kernel's (one block per individual, no groups), whose parity with the oracle test_gpu_parity.py checks."""
+    from tests.gpu_util import gpu_eval
+    col = colonies.make_colony(3, 300000)
+    genomes = col.genomes.copy()
+    off = np.concatenate([[0], np.cumsum(col.lengths, dtype=np.int64)])
+    rng = np.random.default_rng(5)
+    bad = rng.choice(col.P, 3000, replace=False)
+    genomes[off[bad]] = token(OP["ADD"], 0)                         # an operator on an empty stack
+    N = 80                                                         # (a ragged pass keeps the blockwise run short)
+    a = gpu_eval(genomes, col.lengths, col.consts, col.X[:N], col.y[:N], col.tax)
+    b = gpu_eval(genomes, col.lengths, col.consts, col.X[:N], col.y[:N], col.tax, fn="beagle_eval_blockwise")
+    assert np.array_equal(_bits(a), _bits(b))
+    assert np.all(_bits(a[bad]) == QNAN)
+    assert np.isfinite(a).sum() > 0.9 * (col.P - len(bad))
+
+
 @pytest.mark.parametrize("budget_frac,pinned", [(2.5, True), (0.37, True), (0.11, False), (0.013, True)])
 def test_chunked_bitwise_equals_unchunked(budget_frac, pinned):
     from tests.gpu_util import gpu_eval, gpu_eval_chunked
