@@ -20,8 +20,8 @@ def _bits(a):
 
 
 def _texts(rng, n, d, names):
-    from tests.test_gpu_edges import _random_gcl_programs
-    return _random_gcl_programs(rng, n, d, names)
+    from tests.util import random_gcl_programs
+    return random_gcl_programs(rng, n, d, names)
 
 
 HOT = ["ADD", "SUB", "MUL", "DIV", "SIN", "COS", "LOG", "SQRT", "EXP"]

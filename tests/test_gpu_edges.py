@@ -11,7 +11,7 @@ import pytest
 from paper_2607_06731_b200 import colonies
 from paper_2607_06731_b200.colonies import OP, token
 from tests import parity
-from tests.util import asm, pack
+from tests.util import asm, pack, random_gcl_programs
 
 pytestmark = pytest.mark.gpu
 
@@ -338,22 +338,6 @@ def test_every_operand_kind_combination(oracle, N, d):
     assert rep["malformed"] == 0
 
 
-def _random_gcl_programs(rng, n_prog, d, names):
-    progs_text = []
-    while len(progs_text) < n_prog:
-        toks, depth = [], 0
-        for _ in range(int(rng.integers(3, 60))):
-            nm = names[int(rng.integers(len(names)))]
-            need = 2 if nm in ("ADD", "SUB", "MUL", "DIV", "SWAP", "POW") else 1
-            if depth < need or (nm == "DUP" and depth >= 30) or rng.random() < 0.35:
-                toks.append(f"x{int(rng.integers(d))}" if rng.random() < 0.8 else f"{rng.uniform(-3, 3):.4f}"); depth += 1
-            else:
-                toks.append(nm); depth += {"DUP": 1, "DEL": -1}.get(nm, -1 if need == 2 and nm != "SWAP" else 0)
-        if depth >= 1:
-            progs_text.append(" ".join(toks))
-    return progs_text
-
-
 @pytest.mark.parametrize("N,d", [(512, 3), (1024, 9), (200, 16)])
 def test_stack_commands_and_exact_unaries(oracle, N, d):
     """DUP SWAP DEL SIGN SQUARE CUBE (Table 3): random programs mixing them with the eleven
@@ -365,7 +349,7 @@ def test_stack_commands_and_exact_unaries(oracle, N, d):
     y = (X[:, 0] * X[:, 1]).astype(np.float32)
     names = ["ADD", "SUB", "MUL", "DIV", "SIN", "COS", "LOG", "SQRT", "EXP", "SIGN", "SQUARE", "CUBE", "DUP", "SWAP", "DEL",
              "CBRT", "TAN", "ARCSIN", "ARCCOS", "ARCTAN", "TANH", "POW"]
-    texts = _random_gcl_programs(rng, 600, d, names)
+    texts = random_gcl_programs(rng, 600, d, names)
     texts += ["0 -9.280686 8.983309 ADD DEL x1 ADD DUP MUL x0 DUP ADD DUP ADD x2 MUL SUB SQRT x1 SUB x0 DIV 0.5 MUL",
               "x2 x0 MUL -2 MUL DUP ADD 3 4 SUB 2.7182817 SUB DUP DIV DEL x1 SQUARE ADD SQRT x1 SUB x0 DIV 0.5 MUL"]
     consts = []
@@ -379,7 +363,7 @@ def test_stack_commands_and_exact_unaries(oracle, N, d):
     assert len(rep["bad"]) == 0, parity.describe(rep, a, orc)
     assert rep["malformed"] == 0 and rep["strict"] > 100
     # correctly rounded commands only: per-case outputs equal the oracle's fp32 mirror bit for bit
-    exact = _random_gcl_programs(rng, 200, d, ["ADD", "SUB", "MUL", "SIGN", "SQUARE", "CUBE", "DUP", "SWAP", "DEL"])
+    exact = random_gcl_programs(rng, 200, d, ["ADD", "SUB", "MUL", "SIGN", "SQUARE", "CUBE", "DUP", "SWAP", "DEL"])
     consts2 = []
     progs2 = [asm(t, consts2)[0] for t in exact]
     g2, l2, c2 = pack(progs2, consts2)
@@ -449,7 +433,7 @@ def test_copy_paste_variables(oracle):
     for i in range(len(pairs)):
         assert np.array_equal(out[2 * i].view(np.uint32), out[2 * i + 1].view(np.uint32)), pairs[i]
     names = ["ADD", "SUB", "MUL", "DIV", "SIN", "COS", "SQRT", "EXP", "SQUARE", "DUP", "SWAP", "DEL", "TANH"]
-    texts = [_with_variables(rng, t, d) for t in _random_gcl_programs(rng, 400, d, names)]
+    texts = [_with_variables(rng, t, d) for t in random_gcl_programs(rng, 400, d, names)]
     texts = [t for t in texts if len(t.split()) <= 200]
     consts = []
     progs = [asm(t, consts)[0] for t in texts]

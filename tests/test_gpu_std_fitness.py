@@ -18,8 +18,8 @@ def _bits(a):
 
 
 def _texts(rng, n, d, names):
-    from tests.test_gpu_edges import _random_gcl_programs
-    return _random_gcl_programs(rng, n, d, names)
+    from tests.util import random_gcl_programs
+    return random_gcl_programs(rng, n, d, names)
 
 
 @pytest.mark.parametrize("power", [1, 2, 3, 8])
@@ -63,7 +63,15 @@ def test_std_parity_random_programs(oracle, N, d, power, seed):
     orc = oracle.evaluate_std(g, l, c, X, y, power, M, 50.0)
     rep = parity.compare(a, orc)
     assert len(rep["bad"]) == 0, parity.describe(rep, a, orc)
-    assert rep["strict"] + rep["conditioned"] > 0.5 * len(texts)
+    # non-vacuity: a floor on the STRICT share of the value-checked individuals (those held to north_star's tolerance
+    # unchanged), as tests/test_gpu_parity.py has for the MSE. The Std bound charges |dt| + 1 for every case whose
+    # unrounded reward is within dt of a rounding boundary, so it is coarser than the MSE bound: under the oracle alone
+    # 75 % / 60 % / 42 % / 58 % of these four colonies are STRICT.
+    checked = rep["strict"] + rep["conditioned"]
+    print(f"std parity N={N} d={d} power={power}: {parity.describe(rep, a, orc)}; "
+          f"bit-equal to the oracle: {int((a == orc['fitness']).sum())} of {len(texts)}")
+    assert checked > 0.5 * len(texts)
+    assert rep["strict"] >= 0.4 * checked, rep
     assert np.all(a[np.isfinite(a)] == np.round(a[np.isfinite(a)] + 50.0 * l[np.isfinite(a)]) - 50.0 * l[np.isfinite(a)])   # integer scores
 
 

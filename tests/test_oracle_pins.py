@@ -585,6 +585,35 @@ def test_P17_pow_reduces_to_numpy_and_identities(oracle):
     assert o[0] == -8.0 and o[1] == 4.0 and np.isnan(o[2]) and o[3] == 0.0 and o[4] == np.inf and o[5] == 1.0 and o[6] == 1.0 and np.isnan(o[7])
 
 
+def test_P17b_bound_is_a_bound_for_pow(oracle):
+    """|fit64 - fit32mirror| <= E_p on random programs that contain POW: the corner bound of run_case's POW (the four
+    corners of the operand box, UNSTABLE when the box reaches a base <= 0 or a NaN) is a bound, as P11 / P11b / P16 show
+    for the other commands. Bases are kept positive by construction often enough that most programs stay unflagged."""
+    rng = np.random.default_rng(171)
+    X = rng.uniform(0.3, 3.0, (96, 3)).astype(np.float32)
+    y = (X[:, 0] ** X[:, 1]).astype(np.float32)
+    progs, consts = [], []
+    shapes = ["x{a} x{b} POW", "x{a} {c:.3f} POW", "x{a} x{b} MUL x{c2} POW", "x{a} SQRT x{b} {c:.3f} MUL POW",
+              "x{a} x{b} POW x{c2} ADD", "x{a} {c:.3f} ADD x{b} SIN POW", "x{a} x{b} POW x{c2} x{a} POW MUL",
+              "x{a} x{b} DIV x{c2} POW {c:.3f} SUB", "{c:.3f} x{a} POW", "x{a} x{b} POW x{c2} POW"]
+    for i in range(400):
+        a, b, c2 = (int(v) for v in rng.integers(0, 3, 3))
+        progs.append(asm(shapes[i % len(shapes)].format(a=a, b=b, c2=c2, c=float(rng.uniform(0.2, 2.5))), consts)[0])
+    c = np.array(consts, np.float32)
+    ieee = oracle.contract(oracle.CONTRACT_IEEE)
+    t = ev(oracle, progs, c, X, y, contract_=ieee)
+    m = ev(oracle, progs, c, X, y, contract_=ieee, mode=1)
+    assert not np.any(t["flags"] & oracle.FLAG_MALFORMED)
+    fin = np.isfinite(t["fitness"]) & np.isfinite(m["fitness"]) & ((t["flags"] & 6) == 0)
+    assert fin.sum() >= 300, fin.sum()
+    diff = np.abs(t["fitness"].astype(np.float64) - m["fitness"].astype(np.float64))
+    slack = 2.0 ** -23 * np.abs(t["fitness"].astype(np.float64))          # the two final float casts
+    assert np.all(diff[fin] <= t["bound"][fin] + slack[fin]), np.flatnonzero(fin & (diff > t["bound"] + slack))[:5]
+    # and it is not vacuous: most of them certify north_star's tolerance
+    tol = np.maximum(1e-4 * np.abs(t["fitness"][fin].astype(np.float64)), 1e-6)
+    assert (4 * t["bound"][fin] <= tol).mean() > 0.8
+
+
 def test_P18_copy_paste_variables(oracle):
     rng = np.random.default_rng(19)
     X = rng.uniform(-3, 3, (64, 2)).astype(np.float32)
@@ -720,8 +749,8 @@ def test_P19_correlation_bound_is_a_bound(oracle):
     N, d = 512, 3
     X = rng.uniform(-3, 3, (N, d)).astype(np.float32)
     y = (X[:, 0] * X[:, 1] - X[:, 2]).astype(np.float32)
-    from tests.test_gpu_edges import _random_gcl_programs
-    texts = _random_gcl_programs(rng, 400, d, ["ADD", "SUB", "MUL", "DIV", "SIN", "COS", "SQRT", "EXP", "LOG"])
+    from tests.util import random_gcl_programs
+    texts = random_gcl_programs(rng, 400, d, ["ADD", "SUB", "MUL", "DIV", "SIN", "COS", "SQRT", "EXP", "LOG"])
     consts = []
     progs = [asm(t, consts)[0] for t in texts]
     g, l, cst = pack(progs, consts)
@@ -835,3 +864,29 @@ def test_P21_std_rewards_by_hand(oracle):
         qp = {1: q, 2: q * q, 3: (q * q) * q, 8: ((q * q) * (q * q)) * ((q * q) * (q * q))}[power]
         t = np.float32(M_SCORE) * qp - np.where(a * b < 0, np.float32(M_SCORE) / np.float32(11), np.float32(0))
         assert evs(oracle, ["x0"], a.reshape(-1, 1), b, power)["fitness"][0] == np.rint(t.astype(np.float32)).sum()
+
+
+@pytest.mark.parametrize("power", [1, 2, 3, 8])
+def test_P21b_std_bound_is_a_bound(oracle, power):
+    """The bound E of orc_eval_std is a bound: the score computed from the fp32 mirror's outputs (mode 1: every command
+    rounded to fp32) differs from the score computed from the fp64 outputs (mode 0) by at most E, for every unflagged
+    individual of >= 300 random programs per power; and E is not vacuous (most individuals have E below one reward
+    step per 16 cases)."""
+    rng = np.random.default_rng(210 + power)
+    N, d = 256, 3
+    X = rng.uniform(-3, 3, (N, d)).astype(np.float32)
+    y = (X[:, 0] * X[:, 1] + np.sin(X[:, 2])).astype(np.float32)
+    from tests.util import random_gcl_programs
+    texts = random_gcl_programs(rng, 500, d, ["ADD", "SUB", "MUL", "DIV", "SIN", "COS", "SQRT", "EXP", "LOG"])
+    consts = []
+    progs = [asm(t, consts)[0] for t in texts]
+    g, l, cst = pack(progs, consts)
+    ieee = oracle.contract(oracle.CONTRACT_IEEE)
+    t = oracle.evaluate_std(g, l, cst, X, y, power, M_SCORE, 0.0, contract_=ieee, mode=0)
+    m = oracle.evaluate_std(g, l, cst, X, y, power, M_SCORE, 0.0, contract_=ieee, mode=1)
+    ok = (t["flags"] == 0) & np.isfinite(t["fitness"]) & np.isfinite(m["fitness"])
+    assert ok.sum() >= 300, ok.sum()
+    diff = np.abs(t["fitness"].astype(np.float64) - m["fitness"].astype(np.float64))
+    assert np.all(diff[ok] <= t["bound"][ok]), (np.flatnonzero(ok & (diff > t["bound"]))[:5], diff[ok].max())
+    assert (t["bound"][ok] <= N / 16).mean() > 0.6, (t["bound"][ok] <= N / 16).mean()
+

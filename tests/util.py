@@ -46,3 +46,22 @@ def pack(programs, consts):
     lengths = np.array([len(p) for p in programs], np.int32)
     genomes = np.concatenate(programs).astype(np.int32) if programs else np.zeros(0, np.int32)
     return genomes, lengths, np.asarray(consts, np.float32)
+
+
+def random_gcl_programs(rng, n_prog, d, names):
+    """Seeded random postfix programs as text over the commands in `names` (plus terminals x0..x{d-1} and constants):
+    a command is taken when the stack holds its operands, else a terminal is pushed; kept when something is left on
+    the stack. Shapes only, no arithmetic."""
+    progs_text = []
+    while len(progs_text) < n_prog:
+        toks, depth = [], 0
+        for _ in range(int(rng.integers(3, 60))):
+            nm = names[int(rng.integers(len(names)))]
+            need = 2 if nm in ("ADD", "SUB", "MUL", "DIV", "SWAP", "POW") else 1
+            if depth < need or (nm == "DUP" and depth >= 30) or rng.random() < 0.35:
+                toks.append(f"x{int(rng.integers(d))}" if rng.random() < 0.8 else f"{rng.uniform(-3, 3):.4f}"); depth += 1
+            else:
+                toks.append(nm); depth += {"DUP": 1, "DEL": -1}.get(nm, -1 if need == 2 and nm != "SWAP" else 0)
+        if depth >= 1:
+            progs_text.append(" ".join(toks))
+    return progs_text
