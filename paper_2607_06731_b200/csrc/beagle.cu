@@ -574,8 +574,10 @@ __global__ void __launch_bounds__(kCompileThreads, 8) k_compile(const CompilePar
         out[n] = (xmask & 1u) ? make_uint2((t0 << kColAShift) | H_LX, 0u) : make_uint2(H_LC, t0);
         ++n;
     }
-    out[n] = make_uint2(H_END, 0u);
-    out[n + 1] = make_uint2(H_END, 0u);
+    // the END record carries what a7 needs (interp.cuh, variant 2): the stride to the next program of a group, the
+    // individual; the record after it the length as a float (for the tax)
+    out[n] = make_uint2(H_END | ((uint32_t)stride << 8), (uint32_t)p);
+    out[n + 1] = make_uint2(__float_as_uint((float)len), 0u);
     out[n + 2] = make_uint2(H_END, 0u);
     q.meta[i] = make_int4(p, (int)(ua_e >> 1), (n + 2 + 1) & ~1, len);
 }
@@ -718,9 +720,10 @@ static beagle_status init_once()
     w.device_ok = (prop.major == 10);
     w.inited = true;
     if (!w.device_ok) return BEAGLE_ERR_UNSUPPORTED;
-    CU(cudaFuncSetAttribute(k_eval<BEAGLE_FIT_MSE>, cudaFuncAttributeMaxDynamicSharedMemorySize, w.smem_optin));
-    CU(cudaFuncSetAttribute(k_eval<BEAGLE_FIT_CORRELATION>, cudaFuncAttributeMaxDynamicSharedMemorySize, w.smem_optin));
-    CU(cudaFuncSetAttribute(k_eval<BEAGLE_FIT_STD>, cudaFuncAttributeMaxDynamicSharedMemorySize, w.smem_optin));
+    CU(cudaFuncSetAttribute(k_eval<BEAGLE_FIT_MSE, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, w.smem_optin));
+    CU(cudaFuncSetAttribute(k_eval<BEAGLE_FIT_MSE, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, w.smem_optin));
+    CU(cudaFuncSetAttribute(k_eval<BEAGLE_FIT_CORRELATION, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, w.smem_optin));
+    CU(cudaFuncSetAttribute(k_eval<BEAGLE_FIT_STD, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, w.smem_optin));
     { uint32_t lut[kLutSize]; make_compile_lut(lut); CU(cudaMemcpyToSymbol(g_compile_lut, lut, sizeof(lut))); }
     CU(cudaMalloc(&w.bins, sizeof(int) * kNumBins));
     CU(cudaMalloc(&w.cursor, sizeof(int) * kNumBins));
@@ -912,9 +915,10 @@ static beagle_status run_eval(const int32_t* genomes, const int32_t* lengths, co
     attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
     attr[0].val.programmaticStreamSerializationAllowed = 1;
     cfg.attrs = attr; cfg.numAttrs = 1;
-    if (g_fit.kind == BEAGLE_FIT_CORRELATION) CU(cudaLaunchKernelEx(&cfg, k_eval<BEAGLE_FIT_CORRELATION>, prm));
-    else if (g_fit.kind == BEAGLE_FIT_STD) CU(cudaLaunchKernelEx(&cfg, k_eval<BEAGLE_FIT_STD>, prm));
-    else CU(cudaLaunchKernelEx(&cfg, k_eval<BEAGLE_FIT_MSE>, prm));
+    if (g_fit.kind == BEAGLE_FIT_CORRELATION) CU(cudaLaunchKernelEx(&cfg, k_eval<BEAGLE_FIT_CORRELATION, false>, prm));
+    else if (g_fit.kind == BEAGLE_FIT_STD) CU(cudaLaunchKernelEx(&cfg, k_eval<BEAGLE_FIT_STD, false>, prm));
+    else if (outputs || !fitness) CU(cudaLaunchKernelEx(&cfg, k_eval<BEAGLE_FIT_MSE, false>, prm));
+    else CU(cudaLaunchKernelEx(&cfg, k_eval<BEAGLE_FIT_MSE, true>, prm));
     ++g_launches;
     if (prof) { CU(cudaEventRecord(w.ev_k[2 * w.prof_n + 1], st)); ++w.prof_n; }
     // slow path: individuals whose micro-ops did not fit the promised workspace (normally none)

@@ -45,34 +45,34 @@
     "abs.f32 t" #k ", " B ";\n" \
     "setp.lt.f32 p" #k ", t" #k ", " BGI_EPS ";\n" \
     "selp.f32 " DST ", " BGI_ONE ", q" #k ", p" #k ";\n"
-#define BGI_SIN(k)  "sin.approx.ftz.f32 %" #k ", %" #k ";\n"
-#define BGI_COS(k)  "cos.approx.ftz.f32 %" #k ", %" #k ";\n"
-#define BGI_SQRT(k) "abs.f32 t" #k ", %" #k ";\n" "sqrt.approx.ftz.f32 %" #k ", t" #k ";\n"
+#define BGI_SIN(k)  "sin.approx.ftz.f32 " BGI_A #k ", " BGI_A #k ";\n"
+#define BGI_COS(k)  "cos.approx.ftz.f32 " BGI_A #k ", " BGI_A #k ";\n"
+#define BGI_SQRT(k) "abs.f32 t" #k ", " BGI_A #k ";\n" "sqrt.approx.ftz.f32 " BGI_A #k ", t" #k ";\n"
 #define BGI_LOG(k) \
-    "abs.f32 t" #k ", %" #k ";\n" \
+    "abs.f32 t" #k ", " BGI_A #k ";\n" \
     "lg2.approx.ftz.f32 q" #k ", t" #k ";\n" \
     "mul.rn.f32 q" #k ", q" #k ", " BGI_LN2 ";\n" \
     "setp.lt.f32 p" #k ", t" #k ", " BGI_EPS ";\n" \
-    "selp.f32 %" #k ", " BGI_ZERO ", q" #k ", p" #k ";\n"
+    "selp.f32 " BGI_A #k ", " BGI_ZERO ", q" #k ", p" #k ";\n"
 #define BGI_EXP(k) \
-    "min.NaN.f32 t" #k ", %" #k ", " BGI_80 ";\n" \
+    "min.NaN.f32 t" #k ", " BGI_A #k ", " BGI_80 ";\n" \
     "mul.rn.f32 t" #k ", t" #k ", " BGI_LOG2E ";\n" \
-    "ex2.approx.ftz.f32 %" #k ", t" #k ";\n"
+    "ex2.approx.ftz.f32 " BGI_A #k ", t" #k ";\n"
 
 // second operand in x<k> (a variable or a slot, loaded from tensor / local memory)
-#define BGI_ADDX(k)  "add.rn.f32 %" #k ", %" #k ", x" #k ";\n"
-#define BGI_SUBX(k)  "sub.rn.f32 %" #k ", %" #k ", x" #k ";\n"
-#define BGI_MULX(k)  "mul.rn.f32 %" #k ", %" #k ", x" #k ";\n"
-#define BGI_RSUBX(k) "sub.rn.f32 %" #k ", x" #k ", %" #k ";\n"
-#define BGI_DIVX(k)  BGI_DIV("%" #k, "%" #k, "x" #k, k)
-#define BGI_RDIVX(k) BGI_DIV("%" #k, "x" #k, "%" #k, k)
+#define BGI_ADDX(k)  "add.rn.f32 " BGI_A #k ", " BGI_A #k ", x" #k ";\n"
+#define BGI_SUBX(k)  "sub.rn.f32 " BGI_A #k ", " BGI_A #k ", x" #k ";\n"
+#define BGI_MULX(k)  "mul.rn.f32 " BGI_A #k ", " BGI_A #k ", x" #k ";\n"
+#define BGI_RSUBX(k) "sub.rn.f32 " BGI_A #k ", x" #k ", " BGI_A #k ";\n"
+#define BGI_DIVX(k)  BGI_DIV(BGI_A #k, BGI_A #k, "x" #k, k)
+#define BGI_RDIVX(k) BGI_DIV(BGI_A #k, "x" #k, BGI_A #k, k)
 // second operand = constant (cv)
-#define BGI_LC(k)    "mov.f32 %" #k ", cv;\n"
-#define BGI_ADDC(k)  "add.rn.f32 %" #k ", %" #k ", cv;\n"
-#define BGI_SUBC(k)  "sub.rn.f32 %" #k ", %" #k ", cv;\n"
-#define BGI_MULC(k)  "mul.rn.f32 %" #k ", %" #k ", cv;\n"
-#define BGI_RSUBC(k) "sub.rn.f32 %" #k ", cv, %" #k ";\n"
-#define BGI_RDIVC(k) BGI_DIV("%" #k, "cv", "%" #k, k)
+#define BGI_LC(k)    "mov.f32 " BGI_A #k ", cv;\n"
+#define BGI_ADDC(k)  "add.rn.f32 " BGI_A #k ", " BGI_A #k ", cv;\n"
+#define BGI_SUBC(k)  "sub.rn.f32 " BGI_A #k ", " BGI_A #k ", cv;\n"
+#define BGI_MULC(k)  "mul.rn.f32 " BGI_A #k ", " BGI_A #k ", cv;\n"
+#define BGI_RSUBC(k) "sub.rn.f32 " BGI_A #k ", cv, " BGI_A #k ";\n"
+#define BGI_RDIVC(k) BGI_DIV(BGI_A #k, "cv", BGI_A #k, k)
 
 // ---- handler frame ---------------------------------------------------------------------------------------
 // entry: (h, o) = this micro-op's record, pc = its shared-memory address. NEXT replaces (h, o) by the next
@@ -82,7 +82,7 @@
 #define BGI_LDTM(R, ADDR) "tcgen05.ld.sync.aligned.32x32b.x16.b32 {" BGI_R16(R) "}, [" ADDR "];\n"
 #define BGI_DISPATCH "bra.uni DISP_%=;\n"
 // fresh value: acc = X[colA], colA = h[31:21]
-#define BGI_LXA     "shr.u32 e, h, 21;\n" "add.u32 e, e, xb;\n" BGI_LDTM("%", "e")
+#define BGI_LXA     "shr.u32 e, h, 21;\n" "add.u32 e, e, xb;\n" BGI_LDTM(BGI_A, "e")
 // x = local slot memory, 16 floats per slot per lane at byte offset o
 #define BGI_GETM \
     "cvt.u64.u32 ma, o;\n" \
@@ -95,17 +95,17 @@
 // "push acc" in front of a fresh value: P_<entry> pushes to the warp's tensor-memory slot stack (spt), M_<entry>
 // to the local-memory slot at byte offset h[20:10]; both fall / branch into the entry itself.
 #define BGI_PUSHT \
-    "tcgen05.st.sync.aligned.32x32b.x16.b32 [spt], {" BGI_R16("%") "};\n" \
+    "tcgen05.st.sync.aligned.32x32b.x16.b32 [spt], {" BGI_R16(BGI_A) "};\n" \
     "tcgen05.wait::st.sync.aligned;\n" \
     "add.u32 spt, spt, 16;\n"
 #define BGI_PUSHM \
     "bfe.u32 e, h, 10, 11;\n" \
     "cvt.u64.u32 ma, e;\n" \
     "add.u64 ma, ma, mbase;\n" \
-    "st.local.v4.f32 [ma], {%0, %1, %2, %3};\n" \
-    "st.local.v4.f32 [ma+16], {%4, %5, %6, %7};\n" \
-    "st.local.v4.f32 [ma+32], {%8, %9, %10, %11};\n" \
-    "st.local.v4.f32 [ma+48], {%12, %13, %14, %15};\n"
+    "st.local.v4.f32 [ma], {" BGI_A "0, " BGI_A "1, " BGI_A "2, " BGI_A "3};\n" \
+    "st.local.v4.f32 [ma+16], {" BGI_A "4, " BGI_A "5, " BGI_A "6, " BGI_A "7};\n" \
+    "st.local.v4.f32 [ma+32], {" BGI_A "8, " BGI_A "9, " BGI_A "10, " BGI_A "11};\n" \
+    "st.local.v4.f32 [ma+48], {" BGI_A "12, " BGI_A "13, " BGI_A "14, " BGI_A "15};\n"
 #define BGI_PUSHES(ENTRY) \
     "M_" #ENTRY "_%=:\n" BGI_PUSHM "bra.uni L_" #ENTRY "_%=;\n" \
     "P_" #ENTRY "_%=:\n" BGI_PUSHT
@@ -141,15 +141,15 @@
     BGI_PUSHES(LX) "L_LX_%=:\n" BGI_LXA BGI_NEXT BGI_WAITLD BGI_DISPATCH \
     BGI_PUSHES(LC) "L_LC_%=:\n" "mov.b32 cv, o;\n" BGI_NEXT BGI_K16(BGI_LC) BGI_DISPATCH \
     BGI_PUSHES(LS) "L_LS_%=:\n" "add.u32 xa, o, db;\n" BGI_NEXT \
-    "ld.shared.v4.f32 {%0, %1, %2, %3}, [xa];\n" \
-    "ld.shared.v4.f32 {%4, %5, %6, %7}, [xa+512];\n" \
-    "ld.shared.v4.f32 {%8, %9, %10, %11}, [xa+1024];\n" \
-    "ld.shared.v4.f32 {%12, %13, %14, %15}, [xa+1536];\n" BGI_DISPATCH \
+    "ld.shared.v4.f32 {" BGI_A "0, " BGI_A "1, " BGI_A "2, " BGI_A "3}, [xa];\n" \
+    "ld.shared.v4.f32 {" BGI_A "4, " BGI_A "5, " BGI_A "6, " BGI_A "7}, [xa+512];\n" \
+    "ld.shared.v4.f32 {" BGI_A "8, " BGI_A "9, " BGI_A "10, " BGI_A "11}, [xa+1024];\n" \
+    "ld.shared.v4.f32 {" BGI_A "12, " BGI_A "13, " BGI_A "14, " BGI_A "15}, [xa+1536];\n" BGI_DISPATCH \
     BGI_PUSHES(LG) "L_LG_%=:\n" "cvt.u64.u32 ma, o;\n" "add.u64 ma, ma, gb;\n" BGI_NEXT \
-    "ld.global.nc.v4.f32 {%0, %1, %2, %3}, [ma];\n" \
-    "ld.global.nc.v4.f32 {%4, %5, %6, %7}, [ma+512];\n" \
-    "ld.global.nc.v4.f32 {%8, %9, %10, %11}, [ma+1024];\n" \
-    "ld.global.nc.v4.f32 {%12, %13, %14, %15}, [ma+1536];\n" BGI_DISPATCH
+    "ld.global.nc.v4.f32 {" BGI_A "0, " BGI_A "1, " BGI_A "2, " BGI_A "3}, [ma];\n" \
+    "ld.global.nc.v4.f32 {" BGI_A "4, " BGI_A "5, " BGI_A "6, " BGI_A "7}, [ma+512];\n" \
+    "ld.global.nc.v4.f32 {" BGI_A "8, " BGI_A "9, " BGI_A "10, " BGI_A "11}, [ma+1024];\n" \
+    "ld.global.nc.v4.f32 {" BGI_A "12, " BGI_A "13, " BGI_A "14, " BGI_A "15}, [ma+1536];\n" BGI_DISPATCH
 
 // ---- the dispatcher: the one indexed branch ----------------------------------------------------------------
 #define BGI_DISPATCHER \
@@ -174,8 +174,7 @@
     BGI_FRESH(BGI_T) BGI_FRESH(BGI_TP) BGI_FRESH(BGI_TM) BGI_T(MULR) \
     "L_END_%=;\n"
 
-#define BGI_OUT(k) "mov.f32 %" #k ", %" #k ";\n"
-
+// ---- variant 1: one program, one pass; the accumulator is the asm's output operands %0..%15 ------------------
 // Operands: %0..%15 = acc (used in place), %16 = shared address of the records, %17 = xb, %18 = sb, %19 = rb, %20 = db (this lane's
 // shared-memory address of the staged unary rows of this pass), %21 = gb (the same in global memory).
 #define BGI_ASM \
@@ -202,15 +201,114 @@
 #define BGI_ACC_OUT(A) "=&f"(A[0]), "=&f"(A[1]), "=&f"(A[2]), "=&f"(A[3]), "=&f"(A[4]), "=&f"(A[5]), "=&f"(A[6]), "=&f"(A[7]), \
                        "=&f"(A[8]), "=&f"(A[9]), "=&f"(A[10]), "=&f"(A[11]), "=&f"(A[12]), "=&f"(A[13]), "=&f"(A[14]), "=&f"(A[15])
 
+// ---- variant 2: a whole GROUP of programs, all passes, with a7 inside the block (MSE fitness) ----------------------
+// The END record of a program carries what the frame around variant 1 read from the queue window: rec[n] = { H_END |
+// stride << 8, p }, rec[n+1] = { (float)L, 0 } (k_compile). END is then a handler like the others: residual against y
+// in the canonical order (DESIGN.md §7 "summation order"), next pass (the operand bases move on, the records are
+// run again) or the butterfly, the mean, the length tax, the store of fitness[p]; the next program of the group starts
+// `stride` records after the start of this one. One entry into the block per group instead of one per program and pass.
+// Operands: %0 records of the group, %1 xb of pass 0, %2 sb, %3 rb of pass 0, %4 db of pass 0, %5 gb of pass 0,
+// %6 this lane's address of y (float4 index lane of pass 0), %7 programs in the group, %8 passes, %9 / %10 columns per
+// pass of the variable / reciprocal block, %11 = n - 4 * lane (a case k of 128-case block g of pass s counts when
+// 512 s + 128 g + k < that), %12 = (float)n, %13 = 1 / n when n is a power of two (the mean is then an exact scaling,
+// bit-identical to the division), else 0, %14 tax, %15 fitness, %16 != 0: this lane stores (lane 0), %17 = n.
+#define BGI_SQ(k)   "sub.rn.f32 t" #k ", " BGI_A #k ", x" #k ";\n" "fma.rn.f32 sum, t" #k ", t" #k ", sum;\n"
+#define BGI_SQR(k, LIM) "setp.lt.s32 p" #k ", " LIM ", nrem;\n" "sub.rn.f32 t" #k ", " BGI_A #k ", x" #k ";\n" "@p" #k " fma.rn.f32 sum, t" #k ", t" #k ", sum;\n"
+#define BGI_BFLY(M) "shfl.sync.bfly.b32 cv, sum, " #M ", 0x1f, 0xffffffff;\n" "add.rn.f32 sum, sum, cv;\n"
+#define BGI_LDY \
+    "ld.shared.v4.f32 {x0, x1, x2, x3}, [ya];\n" \
+    "ld.shared.v4.f32 {x4, x5, x6, x7}, [ya+512];\n" \
+    "ld.shared.v4.f32 {x8, x9, x10, x11}, [ya+1024];\n" \
+    "ld.shared.v4.f32 {x12, x13, x14, x15}, [ya+1536];\n"
+#define BGI_END_GROUP \
+    "L_END_%=:\n" \
+    BGI_LDY \
+    "setp.lt.s32 pr, nleft, 512;\n"               /* a ragged last pass: the padded cases do not count */ \
+    "@pr bra.uni RAG_%=;\n" \
+    BGI_K16(BGI_SQ) \
+    "bra.uni PASSED_%=;\n" \
+    "RAG_%=:\n" \
+    BGI_SQR(0, "0") BGI_SQR(1, "1") BGI_SQR(2, "2") BGI_SQR(3, "3") \
+    BGI_SQR(4, "128") BGI_SQR(5, "129") BGI_SQR(6, "130") BGI_SQR(7, "131") \
+    BGI_SQR(8, "256") BGI_SQR(9, "257") BGI_SQR(10, "258") BGI_SQR(11, "259") \
+    BGI_SQR(12, "384") BGI_SQR(13, "385") BGI_SQR(14, "386") BGI_SQR(15, "387") \
+    "PASSED_%=:\n" \
+    "add.u32 ps, ps, 1;\n" \
+    "setp.lt.u32 pr, ps, %8;\n" \
+    "@!pr bra.uni FIN_%=;\n" \
+    "add.u32 xb, xb, %9;\n" "add.u32 rb, rb, %10;\n" "add.u32 db, db, 2048;\n" "add.u64 gb, gb, 2048;\n" \
+    "add.u32 ya, ya, 2048;\n" "sub.s32 nrem, nrem, 512;\n" "sub.s32 nleft, nleft, 512;\n" \
+    "mov.u32 pc, pc0;\n" "mov.u32 spt, %2;\n" \
+    "ld.shared.v2.b32 {h, o}, [pc];\n" \
+    "bra.uni DISP_%=;\n" \
+    "FIN_%=:\n" \
+    "ld.shared.f32 q0, [pc+8];\n"                 /* (float)L */ \
+    BGI_BFLY(16) BGI_BFLY(8) BGI_BFLY(4) BGI_BFLY(2) BGI_BFLY(1) \
+    "setp.neu.f32 pr, %13, 0f00000000;\n" \
+    "@pr bra.uni MEANM_%=;\n" \
+    "div.rn.f32 sum, sum, %12;\n" \
+    "bra.uni MEAND_%=;\n" \
+    "MEANM_%=:\n" \
+    "mul.rn.f32 sum, sum, %13;\n" \
+    "MEAND_%=:\n" \
+    "fma.rn.f32 sum, %14, q0, sum;\n" \
+    "mul.wide.u32 ma, o, 4;\n" "add.u64 ma, ma, %15;\n" \
+    "setp.ne.u32 pr, %16, 0;\n" \
+    "@pr st.global.f32 [ma], sum;\n" \
+    "sub.u32 gc, gc, 1;\n" \
+    "setp.eq.u32 pr, gc, 0;\n" \
+    "@pr bra.uni EXIT_%=;\n" \
+    "shr.u32 e, h, 8;\n" "shl.b32 e, e, 3;\n" "add.u32 pc0, pc0, e;\n" "mov.u32 pc, pc0;\n" \
+    "mov.u32 xb, %1;\n" "mov.u32 rb, %3;\n" "mov.u32 db, %4;\n" "mov.u64 gb, %5;\n" "mov.u32 ya, %6;\n" \
+    "mov.u32 spt, %2;\n" "mov.s32 nrem, %11;\n" "mov.s32 nleft, %17;\n" "mov.u32 ps, 0;\n" "mov.f32 sum, 0f00000000;\n" \
+    "ld.shared.v2.b32 {h, o}, [pc];\n" \
+    "bra.uni DISP_%=;\n"
+
+#define BGI_ASM_GROUP \
+    "{\n" \
+    ".reg .f32 a<16>, x<16>, t<16>, q<16>, cv, sum;\n" \
+    ".reg .pred p<16>, pr;\n" \
+    ".reg .b32 h, o, hn, pc, pc0, xa, xb, rb, db, spt, e, ya, gc, ps;\n" \
+    ".reg .s32 nrem, nleft;\n" \
+    ".reg .b64 ma, mbase, gb;\n" \
+    ".local .align 16 .b8 slotmem[1984];\n" \
+    BGI_TABLE \
+    "mov.u32 pc, %0;\n" "mov.u32 pc0, %0;\n" \
+    "mov.u32 xb, %1;\n" "mov.u32 spt, %2;\n" "mov.u32 rb, %3;\n" "mov.u32 db, %4;\n" "mov.u64 gb, %5;\n" \
+    "mov.u32 ya, %6;\n" "mov.u32 gc, %7;\n" "mov.s32 nrem, %11;\n" "mov.s32 nleft, %17;\n" "mov.u32 ps, 0;\n" "mov.f32 sum, 0f00000000;\n" \
+    "mov.u64 mbase, slotmem;\n" \
+    "ld.shared.v2.b32 {h, o}, [pc];\n" \
+    BGI_DISPATCHER \
+    BGI_HANDLERS \
+    BGI_END_GROUP \
+    "EXIT_%=:\n" \
+    "}\n"
+
 namespace beagle {
 
 static_assert(kMemSlots * 64 == 1984 && kCasesPerLane == 16, "interp.cuh is written for 16 cases per lane and 31 memory slots");
 static_assert(H_COUNT == 83, "BGI_TABLE lists the handlers in the order of uop.cuh's enum");
 
 // acc[k] = the program's output on case (pass * 512 + (k/4)*128 + lane*4 + k%4)
+#define BGI_A "%"
 __device__ __forceinline__ void interp_run(uint32_t rec, uint32_t xb, uint32_t sb, uint32_t rb, uint32_t db, const float* gb, float (&acc)[16])
 {
     asm volatile(BGI_ASM : BGI_ACC_OUT(acc) : "r"(rec), "r"(xb), "r"(sb), "r"(rb), "r"(db), "l"(gb) : "memory");
 }
+#undef BGI_A
+
+// a group of `count` programs whose record blocks follow one another from `rec` on, every pass, fitness[p] stored
+struct GroupArgs {
+    uint32_t xb, sb, rb, db; const float* gb; uint32_t ya; uint32_t passes, xstride, rstride; int nrem;
+    float nf, inv_n, tax; float* fitness; uint32_t lane0; int n;
+};
+#define BGI_A "a"
+__device__ __forceinline__ void interp_group(uint32_t rec, uint32_t count, const GroupArgs& g)
+{
+    asm volatile(BGI_ASM_GROUP :: "r"(rec), "r"(g.xb), "r"(g.sb), "r"(g.rb), "r"(g.db), "l"(g.gb), "r"(g.ya), "r"(count),
+                 "r"(g.passes), "r"(g.xstride), "r"(g.rstride), "r"(g.nrem), "f"(g.nf), "f"(g.inv_n), "f"(g.tax), "l"(g.fitness),
+                 "r"(g.lane0), "r"(g.n) : "memory");
+}
+#undef BGI_A
 
 } // namespace beagle
