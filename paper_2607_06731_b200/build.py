@@ -12,7 +12,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 SRC_DIR = os.path.join(_HERE, "csrc")
 LIB = os.path.join(_HERE, "libbeagle_b200.so")
 SOURCES = ["beagle.cu"]
-DEPS = ["beagle.cu", "eval_kernel.inc", "ops.cuh", "uop.cuh", "interp.cuh", os.path.join("..", "..", "include", "beagle.h")]
+DEPS = sorted(f for f in os.listdir(SRC_DIR) if f.endswith((".cu", ".cuh", ".inc"))) + [os.path.join("..", "..", "include", "beagle.h")]
 
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
               "-Xcompiler", "-fPIC", "-shared", "--fmad=false"]

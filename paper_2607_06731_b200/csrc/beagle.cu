@@ -306,67 +306,11 @@ __global__ void k_perm_from_sched(const int4* __restrict__ sched, const Header* 
     if (i < P) perm[i] = i < hdr->n_sorted ? sched[i].x : -1;
 }
 
-// ---- the compiler's decision table ------------------------------------------------------------------------
-// What an operator token emits depends only on (command, is each operand computed, is each terminal operand a
-// variable): 20 + 64 cases. They are tabulated once on the host (make_compile_lut, the rules in words in
-// uop.cuh) so that the per-token walk of k_compile is the same straight-line code for every lane of a warp.
-enum : uint32_t {
-    LUT_OSEL_A = 1u << 8, LUT_OSEL_B = 2u << 8,      // o = the value of operand a | b (a column or a constant)
-    LUT_CSEL_A = 1u << 10, LUT_CSEL_B = 2u << 10,    // first-operand column (h[31:21]) = operand a | b
-    LUT_PUSH = 1u << 12,                             // a fresh value: the handler's push entry if acc is live
-    LUT_DCP = 1u << 13, LUT_DCM = 1u << 14,          // computed entries +1 | -1
-    LUT_SLOT = 1u << 15,                             // pops a slot: local-memory variant beyond S_T
-    LUT_DIVC = 1u << 16,                             // o is a constant divisor: o = rcp(o), or acc = 1 if |o| < eps
-    LUT_DBL = 1u << 17,                              // two records: first acc = c (LC), then this one
-    LUT_EMIT = 1u << 18,
-    LUT_FSEL_A = 1u << 19,                           // LUT_DBL: the first record's constant is operand a (else b)
-    LUT_DIVV = 1u << 20,                             // o is a variable divisor: a reciprocal row may replace the division
-    LUT_UNV = 1u << 21                               // a unary command on a variable: its staged row may replace it
-};
-constexpr int kLutUnary = 0, kLutBinary = 32, kLutNone = 127, kLutSize = 128;
-__device__ uint32_t g_compile_lut[kLutSize];
-
-static void make_compile_lut(uint32_t* lut)
-{
-    for (int i = 0; i < kLutSize; ++i) lut[i] = 0;
-    for (uint32_t kk = 0; kk < 5; ++kk)
-        for (int rb = 0; rb < 2; ++rb)
-            for (int xb = 0; xb < 2; ++xb) {
-                uint32_t e;
-                if (rb) e = LUT_EMIT | (H_SIN + kk);
-                else if (xb) e = LUT_EMIT | LUT_PUSH | LUT_DCP | LUT_CSEL_B | LUT_UNV | (H_LX_SIN + kk);
-                else e = LUT_EMIT | LUT_DBL | LUT_DCP | (H_SIN + kk);
-                lut[kLutUnary + (kk << 2 | rb << 1 | xb)] = e;
-            }
-    const uint32_t hS[4] = { H_ADDS, H_RSUBS, H_MULS, H_RDIVS };            // j: ADD SUB MUL DIV
-    const uint32_t hX[4] = { H_ADDX, H_SUBX, H_MULX, H_DIVX | LUT_DIVV }, hRX[4] = { H_ADDX, H_RSUBX, H_MULX, H_RDIVX };
-    const uint32_t hC[4] = { H_ADDC, H_SUBC, H_MULC, H_MULC | LUT_DIVC }, hRC[4] = { H_ADDC, H_RSUBC, H_MULC, H_RDIVC };
-    const uint32_t hLXX[4] = { H_LX_ADDX, H_LX_SUBX, H_LX_MULX, H_LX_DIVX | LUT_DIVV };
-    const uint32_t hLXC[4] = { H_LX_ADDC, H_LX_SUBC, H_LX_MULC, H_LX_MULC | LUT_DIVC };
-    const uint32_t hLXRC[4] = { H_LX_ADDC, H_LX_RSUBC, H_LX_MULC, H_LX_RDIVC };
-    for (int j = 0; j < 4; ++j)
-        for (int ra = 0; ra < 2; ++ra) for (int rb = 0; rb < 2; ++rb)
-            for (int xa = 0; xa < 2; ++xa) for (int xb = 0; xb < 2; ++xb) {
-                uint32_t e;
-                if (ra && rb) e = LUT_EMIT | LUT_SLOT | LUT_DCM | hS[j];
-                else if (ra) e = LUT_EMIT | LUT_OSEL_B | (xb ? hX[j] : hC[j]);
-                else if (rb) e = LUT_EMIT | LUT_OSEL_A | (xa ? hRX[j] : hRC[j]);
-                else if (xa && xb) e = LUT_EMIT | LUT_PUSH | LUT_DCP | LUT_CSEL_A | LUT_OSEL_B | hLXX[j];
-                else if (xa) e = LUT_EMIT | LUT_PUSH | LUT_DCP | LUT_CSEL_A | LUT_OSEL_B | hLXC[j];
-                else if (xb) e = LUT_EMIT | LUT_PUSH | LUT_DCP | LUT_CSEL_B | LUT_OSEL_A | hLXRC[j];
-                else e = LUT_EMIT | LUT_DBL | LUT_DCP | LUT_FSEL_A | LUT_OSEL_B | hC[j];
-                lut[kLutBinary + (j << 4 | ra << 3 | rb << 2 | xa << 1 | xb)] = e;
-            }
-}
-
 // ---- a3/a5: the tree compiler ----------------------------------------------------------------------------
-// One lane per individual, in length-sorted order (the lanes of a warp run programs of equal length; k_scatter
-// left each lane's start record: index, length, token offset, record base). One walk over the postfix program
-// with an abstract stack whose entries are either a terminal that has not been evaluated yet (its value is
-// kept) or "computed": well-formedness
-// (D3) and the micro-ops of uop.cuh, in the program's own evaluation order.
-//   acc always holds the topmost computed entry; the computed entry with c others below it that is not
-//   in acc sits in slot c (tensor memory while c < S_T, local memory beyond).
+// in length-sorted order (k_scatter left each individual's start record: index, length, token offset, record base):
+// well-formedness (D3), maximum stack depth, and the micro-ops of uop.cuh in the program's own evaluation
+// order. acc always holds the topmost computed entry; the computed entry with c others below it that is not in acc
+// sits in slot c (tensor memory while c < S_T, local memory beyond).
 struct CompileParams {
     const uint32_t* genomes; const int4* sched;   // one start record per sorted position (k_scatter)
     const float* consts; long long n_consts; int d; int tmem_slots; int k_rcp; int k_un; int un_row_bytes;
@@ -375,212 +319,7 @@ struct CompileParams {
     float* fitness; float* outputs; int n_cases; int emit;
 };
 
-// A warp owns 32 consecutive individuals of the sorted order (equal or nearly equal lengths), one per lane.
-// Every lane walks its own program eight tokens at a time: the eight tokens, then the constants they name,
-// are fetched by two batches of independent loads (the 128-byte line a lane reads serves its next 32 tokens
-// from L1), and the walk itself is table-driven, the same straight-line code for every lane.
-constexpr int kCompBatch = 8;
-
-// The rest of Table 3 as the compiler sees it. The walk of k_compile knows the interpreter's eleven commands only
-// and calls anything else malformed, in straight-line code. A lane whose program failed that test walks it once more
-// here with the rules of the whole language (stack effect and depth of DUP SWAP DEL POW SIGN .. TANH, COPY @k /
-// PASTE @k in pairs): a program that passes is well-formed and goes to the blockwise kernel (slow list); the walk
-// costs about ten instructions per token and only the lanes that need it take it.
-// Returns the maximum stack depth, or 0 when the program is malformed.
-__device__ __noinline__ int check_full_language(const uint32_t* __restrict__ tok, int len, int d, long long n_consts)
-{
-    int sp = 0, mx = 0;
-    uint32_t vlive = 0;                            // COPY / PASTE variables that hold a value
-    for (int t = 0; t < len; ++t) {
-        const uint32_t w = __ldg(tok + t);
-        const uint32_t op = tok_op(w), arg = tok_arg(w);
-        int need, push;
-        bool argok = arg == 0;
-        if (op == OPC_CONST) { need = 0; push = 1; argok = (long long)arg < n_consts; }
-        else if (op == OPC_LOAD) { need = 0; push = 1; argok = (int)arg < d; }
-        else if ((op - OPC_ADD) < 4u || op == OPC_POW) { need = 2; push = -1; }
-        else if ((op - OPC_SIN) < 5u || (op - OPC_SIGN) <= (uint32_t)(OPC_TANH - OPC_SIGN)) { need = 1; push = 0; }
-        else if (op == OPC_DUP) { need = 1; push = 1; }
-        else if (op == OPC_SWAP) { need = 2; push = 0; }
-        else if (op == OPC_DEL) { need = 1; push = -1; }
-        else if (op == OPC_COPY || op == OPC_PASTE) {
-            const bool paste = op == OPC_PASTE;
-            need = paste ? 0 : 1; push = paste ? 1 : 0;
-            argok = arg < (uint32_t)BEAGLE_MAX_VARS && (((vlive >> (arg & 31u)) & 1u) != 0) == paste;
-            vlive ^= 1u << (arg & 31u);
-        }
-        else return 0;
-        if (!argok || sp < need || sp + push > BEAGLE_MAX_STACK) return 0;
-        sp += push; mx = max(mx, sp);
-    }
-    return (sp >= 1 && vlive == 0) ? mx : 0;       // a COPY left without its PASTE is malformed
-}
-
-__global__ void __launch_bounds__(kCompileThreads, 8) k_compile(const CompileParams q)
-{
-    __shared__ uint32_t lut[kLutSize];
-    // release the dependent launch (k_eval, run_eval): once every block of this grid has started, the interpreter's
-    // CTAs may take the SMs that fall idle and run their prologue; they wait for this grid's completion before
-    // they read its output
-    asm volatile("griddepcontrol.launch_dependents;");
-    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    if (threadIdx.x < kLutSize) lut[threadIdx.x] = g_compile_lut[threadIdx.x];
-    __syncthreads();
-    const int n_sorted = q.hdr->n_sorted;
-    const int i0 = (blockIdx.x * (kCompileThreads / 32) + warp) * 32;
-    if (i0 >= n_sorted) return;
-    const int i = i0 + lane;
-    const bool valid = i < n_sorted;
-    const int4 sc = valid ? q.sched[i] : make_int4(0, 0, 0, 0);     // k_scatter's start record: p, token offset, record base, length
-    const int len = sc.w & 0x3ff;                  // (p and the record base are read again after the walk: three registers
-                                                   // fewer to keep through it)
-    const long long toff = (long long)(((unsigned long long)((unsigned int)sc.w >> 10 & 0xffu) << 32) | (unsigned int)sc.y);
-    const int stride = uop_stride(len);
-    const long long ua = (long long)(((unsigned long long)((unsigned int)sc.w >> 18 & 0xffu) << 32) | (unsigned int)sc.z);
-    const bool fits = ua + stride <= q.ucap;
-    const bool wr = valid && q.emit && fits;
-    int maxlen = len;
-#pragma unroll
-    for (int m = 16; m >= 1; m >>= 1) maxlen = max(maxlen, __shfl_xor_sync(0xffffffffu, maxlen, m));
-
-    // The abstract stack. rmask / xmask are shift registers with the top of the stack at bit 0 (bit k: the
-    // entry k below the top is computed / is a variable, else a constant); t0 .. t3 are the values of the four
-    // topmost entries (a variable's column or a constant's bits), the deeper ones wait in stk[].
-    uint32_t stk[BEAGLE_MAX_STACK];
-    uint32_t rmask = 0, xmask = 0, t0 = 0, t1 = 0, t2 = 0, t3 = 0;
-    int sp = 0, mx = 0;
-    int c = 0;                                     // computed entries on the stack (the topmost one is acc)
-    bool ok = valid, slow = false;
-    const int S_T = q.tmem_slots;
-    // variables whose division is a multiplication by a staged reciprocal row
-    const uint32_t rcp_ok = ~q.hdr->rcp_unsafe & ((q.k_rcp >= 32) ? 0xFFFFFFFFu : ((1u << q.k_rcp) - 1u));
-    const uint32_t* gtok = q.genomes + toff;
-    uint2* po = q.uops + ua;                       // where the next record goes
-
-    auto load_batch = [&](int c0, uint32_t (&w)[kCompBatch]) {
-#pragma unroll
-        for (int u = 0; u < kCompBatch; ++u) w[u] = (c0 + u < len) ? __ldg(gtok + c0 + u) : 0u;
-    };
-    // a CONST token with a valid index is replaced by its constant; the mask (bit u) remembers which ones
-    auto resolve = [&](uint32_t (&w)[kCompBatch]) -> uint32_t {
-        uint32_t cm = 0;
-#pragma unroll
-        for (int u = 0; u < kCompBatch; ++u)
-            if (tok_op(w[u]) == OPC_CONST && (long long)tok_arg(w[u]) < q.n_consts) {
-                w[u] = __float_as_uint(__ldg(q.consts + tok_arg(w[u])));
-                cm |= 1u << u;
-            }
-        return cm;
-    };
-    // two batches ahead: tokens of batch i+2 and constants of batch i+1 are in flight while batch i is walked
-    uint32_t wA[kCompBatch], wB[kCompBatch], wC[kCompBatch];
-    load_batch(0, wA);
-    load_batch(kCompBatch, wB);
-    uint32_t cmA = resolve(wA), cmB = 0;
-
-    for (int c0 = 0; c0 < maxlen; c0 += kCompBatch) {
-        load_batch(c0 + 2 * kCompBatch, wC);
-        cmB = resolve(wB);
-        const int tend = len - c0;                 // this lane's tokens in the batch (may be <= 0 or > 8)
-#pragma unroll
-        for (int t = 0; t < kCompBatch; ++t) {
-            const bool live = ok && t < tend;
-            const uint32_t w = wA[t];
-            const bool isc = (cmA >> t) & 1u;
-            const uint32_t op = isc ? (uint32_t)OPC_CONST : tok_op(w), arg = tok_arg(w);
-            const bool isT = (op - OPC_CONST) < 2u, isB = (op - OPC_ADD) < 4u, isU = (op - OPC_SIN) < 5u;
-            const uint32_t key = isB ? (uint32_t)kLutBinary + ((op - OPC_ADD) << 4) + ((rmask & 3u) << 2 | (xmask & 3u))
-                               : isU ? (uint32_t)kLutUnary + ((op - OPC_SIN) << 2) + ((rmask & 1u) << 1 | (xmask & 1u)) : (uint32_t)kLutNone;
-            const uint32_t e = lut[key];
-            // well-formedness (D3); a CONST token that was not replaced has an index out of range
-            const bool good = isT ? ((isc || (op == OPC_LOAD && (int)arg < q.d)) && sp < BEAGLE_MAX_STACK)
-                                  : ((isB || isU) && arg == 0 && sp >= (isB ? 2 : 1));
-            ok = ok && (good || t >= tend);
-            const bool run = live && good;
-            // the record (operand a = second from the top = t1, operand b = top = t0)
-            const int s1 = c - 1;
-            const uint32_t pb = (c == 0 || !(e & (LUT_PUSH | LUT_DBL))) ? 0u
-                              : (s1 < S_T ? (uint32_t)H_PUSHT : (uint32_t)H_PUSHM + ((uint32_t)((s1 - S_T) * 64) << kPushShift));
-            uint32_t o = (e & LUT_OSEL_A) ? t1 : (e & LUT_OSEL_B) ? t0 : 0u;
-            const uint32_t colA = (e & LUT_CSEL_A) ? t1 : (e & LUT_CSEL_B) ? t0 : 0u;
-            uint32_t h = (e & 0xFFu) + (colA << kColAShift) + ((e & LUT_PUSH) ? pb : 0u);
-            if (e & LUT_SLOT) { const int s2 = c - 2; if (s2 >= S_T) { h += H_ADDM - H_ADDS; o = (uint32_t)((s2 - S_T) * 64); } }
-            if (e & LUT_UNV) {                     // f(X[j]) = the staged row (f, j): shared memory, else global
-                const int j = (int)(t0 / kCasesPerLane), f = (int)(op - OPC_SIN);
-                h = pb + (j < q.k_un ? (uint32_t)H_LS : (uint32_t)H_LG);
-                o = (uint32_t)((j < q.k_un ? f * q.k_un + j : f * q.d + j) * q.un_row_bytes);
-            }
-            if ((e & LUT_DIVV) && ((rcp_ok >> (o / kCasesPerLane)) & 1u))     // acc / X[o] = acc * (1/X)[o]
-                h += (e & LUT_PUSH) ? (uint32_t)(H_LX_MULR - H_LX_DIVX) : (uint32_t)(H_MULR - H_DIVX);
-            if (e & LUT_DIVC) {                    // x / c = x * rcp(c) with the division handler's own rcp; protected: 1
-                const float cf = __uint_as_float(o);
-                const bool tiny = fabsf(cf) < kEps;
-                o = tiny ? 0x3F800000u : __float_as_uint(mufu_rcp(cf));
-                h = tiny ? ((e & LUT_PUSH) ? pb : 0u) + (uint32_t)H_LC : h;
-            }
-            if (run && (e & LUT_DBL)) {            // rare: a constant has to become acc first
-                if (wr) *po = make_uint2(pb + H_LC, (e & LUT_FSEL_A) ? t1 : t0);
-                ++po;
-            }
-            const bool em = run && (e & LUT_EMIT);
-            if (wr && em) *po = make_uint2(h, o);
-            po += em ? 1 : 0;
-            // the abstract stack, without branches
-            const bool pushT = run && isT, popB = run && isB, unU = run && isU;
-            const uint32_t val = isc ? w : arg * (uint32_t)kCasesPerLane;
-            if (pushT) stk[sp & 31] = val;
-            const uint32_t deeper = stk[(sp - 5) & 31];        // wanted two pops from now at the earliest: its latency hides
-            const uint32_t n1 = pushT ? t0 : popB ? t2 : t1, n2 = pushT ? t1 : popB ? t3 : t2, n3 = pushT ? t2 : popB ? deeper : t3;
-            t0 = pushT ? val : t0; t1 = n1; t2 = n2; t3 = n3;
-            rmask = pushT ? rmask << 1 : popB ? (rmask >> 1) | 1u : unU ? rmask | 1u : rmask;
-            xmask = pushT ? (xmask << 1) | (isc ? 0u : 1u) : popB ? xmask >> 1 : xmask;
-            sp += pushT ? 1 : popB ? -1 : 0;
-            mx = max(mx, sp);
-            c += !run ? 0 : (e & LUT_DCP) ? 1 : (e & LUT_DCM) ? -1 : 0;
-        }
-#pragma unroll
-        for (int u = 0; u < kCompBatch; ++u) { wA[u] = wB[u]; wB[u] = wC[u]; }
-        cmA = cmB;
-    }
-    if (!valid) return;
-    const int4 sce = q.sched[i];
-    const int p = sce.x;
-    const long long ua_e = (long long)(((unsigned long long)((unsigned int)sce.w >> 18 & 0xffu) << 32) | (unsigned int)sce.z);
-    uint2* const po0 = q.uops + ua_e;
-    int n = (int)(po - po0);
-    ok &= (sp >= 1);
-    if (!ok) {                                     // not a program of the eleven commands: the whole language? (rare)
-        mx = check_full_language(gtok, len, q.d, q.n_consts);
-        ok = slow = mx > 0;
-    }
-    if (!ok) {
-        q.depth[p] = 0;
-        if (q.fitness) q.fitness[p] = __uint_as_float(0x7FC00000u);
-        if (q.outputs) for (int cc = 0; cc < q.n_cases; ++cc) q.outputs[(size_t)p * q.n_cases + cc] = __uint_as_float(0x7FC00000u);
-        q.meta[i] = make_int4(p, 0, 0, len);
-        atomicAdd(&q.hdr->n_malformed, 1);
-        return;
-    }
-    q.depth[p] = mx;
-    if (!q.emit) { q.meta[i] = make_int4(p, 0, 0, len); return; }
-    if (!fits || slow) {                           // the workspace promise of beagle_reserve was broken, or a command
-                                                   // beyond the interpreter's eleven: the blockwise kernel takes it
-        q.slow_list[atomicAdd(&q.hdr->n_slow, 1)] = p;
-        q.meta[i] = make_int4(p, 0, 0, len);
-        return;
-    }
-    uint2* out = po0;
-    if (!(rmask & 1u)) {                           // the result is a bare terminal
-        out[n] = (xmask & 1u) ? make_uint2((t0 << kColAShift) | H_LX, 0u) : make_uint2(H_LC, t0);
-        ++n;
-    }
-    // the END record carries what a7 needs (interp.cuh, variant 2): the stride to the next program of a group, the
-    // individual; the record after it the length as a float (for the tax)
-    out[n] = make_uint2(H_END | ((uint32_t)stride << 8), (uint32_t)p);
-    out[n + 1] = make_uint2(__float_as_uint((float)len), 0u);
-    out[n + 2] = make_uint2(H_END, 0u);
-    q.meta[i] = make_int4(p, (int)(ua_e >> 1), (n + 2 + 1) & ~1, len);
-}
+#include "compile_kernel.inc"
 
 // ---- the interpreter kernel -----------------------------------------------------------------------------
 #include "eval_kernel.inc"
@@ -724,7 +463,7 @@ static beagle_status init_once()
     CU(cudaFuncSetAttribute(k_eval<BEAGLE_FIT_MSE, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, w.smem_optin));
     CU(cudaFuncSetAttribute(k_eval<BEAGLE_FIT_CORRELATION, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, w.smem_optin));
     CU(cudaFuncSetAttribute(k_eval<BEAGLE_FIT_STD, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, w.smem_optin));
-    { uint32_t lut[kLutSize]; make_compile_lut(lut); CU(cudaMemcpyToSymbol(g_compile_lut, lut, sizeof(lut))); }
+    { uint32_t lut[kCtSize]; make_walk_lut(lut); CU(cudaMemcpyToSymbol(g_walk_lut, lut, sizeof(lut))); }
     CU(cudaMalloc(&w.bins, sizeof(int) * kNumBins));
     CU(cudaMalloc(&w.cursor, sizeof(int) * kNumBins));
     CU(cudaMemset(w.bins, 0, sizeof(int) * kNumBins));

@@ -59,6 +59,11 @@
     "mul.rn.f32 t" #k ", t" #k ", " BGI_LOG2E ";\n" \
     "ex2.approx.ftz.f32 " BGI_A #k ", t" #k ";\n"
 
+#define BGI_NEG(k)  "neg.f32 " BGI_A #k ", " BGI_A #k ";\n"
+#define BGI_SQRE(k) "mul.rn.f32 " BGI_A #k ", " BGI_A #k ", " BGI_A #k ";\n"
+#define BGI_CUBE(k) "mul.rn.f32 t" #k ", " BGI_A #k ", " BGI_A #k ";\n" "mul.rn.f32 " BGI_A #k ", t" #k ", " BGI_A #k ";\n"
+#define BGI_MOVX(k) "mov.f32 " BGI_A #k ", x" #k ";\n"
+
 // second operand in x<k> (a variable or a slot, loaded from tensor / local memory)
 #define BGI_ADDX(k)  "add.rn.f32 " BGI_A #k ", " BGI_A #k ", x" #k ";\n"
 #define BGI_SUBX(k)  "sub.rn.f32 " BGI_A #k ", " BGI_A #k ", x" #k ";\n"
@@ -127,6 +132,21 @@
 #define BGI_UNARY(OP, BODY) "L_" #OP "_%=:\n" BGI_NEXT BGI_K16(BODY) BGI_DISPATCH
 #define BGI_ENTRY_LX(OP)  BGI_PUSHES(LX_##OP) "L_LX_" #OP "_%=:\n" BGI_LXA BGI_WAITLD "bra.uni L_" #OP "_%=;\n"
 
+// GCL's stack commands on computed values (uop.cuh): POP (DEL) and SWAP of the slot on top, tensor or local memory
+#define BGI_STM(ADDR, R) \
+    "st.local.v4.f32 [" ADDR "], {" R "0, " R "1, " R "2, " R "3};\n" \
+    "st.local.v4.f32 [" ADDR "+16], {" R "4, " R "5, " R "6, " R "7};\n" \
+    "st.local.v4.f32 [" ADDR "+32], {" R "8, " R "9, " R "10, " R "11};\n" \
+    "st.local.v4.f32 [" ADDR "+48], {" R "12, " R "13, " R "14, " R "15};\n"
+#define BGI_STACKOPS \
+    "L_POPS_%=:\n" "sub.u32 spt, spt, 16;\n" BGI_LDTM(BGI_A, "spt") BGI_NEXT BGI_WAITLD BGI_DISPATCH \
+    "L_POPM_%=:\n" BGI_GETM BGI_NEXT BGI_K16(BGI_MOVX) BGI_DISPATCH \
+    "L_SWAPS_%=:\n" "sub.u32 xa, spt, 16;\n" BGI_LDTM("x", "xa") BGI_WAITLD \
+    "tcgen05.st.sync.aligned.32x32b.x16.b32 [xa], {" BGI_R16(BGI_A) "};\n" "tcgen05.wait::st.sync.aligned;\n" \
+    BGI_NEXT BGI_K16(BGI_MOVX) BGI_DISPATCH \
+    "L_SWAPM_%=:\n" BGI_GETM BGI_STM("ma", BGI_A) BGI_NEXT BGI_K16(BGI_MOVX) BGI_DISPATCH \
+    BGI_PUSHES(KEEP) "L_KEEP_%=:\n" BGI_NEXT BGI_DISPATCH
+
 #define BGI_HANDLERS \
     BGI_UNARY(SIN, BGI_SIN) BGI_UNARY(COS, BGI_COS) BGI_UNARY(LOG, BGI_LOG) BGI_UNARY(SQRT, BGI_SQRT) BGI_UNARY(EXP, BGI_EXP) \
     BGI_ENTRY_LX(SIN) BGI_ENTRY_LX(COS) BGI_ENTRY_LX(LOG) BGI_ENTRY_LX(SQRT) BGI_ENTRY_LX(EXP) \
@@ -149,7 +169,10 @@
     "ld.global.nc.v4.f32 {" BGI_A "0, " BGI_A "1, " BGI_A "2, " BGI_A "3}, [ma];\n" \
     "ld.global.nc.v4.f32 {" BGI_A "4, " BGI_A "5, " BGI_A "6, " BGI_A "7}, [ma+512];\n" \
     "ld.global.nc.v4.f32 {" BGI_A "8, " BGI_A "9, " BGI_A "10, " BGI_A "11}, [ma+1024];\n" \
-    "ld.global.nc.v4.f32 {" BGI_A "12, " BGI_A "13, " BGI_A "14, " BGI_A "15}, [ma+1536];\n" BGI_DISPATCH
+    "ld.global.nc.v4.f32 {" BGI_A "12, " BGI_A "13, " BGI_A "14, " BGI_A "15}, [ma+1536];\n" BGI_DISPATCH \
+    BGI_UNARY(NEG, BGI_NEG) BGI_UNARY(SQR, BGI_SQRE) BGI_UNARY(CUBE, BGI_CUBE) \
+    BGI_ENTRY_LX(NEG) BGI_ENTRY_LX(SQR) BGI_ENTRY_LX(CUBE) \
+    BGI_STACKOPS
 
 // ---- the dispatcher: the one indexed branch ----------------------------------------------------------------
 #define BGI_DISPATCHER \
@@ -161,17 +184,18 @@
 #define BGI_TP(L) "P_" #L "_%=, "
 #define BGI_TM(L) "M_" #L "_%=, "
 #define BGI_FRESH(T) \
-    T(LX) T(LC) T(LX_SIN) T(LX_COS) T(LX_LOG) T(LX_SQRT) T(LX_EXP) \
+    T(LX) T(LC) T(LX_SIN) T(LX_COS) T(LX_LOG) T(LX_SQRT) T(LX_EXP) T(LX_NEG) T(LX_SQR) T(LX_CUBE) \
     T(LX_ADDX) T(LX_SUBX) T(LX_MULX) T(LX_DIVX) \
-    T(LX_ADDC) T(LX_SUBC) T(LX_MULC) T(LX_RSUBC) T(LX_RDIVC) T(LX_MULR) T(LS) T(LG)
+    T(LX_ADDC) T(LX_SUBC) T(LX_MULC) T(LX_RSUBC) T(LX_RDIVC) T(LX_MULR) T(LS) T(LG) T(KEEP)
 #define BGI_TABLE \
     "TBL_%=: .branchtargets " \
-    BGI_T(END) BGI_T(SIN) BGI_T(COS) BGI_T(LOG) BGI_T(SQRT) BGI_T(EXP) \
+    BGI_T(END) BGI_T(SIN) BGI_T(COS) BGI_T(LOG) BGI_T(SQRT) BGI_T(EXP) BGI_T(NEG) BGI_T(SQR) BGI_T(CUBE) \
     BGI_T(ADDX) BGI_T(SUBX) BGI_T(MULX) BGI_T(DIVX) BGI_T(RSUBX) BGI_T(RDIVX) \
     BGI_T(ADDS) BGI_T(MULS) BGI_T(RSUBS) BGI_T(RDIVS) \
     BGI_T(ADDM) BGI_T(MULM) BGI_T(RSUBM) BGI_T(RDIVM) \
     BGI_T(ADDC) BGI_T(SUBC) BGI_T(MULC) BGI_T(RSUBC) BGI_T(RDIVC) \
-    BGI_FRESH(BGI_T) BGI_FRESH(BGI_TP) BGI_FRESH(BGI_TM) BGI_T(MULR) \
+    BGI_T(MULR) BGI_T(POPS) BGI_T(POPM) BGI_T(SWAPS) BGI_T(SWAPM) \
+    BGI_FRESH(BGI_T) BGI_FRESH(BGI_TP) BGI_FRESH(BGI_TM) \
     "L_END_%=;\n"
 
 // ---- variant 1: one program, one pass; the accumulator is the asm's output operands %0..%15 ------------------
@@ -287,7 +311,7 @@
 namespace beagle {
 
 static_assert(kMemSlots * 64 == 1984 && kCasesPerLane == 16, "interp.cuh is written for 16 cases per lane and 31 memory slots");
-static_assert(H_COUNT == 83, "BGI_TABLE lists the handlers in the order of uop.cuh's enum");
+static_assert(H_COUNT == 102 && H_KEEP == H_FRESH0 + H_NFRESH - 1, "BGI_TABLE lists the handlers in the order of uop.cuh's enum");
 
 // acc[k] = the program's output on case (pass * 512 + (k/4)*128 + lane*4 + k%4)
 #define BGI_A "%"

@@ -44,29 +44,33 @@ constexpr int kMemSlots = 31;              // a 32-entry stack pushes at most 31
 
 enum : uint32_t {
     H_END = 0,
-    // acc = f(acc)
-    H_SIN = 1, H_COS = 2, H_LOG = 3, H_SQRT = 4, H_EXP = 5,
+    // acc = f(acc)                                (NEG SQR CUBE: GCL's SIGN SQUARE CUBE)
+    H_SIN = 1, H_COS = 2, H_LOG = 3, H_SQRT = 4, H_EXP = 5, H_NEG = 6, H_SQR = 7, H_CUBE = 8,
     // acc = acc op X[o] | X[o] op acc            (x <- tensor memory, variable column)
-    H_ADDX = 6, H_SUBX = 7, H_MULX = 8, H_DIVX = 9, H_RSUBX = 10, H_RDIVX = 11,
+    H_ADDX = 9, H_SUBX = 10, H_MULX = 11, H_DIVX = 12, H_RSUBX = 13, H_RDIVX = 14,
     // acc = slot op acc                          (x <- tensor memory, slot column)
-    H_ADDS = 12, H_MULS = 13, H_RSUBS = 14, H_RDIVS = 15,
+    H_ADDS = 15, H_MULS = 16, H_RSUBS = 17, H_RDIVS = 18,
     // acc = slot op acc                          (x <- local memory)
-    H_ADDM = 16, H_MULM = 17, H_RSUBM = 18, H_RDIVM = 19,
+    H_ADDM = 19, H_MULM = 20, H_RSUBM = 21, H_RDIVM = 22,
     // acc = acc op c | c op acc
-    H_ADDC = 20, H_SUBC = 21, H_MULC = 22, H_RSUBC = 23, H_RDIVC = 24,
+    H_ADDC = 23, H_SUBC = 24, H_MULC = 25, H_RSUBC = 26, H_RDIVC = 27,
+    H_MULR = 28,                                // acc = acc * (1 / X)[o]
+    // GCL's stack commands on computed values: DEL of the top computed value, SWAP of the two topmost ones
+    H_POPS = 29, H_POPM = 30,                   // acc = slot (tensor memory: the top of the slot stack | local memory at byte offset o)
+    H_SWAPS = 31, H_SWAPM = 32,                 // acc <-> slot
     // fresh values: acc = X[colA] (then the command)
-    H_LX = 25, H_LC = 26,                                             // acc = X[colA] | acc = c
-    H_LX_SIN = 27, H_LX_COS = 28, H_LX_LOG = 29, H_LX_SQRT = 30, H_LX_EXP = 31,
-    H_LX_ADDX = 32, H_LX_SUBX = 33, H_LX_MULX = 34, H_LX_DIVX = 35,
-    H_LX_ADDC = 36, H_LX_SUBC = 37, H_LX_MULC = 38, H_LX_RSUBC = 39, H_LX_RDIVC = 40,
-    H_LX_MULR = 41,                             // acc = X[colA] * (1 / X)[o]: division by a variable whose reciprocal row is staged
-    H_LS = 42,                                  // acc = F[o]: a staged row of f(X[j]) in shared memory (f unary, loop-invariant)
-    H_LG = 43,                                  // acc = F[o]: the same row read from global memory (L2) when shared memory is full
-    H_FRESH0 = H_LX, H_NFRESH = 19,             // the fresh-value handlers H_LX .. H_LG
+    H_LX = 33, H_LC = 34,                                             // acc = X[colA] | acc = c
+    H_LX_SIN = 35, H_LX_COS = 36, H_LX_LOG = 37, H_LX_SQRT = 38, H_LX_EXP = 39, H_LX_NEG = 40, H_LX_SQR = 41, H_LX_CUBE = 42,
+    H_LX_ADDX = 43, H_LX_SUBX = 44, H_LX_MULX = 45, H_LX_DIVX = 46,
+    H_LX_ADDC = 47, H_LX_SUBC = 48, H_LX_MULC = 49, H_LX_RSUBC = 50, H_LX_RDIVC = 51,
+    H_LX_MULR = 52,                             // acc = X[colA] * (1 / X)[o]: division by a variable whose reciprocal row is staged
+    H_LS = 53,                                  // acc = F[o]: a staged row of f(X[j]) in shared memory (f unary, loop-invariant)
+    H_LG = 54,                                  // acc = F[o]: the same row read from global memory (L2) when shared memory is full
+    H_KEEP = 55,                                // acc = acc: with its push entry, DUP of a computed value (the copy goes to a slot)
+    H_FRESH0 = H_LX, H_NFRESH = 23,             // the fresh-value handlers H_LX .. H_KEEP
     H_PUSHT = H_NFRESH,                         // + handler: push acc to the tensor-memory slot stack first
     H_PUSHM = 2 * H_NFRESH,                     // + handler: push acc to the local slot at byte offset h[20:10] first
-    H_MULR = H_FRESH0 + 3 * H_NFRESH,           // acc = acc * (1 / X)[o]
-    H_COUNT = H_MULR + 1
+    H_COUNT = H_FRESH0 + 3 * H_NFRESH
 };
 
 constexpr int kPushShift = 10, kColAShift = 21;
