@@ -66,7 +66,8 @@ struct Header {                                // device-resident results of the
     long long uop_entries;                     // micro-op entries reserved by the bins
     int n_sorted;                              // individuals with an in-range length (= entries of perm[])
     int max_len;                               // longest in-range length (>= 1 if n_sorted > 0)
-    int n_slow;                                // individuals whose micro-ops did not fit the workspace
+    int n_slow;                                // individuals the blockwise kernel takes (POW, library functions, variables; or no room)
+    int n_general;                             // individuals k_compile's walk turned down (k_compile_general)
     int n_malformed;
     unsigned int queue;                        // work-queue cursor of the interpreter kernel
     unsigned int rcp_unsafe;                   // bit j: some case of variable j has |x| < 1e-6f (its division is protected)
@@ -217,7 +218,7 @@ __global__ void __launch_bounds__(1024) k_len_pass2(long long* __restrict__ bsum
         hdr->T = carry_s;
         hdr->n_sorted = (int)carry2_s;
         hdr->max_len = maxlen_s;
-        hdr->n_slow = 0; hdr->n_malformed = 0;
+        hdr->n_slow = 0; hdr->n_malformed = 0; hdr->n_general = 0;
         hdr->queue = 0;
         hdr->rcp_unsafe = unsafe_s;
     }
@@ -315,7 +316,7 @@ struct CompileParams {
     const uint32_t* genomes; const int4* sched;   // one start record per sorted position (k_scatter)
     const float* consts; long long n_consts; int d; int tmem_slots; int k_rcp; int k_un; int un_row_bytes;
     Header* hdr;
-    uint2* uops; long long ucap; int4* meta; int* depth; int* slow_list;
+    uint2* uops; long long ucap; int4* meta; int* depth; int* slow_list; int* gen_list;
     float* fitness; float* outputs; int n_cases; int emit;
 };
 
@@ -463,7 +464,7 @@ static beagle_status init_once()
     CU(cudaFuncSetAttribute(k_eval<BEAGLE_FIT_MSE, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, w.smem_optin));
     CU(cudaFuncSetAttribute(k_eval<BEAGLE_FIT_CORRELATION, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, w.smem_optin));
     CU(cudaFuncSetAttribute(k_eval<BEAGLE_FIT_STD, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, w.smem_optin));
-    { uint32_t lut[kCtSize]; make_walk_lut(lut); CU(cudaMemcpyToSymbol(g_walk_lut, lut, sizeof(lut))); }
+    { uint32_t lut[kLutSize]; make_compile_lut(lut); CU(cudaMemcpyToSymbol(g_compile_lut, lut, sizeof(lut))); }
     CU(cudaMalloc(&w.bins, sizeof(int) * kNumBins));
     CU(cudaMalloc(&w.cursor, sizeof(int) * kNumBins));
     CU(cudaMemset(w.bins, 0, sizeof(int) * kNumBins));
@@ -492,7 +493,7 @@ static beagle_status reserve_P(long long P)
     CU(cudaMalloc(&w.depth, sizeof(int) * P));
     CU(cudaMalloc(&w.sched, sizeof(int4) * P));
     CU(cudaMalloc(&w.meta, sizeof(int4) * P));
-    CU(cudaMalloc(&w.slow_list, sizeof(int) * P));
+    CU(cudaMalloc(&w.slow_list, sizeof(int) * 2 * P));       // + the list of k_compile_general
     CU(cudaMalloc(&w.bsum, sizeof(long long) * (nb + 1)));
     w.cap_P = P;
     return BEAGLE_OK;
@@ -614,9 +615,12 @@ static beagle_status run_prepass(const int32_t* genomes, const int32_t* lengths,
         const TmemPlan tp = tmem_plan(N, d);
         q.consts = consts; q.n_consts = n_consts; q.d = d; q.tmem_slots = tp.tmem_slots; q.k_rcp = tp.k_rcp; q.k_un = tp.k_un; q.un_row_bytes = npad * 4;
         q.hdr = w.hdr; q.uops = w.uops; q.ucap = w.cap_U; q.meta = w.meta; q.depth = w.depth;
-        q.slow_list = w.slow_list; q.fitness = fitness; q.outputs = outputs; q.n_cases = N; q.emit = emit ? 1 : 0;
+        q.slow_list = w.slow_list; q.gen_list = w.slow_list + w.cap_P; q.fitness = fitness; q.outputs = outputs; q.n_cases = N; q.emit = emit ? 1 : 0;
         k_compile<<<(unsigned)((P + kCompileThreads - 1) / kCompileThreads), kCompileThreads, 0, st>>>(q);
-        ++g_launches;
+        long long gb = (P + kCompileThreads - 1) / kCompileThreads;
+        const long long gcap = (long long)w.num_sms * 16;
+        k_compile_general<<<(unsigned)(gb > gcap ? gcap : gb), kCompileThreads, 0, st>>>(q);
+        g_launches += 2;
     }
     CU(cudaGetLastError());
     return BEAGLE_OK;
