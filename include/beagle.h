@@ -16,14 +16,22 @@
  *   - All pointers are borrowed for the duration of the enqueued work; the library never frees or
  *     keeps user memory. Scratch lives in a library-owned workspace (see beagle_reserve).
  *   - Calls enqueue work on `stream` (a cudaStream_t passed as void*, NULL = legacy default
- *     stream) and return without synchronising, unless the workspace has to grow (then one
- *     cudaMalloc happens first; call beagle_reserve to avoid it).
+ *     stream) and return without synchronising. Blocking: the host is blocked in exactly two
+ *     cases, both "the library-owned workspace has to grow": (a) P is larger than every earlier P
+ *     and than beagle_reserve's P_max (cudaDeviceSynchronize + cudaMalloc of the per-individual
+ *     arrays); (b) the micro-op workspace is not known to hold the call, i.e. it is smaller than
+ *     the worst case (516 records per individual) and no beagle_reserve(P_max, T_max) with
+ *     P <= P_max covers it: the token total is then read back (one cudaStreamSynchronize of
+ *     `stream`) and the workspace grown. After beagle_reserve(P_max, T_max), calls with P <= P_max
+ *     and at most T_max tokens only enqueue and can be captured in a CUDA graph. Inside a stream
+ *     capture a call that would have to block returns BEAGLE_ERR_NOT_RESERVED and enqueues nothing.
  *   - Argument errors are returned synchronously and nothing is enqueued.
  *   - Data-dependent problems are reported in band: a malformed individual gets the canonical
  *     quiet NaN 0x7FC00000 as its fitness and never causes an out-of-bounds access.
  *   - Lower fitness is better for beagle_eval (MSE); the score-type fitness functions of beagle_eval_fit are
  *     maximised. A non-finite fitness marks an invalid individual.
- *   - One call at a time per process (the workspace is shared); calls are not re-entrant.
+ *   - One call at a time per process, on one device (the workspace is shared and belongs to the device that was
+ *     current at the first call); calls are not re-entrant. The fitness function is an argument, never state.
  */
 #ifndef BEAGLE_H_
 #define BEAGLE_H_
@@ -48,9 +56,11 @@ extern "C" {
 #define BEAGLE_OP_LOG   0x09 /* a -> |a| < 1e-6f ? 0 : ln|a|    (protected) PAPER.md:253     */
 #define BEAGLE_OP_SQRT  0x0A /* a -> sqrt|a|                    (protected) PAPER.md:249     */
 #define BEAGLE_OP_EXP   0x0B /* a -> exp(a > 80 ? 80 : a)       (clamped)     */
-/* The rest of Table 3 in its own order from 0x10. Built: the stack commands and the exact unary ones. An
- * individual that uses one of them is evaluated by the blockwise kernel inside the same call (same definition,
- * same summation order, lower throughput); the interpreter's micro-ops cover the eleven commands above.         */
+/* The rest of Table 3 in its own order from 0x10. DUP SWAP DEL SIGN SQUARE CUBE are compiled to
+ * micro-ops and run on the interpreter like the eleven commands above (the stack commands are resolved at compile
+ * time on terminals and cost a slot move on computed values). An individual that uses POW, one of the six library
+ * functions or COPY / PASTE is evaluated by the blockwise kernel inside the same call (same definition, same
+ * summation order, bit-identical where both apply, lower throughput).                                           */
 #define BEAGLE_OP_DUP    0x10 /* a -> a a     */
 #define BEAGLE_OP_SWAP   0x11 /* a b -> b a     */
 #define BEAGLE_OP_DEL    0x12 /* a ->     */
@@ -84,7 +94,9 @@ enum {
     BEAGLE_ERR_INVALID_ARG = -1, /* null pointer with P > 0, size out of range                   */
     BEAGLE_ERR_UNSUPPORTED = -2, /* device is not sm_100, or not enough shared memory            */
     BEAGLE_ERR_CUDA = -3,        /* a CUDA call failed; see beagle_last_cuda_error               */
-    BEAGLE_ERR_NOMEM = -4        /* workspace or staging allocation failed                       */
+    BEAGLE_ERR_NOMEM = -4,       /* workspace or staging allocation failed                       */
+    BEAGLE_ERR_NOT_RESERVED = -5 /* the call would have to block (grow its workspace) inside a
+                                    stream capture; nothing was enqueued: beagle_reserve first    */
 };
 
 /* beagle_eval — score a device-resident colony.
@@ -111,10 +123,10 @@ enum {
  *
  * Device resources: the interpreter kernel takes all 512 tensor-memory columns and up to 227 KB of shared
  * memory of every SM for the duration of the call (one CTA per SM). When the fitness cases do not fit tensor
- * memory (d > 32 at N <= 512, d > 16 at N > 512) the call runs the blockwise kernel instead: same result bit for
- * bit, lower throughput.
+ * memory (d > 16 at N > 512; d <= 32 always fits at N <= 512) the call runs the blockwise kernel instead: same
+ * result bit for bit, lower throughput.
  *
- * Malformed (fitness = quiet NaN 0x7FC00000): length outside [1,512], unknown opcode, non-zero
+ * Malformed (fitness = quiet NaN 0x7FC00000): length outside [1,512], an opcode outside the table above, non-zero
  * arg on an operator, CONST arg >= n_consts, LOAD arg >= d, a command that needs more entries than the
  * stack holds, depth above 32, an empty stack at the end (DEL can empty it in between).
  * The extent of `genomes` is trusted to be sum of the in-range lengths.                          */
@@ -158,16 +170,17 @@ beagle_status beagle_eval_fit(const int32_t* genomes, const int32_t* lengths, in
  * the device budget ("manages populations in batches to ensure the GPU memory is
  * never exceeded"; R19). The colony is cut at individual boundaries into chunks of at
  * most device_budget_bytes/K bytes of tokens+lengths, K = device_budget_bytes / 32 MiB clamped to 2..8 staging
- * buffers; the chunks after chunk c are copied host-to-device on an internal copy stream while chunk c is
- * evaluated on `stream`.
+ * buffers (beagle_set_chunk_target changes the 32 MiB); chunk c goes to buffer c mod K, and the chunks after chunk c
+ * are copied host-to-device on an internal copy stream while chunk c is evaluated on `stream`.
  * fitness_out is bit-identical to beagle_eval on the whole colony, for any budget.
  *
  *   h_genomes, h_lengths, h_consts   HOST (pinned memory for overlap; pageable memory works but
  *                                    the copies then do not overlap)
  *   X, y, fitness_out                DEVICE, as in beagle_eval
- *   device_budget_bytes              cap on device bytes used for genome staging (both buffers);
- *                                    must hold two maximum-length individuals:
- *                                    >= 2 * 4 * (BEAGLE_MAX_LEN + 1)
+ *   device_budget_bytes              cap on device bytes used for genome staging (all K buffers together);
+ *                                    every buffer must hold one maximum-length individual: at least
+ *                                    2 * 4 * (BEAGLE_MAX_LEN + 64) = 4608 bytes, else BEAGLE_ERR_INVALID_ARG
+ * The first call with a new budget allocates the staging buffers (blocking; beagle_reserve_chunked does it ahead).
  * Completion of `stream` implies completion of everything, copies included. The host arrays must
  * stay valid and unchanged until then.                                                           */
 beagle_status beagle_eval_chunked(const int32_t* h_genomes, const int32_t* h_lengths, int64_t P,
@@ -207,8 +220,9 @@ beagle_status beagle_rank(const float* fitness, int64_t P, const int64_t* sample
 /* beagle_eval_blockwise — prior art kept as a measured baseline, not the product: the paper's own
  * mapping (one CUDA block per individual, one thread per fitness case, a 32-entry
  * per-thread stack in local memory, block aggregation in shared memory), same arguments and the
- * same definition of the result as beagle_eval. Its summation order differs, so results agree
- * with beagle_eval to rounding, not bitwise.                                                     */
+ * same definition of the result as beagle_eval, the same per-command functions and the same
+ * summation order: its results are bit-identical to beagle_eval's (tests/test_gpu_edges.py). It
+ * is also the kernel that takes, inside beagle_eval, the individuals the interpreter cannot.    */
 beagle_status beagle_eval_blockwise(const int32_t* genomes, const int32_t* lengths, int64_t P,
                                     const float* consts, int64_t n_consts,
                                     const float* X, const float* y, int32_t N, int32_t d,
@@ -224,10 +238,17 @@ beagle_status beagle_debug_outputs(const int32_t* genomes, const int32_t* length
 /* beagle_debug_schedule — test only: copies what the scheduling pre-pass (offsets, per-program
  * scan, length-sorted permutation) produced for the last beagle_eval/debug call on `stream`.
  * Any pointer may be NULL. DEVICE outputs: off[P] (int64 exclusive prefix sum), depth[P] (int32
- * maximum stack depth, 0 if malformed), perm[P] (int32, the evaluation order: individuals grouped
- * by depth class, longest first). Enqueued on `stream`.                                          */
+ * maximum stack depth, 0 if malformed), perm[P] (int32, the evaluation order: the individuals with a
+ * length in [1, 512] sorted by length, longest first, then -1 for the others). Enqueued on `stream`. */
 beagle_status beagle_debug_schedule(int64_t P, int64_t* off, int32_t* depth, int32_t* perm,
                                     void* stream);
+
+/* beagle_debug_counts — test only: what the pre-pass of the last beagle_eval / debug call on `stream` (for a chunked
+ * call: of its last chunk) counted. HOST outputs, any may be NULL; synchronises `stream`. n_sorted: individuals with a
+ * length in [1, 512]; n_general: of those, the ones that are not trees of the eleven hot-path commands (compiled by
+ * k_compile_general); n_slow: individuals handed to the blockwise kernel (POW, library functions, COPY / PASTE, or no
+ * room in the workspace); n_malformed: in-range individuals that are not programs (D3).               */
+beagle_status beagle_debug_counts(int32_t* n_sorted, int32_t* n_general, int32_t* n_slow, int32_t* n_malformed, void* stream);
 
 /* Limits compiled into the library (any pointer may be NULL). */
 void beagle_limits(int32_t* max_len, int32_t* max_stack, int32_t* max_n, int32_t* max_d);
@@ -239,7 +260,9 @@ const char* beagle_status_string(beagle_status s);
 int32_t beagle_last_cuda_error(void);
 
 /* Pre-size the workspace for colonies of up to P_max individuals and T_max tokens so that later
- * calls are allocation-free. Synchronises the device if it has to reallocate. */
+ * calls with P <= P_max and at most T_max tokens never block (see "Blocking" above). T_max = 0 sizes the
+ * per-individual arrays only. Synchronises the device if it has to reallocate. Individuals of a call that breaks
+ * the promise (more tokens than T_max) and do not fit are evaluated by the blockwise kernel: same results. */
 beagle_status beagle_reserve(int64_t P_max, int64_t T_max);
 
 /* Pre-size the staging buffers of beagle_eval_chunked for this budget. */
@@ -250,6 +273,11 @@ void beagle_release(void);
 
 /* Number of kernels the most recent beagle_eval* call launched (for bench.py's gpu_launches). */
 int32_t beagle_last_launch_count(void);
+
+/* Size the staging buffers of beagle_eval_chunked aim at (default 32 MiB; bytes <= 0 restores it): the budget is
+ * cut into K = budget / target buffers, 2 <= K <= 8. beagle_chunk_buffers returns the K in use (0: none yet). */
+void    beagle_set_chunk_target(int64_t bytes);
+int32_t beagle_chunk_buffers(void);
 
 /* Profiling hooks for bench.py's roofline line. While profiling is on (on = n > 0), every n-th beagle_eval
  * call, starting with the first, brackets its evaluation kernels (the interpreter launches, without the scheduling

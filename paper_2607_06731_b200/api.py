@@ -17,6 +17,7 @@ ERR_INVALID_ARG = -1
 ERR_UNSUPPORTED = -2
 ERR_CUDA = -3
 ERR_NOMEM = -4
+ERR_NOT_RESERVED = -5
 
 
 class BeagleError(RuntimeError):
@@ -39,6 +40,7 @@ _SIGNATURES = {
     "beagle_eval_blockwise": (_i32, [_vp, _vp, _i64, _vp, _i64, _vp, _vp, _i32, _i32, _f32, _vp, _vp]),
     "beagle_debug_outputs": (_i32, [_vp, _vp, _i64, _vp, _i64, _vp, _i32, _i32, _vp, _vp]),
     "beagle_debug_schedule": (_i32, [_i64, _vp, _vp, _vp, _vp]),
+    "beagle_debug_counts": (_i32, [ctypes.POINTER(_i32)] * 4 + [_vp]),
     "beagle_limits": (None, [ctypes.POINTER(_i32)] * 4),
     "beagle_status_string": (ctypes.c_char_p, [_i32]),
     "beagle_last_cuda_error": (_i32, []),
@@ -46,6 +48,8 @@ _SIGNATURES = {
     "beagle_reserve_chunked": (_i32, [_i64]),
     "beagle_release": (None, []),
     "beagle_last_launch_count": (_i32, []),
+    "beagle_set_chunk_target": (None, [_i64]),
+    "beagle_chunk_buffers": (_i32, []),
     "beagle_set_profiling": (None, [_i32]),
     "beagle_profiled_eval_kernel_ms": (_f32, [ctypes.POINTER(_i32)]),
 }
@@ -143,6 +147,12 @@ def beagle_debug_schedule(P, off, depth, perm, stream=0):
            "beagle_debug_schedule")
 
 
+def beagle_debug_counts(stream=0):
+    v = [_i32() for _ in range(4)]
+    _check(lib().beagle_debug_counts(*[ctypes.byref(x) for x in v], int(stream) or None), "beagle_debug_counts")
+    return dict(n_sorted=v[0].value, n_general=v[1].value, n_slow=v[2].value, n_malformed=v[3].value)
+
+
 def beagle_limits():
     v = [_i32() for _ in range(4)]
     lib().beagle_limits(*[ctypes.byref(x) for x in v])
@@ -171,6 +181,14 @@ def beagle_release():
 
 def beagle_last_launch_count() -> int:
     return lib().beagle_last_launch_count()
+
+
+def beagle_set_chunk_target(nbytes):
+    lib().beagle_set_chunk_target(int(nbytes))
+
+
+def beagle_chunk_buffers() -> int:
+    return lib().beagle_chunk_buffers()
 
 
 def beagle_set_profiling(on):

@@ -55,7 +55,8 @@ constexpr int kGroupStages = BEAGLE_GROUP_STAGES;   // stages per ring when the 
 #endif
 constexpr int kEvalThreads = BEAGLE_EVAL_THREADS;   // 32 warps (8 per scheduler): 64 registers per thread
 constexpr int kStageBufsMax = 8;               // beagle_eval_chunked: staging buffers the device budget is cut into
-constexpr long long kStageTarget = 32ll << 20;  // ... of about this size each (at least two)
+constexpr long long kStageTarget = 32ll << 20;  // ... of about this size each (at least two); beagle_set_chunk_target overrides it
+static long long g_stage_target = kStageTarget;
 constexpr int kProfMax = 256;                  // beagle_set_profiling: recorded calls
 constexpr int kEvalMetaBytes = 64 * 16;           // per-warp window of the work queue (64 x int4)
 constexpr int kCasePad = 512;                  // staged cases are padded to a multiple of 32*K
@@ -436,7 +437,7 @@ struct Workspace {
     float* stage_consts = nullptr; long long stage_consts_cap = 0;
     cudaStream_t copy_stream = nullptr; cudaEvent_t ev_copied[kStageBufsMax] = {}, ev_free[kStageBufsMax] = {};
     cudaEvent_t ev_k[2 * kProfMax] = {}; int prof_n = 0;
-    int num_sms = 0; int smem_optin = 0; bool device_ok = false; bool inited = false;
+    int num_sms = 0; int smem_optin = 0; bool device_ok = false; bool inited = false; bool need_T_readback = false;
 };
 static Workspace g_ws;
 static int32_t g_last_cuda = 0;
@@ -444,7 +445,7 @@ static int32_t g_launches = 0;
 static int32_t g_profiling = 0;     // 0: off; n > 0: every n-th call is bracketed by events
 static int32_t g_prof_calls = 0;
 struct FitSel { int kind; float M; int power; };
-static FitSel g_fit = { BEAGLE_FIT_MSE, 0.f, 1 };   // set by the entry point for the duration of its call
+static const FitSel kFitMse = { BEAGLE_FIT_MSE, 0.f, 1 };   // the fitness function is an argument all the way down, never state
 
 #define CU(call) do { cudaError_t e_ = (call); if (e_ != cudaSuccess) { g_last_cuda = (int32_t)e_; \
     return (e_ == cudaErrorMemoryAllocation) ? BEAGLE_ERR_NOMEM : BEAGLE_ERR_CUDA; } } while (0)
@@ -458,8 +459,7 @@ static beagle_status init_once()
     w.num_sms = prop.multiProcessorCount;
     w.smem_optin = (int)prop.sharedMemPerBlockOptin;
     w.device_ok = (prop.major == 10);
-    w.inited = true;
-    if (!w.device_ok) return BEAGLE_ERR_UNSUPPORTED;
+    if (!w.device_ok) { w.inited = true; return BEAGLE_ERR_UNSUPPORTED; }
     CU(cudaFuncSetAttribute(k_eval<BEAGLE_FIT_MSE, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, w.smem_optin));
     CU(cudaFuncSetAttribute(k_eval<BEAGLE_FIT_MSE, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, w.smem_optin));
     CU(cudaFuncSetAttribute(k_eval<BEAGLE_FIT_CORRELATION, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, w.smem_optin));
@@ -476,6 +476,7 @@ static beagle_status init_once()
     CU(cudaMalloc(&w.hdr, sizeof(Header)));
     CU(cudaMemset(w.hdr, 0, sizeof(Header)));
     CU(cudaMallocHost(&w.h_T, sizeof(long long)));
+    w.inited = true;                               // only now: a failed allocation above is tried again by the next call
     return BEAGLE_OK;
 }
 
@@ -486,8 +487,9 @@ static beagle_status reserve_P(long long P)
     CU(cudaDeviceSynchronize());
     cudaFree(w.off); cudaFree(w.depth); cudaFree(w.meta); cudaFree(w.sched);
     cudaFree(w.slow_list); cudaFree(w.bsum);
-    w.off = nullptr; w.depth = nullptr; w.meta = nullptr;
+    w.off = nullptr; w.depth = nullptr; w.meta = nullptr; w.sched = nullptr;
     w.slow_list = nullptr; w.bsum = nullptr; w.cap_P = 0;
+    (void)cudaGetLastError();                      // the frees are best effort: their status is not the call's
     const long long nb = (P + kScanBlock - 1) / kScanBlock;
     CU(cudaMalloc(&w.off, sizeof(long long) * (P + 1)));
     CU(cudaMalloc(&w.depth, sizeof(int) * P));
@@ -504,7 +506,10 @@ static beagle_status reserve_U(long long U)
     Workspace& w = g_ws;
     if (U <= w.cap_U) return BEAGLE_OK;
     CU(cudaDeviceSynchronize());
+    // meta[] and the TMA source address carry the record base in 16-byte units as 32 bits: 2^33 records (64 GiB)
+    if (U > (1ll << 33)) return BEAGLE_ERR_UNSUPPORTED;
     cudaFree(w.uops); w.uops = nullptr; w.cap_U = 0;
+    (void)cudaGetLastError();
     CU(cudaMalloc(&w.uops, sizeof(uint2) * U));
     w.cap_U = U;
     return BEAGLE_OK;
@@ -519,7 +524,7 @@ static long long uop_entries_bound(long long P, long long T) { return T + 4 * P 
 // possible. fast == false: the variable block alone does not fit (d > 32 at N <= 512, d > 16 beyond), and the
 // call takes the blockwise kernel.
 struct TmemPlan { bool fast; int threads; int rcp_col0; int k_rcp; int slot_col0; int tmem_slots; int k_un; int ring_bytes; size_t smem; int off_ys, off_meta, off_un, off_ring; };
-static TmemPlan tmem_plan(int N, int d)
+static TmemPlan tmem_plan(int N, int d, int fit_kind)
 {
     TmemPlan t = { false, kEvalThreads, 0, 0, 0, 0, 0, 0, 0 };
     const int passes = (N + kCasesPerPass - 1) / kCasesPerPass;
@@ -554,7 +559,7 @@ static TmemPlan tmem_plan(int N, int d)
     // every warp keeps room for at least one stage of the longest program
     const int warps = t.threads / 32;
     const int npad = (N + kCasePad - 1) / kCasePad * kCasePad;
-    const long long fixed = ((64 + warps * kStagesMax * 8 + 127) & ~127) + (long long)npad * 4 * (g_fit.kind == BEAGLE_FIT_CORRELATION ? 2 : 1)
+    const long long fixed = ((64 + warps * kStagesMax * 8 + 127) & ~127) + (long long)npad * 4 * (fit_kind == BEAGLE_FIT_CORRELATION ? 2 : 1)
                             + (long long)kEvalMetaBytes * warps;      // correlation: y and the centred y (eval_kernel.inc)
     const long long spare = (long long)g_ws.smem_optin - fixed - (long long)warps * ((kStageBytesMax + 127) & ~127);
     long long ku = spare / (5ll * npad * 4);
@@ -582,11 +587,44 @@ static beagle_status check_args(const void* genomes, const void* lengths, int64_
     return BEAGLE_OK;
 }
 
+// The only places where a call may block the host (include/beagle.h "Blocking"): the per-individual arrays grow when P
+// exceeds what was ever reserved or used; the micro-op workspace grows when it is not known to hold the call. T_known < 0:
+// the token count is not known on the host; the workspace is known to be enough when it holds the worst case, or when
+// beagle_reserve promised a bound for colonies of this size; otherwise the token total is read back once, after the
+// length scan of run_prepass (one cudaStreamSynchronize). Inside a stream capture nothing of this can be done: the call returns
+// BEAGLE_ERR_NOT_RESERVED and enqueues nothing.
+static bool is_capturing(cudaStream_t st)
+{
+    cudaStreamCaptureStatus cs = cudaStreamCaptureStatusNone;
+    if (cudaStreamIsCapturing(st, &cs) != cudaSuccess) { (void)cudaGetLastError(); return false; }
+    return cs != cudaStreamCaptureStatusNone;
+}
+
+static beagle_status ready_or_grow(long long P, long long T_known, bool emit, cudaStream_t st)
+{
+    Workspace& w = g_ws;
+    const bool cap = is_capturing(st);
+    if (P > w.cap_P) {
+        if (cap) return BEAGLE_ERR_NOT_RESERVED;
+        beagle_status s = reserve_P(P); if (s != BEAGLE_OK) return s;
+    }
+    if (!emit) return BEAGLE_OK;
+    long long need = 0;
+    if (T_known >= 0) need = uop_entries_bound(P, T_known);
+    else if (w.cap_U >= (long long)uop_stride(BEAGLE_MAX_LEN) * P) need = 0;           // worst case fits
+    else if (P <= w.promised_P && w.promised_T > 0) need = 0;                           // promised by beagle_reserve
+    else need = -1;
+    if (need == 0 || (need > 0 && need <= w.cap_U)) return BEAGLE_OK;
+    if (cap) return BEAGLE_ERR_NOT_RESERVED;
+    if (need < 0) { w.need_T_readback = true; return BEAGLE_OK; }                      // run_prepass reads it after its scan
+    return reserve_U(need);
+}
+
 // a2 + a3 + the compile step of a5 (+ the transpose of a4). T_known < 0: the token count is not known
 // on the host; unless beagle_reserve promised a bound, it is read back once (one stream synchronisation).
 static beagle_status run_prepass(const int32_t* genomes, const int32_t* lengths, long long P, const float* consts,
                                  long long n_consts, const float* X, const float* y, int N, int d, float* fitness,
-                                 float* outputs, long long T_known, bool emit, cudaStream_t st)
+                                 float* outputs, long long T_known, bool emit, const FitSel& fit, cudaStream_t st)
 {
     Workspace& w = g_ws;
     const int nb = (int)((P + kScanBlock - 1) / kScanBlock);
@@ -594,16 +632,11 @@ static beagle_status run_prepass(const int32_t* genomes, const int32_t* lengths,
     k_len_pass1<<<nb, kScanThreads, 0, st>>>(lengths, P, w.bsum, w.bins);
     k_len_pass2<<<1, 1024, 0, st>>>(w.bsum, nb, w.hdr, w.bins, w.cursor, w.binstart, w.binubase, X, y, N, d, npad, w.xt, w.ung);
     g_launches += 2;
-    if (emit) {
-        long long need = -1;
-        if (T_known >= 0) need = uop_entries_bound(P, T_known);
-        else if (w.cap_U >= (long long)uop_stride(BEAGLE_MAX_LEN) * P) need = 0;            // worst case fits
-        else if (P <= w.promised_P && w.promised_T > 0) need = 0;                           // promised by beagle_reserve
-        else {
-            CU(cudaMemcpyAsync(w.h_T, &w.hdr->T, sizeof(long long), cudaMemcpyDeviceToHost, st));
-            CU(cudaStreamSynchronize(st));
-            need = uop_entries_bound(P, *w.h_T);
-        }
+    if (emit && w.need_T_readback) {               // ready_or_grow: the one read-back of an un-reserved call
+        w.need_T_readback = false;
+        CU(cudaMemcpyAsync(w.h_T, &w.hdr->T, sizeof(long long), cudaMemcpyDeviceToHost, st));
+        CU(cudaStreamSynchronize(st));
+        const long long need = uop_entries_bound(P, *w.h_T);
         if (need > w.cap_U) { beagle_status s = reserve_U(need); if (s != BEAGLE_OK) return s; }
     }
     k_scatter<<<nb, kScanThreads, 0, st>>>(lengths, P, w.bsum, w.binstart, w.cursor, w.off, w.depth,
@@ -612,7 +645,7 @@ static beagle_status run_prepass(const int32_t* genomes, const int32_t* lengths,
     {
         CompileParams q;
         q.genomes = reinterpret_cast<const uint32_t*>(genomes); q.sched = w.sched;
-        const TmemPlan tp = tmem_plan(N, d);
+        const TmemPlan tp = tmem_plan(N, d, fit.kind);
         q.consts = consts; q.n_consts = n_consts; q.d = d; q.tmem_slots = tp.tmem_slots; q.k_rcp = tp.k_rcp; q.k_un = tp.k_un; q.un_row_bytes = npad * 4;
         q.hdr = w.hdr; q.uops = w.uops; q.ucap = w.cap_U; q.meta = w.meta; q.depth = w.depth;
         q.slow_list = w.slow_list; q.gen_list = w.slow_list + w.cap_P; q.fitness = fitness; q.outputs = outputs; q.n_cases = N; q.emit = emit ? 1 : 0;
@@ -628,16 +661,16 @@ static beagle_status run_prepass(const int32_t* genomes, const int32_t* lengths,
 
 static beagle_status run_eval(const int32_t* genomes, const int32_t* lengths, const float* consts, const float* X,
                               const float* y, long long P, int N, int d, float tax, float* fitness, float* outputs,
-                              cudaStream_t st)
+                              const FitSel& fit, cudaStream_t st)
 {
     Workspace& w = g_ws;
     const int npad = (N + kCasePad - 1) / kCasePad * kCasePad;
     EvalParams prm;
-    const TmemPlan tp = tmem_plan(N, d);
+    const TmemPlan tp = tmem_plan(N, d, fit.kind);
     if (!tp.fast) return BEAGLE_ERR_UNSUPPORTED;   // callers check first
     prm.rcp_col0 = tp.rcp_col0; prm.k_rcp = tp.k_rcp; prm.slot_col0 = tp.slot_col0; prm.tmem_slots = tp.tmem_slots;
     prm.meta = w.meta; prm.uops = w.uops; prm.hdr = w.hdr; prm.xt = w.xt; prm.ung = w.ung;
-    prm.fitness = fitness; prm.outputs = outputs; prm.tax = tax; prm.M = g_fit.M; prm.power = g_fit.power; prm.n = N; prm.npad = npad; prm.d = d;
+    prm.fitness = fitness; prm.outputs = outputs; prm.tax = tax; prm.M = fit.M; prm.power = fit.power; prm.n = N; prm.npad = npad; prm.d = d;
     const bool prof = g_profiling && w.prof_n < kProfMax && (g_prof_calls++ % g_profiling) == 0;
     if (prof) {
         for (int i = 0; i < 2; ++i)
@@ -658,15 +691,15 @@ static beagle_status run_eval(const int32_t* genomes, const int32_t* lengths, co
     attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
     attr[0].val.programmaticStreamSerializationAllowed = 1;
     cfg.attrs = attr; cfg.numAttrs = 1;
-    if (g_fit.kind == BEAGLE_FIT_CORRELATION) CU(cudaLaunchKernelEx(&cfg, k_eval<BEAGLE_FIT_CORRELATION, false>, prm));
-    else if (g_fit.kind == BEAGLE_FIT_STD) CU(cudaLaunchKernelEx(&cfg, k_eval<BEAGLE_FIT_STD, false>, prm));
+    if (fit.kind == BEAGLE_FIT_CORRELATION) CU(cudaLaunchKernelEx(&cfg, k_eval<BEAGLE_FIT_CORRELATION, false>, prm));
+    else if (fit.kind == BEAGLE_FIT_STD) CU(cudaLaunchKernelEx(&cfg, k_eval<BEAGLE_FIT_STD, false>, prm));
     else if (outputs || !fitness) CU(cudaLaunchKernelEx(&cfg, k_eval<BEAGLE_FIT_MSE, false>, prm));
     else CU(cudaLaunchKernelEx(&cfg, k_eval<BEAGLE_FIT_MSE, true>, prm));
     ++g_launches;
     if (prof) { CU(cudaEventRecord(w.ev_k[2 * w.prof_n + 1], st)); ++w.prof_n; }
     // slow path: individuals whose micro-ops did not fit the promised workspace (normally none)
     k_eval_blockwise<<<w.num_sms * 2, (N + 31) / 32 * 32, 0, st>>>(genomes, w.off, lengths, w.depth, consts, X, y, N, d, tax,
-                                                                   fitness, outputs, w.slow_list, &w.hdr->n_slow, P, g_fit.kind, g_fit.M, g_fit.power);
+                                                                   fitness, outputs, w.slow_list, &w.hdr->n_slow, P, fit.kind, fit.M, fit.power);
     ++g_launches;
     CU(cudaGetLastError());
     return BEAGLE_OK;
@@ -677,15 +710,15 @@ static beagle_status run_eval(const int32_t* genomes, const int32_t* lengths, co
 // whose results are bit-identical (same per-command functions, same summation order).
 static beagle_status run_colony(const int32_t* genomes, const int32_t* lengths, long long P, const float* consts,
                                 long long n_consts, const float* X, const float* y, int N, int d, float tax,
-                                float* fitness, float* outputs, long long T_known, cudaStream_t st)
+                                float* fitness, float* outputs, long long T_known, const FitSel& fit, cudaStream_t st)
 {
     Workspace& w = g_ws;
-    const bool fast = tmem_plan(N, d).fast;
-    beagle_status s = run_prepass(genomes, lengths, P, consts, n_consts, X, y, N, d, fitness, outputs, T_known, fast, st);
+    const bool fast = tmem_plan(N, d, fit.kind).fast;
+    beagle_status s = run_prepass(genomes, lengths, P, consts, n_consts, X, y, N, d, fitness, outputs, T_known, fast, fit, st);
     if (s != BEAGLE_OK) return s;
-    if (fast) return run_eval(genomes, lengths, consts, X, y, P, N, d, tax, fitness, outputs, st);
+    if (fast) return run_eval(genomes, lengths, consts, X, y, P, N, d, tax, fitness, outputs, fit, st);
     k_eval_blockwise<<<(unsigned)P, (N + 31) / 32 * 32, 0, st>>>(genomes, w.off, lengths, w.depth, consts, X, y, N, d, tax,
-                                                                fitness, outputs, nullptr, nullptr, P, g_fit.kind, g_fit.M, g_fit.power);
+                                                                fitness, outputs, nullptr, nullptr, P, fit.kind, fit.M, fit.power);
     ++g_launches;
     CU(cudaGetLastError());
     return BEAGLE_OK;
@@ -709,20 +742,30 @@ static bool decode_fit(int32_t fit, int* kind, int* power)
     }
 }
 
-extern "C" {
+static beagle_status eval_chunked_impl(const int32_t*, const int32_t*, int64_t, const float*, int64_t, const float*, const float*,
+                                       int32_t, int32_t, float, float*, int64_t, const FitSel&, void*);
 
-beagle_status beagle_eval(const int32_t* genomes, const int32_t* lengths, int64_t P,
-                          const float* consts, int64_t n_consts, const float* X, const float* y,
-                          int32_t N, int32_t d, float tax, float* fitness_out, void* stream)
+static beagle_status eval_impl(const int32_t* genomes, const int32_t* lengths, int64_t P,
+                               const float* consts, int64_t n_consts, const float* X, const float* y,
+                               int32_t N, int32_t d, float tax, float* fitness_out, const FitSel& fit, void* stream)
 {
     beagle_status s = check_args(genomes, lengths, P, consts, n_consts, X, y, N, d, fitness_out);
     if (s != BEAGLE_OK) return s;
     g_launches = 0;
     if (P == 0) return BEAGLE_OK;
     if ((s = init_once()) != BEAGLE_OK) return s;
-    if ((s = reserve_P(P)) != BEAGLE_OK) return s;
     cudaStream_t st = (cudaStream_t)stream;
-    return run_colony(genomes, lengths, P, consts, n_consts, X, y, N, d, tax, fitness_out, nullptr, -1, st);
+    if ((s = ready_or_grow(P, -1, tmem_plan(N, d, fit.kind).fast, st)) != BEAGLE_OK) return s;
+    return run_colony(genomes, lengths, P, consts, n_consts, X, y, N, d, tax, fitness_out, nullptr, -1, fit, st);
+}
+
+extern "C" {
+
+beagle_status beagle_eval(const int32_t* genomes, const int32_t* lengths, int64_t P,
+                          const float* consts, int64_t n_consts, const float* X, const float* y,
+                          int32_t N, int32_t d, float tax, float* fitness_out, void* stream)
+{
+    return eval_impl(genomes, lengths, P, consts, n_consts, X, y, N, d, tax, fitness_out, kFitMse, stream);
 }
 
 beagle_status beagle_eval_fit(const int32_t* genomes, const int32_t* lengths, int64_t P,
@@ -731,10 +774,8 @@ beagle_status beagle_eval_fit(const int32_t* genomes, const int32_t* lengths, in
 {
     int kind, power;
     if (!decode_fit(fit, &kind, &power)) return BEAGLE_ERR_INVALID_ARG;
-    g_fit.kind = kind; g_fit.M = M; g_fit.power = power;
-    const beagle_status s = beagle_eval(genomes, lengths, P, consts, n_consts, X, y, N, d, tax, fitness_out, stream);
-    g_fit.kind = BEAGLE_FIT_MSE; g_fit.M = 0.f;
-    return s;
+    const FitSel sel = { kind, M, power };
+    return eval_impl(genomes, lengths, P, consts, n_consts, X, y, N, d, tax, fitness_out, sel, stream);
 }
 
 beagle_status beagle_rank(const float* fitness, int64_t P, const int64_t* sample_idx, int32_t n_sample,
@@ -770,9 +811,9 @@ beagle_status beagle_debug_outputs(const int32_t* genomes, const int32_t* length
     g_launches = 0;
     if (P == 0) return BEAGLE_OK;
     if ((s = init_once()) != BEAGLE_OK) return s;
-    if ((s = reserve_P(P)) != BEAGLE_OK) return s;
     cudaStream_t st = (cudaStream_t)stream;
-    return run_colony(genomes, lengths, P, consts, n_consts, X, nullptr, N, d, 0.f, nullptr, out_PxN, -1, st);
+    if ((s = ready_or_grow(P, -1, tmem_plan(N, d, BEAGLE_FIT_MSE).fast, st)) != BEAGLE_OK) return s;
+    return run_colony(genomes, lengths, P, consts, n_consts, X, nullptr, N, d, 0.f, nullptr, out_PxN, -1, kFitMse, st);
 }
 
 beagle_status beagle_eval_blockwise(const int32_t* genomes, const int32_t* lengths, int64_t P,
@@ -784,14 +825,14 @@ beagle_status beagle_eval_blockwise(const int32_t* genomes, const int32_t* lengt
     g_launches = 0;
     if (P == 0) return BEAGLE_OK;
     if ((s = init_once()) != BEAGLE_OK) return s;
-    if ((s = reserve_P(P)) != BEAGLE_OK) return s;
     cudaStream_t st = (cudaStream_t)stream;
+    if ((s = ready_or_grow(P, -1, false, st)) != BEAGLE_OK) return s;
     Workspace& w = g_ws;
     // k_compile runs as the well-formedness check only (depth[]); it emits no micro-ops
-    if ((s = run_prepass(genomes, lengths, P, consts, n_consts, X, y, N, d, fitness_out, nullptr, -1, false, st)) != BEAGLE_OK) return s;
+    if ((s = run_prepass(genomes, lengths, P, consts, n_consts, X, y, N, d, fitness_out, nullptr, -1, false, kFitMse, st)) != BEAGLE_OK) return s;
     const int threads = (N + 31) / 32 * 32;
     k_eval_blockwise<<<(unsigned)P, threads, 0, st>>>(genomes, w.off, lengths, w.depth, consts, X, y, N, d, tax,
-                                                      fitness_out, nullptr, nullptr, nullptr, P, g_fit.kind, g_fit.M, g_fit.power);
+                                                      fitness_out, nullptr, nullptr, nullptr, P, BEAGLE_FIT_MSE, 0.f, 1);
     ++g_launches;
     CU(cudaGetLastError());
     return BEAGLE_OK;
@@ -817,7 +858,7 @@ beagle_status beagle_reserve_chunked(int64_t device_budget_bytes)
     if (s != BEAGLE_OK) return s;
     // the budget is cut into K staging buffers of about 32 MiB (2 <= K <= 8): a chunk is copied while the ones before it
     // are evaluated, and the finer the chunks the less of the first copy and of the last evaluation is exposed
-    long long K = device_budget_bytes / kStageTarget;
+    long long K = device_budget_bytes / g_stage_target;
     K = K < 2 ? 2 : (K > kStageBufsMax ? kStageBufsMax : K);
     const long long half = (device_budget_bytes / K) & ~255ll;
     if (half < 4ll * (BEAGLE_MAX_LEN + 1)) return BEAGLE_ERR_INVALID_ARG;
@@ -835,14 +876,13 @@ beagle_status beagle_reserve_chunked(int64_t device_budget_bytes)
         for (int i = 1; i < (int)K; ++i) w.stage[i] = w.stage[0] + (size_t)i * half;
         w.stage_bytes = half; w.stage_n = (int)K;
     }
-    // workspace of one chunk: at most cap_words individuals and 2 * cap_words micro-op entries
+    // workspace of one chunk: lengths + tokens fill at most cap_words words; an individual of L tokens takes at most
+    // L + 4 records, and the most records per word come from one-token programs: 5 records for 2 words
     const long long cap_words = half / 4 - 3;
-    if ((s = reserve_U(2 * cap_words + 2)) != BEAGLE_OK) return s;
+    if ((s = reserve_U(5 * cap_words / 2 + 4)) != BEAGLE_OK) return s;
     return BEAGLE_OK;
 }
 
-beagle_status beagle_eval_chunked(const int32_t*, const int32_t*, int64_t, const float*, int64_t, const float*, const float*,
-                                  int32_t, int32_t, float, float*, int64_t, void*);
 beagle_status beagle_eval_chunked_fit(const int32_t* h_genomes, const int32_t* h_lengths, int64_t P,
                                       const float* h_consts, int64_t n_consts, const float* X, const float* y,
                                       int32_t N, int32_t d, int32_t fit, float M, float tax, float* fitness_out,
@@ -850,11 +890,8 @@ beagle_status beagle_eval_chunked_fit(const int32_t* h_genomes, const int32_t* h
 {
     int kind, power;
     if (!decode_fit(fit, &kind, &power)) return BEAGLE_ERR_INVALID_ARG;
-    g_fit.kind = kind; g_fit.M = M; g_fit.power = power;
-    const beagle_status s = beagle_eval_chunked(h_genomes, h_lengths, P, h_consts, n_consts, X, y, N, d, tax, fitness_out,
-                                                device_budget_bytes, stream);
-    g_fit.kind = BEAGLE_FIT_MSE; g_fit.M = 0.f;
-    return s;
+    const FitSel sel = { kind, M, power };
+    return eval_chunked_impl(h_genomes, h_lengths, P, h_consts, n_consts, X, y, N, d, tax, fitness_out, device_budget_bytes, sel, stream);
 }
 
 beagle_status beagle_eval_chunked(const int32_t* h_genomes, const int32_t* h_lengths, int64_t P,
@@ -862,9 +899,19 @@ beagle_status beagle_eval_chunked(const int32_t* h_genomes, const int32_t* h_len
                                   int32_t N, int32_t d, float tax, float* fitness_out,
                                   int64_t device_budget_bytes, void* stream)
 {
+    return eval_chunked_impl(h_genomes, h_lengths, P, h_consts, n_consts, X, y, N, d, tax, fitness_out, device_budget_bytes, kFitMse, stream);
+}
+
+} // extern "C"
+
+static beagle_status eval_chunked_impl(const int32_t* h_genomes, const int32_t* h_lengths, int64_t P,
+                                       const float* h_consts, int64_t n_consts, const float* X, const float* y,
+                                       int32_t N, int32_t d, float tax, float* fitness_out,
+                                       int64_t device_budget_bytes, const FitSel& fit, void* stream)
+{
     beagle_status s = check_args(h_genomes, h_lengths, P, h_consts, n_consts, X, y, N, d, fitness_out);
     if (s != BEAGLE_OK) return s;
-    if (device_budget_bytes < 2ll * 4 * (BEAGLE_MAX_LEN + 1)) return BEAGLE_ERR_INVALID_ARG;
+    if (device_budget_bytes < 2ll * 4 * (BEAGLE_MAX_LEN + 64)) return BEAGLE_ERR_INVALID_ARG;   // 4608: include/beagle.h
     g_launches = 0;
     if (P == 0) return BEAGLE_OK;
     if ((s = beagle_reserve_chunked(device_budget_bytes)) != BEAGLE_OK) return s;
@@ -915,7 +962,8 @@ beagle_status beagle_eval_chunked(const int32_t* h_genomes, const int32_t* h_len
             CU(cudaMemcpyAsync(d_tok, h_genomes + tok0, sizeof(int32_t) * ntok, cudaMemcpyHostToDevice, w.copy_stream));
         CU(cudaEventRecord(w.ev_copied[b], w.copy_stream));
         CU(cudaStreamWaitEvent(st, w.ev_copied[b], 0));
-        if ((s = run_colony(d_tok, d_len, np, w.stage_consts, n_consts, X, y, N, d, tax, fitness_out + p0, nullptr, ntok, st)) != BEAGLE_OK) return s;
+        if ((s = ready_or_grow(np, ntok, tmem_plan(N, d, fit.kind).fast, st)) != BEAGLE_OK) return s;     // (reserved: a no-op)
+        if ((s = run_colony(d_tok, d_len, np, w.stage_consts, n_consts, X, y, N, d, tax, fitness_out + p0, nullptr, ntok, fit, st)) != BEAGLE_OK) return s;
         CU(cudaEventRecord(w.ev_free[b], st));
         total_launches += g_launches; g_launches = 0;
         p0 = p1; tok0 += ntok;
@@ -923,6 +971,8 @@ beagle_status beagle_eval_chunked(const int32_t* h_genomes, const int32_t* h_len
     g_launches = total_launches;
     return BEAGLE_OK;
 }
+
+extern "C" {
 
 void beagle_limits(int32_t* max_len, int32_t* max_stack, int32_t* max_n, int32_t* max_d)
 {
@@ -940,6 +990,7 @@ const char* beagle_status_string(beagle_status s)
     case BEAGLE_ERR_UNSUPPORTED: return "unsupported device or configuration (needs sm_100 and enough shared memory)";
     case BEAGLE_ERR_CUDA: return "CUDA error (see beagle_last_cuda_error)";
     case BEAGLE_ERR_NOMEM: return "out of device memory";
+    case BEAGLE_ERR_NOT_RESERVED: return "the workspace would have to grow inside a stream capture: call beagle_reserve first";
     default: return "unknown status";
     }
 }
@@ -966,13 +1017,31 @@ void beagle_release(void)
     cudaFree(w.off); cudaFree(w.depth); cudaFree(w.meta); cudaFree(w.sched);
     cudaFree(w.slow_list); cudaFree(w.bsum); cudaFree(w.uops);
     cudaFree(w.stage[0]); cudaFree(w.stage_consts); cudaFree(w.rank_hist); w.rank_hist = nullptr;
-    w.off = nullptr; w.depth = nullptr; w.meta = nullptr;
+    (void)cudaGetLastError();
+    w.off = nullptr; w.depth = nullptr; w.meta = nullptr; w.sched = nullptr;
     w.slow_list = nullptr; w.bsum = nullptr; w.uops = nullptr; w.cap_P = 0; w.cap_U = 0;
     w.promised_P = 0; w.promised_T = 0;
     w.stage[0] = nullptr; w.stage_bytes = 0; w.stage_n = 0; w.stage_consts = nullptr; w.stage_consts_cap = 0;
 }
 
 int32_t beagle_last_launch_count(void) { return g_launches; }
+
+beagle_status beagle_debug_counts(int32_t* n_sorted, int32_t* n_general, int32_t* n_slow, int32_t* n_malformed, void* stream)
+{
+    Header h;
+    if (!g_ws.hdr) return BEAGLE_ERR_INVALID_ARG;
+    CU(cudaMemcpyAsync(&h, g_ws.hdr, sizeof(Header), cudaMemcpyDeviceToHost, (cudaStream_t)stream));
+    CU(cudaStreamSynchronize((cudaStream_t)stream));
+    if (n_sorted) *n_sorted = h.n_sorted;
+    if (n_general) *n_general = h.n_general;
+    if (n_slow) *n_slow = h.n_slow;
+    if (n_malformed) *n_malformed = h.n_malformed;
+    return BEAGLE_OK;
+}
+
+void beagle_set_chunk_target(int64_t bytes) { g_stage_target = bytes > 0 ? bytes : kStageTarget; }
+
+int32_t beagle_chunk_buffers(void) { return g_ws.stage_n; }
 
 void beagle_set_profiling(int32_t on) { g_profiling = on < 0 ? 0 : on; g_prof_calls = 0; if (on) g_ws.prof_n = 0; }
 
