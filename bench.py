@@ -29,13 +29,57 @@ if ROOT not in sys.path:
 
 METRIC = "gp_ops_per_sec"
 UNIT = "GPops/s"            # 1 GP op = 1 token evaluated on 1 fitness case
-SM_COUNT = 148
 FP32_LANES_PER_SM = 128     # 4 schedulers x 32 lanes (B200_PROFILING.md / DESIGN.md §8)
 
 
-def fp32_issue_peak(sm_mhz: float) -> float:
-    """FP32 lane-instructions per second: the 'alu' roofline of DESIGN.md §8 (1 GP op = 1 lane-instr)."""
-    return SM_COUNT * FP32_LANES_PER_SM * sm_mhz * 1e6
+def fp32_issue_peak(sm_mhz: float, sm_count: int) -> float:
+    """FP32 lane-instructions per second: the 'alu' roofline of DESIGN.md §8 (1 GP op = 1 lane-instr).
+    sm_count comes from the device (cudaGetDeviceProperties), not from a constant."""
+    return sm_count * FP32_LANES_PER_SM * sm_mhz * 1e6
+
+
+# SURVEY.md §8(d) "Algorithmic work per unit": issue slots / MUFU-pipe instructions / shared-memory words per token x case,
+# by opcode class, for the cheapest correct implementation the survey names. The f1 commands added with the same logic:
+# SIGN, SQUARE one instruction, CUBE two, DUP / SWAP / DEL one move at most.
+MIX_WEIGHTS = {  # name: (issue, mufu, smem words)
+    "LOAD": (1, 0, 1), "CONST": (1, 0, 0), "ADD": (1, 0, 0), "SUB": (1, 0, 0), "MUL": (1, 0, 0),
+    "DIV": (4, 1, 0), "SQRT": (3, 1, 0), "EXP": (3, 1, 0), "LOG": (4, 1, 0), "SIN": (2, 1, 0), "COS": (2, 1, 0),
+    "SIGN": (1, 0, 0), "SQUARE": (1, 0, 0), "CUBE": (2, 0, 0), "DUP": (1, 0, 0), "SWAP": (1, 0, 0), "DEL": (0, 0, 0),
+}
+
+
+def mix_ceilings(token_hist):
+    """Fractions of the FP32 issue roofline that the realised token mix allows: the issue ceiling
+    1 / mean issue slots per GP op; the MUFU ceiling (16 lanes per clock and SM against 128: a MUFU instruction on every
+    token would allow 1/8); the shared-memory ceiling (32 words per clock and SM against 128 GP ops). The binding one is the
+    smallest. Commands without a weight (POW, library functions, variables: blockwise kernel) are left out and reported."""
+    tot = sum(v for k, v in token_hist.items() if k in MIX_WEIGHTS)
+    other = sum(v for k, v in token_hist.items() if k not in MIX_WEIGHTS)
+    if tot == 0:
+        return None
+    issue = sum(MIX_WEIGHTS[k][0] * v for k, v in token_hist.items() if k in MIX_WEIGHTS) / tot
+    mufu = sum(MIX_WEIGHTS[k][1] * v for k, v in token_hist.items() if k in MIX_WEIGHTS) / tot
+    smem = sum(MIX_WEIGHTS[k][2] * v for k, v in token_hist.items() if k in MIX_WEIGHTS) / tot
+    c = {"issue_slots_per_gp_op": issue, "mufu_per_gp_op": mufu, "smem_words_per_gp_op": smem,
+         "issue_ceiling": 1.0 / issue if issue else None, "mufu_ceiling": 1.0 / (8.0 * mufu) if mufu else None,
+         "smem_ceiling": 1.0 / (4.0 * smem) if smem else None, "tokens_without_weight": other}
+    c["ceiling"] = min(v for v in (c["issue_ceiling"], c["mufu_ceiling"], c["smem_ceiling"]) if v)
+    return c
+
+
+def dram_traffic_table():
+    """dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from the ncu --set full captures
+    summarised in profiles/r2_dram_traffic.csv (columns: config,fitness,kernel,dram_read_bytes,dram_write_bytes)."""
+    t = {}
+    try:
+        with open(os.path.join(ROOT, "profiles", "r2_dram_traffic.csv")) as f:
+            for line in f:
+                c = [x.strip() for x in line.split(",")]
+                if len(c) >= 5 and c[0].isdigit():
+                    t[(int(c[0]), c[1], c[2])] = int(c[3]) + int(c[4])
+    except OSError:
+        pass
+    return t
 
 
 def measured_peaks():
@@ -172,9 +216,15 @@ def cpu_baseline(col, target_seconds=12.0):
     rate0, dt0, _, threads = oracle_rate(col, 2048)
     n = int(min(col.P, max(2048, 2048 * target_seconds / max(dt0, 1e-3))))
     rate, dt, ops, threads = oracle_rate(col, n)
+    # SURVEY.md §8(d) "CPU baseline (i)": the same function on ONE thread (the oracle is single-threaded; the fan-out
+    # above is wall-time plumbing), on a sample sized for a few seconds
+    n1 = int(min(col.P, max(512, n / max(threads, 1) / 3)))
+    rate1, dt1, ops1, _ = oracle_rate(col, n1, threads=1)
     return {"value": rate / 1e9, "unit": UNIT, "cores": threads, "kind": "oracle",
             "sample": f"first {n} individuals of the workload ({ops / 1e9:.3f} GPops, fp64 + error bound, "
-                      f"{dt:.1f} s wall on {threads} threads)"}
+                      f"{dt:.1f} s wall on {threads} threads)",
+            "one_thread": {"value": rate1 / 1e9, "unit": UNIT, "cores": 1,
+                           "sample": f"first {n1} individuals ({ops1 / 1e9:.3f} GPops, {dt1:.1f} s)"}}
 
 
 # ------------------------------------------------------------------------------------------------
@@ -229,7 +279,8 @@ def run_ours(args):
 
     cfg = colonies.CONFIGS[args.config]
     P = cfg.P if args.population is None else args.population
-    tokens, lengths, consts = colonies.generate_programs(cfg, P, seed_offset=rank_seed_offset(rank))
+    tokens, lengths, consts = colonies.generate_programs(cfg, P, seed_offset=rank_seed_offset(rank), gcl_mix=args.gcl_mix)
+    sm_count = torch.cuda.get_device_properties(dev).multi_processor_count
     Xh, yh, _ = colonies.make_dataset(cfg)
     N, d = Xh.shape
     T = int(tokens.shape[0])
@@ -290,9 +341,20 @@ def run_ours(args):
     torch.cuda.synchronize(); dist_barrier(world)
     ms_local = ev0.elapsed_time(ev1)
     n_prof, eval_ms = api.beagle_profiled_eval_kernel_ms()
+    _, prepass_ms = api.beagle_profiled_prepass_ms()
     api.beagle_set_profiling(False)
+    counts = api.beagle_debug_counts(sp) if resident else None
     clk = clocks.stop() if clocks else None
     value, ms_max = job_throughput(units, args.steps, ms_local, world, dev)
+
+    # ---- SURVEY.md §8(d) protocol beside the contract's K-step mean: 20 calls, CUDA events around each, median and best
+    per_call = []
+    if resident:
+        evs = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(20)]
+        for a, b in evs:
+            a.record(stream); step(); b.record(stream)
+        torch.cuda.synchronize()
+        per_call = sorted(a.elapsed_time(b) for a, b in evs)
 
     # ---- end-to-end leg: pinned host buffers -> C-ABI -> result back on the host, every step -------
     for _ in range(min(args.warmup, 3)):
@@ -313,7 +375,13 @@ def run_ours(args):
         return 0
     peaks = measured_peaks()
     sm_max = float(peaks.get("sm_max_mhz", 1965.0))
-    peak = fp32_issue_peak(sm_max)
+    peak = fp32_issue_peak(sm_max, sm_count)
+    stats = colonies.colony_stats(tokens, lengths)
+    mix = mix_ceilings(stats["token_hist"])
+    traffic = dram_traffic_table()
+    pre_bytes = 4 * T + 4 * len(consts) + 4 * P + 16 * P          # tokens, constants, lengths, start records: read once
+    n_cmd = T - stats["token_hist"]["CONST"] - stats["token_hist"]["LOAD"]     # one 8-byte micro-op record per command token
+    pre_bytes_out = 8 * (n_cmd + 3 * P) + 16 * P + 16 * P + 4 * P + 8 * P    # records (+ 3 per program), start records, meta, depth, offsets
     kernel_rate = units / (eval_ms * 1e-3) if (resident and n_prof > 0 and eval_ms > 0) else None
     fit = hout.numpy()
     line = {
@@ -321,13 +389,18 @@ def run_ours(args):
         "warmup": args.warmup, "ms_per_step": ms_max / args.steps, "higher_is_better": True,
         "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
         "config": {"workload": workload_name(cfg) + ("" if args.population is None else f" [first {P}]"),
-                   "fitness": args.fit,
+                   "fitness": args.fit, "gcl_mix": args.gcl_mix,
                    "tokens": T, "gp_ops_per_step": units, "timed": "beagle_eval, inputs resident in HBM" if resident
                    else "beagle_eval_chunked from pinned host memory (the colony exceeds its device budget)",
                    "l2": f"token stream {4 * T / 1e6:.0f} MB per step vs 126 MB L2 (inputs larger than L2)"
                    if 4 * T > 126e6 else f"token stream {4 * T / 1e6:.1f} MB fits L2; no flush (ALU-bound path)",
                    "parallelism": f"dp{world} (independent colonies, no collective)"},
         "pct_of_fp32_issue_roofline": 100.0 * value / world / peak,
+        "pct_of_mix_weighted_ceiling": None if not mix else 100.0 * value / world / peak / mix["ceiling"],
+        "mix": mix,
+        "step_ms_median_of_20": per_call[len(per_call) // 2] if per_call else None,
+        "step_ms_best_of_20": per_call[0] if per_call else None,
+        "prepass_counts": counts,
         "clocks": clk,
         "e2e": {"value": e2e_value / 1e9, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
                 "steps": e2e_steps, "via": f"beagle_eval_chunked(pinned host genomes, budget {budget >> 20} MiB) + D2H of fitness"},
@@ -336,10 +409,19 @@ def run_ours(args):
                      "achieved": None if kernel_rate is None else kernel_rate / 1e12,
                      "peak": peak / 1e12, "unit": "T lane-instr/s (1 GP op = 1 FP32 lane-instruction)",
                      "frac": None if kernel_rate is None else kernel_rate / peak,
-                     "peak_basis": f"148 SMs x 128 FP32 lanes x {sm_max:.0f} MHz (MEASURED_PEAKS.json sm_max_mhz; DESIGN.md §8)",
+                     "peak_basis": f"{sm_count} SMs (device properties) x 128 FP32 lanes x {sm_max:.0f} MHz (MEASURED_PEAKS.json sm_max_mhz; DESIGN.md §8)",
                      "kernel_ms": eval_ms if n_prof else None, "kernel_launches_timed": n_prof, "kernel_share_of_step": (eval_ms / (ms_local / args.steps)) if n_prof else None,
                      "hbm_gbs_on_genome_stream": None if kernel_rate is None else (4 * T + 12 * P) / (eval_ms * 1e-3) / 1e9,
-                     "traffic": TRAFFIC_BYTES.get(args.config)},
+                     "traffic": traffic.get((args.config, args.fit, "k_eval")) if args.gcl_mix == "hot" else None},
+        # the pre-pass (scan, sort, compile) against the HBM roofline: the token stream is read here
+        "roofline_prepass": None if not (resident and n_prof > 0 and prepass_ms > 0) else {
+            "bound": "hbm", "kernel": "k_len_pass1/2, k_scatter, k_compile, k_compile_general",
+            "achieved": (pre_bytes + pre_bytes_out) / (prepass_ms * 1e-3) / 1e9, "peak": float(peaks.get("hbm_gbs", 6650.0)),
+            "unit": "GB/s", "frac": (pre_bytes + pre_bytes_out) / (prepass_ms * 1e-3) / 1e9 / float(peaks.get("hbm_gbs", 6650.0)),
+            "peak_basis": "MEASURED_PEAKS.json hbm_gbs (copy bandwidth)" if "hbm_gbs" in peaks else "fallback 6650 GB/s (B200_PROFILING.md)",
+            "algorithmic_bytes": pre_bytes + pre_bytes_out, "prepass_ms": prepass_ms,
+            "genome_stream_gbs": 4 * T / (prepass_ms * 1e-3) / 1e9,
+            "traffic": traffic.get((args.config, args.fit, "k_compile")) if args.gcl_mix == "hot" else None},
         "result_check": {"finite": int(np.isfinite(fit).sum()), "nan": int(np.isnan(fit).sum()),
                          "inf": int(np.isinf(fit).sum())},
     }
@@ -367,11 +449,6 @@ def run_ours(args):
     return 0
 
 
-# dram__bytes_read.sum + dram__bytes_write.sum of the dominant kernel, per launch, from the ncu --set full
-# capture summarised under profiles/ (None until a capture exists for that config).
-TRAFFIC_BYTES = {3: 358849024 + 31903232}   # profiles/r1_ncu_config3_grouped.md (k_eval, config 3: dram read + write)
-
-
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -380,6 +457,9 @@ def main():
     ap.add_argument("--config", type=int, default=3, choices=[1, 2, 3, 4, 5])
     ap.add_argument("--population", type=int, default=None, help="first P individuals only (debugging; not a bench value)")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--gcl-mix", default="hot", choices=["hot", "f1"],
+                    help="hot: the eleven commands of BASELINE.json's configs; f1: the same trees with SIGN SQUARE CUBE and "
+                         "DUP SWAP DEL woven in (SURVEY f1; not BASELINE.json's metric)")
     ap.add_argument("--fit", default="mse", choices=["mse", "correlation", "std", "std_hyper"],
                     help="fitness function; mse is BASELINE.json's metric, correlation the paper's default objective (f2)")
     ap.add_argument("--e2e-steps", type=int, default=5)

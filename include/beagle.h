@@ -280,8 +280,8 @@ void    beagle_set_chunk_target(int64_t bytes);
 int32_t beagle_chunk_buffers(void);
 
 /* Profiling hooks for bench.py's roofline line. While profiling is on (on = n > 0), every n-th beagle_eval
- * call, starting with the first, brackets its evaluation kernels (the interpreter launches, without the scheduling
- * pre-pass) with a pair of CUDA events on `stream` (at most 256 calls are recorded; later ones are not). The two
+ * call, starting with the first, brackets its pre-pass and its evaluation kernels (the interpreter launches) with
+ * three CUDA events on `stream` (at most 256 calls are recorded; later ones are not). The two
  * event records cost a call about 12 us of stream bubbles and keep k_eval from starting under the tail of
  * k_compile, which is why a bench may want n > 1.
  * beagle_profiled_eval_kernel_ms synchronises on the recorded events, stores the number of
@@ -289,6 +289,9 @@ int32_t beagle_chunk_buffers(void);
  * (< 0 if nothing was recorded). beagle_set_profiling(1) clears the record. */
 void  beagle_set_profiling(int32_t on);
 float beagle_profiled_eval_kernel_ms(int32_t* n_calls);
+/* The same for the pre-pass of the recorded calls (a2-a3 and the compile step of a5: from the start of the call to
+ * the start of the interpreter), mean device time in milliseconds. */
+float beagle_profiled_prepass_ms(int32_t* n_calls);
 
 #ifdef __cplusplus
 }

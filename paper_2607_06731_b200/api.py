@@ -52,6 +52,7 @@ _SIGNATURES = {
     "beagle_chunk_buffers": (_i32, []),
     "beagle_set_profiling": (None, [_i32]),
     "beagle_profiled_eval_kernel_ms": (_f32, [ctypes.POINTER(_i32)]),
+    "beagle_profiled_prepass_ms": (_f32, [ctypes.POINTER(_i32)]),
 }
 EXPORTS = tuple(_SIGNATURES)
 
@@ -200,6 +201,13 @@ def beagle_profiled_eval_kernel_ms():
     """(number of recorded calls, mean device ms of their evaluation kernels)."""
     n = _i32(0)
     ms = float(lib().beagle_profiled_eval_kernel_ms(ctypes.byref(n)))
+    return n.value, ms
+
+
+def beagle_profiled_prepass_ms():
+    """(number of recorded calls, mean device ms of their pre-pass: scan, sort, compile)."""
+    n = _i32(0)
+    ms = float(lib().beagle_profiled_prepass_ms(ctypes.byref(n)))
     return n.value, ms
 
 

@@ -49,7 +49,7 @@ def _gen():
         _lib.colony_generate.argtypes = [
             ctypes.c_int, ctypes.c_uint64, ctypes.c_int64, ctypes.c_int, ctypes.c_int, ctypes.c_int,
             ctypes.c_void_p, ctypes.c_int, ctypes.c_void_p, ctypes.c_int, ctypes.c_double,
-            ctypes.c_int, ctypes.c_double, ctypes.c_double, ctypes.c_int,
+            ctypes.c_int, ctypes.c_double, ctypes.c_double, ctypes.c_int, ctypes.c_int,
             ctypes.c_void_p, ctypes.c_void_p, ctypes.c_void_p,
             ctypes.POINTER(ctypes.c_int64), ctypes.POINTER(ctypes.c_int64)]
     return _lib
@@ -193,12 +193,21 @@ def make_dataset(cfg: ColonyConfig):
     return X.astype(np.float32), y.astype(np.float32), expr
 
 
-def generate_programs(cfg: ColonyConfig, P: int | None = None, seed_offset: int = 0):
+_F1_UNARY = (OP["SIGN"], OP["SQUARE"], OP["CUBE"])
+
+
+def generate_programs(cfg: ColonyConfig, P: int | None = None, seed_offset: int = 0, gcl_mix: str = "hot"):
     """tokens int32[T], lengths int32[P], consts float32[C] for the first P individuals of cfg.
-    seed_offset != 0 draws a different colony of the same shape (bench.py: one per rank)."""
+    seed_offset != 0 draws a different colony of the same shape (bench.py: one per rank).
+    gcl_mix = "f1" (G-tree configs): SIGN SQUARE CUBE join the unary commands and DUP SWAP DEL are woven into the
+    trees (gen.c "f1 mix"): the colony then speaks the part of the paper's language the interpreter runs."""
     P = cfg.P if P is None else int(P)
     seed = 0xBEA61E00 + cfg.number + int(seed_offset)
-    un = (ctypes.c_int * len(cfg.unary))(*cfg.unary)
+    f1 = gcl_mix == "f1"
+    if f1 and cfg.kind != 0:
+        raise ValueError("the f1 mix is defined for the tree-generated configs 1-4")
+    unary = tuple(cfg.unary) + (_F1_UNARY if f1 else ())
+    un = (ctypes.c_int * len(unary))(*unary)
     bn = (ctypes.c_int * len(cfg.binary))(*cfg.binary)
     lengths = np.empty(P, np.int32)
     T = ctypes.c_int64(0)
@@ -206,9 +215,9 @@ def generate_programs(cfg: ColonyConfig, P: int | None = None, seed_offset: int 
     g = _gen()
 
     def call(tok, con):
-        g.colony_generate(cfg.kind, seed, P, cfg.dmin, cfg.dmax, cfg.lcap, un, len(cfg.unary),
+        g.colony_generate(cfg.kind, seed, P, cfg.dmin, cfg.dmax, cfg.lcap, un, len(unary),
                           bn, len(cfg.binary), cfg.q_u, cfg.d, cfg.clo, cfg.chi,
-                          int(cfg.designed_invalid), lengths.ctypes.data_as(ctypes.c_void_p),
+                          int(cfg.designed_invalid), int(f1), lengths.ctypes.data_as(ctypes.c_void_p),
                           None if tok is None else tok.ctypes.data_as(ctypes.c_void_p),
                           None if con is None else con.ctypes.data_as(ctypes.c_void_p),
                           ctypes.byref(T), ctypes.byref(C))

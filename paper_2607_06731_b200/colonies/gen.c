@@ -7,6 +7,10 @@
  *   G-tree   ramped half-and-half trees (configs 1-4), emitted in postfix.
  *   G-len    exact-length linear sampler with Zipf(1) lengths on 1..512 (config 5), plus the four
  *            designed-invalid suffixes.
+ *   f1 mix   (bench.py --gcl-mix f1) G-tree with the paper's stack commands woven in (Table 3): a binary node
+ *            becomes `A DUP op` (both operands the same subtree) with probability 0.15 or gets a SWAP in front of its
+ *            command with probability 0.15; a terminal becomes `t t' DEL` with probability 0.05. Programs stay
+ *            well-formed and within the token cap. SIGN SQUARE CUBE come in through the caller's unary set.
  * Constants: the k-th CONST token in population order gets index k mod 2^24 of the side table.
  */
 #include <stdint.h>
@@ -14,7 +18,7 @@
 #include <math.h>
 
 enum { OP_CONST = 1, OP_LOAD = 2, OP_ADD = 3, OP_SUB = 4, OP_MUL = 5, OP_DIV = 6,
-       OP_SIN = 7, OP_COS = 8, OP_LOG = 9, OP_SQRT = 10, OP_EXP = 11 };
+       OP_SIN = 7, OP_COS = 8, OP_LOG = 9, OP_SQRT = 10, OP_EXP = 11, OP_DUP = 0x10, OP_SWAP = 0x11, OP_DEL = 0x12 };
 #define TOK(op, arg) ((int32_t)(((uint32_t)(arg) << 8) | (uint32_t)(op)))
 #define MAXC (1 << 24)
 
@@ -29,8 +33,8 @@ static inline double rng_u(rng_t* r) { return (double)(rng_next(r) >> 11) * (1.0
 static inline int rng_int(rng_t* r, int n) { int k = (int)(rng_u(r) * n); return k < n ? k : n - 1; }
 
 typedef struct {
-    int n_un, n_bin, d;
-    int un[8], bin[8];
+    int n_un, n_bin, d, f1;
+    int un[16], bin[8];
     double q_u, clo, chi;
 } opset_t;
 
@@ -54,8 +58,11 @@ static void emit_const(prog_t* g, float c) { g->cval[g->nc++] = c; g->tok[g->n++
 /* returns the number of tokens emitted for this subtree */
 static int gen_tree(prog_t* g, rng_t* r, const opset_t* o, int depth_left, int budget, int grow, int root) {
     int start = g->n;
-    if (depth_left == 0 || budget < 2) { emit_terminal(g, r, o); return 1; }
-    if (grow && !root && rng_u(r) < 0.3) { emit_terminal(g, r, o); return 1; }
+    if (depth_left == 0 || budget < 2 || (grow && !root && rng_u(r) < 0.3)) {
+        emit_terminal(g, r, o);
+        if (o->f1 && budget >= 3 && rng_u(r) < 0.05) { emit_terminal(g, r, o); g->tok[g->n++] = TOK(OP_DEL, 0); }
+        return g->n - start;
+    }
     int unary = (budget < 3) ? 1 : (rng_u(r) < o->q_u);
     if (unary) {
         int op = o->un[rng_int(r, o->n_un)];
@@ -65,8 +72,19 @@ static int gen_tree(prog_t* g, rng_t* r, const opset_t* o, int depth_left, int b
         int op = o->bin[rng_int(r, o->n_bin)];
         int lb = (budget - 1 + 1) / 2;           /* ceil((budget-1)/2) */
         if (lb > budget - 2) lb = budget - 2;
-        int ls = gen_tree(g, r, o, depth_left - 1, lb, grow, 0);
-        gen_tree(g, r, o, depth_left - 1, budget - 1 - ls, grow, 0);
+        double f = o->f1 ? rng_u(r) : 1.0;
+        if (f < 0.15) {                          /* A DUP op */
+            gen_tree(g, r, o, depth_left - 1, lb, grow, 0);
+            g->tok[g->n++] = TOK(OP_DUP, 0);
+        } else if (f < 0.30 && budget >= 4) {    /* A B SWAP op */
+            if (lb > budget - 3) lb = budget - 3;
+            int ls = gen_tree(g, r, o, depth_left - 1, lb, grow, 0);
+            gen_tree(g, r, o, depth_left - 1, budget - 2 - ls, grow, 0);
+            g->tok[g->n++] = TOK(OP_SWAP, 0);
+        } else {
+            int ls = gen_tree(g, r, o, depth_left - 1, lb, grow, 0);
+            gen_tree(g, r, o, depth_left - 1, budget - 1 - ls, grow, 0);
+        }
         g->tok[g->n++] = TOK(op, 0);
     }
     return g->n - start;
@@ -106,11 +124,11 @@ static int zipf_len(rng_t* r, const double* cdf, int n) {
  * again with tokens (T words) and consts (min(C, 2^24) floats). Returns 0.                    */
 int colony_generate(int kind, uint64_t seed, int64_t P, int dmin, int dmax, int lcap,
                     const int* un, int n_un, const int* bin, int n_bin, double q_u,
-                    int d, double clo, double chi, int designed_invalid,
+                    int d, double clo, double chi, int designed_invalid, int f1_mix,
                     int32_t* lengths, int32_t* tokens, float* consts,
                     int64_t* T_out, int64_t* C_out) {
     opset_t o; memset(&o, 0, sizeof o);
-    o.n_un = n_un; o.n_bin = n_bin; o.d = d; o.q_u = q_u; o.clo = clo; o.chi = chi;
+    o.n_un = n_un; o.n_bin = n_bin; o.d = d; o.q_u = q_u; o.clo = clo; o.chi = chi; o.f1 = f1_mix;
     for (int i = 0; i < n_un; ++i) o.un[i] = un[i];
     for (int i = 0; i < n_bin; ++i) o.bin[i] = bin[i];
     double cdf[512]; double acc = 0.0;

@@ -57,6 +57,9 @@ constexpr int kEvalThreads = BEAGLE_EVAL_THREADS;   // 32 warps (8 per scheduler
 constexpr int kStageBufsMax = 8;               // beagle_eval_chunked: staging buffers the device budget is cut into
 constexpr long long kStageTarget = 32ll << 20;  // ... of about this size each (at least two); beagle_set_chunk_target overrides it
 static long long g_stage_target = kStageTarget;
+#ifndef BEAGLE_PLAN_W8
+#define BEAGLE_PLAN_W8 0
+#endif
 constexpr int kProfMax = 256;                  // beagle_set_profiling: recorded calls
 constexpr int kEvalMetaBytes = 64 * 16;           // per-warp window of the work queue (64 x int4)
 constexpr int kCasePad = 512;                  // staged cases are padded to a multiple of 32*K
@@ -436,7 +439,7 @@ struct Workspace {
     long long stage_bytes = 0; int stage_n = 0; unsigned char* stage[kStageBufsMax] = {};   // stage[0] owns the allocation
     float* stage_consts = nullptr; long long stage_consts_cap = 0;
     cudaStream_t copy_stream = nullptr; cudaEvent_t ev_copied[kStageBufsMax] = {}, ev_free[kStageBufsMax] = {};
-    cudaEvent_t ev_k[2 * kProfMax] = {}; int prof_n = 0;
+    cudaEvent_t ev_k[2 * kProfMax] = {}; cudaEvent_t ev_p[kProfMax] = {}; int prof_n = 0; bool prof_this = false;
     int num_sms = 0; int smem_optin = 0; bool device_ok = false; bool inited = false; bool need_T_readback = false;
 };
 static Workspace g_ws;
@@ -545,7 +548,7 @@ static TmemPlan tmem_plan(int N, int d, int fit_kind)
     for (int c = 6; c <= wq_max; ++c)
         for (int kk = 0; kk <= d; ++kk) {
             if (free0 - passes * kk < 0 || (free0 - passes * kk) / c < S) break;
-            const int score = (c >= 7 ? 10000 : 0) + kk * 10 + c;
+            const int score = (c >= 7 ? 10000 : 0) + (c >= 8 ? BEAGLE_PLAN_W8 : 0) + kk * 10 + c;
             if (score > best) { best = score; wq = c; k = kk; }
         }
     const int free_rows = free0 - passes * k;
@@ -629,6 +632,12 @@ static beagle_status run_prepass(const int32_t* genomes, const int32_t* lengths,
     Workspace& w = g_ws;
     const int nb = (int)((P + kScanBlock - 1) / kScanBlock);
     const int npad = (N + kCasePad - 1) / kCasePad * kCasePad;
+    // beagle_set_profiling: every n-th call is bracketed by events: pre-pass start, interpreter start, interpreter end
+    w.prof_this = emit && g_profiling && w.prof_n < kProfMax && (g_prof_calls++ % g_profiling) == 0;
+    if (w.prof_this) {
+        if (!w.ev_p[w.prof_n]) CU(cudaEventCreate(&w.ev_p[w.prof_n]));
+        CU(cudaEventRecord(w.ev_p[w.prof_n], st));
+    }
     k_len_pass1<<<nb, kScanThreads, 0, st>>>(lengths, P, w.bsum, w.bins);
     k_len_pass2<<<1, 1024, 0, st>>>(w.bsum, nb, w.hdr, w.bins, w.cursor, w.binstart, w.binubase, X, y, N, d, npad, w.xt, w.ung);
     g_launches += 2;
@@ -651,7 +660,7 @@ static beagle_status run_prepass(const int32_t* genomes, const int32_t* lengths,
         q.slow_list = w.slow_list; q.gen_list = w.slow_list + w.cap_P; q.fitness = fitness; q.outputs = outputs; q.n_cases = N; q.emit = emit ? 1 : 0;
         k_compile<<<(unsigned)((P + kCompileThreads - 1) / kCompileThreads), kCompileThreads, 0, st>>>(q);
         long long gb = (P + kCompileThreads - 1) / kCompileThreads;
-        const long long gcap = (long long)w.num_sms * 16;
+        const long long gcap = (long long)w.num_sms * 8;       // (an empty list costs the launch of these blocks: 8 us at 16 per SM, 3 at 4)
         k_compile_general<<<(unsigned)(gb > gcap ? gcap : gb), kCompileThreads, 0, st>>>(q);
         g_launches += 2;
     }
@@ -671,7 +680,7 @@ static beagle_status run_eval(const int32_t* genomes, const int32_t* lengths, co
     prm.rcp_col0 = tp.rcp_col0; prm.k_rcp = tp.k_rcp; prm.slot_col0 = tp.slot_col0; prm.tmem_slots = tp.tmem_slots;
     prm.meta = w.meta; prm.uops = w.uops; prm.hdr = w.hdr; prm.xt = w.xt; prm.ung = w.ung;
     prm.fitness = fitness; prm.outputs = outputs; prm.tax = tax; prm.M = fit.M; prm.power = fit.power; prm.n = N; prm.npad = npad; prm.d = d;
-    const bool prof = g_profiling && w.prof_n < kProfMax && (g_prof_calls++ % g_profiling) == 0;
+    const bool prof = w.prof_this;
     if (prof) {
         for (int i = 0; i < 2; ++i)
             if (!w.ev_k[2 * w.prof_n + i]) CU(cudaEventCreate(&w.ev_k[2 * w.prof_n + i]));
@@ -1044,6 +1053,22 @@ void beagle_set_chunk_target(int64_t bytes) { g_stage_target = bytes > 0 ? bytes
 int32_t beagle_chunk_buffers(void) { return g_ws.stage_n; }
 
 void beagle_set_profiling(int32_t on) { g_profiling = on < 0 ? 0 : on; g_prof_calls = 0; if (on) g_ws.prof_n = 0; }
+
+float beagle_profiled_prepass_ms(int32_t* n_calls)
+{
+    Workspace& w = g_ws;
+    if (n_calls) *n_calls = 0;
+    if (w.prof_n <= 0) return -1.f;
+    double sum = 0.0;
+    for (int i = 0; i < w.prof_n; ++i) {
+        float ms = 0.f;
+        if (cudaEventSynchronize(w.ev_k[2 * i]) != cudaSuccess) return -1.f;
+        if (cudaEventElapsedTime(&ms, w.ev_p[i], w.ev_k[2 * i]) != cudaSuccess) return -1.f;
+        sum += ms;
+    }
+    if (n_calls) *n_calls = w.prof_n;
+    return (float)(sum / w.prof_n);
+}
 
 float beagle_profiled_eval_kernel_ms(int32_t* n_calls)
 {
