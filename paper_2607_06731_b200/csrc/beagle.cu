@@ -72,6 +72,7 @@ struct Header {                                // device-resident results of the
     int max_len;                               // longest in-range length (>= 1 if n_sorted > 0)
     int n_slow;                                // individuals the blockwise kernel takes (POW, library functions, variables; or no room)
     int n_general;                             // individuals k_compile's walk turned down (k_compile_general)
+    int n_f1;                                  // individuals compiled with DUP SWAP DEL SIGN SQUARE CUBE (picks k_compile<F1> next time)
     int n_malformed;
     unsigned int queue;                        // work-queue cursor of the interpreter kernel
     unsigned int rcp_unsafe;                   // bit j: some case of variable j has |x| < 1e-6f (its division is protected)
@@ -222,7 +223,7 @@ __global__ void __launch_bounds__(1024) k_len_pass2(long long* __restrict__ bsum
         hdr->T = carry_s;
         hdr->n_sorted = (int)carry2_s;
         hdr->max_len = maxlen_s;
-        hdr->n_slow = 0; hdr->n_malformed = 0; hdr->n_general = 0;
+        hdr->n_slow = 0; hdr->n_malformed = 0; hdr->n_general = 0; hdr->n_f1 = 0;
         hdr->queue = 0;
         hdr->rcp_unsafe = unsafe_s;
     }
@@ -338,9 +339,13 @@ __global__ void __launch_bounds__(1024) k_eval_blockwise(
     const int32_t* __restrict__ genomes, const long long* __restrict__ off, const int32_t* __restrict__ lengths,
     const int* __restrict__ depth, const float* __restrict__ consts, const float* __restrict__ X,
     const float* __restrict__ y, int n, int d, float tax, float* __restrict__ fitness, float* __restrict__ outputs,
-    const int* __restrict__ list, const int* __restrict__ count, long long P, int fit, float M, int power)
+    const int* __restrict__ list, const int* __restrict__ count, long long P, int fit, float M, int power,
+    const int* __restrict__ n_f1, int* __restrict__ h_f1)
 {
     __shared__ float res[BEAGLE_MAX_N];
+    // the last kernel of a call tells the host (pinned, mapped memory) how many programs used the f1 commands: the next
+    // call picks its k_compile instantiation by it (no copy, no synchronisation)
+    if (h_f1 && blockIdx.x == 0 && threadIdx.x == 0) *h_f1 = *n_f1;
     bool y_finite = true;
     if (fit == BEAGLE_FIT_CORRELATION) y_finite = __syncthreads_and(threadIdx.x >= n || finite32(__ldg(y + threadIdx.x)));
     const long long total = list ? (long long)*count : P;
@@ -433,7 +438,7 @@ struct Workspace {
     int* slow_list = nullptr; long long* bsum = nullptr;
     uint2* uops = nullptr;
     int* bins = nullptr; int* cursor = nullptr; int* binstart = nullptr; long long* binubase = nullptr;
-    float* xt = nullptr; float* ung = nullptr; Header* hdr = nullptr; long long* h_T = nullptr;
+    float* xt = nullptr; float* ung = nullptr; Header* hdr = nullptr; long long* h_T = nullptr; int* h_f1 = nullptr;
     unsigned long long* rank_hist = nullptr;   // beagle_rank's histogram when the caller wants none
     // chunked staging
     long long stage_bytes = 0; int stage_n = 0; unsigned char* stage[kStageBufsMax] = {};   // stage[0] owns the allocation
@@ -479,6 +484,8 @@ static beagle_status init_once()
     CU(cudaMalloc(&w.hdr, sizeof(Header)));
     CU(cudaMemset(w.hdr, 0, sizeof(Header)));
     CU(cudaMallocHost(&w.h_T, sizeof(long long)));
+    CU(cudaMallocHost(&w.h_f1, sizeof(int)));
+    *w.h_f1 = 0;
     w.inited = true;                               // only now: a failed allocation above is tried again by the next call
     return BEAGLE_OK;
 }
@@ -658,7 +665,10 @@ static beagle_status run_prepass(const int32_t* genomes, const int32_t* lengths,
         q.consts = consts; q.n_consts = n_consts; q.d = d; q.tmem_slots = tp.tmem_slots; q.k_rcp = tp.k_rcp; q.k_un = tp.k_un; q.un_row_bytes = npad * 4;
         q.hdr = w.hdr; q.uops = w.uops; q.ucap = w.cap_U; q.meta = w.meta; q.depth = w.depth;
         q.slow_list = w.slow_list; q.gen_list = w.slow_list + w.cap_P; q.fitness = fitness; q.outputs = outputs; q.n_cases = N; q.emit = emit ? 1 : 0;
-        k_compile<<<(unsigned)((P + kCompileThreads - 1) / kCompileThreads), kCompileThreads, 0, st>>>(q);
+        // the previous call's count of f1 programs, copied to pinned memory without a synchronisation: possibly stale, only a
+        // guess at which instantiation is faster for this colony
+        if (*w.h_f1 > 0) k_compile<true><<<(unsigned)((P + kCompileThreads - 1) / kCompileThreads), kCompileThreads, 0, st>>>(q);
+        else k_compile<false><<<(unsigned)((P + kCompileThreads - 1) / kCompileThreads), kCompileThreads, 0, st>>>(q);
         long long gb = (P + kCompileThreads - 1) / kCompileThreads;
         const long long gcap = (long long)w.num_sms * 8;       // (an empty list costs the launch of these blocks: 8 us at 16 per SM, 3 at 4)
         k_compile_general<<<(unsigned)(gb > gcap ? gcap : gb), kCompileThreads, 0, st>>>(q);
@@ -708,7 +718,8 @@ static beagle_status run_eval(const int32_t* genomes, const int32_t* lengths, co
     if (prof) { CU(cudaEventRecord(w.ev_k[2 * w.prof_n + 1], st)); ++w.prof_n; }
     // slow path: individuals whose micro-ops did not fit the promised workspace (normally none)
     k_eval_blockwise<<<w.num_sms * 2, (N + 31) / 32 * 32, 0, st>>>(genomes, w.off, lengths, w.depth, consts, X, y, N, d, tax,
-                                                                   fitness, outputs, w.slow_list, &w.hdr->n_slow, P, fit.kind, fit.M, fit.power);
+                                                                   fitness, outputs, w.slow_list, &w.hdr->n_slow, P, fit.kind, fit.M, fit.power,
+                                                                   &w.hdr->n_f1, w.h_f1);
     ++g_launches;
     CU(cudaGetLastError());
     return BEAGLE_OK;
@@ -727,7 +738,7 @@ static beagle_status run_colony(const int32_t* genomes, const int32_t* lengths, 
     if (s != BEAGLE_OK) return s;
     if (fast) return run_eval(genomes, lengths, consts, X, y, P, N, d, tax, fitness, outputs, fit, st);
     k_eval_blockwise<<<(unsigned)P, (N + 31) / 32 * 32, 0, st>>>(genomes, w.off, lengths, w.depth, consts, X, y, N, d, tax,
-                                                                fitness, outputs, nullptr, nullptr, P, fit.kind, fit.M, fit.power);
+                                                                fitness, outputs, nullptr, nullptr, P, fit.kind, fit.M, fit.power, nullptr, nullptr);
     ++g_launches;
     CU(cudaGetLastError());
     return BEAGLE_OK;
@@ -841,7 +852,7 @@ beagle_status beagle_eval_blockwise(const int32_t* genomes, const int32_t* lengt
     if ((s = run_prepass(genomes, lengths, P, consts, n_consts, X, y, N, d, fitness_out, nullptr, -1, false, kFitMse, st)) != BEAGLE_OK) return s;
     const int threads = (N + 31) / 32 * 32;
     k_eval_blockwise<<<(unsigned)P, threads, 0, st>>>(genomes, w.off, lengths, w.depth, consts, X, y, N, d, tax,
-                                                      fitness_out, nullptr, nullptr, nullptr, P, BEAGLE_FIT_MSE, 0.f, 1);
+                                                      fitness_out, nullptr, nullptr, nullptr, P, BEAGLE_FIT_MSE, 0.f, 1, nullptr, nullptr);
     ++g_launches;
     CU(cudaGetLastError());
     return BEAGLE_OK;
