@@ -75,6 +75,7 @@ struct Header {                                // device-resident results of the
     int n_f1;                                  // individuals compiled with DUP SWAP DEL SIGN SQUARE CUBE (picks k_compile<F1> next time)
     int n_malformed;
     unsigned int queue;                        // work-queue cursor of the interpreter kernel
+    unsigned int queue2;                       // ... of the second launch of a split call
     unsigned int rcp_unsafe;                   // bit j: some case of variable j has |x| < 1e-6f (its division is protected)
 };
 
@@ -88,6 +89,13 @@ struct EvalParams {
     int slot_col0;      // first tensor-memory column of the slot blocks
     int tmem_slots;     // S_T: slots per warp held in tensor memory (the deeper ones are in local memory)
     int off_ys, off_meta, off_un, off_ring;   // shared-memory layout, byte offsets: y (and centred y), queue windows, unary rows, rings
+    // a call with 513..1024 cases and the MSE fitness is SPLIT into one launch per pass of 512 cases: a launch then stages one
+    // pass's variable rows, which leaves a slot row more per warp (half as many pushes go to local memory)
+    int pass0, npass;   // first pass and number of passes this launch covers
+    int un_w;           // cases per staged unary row: all padded cases, or 512 in a split call
+    int ung_off;        // offset of this launch's rows in ung[]
+    int pmode;          // 0: one launch does everything; 1 | 2: first | second launch of a split call (interp.cuh)
+    float* partial;     // split call: the lanes' sums after pass 0, 32 floats per individual
 };
 
 // ---- PTX helpers: mbarrier, TMA bulk copy -----------------------------------------------------------
@@ -150,7 +158,7 @@ __global__ void __launch_bounds__(1024) k_len_pass2(long long* __restrict__ bsum
                                                     int* __restrict__ bins, int* __restrict__ cursor,
                                                     int* __restrict__ binstart, long long* __restrict__ binubase,
                                                     const float* __restrict__ X, const float* __restrict__ y,
-                                                    int n, int d, int npad, float* __restrict__ xt, float* __restrict__ ung)
+                                                    int n, int d, int npad, float* __restrict__ xt, float* __restrict__ ung, int split)
 {
     __shared__ long long wtot[32];
     __shared__ long long carry_s;
@@ -224,7 +232,7 @@ __global__ void __launch_bounds__(1024) k_len_pass2(long long* __restrict__ bsum
         hdr->n_sorted = (int)carry2_s;
         hdr->max_len = maxlen_s;
         hdr->n_slow = 0; hdr->n_malformed = 0; hdr->n_general = 0; hdr->n_f1 = 0;
-        hdr->queue = 0;
+        hdr->queue = 0; hdr->queue2 = 0;
         hdr->rcp_unsafe = unsafe_s;
     }
     // transpose: xt[j][i] = X[i][j] (j < d), xt[d][i] = y[i]; cases i >= n are zero
@@ -234,8 +242,10 @@ __global__ void __launch_bounds__(1024) k_len_pass2(long long* __restrict__ bsum
         if (i < n) v = (j < d) ? X[(size_t)i * d + j] : (y ? y[i] : 0.f);
         xt[e] = v;
         if (j < d) {                               // the unary rows f(X[j]) (uop.cuh H_LS / H_LG), the handlers' own functions
-            const size_t fs = (size_t)d * npad;
-            ung[e] = op_sin(v); ung[fs + e] = op_cos(v); ung[2 * fs + e] = op_log(v); ung[3 * fs + e] = op_sqrt(v); ung[4 * fs + e] = op_exp(v);
+            // layout: ung[(f * d + j) * npad + i]; in a split call one block of 5 d rows of 512 cases per pass
+            const size_t fs = split ? (size_t)d * kCasesPerPass : (size_t)d * npad;
+            const size_t b = split ? (size_t)(i / kCasesPerPass) * 5 * fs + (size_t)j * kCasesPerPass + (i % kCasesPerPass) : (size_t)e;
+            ung[b] = op_sin(v); ung[fs + b] = op_cos(v); ung[2 * fs + b] = op_log(v); ung[3 * fs + b] = op_sqrt(v); ung[4 * fs + b] = op_exp(v);
         }
     }
 }
@@ -435,7 +445,7 @@ struct Workspace {
     long long cap_P = 0, cap_U = 0;            // individuals / micro-op entries the workspace holds
     long long promised_P = 0, promised_T = 0;  // beagle_reserve: calls with P <= promised_P have T <= promised_T
     long long* off = nullptr; int* depth = nullptr; int4* meta = nullptr; int4* sched = nullptr;
-    int* slow_list = nullptr; long long* bsum = nullptr;
+    int* slow_list = nullptr; long long* bsum = nullptr; float* partial = nullptr;
     uint2* uops = nullptr;
     int* bins = nullptr; int* cursor = nullptr; int* binstart = nullptr; long long* binubase = nullptr;
     float* xt = nullptr; float* ung = nullptr; Header* hdr = nullptr; long long* h_T = nullptr; int* h_f1 = nullptr;
@@ -496,9 +506,9 @@ static beagle_status reserve_P(long long P)
     if (P <= w.cap_P) return BEAGLE_OK;
     CU(cudaDeviceSynchronize());
     cudaFree(w.off); cudaFree(w.depth); cudaFree(w.meta); cudaFree(w.sched);
-    cudaFree(w.slow_list); cudaFree(w.bsum);
+    cudaFree(w.slow_list); cudaFree(w.bsum); cudaFree(w.partial);
     w.off = nullptr; w.depth = nullptr; w.meta = nullptr; w.sched = nullptr;
-    w.slow_list = nullptr; w.bsum = nullptr; w.cap_P = 0;
+    w.slow_list = nullptr; w.bsum = nullptr; w.partial = nullptr; w.cap_P = 0;
     (void)cudaGetLastError();                      // the frees are best effort: their status is not the call's
     const long long nb = (P + kScanBlock - 1) / kScanBlock;
     CU(cudaMalloc(&w.off, sizeof(long long) * (P + 1)));
@@ -507,6 +517,7 @@ static beagle_status reserve_P(long long P)
     CU(cudaMalloc(&w.meta, sizeof(int4) * P));
     CU(cudaMalloc(&w.slow_list, sizeof(int) * 2 * P));       // + the list of k_compile_general
     CU(cudaMalloc(&w.bsum, sizeof(long long) * (nb + 1)));
+    CU(cudaMalloc(&w.partial, sizeof(float) * 32 * P));              // split calls (more than 512 cases): the lanes' sums after pass 0
     w.cap_P = P;
     return BEAGLE_OK;
 }
@@ -533,11 +544,11 @@ static long long uop_entries_bound(long long P, long long T) { return T + 4 * P 
 // quarter (8, 7 or 6: 1024, 896 or 768 threads) is chosen so that three slot rows per warp remain when
 // possible. fast == false: the variable block alone does not fit (d > 32 at N <= 512, d > 16 beyond), and the
 // call takes the blockwise kernel.
-struct TmemPlan { bool fast; int threads; int rcp_col0; int k_rcp; int slot_col0; int tmem_slots; int k_un; int ring_bytes; size_t smem; int off_ys, off_meta, off_un, off_ring; };
-static TmemPlan tmem_plan(int N, int d, int fit_kind)
+struct TmemPlan { bool split; bool fast; int threads; int rcp_col0; int k_rcp; int slot_col0; int tmem_slots; int k_un; int ring_bytes; size_t smem; int off_ys, off_meta, off_un, off_ring; };
+static TmemPlan tmem_plan(int N, int d, int fit_kind, bool split)
 {
-    TmemPlan t = { false, kEvalThreads, 0, 0, 0, 0, 0, 0, 0 };
-    const int passes = (N + kCasesPerPass - 1) / kCasesPerPass;
+    TmemPlan t = { split, false, kEvalThreads, 0, 0, 0, 0, 0, 0, 0 };
+    const int passes = split ? 1 : (N + kCasesPerPass - 1) / kCasesPerPass;      // passes a launch stages
     const int rows = kTmemCols / kCasesPerLane;                  // 32
     const int xrows = passes * d;
     if (xrows > rows) return t;
@@ -572,9 +583,10 @@ static TmemPlan tmem_plan(int N, int d, int fit_kind)
     const long long fixed = ((64 + warps * kStagesMax * 8 + 127) & ~127) + (long long)npad * 4 * (fit_kind == BEAGLE_FIT_CORRELATION ? 2 : 1)
                             + (long long)kEvalMetaBytes * warps;      // correlation: y and the centred y (eval_kernel.inc)
     const long long spare = (long long)g_ws.smem_optin - fixed - (long long)warps * ((kStageBytesMax + 127) & ~127);
-    long long ku = spare / (5ll * npad * 4);
+    const int un_w = split ? kCasesPerPass : npad;
+    long long ku = spare / (5ll * un_w * 4);
     t.k_un = (int)(ku < 0 ? 0 : (ku > d ? d : ku));
-    const long long un_bytes = 5ll * t.k_un * npad * 4;
+    const long long un_bytes = 5ll * t.k_un * un_w * 4;
     long long ring = ((g_ws.smem_optin - fixed - un_bytes) / warps) & ~127ll;
     if (ring > (long long)kStagesMax * kStageBytesMax) ring = (long long)kStagesMax * kStageBytesMax;
     t.ring_bytes = (int)ring;
@@ -583,6 +595,18 @@ static TmemPlan tmem_plan(int N, int d, int fit_kind)
     t.off_meta = (int)(fixed - (long long)kEvalMetaBytes * warps);
     t.off_un = (int)fixed; t.off_ring = (int)(fixed + un_bytes);
     return t;
+}
+
+// A call with 513..1024 cases that ends in the grouped MSE interpreter (no per-case outputs, no other fitness function) is
+// split into one launch per pass (EvalParams::pmode); everything else stages all passes in one launch.
+static TmemPlan plan_for(int N, int d, const FitSel& fit, bool mse_fitness_only)
+{
+    const TmemPlan whole = tmem_plan(N, d, fit.kind, false);
+    if (!(N > kCasesPerPass && fit.kind == BEAGLE_FIT_MSE && mse_fitness_only)) return whole;
+    // worth a second launch only where it buys slot rows (or makes the variable block fit at all): config 4's 9 variables
+    // leave 2 slot rows per warp in one launch and 3 in two; config 2's 3 variables leave 3 either way
+    const TmemPlan split = tmem_plan(N, d, fit.kind, true);
+    return (!whole.fast || split.tmem_slots > whole.tmem_slots) ? split : whole;
 }
 
 static beagle_status check_args(const void* genomes, const void* lengths, int64_t P, const void* consts,
@@ -646,7 +670,7 @@ static beagle_status run_prepass(const int32_t* genomes, const int32_t* lengths,
         CU(cudaEventRecord(w.ev_p[w.prof_n], st));
     }
     k_len_pass1<<<nb, kScanThreads, 0, st>>>(lengths, P, w.bsum, w.bins);
-    k_len_pass2<<<1, 1024, 0, st>>>(w.bsum, nb, w.hdr, w.bins, w.cursor, w.binstart, w.binubase, X, y, N, d, npad, w.xt, w.ung);
+    k_len_pass2<<<1, 1024, 0, st>>>(w.bsum, nb, w.hdr, w.bins, w.cursor, w.binstart, w.binubase, X, y, N, d, npad, w.xt, w.ung, plan_for(N, d, fit, fitness && !outputs).split ? 1 : 0);
     g_launches += 2;
     if (emit && w.need_T_readback) {               // ready_or_grow: the one read-back of an un-reserved call
         w.need_T_readback = false;
@@ -661,8 +685,8 @@ static beagle_status run_prepass(const int32_t* genomes, const int32_t* lengths,
     {
         CompileParams q;
         q.genomes = reinterpret_cast<const uint32_t*>(genomes); q.sched = w.sched;
-        const TmemPlan tp = tmem_plan(N, d, fit.kind);
-        q.consts = consts; q.n_consts = n_consts; q.d = d; q.tmem_slots = tp.tmem_slots; q.k_rcp = tp.k_rcp; q.k_un = tp.k_un; q.un_row_bytes = npad * 4;
+        const TmemPlan tp = plan_for(N, d, fit, fitness && !outputs);
+        q.consts = consts; q.n_consts = n_consts; q.d = d; q.tmem_slots = tp.tmem_slots; q.k_rcp = tp.k_rcp; q.k_un = tp.k_un; q.un_row_bytes = (tp.split ? kCasesPerPass : npad) * 4;
         q.hdr = w.hdr; q.uops = w.uops; q.ucap = w.cap_U; q.meta = w.meta; q.depth = w.depth;
         q.slow_list = w.slow_list; q.gen_list = w.slow_list + w.cap_P; q.fitness = fitness; q.outputs = outputs; q.n_cases = N; q.emit = emit ? 1 : 0;
         // the previous call's count of f1 programs, copied to pinned memory without a synchronisation: possibly stale, only a
@@ -685,7 +709,7 @@ static beagle_status run_eval(const int32_t* genomes, const int32_t* lengths, co
     Workspace& w = g_ws;
     const int npad = (N + kCasePad - 1) / kCasePad * kCasePad;
     EvalParams prm;
-    const TmemPlan tp = tmem_plan(N, d, fit.kind);
+    const TmemPlan tp = plan_for(N, d, fit, fitness && !outputs);
     if (!tp.fast) return BEAGLE_ERR_UNSUPPORTED;   // callers check first
     prm.rcp_col0 = tp.rcp_col0; prm.k_rcp = tp.k_rcp; prm.slot_col0 = tp.slot_col0; prm.tmem_slots = tp.tmem_slots;
     prm.meta = w.meta; prm.uops = w.uops; prm.hdr = w.hdr; prm.xt = w.xt; prm.ung = w.ung;
@@ -701,6 +725,9 @@ static beagle_status run_eval(const int32_t* genomes, const int32_t* lengths, co
     prm.off_ys = tp.off_ys; prm.off_meta = tp.off_meta; prm.off_un = tp.off_un; prm.off_ring = tp.off_ring;
     if (prm.ring_bytes < kStageBytesMax) return BEAGLE_ERR_UNSUPPORTED;
     prm.queue = &w.hdr->queue;
+    const int passes_all = (N + kCasesPerPass - 1) / kCasesPerPass;
+    prm.pass0 = 0; prm.npass = tp.split ? 1 : passes_all; prm.un_w = tp.split ? kCasesPerPass : npad; prm.ung_off = 0;
+    prm.pmode = tp.split ? 1 : 0; prm.partial = w.partial;
     // programmatic dependent launch: k_eval's prologue (tensor-memory allocation, staging of X, y and the unary rows)
     // overlaps the tail of k_compile, which releases its dependents at its start; k_eval waits (griddepcontrol.wait)
     // before it touches the compiler's output
@@ -715,6 +742,12 @@ static beagle_status run_eval(const int32_t* genomes, const int32_t* lengths, co
     else if (outputs || !fitness) CU(cudaLaunchKernelEx(&cfg, k_eval<BEAGLE_FIT_MSE, false>, prm));
     else CU(cudaLaunchKernelEx(&cfg, k_eval<BEAGLE_FIT_MSE, true>, prm));
     ++g_launches;
+    if (tp.split) {                                // the second pass: its own variable rows, the lanes' sums taken back
+        prm.pass0 = 1; prm.pmode = 2; prm.ung_off = 5 * d * kCasesPerPass; prm.queue = &w.hdr->queue2;
+        cfg.numAttrs = 0;
+        CU(cudaLaunchKernelEx(&cfg, k_eval<BEAGLE_FIT_MSE, true>, prm));
+        ++g_launches;
+    }
     if (prof) { CU(cudaEventRecord(w.ev_k[2 * w.prof_n + 1], st)); ++w.prof_n; }
     // slow path: individuals whose micro-ops did not fit the promised workspace (normally none)
     k_eval_blockwise<<<w.num_sms * 2, (N + 31) / 32 * 32, 0, st>>>(genomes, w.off, lengths, w.depth, consts, X, y, N, d, tax,
@@ -733,7 +766,7 @@ static beagle_status run_colony(const int32_t* genomes, const int32_t* lengths, 
                                 float* fitness, float* outputs, long long T_known, const FitSel& fit, cudaStream_t st)
 {
     Workspace& w = g_ws;
-    const bool fast = tmem_plan(N, d, fit.kind).fast;
+    const bool fast = plan_for(N, d, fit, fitness && !outputs).fast;
     beagle_status s = run_prepass(genomes, lengths, P, consts, n_consts, X, y, N, d, fitness, outputs, T_known, fast, fit, st);
     if (s != BEAGLE_OK) return s;
     if (fast) return run_eval(genomes, lengths, consts, X, y, P, N, d, tax, fitness, outputs, fit, st);
@@ -775,7 +808,7 @@ static beagle_status eval_impl(const int32_t* genomes, const int32_t* lengths, i
     if (P == 0) return BEAGLE_OK;
     if ((s = init_once()) != BEAGLE_OK) return s;
     cudaStream_t st = (cudaStream_t)stream;
-    if ((s = ready_or_grow(P, -1, tmem_plan(N, d, fit.kind).fast, st)) != BEAGLE_OK) return s;
+    if ((s = ready_or_grow(P, -1, plan_for(N, d, fit, true).fast, st)) != BEAGLE_OK) return s;
     return run_colony(genomes, lengths, P, consts, n_consts, X, y, N, d, tax, fitness_out, nullptr, -1, fit, st);
 }
 
@@ -832,7 +865,7 @@ beagle_status beagle_debug_outputs(const int32_t* genomes, const int32_t* length
     if (P == 0) return BEAGLE_OK;
     if ((s = init_once()) != BEAGLE_OK) return s;
     cudaStream_t st = (cudaStream_t)stream;
-    if ((s = ready_or_grow(P, -1, tmem_plan(N, d, BEAGLE_FIT_MSE).fast, st)) != BEAGLE_OK) return s;
+    if ((s = ready_or_grow(P, -1, plan_for(N, d, kFitMse, false).fast, st)) != BEAGLE_OK) return s;
     return run_colony(genomes, lengths, P, consts, n_consts, X, nullptr, N, d, 0.f, nullptr, out_PxN, -1, kFitMse, st);
 }
 
@@ -982,7 +1015,7 @@ static beagle_status eval_chunked_impl(const int32_t* h_genomes, const int32_t* 
             CU(cudaMemcpyAsync(d_tok, h_genomes + tok0, sizeof(int32_t) * ntok, cudaMemcpyHostToDevice, w.copy_stream));
         CU(cudaEventRecord(w.ev_copied[b], w.copy_stream));
         CU(cudaStreamWaitEvent(st, w.ev_copied[b], 0));
-        if ((s = ready_or_grow(np, ntok, tmem_plan(N, d, fit.kind).fast, st)) != BEAGLE_OK) return s;     // (reserved: a no-op)
+        if ((s = ready_or_grow(np, ntok, plan_for(N, d, fit, true).fast, st)) != BEAGLE_OK) return s;     // (reserved: a no-op)
         if ((s = run_colony(d_tok, d_len, np, w.stage_consts, n_consts, X, y, N, d, tax, fitness_out + p0, nullptr, ntok, fit, st)) != BEAGLE_OK) return s;
         CU(cudaEventRecord(w.ev_free[b], st));
         total_launches += g_launches; g_launches = 0;
@@ -1035,7 +1068,7 @@ void beagle_release(void)
     Workspace& w = g_ws;
     cudaDeviceSynchronize();
     cudaFree(w.off); cudaFree(w.depth); cudaFree(w.meta); cudaFree(w.sched);
-    cudaFree(w.slow_list); cudaFree(w.bsum); cudaFree(w.uops);
+    cudaFree(w.slow_list); cudaFree(w.bsum); cudaFree(w.uops); cudaFree(w.partial); w.partial = nullptr;
     cudaFree(w.stage[0]); cudaFree(w.stage_consts); cudaFree(w.rank_hist); w.rank_hist = nullptr;
     (void)cudaGetLastError();
     w.off = nullptr; w.depth = nullptr; w.meta = nullptr; w.sched = nullptr;

@@ -236,6 +236,10 @@
 // pass of the variable / reciprocal block, %11 = n - 4 * lane (a case k of 128-case block g of pass s counts when
 // 512 s + 128 g + k < that), %12 = (float)n, %13 = 1 / n when n is a power of two (the mean is then an exact scaling,
 // bit-identical to the division), else 0, %14 tax, %15 fitness, %16 != 0: this lane stores (lane 0), %17 = n.
+// A call with more than 512 cases is SPLIT into one launch per pass (eval_kernel.inc): %18 = the lanes' parked sums
+// (32 floats per individual), %19 = 0 one launch does everything, 1 the launch of pass 0 (parks the sums), 2 the launch
+// of pass 1 (takes them back before its own residuals: the lane's chain of fma continues as if there had been one launch),
+// %20 = 4 * lane.
 #define BGI_SQ(k)   "sub.rn.f32 t" #k ", " BGI_A #k ", x" #k ";\n" "fma.rn.f32 sum, t" #k ", t" #k ", sum;\n"
 #define BGI_SQR(k, LIM) "setp.lt.s32 p" #k ", " LIM ", nrem;\n" "sub.rn.f32 t" #k ", " BGI_A #k ", x" #k ";\n" "@p" #k " fma.rn.f32 sum, t" #k ", t" #k ", sum;\n"
 #define BGI_BFLY(M) "shfl.sync.bfly.b32 cv, sum, " #M ", 0x1f, 0xffffffff;\n" "add.rn.f32 sum, sum, cv;\n"
@@ -246,6 +250,11 @@
     "ld.shared.v4.f32 {x12, x13, x14, x15}, [ya+1536];\n"
 #define BGI_END_GROUP \
     "L_END_%=:\n" \
+    "setp.eq.u32 pr, %19, 2;\n"                   /* second launch of a split call: the lane's sum of pass 0 comes back */ \
+    "@!pr bra.uni NOPART_%=;\n" \
+    "mul.wide.u32 ma, o, 128;\n" "add.u64 ma, ma, %18;\n" "cvt.u64.u32 mb, %20;\n" "add.u64 ma, ma, mb;\n" \
+    "ld.global.f32 sum, [ma];\n" \
+    "NOPART_%=:\n" \
     BGI_LDY \
     "setp.lt.s32 pr, nleft, 512;\n"               /* a ragged last pass: the padded cases do not count */ \
     "@pr bra.uni RAG_%=;\n" \
@@ -266,6 +275,12 @@
     "ld.shared.v2.b32 {h, o}, [pc];\n" \
     "bra.uni DISP_%=;\n" \
     "FIN_%=:\n" \
+    "setp.eq.u32 pr, %19, 1;\n"                   /* first launch of a split call: park the lane's sum, no fitness yet */ \
+    "@!pr bra.uni FINAL_%=;\n" \
+    "mul.wide.u32 ma, o, 128;\n" "add.u64 ma, ma, %18;\n" "cvt.u64.u32 mb, %20;\n" "add.u64 ma, ma, mb;\n" \
+    "st.global.f32 [ma], sum;\n" \
+    "bra.uni NEXTP_%=;\n" \
+    "FINAL_%=:\n" \
     "ld.shared.f32 q0, [pc+8];\n"                 /* (float)L */ \
     BGI_BFLY(16) BGI_BFLY(8) BGI_BFLY(4) BGI_BFLY(2) BGI_BFLY(1) \
     "setp.neu.f32 pr, %13, 0f00000000;\n" \
@@ -279,6 +294,7 @@
     "mul.wide.u32 ma, o, 4;\n" "add.u64 ma, ma, %15;\n" \
     "setp.ne.u32 pr, %16, 0;\n" \
     "@pr st.global.f32 [ma], sum;\n" \
+    "NEXTP_%=:\n" \
     "sub.u32 gc, gc, 1;\n" \
     "setp.eq.u32 pr, gc, 0;\n" \
     "@pr bra.uni EXIT_%=;\n" \
@@ -294,7 +310,7 @@
     ".reg .pred p<16>, pr;\n" \
     ".reg .b32 h, o, hn, pc, pc0, xa, xb, rb, db, spt, e, ya, gc, ps;\n" \
     ".reg .s32 nrem, nleft;\n" \
-    ".reg .b64 ma, mbase, gb;\n" \
+    ".reg .b64 ma, mb, mbase, gb;\n" \
     ".local .align 16 .b8 slotmem[1984];\n" \
     BGI_TABLE \
     "mov.u32 pc, %0;\n" "mov.u32 pc0, %0;\n" \
@@ -324,14 +340,14 @@ __device__ __forceinline__ void interp_run(uint32_t rec, uint32_t xb, uint32_t s
 // a group of `count` programs whose record blocks follow one another from `rec` on, every pass, fitness[p] stored
 struct GroupArgs {
     uint32_t xb, sb, rb, db; const float* gb; uint32_t ya; uint32_t passes, xstride, rstride; int nrem;
-    float nf, inv_n, tax; float* fitness; uint32_t lane0; int n;
+    float nf, inv_n, tax; float* fitness; uint32_t lane0; int n; float* partial; uint32_t pmode, lane4;
 };
 #define BGI_A "a"
 __device__ __forceinline__ void interp_group(uint32_t rec, uint32_t count, const GroupArgs& g)
 {
     asm volatile(BGI_ASM_GROUP :: "r"(rec), "r"(g.xb), "r"(g.sb), "r"(g.rb), "r"(g.db), "l"(g.gb), "r"(g.ya), "r"(count),
                  "r"(g.passes), "r"(g.xstride), "r"(g.rstride), "r"(g.nrem), "f"(g.nf), "f"(g.inv_n), "f"(g.tax), "l"(g.fitness),
-                 "r"(g.lane0), "r"(g.n) : "memory");
+                 "r"(g.lane0), "r"(g.n), "l"(g.partial), "r"(g.pmode), "r"(g.lane4) : "memory");
 }
 #undef BGI_A
 
