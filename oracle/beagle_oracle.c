@@ -32,8 +32,9 @@
  * P6 commutativity/antisymmetry, P7 protected-operator edge table, P8 brute force of all programs
  * of <= 3 tokens against an independent recursive evaluator (oracle/infix_check.py), P9 power-of-two
  * scaling, P10 overflow semantics, P11 the bound is a bound (fp32 mirror), P12 case duplication.
- * P13-P18 the rest of Table 3, P19 the correlation fitness (orc_eval_corr).
- * Parity unpinned: nothing on the hot path.
+ * P13-P18 the rest of Table 3 (P17b: the corner bound of POW is a bound), P19 the correlation fitness (orc_eval_corr),
+ * P21 / P21b the Std family (orc_eval_std: Eq. 5 by hand; its bound E is a bound).
+ * Parity unpinned: nothing (every value and every bound the parity rule uses has a pin of its own).
  */
 #include <float.h>
 #include <math.h>
