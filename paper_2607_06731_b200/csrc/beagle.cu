@@ -478,7 +478,9 @@ static beagle_status init_once()
     w.smem_optin = (int)prop.sharedMemPerBlockOptin;
     w.device_ok = (prop.major == 10);
     if (!w.device_ok) { w.inited = true; return BEAGLE_ERR_UNSUPPORTED; }
-    CU(cudaFuncSetAttribute(k_eval<BEAGLE_FIT_MSE, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, w.smem_optin));
+    CU(cudaFuncSetAttribute(k_eval<BEAGLE_FIT_MSE, true, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, w.smem_optin));
+    CU(cudaFuncSetAttribute(k_eval<BEAGLE_FIT_MSE, true, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, w.smem_optin));
+    CU(cudaFuncSetAttribute(k_eval<BEAGLE_FIT_MSE, true, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, w.smem_optin));
     CU(cudaFuncSetAttribute(k_eval<BEAGLE_FIT_MSE, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, w.smem_optin));
     CU(cudaFuncSetAttribute(k_eval<BEAGLE_FIT_CORRELATION, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, w.smem_optin));
     CU(cudaFuncSetAttribute(k_eval<BEAGLE_FIT_STD, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, w.smem_optin));
@@ -740,12 +742,13 @@ static beagle_status run_eval(const int32_t* genomes, const int32_t* lengths, co
     if (fit.kind == BEAGLE_FIT_CORRELATION) CU(cudaLaunchKernelEx(&cfg, k_eval<BEAGLE_FIT_CORRELATION, false>, prm));
     else if (fit.kind == BEAGLE_FIT_STD) CU(cudaLaunchKernelEx(&cfg, k_eval<BEAGLE_FIT_STD, false>, prm));
     else if (outputs || !fitness) CU(cudaLaunchKernelEx(&cfg, k_eval<BEAGLE_FIT_MSE, false>, prm));
-    else CU(cudaLaunchKernelEx(&cfg, k_eval<BEAGLE_FIT_MSE, true>, prm));
+    else if (tp.split) CU(cudaLaunchKernelEx(&cfg, k_eval<BEAGLE_FIT_MSE, true, 1>, prm));
+    else CU(cudaLaunchKernelEx(&cfg, k_eval<BEAGLE_FIT_MSE, true, 0>, prm));
     ++g_launches;
     if (tp.split) {                                // the second pass: its own variable rows, the lanes' sums taken back
         prm.pass0 = 1; prm.pmode = 2; prm.ung_off = 5 * d * kCasesPerPass; prm.queue = &w.hdr->queue2;
         cfg.numAttrs = 0;
-        CU(cudaLaunchKernelEx(&cfg, k_eval<BEAGLE_FIT_MSE, true>, prm));
+        CU(cudaLaunchKernelEx(&cfg, k_eval<BEAGLE_FIT_MSE, true, 2>, prm));
         ++g_launches;
     }
     if (prof) { CU(cudaEventRecord(w.ev_k[2 * w.prof_n + 1], st)); ++w.prof_n; }

@@ -340,14 +340,15 @@ __device__ __forceinline__ void interp_run(uint32_t rec, uint32_t xb, uint32_t s
 // a group of `count` programs whose record blocks follow one another from `rec` on, every pass, fitness[p] stored
 struct GroupArgs {
     uint32_t xb, sb, rb, db; const float* gb; uint32_t ya; uint32_t passes, xstride, rstride; int nrem;
-    float nf, inv_n, tax; float* fitness; uint32_t lane0; int n; float* partial; uint32_t pmode, lane4;
+    float nf, inv_n, tax; float* fitness; uint32_t lane0; int n; float* partial; uint32_t lane4;
 };
 #define BGI_A "a"
+template <int PMODE>                               // an immediate: ptxas folds the two tests of the END handler away
 __device__ __forceinline__ void interp_group(uint32_t rec, uint32_t count, const GroupArgs& g)
 {
     asm volatile(BGI_ASM_GROUP :: "r"(rec), "r"(g.xb), "r"(g.sb), "r"(g.rb), "r"(g.db), "l"(g.gb), "r"(g.ya), "r"(count),
                  "r"(g.passes), "r"(g.xstride), "r"(g.rstride), "r"(g.nrem), "f"(g.nf), "f"(g.inv_n), "f"(g.tax), "l"(g.fitness),
-                 "r"(g.lane0), "r"(g.n), "l"(g.partial), "r"(g.pmode), "r"(g.lane4) : "memory");
+                 "r"(g.lane0), "r"(g.n), "l"(g.partial), "n"(PMODE), "r"(g.lane4) : "memory");
 }
 #undef BGI_A
 
