@@ -54,7 +54,7 @@ def test_parity_blockwise_baseline(oracle, number):
     _check(col, oracle, fit)
 
 
-@pytest.mark.parametrize("number,stride", [(3, 401), (4, 1601)])
+@pytest.mark.parametrize("number,stride", [(3, 41), (4, 161)])
 def test_parity_full_size_sampled(oracle, number, stride):
     """BASELINE.json's full sizes in the configuration bench.py times; the oracle checks every
     `stride`-th individual plus the longest and the deepest ones."""
@@ -62,7 +62,7 @@ def test_parity_full_size_sampled(oracle, number, stride):
     col = colonies.make_colony(number)
     fit = gpu_eval(col.genomes, col.lengths, col.consts, col.X, col.y, col.tax)
     sel = np.arange(0, col.P, stride)
-    longest = np.argsort(-col.lengths, kind="stable")[:256]
+    longest = np.argsort(-col.lengths, kind="stable")[:2048]
     sel = np.unique(np.concatenate([sel, longest]))
     _check(col, oracle, fit, sel)
     # properties that hold at any size: every individual got a value; tax*L is a lower bound of
@@ -74,7 +74,8 @@ def test_parity_full_size_sampled(oracle, number, stride):
 
 def test_parity_config5_chunked_sampled(oracle):
     """Config 5's mechanism (chunked streaming from pinned host memory under a device budget) at a
-    reduced population; the budget is scaled so that the same number of chunks (~3) results."""
+    reduced population and a budget of 0.8 of its tokens (two staging buffers, three chunks); config 5 at its own size and
+    budget: tests/test_gpu_prepass_and_chunks.py::test_config5_as_configured."""
     from tests.gpu_util import gpu_eval_chunked, gpu_eval
     col = colonies.make_colony(5, 262144)
     budget = int(col.T * 4 * 0.8) & ~255
