@@ -242,3 +242,30 @@ def test_stack_commands_run_on_the_interpreter(oracle, N, d):
     orc = oracle.evaluate_parallel(g, l, c, X, y, 0.001)
     rep = parity.compare(a, orc)
     assert len(rep["bad"]) == 0, parity.describe(rep, a, orc)
+
+
+@pytest.mark.parametrize("N,d", [(513, 9), (700, 12), (1000, 20), (1023, 32), (1024, 17)])
+def test_split_passes_ragged_and_wide(oracle, N, d):
+    """Calls with more than 512 cases whose variable rows crowd the slot rows are split into one interpreter launch per pass
+    (DESIGN.md §7): ragged second passes, variable counts that fit tensor memory only when split (d > 16), deep stacks;
+    bit-identical to the blockwise kernel, parity with the oracle, and bitwise equal to the per-case outputs' own sum order
+    (the chunked call, which cuts the colony differently, gives the same bits)."""
+    from tests.gpu_util import gpu_eval, gpu_eval_chunked
+    from tests.util import random_gcl_programs
+    rng = np.random.default_rng(1000 + N + d)
+    X = rng.uniform(-3, 3, (N, d)).astype(np.float32)
+    y = (X[:, 0] * X[:, d - 1] - np.cos(X[:, d // 2])).astype(np.float32)
+    names = ["ADD", "SUB", "MUL", "DIV", "SIN", "COS", "LOG", "SQRT", "EXP", "SQUARE", "DUP", "SWAP"]
+    texts = random_gcl_programs(rng, 1500, d, names)
+    deep = " ".join(f"x{j % d} SIN" for j in range(20)) + " ADD" * 19          # 20 computed values waiting: slots in local memory
+    consts = []
+    progs = [asm(t, consts)[0] for t in texts + [deep] * 8]
+    g, l, c = pack(progs, consts)
+    a = gpu_eval(g, l, c, X, y, 0.001)
+    b = gpu_eval(g, l, c, X, y, 0.001, fn="beagle_eval_blockwise")
+    assert np.array_equal(_bits(a), _bits(b))
+    ch = gpu_eval_chunked(g, l, c, X, y, 0.001, 64 << 10)
+    assert np.array_equal(_bits(a), _bits(ch))
+    orc = oracle.evaluate_parallel(g, l, c, X, y, 0.001)
+    rep = parity.compare(a, orc)
+    assert len(rep["bad"]) == 0, parity.describe(rep, a, orc)
