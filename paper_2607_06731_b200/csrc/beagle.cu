@@ -350,12 +350,14 @@ __global__ void __launch_bounds__(1024) k_eval_blockwise(
     const int* __restrict__ depth, const float* __restrict__ consts, const float* __restrict__ X,
     const float* __restrict__ y, int n, int d, float tax, float* __restrict__ fitness, float* __restrict__ outputs,
     const int* __restrict__ list, const int* __restrict__ count, long long P, int fit, float M, int power,
-    const int* __restrict__ n_f1, int* __restrict__ h_f1)
+    const Header* __restrict__ hdr, int* __restrict__ h_f1)
 {
     __shared__ float res[BEAGLE_MAX_N];
     // the last kernel of a call tells the host (pinned, mapped memory) how many programs used the f1 commands: the next
     // call picks its k_compile instantiation by it (no copy, no synchronisation)
-    if (h_f1 && blockIdx.x == 0 && threadIdx.x == 0) *h_f1 = *n_f1;
+    // (h_f1[0] programs with f1 commands, [1] programs k_compile_general had to take, [2] programs on the slow list: the
+    // last two size the grids of those two kernels, which are launched whether their lists are empty or not)
+    if (h_f1 && blockIdx.x == 0 && threadIdx.x == 0) { h_f1[0] = hdr->n_f1; h_f1[1] = hdr->n_general; h_f1[2] = hdr->n_slow; }
     bool y_finite = true;
     if (fit == BEAGLE_FIT_CORRELATION) y_finite = __syncthreads_and(threadIdx.x >= n || finite32(__ldg(y + threadIdx.x)));
     const long long total = list ? (long long)*count : P;
@@ -496,8 +498,8 @@ static beagle_status init_once()
     CU(cudaMalloc(&w.hdr, sizeof(Header)));
     CU(cudaMemset(w.hdr, 0, sizeof(Header)));
     CU(cudaMallocHost(&w.h_T, sizeof(long long)));
-    CU(cudaMallocHost(&w.h_f1, sizeof(int)));
-    *w.h_f1 = 0;
+    CU(cudaMallocHost(&w.h_f1, 4 * sizeof(int)));
+    w.h_f1[0] = 0; w.h_f1[1] = 1; w.h_f1[2] = 1;   // the first call launches full grids
     w.inited = true;                               // only now: a failed allocation above is tried again by the next call
     return BEAGLE_OK;
 }
@@ -696,7 +698,9 @@ static beagle_status run_prepass(const int32_t* genomes, const int32_t* lengths,
         if (*w.h_f1 > 0) k_compile<true><<<(unsigned)((P + kCompileThreads - 1) / kCompileThreads), kCompileThreads, 0, st>>>(q);
         else k_compile<false><<<(unsigned)((P + kCompileThreads - 1) / kCompileThreads), kCompileThreads, 0, st>>>(q);
         long long gb = (P + kCompileThreads - 1) / kCompileThreads;
-        const long long gcap = (long long)w.num_sms * 8;       // (an empty list costs the launch of these blocks: 8 us at 16 per SM, 3 at 4)
+        // an empty list costs the launch of the blocks that would walk it (8 us at 16 per SM): a few blocks when the previous
+        // call's list was empty (the grid strides over the list, so a wrong guess only moves time)
+        const long long gcap = w.h_f1[1] > 0 ? (long long)w.num_sms * 8 : 8;
         k_compile_general<<<(unsigned)(gb > gcap ? gcap : gb), kCompileThreads, 0, st>>>(q);
         g_launches += 2;
     }
@@ -753,9 +757,9 @@ static beagle_status run_eval(const int32_t* genomes, const int32_t* lengths, co
     }
     if (prof) { CU(cudaEventRecord(w.ev_k[2 * w.prof_n + 1], st)); ++w.prof_n; }
     // slow path: individuals whose micro-ops did not fit the promised workspace (normally none)
-    k_eval_blockwise<<<w.num_sms * 2, (N + 31) / 32 * 32, 0, st>>>(genomes, w.off, lengths, w.depth, consts, X, y, N, d, tax,
+    k_eval_blockwise<<<w.h_f1[2] > 0 ? w.num_sms * 2 : 4, (N + 31) / 32 * 32, 0, st>>>(genomes, w.off, lengths, w.depth, consts, X, y, N, d, tax,
                                                                    fitness, outputs, w.slow_list, &w.hdr->n_slow, P, fit.kind, fit.M, fit.power,
-                                                                   &w.hdr->n_f1, w.h_f1);
+                                                                   w.hdr, w.h_f1);
     ++g_launches;
     CU(cudaGetLastError());
     return BEAGLE_OK;
