@@ -486,7 +486,8 @@ static beagle_status init_once()
     CU(cudaFuncSetAttribute(k_eval<BEAGLE_FIT_MSE, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, w.smem_optin));
     CU(cudaFuncSetAttribute(k_eval<BEAGLE_FIT_CORRELATION, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, w.smem_optin));
     CU(cudaFuncSetAttribute(k_eval<BEAGLE_FIT_STD, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, w.smem_optin));
-    { uint32_t lut[kLutSize]; make_compile_lut(lut); CU(cudaMemcpyToSymbol(g_compile_lut, lut, sizeof(lut))); }
+    { uint32_t lut[kW2Size]; uint2 tt[kTok2Size]; make_walk2_tabs(lut, tt);
+      CU(cudaMemcpyToSymbol(g_walk2_lut, lut, sizeof(lut))); CU(cudaMemcpyToSymbol(g_tok2, tt, sizeof(tt))); }
     CU(cudaMalloc(&w.bins, sizeof(int) * kNumBins));
     CU(cudaMalloc(&w.cursor, sizeof(int) * kNumBins));
     CU(cudaMemset(w.bins, 0, sizeof(int) * kNumBins));
