@@ -250,6 +250,21 @@ beagle_status beagle_debug_schedule(int64_t P, int64_t* off, int32_t* depth, int
  * room in the workspace); n_malformed: in-range individuals that are not programs (D3).               */
 beagle_status beagle_debug_counts(int32_t* n_sorted, int32_t* n_general, int32_t* n_slow, int32_t* n_malformed, void* stream);
 
+/* beagle_debug_plan — test only, HOST only, needs no device: the plan of tensor memory and shared memory (DESIGN.md section 7,
+ * "the plan of the 32 TMEM rows") that a call with N cases, d variables, fitness function `fit` (BEAGLE_FIT_*) and, for
+ * fitness_only != 0, no per-case outputs would get on a device with smem_optin bytes of opt-in shared memory per block.
+ * out12 (HOST): 0 fast (the interpreter takes the call; 0: the blockwise kernel), 1 split (one launch per pass of 512 cases),
+ * 2 threads per block, 3 variable rows, 4 reciprocal rows, 5 slot rows per warp, 6 variables with staged unary rows,
+ * 7 bytes of a warp's record ring, 8 dynamic shared memory in bytes, 9-11 byte offsets of y, the unary rows, the rings.
+ * BEAGLE_ERR_INVALID_ARG for arguments out of range. */
+beagle_status beagle_debug_plan(int32_t N, int32_t d, int32_t fit, int32_t fitness_only, int32_t smem_optin, int32_t* out12);
+
+/* beagle_debug_walk_tables — test only, HOST only: the two tables that drive the tree compiler's walk, as the device gets them:
+ * lut160 = 10 rows (nothing; SIN COS LOG SQRT EXP; ADD SUB MUL DIV) of 16 entries indexed by what the two topmost stack entries
+ * are (a computed? b computed? a a variable? b a variable?), tok130 = 65 pairs of words per opcode byte (64: past the end of the
+ * program). Either may be NULL. Field layout: compile_kernel.inc. */
+void beagle_debug_walk_tables(uint32_t* lut160, uint32_t* tok130);
+
 /* Limits compiled into the library (any pointer may be NULL). */
 void beagle_limits(int32_t* max_len, int32_t* max_stack, int32_t* max_n, int32_t* max_d);
 

@@ -1087,6 +1087,34 @@ void beagle_release(void)
 
 int32_t beagle_last_launch_count(void) { return g_launches; }
 
+// host only, no device needed: the plan of the 32 tensor-memory rows and of shared memory a call with these arguments would
+// get on a device with smem_optin bytes of opt-in shared memory per block
+beagle_status beagle_debug_plan(int32_t N, int32_t d, int32_t fit, int32_t fitness_only, int32_t smem_optin, int32_t* out12)
+{
+    int kind, power;
+    if (!out12 || !decode_fit(fit, &kind, &power) || N < 1 || N > BEAGLE_MAX_N || d < 1 || d > BEAGLE_MAX_D || smem_optin < 0)
+        return BEAGLE_ERR_INVALID_ARG;
+    const FitSel sel = { kind, 0.f, power };
+    const int saved = g_ws.smem_optin;
+    g_ws.smem_optin = smem_optin;
+    const TmemPlan tp = plan_for(N, d, sel, fitness_only != 0);
+    g_ws.smem_optin = saved;
+    const int passes = tp.split ? 1 : (N + kCasesPerPass - 1) / kCasesPerPass;
+    const int v[12] = { tp.fast ? 1 : 0, tp.split ? 1 : 0, tp.threads, passes * d, passes * tp.k_rcp, tp.tmem_slots, tp.k_un, tp.ring_bytes,
+                        (int)tp.smem, tp.off_ys, tp.off_un, tp.off_ring };
+    for (int i = 0; i < 12; ++i) out12[i] = v[i];
+    return BEAGLE_OK;
+}
+
+// host only: the two tables of the tree compiler's walk as the device gets them (compile_kernel.inc: make_walk2_tabs)
+void beagle_debug_walk_tables(uint32_t* lut160, uint32_t* tok130)
+{
+    uint32_t lut[kW2Size]; uint2 tt[kTok2Size];
+    make_walk2_tabs(lut, tt);
+    if (lut160) for (int i = 0; i < kW2Size; ++i) lut160[i] = lut[i];
+    if (tok130) for (int i = 0; i < kTok2Size; ++i) { tok130[2 * i] = tt[i].x; tok130[2 * i + 1] = tt[i].y; }
+}
+
 beagle_status beagle_debug_counts(int32_t* n_sorted, int32_t* n_general, int32_t* n_slow, int32_t* n_malformed, void* stream)
 {
     Header h;
