@@ -259,6 +259,14 @@ beagle_status beagle_debug_counts(int32_t* n_sorted, int32_t* n_general, int32_t
  * BEAGLE_ERR_INVALID_ARG for arguments out of range. */
 beagle_status beagle_debug_plan(int32_t N, int32_t d, int32_t fit, int32_t fitness_only, int32_t smem_optin, int32_t* out12);
 
+/* beagle_debug_chunk_plan — test only, HOST only, needs no device: the chunks beagle_eval_chunked would cut a colony with these
+ * HOST lengths into under this budget (the same code: the budget cut into K buffers, beagle_set_chunk_target; a chunk = as many
+ * whole individuals as fit one buffer at one word per individual plus one per token, three words spare). ends[i] (HOST, up to
+ * max_ends entries, may be NULL) = the index after the last individual of chunk i; *n_chunks, *n_buffers (K), *buffer_bytes: any may
+ * be NULL. BEAGLE_ERR_INVALID_ARG as beagle_eval_chunked for the same arguments. */
+beagle_status beagle_debug_chunk_plan(const int32_t* h_lengths, int64_t P, int64_t device_budget_bytes, int64_t* ends, int64_t max_ends,
+                                      int64_t* n_chunks, int32_t* n_buffers, int64_t* buffer_bytes);
+
 /* beagle_debug_walk_tables — test only, HOST only: the two tables that drive the tree compiler's walk, as the device gets them:
  * lut160 = 10 rows (nothing; SIN COS LOG SQRT EXP; ADD SUB MUL DIV) of 16 entries indexed by what the two topmost stack entries
  * are (a computed? b computed? a a variable? b a variable?), tok130 = 65 pairs of words per opcode byte (64: past the end of the

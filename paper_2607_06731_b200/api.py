@@ -42,6 +42,7 @@ _SIGNATURES = {
     "beagle_debug_schedule": (_i32, [_i64, _vp, _vp, _vp, _vp]),
     "beagle_debug_counts": (_i32, [ctypes.POINTER(_i32)] * 4 + [_vp]),
     "beagle_debug_plan": (_i32, [_i32, _i32, _i32, _i32, _i32, ctypes.POINTER(_i32)]),
+    "beagle_debug_chunk_plan": (_i32, [_vp, _i64, _i64, _vp, _i64, ctypes.POINTER(_i64), ctypes.POINTER(_i32), ctypes.POINTER(_i64)]),
     "beagle_debug_walk_tables": (None, [ctypes.POINTER(ctypes.c_uint32), ctypes.POINTER(ctypes.c_uint32)]),
     "beagle_limits": (None, [ctypes.POINTER(_i32)] * 4),
     "beagle_status_string": (ctypes.c_char_p, [_i32]),

@@ -803,6 +803,41 @@ static bool decode_fit(int32_t fit, int* kind, int* power)
     }
 }
 
+// ---- a8's host logic: how a budget is cut into staging buffers, and where a chunk ends (pure functions) -------------------
+// The budget is cut into K staging buffers of about g_stage_target bytes (2 <= K <= 8), each a multiple of 256 bytes; false: a
+// buffer could not hold one maximum-length individual.
+static bool stage_layout(long long budget, long long* K_out, long long* bytes_out)
+{
+    long long K = budget / g_stage_target;
+    K = K < 2 ? 2 : (K > kStageBufsMax ? kStageBufsMax : K);
+    const long long half = (budget / K) & ~255ll;
+    *K_out = K; *bytes_out = half;
+    return half >= 4ll * (BEAGLE_MAX_LEN + 1);
+}
+
+// The chunk that starts at individual p0 ends before individual p1 (returned): as many whole individuals as fit cap_words
+// words, one word per length plus one per token (a length outside 1..512 counts no tokens). *ntok: the chunk's tokens.
+static long long chunk_end(const int32_t* h_lengths, long long P, long long p0, long long cap_words, long long* ntok_out)
+{
+    long long words = 0, p1 = p0, ntok = 0;
+    // whole blocks of 4096 lengths first (a branch-free sum the host compiler vectorises: the scan of the first
+    // chunk is on the critical path, nothing is in flight yet), then one by one up to the boundary
+    while (p1 + 4096 <= P) {
+        long long bt = 0;
+        const int32_t* hl = h_lengths + p1;
+        for (int k = 0; k < 4096; ++k) { const int32_t v = hl[k]; bt += (v >= 1 && v <= BEAGLE_MAX_LEN) ? v : 0; }
+        if (words + bt + 4096 > cap_words) break;
+        words += bt + 4096; ntok += bt; p1 += 4096;
+    }
+    while (p1 < P) {
+        const int l = (h_lengths[p1] >= 1 && h_lengths[p1] <= BEAGLE_MAX_LEN) ? h_lengths[p1] : 0;
+        if (words + l + 1 > cap_words) break;
+        words += l + 1; ntok += l; ++p1;
+    }
+    *ntok_out = ntok;
+    return p1;
+}
+
 static beagle_status eval_chunked_impl(const int32_t*, const int32_t*, int64_t, const float*, int64_t, const float*, const float*,
                                        int32_t, int32_t, float, float*, int64_t, const FitSel&, void*);
 
@@ -919,10 +954,8 @@ beagle_status beagle_reserve_chunked(int64_t device_budget_bytes)
     if (s != BEAGLE_OK) return s;
     // the budget is cut into K staging buffers of about 32 MiB (2 <= K <= 8): a chunk is copied while the ones before it
     // are evaluated, and the finer the chunks the less of the first copy and of the last evaluation is exposed
-    long long K = device_budget_bytes / g_stage_target;
-    K = K < 2 ? 2 : (K > kStageBufsMax ? kStageBufsMax : K);
-    const long long half = (device_budget_bytes / K) & ~255ll;
-    if (half < 4ll * (BEAGLE_MAX_LEN + 1)) return BEAGLE_ERR_INVALID_ARG;
+    long long K, half;
+    if (!stage_layout(device_budget_bytes, &K, &half)) return BEAGLE_ERR_INVALID_ARG;
     if (!w.copy_stream) {
         CU(cudaStreamCreateWithFlags(&w.copy_stream, cudaStreamNonBlocking));
         for (int i = 0; i < kStageBufsMax; ++i) {
@@ -998,21 +1031,8 @@ static beagle_status eval_chunked_impl(const int32_t* h_genomes, const int32_t* 
     long long p0 = 0, tok0 = 0;
     int total_launches = 0;
     for (int c = 0; p0 < P; ++c) {
-        long long words = 0, p1 = p0, ntok = 0;
-        // whole blocks of 4096 lengths first (a branch-free sum the host compiler vectorises: the scan of the first
-        // chunk is on the critical path, nothing is in flight yet), then one by one up to the boundary
-        while (p1 + 4096 <= P) {
-            long long bt = 0;
-            const int32_t* hl = h_lengths + p1;
-            for (int k = 0; k < 4096; ++k) { const int32_t v = hl[k]; bt += (v >= 1 && v <= BEAGLE_MAX_LEN) ? v : 0; }
-            if (words + bt + 4096 > cap_words) break;
-            words += bt + 4096; ntok += bt; p1 += 4096;
-        }
-        while (p1 < P) {
-            const int l = (h_lengths[p1] >= 1 && h_lengths[p1] <= BEAGLE_MAX_LEN) ? h_lengths[p1] : 0;
-            if (words + l + 1 > cap_words) break;
-            words += l + 1; ntok += l; ++p1;
-        }
+        long long ntok = 0;
+        const long long p1 = chunk_end(h_lengths, P, p0, cap_words, &ntok);
         const long long np = p1 - p0;
         const int b = c % w.stage_n;
         int32_t* d_len = reinterpret_cast<int32_t*>(w.stage[b]);
@@ -1103,6 +1123,28 @@ beagle_status beagle_debug_plan(int32_t N, int32_t d, int32_t fit, int32_t fitne
     const int v[12] = { tp.fast ? 1 : 0, tp.split ? 1 : 0, tp.threads, passes * d, passes * tp.k_rcp, tp.tmem_slots, tp.k_un, tp.ring_bytes,
                         (int)tp.smem, tp.off_ys, tp.off_un, tp.off_ring };
     for (int i = 0; i < 12; ++i) out12[i] = v[i];
+    return BEAGLE_OK;
+}
+
+// host only: the chunks beagle_eval_chunked would cut this colony into under this budget (the same two functions)
+beagle_status beagle_debug_chunk_plan(const int32_t* h_lengths, int64_t P, int64_t device_budget_bytes, int64_t* ends, int64_t max_ends,
+                                      int64_t* n_chunks, int32_t* n_buffers, int64_t* buffer_bytes)
+{
+    if (P < 0 || (P > 0 && !h_lengths) || device_budget_bytes < 2ll * 4 * (BEAGLE_MAX_LEN + 64)) return BEAGLE_ERR_INVALID_ARG;
+    long long K, half;
+    if (!stage_layout(device_budget_bytes, &K, &half)) return BEAGLE_ERR_INVALID_ARG;
+    if (n_buffers) *n_buffers = (int32_t)K;
+    if (buffer_bytes) *buffer_bytes = half;
+    const long long cap_words = half / 4 - 3;
+    long long n = 0;
+    for (long long p0 = 0; p0 < P; ++n) {
+        long long ntok = 0;
+        const long long p1 = chunk_end(h_lengths, P, p0, cap_words, &ntok);
+        if (p1 == p0) return BEAGLE_ERR_INVALID_ARG;      // (cannot happen: a buffer holds a maximum-length individual)
+        if (ends && n < max_ends) ends[n] = p1;
+        p0 = p1;
+    }
+    if (n_chunks) *n_chunks = n;
     return BEAGLE_OK;
 }
 

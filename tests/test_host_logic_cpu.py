@@ -206,3 +206,72 @@ def test_token_table(tables):
             assert px(int(tok[i][1]))["need"] == 63 and int(tok[i][0]) == 0
     pad = px(int(tok[64][1]))
     assert (pad["delta"], pad["sh"], pad["need"], pad["lim"], pad["or1"], pad["kind"]) == (0, 1, 0, 63, 0, 0)
+
+
+# ---- a8: how a budget is cut into staging buffers and a colony into chunks -------------------------------------------
+def chunk_plan(lengths, budget):
+    lengths = np.ascontiguousarray(lengths, dtype=np.int32)
+    max_ends = len(lengths) + 1
+    ends = np.zeros(max_ends, dtype=np.int64)
+    n, K, nbytes = ctypes.c_int64(0), ctypes.c_int32(0), ctypes.c_int64(0)
+    st = api.lib().beagle_debug_chunk_plan(lengths.ctypes.data, len(lengths), budget, ends.ctypes.data, max_ends,
+                                           ctypes.byref(n), ctypes.byref(K), ctypes.byref(nbytes))
+    return st, ends[:n.value].copy(), K.value, nbytes.value
+
+
+def check_chunks(lengths, budget):
+    """The properties a chunking must have, whatever the algorithm: contiguous, whole individuals, every chunk fits its
+    buffer, and greedy (the next individual would not have fitted)."""
+    st, ends, K, nbytes = chunk_plan(lengths, budget)
+    assert st == api.OK
+    assert 2 <= K <= 8 and nbytes % 256 == 0 and K * nbytes <= budget
+    lengths = np.asarray(lengths, dtype=np.int64)
+    tok = np.where((lengths >= 1) & (lengths <= 512), lengths, 0)
+    assert len(ends) >= 1 and ends[-1] == len(lengths) and (np.diff(np.concatenate(([0], ends))) > 0).all()
+    p0 = 0
+    for p1 in ends:
+        np_, nt = p1 - p0, int(tok[p0:p1].sum())
+        # the buffer holds the chunk's lengths (padded to a multiple of four) and then its tokens
+        assert 4 * (((np_ + 3) & ~3) + nt) <= nbytes
+        if p1 < len(lengths):
+            assert 4 * (np_ + 1 + nt + int(tok[p1]) + 3) > nbytes          # greedy: one more would not fit
+        p0 = p1
+    return len(ends), K, nbytes
+
+
+def test_chunk_plan_properties_on_random_colonies():
+    rng = np.random.default_rng(20260705)
+    for budget in (4608, 10_000, 64 << 10, 1 << 20, 5 << 20):
+        for _ in range(3):
+            P = int(rng.integers(1, 60_000))
+            lengths = rng.integers(1, 513, size=P)
+            lengths[rng.random(P) < 0.01] = 0                    # out-of-range lengths: an entry without tokens
+            lengths[rng.random(P) < 0.01] = 700
+            check_chunks(lengths, budget)
+    # exactly one maximum-length individual per buffer at the smallest budget the call accepts
+    n, K, nbytes = check_chunks(np.full(7, 512), 4608)
+    assert (n, K) == (7, 2)
+
+
+def test_chunk_plan_buffers_follow_the_budget():
+    ones = np.ones(10, dtype=np.int32)
+    MiB = 1 << 20
+    for budget, K in ((64 * MiB, 2), (96 * MiB, 3), (160 * MiB, 5), (256 * MiB, 8), (1024 * MiB, 8)):
+        st, _, k, nbytes = chunk_plan(ones, budget)
+        assert st == api.OK and k == K and nbytes == (budget // K) & ~255
+    api.beagle_set_chunk_target(8 * MiB)
+    try:
+        assert chunk_plan(ones, 24 * MiB)[2] == 3
+    finally:
+        api.beagle_set_chunk_target(0)
+    assert chunk_plan(ones, 24 * MiB)[2] == 2
+    assert chunk_plan(ones, 4607)[0] == api.ERR_INVALID_ARG
+
+
+def test_chunk_plan_of_config5_is_ten_chunks_over_eight_buffers():
+    # BASELINE.json configs[4]: P = 4,194,304, lengths up to 512, a budget of 1 GiB (DESIGN.md §5): the chunking the full-size GPU
+    # test and bench.py --config 5 run (more chunks than buffers: buffers are reused)
+    cfg = colonies.CONFIGS[5]
+    _, lengths, _ = colonies.generate_programs(cfg, cfg.P, seed_offset=0)
+    n, K, nbytes = check_chunks(lengths, cfg.budget_bytes)
+    assert K == 8 and n == 10
