@@ -322,6 +322,9 @@ def test_malformed_programs_get_canonical_nan(oracle):
         np.array([T(0x10)], np.int32),                                      # reserved (DUP)
         np.array([T(C.OP["LOAD"], 0), T(C.OP["SIN"], 5)], np.int32),        # operator with arg
         np.array([T(C.OP["LOAD"], 0)] * 33 + [T(C.OP["ADD"])] * 32, np.int32),  # depth 33
+        np.array([T(C.OP["LOAD"], 0), T(C.OP["ADD"]), T(C.OP["LOAD"], 1)], np.int32),       # binary with one operand, depth 1 at the end
+        np.array([T(C.OP["LOAD"], 0), T(C.OP["LOAD"], 1), T(C.OP["ADD"], 7)], np.int32),    # binary operator with arg
+        np.array([T(C.OP["LOAD"], 0), T(C.OP["LOAD"], 1), T(C.OP["DIV"], 1)], np.int32),
     ]
     good = [np.array([T(C.OP["LOAD"], 0)] * 32 + [T(C.OP["ADD"])] * 31, np.int32),  # depth 32 is fine
             np.array([T(C.OP["LOAD"], 0), T(C.OP["LOAD"], 1)], np.int32)]            # final depth 2 (R8)
@@ -337,6 +340,13 @@ def test_malformed_programs_get_canonical_nan(oracle):
     l = np.array([0, -3, 600, 1], np.int32)
     rr = oracle.evaluate(g, l, consts, X, y, 0.0)
     assert np.all(rr["fitness"].view(np.uint32)[:3] == QNAN_BITS) and rr["fitness"][3] == 1.0
+    # the longest program there is: 512 tokens exactly (x0, 255 times "x0 ADD", SIN) = sin(256) on X = 1; 513 tokens: malformed
+    longest = [T(C.OP["LOAD"], 0)] + [T(C.OP["LOAD"], 0), T(C.OP["ADD"])] * 255 + [T(C.OP["SIN"])]
+    assert len(longest) == 512
+    g2 = np.array(longest + longest + [T(C.OP["SIN"])], np.int32)
+    r5 = oracle.evaluate(g2, np.array([512, 513], np.int32), consts, X, y, 0.0, want_outputs=True)
+    assert r5["depth"][0] == 2 and r5["outputs"][0][0] == pytest.approx(math.sin(256.0), rel=1e-12)
+    assert r5["fitness"].view(np.uint32)[1] == QNAN_BITS
 
 
 # ---- P11: the bound is a bound (fp32 mirror vs fp64 truth) -----------------------------------------
@@ -890,3 +900,185 @@ def test_P21b_std_bound_is_a_bound(oracle, power):
     assert np.all(diff[ok] <= t["bound"][ok]), (np.flatnonzero(ok & (diff > t["bound"]))[:5], diff[ok].max())
     assert (t["bound"][ok] <= N / 16).mean() > 0.6, (t["bound"][ok] <= N / 16).mean()
 
+
+
+# ---- P22: the fp32 mirror (mode 1) is a step-by-step fp32 evaluator -------------------------------------------------
+# The mirror is what the arithmetic-only GPU tests compare against bit for bit, so its own rounding points are pinned: every
+# command's result, the residual, its square (D5) are rounded to fp32; the sum is carried in fp64 and rounded once.
+def test_P22_mirror_rounds_every_step_like_numpy_float32(oracle):
+    f32 = np.float32
+    # (1) the residual is rounded before it is squared: out = 1, y = -2^-24: r = 1 + 2^-24 ties to 1.0 in fp32, r^2 = 1;
+    #     squaring the unrounded residual would give 1 + 2^-23
+    X = np.array([[1.0]], f32)
+    y = np.array([-2.0 ** -24], f32)
+    r = oracle.evaluate(*pack([asm("x0")[0]], np.zeros(1, f32))[:2], np.zeros(1, f32), X, y, 0.0, mode=1)
+    assert r["fitness"][0] == f32(1.0)
+    r0 = oracle.evaluate(*pack([asm("x0")[0]], np.zeros(1, f32))[:2], np.zeros(1, f32), X, y, 0.0, mode=0)
+    assert r0["fitness"][0] == f32(1.0 + 2.0 ** -23)          # the truth mode keeps the fp64 residual
+    # (2) random arithmetic programs against numpy float32, command by command, residual and square included
+    rng = np.random.default_rng(22)
+    N, d = 16, 3
+    Xr = rng.uniform(-3, 3, (N, d)).astype(f32)
+    yr = rng.uniform(-3, 3, N).astype(f32)
+    consts = np.array([0.3, -1.7, 2.5], f32)
+    texts = ["x0 x1 MUL x2 ADD", "x0 c0 SUB x1 c1 MUL MUL", "x0 x0 MUL x1 x1 MUL ADD x2 SUB", "c2 x1 SUB x0 MUL x2 x2 MUL ADD c1 ADD",
+             "x0 x1 ADD x2 MUL x0 SUB x1 MUL c0 ADD"]
+    vals = {"c0": consts[0], "c1": consts[1], "c2": consts[2]}
+    progs = []
+    for t in texts:
+        toks = []
+        for w in t.split():
+            if w[0] == "x": toks.append(C.token(C.OP["LOAD"], int(w[1:])))
+            elif w[0] == "c": toks.append(C.token(C.OP["CONST"], int(w[1:])))
+            else: toks.append(C.token(C.OP[w]))
+        progs.append(np.array(toks, np.int32))
+    g, l, c = pack(progs, consts)
+    got = oracle.evaluate(g, l, c, Xr, yr, 0.0, mode=1, want_outputs=True)
+    for k, t in enumerate(texts):
+        S = 0.0
+        for i in range(N):
+            st = []
+            for w in t.split():
+                if w[0] == "x": st.append(Xr[i, int(w[1:])])
+                elif w[0] == "c": st.append(vals[w])
+                else:
+                    b, a = st.pop(), st.pop()
+                    st.append({"ADD": a + b, "SUB": a - b, "MUL": a * b}[w])        # numpy float32 scalars: one rounding each
+            assert isinstance(st[-1], np.float32) and got["outputs"][k][i] == float(st[-1])
+            res = st[-1] - yr[i]
+            S += float(res * res)                                                    # fp32 residual, fp32 square, fp64 sum
+        assert got["fitness"][k] == f32(S / N)
+
+
+# ---- P23: the parts of the bounds that only show when the INPUT of a command carries a large error ------------------------
+# (found by mutating the oracle: with inputs that are only one rounding off, dropping the propagated input error of the library
+# functions, half of POW's corners or the correlation's A / B terms went unnoticed). "noise(c)" = K x0 + c - K x0 is c exactly,
+# and c +- K u |x0| in fp32: a value with a large, honest error bound.
+def _noise(c, K=3000.0):
+    return f"x0 {K:.1f} MUL {c:.4f} ADD x0 {K:.1f} MUL SUB"
+
+
+def test_P23_bounds_hold_when_inputs_carry_large_errors(oracle):
+    rng = np.random.default_rng(23)
+    X = rng.uniform(0.5, 3.0, (128, 2)).astype(np.float32)
+    y = np.zeros(128, np.float32)
+    progs, consts = [], []
+    for f in ["CBRT", "TAN", "ARCSIN", "ARCCOS", "ARCTAN", "TANH", "SIN", "COS", "EXP", "LOG", "SQRT", "SQUARE", "CUBE"]:
+        for c0 in (0.31, -0.47, 0.83, 0.12):
+            progs.append(asm(f"{_noise(c0)} {f}", consts)[0])
+            progs.append(asm(f"{_noise(c0)} {f} x1 MUL", consts)[0])
+    for c0, c1 in ((1.7, 0.6), (0.4, 2.3), (2.9, -1.2), (1.1, 1.9), (0.7, -0.4), (2.2, 0.3)):
+        progs.append(asm(f"{_noise(c0)} {_noise(c1)} POW", consts)[0])         # both operands of POW uncertain: all four corners matter
+        progs.append(asm(f"{_noise(c0)} x1 POW", consts)[0])
+        progs.append(asm(f"x1 {_noise(c1)} POW", consts)[0])
+        progs.append(asm(f"{_noise(c0)} {_noise(c1)} DIV", consts)[0])
+        progs.append(asm(f"{_noise(c0)} {_noise(c1)} MUL", consts)[0])
+    c = np.array(consts, np.float32)
+    ieee = oracle.contract(oracle.CONTRACT_IEEE)
+    t = ev(oracle, progs, c, X, y, contract_=ieee)
+    m = ev(oracle, progs, c, X, y, contract_=ieee, mode=1)
+    fin = np.isfinite(t["fitness"]) & np.isfinite(m["fitness"]) & ((t["flags"] & 6) == 0)
+    assert fin.sum() >= 100, fin.sum()
+    diff = np.abs(t["fitness"].astype(np.float64) - m["fitness"].astype(np.float64))
+    slack = 2.0 ** -23 * np.abs(t["fitness"].astype(np.float64))
+    bad = np.flatnonzero(fin & (diff > t["bound"] + slack))
+    assert len(bad) == 0, bad[:5]
+    # the errors are really large here (hundreds of roundings), and the bound is not orders of magnitude above them
+    rel = diff[fin] / np.maximum(np.abs(t["fitness"][fin].astype(np.float64)), 1e-30)
+    assert np.median(rel) > 20 * 2.0 ** -24
+    assert np.median(t["bound"][fin] / np.maximum(diff[fin], 1e-300)) < 1e4
+
+
+def test_P23_correlation_bound_with_noisy_outputs(oracle):
+    rng = np.random.default_rng(231)
+    N = 256
+    X = rng.uniform(0.5, 3.0, (N, 2)).astype(np.float32)
+    y = (X[:, 0] * 1.5 - X[:, 1]).astype(np.float32)
+    consts = []
+    # a small signal plus the noisy constant: the noise is a few per cent of the signal's spread, so r^2 really moves
+    texts = [f"x0 1.5 MUL x1 SUB {sc:.4f} MUL {_noise(c0, K)} ADD" for sc in (0.01, 0.003) for c0 in (0.3, -0.8) for K in (3000.0, 20000.0)]
+    texts += [f"x0 x1 MUL {sc:.4f} MUL {_noise(c0, K)} ADD" for sc in (0.01, 0.004) for c0 in (0.7,) for K in (3000.0, 10000.0)]
+    progs = [asm(t, consts)[0] for t in texts]
+    g, l, cst = pack(progs, consts)
+    ieee = oracle.contract(oracle.CONTRACT_IEEE)
+    r = oracle.evaluate_corr(g, l, cst, X, y, M_SCORE, 0.0, contract_=ieee)
+    outs = oracle.evaluate(g, l, cst, X, y, 0.0, mode=1, want_outputs=True, contract_=ieee)["outputs"]      # the fp32 mirror's outputs
+    checked, large = 0, 0
+    for p in range(len(progs)):
+        if r["flags"][p] != 0:
+            continue
+        f = outs[p]                                      # float64 holding fp32 values; the sums below in fp64: only the outputs differ
+        df, dy = f - f.mean(), y.astype(np.float64) - y.astype(np.float64).mean()
+        r2 = (df @ dy) ** 2 / ((df @ df) * (dy @ dy))
+        score = M_SCORE * r2 * r2 * N
+        err = abs(score - float(r["fitness"][p]))
+        assert err <= r["bound"][p] + np.spacing(np.float32(score)), (texts[p], score, r["fitness"][p], r["bound"][p])
+        large += err > 1000 * 2.0 ** -24 * abs(score)    # off by far more than rounding: only the terms A and B cover this
+        checked += 1
+    assert checked >= 6 and large >= 4, (checked, large)
+
+
+def test_P23_summation_term_covers_an_fp32_sum(oracle):
+    """E_S carries (sum_per_case N + sum_const) u S for the fp32 summation the device does and the oracle does not (its sum is
+    fp64). One large square followed by 511 small ones that an fp32 running sum rounds away, in the device's order (DESIGN.md
+    §7 'summation order', restated) and, under the IEEE contract ('any order'), plainly one after the other."""
+    f32 = np.float32
+    N = 512
+    x = np.full(N, 2.0 ** -13 * 1.4, f32); x[0] = 1.0             # squares: 1 and 511 times about 0.98 * 2^-25 (under half an ulp of 1)
+    X = x.reshape(N, 1)
+    y = np.zeros(N, f32)
+    prog = asm("x0")[0]
+    q = (x.astype(np.float64)) ** 2
+    # sequential fp32
+    s = f32(0)
+    for i in range(N):
+        s = f32(s + f32(x[i] * x[i]))
+    seq = float(f32(s / f32(N)))
+    # the device's order: lane l holds cases 128 b + 4 l + e (b = block of 128, e = 0..3), fma chain, then a 5-level xor butterfly
+    lanes = np.zeros(32, f32)
+    for b in range(N // 128):
+        for l in range(32):
+            for e in range(4):
+                i = 128 * b + 4 * l + e
+                lanes[l] = f32(float(x[i]) * float(x[i]) + float(lanes[l]))      # fma: one rounding
+    for m in (16, 8, 4, 2, 1):
+        lanes = np.array([f32(lanes[l] + lanes[l ^ m]) for l in range(32)], f32)
+    dev = float(f32(lanes[0] / f32(N)))
+    exact = q.sum() / N
+    ieee, b200 = oracle.contract(oracle.CONTRACT_IEEE), oracle.contract(oracle.CONTRACT_B200)
+    ti = ev(oracle, [prog], np.zeros(1, f32), X, y, contract_=ieee)
+    tb = ev(oracle, [prog], np.zeros(1, f32), X, y, contract_=b200)
+    assert abs(float(ti["fitness"][0]) - exact) <= 2.0 ** -24 * exact
+    assert abs(seq - exact) > 10 * 2.0 ** -24 * exact                       # the running sum really lost the small squares
+    assert abs(seq - exact) <= ti["bound"][0]                               # any order: N u S
+    assert abs(dev - exact) <= tb["bound"][0]                               # the device's order: (N / 32 + 5) u S
+    assert tb["bound"][0] < ti["bound"][0] and ti["bound"][0] < 600 * 2.0 ** -24 * exact
+
+
+def test_P23_overflow_edge_is_flagged_class_unstable(oracle):
+    f32 = np.float32
+    big = f32((2.0 - 2.0 ** -23) * 2.0 ** 63)                # big * 2^64 = FLT_MAX exactly
+    prog = asm("x0 x1 MUL")[0]
+    cases = [(big, f32(2.0 ** 64)),                          # the product is FLT_MAX itself: one rounding decides finite or +inf
+             (big, f32(2.0 ** 63)),                          # half of it
+             (big, f32(2.0 ** 64 * (1 + 2.0 ** -22)))]       # two ulps above: +inf for any evaluator within the contract
+    out = []
+    for a, b in cases:
+        r = ev(oracle, [prog], np.zeros(1, f32), np.array([[a, b]], f32), np.zeros(1, f32), want_outputs=True)
+        out.append((int(r["flags"][0]), float(r["outputs"][0][0])))
+    assert out[0][0] & oracle.FLAG_CLASS_UNSTABLE and out[0][1] == 3.4028234663852886e38
+    assert not out[1][0] & oracle.FLAG_CLASS_UNSTABLE and math.isfinite(out[1][1])
+    assert not out[2][0] & oracle.FLAG_CLASS_UNSTABLE and out[2][1] == math.inf
+
+
+def test_P23_published_contract_numbers(oracle):
+    """orc_default_contract(1) is DESIGN.md §6's table, retyped there from the device's measured accuracy: the numbers the GPU
+    contract test (tests/test_gpu_op_contract.py) holds the device to are the ones the oracle's bound uses."""
+    c = oracle.contract(oracle.CONTRACT_B200)
+    want = dict(c_add=1.0, c_mul=1.0, c_div=3.5, c_sqrt=3.0, c_exp=6.0, c_exp_arg=2.5, c_log_rel=5.0, c_log_abs=4.0,
+                c_sin_abs=12.0, c_sin_arg=3.0, sum_per_case=1.0 / 32.0, sum_const=5.0, c_pow=10.0)
+    for k, v in want.items():
+        assert getattr(c, k) == v, k
+    assert list(c.c_fun) == [3.0, 6.0, 4.0, 4.0, 4.0, 4.0]
+    i = oracle.contract(oracle.CONTRACT_IEEE)
+    assert (i.c_add, i.c_mul, i.c_div, i.c_sqrt, i.sum_per_case, i.sum_const) == (1.0, 1.0, 1.0, 1.0, 1.0, 0.0)
