@@ -63,6 +63,13 @@ def test_plan_invariants_over_all_shapes():
                     assert p["smem"] <= SMEM_OPTIN_B200
                     assert p["ring"] >= STAGE_BYTES_MAX, (N, d, fit, fo, p)   # run_eval would refuse the call otherwise
                     assert p["off_ys"] < p["off_un"] <= p["off_ring"] < p["smem"]
+                    # between y and the unary rows: the padded targets (twice for the correlation fitness: y and the centred y)
+                    # and one 64-entry window of the work queue per warp
+                    npad = (N + 511) // 512 * 512
+                    assert p["off_un"] - p["off_ys"] == 4 * npad * (2 if fit == api.FIT_CORRELATION else 1) + 64 * 16 * (p["threads"] // 32)
+                    # bulk copies land on 128-byte boundaries: the rings start on one and are a multiple of it long
+                    assert p["off_ring"] % 128 == 0 and p["ring"] % 128 == 0 and p["off_ys"] % 128 == 0
+                    assert p["off_ring"] + p["ring"] * (p["threads"] // 32) <= p["smem"]
                     assert p["split"] == 0 or (fit == api.FIT_MSE and fo and N > 512)
     assert n_fast > 4000
 
@@ -251,6 +258,19 @@ def test_chunk_plan_properties_on_random_colonies():
     # exactly one maximum-length individual per buffer at the smallest budget the call accepts
     n, K, nbytes = check_chunks(np.full(7, 512), 4608)
     assert (n, K) == (7, 2)
+
+
+def test_chunk_plan_block_scan_with_out_of_range_lengths():
+    # buffers large enough for the planner's fast path (whole blocks of 4096 lengths at a time), on a colony with lengths outside
+    # 1..512 in it: they take a word each and no tokens, in the fast path as in the slow one
+    rng = np.random.default_rng(4096)
+    P = 150_000
+    lengths = rng.integers(1, 513, size=P)
+    lengths[rng.random(P) < 0.02] = 0
+    lengths[rng.random(P) < 0.02] = 700
+    lengths[rng.random(P) < 0.01] = -5
+    n, K, nbytes = check_chunks(lengths, 64 << 20)
+    assert K == 2 and n >= 2 and nbytes // 4 > 3 * 4096 * 257
 
 
 def test_chunk_plan_buffers_follow_the_budget():
