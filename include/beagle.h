@@ -273,6 +273,19 @@ beagle_status beagle_debug_chunk_plan(const int32_t* h_lengths, int64_t P, int64
  * program). Either may be NULL. Field layout: compile_kernel.inc. */
 void beagle_debug_walk_tables(uint32_t* lut160, uint32_t* tok130);
 
+/* beagle_debug_compile — test only, HOST only, needs no device: the compiler of the whole language (the function k_compile_general runs
+ * one lane per program on the device, compiled for the host as well) on ONE program. tokens: HOST, len words (1..512); consts: HOST;
+ * tmem_slots, k_rcp, k_un, un_row_bytes: the plan the records are compiled for (beagle_debug_plan: slot rows per warp, variables with
+ * a reciprocal row, variables with staged unary rows, bytes per staged row); rcp_unsafe: bit j set = variable j has a case with
+ * |x| < 1e-6f (its division is protected: no reciprocal row). Outputs (HOST): *depth = the maximum stack depth, 0 if the program is
+ * malformed (D3); *slow = 1 if it is handed to the blockwise kernel (POW, a library function, COPY / PASTE); otherwise
+ * records[2 i], records[2 i + 1] = the words h, o of micro-op i (csrc/uop.cuh; room for len + 1 records) and *n_records their number,
+ * before the END record. One difference from the device: the reciprocal a constant divisor is folded to is the IEEE 1 / c here,
+ * the division handler's rcp.approx there. BEAGLE_ERR_INVALID_ARG for arguments out of range. */
+beagle_status beagle_debug_compile(const int32_t* tokens, int32_t len, const float* consts, int64_t n_consts, int32_t d,
+                                   int32_t tmem_slots, int32_t k_rcp, int32_t k_un, int32_t un_row_bytes, uint32_t rcp_unsafe,
+                                   uint32_t* records, int32_t* n_records, int32_t* depth, int32_t* slow);
+
 /* Limits compiled into the library (any pointer may be NULL). */
 void beagle_limits(int32_t* max_len, int32_t* max_stack, int32_t* max_n, int32_t* max_d);
 

@@ -43,6 +43,8 @@ _SIGNATURES = {
     "beagle_debug_counts": (_i32, [ctypes.POINTER(_i32)] * 4 + [_vp]),
     "beagle_debug_plan": (_i32, [_i32, _i32, _i32, _i32, _i32, ctypes.POINTER(_i32)]),
     "beagle_debug_chunk_plan": (_i32, [_vp, _i64, _i64, _vp, _i64, ctypes.POINTER(_i64), ctypes.POINTER(_i32), ctypes.POINTER(_i64)]),
+    "beagle_debug_compile": (_i32, [_vp, _i32, _vp, _i64, _i32, _i32, _i32, _i32, _i32, ctypes.c_uint32, _vp,
+                                    ctypes.POINTER(_i32), ctypes.POINTER(_i32), ctypes.POINTER(_i32)]),
     "beagle_debug_walk_tables": (None, [ctypes.POINTER(ctypes.c_uint32), ctypes.POINTER(ctypes.c_uint32)]),
     "beagle_limits": (None, [ctypes.POINTER(_i32)] * 4),
     "beagle_status_string": (ctypes.c_char_p, [_i32]),
@@ -155,6 +157,19 @@ def beagle_debug_counts(stream=0):
     v = [_i32() for _ in range(4)]
     _check(lib().beagle_debug_counts(*[ctypes.byref(x) for x in v], int(stream) or None), "beagle_debug_counts")
     return dict(n_sorted=v[0].value, n_general=v[1].value, n_slow=v[2].value, n_malformed=v[3].value)
+
+
+def beagle_debug_compile(tokens, consts, d, tmem_slots, k_rcp, k_un, un_row_bytes, rcp_unsafe=0):
+    """One program through the host build of the device's general compiler: (depth, slow, records uint32[n, 2]); numpy in, numpy out."""
+    import numpy as np
+    tokens = np.ascontiguousarray(tokens, np.int32)
+    consts = np.ascontiguousarray(consts, np.float32)
+    rec = np.zeros((len(tokens) + 1, 2), np.uint32)
+    n, depth, slow = _i32(0), _i32(0), _i32(0)
+    _check(lib().beagle_debug_compile(_ptr(tokens), len(tokens), _ptr(consts) if len(consts) else None, len(consts), int(d),
+                                      int(tmem_slots), int(k_rcp), int(k_un), int(un_row_bytes), int(rcp_unsafe), _ptr(rec),
+                                      ctypes.byref(n), ctypes.byref(depth), ctypes.byref(slow)), "beagle_debug_compile")
+    return depth.value, bool(slow.value), rec[: n.value]
 
 
 def beagle_limits():

@@ -1157,6 +1157,27 @@ void beagle_debug_walk_tables(uint32_t* lut160, uint32_t* tok130)
     if (tok130) for (int i = 0; i < kTok2Size; ++i) { tok130[2 * i] = tt[i].x; tok130[2 * i + 1] = tt[i].y; }
 }
 
+// host only: compile_general (compile_kernel.inc), the compiler of the whole language that k_compile_general runs one lane per
+// program, compiled for the host and run on one program
+beagle_status beagle_debug_compile(const int32_t* tokens, int32_t len, const float* consts, int64_t n_consts, int32_t d,
+                                   int32_t tmem_slots, int32_t k_rcp, int32_t k_un, int32_t un_row_bytes, uint32_t rcp_unsafe,
+                                   uint32_t* records, int32_t* n_records, int32_t* depth, int32_t* slow)
+{
+    if (!tokens || len < 1 || len > BEAGLE_MAX_LEN || d < 1 || d > BEAGLE_MAX_D || n_consts < 0 || n_consts > BEAGLE_MAX_CONSTS
+        || (n_consts > 0 && !consts) || tmem_slots < 0 || tmem_slots > kMemSlots || k_rcp < 0 || k_rcp > d || k_un < 0 || k_un > d
+        || un_row_bytes < 0 || !records || !n_records || !depth || !slow)
+        return BEAGLE_ERR_INVALID_ARG;
+    CompileParams q = {};
+    q.consts = consts; q.n_consts = n_consts; q.d = d; q.tmem_slots = tmem_slots; q.k_rcp = k_rcp; q.k_un = k_un; q.un_row_bytes = un_row_bytes;
+    const uint32_t rcp_ok = ~rcp_unsafe & ((k_rcp >= 32) ? 0xFFFFFFFFu : ((1u << k_rcp) - 1u));       // as the kernels form it
+    uint2 out[BEAGLE_MAX_LEN + 4];
+    int n = 0; bool sl = false;
+    const int mx = compile_general(q, reinterpret_cast<const uint32_t*>(tokens), len, out, true, rcp_ok, &n, &sl);
+    *depth = mx; *slow = (mx > 0 && sl) ? 1 : 0; *n_records = (mx > 0 && !sl) ? n : 0;
+    if (mx > 0 && !sl) for (int i = 0; i < n; ++i) { records[2 * i] = out[i].x; records[2 * i + 1] = out[i].y; }
+    return BEAGLE_OK;
+}
+
 beagle_status beagle_debug_counts(int32_t* n_sorted, int32_t* n_general, int32_t* n_slow, int32_t* n_malformed, void* stream)
 {
     Header h;

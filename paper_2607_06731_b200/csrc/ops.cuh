@@ -11,6 +11,7 @@
 // The protected tests are selects, not branches, so a warp never diverges on data.
 #pragma once
 #include <stdint.h>
+#include <string.h>
 
 namespace beagle {
 
@@ -57,7 +58,23 @@ __device__ __forceinline__ float op_tanh(float a) { return tanhf(a); }          
 __device__ __forceinline__ float op_pow(float a, float b) { return powf(a, b); }
 
 // token fields (D1)
-__device__ __forceinline__ uint32_t tok_op(uint32_t w) { return w & 0xFFu; }
-__device__ __forceinline__ uint32_t tok_arg(uint32_t w) { return w >> 8; }
+__host__ __device__ __forceinline__ uint32_t tok_op(uint32_t w) { return w & 0xFFu; }
+__host__ __device__ __forceinline__ uint32_t tok_arg(uint32_t w) { return w >> 8; }
+
+// What compile_general needs in both worlds: it is compiled for the host too, so that the rules of the whole language and the
+// records they emit can be tested without a device (beagle_debug_compile, test only; the device code is unchanged by this).
+// On the host the reciprocal of a constant divisor is the IEEE one: a stand-in for the division handler's rcp.approx, which
+// only the device has (a host-compiled record of "x / c" therefore carries 1/c to half an ulp instead of the device's bits).
+#ifdef __CUDA_ARCH__
+#define BG_LDG(p) __ldg(p)
+__device__ __forceinline__ uint32_t f32_bits(float f) { return __float_as_uint(f); }
+__device__ __forceinline__ float bits_f32(uint32_t u) { return __uint_as_float(u); }
+__device__ __forceinline__ float rcp_of_const(float c) { return mufu_rcp(c); }
+#else
+#define BG_LDG(p) (*(p))
+inline uint32_t f32_bits(float f) { uint32_t u; memcpy(&u, &f, 4); return u; }
+inline float bits_f32(uint32_t u) { float f; memcpy(&f, &u, 4); return f; }
+inline float rcp_of_const(float c) { return 1.0f / c; }
+#endif
 
 } // namespace beagle

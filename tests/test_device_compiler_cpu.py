@@ -1,0 +1,303 @@
+"""CPU-only: the device's compiler of the whole language, run on the host (beagle_debug_compile = compile_general of
+csrc/compile_kernel.inc compiled for the host too; the device code is the same source and its SASS is unchanged).
+
+Two things are checked against the oracle, which shares nothing with it:
+- the static check (D3): the maximum stack depth it reports is the oracle's depth_out, and it calls a program malformed
+  exactly when the oracle does, on random programs of the whole language and on corrupted ones;
+- the micro-ops it emits (csrc/uop.cuh) compute the program: a small micro-op machine, written here from uop.cuh's description of
+  each handler (accumulator, slot stack in tensor memory, slots in local memory, folded terminals, reversed operands, staged unary
+  rows, reciprocal rows), runs the records in numpy fp32 and the fitness it arrives at passes the same three-class parity rule
+  against the oracle as the GPU does (tests/parity.py), for every plan of slots / reciprocal rows / staged rows.
+What this does not cover: k_compile's table-driven walk (a different implementation of the same step, device only: its tables are
+checked in test_host_logic_cpu.py and its output is compared bit for bit on the GPU) and the handlers' own arithmetic (GPU tests).
+"""
+import numpy as np
+import pytest
+
+from paper_2607_06731_b200 import api, colonies
+from tests import parity
+from tests.util import asm, pack, random_gcl_programs
+
+EPS = np.float32(1e-6)
+H_FRESH0, H_NFRESH = 33, 23
+NAMES = {0: "END", 1: "SIN", 2: "COS", 3: "LOG", 4: "SQRT", 5: "EXP", 6: "NEG", 7: "SQR", 8: "CUBE",
+         9: "ADDX", 10: "SUBX", 11: "MULX", 12: "DIVX", 13: "RSUBX", 14: "RDIVX",
+         15: "ADDS", 16: "MULS", 17: "RSUBS", 18: "RDIVS", 19: "ADDM", 20: "MULM", 21: "RSUBM", 22: "RDIVM",
+         23: "ADDC", 24: "SUBC", 25: "MULC", 26: "RSUBC", 27: "RDIVC", 28: "MULR",
+         29: "POPS", 30: "POPM", 31: "SWAPS", 32: "SWAPM",
+         33: "LX", 34: "LC", 35: "LX_SIN", 36: "LX_COS", 37: "LX_LOG", 38: "LX_SQRT", 39: "LX_EXP", 40: "LX_NEG", 41: "LX_SQR",
+         42: "LX_CUBE", 43: "LX_ADDX", 44: "LX_SUBX", 45: "LX_MULX", 46: "LX_DIVX", 47: "LX_ADDC", 48: "LX_SUBC", 49: "LX_MULC",
+         50: "LX_RSUBC", 51: "LX_RDIVC", 52: "LX_MULR", 53: "LS", 54: "LG", 55: "KEEP"}
+
+
+def _f32(a):
+    return np.asarray(a, np.float32)
+
+
+def _div(a, b):                                    # DESIGN.md D2: |b| < 1e-6f ? 1 : a / b
+    q = _f32(a) / _f32(b)
+    return np.where(np.abs(b) < EPS, np.float32(1), q).astype(np.float32)
+
+
+def _unary(name, a):
+    a = _f32(a)
+    if name == "SIN": return np.sin(a)
+    if name == "COS": return np.cos(a)
+    if name == "LOG": return np.where(np.abs(a) < EPS, np.float32(0), np.log(np.abs(a))).astype(np.float32)
+    if name == "SQRT": return np.sqrt(np.abs(a))
+    if name == "EXP": return np.exp(np.where(a > 80, np.float32(80), a)).astype(np.float32)      # NaN > 80 is false: NaN passes
+    if name == "NEG": return -a
+    if name == "SQR": return a * a
+    if name == "CUBE": return (a * a) * a
+    raise AssertionError(name)
+
+
+def _binary(name, a, b):                           # a op b
+    if name == "ADD": return _f32(a) + _f32(b)
+    if name == "SUB": return _f32(a) - _f32(b)
+    if name == "MUL": return _f32(a) * _f32(b)
+    if name == "DIV": return _div(a, b)
+    raise AssertionError(name)
+
+
+def run_records(rec, X, d, S_T, k_rcp, k_un, un_row_bytes):
+    """The micro-op machine of csrc/uop.cuh on N cases at once (fp32). Returns the accumulator after the last record.
+    Also checks the discipline the compiler owes the interpreter: a tensor-memory push only while fewer than S_T slots are
+    there, a pop only of what was pushed, local slots read only after they were written, reciprocal and staged rows only of
+    the variables that have them."""
+    N = X.shape[0]
+    acc = None
+    tstack, mem = [], {}
+    fun = ["SIN", "COS", "LOG", "SQRT", "EXP"]
+
+    def var(col):
+        assert col % 16 == 0 and col // 16 < d, col
+        return X[:, col // 16]
+
+    def const(o):
+        return np.full(N, np.array([o], np.uint32).view(np.float32)[0], np.float32)
+
+    with np.errstate(all="ignore"):
+        for h, o in rec.tolist():
+            hn = h & 255
+            assert hn != 0 and hn < H_FRESH0 + 3 * H_NFRESH, hn
+            if hn >= H_FRESH0:                     # a fresh value: its push entry first
+                push, hn = divmod(hn - H_FRESH0, H_NFRESH)
+                hn += H_FRESH0
+                if push == 1:
+                    assert acc is not None and len(tstack) < S_T, (len(tstack), S_T)
+                    tstack.append(acc)
+                elif push == 2:
+                    off = (h >> 10) & 0x7FF
+                    assert acc is not None and off % 64 == 0 and off // 64 < 31 and len(tstack) == S_T
+                    mem[off] = acc
+            name = NAMES[hn]
+            colA = h >> 21
+            if name in ("SIN", "COS", "LOG", "SQRT", "EXP", "NEG", "SQR", "CUBE"):
+                acc = _unary(name, acc)
+            elif name[:-1] in ("ADD", "SUB", "MUL", "DIV", "RSUB", "RDIV") and name[-1] in "XSMC":
+                if name[-1] == "X": x = var(o)
+                elif name[-1] == "S": x = tstack.pop()
+                elif name[-1] == "M": x = mem.pop(o)
+                else: x = const(o)
+                op = name[:-1]
+                acc = _binary(op[1:], x, acc) if op[0] == "R" else _binary(op, acc, x)
+            elif name == "MULR":
+                assert o // 16 < k_rcp
+                acc = acc * (np.float32(1) / var(o))
+            elif name == "POPS": acc = tstack.pop()
+            elif name == "POPM": acc = mem.pop(o)
+            elif name == "SWAPS": acc, tstack[-1] = tstack[-1], acc
+            elif name == "SWAPM": acc, mem[o] = mem[o], acc
+            elif name == "LX": acc = var(colA)
+            elif name == "LC": acc = const(o)
+            elif name == "KEEP": pass
+            elif name in ("LS", "LG"):
+                assert un_row_bytes > 0 and o % un_row_bytes == 0
+                f, j = divmod(o // un_row_bytes, k_un if name == "LS" else d)
+                assert f < 5 and (j < k_un if name == "LS" else k_un <= j < d), (name, f, j)
+                acc = _unary(fun[f], X[:, j])
+            elif name == "LX_MULR":
+                assert o // 16 < k_rcp
+                acc = var(colA) * (np.float32(1) / var(o))
+            elif name.startswith("LX_"):
+                rest = name[3:]
+                if rest in ("SIN", "COS", "LOG", "SQRT", "EXP", "NEG", "SQR", "CUBE"):
+                    acc = _unary(rest, var(colA))
+                else:
+                    x = var(o) if rest[-1] == "X" else const(o)
+                    op = rest[:-1]
+                    acc = _binary(op[1:], x, var(colA)) if op[0] == "R" else _binary(op, var(colA), x)
+            else:
+                raise AssertionError(name)
+            acc = _f32(acc)
+    return acc                                     # (a program may leave more than its result on the stack: slots may still hold values)
+
+
+def _fitness(out, y, tax, L):
+    with np.errstate(all="ignore"):
+        r = _f32(out) - _f32(y)
+        return np.float32(np.float32(np.sum(r * r, dtype=np.float32)) / np.float32(len(y)) + np.float32(tax) * np.float32(L))
+
+
+def _check_colony(oracle, genomes, lengths, consts, X, y, tax, plans, expect_slow=None):
+    """Every program through the device's compiler (host build) for each plan; the records through the machine; against the oracle."""
+    d = X.shape[1]
+    orc = oracle.evaluate(genomes, lengths, consts, X, y, tax)
+    unsafe = 0
+    for j in range(d):
+        if np.any(np.abs(X[:, j]) < EPS):
+            unsafe |= 1 << j
+    off = np.concatenate([[0], np.cumsum(lengths, dtype=np.int64)])
+    n_slow = 0
+    for S_T, k_rcp, k_un in plans:
+        fit = np.full(len(lengths), np.nan, np.float32)
+        ran = np.zeros(len(lengths), bool)
+        for p in range(len(lengths)):
+            tok = genomes[off[p]:off[p + 1]]
+            depth, slow, rec = api.beagle_debug_compile(tok, consts, d, S_T, k_rcp, k_un, 4 * 512, unsafe)
+            assert depth == orc["depth"][p], (p, depth, int(orc["depth"][p]))
+            assert (depth == 0) == bool(orc["flags"][p] & oracle.FLAG_MALFORMED), p
+            if depth == 0:
+                continue
+            if slow:
+                n_slow += 1
+                continue
+            assert 1 <= len(rec) <= len(tok)                     # terminals are folded: never more records than tokens
+            out = run_records(rec, X, d, S_T, k_rcp, k_un, 4 * 512)
+            fit[p] = _fitness(out, y, tax, len(tok))
+            ran[p] = True
+        sel = np.nonzero(ran)[0]
+        sub = {k: orc[k][sel] for k in ("fitness", "bound", "flags", "depth")}
+        rep = parity.compare(fit[sel], sub)
+        assert len(rep["bad"]) == 0, parity.describe(rep, fit[sel], sub)
+        assert rep["strict"] >= 0.5 * (rep["strict"] + rep["conditioned"])          # the rule is not vacuous here either
+    if expect_slow is not None:
+        assert (n_slow > 0) == expect_slow
+    return orc
+
+
+PLANS = [(3, 0, 0), (0, 0, 0), (1, 2, 1), (2, 3, 3)]          # (slot rows in tensor memory, reciprocal rows, staged unary rows)
+
+
+def _cases(rng, N, d, lo=-2.0, hi=2.0, zero_in=None):
+    X = rng.uniform(lo, hi, size=(N, d)).astype(np.float32)
+    if zero_in is not None:
+        X[3, zero_in] = 0.0                        # a protected division by this variable: no reciprocal row for it
+    y = (X[:, 0] * X[:, 1 % d] - X[:, (2 % d)]).astype(np.float32)
+    return X, y
+
+
+def test_hot_path_trees_compile_to_records_that_compute_them(oracle):
+    """Colonies of the five configs' generators (the eleven tree commands; config 5's exact-length programs go 32 deep)."""
+    for number, P in ((1, 300), (3, 300), (4, 200), (5, 400)):
+        cfg = colonies.CONFIGS[number]
+        g, l, c = colonies.generate_programs(cfg, P)
+        X, y, _ = colonies.make_dataset(cfg)
+        orc = _check_colony(oracle, g, l, c, X[:48], y[:48], cfg.tax, PLANS[:3] if number != 5 else PLANS, expect_slow=False)
+        if number == 5:
+            assert orc["depth"].max() >= 20        # deep stacks: slots beyond the tensor-memory rows are exercised
+
+
+def test_the_papers_whole_language(oracle):
+    """DUP SWAP DEL SIGN SQUARE CUBE are compiled (resolved on the abstract stack, a slot move for computed values); POW, the six
+    library functions and COPY / PASTE are checked and handed to the blockwise kernel."""
+    rng = np.random.default_rng(7)
+    d = 3
+    fast = ["ADD", "SUB", "MUL", "DIV", "SIN", "COS", "LOG", "SQRT", "EXP", "DUP", "SWAP", "DEL", "SIGN", "SQUARE", "CUBE"]
+    texts = random_gcl_programs(rng, 700, d, fast)
+    cl = []
+    progs = [asm(t, cl)[0] for t in texts]
+    g, l, c = pack(progs, cl)
+    X, y = _cases(rng, 40, d, zero_in=1)
+    _check_colony(oracle, g, l, c, X, y, 1e-3, PLANS, expect_slow=False)
+    texts = random_gcl_programs(rng, 300, d, fast + ["POW", "TANH", "ARCTAN", "CBRT", "TAN", "ARCSIN", "ARCCOS"])
+    texts += ["x0 COPY@3 x1 ADD PASTE@3 MUL", "x0 x1 COPY@0 ADD PASTE@0 SUB"]
+    cl = []
+    progs = [asm(t, cl)[0] for t in texts]
+    g, l, c = pack(progs, cl)
+    _check_colony(oracle, g, l, c, X, y, 1e-3, PLANS[:2], expect_slow=True)
+
+
+def _gcl_to_asm(text):
+    """GCL text as the paper prints it ('LOAD b:1; CONST 0.5; MUL;') -> the test assembler's text."""
+    out = []
+    for cmd in [c.strip() for c in text.split(";") if c.strip()]:
+        parts = cmd.split()
+        out.append("x" + parts[1].split(":")[1] if parts[0] == "LOAD" else parts[1] if parts[0] == "CONST" else {"LN": "LOG"}.get(parts[0], parts[0]))
+    return " ".join(out)
+
+
+def test_the_papers_printed_genomes(oracle):
+    """tests/golden/paper_genomes.txt: the quadratic-formula genomes, DUP / DEL / SQUARE included,
+    are compiled (none is handed to the blockwise kernel) and their records compute what the oracle computes."""
+    import os
+    path = os.path.join(os.path.dirname(__file__), "golden", "paper_genomes.txt")
+    rows = [ln.split("|") for ln in open(path) if ln.strip() and not ln.startswith("#")]
+    assert [int(r[1]) for r in rows] == [12, 12, 24, 25]
+    rng = np.random.default_rng(11)
+    cl = []
+    progs = [asm(_gcl_to_asm(r[2]), cl)[0] for r in rows]
+    assert [len(t) for t in progs] == [12, 12, 24, 25]
+    g, l, c = pack(progs, cl)
+    X, y = _cases(rng, 40, 3, lo=1.0, hi=3.0)
+    _check_colony(oracle, g, l, c, X, y, 1e-3, PLANS, expect_slow=False)
+
+
+def test_corrupted_programs_are_malformed_exactly_when_the_oracle_says_so(oracle):
+    """Single-token corruptions of well-formed programs (an unknown opcode, an argument on a command, a variable or a constant
+    that does not exist, a token dropped or doubled, a COPY without its PASTE): the device's static check and the oracle's agree
+    on every one, and on the depth of the ones that stay programs."""
+    rng = np.random.default_rng(2607)
+    d = 4
+    names = ["ADD", "SUB", "MUL", "DIV", "SIN", "EXP", "DUP", "SWAP", "DEL", "SQUARE", "POW", "TANH"]
+    texts = random_gcl_programs(rng, 600, d, names)
+    cl = []
+    progs = [asm(t, cl)[0].copy() for t in texts]
+    OP = colonies.OP
+    out = []
+    for tok in progs:
+        k = int(rng.integers(8))
+        i = int(rng.integers(len(tok)))
+        if k == 0: tok[i] = colonies.token(int(rng.choice([0, 0x0C, 0x0F, 0x1F, 0x40, 0xFF])), 0)
+        elif k == 1: tok[i] = colonies.token(OP["ADD"], 1 + int(rng.integers(5)))
+        elif k == 2: tok[i] = colonies.token(OP["LOAD"], d + int(rng.integers(3)))
+        elif k == 3: tok[i] = colonies.token(OP["CONST"], len(cl) + int(rng.integers(3)))
+        elif k == 4: tok = np.delete(tok, i)
+        elif k == 5: tok = np.insert(tok, i, tok[i])
+        elif k == 6: tok = np.insert(tok, len(tok), colonies.token(OP["COPY"], int(rng.integers(32))))
+        elif k == 7: tok = np.insert(tok, i, colonies.token(OP["PASTE"], int(rng.integers(34))))
+        if len(tok) >= 1:
+            out.append(tok.astype(np.int32))
+    # and the limits of the stack: 32 terminals are a program, 33 are not
+    ld = colonies.token(OP["LOAD"], 0)
+    add = colonies.token(OP["ADD"])
+    out.append(np.array([ld] * 32 + [add] * 31, np.int32))
+    out.append(np.array([ld] * 33 + [add] * 32, np.int32))
+    g, l, c = pack(out, cl)
+    X, y = _cases(rng, 8, d)
+    orc = oracle.evaluate(g, l, c, X, y, 1e-3)
+    off = np.concatenate([[0], np.cumsum(l, dtype=np.int64)])
+    n_bad = 0
+    for p in range(len(l)):
+        depth, slow, rec = api.beagle_debug_compile(g[off[p]:off[p + 1]], c, d, 2, 1, 1, 2048, 0)
+        assert depth == orc["depth"][p], (p, depth, int(orc["depth"][p]))
+        assert (depth == 0) == bool(orc["flags"][p] & oracle.FLAG_MALFORMED), p
+        n_bad += depth == 0
+    assert 0.3 * len(l) < n_bad < 0.9 * len(l)     # the corruptions bite, and some programs survive them
+    assert orc["depth"][-2] == 32 and orc["depth"][-1] == 0
+
+
+def test_debug_compile_argument_errors():
+    import ctypes
+    l = api.lib()
+    tok = np.array([colonies.token(colonies.OP["LOAD"], 0)], np.int32)
+    rec = np.zeros((4, 2), np.uint32)
+    n, dep, sl = ctypes.c_int32(), ctypes.c_int32(), ctypes.c_int32()
+    def call(tokens=tok.ctypes.data, ln=1, d=1, S=0, kr=0, ku=0):
+        return l.beagle_debug_compile(tokens, ln, None, 0, d, S, kr, ku, 2048, 0, rec.ctypes.data, ctypes.byref(n), ctypes.byref(dep), ctypes.byref(sl))
+    assert call() == api.OK and dep.value == 1 and n.value == 1
+    assert call(tokens=None) == api.ERR_INVALID_ARG
+    assert call(ln=0) == api.ERR_INVALID_ARG and call(ln=513) == api.ERR_INVALID_ARG
+    assert call(d=0) == api.ERR_INVALID_ARG and call(d=33) == api.ERR_INVALID_ARG
+    assert call(S=32) == api.ERR_INVALID_ARG and call(kr=2) == api.ERR_INVALID_ARG and call(ku=2) == api.ERR_INVALID_ARG
