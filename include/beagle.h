@@ -286,6 +286,11 @@ beagle_status beagle_debug_compile(const int32_t* tokens, int32_t len, const flo
                                    int32_t tmem_slots, int32_t k_rcp, int32_t k_un, int32_t un_row_bytes, uint32_t rcp_unsafe,
                                    uint32_t* records, int32_t* n_records, int32_t* depth, int32_t* slow);
 
+/* beagle_debug_std_reward — test only, HOST only, needs no device: the reward of each (f[i], y[i]) pair under the Std family
+ * (BEAGLE_FIT_STD, _SQUARE, _CUBE, _HYPER; Eq. 5), computed by the device's own function compiled for the host (the integer is decided
+ * in fp32: the same IEEE operations in the same order on both). f, y, out: HOST, n floats. BEAGLE_ERR_INVALID_ARG for another `fit`. */
+beagle_status beagle_debug_std_reward(const float* f, const float* y, int64_t n, int32_t fit, float M, float* out);
+
 /* Limits compiled into the library (any pointer may be NULL). */
 void beagle_limits(int32_t* max_len, int32_t* max_stack, int32_t* max_n, int32_t* max_d);
 

@@ -45,6 +45,7 @@ _SIGNATURES = {
     "beagle_debug_chunk_plan": (_i32, [_vp, _i64, _i64, _vp, _i64, ctypes.POINTER(_i64), ctypes.POINTER(_i32), ctypes.POINTER(_i64)]),
     "beagle_debug_compile": (_i32, [_vp, _i32, _vp, _i64, _i32, _i32, _i32, _i32, _i32, ctypes.c_uint32, _vp,
                                     ctypes.POINTER(_i32), ctypes.POINTER(_i32), ctypes.POINTER(_i32)]),
+    "beagle_debug_std_reward": (_i32, [_vp, _vp, _i64, _i32, _f32, _vp]),
     "beagle_debug_walk_tables": (None, [ctypes.POINTER(ctypes.c_uint32), ctypes.POINTER(ctypes.c_uint32)]),
     "beagle_limits": (None, [ctypes.POINTER(_i32)] * 4),
     "beagle_status_string": (ctypes.c_char_p, [_i32]),
@@ -170,6 +171,15 @@ def beagle_debug_compile(tokens, consts, d, tmem_slots, k_rcp, k_un, un_row_byte
                                       int(tmem_slots), int(k_rcp), int(k_un), int(un_row_bytes), int(rcp_unsafe), _ptr(rec),
                                       ctypes.byref(n), ctypes.byref(depth), ctypes.byref(slow)), "beagle_debug_compile")
     return depth.value, bool(slow.value), rec[: n.value]
+
+
+def beagle_debug_std_reward(f, y, fit, M):
+    """Rewards of the pairs (f[i], y[i]) by the device's std_reward compiled for the host; numpy in, numpy out."""
+    import numpy as np
+    f = np.ascontiguousarray(f, np.float32); y = np.ascontiguousarray(y, np.float32)
+    out = np.empty(len(f), np.float32)
+    _check(lib().beagle_debug_std_reward(_ptr(f), _ptr(y), len(f), int(fit), float(M), _ptr(out)), "beagle_debug_std_reward")
+    return out
 
 
 def beagle_limits():

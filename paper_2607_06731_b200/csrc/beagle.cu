@@ -1157,6 +1157,16 @@ void beagle_debug_walk_tables(uint32_t* lut160, uint32_t* tok130)
     if (tok130) for (int i = 0; i < kTok2Size; ++i) { tok130[2 * i] = tt[i].x; tok130[2 * i + 1] = tt[i].y; }
 }
 
+// host only: std_reward (fit_std.cuh), the reward of one (output, target) pair of the Std family, compiled for the host
+beagle_status beagle_debug_std_reward(const float* f, const float* y, int64_t n, int32_t fit, float M, float* out)
+{
+    int kind, power;
+    if (n < 0 || (n > 0 && (!f || !y || !out)) || !decode_fit(fit, &kind, &power) || kind != BEAGLE_FIT_STD) return BEAGLE_ERR_INVALID_ARG;
+    const float pen = M / 11.f;                   // the kernels' __fdiv_rn(M, 11.f)
+    for (int64_t i = 0; i < n; ++i) out[i] = std_reward(f[i], y[i], M, pen, power);
+    return BEAGLE_OK;
+}
+
 // host only: compile_general (compile_kernel.inc), the compiler of the whole language that k_compile_general runs one lane per
 // program, compiled for the host and run on one program
 beagle_status beagle_debug_compile(const int32_t* tokens, int32_t len, const float* consts, int64_t n_consts, int32_t d,

@@ -8,25 +8,46 @@
 // it is still taken in the fixed order of the other reductions.
 #pragma once
 #include <stdint.h>
+#include <string.h>
+#include <math.h>
+
+// std_reward is compiled for the host too (beagle_debug_std_reward, test only: the integer a reward is rounded to is decided by fp32
+// arithmetic, and a CPU test holds this function against the oracle's bit for bit). The device build is these intrinsics, unchanged;
+// on the host the same IEEE single-precision operations written plainly (no contraction: mul and sub are separate statements and the
+// host build has no fused multiply-add to contract them into).
+#ifdef __CUDA_ARCH__
+#define BGS_DIV(a, b) __fdiv_rn(a, b)
+#define BGS_MUL(a, b) __fmul_rn(a, b)
+#define BGS_SUB(a, b) __fsub_rn(a, b)
+#define BGS_INF       __int_as_float(0x7f800000)
+#define BGS_BITS(f)   __float_as_int(f)
+#else
+namespace beagle { inline int std_bits_host(float f) { int i; memcpy(&i, &f, 4); return i; } }
+#define BGS_DIV(a, b) ((float)(a) / (float)(b))
+#define BGS_MUL(a, b) ((float)(a) * (float)(b))
+#define BGS_SUB(a, b) ((float)(a) - (float)(b))
+#define BGS_INF       INFINITY
+#define BGS_BITS(f)   beagle::std_bits_host(f)
+#endif
 
 namespace beagle {
 
 // Straight-line (selects, no branches: the cases of a lane take the same path); the arithmetic and its order are the
 // oracle's. yv: the target is finite (it does not change with the individual).
-__device__ __forceinline__ float std_reward(float f, float y, float M, float pen, int power)
+__host__ __device__ __forceinline__ float std_reward(float f, float y, float M, float pen, int power)
 {
     const float a = fabsf(f), b = fabsf(y);
-    const bool vf = a < __int_as_float(0x7f800000), vy = b < __int_as_float(0x7f800000);
+    const bool vf = a < BGS_INF, vy = b < BGS_INF;
     const float mx = fmaxf(a, b), mn = fminf(a, b);
-    const float q = __fdiv_rn(mn, mx);                       // 0/0, inf/inf: NaN, replaced below
+    const float q = BGS_DIV(mn, mx);                         // 0/0, inf/inf: NaN, replaced below
     float qp = q;
-    if (power == 2) qp = __fmul_rn(q, q);                    // warp-uniform
-    else if (power == 3) qp = __fmul_rn(__fmul_rn(q, q), q);
-    else if (power == 8) { qp = __fmul_rn(q, q); qp = __fmul_rn(qp, qp); qp = __fmul_rn(qp, qp); }
-    const float t = __fmul_rn(M, qp);
+    if (power == 2) qp = BGS_MUL(q, q);                      // warp-uniform
+    else if (power == 3) qp = BGS_MUL(BGS_MUL(q, q), q);
+    else if (power == 8) { qp = BGS_MUL(q, q); qp = BGS_MUL(qp, qp); qp = BGS_MUL(qp, qp); }
+    const float t = BGS_MUL(M, qp);
     // opposite signs: both non-zero and the sign bits differ (decided on the signs, not on a product that may underflow)
-    const bool opp = mn > 0.f && ((__float_as_int(f) ^ __float_as_int(y)) < 0);
-    float r = rintf(opp ? __fsub_rn(t, pen) : t);
+    const bool opp = mn > 0.f && ((BGS_BITS(f) ^ BGS_BITS(y)) < 0);
+    float r = rintf(opp ? BGS_SUB(t, pen) : t);
     r = mx == 0.f ? M : r;
     return (vf && vy) ? r : (vf != vy ? -M : M);
 }

@@ -301,3 +301,55 @@ def test_debug_compile_argument_errors():
     assert call(ln=0) == api.ERR_INVALID_ARG and call(ln=513) == api.ERR_INVALID_ARG
     assert call(d=0) == api.ERR_INVALID_ARG and call(d=33) == api.ERR_INVALID_ARG
     assert call(S=32) == api.ERR_INVALID_ARG and call(kr=2) == api.ERR_INVALID_ARG and call(ku=2) == api.ERR_INVALID_ARG
+
+
+# ---- the Std family's reward: the device's function, compiled for the host, against the oracle's, bit for bit -----------------
+def _oracle_rewards(oracle, f, y, power, M):
+    """reward(f[k], y[i]) for every pair of the two sweeps, from the oracle: programs 'CONST f[k]' on the one-case dataset y[i],
+    tax 0, so that the fitness of a program is the reward of its one case."""
+    tok = np.array([colonies.token(colonies.OP["CONST"], k) for k in range(len(f))], np.int32)
+    lengths = np.ones(len(f), np.int32)
+    out = np.empty((len(y), len(f)), np.float32)
+    X = np.zeros((1, 1), np.float32)
+    for i, yi in enumerate(y):
+        r = oracle.evaluate_std(tok, lengths, f, X, np.array([yi], np.float32), power, M, 0.0, mode=1)
+        out[i] = r["fitness"]
+    return out
+
+
+@pytest.mark.parametrize("fit,power", [(api.FIT_STD, 1), (api.FIT_STD_SQUARE, 2), (api.FIT_STD_CUBE, 3), (api.FIT_STD_HYPER, 8)])
+def test_std_reward_of_the_device_is_the_oracles_bit_for_bit(oracle, fit, power):
+    """Eq. 5 decides an integer by floating point, so both sides take the decision in fp32 in one stated order (R25).
+    Here the device's own function (csrc/fit_std.cuh, host build) meets the oracle's on a sweep that has every branch: equal and
+    opposite signs, zeros of both signs, denormals, huge and tiny ratios, ratios on both sides of the rounding boundaries and ties,
+    infinities and NaN on either side."""
+    rng = np.random.default_rng(500 + power)
+    M = 10000.0
+    special = np.array([0.0, -0.0, 1e-45, -1e-45, 1e-38, 3.4e38, -3.4e38, np.inf, -np.inf, np.nan, 1.0, -1.0, 0.5, 2.0, 3.0, -3.0], np.float32)
+    mags = np.exp(rng.uniform(np.log(1e-6), np.log(1e6), 150)).astype(np.float32) * rng.choice([-1, 1], 150).astype(np.float32)
+    # ratios whose M q^p is near k + 1/2: q = ((k + 1/2) / M)^(1/p) against a target of 1, and its neighbours in fp32
+    k = rng.integers(0, 10000, 60).astype(np.float64)
+    q = (((k + 0.5) / M) ** (1.0 / power)).astype(np.float32)
+    near = np.concatenate([q, np.nextafter(q, np.float32(0)), np.nextafter(q, np.float32(2)), -q])
+    f = np.concatenate([special, mags, near]).astype(np.float32)
+    y = np.concatenate([special, np.array([1.0, -1.0, 7.25, -0.3], np.float32), mags[:12]]).astype(np.float32)
+    want = _oracle_rewards(oracle, f, y, power, M)
+    n_ties = 0
+    for i, yi in enumerate(y):
+        got = api.beagle_debug_std_reward(f, np.full(len(f), yi, np.float32), fit, M)
+        assert np.array_equal(got.view(np.uint32), want[i].view(np.uint32)), \
+            (float(yi), [(float(a), float(b), float(c)) for a, b, c in zip(f, got, want[i]) if b != c][:5])
+        assert np.all(got == np.rint(got)) and np.all(np.abs(got) <= M)          # integers within [-M, M]
+    # the sweep reaches every branch of Eq. 5
+    allw = want.ravel()
+    assert (allw == M).any() and (allw == -M).any() and (allw < 0).any() and (allw == 0).any()
+    assert len(np.unique(allw)) > 300
+
+
+def test_std_reward_argument_errors():
+    one = np.zeros(1, np.float32)
+    l = api.lib()
+    assert l.beagle_debug_std_reward(one.ctypes.data, one.ctypes.data, 1, api.FIT_MSE, 1.0, one.ctypes.data) == api.ERR_INVALID_ARG
+    assert l.beagle_debug_std_reward(one.ctypes.data, one.ctypes.data, 1, api.FIT_CORRELATION, 1.0, one.ctypes.data) == api.ERR_INVALID_ARG
+    assert l.beagle_debug_std_reward(None, one.ctypes.data, 1, api.FIT_STD, 1.0, one.ctypes.data) == api.ERR_INVALID_ARG
+    assert l.beagle_debug_std_reward(None, None, 0, api.FIT_STD, 1.0, None) == api.OK
