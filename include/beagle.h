@@ -286,6 +286,15 @@ beagle_status beagle_debug_compile(const int32_t* tokens, int32_t len, const flo
                                    int32_t tmem_slots, int32_t k_rcp, int32_t k_un, int32_t un_row_bytes, uint32_t rcp_unsafe,
                                    uint32_t* records, int32_t* n_records, int32_t* depth, int32_t* slow);
 
+/* beagle_debug_walk — test only, HOST only, needs no device: the body of k_compile's table-driven walk (csrc/walk_body.inc, the source
+ * both the kernel and this call are compiled from) on ONE program; f1 != 0: the instantiation that also takes DUP SWAP DEL SIGN SQUARE
+ * CUBE. Arguments as beagle_debug_compile. *taken = 1 if the walk compiled the program, 0 if it turned it down (anything that is not
+ * a well-formed program of its commands: k_compile_general looks at those); for taken programs *depth, records and *n_records as
+ * beagle_debug_compile, *used_f1 = 1 if one of the six extra commands occurred. Same difference from the device (1 / c in IEEE). */
+beagle_status beagle_debug_walk(const int32_t* tokens, int32_t len, const float* consts, int64_t n_consts, int32_t d,
+                                int32_t tmem_slots, int32_t k_rcp, int32_t k_un, int32_t un_row_bytes, uint32_t rcp_unsafe, int32_t f1,
+                                uint32_t* records, int32_t* n_records, int32_t* depth, int32_t* taken, int32_t* used_f1);
+
 /* beagle_debug_std_reward — test only, HOST only, needs no device: the reward of each (f[i], y[i]) pair under the Std family
  * (BEAGLE_FIT_STD, _SQUARE, _CUBE, _HYPER; Eq. 5), computed by the device's own function compiled for the host (the integer is decided
  * in fp32: the same IEEE operations in the same order on both). f, y, out: HOST, n floats. BEAGLE_ERR_INVALID_ARG for another `fit`. */

@@ -45,6 +45,8 @@ _SIGNATURES = {
     "beagle_debug_chunk_plan": (_i32, [_vp, _i64, _i64, _vp, _i64, ctypes.POINTER(_i64), ctypes.POINTER(_i32), ctypes.POINTER(_i64)]),
     "beagle_debug_compile": (_i32, [_vp, _i32, _vp, _i64, _i32, _i32, _i32, _i32, _i32, ctypes.c_uint32, _vp,
                                     ctypes.POINTER(_i32), ctypes.POINTER(_i32), ctypes.POINTER(_i32)]),
+    "beagle_debug_walk": (_i32, [_vp, _i32, _vp, _i64, _i32, _i32, _i32, _i32, _i32, ctypes.c_uint32, _i32, _vp,
+                                 ctypes.POINTER(_i32), ctypes.POINTER(_i32), ctypes.POINTER(_i32), ctypes.POINTER(_i32)]),
     "beagle_debug_std_reward": (_i32, [_vp, _vp, _i64, _i32, _f32, _vp]),
     "beagle_debug_walk_tables": (None, [ctypes.POINTER(ctypes.c_uint32), ctypes.POINTER(ctypes.c_uint32)]),
     "beagle_limits": (None, [ctypes.POINTER(_i32)] * 4),
@@ -171,6 +173,19 @@ def beagle_debug_compile(tokens, consts, d, tmem_slots, k_rcp, k_un, un_row_byte
                                       int(tmem_slots), int(k_rcp), int(k_un), int(un_row_bytes), int(rcp_unsafe), _ptr(rec),
                                       ctypes.byref(n), ctypes.byref(depth), ctypes.byref(slow)), "beagle_debug_compile")
     return depth.value, bool(slow.value), rec[: n.value]
+
+
+def beagle_debug_walk(tokens, consts, d, tmem_slots, k_rcp, k_un, un_row_bytes, rcp_unsafe=0, f1=False):
+    """One program through the host build of k_compile's walk: (taken, depth, used_f1, records uint32[n, 2]); numpy in, numpy out."""
+    import numpy as np
+    tokens = np.ascontiguousarray(tokens, np.int32)
+    consts = np.ascontiguousarray(consts, np.float32)
+    rec = np.zeros((len(tokens) + 8, 2), np.uint32)
+    n, depth, taken, used = _i32(0), _i32(0), _i32(0), _i32(0)
+    _check(lib().beagle_debug_walk(_ptr(tokens), len(tokens), _ptr(consts) if len(consts) else None, len(consts), int(d),
+                                   int(tmem_slots), int(k_rcp), int(k_un), int(un_row_bytes), int(rcp_unsafe), int(bool(f1)), _ptr(rec),
+                                   ctypes.byref(n), ctypes.byref(depth), ctypes.byref(taken), ctypes.byref(used)), "beagle_debug_walk")
+    return bool(taken.value), depth.value, bool(used.value), rec[: n.value]
 
 
 def beagle_debug_std_reward(f, y, fit, M):

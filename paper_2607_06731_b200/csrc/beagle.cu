@@ -1167,6 +1167,34 @@ beagle_status beagle_debug_std_reward(const float* f, const float* y, int64_t n,
     return BEAGLE_OK;
 }
 
+// host only: the body of k_compile's walk (walk_body.inc) on one program
+beagle_status beagle_debug_walk(const int32_t* tokens, int32_t len, const float* consts, int64_t n_consts, int32_t d,
+                                int32_t tmem_slots, int32_t k_rcp, int32_t k_un, int32_t un_row_bytes, uint32_t rcp_unsafe, int32_t f1,
+                                uint32_t* records, int32_t* n_records, int32_t* depth, int32_t* taken, int32_t* used_f1)
+{
+    if (!tokens || len < 1 || len > BEAGLE_MAX_LEN || d < 1 || d > BEAGLE_MAX_D || n_consts < 0 || n_consts > BEAGLE_MAX_CONSTS
+        || (n_consts > 0 && !consts) || tmem_slots < 0 || tmem_slots > kMemSlots || k_rcp < 0 || k_rcp > d || k_un < 0 || k_un > d
+        || un_row_bytes < 0 || !records || !n_records || !depth || !taken || !used_f1)
+        return BEAGLE_ERR_INVALID_ARG;
+    Header hdr = {}; hdr.rcp_unsafe = rcp_unsafe;
+    uint2 uops[BEAGLE_MAX_LEN + 8] = {};
+    int4 meta[1] = {}; int dep[1] = { 0 }; int gen_list[1] = { -1 }, slow_list[1] = { -1 };
+    CompileParams q = {};
+    q.genomes = reinterpret_cast<const uint32_t*>(tokens);
+    q.consts = consts; q.n_consts = n_consts; q.d = d; q.tmem_slots = tmem_slots; q.k_rcp = k_rcp; q.k_un = k_un; q.un_row_bytes = un_row_bytes;
+    q.hdr = &hdr; q.uops = uops; q.ucap = BEAGLE_MAX_LEN + 8; q.meta = meta; q.depth = dep; q.slow_list = slow_list; q.gen_list = gen_list;
+    q.emit = 1;
+    if (f1) walk_host<true>(q, len); else walk_host<false>(q, len);
+    *taken = hdr.n_general == 0 ? 1 : 0;
+    *depth = *taken ? dep[0] : 0;
+    *used_f1 = hdr.n_f1;
+    int n = 0;
+    if (*taken) { while (n < BEAGLE_MAX_LEN + 4 && (uops[n].x & 255u) != H_END) ++n; }
+    *n_records = n;
+    for (int k = 0; k < n; ++k) { records[2 * k] = uops[k].x; records[2 * k + 1] = uops[k].y; }
+    return BEAGLE_OK;
+}
+
 // host only: compile_general (compile_kernel.inc), the compiler of the whole language that k_compile_general runs one lane per
 // program, compiled for the host and run on one program
 beagle_status beagle_debug_compile(const int32_t* tokens, int32_t len, const float* consts, int64_t n_consts, int32_t d,

@@ -353,3 +353,106 @@ def test_std_reward_argument_errors():
     assert l.beagle_debug_std_reward(one.ctypes.data, one.ctypes.data, 1, api.FIT_CORRELATION, 1.0, one.ctypes.data) == api.ERR_INVALID_ARG
     assert l.beagle_debug_std_reward(None, one.ctypes.data, 1, api.FIT_STD, 1.0, one.ctypes.data) == api.ERR_INVALID_ARG
     assert l.beagle_debug_std_reward(None, None, 0, api.FIT_STD, 1.0, None) == api.OK
+
+
+# ---- k_compile's own walk (csrc/walk_body.inc: the source the kernel and beagle_debug_walk are both compiled from) ---------------
+HOT = {colonies.OP[n] for n in ("CONST", "LOAD", "ADD", "SUB", "MUL", "DIV", "SIN", "COS", "LOG", "SQRT", "EXP")}
+F1 = {colonies.OP[n] for n in ("DUP", "SWAP", "DEL", "SIGN", "SQUARE", "CUBE")}
+
+
+def _check_walk(oracle, genomes, lengths, consts, X, y, tax, plans, run_machine=True):
+    """Every program through the walk's host build, both instantiations, for each plan. The walk takes a program exactly when it is
+    a well-formed program of its commands (the oracle's static check decides well-formed); what it takes it compiles to the records
+    the general compiler emits (the two are different code: a table-driven loop and a switch), with the oracle's depth; the records
+    compute the program (the micro-op machine against the oracle's fitness)."""
+    d = X.shape[1]
+    orc = oracle.evaluate(genomes, lengths, consts, X, y, tax)
+    unsafe = sum(1 << j for j in range(d) if np.any(np.abs(X[:, j]) < EPS))
+    off = np.concatenate([[0], np.cumsum(lengths, dtype=np.int64)])
+    taken_n = {False: 0, True: 0}
+    for S_T, k_rcp, k_un in plans:
+        fit = np.full(len(lengths), np.nan, np.float32)
+        ran = np.zeros(len(lengths), bool)
+        for p in range(len(lengths)):
+            tok = genomes[off[p]:off[p + 1]]
+            ops = set((tok.view(np.uint32) & 0xFF).tolist())
+            wellformed = not (orc["flags"][p] & oracle.FLAG_MALFORMED)
+            gdepth, gslow, grec = api.beagle_debug_compile(tok, consts, d, S_T, k_rcp, k_un, 2048, unsafe)
+            for f1 in (False, True):
+                taken, depth, used, rec = api.beagle_debug_walk(tok, consts, d, S_T, k_rcp, k_un, 2048, unsafe, f1=f1)
+                mine = ops <= (HOT | F1 if f1 else HOT)
+                assert taken == (wellformed and mine), (p, f1, taken, wellformed, sorted(ops))
+                if not taken:
+                    continue
+                taken_n[f1] += 1
+                assert depth == orc["depth"][p] and not gslow, (p, f1, depth, int(orc["depth"][p]))
+                assert used == (f1 and bool(ops & F1)), (p, f1, used)
+                assert np.array_equal(rec, grec), (p, f1, rec.tolist(), grec.tolist())
+            if run_machine and wellformed and ops <= HOT | F1:
+                _, _, _, rec = api.beagle_debug_walk(tok, consts, d, S_T, k_rcp, k_un, 2048, unsafe, f1=True)
+                fit[p] = _fitness(run_records(rec, X, d, S_T, k_rcp, k_un, 2048), y, tax, len(tok))
+                ran[p] = True
+        if run_machine:
+            sel = np.nonzero(ran)[0]
+            sub = {k: orc[k][sel] for k in ("fitness", "bound", "flags", "depth")}
+            rep = parity.compare(fit[sel], sub)
+            assert len(rep["bad"]) == 0, parity.describe(rep, fit[sel], sub)
+    return taken_n
+
+
+def test_walk_takes_and_compiles_the_hot_path_colonies(oracle):
+    for number, P in ((1, 300), (2, 200), (3, 300), (4, 200), (5, 400)):
+        cfg = colonies.CONFIGS[number]
+        g, l, c = colonies.generate_programs(cfg, P)
+        X, y, _ = colonies.make_dataset(cfg)
+        taken = _check_walk(oracle, g, l, c, X[:48], y[:48], cfg.tax, PLANS if number == 5 else PLANS[:2])
+        assert taken[False] == taken[True] == P * (len(PLANS) if number == 5 else 2)      # every program of the five configs is the walk's
+
+
+def test_walk_f1_instantiation_takes_the_stack_commands(oracle):
+    cfg = colonies.CONFIGS[3]
+    g, l, c = colonies.generate_programs(cfg, 400, gcl_mix="f1")
+    X, y, _ = colonies.make_dataset(cfg)
+    taken = _check_walk(oracle, g, l, c, X[:40], y[:40], cfg.tax, PLANS[:3])
+    assert taken[True] == 400 * 3 and taken[False] < 0.3 * 400 * 3          # 88 % of the f1 mix's programs use one of the six
+    rng = np.random.default_rng(77)
+    texts = random_gcl_programs(rng, 500, 3, ["ADD", "SUB", "MUL", "DIV", "SIN", "LOG", "EXP", "DUP", "SWAP", "DEL", "SIGN", "SQUARE", "CUBE"])
+    cl = []
+    progs = [asm(t, cl)[0] for t in texts]
+    gg, ll, cc = pack(progs, cl)
+    Xr, yr = _cases(rng, 40, 3, zero_in=0)
+    _check_walk(oracle, gg, ll, cc, Xr, yr, 1e-3, PLANS)
+
+
+def test_walk_turns_down_exactly_what_is_not_its_own(oracle):
+    """Programs of the whole language and corrupted ones: the walk takes the well-formed programs of its commands and nothing else
+    (a program it turns down is looked at again by the general compiler on the device: nothing is lost, only time)."""
+    rng = np.random.default_rng(4242)
+    d = 4
+    names = ["ADD", "SUB", "MUL", "DIV", "SIN", "EXP", "SQRT", "DUP", "SWAP", "DEL", "SQUARE", "POW", "TANH"]
+    texts = random_gcl_programs(rng, 500, d, names) + random_gcl_programs(rng, 300, d, ["ADD", "SUB", "MUL", "DIV", "COS", "LOG"])
+    cl = []
+    progs = [asm(t, cl)[0].copy() for t in texts]
+    OP = colonies.OP
+    out = []
+    for tok in progs:
+        k = int(rng.integers(10))                  # 0-5: one corruption; 6-9: left alone
+        i = int(rng.integers(len(tok)))
+        if k == 0: tok[i] = colonies.token(int(rng.choice([0, 0x0C, 0x0F, 0x13, 0x1F, 0x40, 0xFF])), 0)
+        elif k == 1: tok[i] = colonies.token(int(tok[i]) & 0xFF, 1 + int(rng.integers(5))) if (int(tok[i]) & 0xFF) > 2 else tok[i]
+        elif k == 2: tok[i] = colonies.token(OP["LOAD"], d + int(rng.integers(3)))
+        elif k == 3: tok[i] = colonies.token(OP["CONST"], len(cl) + int(rng.integers(3)))
+        elif k == 4: tok = np.delete(tok, i)
+        elif k == 5: tok = np.insert(tok, i, tok[i])
+        if len(tok) >= 1:
+            out.append(tok.astype(np.int32))
+    ld, add = colonies.token(OP["LOAD"], 0), colonies.token(OP["ADD"])
+    out.append(np.array([ld] * 32 + [add] * 31, np.int32))          # the deepest stack that is a program
+    out.append(np.array([ld] * 33 + [add] * 32, np.int32))          # one more is not
+    out.append(np.array([ld] * 256 + [add] * 255, np.int32)[:512])  # (and a long one that overflows early)
+    for text in ("x0 DEL", "x0 x1 ADD DEL", "x0 x1 DEL DEL", "x0 DUP DEL DEL", "x0 DEL x1"):      # an empty stack at the end is not a program; in between it is
+        out.append(asm(text)[0])
+    g, l, c = pack(out, cl)
+    X, y = _cases(rng, 8, d)
+    taken = _check_walk(oracle, g, l, c, X, y, 1e-3, [(2, 1, 1)], run_machine=False)
+    assert 0.15 * len(l) < taken[False] < taken[True] < 0.85 * len(l)
