@@ -120,3 +120,44 @@ def test_bench_reference_arm_other_ranks_exit_without_work():
     r = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--impl", "reference", "--gpus", "2"],
                        env=env, capture_output=True, text=True, timeout=120)
     assert r.returncode == 0 and r.stdout.strip() == ""
+
+
+def _c_constants(path, pattern):
+    """name -> int for every `NAME = value` / `#define NAME value` in a C source that matches `pattern` (comments stripped)."""
+    text = re.sub(r"/\*.*?\*/", "", open(path).read(), flags=re.S)
+    out = {}
+    for name, val in re.findall(pattern, text):
+        out[name] = int(val, 0)
+    return out
+
+
+def test_retyped_constants_agree_everywhere():
+    """The opcode numbers, limits, status codes and fitness selectors are typed out in several places that must not share code
+    (the header, the binding, the input generators, the oracle: 'numbers retyped, not shared'): they have to stay the same numbers."""
+    hdr = os.path.join(ROOT, "include", "beagle.h")
+    ops_h = {k[len("BEAGLE_OP_"):]: v for k, v in _c_constants(hdr, r"#define\s+(BEAGLE_OP_[A-Z]+)\s+(0x[0-9A-Fa-f]+|\d+)").items()}
+    assert len(ops_h) == 26 and ops_h == colonies.OP                                     # header == generators / test assembler
+    ops_o = {k[len("OP_"):]: v for k, v in _c_constants(os.path.join(ROOT, "oracle", "beagle_oracle.c"),
+                                                        r"\b(OP_[A-Z]+)\s*=\s*(0x[0-9A-Fa-f]+|\d+)").items()}
+    assert ops_o == ops_h                                                                # == the oracle's own enum
+    ops_g = {k[len("OP_"):]: v for k, v in _c_constants(os.path.join(ROOT, "paper_2607_06731_b200", "colonies", "gen.c"),
+                                                        r"\b(OP_[A-Z]+)\s*=\s*(0x[0-9A-Fa-f]+|\d+)").items()}
+    assert ops_g and all(ops_h[k] == v for k, v in ops_g.items())                        # the C generator names a subset
+    lim = _c_constants(hdr, r"#define\s+(BEAGLE_MAX_[A-Z]+)\s+(\d+)")
+    assert (lim["BEAGLE_MAX_LEN"], lim["BEAGLE_MAX_STACK"], lim["BEAGLE_MAX_N"], lim["BEAGLE_MAX_D"], lim["BEAGLE_MAX_VARS"]) == (512, 32, 1024, 32, 32)
+    olim = _c_constants(os.path.join(ROOT, "oracle", "beagle_oracle.c"), r"#define\s+(ORC_MAX_[A-Z]+)\s+(\d+)")
+    assert (olim["ORC_MAX_LEN"], olim["ORC_MAX_STACK"], olim["ORC_MAX_N"], olim["ORC_MAX_VARS"]) == (512, 32, 1024, 32)
+    st = _c_constants(hdr, r"\b(BEAGLE_(?:OK|ERR_[A-Z_]+))\s*=\s*(-?\d+)")
+    assert st == dict(BEAGLE_OK=api.OK, BEAGLE_ERR_INVALID_ARG=api.ERR_INVALID_ARG, BEAGLE_ERR_UNSUPPORTED=api.ERR_UNSUPPORTED,
+                      BEAGLE_ERR_CUDA=api.ERR_CUDA, BEAGLE_ERR_NOMEM=api.ERR_NOMEM, BEAGLE_ERR_NOT_RESERVED=api.ERR_NOT_RESERVED)
+    for s in st.values():
+        assert api.beagle_status_string(s) != "unknown status"
+    fit = _c_constants(hdr, r"#define\s+(BEAGLE_FIT_[A-Z_]+)\s+(\d+)")
+    assert fit == dict(BEAGLE_FIT_MSE=api.FIT_MSE, BEAGLE_FIT_CORRELATION=api.FIT_CORRELATION, BEAGLE_FIT_STD=api.FIT_STD,
+                       BEAGLE_FIT_STD_SQUARE=api.FIT_STD_SQUARE, BEAGLE_FIT_STD_CUBE=api.FIT_STD_CUBE, BEAGLE_FIT_STD_HYPER=api.FIT_STD_HYPER)
+    # Table 2, typed out in the header, the binding and the ranking oracle
+    m = re.search(r"BEAGLE_TABLE2\[10\]\s*=\s*\{([^}]*)\}", open(hdr).read())
+    table_h = tuple(float(x.strip().rstrip("f")) for x in m.group(1).split(","))
+    from oracle import ranking
+    assert table_h == api.TABLE2 == tuple(float(x) for x in ranking.EXPECTED_CHILDREN)
+    assert abs(sum(table_h) / 10 - 1.0) < 1e-12                                          # the paper's table averages one child
