@@ -286,6 +286,19 @@ beagle_status beagle_debug_compile(const int32_t* tokens, int32_t len, const flo
                                    int32_t tmem_slots, int32_t k_rcp, int32_t k_un, int32_t un_row_bytes, uint32_t rcp_unsafe,
                                    uint32_t* records, int32_t* n_records, int32_t* depth, int32_t* slow);
 
+/* beagle_debug_queue — test only, HOST only, needs no device: the scheduling loop of ONE warp of the interpreter kernel (csrc/queue_body.inc,
+ * the source both k_eval and this call are compiled from) over a given queue. meta4: HOST, `total` entries of four ints as k_compile leaves
+ * them in evaluation order (x = individual, y = record block in 16-byte units, z = records to copy, 0 = nothing to run, w = length);
+ * max_len, ring_bytes, grid, threads: what the launch would have (longest program, bytes of a warp's ring, CTAs, threads per CTA);
+ * grouped != 0: the MSE-without-outputs instantiation (one interpreter entry per group). skip_seed != 0: after each visit of this warp the
+ * queue moves on by 0..3 more batches (other warps' visits); queue_start: where the queue stands when the warp arrives.
+ * events (HOST, cap x 4 ints; *n_events = how many there were): 0 visit (first entry, batch); 1 bulk copy (stage, source in 16-byte units,
+ * bytes); 2 barrier wait (stage, phase parity); 3 a group handed to the interpreter (byte offset in the ring, programs); 4 one program
+ * handed to it (byte offset, individual, length). sizing3: entries per visit, bytes per stage, stages. */
+beagle_status beagle_debug_queue(const int32_t* meta4, int32_t total, int32_t max_len, int32_t ring_bytes, int32_t grid, int32_t threads,
+                                 int32_t grouped, uint32_t skip_seed, uint32_t queue_start, int32_t* events, int32_t cap,
+                                 int32_t* n_events, int32_t* sizing3);
+
 /* beagle_debug_walk — test only, HOST only, needs no device: the body of k_compile's table-driven walk (csrc/walk_body.inc, the source
  * both the kernel and this call are compiled from) on ONE program; f1 != 0: the instantiation that also takes DUP SWAP DEL SIGN SQUARE
  * CUBE. Arguments as beagle_debug_compile. *taken = 1 if the walk compiled the program, 0 if it turned it down (anything that is not

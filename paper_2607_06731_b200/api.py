@@ -45,6 +45,8 @@ _SIGNATURES = {
     "beagle_debug_chunk_plan": (_i32, [_vp, _i64, _i64, _vp, _i64, ctypes.POINTER(_i64), ctypes.POINTER(_i32), ctypes.POINTER(_i64)]),
     "beagle_debug_compile": (_i32, [_vp, _i32, _vp, _i64, _i32, _i32, _i32, _i32, _i32, ctypes.c_uint32, _vp,
                                     ctypes.POINTER(_i32), ctypes.POINTER(_i32), ctypes.POINTER(_i32)]),
+    "beagle_debug_queue": (_i32, [_vp, _i32, _i32, _i32, _i32, _i32, _i32, ctypes.c_uint32, ctypes.c_uint32, _vp, _i32,
+                                  ctypes.POINTER(_i32), ctypes.POINTER(_i32)]),
     "beagle_debug_walk": (_i32, [_vp, _i32, _vp, _i64, _i32, _i32, _i32, _i32, _i32, ctypes.c_uint32, _i32, _vp,
                                  ctypes.POINTER(_i32), ctypes.POINTER(_i32), ctypes.POINTER(_i32), ctypes.POINTER(_i32)]),
     "beagle_debug_std_reward": (_i32, [_vp, _vp, _i64, _i32, _f32, _vp]),
@@ -173,6 +175,21 @@ def beagle_debug_compile(tokens, consts, d, tmem_slots, k_rcp, k_un, un_row_byte
                                       int(tmem_slots), int(k_rcp), int(k_un), int(un_row_bytes), int(rcp_unsafe), _ptr(rec),
                                       ctypes.byref(n), ctypes.byref(depth), ctypes.byref(slow)), "beagle_debug_compile")
     return depth.value, bool(slow.value), rec[: n.value]
+
+
+def beagle_debug_queue(meta4, max_len, ring_bytes, grid, threads, grouped, skip_seed=0, queue_start=0):
+    """One warp of k_eval's scheduling loop on the host: (events int32[n, 4], (batch, stage_bytes, stages)); numpy in, numpy out."""
+    import numpy as np
+    meta4 = np.ascontiguousarray(meta4, np.int32).reshape(-1, 4)
+    cap = 6 * len(meta4) + 64
+    ev = np.zeros((cap, 4), np.int32)
+    n = _i32(0)
+    sizing = (_i32 * 3)()
+    _check(lib().beagle_debug_queue(_ptr(meta4) if len(meta4) else None, len(meta4), int(max_len), int(ring_bytes), int(grid), int(threads),
+                                    int(bool(grouped)), int(skip_seed), int(queue_start), _ptr(ev), cap, ctypes.byref(n), sizing),
+           "beagle_debug_queue")
+    assert n.value <= cap, "event buffer too small"
+    return ev[: n.value], tuple(sizing)
 
 
 def beagle_debug_walk(tokens, consts, d, tmem_slots, k_rcp, k_un, un_row_bytes, rcp_unsafe=0, f1=False):

@@ -1167,6 +1167,24 @@ beagle_status beagle_debug_std_reward(const float* f, const float* y, int64_t n,
     return BEAGLE_OK;
 }
 
+// host only: one warp of k_eval's scheduling loop (queue_body.inc) over a given list of queue entries, as a list of events
+beagle_status beagle_debug_queue(const int32_t* meta4, int32_t total, int32_t max_len, int32_t ring_bytes, int32_t grid, int32_t threads,
+                                 int32_t grouped, uint32_t skip_seed, uint32_t queue_start, int32_t* events, int32_t cap,
+                                 int32_t* n_events, int32_t* sizing3)
+{
+    if (total < 0 || (total > 0 && !meta4) || max_len < 1 || max_len > BEAGLE_MAX_LEN || ring_bytes < kStageBytesMax || grid < 1
+        || threads < 32 || threads > 1024 || (threads & 31) || cap < 0 || (cap > 0 && !events) || !n_events || !sizing3)
+        return BEAGLE_ERR_INVALID_ARG;
+    QueueLog L = { events, cap, 0 };
+    unsigned int queue = queue_start;
+    if (total > 0) {                               // (k_eval returns at once when nothing is sorted)
+        if (grouped) queue_host<true>(reinterpret_cast<const int4*>(meta4), total, max_len, ring_bytes, grid, threads, &queue, skip_seed, L, sizing3);
+        else queue_host<false>(reinterpret_cast<const int4*>(meta4), total, max_len, ring_bytes, grid, threads, &queue, skip_seed, L, sizing3);
+    } else { sizing3[0] = sizing3[1] = sizing3[2] = 0; }
+    *n_events = L.n;
+    return BEAGLE_OK;
+}
+
 // host only: the body of k_compile's walk (walk_body.inc) on one program
 beagle_status beagle_debug_walk(const int32_t* tokens, int32_t len, const float* consts, int64_t n_consts, int32_t d,
                                 int32_t tmem_slots, int32_t k_rcp, int32_t k_un, int32_t un_row_bytes, uint32_t rcp_unsafe, int32_t f1,
