@@ -456,3 +456,51 @@ def test_walk_turns_down_exactly_what_is_not_its_own(oracle):
     X, y = _cases(rng, 8, d)
     taken = _check_walk(oracle, g, l, c, X, y, 1e-3, [(2, 1, 1)], run_machine=False)
     assert 0.15 * len(l) < taken[False] < taken[True] < 0.85 * len(l)
+
+
+def test_random_token_streams_agree_with_the_oracles_static_check(oracle):
+    """Breadth: random words and loosely plausible programs of every length class (what tests/fuzz_device_compiler_asan.py sends through
+    the sanitizer, a smaller dose): the general compiler's verdict (malformed or depth) is the oracle's on every one, the walk takes
+    exactly the well-formed ones made of its commands and emits the general compiler's records, never more records than tokens."""
+    rng = np.random.default_rng(20260)
+    d, n_consts = 6, 16
+    consts = rng.uniform(-3, 3, n_consts).astype(np.float32)
+    valid_ops = np.array([1, 2, 3, 4, 5, 6, 7, 8, 9, 10, 11] + list(range(0x10, 0x1F)), np.uint32)
+    progs = []
+    for k in range(2500):
+        L = int(rng.choice([1, 2, 3, 5, 8, 13, 40, 100, 255, 511, 512])) if rng.random() < 0.3 else int(rng.integers(1, 60))
+        if k % 5 == 0:                             # random words (an opcode byte in range now and then)
+            tok = rng.integers(0, 2**32, L, dtype=np.uint64).astype(np.uint32)
+            tok = np.where(rng.random(L) < 0.5, (tok & 0xFFFFFF00) | rng.choice(valid_ops, L), tok).astype(np.uint32)
+        else:                                      # plausible: stack-aware choice of commands, stray arguments and opcodes
+            tok = np.empty(L, np.uint32)
+            depth = 0
+            for t in range(L):
+                if depth < 2 or rng.random() < 0.45:
+                    op = 1 if rng.random() < 0.3 else 2
+                    arg = int(rng.integers(0, (n_consts if op == 1 else d) + (1 if rng.random() < 0.02 else 0)))
+                    depth += 1
+                else:
+                    op = int(rng.choice(valid_ops))
+                    arg = 0 if rng.random() < 0.98 else int(rng.integers(0, 40))
+                    depth += {3: -1, 4: -1, 5: -1, 6: -1, 0x13: -1, 0x12: -1, 0x10: 1, 0x1E: 1}.get(op, 0)
+                tok[t] = (arg << 8) | op
+        progs.append(tok.view(np.int32))
+    g, l, c = pack(progs, consts)
+    X = rng.uniform(-2, 2, (1, d)).astype(np.float32)
+    orc = oracle.evaluate(g, l, c, X, np.zeros(1, np.float32), 0.0)
+    n_ok = n_taken = 0
+    for p, tok in enumerate(progs):
+        ops = set((tok.view(np.uint32) & 0xFF).tolist())
+        wellformed = not (orc["flags"][p] & oracle.FLAG_MALFORMED)
+        gdepth, gslow, grec = api.beagle_debug_compile(tok, c, d, 2, 3, 2, 2048, 0b101)
+        assert gdepth == orc["depth"][p] and (gdepth == 0) == (not wellformed), (p, gdepth, int(orc["depth"][p]))
+        assert len(grec) <= len(tok)
+        n_ok += wellformed
+        for f1 in (False, True):
+            taken, depth, used, rec = api.beagle_debug_walk(tok, c, d, 2, 3, 2, 2048, 0b101, f1=f1)
+            assert taken == (wellformed and ops <= (HOT | F1 if f1 else HOT)), (p, f1)
+            if taken:
+                n_taken += 1
+                assert depth == gdepth and np.array_equal(rec, grec), (p, f1)
+    assert 0.2 * len(progs) < n_ok < 0.9 * len(progs) and n_taken > 200
