@@ -286,6 +286,19 @@ beagle_status beagle_debug_compile(const int32_t* tokens, int32_t len, const flo
                                    int32_t tmem_slots, int32_t k_rcp, int32_t k_un, int32_t un_row_bytes, uint32_t rcp_unsafe,
                                    uint32_t* records, int32_t* n_records, int32_t* depth, int32_t* slow);
 
+/* beagle_debug_prepass — test only, HOST only, needs no device: the scheduling pre-pass (k_len_pass1, k_len_pass2, k_scatter: offsets, the
+ * length histogram and its scans, the counting sort by length, the start records, the transpose of the cases; csrc/prepass_body.inc, the
+ * source the three kernels are compiled from) run on HOST memory by a small SIMT emulator (one OS thread per CUDA thread of a block,
+ * csrc/simt_host.inc), with the launch shapes of the real call. lengths: P entries (1 <= P <= 2^22); X, y as beagle_eval but HOST; split:
+ * the layout flag of a call split by passes. Outputs (HOST): off[P] (exclusive prefix sum of the in-range lengths), sched4[4 P] (the start
+ * record of each sorted position: individual, token offset (low 32 bits), record base (low 32 bits), length | high bits; positions past
+ * n_sorted are not written), fitness[P] and depth[P] (written for out-of-range lengths only: quiet NaN and 0), xt[(d + 1) * npad] (the
+ * cases variable-major, zero-padded to a multiple of 512, y as row d), hdr6 = { T, micro-op entries reserved, n_sorted, max_len, mask of
+ * variables with a protected case, 0 (-1: the length histogram was not left zeroed for the next call) }, binstart[513], binubase[513]. */
+beagle_status beagle_debug_prepass(const int32_t* lengths, int64_t P, const float* X, const float* y, int32_t N, int32_t d, int32_t split,
+                                   int64_t* off, int32_t* sched4, float* fitness, int32_t* depth, float* xt, int64_t* hdr6,
+                                   int32_t* binstart, int64_t* binubase);
+
 /* beagle_debug_queue — test only, HOST only, needs no device: the scheduling loop of ONE warp of the interpreter kernel (csrc/queue_body.inc,
  * the source both k_eval and this call are compiled from) over a given queue. meta4: HOST, `total` entries of four ints as k_compile leaves
  * them in evaluation order (x = individual, y = record block in 16-byte units, z = records to copy, 0 = nothing to run, w = length);

@@ -45,6 +45,7 @@ _SIGNATURES = {
     "beagle_debug_chunk_plan": (_i32, [_vp, _i64, _i64, _vp, _i64, ctypes.POINTER(_i64), ctypes.POINTER(_i32), ctypes.POINTER(_i64)]),
     "beagle_debug_compile": (_i32, [_vp, _i32, _vp, _i64, _i32, _i32, _i32, _i32, _i32, ctypes.c_uint32, _vp,
                                     ctypes.POINTER(_i32), ctypes.POINTER(_i32), ctypes.POINTER(_i32)]),
+    "beagle_debug_prepass": (_i32, [_vp, _i64, _vp, _vp, _i32, _i32, _i32, _vp, _vp, _vp, _vp, _vp, _vp, _vp, _vp]),
     "beagle_debug_queue": (_i32, [_vp, _i32, _i32, _i32, _i32, _i32, _i32, ctypes.c_uint32, ctypes.c_uint32, _vp, _i32,
                                   ctypes.POINTER(_i32), ctypes.POINTER(_i32)]),
     "beagle_debug_walk": (_i32, [_vp, _i32, _vp, _i64, _i32, _i32, _i32, _i32, _i32, ctypes.c_uint32, _i32, _vp,
@@ -175,6 +176,22 @@ def beagle_debug_compile(tokens, consts, d, tmem_slots, k_rcp, k_un, un_row_byte
                                       int(tmem_slots), int(k_rcp), int(k_un), int(un_row_bytes), int(rcp_unsafe), _ptr(rec),
                                       ctypes.byref(n), ctypes.byref(depth), ctypes.byref(slow)), "beagle_debug_compile")
     return depth.value, bool(slow.value), rec[: n.value]
+
+
+def beagle_debug_prepass(lengths, X, y, split=False):
+    """The scheduling pre-pass on the host (SIMT emulator over the kernels' own source); numpy in, dict of numpy out."""
+    import numpy as np
+    lengths = np.ascontiguousarray(lengths, np.int32)
+    X = np.ascontiguousarray(X, np.float32); y = np.ascontiguousarray(y, np.float32)
+    P, (N, d) = len(lengths), X.shape
+    npad = (N + 511) // 512 * 512
+    out = dict(off=np.full(P, -1, np.int64), sched=np.full((P, 4), -1, np.int32), fitness=np.full(P, -12345.0, np.float32),
+               depth=np.full(P, -7, np.int32), xt=np.full((d + 1, npad), -3.0, np.float32), hdr=np.zeros(6, np.int64),
+               binstart=np.zeros(513, np.int32), binubase=np.zeros(513, np.int64))
+    _check(lib().beagle_debug_prepass(_ptr(lengths), P, _ptr(X), _ptr(y), N, d, int(bool(split)), _ptr(out["off"]), _ptr(out["sched"]),
+                                      _ptr(out["fitness"]), _ptr(out["depth"]), _ptr(out["xt"]), _ptr(out["hdr"]),
+                                      _ptr(out["binstart"]), _ptr(out["binubase"])), "beagle_debug_prepass")
+    return out
 
 
 def beagle_debug_queue(meta4, max_len, ring_bytes, grid, threads, grouped, skip_seed=0, queue_start=0):

@@ -13,6 +13,12 @@
 #include <stdint.h>
 #include <stdio.h>
 #include <string.h>
+#include <pthread.h>          // simt_host.inc (test only)
+#include <map>
+#include <mutex>
+#include <string>
+#include <thread>
+#include <vector>
 
 #include "../../include/beagle.h"
 #include "ops.cuh"
@@ -118,37 +124,34 @@ __device__ __forceinline__ void tma_bulk_g2s(void* dst, const void* src, uint32_
                  ::"r"(smem_u32(dst)), "l"(src), "r"(bytes), "r"(smem_u32(bar)) : "memory");
 }
 
-__device__ __forceinline__ int clamp_len(int l) { return (l >= 1 && l <= BEAGLE_MAX_LEN) ? l : 0; }
+__host__ __device__ __forceinline__ int clamp_len(int l) { return (l >= 1 && l <= BEAGLE_MAX_LEN) ? l : 0; }
 __device__ __host__ __forceinline__ int uop_stride(int len) { return (len + 3 + 1) & ~1; }   // records: n <= len micro-ops + 3; even
 
+// The bodies of the three pre-pass kernels are prepass_body.inc; these are the device's meanings of its macros.
+#define PB_SHARED(type, name, count) __shared__ type name[count];
+#define PB_SHARED1(type, name) __shared__ type name;
+#define PB_TID threadIdx.x
+#define PB_BID blockIdx.x
+#define PB_BDIM blockDim.x
+#define PB_SYNC __syncthreads();
+#define PB_SHFL_XOR(v, m) __shfl_xor_sync(0xffffffffu, v, m)
+#define PB_SHFL_UP(v, s) __shfl_up_sync(0xffffffffu, v, s)
+#define PB_ATOMIC_ADD(p, v) atomicAdd(p, v)
+#define PB_ATOMIC_MAX(p, v) atomicMax(p, v)
+#define PB_ATOMIC_OR(p, v) atomicOr(p, v)
+#define PB_OP_SIN(v) op_sin(v)
+#define PB_OP_COS(v) op_cos(v)
+#define PB_OP_LOG(v) op_log(v)
+#define PB_OP_SQRT(v) op_sqrt(v)
+#define PB_OP_EXP(v) op_exp(v)
+#define PB_U2F(u) __uint_as_float(u)
 // ---- a2: block sums of the lengths + histogram of the lengths -----------------------------------------
 __global__ void __launch_bounds__(kScanThreads) k_len_pass1(const int32_t* __restrict__ lengths, long long P,
                                                             long long* __restrict__ bsum, int* __restrict__ bins)
 {
-    __shared__ int wsum[kScanThreads / 32];
-    __shared__ int hist[kNumBins];
-    for (int i = threadIdx.x; i < kNumBins; i += kScanThreads) hist[i] = 0;
-    __syncthreads();
-    int v = 0;
-#pragma unroll
-    for (int it = 0; it < kScanItems; ++it) {
-        const long long p = (long long)blockIdx.x * kScanBlock + it * kScanThreads + threadIdx.x;
-        const int len = (p < P) ? clamp_len(lengths[p]) : 0;
-        if (len > 0) atomicAdd(&hist[BEAGLE_MAX_LEN - len], 1);
-        v += len;
-    }
-#pragma unroll
-    for (int m = 16; m >= 1; m >>= 1) v += __shfl_xor_sync(0xffffffffu, v, m);
-    if ((threadIdx.x & 31) == 0) wsum[threadIdx.x >> 5] = v;
-    __syncthreads();
-    if (threadIdx.x == 0) {
-        int t = 0;
-#pragma unroll
-        for (int w = 0; w < kScanThreads / 32; ++w) t += wsum[w];
-        bsum[blockIdx.x] = t;
-    }
-    for (int i = threadIdx.x; i < kNumBins; i += kScanThreads)
-        if (hist[i]) atomicAdd(&bins[i], hist[i]);
+#define PB_SECTION 1
+#include "prepass_body.inc"
+#undef PB_SECTION
 }
 
 // one block: exclusive scan of the block sums in place; exclusive scan of the bins -> binstart[] (positions
@@ -160,94 +163,9 @@ __global__ void __launch_bounds__(1024) k_len_pass2(long long* __restrict__ bsum
                                                     const float* __restrict__ X, const float* __restrict__ y,
                                                     int n, int d, int npad, float* __restrict__ xt, float* __restrict__ ung, int split)
 {
-    __shared__ long long wtot[32];
-    __shared__ long long carry_s;
-    __shared__ long long wtot2[32];
-    __shared__ long long carry2_s;
-    __shared__ int maxlen_s;
-    __shared__ unsigned int unsafe_s;
-    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    if (threadIdx.x == 0) { carry_s = 0; carry2_s = 0; maxlen_s = 0; unsafe_s = 0; }
-    __syncthreads();
-    // which variables ever trigger the division protection (D2): their reciprocal row may not be used
-    for (int e = threadIdx.x; e < n * d; e += blockDim.x)
-        if (fabsf(X[e]) < kEps) atomicOr(&unsafe_s, 1u << (e % d));
-    __syncthreads();
-    for (int base = 0; base < nblocks; base += 1024) {
-        const int i = base + threadIdx.x;
-        long long v = (i < nblocks) ? bsum[i] : 0, inc = v;
-#pragma unroll
-        for (int s = 1; s < 32; s <<= 1) { long long o = __shfl_up_sync(0xffffffffu, inc, s); if (lane >= s) inc += o; }
-        if (lane == 31) wtot[warp] = inc;
-        __syncthreads();
-        if (warp == 0) {
-            long long w = wtot[lane], winc = w;
-#pragma unroll
-            for (int s = 1; s < 32; s <<= 1) { long long o = __shfl_up_sync(0xffffffffu, winc, s); if (lane >= s) winc += o; }
-            wtot[lane] = winc - w;
-        }
-        __syncthreads();
-        const long long carry = carry_s;
-        if (i < nblocks) bsum[i] = carry + wtot[warp] + inc - v;
-        __syncthreads();
-        if (threadIdx.x == 1023) carry_s = carry + wtot[31] + inc;
-        __syncthreads();
-    }
-    // bins: one element per thread (kNumBins = 513 <= 1024)
-    {
-        const int i = threadIdx.x;
-        const int cnt = (i < kNumBins) ? bins[i] : 0;
-        const int len = BEAGLE_MAX_LEN - i;
-        const long long v = cnt, u = (long long)cnt * uop_stride(len);
-        long long inc = v, uinc = u;
-        if (cnt > 0) atomicMax(&maxlen_s, len);
-#pragma unroll
-        for (int s = 1; s < 32; s <<= 1) {
-            const long long o = __shfl_up_sync(0xffffffffu, inc, s), o2 = __shfl_up_sync(0xffffffffu, uinc, s);
-            if (lane >= s) { inc += o; uinc += o2; }
-        }
-        if (lane == 31) { wtot[warp] = inc; wtot2[warp] = uinc; }
-        __syncthreads();
-        if (warp == 0) {
-            const long long w = wtot[lane], w2 = wtot2[lane];
-            long long winc = w, winc2 = w2;
-#pragma unroll
-            for (int s = 1; s < 32; s <<= 1) {
-                const long long o = __shfl_up_sync(0xffffffffu, winc, s), o2 = __shfl_up_sync(0xffffffffu, winc2, s);
-                if (lane >= s) { winc += o; winc2 += o2; }
-            }
-            wtot[lane] = winc - w; wtot2[lane] = winc2 - w2;       // exclusive warp bases
-            if (lane == 31) { carry2_s = winc; hdr->uop_entries = winc2; }
-        }
-        __syncthreads();
-        if (i < kNumBins) {
-            binstart[i] = (int)(wtot[warp] + inc - v);
-            binubase[i] = wtot2[warp] + uinc - u;
-            bins[i] = 0; cursor[i] = 0;            // ready for the next call
-        }
-    }
-    __syncthreads();
-    if (threadIdx.x == 0) {
-        hdr->T = carry_s;
-        hdr->n_sorted = (int)carry2_s;
-        hdr->max_len = maxlen_s;
-        hdr->n_slow = 0; hdr->n_malformed = 0; hdr->n_general = 0; hdr->n_f1 = 0;
-        hdr->queue = 0; hdr->queue2 = 0;
-        hdr->rcp_unsafe = unsafe_s;
-    }
-    // transpose: xt[j][i] = X[i][j] (j < d), xt[d][i] = y[i]; cases i >= n are zero
-    for (int e = threadIdx.x; e < (d + 1) * npad; e += blockDim.x) {
-        const int j = e / npad, i = e - j * npad;
-        float v = 0.f;
-        if (i < n) v = (j < d) ? X[(size_t)i * d + j] : (y ? y[i] : 0.f);
-        xt[e] = v;
-        if (j < d) {                               // the unary rows f(X[j]) (uop.cuh H_LS / H_LG), the handlers' own functions
-            // layout: ung[(f * d + j) * npad + i]; in a split call one block of 5 d rows of 512 cases per pass
-            const size_t fs = split ? (size_t)d * kCasesPerPass : (size_t)d * npad;
-            const size_t b = split ? (size_t)(i / kCasesPerPass) * 5 * fs + (size_t)j * kCasesPerPass + (i % kCasesPerPass) : (size_t)e;
-            ung[b] = op_sin(v); ung[fs + b] = op_cos(v); ung[2 * fs + b] = op_log(v); ung[3 * fs + b] = op_sqrt(v); ung[4 * fs + b] = op_exp(v);
-        }
-    }
+#define PB_SECTION 2
+#include "prepass_body.inc"
+#undef PB_SECTION
 }
 
 // ---- a3: offsets and the counting sort by length ---------------------------------------------------------
@@ -258,61 +176,9 @@ __global__ void __launch_bounds__(kScanThreads) k_scatter(
     float* __restrict__ outputs, int n_cases, const long long* __restrict__ binubase,
     int4* __restrict__ sched)
 {
-    __shared__ int wsum[kScanThreads / 32];
-    __shared__ int cnt[kNumBins];
-    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    for (int i = threadIdx.x; i < kNumBins; i += kScanThreads) cnt[i] = 0;
-    __syncthreads();
-    int lens[kScanItems], rs[kScanItems], offs[kScanItems];
-    int carry = 0;                                   // tokens of the block before the current chunk of 256 programs
-#pragma unroll
-    for (int it = 0; it < kScanItems; ++it) {
-        const long long p = (long long)blockIdx.x * kScanBlock + it * kScanThreads + threadIdx.x;
-        const int len = (p < P) ? clamp_len(lengths[p]) : 0;
-        int inc = len;
-#pragma unroll
-        for (int s = 1; s < 32; s <<= 1) { int o = __shfl_up_sync(0xffffffffu, inc, s); if (lane >= s) inc += o; }
-        if (lane == 31) wsum[warp] = inc;
-        __syncthreads();
-        int wbase = 0, tot = 0;
-#pragma unroll
-        for (int w = 0; w < kScanThreads / 32; ++w) { wbase += (w < warp) ? wsum[w] : 0; tot += wsum[w]; }
-        __syncthreads();
-        lens[it] = len; offs[it] = carry + wbase + inc - len; rs[it] = 0;
-        carry += tot;
-        if (p < P) {
-            if (len > 0) rs[it] = atomicAdd(&cnt[BEAGLE_MAX_LEN - len], 1);
-            else {                                   // length out of range: malformed (D3)
-                depth_out[p] = 0;
-                if (fitness) fitness[p] = __uint_as_float(0x7FC00000u);
-                if (outputs) for (int i = 0; i < n_cases; ++i) outputs[(size_t)p * n_cases + i] = __uint_as_float(0x7FC00000u);
-            }
-        }
-    }
-    __syncthreads();
-    // one global reservation per (block, non-empty bin); cnt[] becomes the block's base in that bin
-    for (int i = threadIdx.x; i < kNumBins; i += kScanThreads)
-        if (cnt[i]) cnt[i] = atomicAdd(&cursor[i], cnt[i]);
-    __syncthreads();
-    const long long b0 = bsum[blockIdx.x];
-#pragma unroll
-    for (int it = 0; it < kScanItems; ++it) {
-        const long long p = (long long)blockIdx.x * kScanBlock + it * kScanThreads + threadIdx.x;
-        if (p >= P) continue;
-        const int len = lens[it];
-        const long long o = b0 + offs[it];
-        off[p] = o;
-        if (len > 0) {
-            // everything the compiler's lane needs to start, at the individual's place in the sorted order
-            const int k = BEAGLE_MAX_LEN - len;
-            const int pos = binstart[k] + cnt[k] + rs[it];
-            // one 16-byte start record: x = p, y = token offset (low 32), z = record base (low 32),
-            // w = length (10 bits) | offset bits 39..32 << 10 | record base bits 39..32 << 18
-            const long long ub = binubase[k] + (long long)(cnt[k] + rs[it]) * uop_stride(len);
-            sched[pos] = make_int4((int)p, (int)(unsigned int)o, (int)(unsigned int)ub,
-                                   len | (int)((o >> 32) & 0xff) << 10 | (int)((ub >> 32) & 0xff) << 18);
-        }
-    }
+#define PB_SECTION 3
+#include "prepass_body.inc"
+#undef PB_SECTION
 }
 
 // debug only (beagle_debug_schedule): the sorted order as an index array; entries past the sorted ones are -1
@@ -785,6 +651,8 @@ static beagle_status run_colony(const int32_t* genomes, const int32_t* lengths, 
     return BEAGLE_OK;
 }
 
+#include "simt_host.inc"
+
 } // namespace beagle
 
 using namespace beagle;
@@ -1164,6 +1032,25 @@ beagle_status beagle_debug_std_reward(const float* f, const float* y, int64_t n,
     if (n < 0 || (n > 0 && (!f || !y || !out)) || !decode_fit(fit, &kind, &power) || kind != BEAGLE_FIT_STD) return BEAGLE_ERR_INVALID_ARG;
     const float pen = M / 11.f;                   // the kernels' __fdiv_rn(M, 11.f)
     for (int64_t i = 0; i < n; ++i) out[i] = std_reward(f[i], y[i], M, pen, power);
+    return BEAGLE_OK;
+}
+
+// host only: the pre-pass kernels k_len_pass1, k_len_pass2, k_scatter (prepass_body.inc) run by the SIMT emulator of simt_host.inc
+beagle_status beagle_debug_prepass(const int32_t* lengths, int64_t P, const float* X, const float* y, int32_t N, int32_t d, int32_t split,
+                                   int64_t* off, int32_t* sched4, float* fitness, int32_t* depth, float* xt, int64_t* hdr6,
+                                   int32_t* binstart, int64_t* binubase)
+{
+    if (P < 1 || P > (1 << 22) || !lengths || !X || !y || N < 1 || N > BEAGLE_MAX_N || d < 1 || d > BEAGLE_MAX_D
+        || !off || !sched4 || !fitness || !depth || !xt || !hdr6 || !binstart || !binubase)
+        return BEAGLE_ERR_INVALID_ARG;
+    const int npad = (N + kCasePad - 1) / kCasePad * kCasePad;
+    std::vector<float> ung((size_t)5 * d * npad, 0.f);
+    Header hdr = {};
+    static_assert(sizeof(long long) == sizeof(int64_t), "off and binubase are passed through as they are");
+    prepass_host(lengths, P, X, y, N, d, split ? 1 : 0, reinterpret_cast<long long*>(off), reinterpret_cast<int4*>(sched4), fitness, depth, xt,
+                 ung.data(), &hdr, binstart, reinterpret_cast<long long*>(binubase));
+    hdr6[0] = hdr.T; hdr6[1] = hdr.uop_entries; hdr6[2] = hdr.n_sorted; hdr6[3] = hdr.max_len; hdr6[4] = hdr.rcp_unsafe;
+    hdr6[5] = hdr.n_malformed;                     // 0, or -1 if the length histogram was not left zeroed for the next call
     return BEAGLE_OK;
 }
 
