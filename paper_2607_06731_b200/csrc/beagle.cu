@@ -9,6 +9,9 @@
 //   a5-a7  k_eval (eval_kernel.inc)    TMA-fed interpreter: fetch, interpret, reduce, tax, store
 //   a8  beagle_eval_chunked            double-buffered H2D on a copy stream
 // PyTorch is not involved: only the CUDA runtime. sm_100a only.
+// Test-only host builds of the device's integer logic (beagle_debug_prepass / _compile / _walk / _queue / _std_reward): the
+// bodies of the pre-pass kernels, of the compiler's walk and of the interpreter's scheduling loop live in prepass_body.inc, walk_body.inc
+// and queue_body.inc, included by the kernels with the device's macros and by host functions with plain C++ ones. No product path uses them.
 #include <cuda_runtime.h>
 #include <stdint.h>
 #include <stdio.h>
