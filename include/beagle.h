@@ -286,6 +286,12 @@ beagle_status beagle_debug_compile(const int32_t* tokens, int32_t len, const flo
                                    int32_t tmem_slots, int32_t k_rcp, int32_t k_un, int32_t un_row_bytes, uint32_t rcp_unsafe,
                                    uint32_t* records, int32_t* n_records, int32_t* depth, int32_t* slow);
 
+/* beagle_debug_rank — test only, HOST only, needs no device: k_rank (csrc/rank_body.inc, the source the kernel is compiled from) run on HOST
+ * memory by the SIMT emulator, `grid` blocks of 256 threads one after the other (beagle_rank launches up to 8 per SM). Arguments as
+ * beagle_rank with HOST pointers; sample_idx is checked here (each in [0, P)); hist_out is required. 1 <= P <= 2^22. */
+beagle_status beagle_debug_rank(const float* fitness, int64_t P, const int64_t* sample_idx, int32_t n_sample, int32_t maximise,
+                                int32_t grid, uint8_t* decile_out, int64_t* hist_out);
+
 /* beagle_debug_prepass — test only, HOST only, needs no device: the scheduling pre-pass (k_len_pass1, k_len_pass2, k_scatter: offsets, the
  * length histogram and its scans, the counting sort by length, the start records, the transpose of the cases; csrc/prepass_body.inc, the
  * source the three kernels are compiled from) run on HOST memory by a small SIMT emulator (one OS thread per CUDA thread of a block,

@@ -45,6 +45,7 @@ _SIGNATURES = {
     "beagle_debug_chunk_plan": (_i32, [_vp, _i64, _i64, _vp, _i64, ctypes.POINTER(_i64), ctypes.POINTER(_i32), ctypes.POINTER(_i64)]),
     "beagle_debug_compile": (_i32, [_vp, _i32, _vp, _i64, _i32, _i32, _i32, _i32, _i32, ctypes.c_uint32, _vp,
                                     ctypes.POINTER(_i32), ctypes.POINTER(_i32), ctypes.POINTER(_i32)]),
+    "beagle_debug_rank": (_i32, [_vp, _i64, _vp, _i32, _i32, _i32, _vp, _vp]),
     "beagle_debug_prepass": (_i32, [_vp, _i64, _vp, _vp, _i32, _i32, _i32, _vp, _vp, _vp, _vp, _vp, _vp, _vp, _vp]),
     "beagle_debug_queue": (_i32, [_vp, _i32, _i32, _i32, _i32, _i32, _i32, ctypes.c_uint32, ctypes.c_uint32, _vp, _i32,
                                   ctypes.POINTER(_i32), ctypes.POINTER(_i32)]),
@@ -176,6 +177,18 @@ def beagle_debug_compile(tokens, consts, d, tmem_slots, k_rcp, k_un, un_row_byte
                                       int(tmem_slots), int(k_rcp), int(k_un), int(un_row_bytes), int(rcp_unsafe), _ptr(rec),
                                       ctypes.byref(n), ctypes.byref(depth), ctypes.byref(slow)), "beagle_debug_compile")
     return depth.value, bool(slow.value), rec[: n.value]
+
+
+def beagle_debug_rank(fitness, sample_idx, maximise, grid=4):
+    """k_rank on the host (SIMT emulator over the kernel's own source): (decile uint8[P], hist int64[10]); numpy in, numpy out."""
+    import numpy as np
+    fitness = np.ascontiguousarray(fitness, np.float32)
+    sample_idx = np.ascontiguousarray(sample_idx, np.int64)
+    dec = np.full(len(fitness), 255, np.uint8)
+    hist = np.full(10, -1, np.int64)
+    _check(lib().beagle_debug_rank(_ptr(fitness), len(fitness), _ptr(sample_idx), len(sample_idx), int(bool(maximise)), int(grid),
+                                   _ptr(dec), _ptr(hist)), "beagle_debug_rank")
+    return dec, hist
 
 
 def beagle_debug_prepass(lengths, X, y, split=False):

@@ -1038,6 +1038,22 @@ beagle_status beagle_debug_std_reward(const float* f, const float* y, int64_t n,
     return BEAGLE_OK;
 }
 
+// host only: k_rank (rank_body.inc) run by the SIMT emulator, `grid` blocks one after the other
+beagle_status beagle_debug_rank(const float* fitness, int64_t P, const int64_t* sample_idx, int32_t n_sample, int32_t maximise,
+                                int32_t grid, uint8_t* decile_out, int64_t* hist_out)
+{
+    if (P < 1 || P > (1 << 22) || n_sample < 1 || n_sample > kRankMaxSample || grid < 1 || grid > 4096 || !fitness || !sample_idx
+        || !decile_out || !hist_out)
+        return BEAGLE_ERR_INVALID_ARG;
+    for (int i = 0; i < n_sample; ++i) if (sample_idx[i] < 0 || sample_idx[i] >= P) return BEAGLE_ERR_INVALID_ARG;
+    unsigned long long hist[10] = {};              // (beagle_rank zeroes the histogram before the launch)
+    for (int b = 0; b < grid; ++b)
+        simt::run_block(kRankThreads, b, [&](simt::Block& blk, int tid) {
+            h_rank(blk, tid, grid, fitness, P, reinterpret_cast<const long long*>(sample_idx), n_sample, maximise != 0, decile_out, hist); });
+    for (int i = 0; i < 10; ++i) hist_out[i] = (int64_t)hist[i];
+    return BEAGLE_OK;
+}
+
 // host only: the pre-pass kernels k_len_pass1, k_len_pass2, k_scatter (prepass_body.inc) run by the SIMT emulator of simt_host.inc
 beagle_status beagle_debug_prepass(const int32_t* lengths, int64_t P, const float* X, const float* y, int32_t N, int32_t d, int32_t split,
                                    int64_t* off, int32_t* sched4, float* fitness, int32_t* depth, float* xt, int64_t* hdr6,

@@ -95,3 +95,21 @@ def test_prepass_argument_errors():
     assert l.beagle_debug_prepass(None, 1, one.ctypes.data, one.ctypes.data, 1, 1, 0, *([one.ctypes.data] * 8)) == api.ERR_INVALID_ARG
     assert l.beagle_debug_prepass(one.ctypes.data, (1 << 22) + 1, one.ctypes.data, one.ctypes.data, 1, 1, 0, *([one.ctypes.data] * 8)) == api.ERR_INVALID_ARG
     assert l.beagle_debug_prepass(one.ctypes.data, 1, one.ctypes.data, one.ctypes.data, 1025, 1, 0, *([one.ctypes.data] * 8)) == api.ERR_INVALID_ARG
+
+
+# ---- k_rank the same way: the kernel's own source under the emulator, against oracle/ranking.py ------------------------
+@pytest.mark.parametrize("P,n_sample,grid,seed", [(1000, 100, 1, 1), (5000, 100, 3, 2), (37, 100, 2, 3), (5000, 7, 4, 4), (3000, 1024, 2, 5), (1, 1, 1, 6)])
+def test_rank_kernel_on_the_host_matches_the_ranking_oracle(P, n_sample, grid, seed):
+    from oracle import ranking as R
+    rng = np.random.default_rng(seed)
+    f = (rng.standard_normal(P) * 100).astype(np.float32)
+    f[rng.random(P) < 0.03] = np.nan                 # NaN is worse than every number (R24)
+    f[rng.random(P) < 0.03] = np.inf
+    if seed % 2:
+        f = np.round(f, 0)                           # many ties: equal fitnesses are not strictly worse
+    sample = rng.integers(0, P, n_sample)
+    for maximise in (False, True):
+        dec, hist = api.beagle_debug_rank(f, sample, maximise, grid)
+        want, whist, _ = R.rank_deciles(f, sample, maximise)
+        assert np.array_equal(dec, want) and np.array_equal(hist, whist)
+        assert hist.sum() == P
