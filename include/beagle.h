@@ -286,6 +286,13 @@ beagle_status beagle_debug_compile(const int32_t* tokens, int32_t len, const flo
                                    int32_t tmem_slots, int32_t k_rcp, int32_t k_un, int32_t un_row_bytes, uint32_t rcp_unsafe,
                                    uint32_t* records, int32_t* n_records, int32_t* depth, int32_t* slow);
 
+/* beagle_debug_corr — test only, HOST only, needs no device: the correlation fitness (BEAGLE_FIT_CORRELATION) of ONE individual from its
+ * per-case outputs f[0..N) and the targets y[0..N) (HOST), by the device's own reduction (csrc/fit_corr.cuh compiled for the host: IEEE
+ * single precision throughout, so the device's bits) on one warp of the SIMT emulator, in the kernels' layout of 16 cases per lane and
+ * pass. len, M, tax as in beagle_eval_fit. pre != 0: full passes with finite targets take the version with the target's side computed
+ * once (the interpreter kernel's way), else the general one (the blockwise kernel's way); the two give the same bits. */
+beagle_status beagle_debug_corr(const float* f, const float* y, int32_t N, int32_t len, float M, float tax, int32_t pre, float* fitness_out);
+
 /* beagle_debug_rank — test only, HOST only, needs no device: k_rank (csrc/rank_body.inc, the source the kernel is compiled from) run on HOST
  * memory by the SIMT emulator, `grid` blocks of 256 threads one after the other (beagle_rank launches up to 8 per SM). Arguments as
  * beagle_rank with HOST pointers; sample_idx is checked here (each in [0, P)); hist_out is required. 1 <= P <= 2^22. */

@@ -45,6 +45,7 @@ _SIGNATURES = {
     "beagle_debug_chunk_plan": (_i32, [_vp, _i64, _i64, _vp, _i64, ctypes.POINTER(_i64), ctypes.POINTER(_i32), ctypes.POINTER(_i64)]),
     "beagle_debug_compile": (_i32, [_vp, _i32, _vp, _i64, _i32, _i32, _i32, _i32, _i32, ctypes.c_uint32, _vp,
                                     ctypes.POINTER(_i32), ctypes.POINTER(_i32), ctypes.POINTER(_i32)]),
+    "beagle_debug_corr": (_i32, [_vp, _vp, _i32, _i32, _f32, _f32, _i32, ctypes.POINTER(_f32)]),
     "beagle_debug_rank": (_i32, [_vp, _i64, _vp, _i32, _i32, _i32, _vp, _vp]),
     "beagle_debug_prepass": (_i32, [_vp, _i64, _vp, _vp, _i32, _i32, _i32, _vp, _vp, _vp, _vp, _vp, _vp, _vp, _vp]),
     "beagle_debug_queue": (_i32, [_vp, _i32, _i32, _i32, _i32, _i32, _i32, ctypes.c_uint32, ctypes.c_uint32, _vp, _i32,
@@ -177,6 +178,16 @@ def beagle_debug_compile(tokens, consts, d, tmem_slots, k_rcp, k_un, un_row_byte
                                       int(tmem_slots), int(k_rcp), int(k_un), int(un_row_bytes), int(rcp_unsafe), _ptr(rec),
                                       ctypes.byref(n), ctypes.byref(depth), ctypes.byref(slow)), "beagle_debug_compile")
     return depth.value, bool(slow.value), rec[: n.value]
+
+
+def beagle_debug_corr(f, y, length, M, tax, pre=False):
+    """The correlation fitness of one individual from its per-case outputs, by the device's reduction on the host (emulated warp)."""
+    import numpy as np
+    f = np.ascontiguousarray(f, np.float32); y = np.ascontiguousarray(y, np.float32)
+    out = _f32(0.0)
+    _check(lib().beagle_debug_corr(_ptr(f), _ptr(y), len(f), int(length), float(M), float(tax), int(bool(pre)), ctypes.byref(out)),
+           "beagle_debug_corr")
+    return np.float32(out.value)
 
 
 def beagle_debug_rank(fitness, sample_idx, maximise, grid=4):

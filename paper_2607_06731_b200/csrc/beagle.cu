@@ -280,7 +280,7 @@ __global__ void __launch_bounds__(1024) k_eval_blockwise(
         __syncthreads();
         if (threadIdx.x < 32 && fitness && fit == BEAGLE_FIT_CORRELATION) {       // f2: fit_corr.cuh, the layout of k_eval
             const int lane = threadIdx.x;
-            CorrState cs = { 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0 };
+            CorrState cs = { 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0.f, 0 };
             for (int c0 = 0; c0 < n; c0 += kCasesPerPass) {
                 float fv[16], yv[16];
 #pragma unroll
@@ -1035,6 +1035,18 @@ beagle_status beagle_debug_std_reward(const float* f, const float* y, int64_t n,
     if (n < 0 || (n > 0 && (!f || !y || !out)) || !decode_fit(fit, &kind, &power) || kind != BEAGLE_FIT_STD) return BEAGLE_ERR_INVALID_ARG;
     const float pen = M / 11.f;                   // the kernels' __fdiv_rn(M, 11.f)
     for (int64_t i = 0; i < n; ++i) out[i] = std_reward(f[i], y[i], M, pen, power);
+    return BEAGLE_OK;
+}
+
+// host only: the correlation fitness of ONE individual from its per-case outputs, by the functions of fit_corr.cuh on an emulated warp
+beagle_status beagle_debug_corr(const float* f, const float* y, int32_t N, int32_t len, float M, float tax, int32_t pre, float* fitness_out)
+{
+    if (!f || !y || !fitness_out || N < 1 || N > BEAGLE_MAX_N || len < 1 || len > BEAGLE_MAX_LEN) return BEAGLE_ERR_INVALID_ARG;
+    alignas(16) float dys[BEAGLE_MAX_N] = {};
+    CorrYPass ypre[2] = {};
+    float out = 0.f;
+    simt::run_block(32, 0, [&](simt::Block& blk, int tid) { h_corr_lane(blk, tid, f, y, N, len, M, tax, pre, dys, ypre, &out); });
+    *fitness_out = out;
     return BEAGLE_OK;
 }
 
