@@ -241,7 +241,7 @@ def beagle_debug_walk(tokens, consts, d, tmem_slots, k_rcp, k_un, un_row_bytes, 
     rec = np.zeros((len(tokens) + 8, 2), np.uint32)
     n, depth, taken, used = _i32(0), _i32(0), _i32(0), _i32(0)
     _check(lib().beagle_debug_walk(_ptr(tokens), len(tokens), _ptr(consts) if len(consts) else None, len(consts), int(d),
-                                   int(tmem_slots), int(k_rcp), int(k_un), int(un_row_bytes), int(rcp_unsafe), int(bool(f1)), _ptr(rec),
+                                   int(tmem_slots), int(k_rcp), int(k_un), int(un_row_bytes), int(rcp_unsafe), int(f1), _ptr(rec),
                                    ctypes.byref(n), ctypes.byref(depth), ctypes.byref(taken), ctypes.byref(used)), "beagle_debug_walk")
     return bool(taken.value), depth.value, bool(used.value), rec[: n.value]
 
