@@ -327,7 +327,8 @@ beagle_status beagle_debug_queue(const int32_t* meta4, int32_t total, int32_t ma
 
 /* beagle_debug_walk — test only, HOST only, needs no device: the body of k_compile's table-driven walk (csrc/walk_body.inc, the source
  * both the kernel and this call are compiled from) on ONE program; f1 != 0: the instantiation that also takes DUP SWAP DEL SIGN SQUARE
- * CUBE (f1 == 2: with the warp-wide vote that guards those commands passed at every token, as for a lane whose neighbours meet them). Arguments as beagle_debug_compile. *taken = 1 if the walk compiled the program, 0 if it turned it down (anything that is not
+ * CUBE (f1 == 2: with the warp-wide vote that guards those commands passed at every token, as for a lane whose neighbours meet them; bits 17:8 of f1: the
+ * walk goes on for that many tokens past the program's end, as for a lane beside a longer program of its warp). Arguments as beagle_debug_compile. *taken = 1 if the walk compiled the program, 0 if it turned it down (anything that is not
  * a well-formed program of its commands: k_compile_general looks at those); for taken programs *depth, records and *n_records as
  * beagle_debug_compile, *used_f1 = 1 if one of the six extra commands occurred. Same difference from the device (1 / c in IEEE). */
 beagle_status beagle_debug_walk(const int32_t* tokens, int32_t len, const float* consts, int64_t n_consts, int32_t d,

@@ -1120,7 +1120,8 @@ beagle_status beagle_debug_walk(const int32_t* tokens, int32_t len, const float*
     q.consts = consts; q.n_consts = n_consts; q.d = d; q.tmem_slots = tmem_slots; q.k_rcp = k_rcp; q.k_un = k_un; q.un_row_bytes = un_row_bytes;
     q.hdr = &hdr; q.uops = uops; q.ucap = BEAGLE_MAX_LEN + 8; q.meta = meta; q.depth = dep; q.slow_list = slow_list; q.gen_list = gen_list;
     q.emit = 1;
-    if (f1) walk_host<true>(q, len, f1 == 2); else walk_host<false>(q, len, false);
+    const int mode = f1 & 0xff, longer = (f1 >> 8) & 0x3ff;      // f1 bits 17:8: a neighbouring lane's program is that much longer
+    if (mode) walk_host<true>(q, len, mode == 2, longer); else walk_host<false>(q, len, false, longer);
     *taken = hdr.n_general == 0 ? 1 : 0;
     *depth = *taken ? dep[0] : 0;
     *used_f1 = hdr.n_f1;

@@ -378,15 +378,16 @@ def _check_walk(oracle, genomes, lengths, consts, X, y, tax, plans, run_machine=
             ops = set((tok.view(np.uint32) & 0xFF).tolist())
             wellformed = not (orc["flags"][p] & oracle.FLAG_MALFORMED)
             gdepth, gslow, grec = api.beagle_debug_compile(tok, consts, d, S_T, k_rcp, k_un, 2048, unsafe)
-            for f1 in (0, 1, 2):                   # 2: the stack commands' vote passed at every token (neighbouring lanes)
+            # 2: the stack commands' vote passed at every token (neighbouring lanes); + (k << 8): a neighbouring lane's program is k longer
+            for f1 in (0, 1, 2, 1 | 3 << 8, 0 | 17 << 8, 2 | 400 << 8):
                 taken, depth, used, rec = api.beagle_debug_walk(tok, consts, d, S_T, k_rcp, k_un, 2048, unsafe, f1=f1)
-                mine = ops <= (HOT | F1 if f1 else HOT)
+                mine = ops <= (HOT | F1 if f1 & 0xff else HOT)
                 assert taken == (wellformed and mine), (p, f1, taken, wellformed, sorted(ops))
                 if not taken:
                     continue
                 taken_n[bool(f1)] += f1 < 2
                 assert depth == orc["depth"][p] and not gslow, (p, f1, depth, int(orc["depth"][p]))
-                assert used == (bool(f1) and bool(ops & F1)), (p, f1, used)
+                assert used == (bool(f1 & 0xff) and bool(ops & F1)), (p, f1, used)
                 assert np.array_equal(rec, grec), (p, f1, rec.tolist(), grec.tolist())
             if run_machine and wellformed and ops <= HOT | F1:
                 _, _, _, rec = api.beagle_debug_walk(tok, consts, d, S_T, k_rcp, k_un, 2048, unsafe, f1=True)
