@@ -302,7 +302,7 @@ beagle_status beagle_debug_rank(const float* fitness, int64_t P, const int64_t* 
 /* beagle_debug_prepass — test only, HOST only, needs no device: the scheduling pre-pass (k_len_pass1, k_len_pass2, k_scatter: offsets, the
  * length histogram and its scans, the counting sort by length, the start records, the transpose of the cases; csrc/prepass_body.inc, the
  * source the three kernels are compiled from) run on HOST memory by a small SIMT emulator (one OS thread per CUDA thread of a block,
- * csrc/simt_host.inc), with the launch shapes of the real call. lengths: P entries (1 <= P <= 2^22); X, y as beagle_eval but HOST; split:
+ * csrc/simt_host.inc), with the launch shapes of the real call. lengths: P entries (1 <= P <= 2^24); X, y as beagle_eval but HOST; split:
  * the layout flag of a call split by passes. Outputs (HOST): off[P] (exclusive prefix sum of the in-range lengths), sched4[4 P] (the start
  * record of each sorted position: individual, token offset (low 32 bits), record base (low 32 bits), length | high bits; positions past
  * n_sorted are not written), fitness[P] and depth[P] (written for out-of-range lengths only: quiet NaN and 0), xt[(d + 1) * npad] (the

@@ -1071,7 +1071,7 @@ beagle_status beagle_debug_prepass(const int32_t* lengths, int64_t P, const floa
                                    int64_t* off, int32_t* sched4, float* fitness, int32_t* depth, float* xt, int64_t* hdr6,
                                    int32_t* binstart, int64_t* binubase)
 {
-    if (P < 1 || P > (1 << 22) || !lengths || !X || !y || N < 1 || N > BEAGLE_MAX_N || d < 1 || d > BEAGLE_MAX_D
+    if (P < 1 || P > (1 << 24) || !lengths || !X || !y || N < 1 || N > BEAGLE_MAX_N || d < 1 || d > BEAGLE_MAX_D
         || !off || !sched4 || !fitness || !depth || !xt || !hdr6 || !binstart || !binubase)
         return BEAGLE_ERR_INVALID_ARG;
     const int npad = (N + kCasePad - 1) / kCasePad * kCasePad;

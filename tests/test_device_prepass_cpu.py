@@ -93,7 +93,7 @@ def test_prepass_argument_errors():
     one = np.zeros(1, np.int32)
     assert l.beagle_debug_prepass(one.ctypes.data, 0, one.ctypes.data, one.ctypes.data, 1, 1, 0, *([one.ctypes.data] * 8)) == api.ERR_INVALID_ARG
     assert l.beagle_debug_prepass(None, 1, one.ctypes.data, one.ctypes.data, 1, 1, 0, *([one.ctypes.data] * 8)) == api.ERR_INVALID_ARG
-    assert l.beagle_debug_prepass(one.ctypes.data, (1 << 22) + 1, one.ctypes.data, one.ctypes.data, 1, 1, 0, *([one.ctypes.data] * 8)) == api.ERR_INVALID_ARG
+    assert l.beagle_debug_prepass(one.ctypes.data, (1 << 24) + 1, one.ctypes.data, one.ctypes.data, 1, 1, 0, *([one.ctypes.data] * 8)) == api.ERR_INVALID_ARG
     assert l.beagle_debug_prepass(one.ctypes.data, 1, one.ctypes.data, one.ctypes.data, 1025, 1, 0, *([one.ctypes.data] * 8)) == api.ERR_INVALID_ARG
 
 
