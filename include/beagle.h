@@ -286,6 +286,7 @@ beagle_status beagle_debug_compile(const int32_t* tokens, int32_t len, const flo
                                    int32_t tmem_slots, int32_t k_rcp, int32_t k_un, int32_t un_row_bytes, uint32_t rcp_unsafe,
                                    uint32_t* records, int32_t* n_records, int32_t* depth, int32_t* slow);
 
+/* (The three calls below run on the SIMT emulator, which needs up to 1024 OS threads at a time: BEAGLE_ERR_UNSUPPORTED if the host refuses them.) */
 /* beagle_debug_corr — test only, HOST only, needs no device: the correlation fitness (BEAGLE_FIT_CORRELATION) of ONE individual from its
  * per-case outputs f[0..N) and the targets y[0..N) (HOST), by the device's own reduction (csrc/fit_corr.cuh compiled for the host: IEEE
  * single precision throughout, so the device's bits) on one warp of the SIMT emulator, in the kernels' layout of 16 cases per lane and

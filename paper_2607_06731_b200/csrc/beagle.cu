@@ -18,7 +18,9 @@
 #include <string.h>
 #include <pthread.h>          // simt_host.inc (test only)
 #include <map>
+#include <atomic>
 #include <mutex>
+#include <system_error>
 #include <string>
 #include <thread>
 #include <vector>
@@ -1045,7 +1047,8 @@ beagle_status beagle_debug_corr(const float* f, const float* y, int32_t N, int32
     alignas(16) float dys[BEAGLE_MAX_N] = {};
     CorrYPass ypre[2] = {};
     float out = 0.f;
-    simt::run_block(32, 0, [&](simt::Block& blk, int tid) { h_corr_lane(blk, tid, f, y, N, len, M, tax, pre, dys, ypre, &out); });
+    if (!simt::run_block(32, 0, [&](simt::Block& blk, int tid) { h_corr_lane(blk, tid, f, y, N, len, M, tax, pre, dys, ypre, &out); }))
+        return BEAGLE_ERR_UNSUPPORTED;
     *fitness_out = out;
     return BEAGLE_OK;
 }
@@ -1060,8 +1063,9 @@ beagle_status beagle_debug_rank(const float* fitness, int64_t P, const int64_t* 
     for (int i = 0; i < n_sample; ++i) if (sample_idx[i] < 0 || sample_idx[i] >= P) return BEAGLE_ERR_INVALID_ARG;
     unsigned long long hist[10] = {};              // (beagle_rank zeroes the histogram before the launch)
     for (int b = 0; b < grid; ++b)
-        simt::run_block(kRankThreads, b, [&](simt::Block& blk, int tid) {
-            h_rank(blk, tid, grid, fitness, P, reinterpret_cast<const long long*>(sample_idx), n_sample, maximise != 0, decile_out, hist); });
+        if (!simt::run_block(kRankThreads, b, [&](simt::Block& blk, int tid) {
+                h_rank(blk, tid, grid, fitness, P, reinterpret_cast<const long long*>(sample_idx), n_sample, maximise != 0, decile_out, hist); }))
+            return BEAGLE_ERR_UNSUPPORTED;
     for (int i = 0; i < 10; ++i) hist_out[i] = (int64_t)hist[i];
     return BEAGLE_OK;
 }
@@ -1078,8 +1082,9 @@ beagle_status beagle_debug_prepass(const int32_t* lengths, int64_t P, const floa
     std::vector<float> ung((size_t)5 * d * npad, 0.f);
     Header hdr = {};
     static_assert(sizeof(long long) == sizeof(int64_t), "off and binubase are passed through as they are");
-    prepass_host(lengths, P, X, y, N, d, split ? 1 : 0, reinterpret_cast<long long*>(off), reinterpret_cast<int4*>(sched4), fitness, depth, xt,
-                 ung.data(), &hdr, binstart, reinterpret_cast<long long*>(binubase));
+    if (!prepass_host(lengths, P, X, y, N, d, split ? 1 : 0, reinterpret_cast<long long*>(off), reinterpret_cast<int4*>(sched4), fitness, depth, xt,
+                      ung.data(), &hdr, binstart, reinterpret_cast<long long*>(binubase)))
+        return BEAGLE_ERR_UNSUPPORTED;             // the host gave the emulator no 1024 threads
     hdr6[0] = hdr.T; hdr6[1] = hdr.uop_entries; hdr6[2] = hdr.n_sorted; hdr6[3] = hdr.max_len; hdr6[4] = hdr.rcp_unsafe;
     hdr6[5] = hdr.n_malformed;                     // 0, or -1 if the length histogram was not left zeroed for the next call
     return BEAGLE_OK;
