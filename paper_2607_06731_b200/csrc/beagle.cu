@@ -1047,8 +1047,10 @@ beagle_status beagle_debug_corr(const float* f, const float* y, int32_t N, int32
     alignas(16) float dys[BEAGLE_MAX_N] = {};
     CorrYPass ypre[2] = {};
     float out = 0.f;
-    if (!simt::run_block(32, 0, [&](simt::Block& blk, int tid) { h_corr_lane(blk, tid, f, y, N, len, M, tax, pre, dys, ypre, &out); }))
-        return BEAGLE_ERR_UNSUPPORTED;
+    try {
+        if (!simt::run_block(32, 0, [&](simt::Block& blk, int tid) { h_corr_lane(blk, tid, f, y, N, len, M, tax, pre, dys, ypre, &out); }))
+            return BEAGLE_ERR_UNSUPPORTED;
+    } catch (...) { return BEAGLE_ERR_NOMEM; }
     *fitness_out = out;
     return BEAGLE_OK;
 }
@@ -1062,10 +1064,12 @@ beagle_status beagle_debug_rank(const float* fitness, int64_t P, const int64_t* 
         return BEAGLE_ERR_INVALID_ARG;
     for (int i = 0; i < n_sample; ++i) if (sample_idx[i] < 0 || sample_idx[i] >= P) return BEAGLE_ERR_INVALID_ARG;
     unsigned long long hist[10] = {};              // (beagle_rank zeroes the histogram before the launch)
+    try {
     for (int b = 0; b < grid; ++b)
         if (!simt::run_block(kRankThreads, b, [&](simt::Block& blk, int tid) {
                 h_rank(blk, tid, grid, fitness, P, reinterpret_cast<const long long*>(sample_idx), n_sample, maximise != 0, decile_out, hist); }))
             return BEAGLE_ERR_UNSUPPORTED;
+    } catch (...) { return BEAGLE_ERR_NOMEM; }
     for (int i = 0; i < 10; ++i) hist_out[i] = (int64_t)hist[i];
     return BEAGLE_OK;
 }
@@ -1078,6 +1082,7 @@ beagle_status beagle_debug_prepass(const int32_t* lengths, int64_t P, const floa
     if (P < 1 || P > (1 << 24) || !lengths || !X || !y || N < 1 || N > BEAGLE_MAX_N || d < 1 || d > BEAGLE_MAX_D
         || !off || !sched4 || !fitness || !depth || !xt || !hdr6 || !binstart || !binubase)
         return BEAGLE_ERR_INVALID_ARG;
+    try {                                          // (host containers inside: no exception may cross the C boundary)
     const int npad = (N + kCasePad - 1) / kCasePad * kCasePad;
     std::vector<float> ung((size_t)5 * d * npad, 0.f);
     Header hdr = {};
@@ -1088,6 +1093,7 @@ beagle_status beagle_debug_prepass(const int32_t* lengths, int64_t P, const floa
     hdr6[0] = hdr.T; hdr6[1] = hdr.uop_entries; hdr6[2] = hdr.n_sorted; hdr6[3] = hdr.max_len; hdr6[4] = hdr.rcp_unsafe;
     hdr6[5] = hdr.n_malformed;                     // 0, or -1 if the length histogram was not left zeroed for the next call
     return BEAGLE_OK;
+    } catch (...) { return BEAGLE_ERR_NOMEM; }
 }
 
 // host only: one warp of k_eval's scheduling loop (queue_body.inc) over a given list of queue entries, as a list of events
